@@ -1,0 +1,205 @@
+/*
+ * oracle/kv_oracle.c -- CPU ORACLE for the paged-KV tier transfer.  TEST INFRASTRUCTURE ONLY.
+ *
+ * Only tests/, __graft_entry__.smoke() and bench.py's cpu_baseline / --impl reference leg may
+ * build, link or call this file.  It shares no code, header, table or helper with the CUDA
+ * path under paper_2606_31093_b200/csrc/, and neither side includes the other.
+ *
+ * What it computes (the method is an exact permutation copy, so the oracle is the definition
+ * written out; citations are PAPER.md line + section, BASELINE.json key):
+ *
+ *   pool addressing   PAPER.md:L207 (sec. 4.1.1 Physical Paging Layer): a parameter has outer
+ *                     dims (layers), slice dims (K/V), a page size, shape and dtype; a region is
+ *                     fetched by (sub_names=layer, page_idx, slice_idx=K|V).  Here:
+ *                       POOL[l][c][g][t][h][d] = *(elem*)(base[l*C+c] + g*page_stride_bytes
+ *                                                         + ((t*H + h)*D + d)*e)
+ *                     in-page order NHD = [token][head][dim] ("NHD block stacks").
+ *   lower-tier layout BASELINE.json:configs[0]: page-first [page][layer][K,V][token][head][dim],
+ *                     dense.  (reading R1.)
+ *   O-pack            PAPER.md:L214 (sec. 4.1.2) "copy and convert pages directly into
+ *                     destination buffers"; SURVEY.md 8(c) Definition O-pack.
+ *   O-unpack          SURVEY.md 8(c) Definition O-unpack; BASELINE.json:configs[4] (re-paging,
+ *                     "sequence order preserved, tail page partially filled and zero-padded");
+ *                     PAPER.md:L238 (session metadata "records the total valid token length").
+ *   layer-first       SURVEY.md 8(f) NEXT-2: buffer [layer][K,V][page][token][head][dim].
+ *
+ * Elements are opaque e-byte bit patterns; nothing is ever interpreted as a float.
+ * All byte offsets are 64-bit.  Loops are in the paper's/SURVEY's index order
+ * (page, layer, K/V, token, head, dim); there is no blocking, fusion or memcpy of rows.
+ *
+ * Pins (tests/test_oracle_pins.py, tests/golden/): hand-computed worked examples W1/W2,
+ * numpy take/transpose/reshape special cases, an independently written "pull" formulation,
+ * round trip, write-once bijectivity, untouched bytes, zero-pad count, 64-bit offsets.
+ * Parity status: PINNED for every function in this file.
+ *
+ * `threads` > 1 splits the OUTER page loop across OpenMP threads (pages are independent);
+ * it exists for the reported CPU baseline and changes no result.
+ */
+#include <stddef.h>
+#include <stdint.h>
+
+#define KVO_OK 0
+#define KVO_ERR_ARG (-1)
+#define KVO_ERR_PAGE_RANGE (-2)
+
+/* copy one element of e bytes, as raw bytes */
+static inline void kvo_copy_elem(uint8_t *dst, const uint8_t *src, uint32_t e) {
+  for (uint32_t b = 0; b < e; ++b) dst[b] = src[b];
+}
+static inline void kvo_zero_elem(uint8_t *dst, uint32_t e) {
+  for (uint32_t b = 0; b < e; ++b) dst[b] = 0;
+}
+
+static int kvo_ids_in_range(const int32_t *ids, uint64_t n, uint32_t num_pages) {
+  for (uint64_t i = 0; i < n; ++i)
+    if (ids[i] < 0 || (uint32_t)ids[i] >= num_pages) return 0;
+  return 1;
+}
+
+/* Buffer element index for the two buffer layouts.
+ *   layout 0, page-first : ((((p*L + l)*C + c)*T + t)*H + h)*D + d
+ *   layout 1, layer-first: ((((l*C + c)*n + p)*T + t)*H + h)*D + d      (n = pages in buffer)
+ */
+static inline uint64_t kvo_buf_index(int layout, uint64_t p, uint64_t n, uint64_t l, uint64_t L,
+                                     uint64_t c, uint64_t C, uint64_t t, uint64_t T, uint64_t h,
+                                     uint64_t H, uint64_t d, uint64_t D) {
+  if (layout == 0) return ((((p * L + l) * C + c) * T + t) * H + h) * D + d;
+  return ((((l * C + c) * n + p) * T + t) * H + h) * D + d;
+}
+
+/* O-pack: buf[p][l][c][t][h][d] = POOL[l][c][ids[p]][t][h][d] */
+int kvo_pack(const void *const *base, uint32_t L, uint32_t C, uint32_t num_pages, uint32_t T,
+             uint32_t H, uint32_t D, uint32_t e, uint64_t page_stride_bytes, const int32_t *ids,
+             uint64_t n, int layout, void *buf, int threads) {
+  if (!base || (!ids && n) || (!buf && n) || !L || !C || !T || !H || !D || !e) return KVO_ERR_ARG;
+  if (layout != 0 && layout != 1) return KVO_ERR_ARG;
+  if (!kvo_ids_in_range(ids, n, num_pages)) return KVO_ERR_PAGE_RANGE;
+  uint8_t *out = (uint8_t *)buf;
+#pragma omp parallel for num_threads(threads) if (threads > 1) schedule(static)
+  for (int64_t p = 0; p < (int64_t)n; ++p)
+    for (uint64_t l = 0; l < L; ++l)
+      for (uint64_t c = 0; c < C; ++c)
+        for (uint64_t t = 0; t < T; ++t)
+          for (uint64_t h = 0; h < H; ++h)
+            for (uint64_t d = 0; d < D; ++d) {
+              const uint8_t *src = (const uint8_t *)base[l * C + c] +
+                                   (uint64_t)ids[p] * page_stride_bytes + ((t * H + h) * D + d) * e;
+              uint64_t o = kvo_buf_index(layout, (uint64_t)p, n, l, L, c, C, t, T, h, H, d, D);
+              kvo_copy_elem(out + o * e, src, e);
+            }
+  return KVO_OK;
+}
+
+/* O-unpack (general re-paging; same-size is Ts == Td, n_tokens = n*Ts):
+ *   n_dst = ceil(n_tokens / Td)
+ *   for q,l,c,u,h,d:  j = q*Td + u
+ *     DST[l][c][dst_ids[q]][u][h][d] = (j < n_tokens) ? src[(j/Ts) ...][j%Ts] : 0
+ * n_src = ceil(n_tokens / Ts) is the number of pages in the source buffer (layer-first needs it).
+ * Nothing else in any destination pool is written.  dst_ids must be distinct (caller checks).
+ */
+int kvo_unpack(const void *src, const int32_t *dst_ids, uint64_t n_dst, void *const *base,
+               uint32_t L, uint32_t C, uint32_t num_pages, uint32_t H, uint32_t D, uint32_t e,
+               uint64_t page_stride_bytes, uint32_t Ts, uint32_t Td, uint64_t n_tokens, int layout,
+               int threads) {
+  if (!base || !L || !C || !Ts || !Td || !H || !D || !e) return KVO_ERR_ARG;
+  if (layout != 0 && layout != 1) return KVO_ERR_ARG;
+  if (n_dst != (n_tokens + Td - 1) / Td) return KVO_ERR_ARG;
+  if ((!src || !dst_ids) && n_dst) return KVO_ERR_ARG;
+  if (!kvo_ids_in_range(dst_ids, n_dst, num_pages)) return KVO_ERR_PAGE_RANGE;
+  const uint8_t *in = (const uint8_t *)src;
+  const uint64_t n_src = (n_tokens + Ts - 1) / Ts;
+#pragma omp parallel for num_threads(threads) if (threads > 1) schedule(static)
+  for (int64_t q = 0; q < (int64_t)n_dst; ++q)
+    for (uint64_t l = 0; l < L; ++l)
+      for (uint64_t c = 0; c < C; ++c)
+        for (uint64_t u = 0; u < Td; ++u)
+          for (uint64_t h = 0; h < H; ++h)
+            for (uint64_t d = 0; d < D; ++d) {
+              uint64_t j = (uint64_t)q * Td + u; /* sequence position, order preserved */
+              uint8_t *dst = (uint8_t *)base[l * C + c] +
+                             (uint64_t)dst_ids[q] * page_stride_bytes + ((u * H + h) * D + d) * e;
+              if (j < n_tokens) {
+                uint64_t o = kvo_buf_index(layout, j / Ts, n_src, l, L, c, C, j % Ts, Ts, h, H, d, D);
+                kvo_copy_elem(dst, in + o * e, e);
+              } else {
+                kvo_zero_elem(dst, e);
+              }
+            }
+  return KVO_OK;
+}
+
+/* O-batched (BASELINE.json:configs[3]): O-pack per request r over
+ * ids[off[r] .. off[r+1]) into its own buffer dsts[r]. */
+int kvo_pack_batched(const void *const *base, uint32_t L, uint32_t C, uint32_t num_pages,
+                     uint32_t T, uint32_t H, uint32_t D, uint32_t e, uint64_t page_stride_bytes,
+                     const int32_t *ids, const int64_t *off, uint32_t R, int layout,
+                     void *const *dsts, int threads) {
+  if (R && (!off || !dsts)) return KVO_ERR_ARG;
+  for (uint32_t r = 0; r < R; ++r) {
+    if (off[r + 1] < off[r]) return KVO_ERR_ARG;
+    if (!kvo_ids_in_range(ids + off[r], (uint64_t)(off[r + 1] - off[r]), num_pages))
+      return KVO_ERR_PAGE_RANGE;
+  }
+  for (uint32_t r = 0; r < R; ++r) {
+    int rc = kvo_pack(base, L, C, num_pages, T, H, D, e, page_stride_bytes, ids + off[r],
+                      (uint64_t)(off[r + 1] - off[r]), layout, dsts[r], threads);
+    if (rc) return rc;
+  }
+  return KVO_OK;
+}
+
+/* O-batched unpack: O-unpack per request r with its own source buffer srcs[r], its own
+ * n_tokens[r] and destination ids dst_ids[off[r] .. off[r+1]) (count must be ceil(n_tokens/Td)). */
+int kvo_unpack_batched(const void *const *srcs, const int32_t *dst_ids, const int64_t *off,
+                       const uint64_t *n_tokens, uint32_t R, void *const *base, uint32_t L,
+                       uint32_t C, uint32_t num_pages, uint32_t H, uint32_t D, uint32_t e,
+                       uint64_t page_stride_bytes, uint32_t Ts, uint32_t Td, int layout,
+                       int threads) {
+  if (R && (!off || !srcs || !n_tokens)) return KVO_ERR_ARG;
+  if (!Td) return KVO_ERR_ARG;
+  for (uint32_t r = 0; r < R; ++r) {
+    if (off[r + 1] < off[r]) return KVO_ERR_ARG;
+    if ((uint64_t)(off[r + 1] - off[r]) != (n_tokens[r] + Td - 1) / Td) return KVO_ERR_ARG;
+    if (!kvo_ids_in_range(dst_ids + off[r], (uint64_t)(off[r + 1] - off[r]), num_pages))
+      return KVO_ERR_PAGE_RANGE;
+  }
+  for (uint32_t r = 0; r < R; ++r) {
+    int rc = kvo_unpack(srcs[r], dst_ids + off[r], (uint64_t)(off[r + 1] - off[r]), base, L, C,
+                        num_pages, H, D, e, page_stride_bytes, Ts, Td, n_tokens[r], layout, threads);
+    if (rc) return rc;
+  }
+  return KVO_OK;
+}
+
+/* Copy-on-write partial-page append ("copies its existing contents into a
+ * writable slot and appends the new data there"):
+ *   for l,c,t,h,d:
+ *     NEW[l][c][new_id][t] = OLD[l][c][old_id][t]            for t <  n_old
+ *                          = app[l][c][t - n_old][h][d]      for n_old <= t < n_old + n_app
+ *                          = untouched                       for t >= n_old + n_app
+ * `app` is dense [layer][K,V][token][head][dim] with n_app tokens.  OLD page is never written.
+ */
+int kvo_cow_append(void *const *base, uint32_t L, uint32_t C, uint32_t num_pages, uint32_t T,
+                   uint32_t H, uint32_t D, uint32_t e, uint64_t page_stride_bytes, int32_t old_id,
+                   int32_t new_id, uint32_t n_old, const void *app, uint32_t n_app) {
+  if (!base || !L || !C || !T || !H || !D || !e) return KVO_ERR_ARG;
+  if ((uint64_t)n_old + n_app > T || old_id == new_id) return KVO_ERR_ARG;
+  if (old_id < 0 || new_id < 0 || (uint32_t)old_id >= num_pages || (uint32_t)new_id >= num_pages)
+    return KVO_ERR_PAGE_RANGE;
+  if (!app && n_app) return KVO_ERR_ARG;
+  for (uint64_t l = 0; l < L; ++l)
+    for (uint64_t c = 0; c < C; ++c)
+      for (uint64_t t = 0; t < (uint64_t)n_old + n_app; ++t)
+        for (uint64_t h = 0; h < H; ++h)
+          for (uint64_t d = 0; d < D; ++d) {
+            uint8_t *slab = (uint8_t *)base[l * C + c];
+            uint8_t *dst = slab + (uint64_t)new_id * page_stride_bytes + ((t * H + h) * D + d) * e;
+            if (t < n_old) {
+              kvo_copy_elem(dst, slab + (uint64_t)old_id * page_stride_bytes + ((t * H + h) * D + d) * e, e);
+            } else {
+              uint64_t o = ((((l * C + c) * n_app) + (t - n_old)) * H + h) * D + d;
+              kvo_copy_elem(dst, (const uint8_t *)app + o * e, e);
+            }
+          }
+  return KVO_OK;
+}

@@ -1,0 +1,418 @@
+"""Pins for the CPU oracle (oracle/kv_oracle.{c,py}) -- nothing here calls the CUDA path.
+
+Each pin is something OTHER than the oracle's own formula: values derived by hand from the
+paper's addressing (tests/golden/), numpy library routines (take / transpose / reshape) for the
+special cases the definition reduces to, a separately written pull formulation, and invariants
+(bijectivity, untouched bytes, zero-pad count, 64-bit offsets).  Citations: PAPER.md:L207
+(sec. 4.1.1 addressing), PAPER.md:L214 (sec. 4.1.2 migration), PAPER.md:L238 (valid token length,
+CoW), BASELINE.json:configs[0] (page-first layout), configs[4] (re-paging), SURVEY.md 8(c).
+"""
+import numpy as np
+import pytest
+from hypothesis import HealthCheck, given, settings
+from hypothesis import strategies as st
+
+from oracle import kv_oracle as ko
+
+IMPLS = {
+    "c": (ko.pack, ko.unpack),
+    "py": (ko.pack_py, ko.unpack_py),
+}
+DT = {1: np.uint8, 2: np.uint16, 4: np.uint32}
+
+
+# ---------------------------------------------------------------------------------------------
+# helpers: pools as a stacked numpy array A[L,C,P,T,H,D] (dense stride) <-> HostPool
+# ---------------------------------------------------------------------------------------------
+def pool_from_array(A: np.ndarray, pad: int = 0, pad_fill: int = 0xA5) -> ko.HostPool:
+    L, C, P, T, H, D = A.shape
+    e = A.dtype.itemsize
+    row = T * H * D * e
+    stride = row + pad
+    slabs = []
+    for l in range(L):
+        for c in range(C):
+            s = np.full((P, stride), pad_fill, dtype=np.uint8)
+            s[:, :row] = A[l, c].reshape(P, -1).view(np.uint8)
+            slabs.append(s.reshape(-1))
+    return ko.HostPool(slabs, L, C, P, T, H, D, e, stride)
+
+
+def array_from_pool(pool: ko.HostPool) -> np.ndarray:
+    row = pool.row_bytes
+    out = np.empty((pool.L, pool.C, pool.num_pages, pool.T, pool.H, pool.D), dtype=DT[pool.e])
+    for l in range(pool.L):
+        for c in range(pool.C):
+            s = pool.slabs[l * pool.C + c].reshape(pool.num_pages, pool.page_stride_bytes)[:, :row]
+            out[l, c] = np.ascontiguousarray(s).view(DT[pool.e]).reshape(pool.num_pages, pool.T,
+                                                                        pool.H, pool.D)
+    return out
+
+
+def w1_array():
+    L, C, P, T, H, D = 2, 2, 4, 2, 1, 2
+    A = np.zeros((L, C, P, T, H, D), dtype=np.uint16)
+    for l in range(L):
+        for c in range(C):
+            for g in range(P):
+                for t in range(T):
+                    for d in range(D):
+                        A[l, c, g, t, 0, d] = 1000 * (2 * l + c) + 4 * g + 2 * t + d
+    return A
+
+
+# ---------------------------------------------------------------------------------------------
+# 1. hand-computed worked examples (tests/golden)
+# ---------------------------------------------------------------------------------------------
+@pytest.mark.parametrize("impl", IMPLS)
+def test_W1_pack_page_first(impl, golden):
+    pack, _ = IMPLS[impl]
+    buf = pack(pool_from_array(w1_array()), [3, 0]).view(np.uint16)
+    assert buf.tolist() == golden("W1_pack_page_first.txt")
+
+
+@pytest.mark.parametrize("impl", IMPLS)
+def test_W1_pack_layer_first(impl, golden):
+    pack, _ = IMPLS[impl]
+    buf = pack(pool_from_array(w1_array()), [3, 0], layout=ko.LAYER_FIRST).view(np.uint16)
+    assert buf.tolist() == golden("W1_pack_layer_first.txt")
+
+
+@pytest.mark.parametrize("impl", IMPLS)
+def test_W2_repage_padded_tail(impl, golden):
+    _, unpack = IMPLS[impl]
+    src = np.array(golden("W1_pack_page_first.txt"), dtype=np.uint16)
+    dst = pool_from_array(np.full((2, 2, 3, 4, 1, 2), 7777, dtype=np.uint16))
+    unpack(src, [2], dst, Ts=2, n_tokens=3)
+    got = np.concatenate([s.view(np.uint16) for s in dst.slabs]).tolist()
+    assert got == golden("W2_repage_padded_tail.txt")
+
+
+# ---------------------------------------------------------------------------------------------
+# 2. special cases that reduce to library routines
+# ---------------------------------------------------------------------------------------------
+SHAPES = [  # L, C, P, T, H, D, e
+    (1, 1, 5, 1, 1, 1, 1),
+    (2, 2, 9, 3, 2, 4, 2),
+    (3, 2, 17, 4, 3, 5, 4),
+    (4, 2, 32, 16, 2, 8, 2),
+    (2, 1, 7, 2, 1, 3, 1),
+]
+
+
+def rand_array(rng, L, C, P, T, H, D, e):
+    return rng.integers(0, 256 ** e, size=(L, C, P, T, H, D), dtype=np.uint64).astype(DT[e])
+
+
+@pytest.mark.parametrize("impl", IMPLS)
+@pytest.mark.parametrize("shape", SHAPES)
+@pytest.mark.parametrize("pad", [0, 8])
+def test_pack_is_numpy_take_transpose(impl, shape, pad):
+    pack, _ = IMPLS[impl]
+    rng = np.random.default_rng(hash(shape) & 0xFFFF)
+    A = rand_array(rng, *shape)
+    P = shape[2]
+    ids = rng.integers(0, P, size=P + 3)  # duplicates allowed for pack (reading 5)
+    pool = pool_from_array(A, pad=pad)
+    got = pack(pool, ids).view(A.dtype)
+    want = np.take(A, ids, axis=2).transpose(2, 0, 1, 3, 4, 5)  # [page][layer][kv][t][h][d]
+    assert np.array_equal(got, want.reshape(-1))
+    got_lf = pack(pool, ids, layout=ko.LAYER_FIRST).view(A.dtype)
+    assert np.array_equal(got_lf, np.take(A, ids, axis=2).reshape(-1))  # [layer][kv][page]...
+
+
+@pytest.mark.parametrize("impl", IMPLS)
+def test_pack_sequential_single_slab_is_memcpy(impl):
+    pack, _ = IMPLS[impl]
+    rng = np.random.default_rng(3)
+    A = rand_array(rng, 1, 1, 11, 4, 2, 3, 2)
+    pool = pool_from_array(A)
+    buf = pack(pool, np.arange(11))
+    assert buf.tobytes() == pool.slabs[0].tobytes()
+
+
+@pytest.mark.parametrize("impl", IMPLS)
+def test_pack_layer_subset_uses_first_layers(impl):
+    pack, _ = IMPLS[impl]
+    rng = np.random.default_rng(4)
+    A = rand_array(rng, 3, 2, 6, 2, 2, 2, 2)
+    ids = [5, 1, 2]
+    got = pack(pool_from_array(A), ids, layer_count=2).view(A.dtype)
+    want = np.take(A[:2], ids, axis=2).transpose(2, 0, 1, 3, 4, 5)
+    assert np.array_equal(got, want.reshape(-1))
+
+
+@pytest.mark.parametrize("impl", IMPLS)
+@pytest.mark.parametrize("Ts,Td,ntok", [(2, 4, 8), (2, 4, 7), (4, 2, 9), (3, 5, 11), (16, 64, 130),
+                                        (4, 4, 12), (4, 4, 10), (6, 4, 1), (1, 7, 20)])
+def test_repage_sequential_is_reshape_plus_zero_fill(impl, Ts, Td, ntok):
+    """Sequence tensor S[L,C,ntok,H,D] cut into Ts-token pages IS the page-first buffer; unpacking
+    into pages 0..n_dst-1 of a pool must give S re-cut into Td-token pages, zero padded."""
+    _, unpack = IMPLS[impl]
+    L, C, H, D, e = 2, 2, 2, 3, 2
+    rng = np.random.default_rng(Ts * 100 + Td)
+    S = rng.integers(1, 65536, size=(L, C, ntok, H, D), dtype=np.uint64).astype(np.uint16)
+    n_src, n_dst = -(-ntok // Ts), -(-ntok // Td)
+    Spad = np.full((L, C, n_src * Ts, H, D), 0xBEEF, dtype=np.uint16)  # stale tail tokens: ignored
+    Spad[:, :, :ntok] = S
+    buf = Spad.reshape(L, C, n_src, Ts, H, D).transpose(2, 0, 1, 3, 4, 5).copy().reshape(-1)
+    P = n_dst + 2
+    dst = pool_from_array(np.full((L, C, P, Td, H, D), 0x7777, dtype=np.uint16))
+    unpack(buf, np.arange(n_dst), dst, Ts=Ts, n_tokens=ntok)
+    B = array_from_pool(dst)
+    seq = B[:, :, :n_dst].reshape(L, C, n_dst * Td, H, D)
+    assert np.array_equal(seq[:, :, :ntok], S)
+    assert np.all(seq[:, :, ntok:] == 0)
+    assert np.all(B[:, :, n_dst:] == 0x7777)  # untouched pages
+    # layer-first source: [layer][kv][page][t][h][d] is Spad's own order
+    dst2 = pool_from_array(np.full((L, C, P, Td, H, D), 0x7777, dtype=np.uint16))
+    unpack(Spad.reshape(-1), np.arange(n_dst), dst2, Ts=Ts, n_tokens=ntok, layout=ko.LAYER_FIRST)
+    assert np.array_equal(array_from_pool(dst2), B)
+
+
+# ---------------------------------------------------------------------------------------------
+# 3. separately written pull formulation: de-linearise every OUTPUT byte offset by div/mod
+# ---------------------------------------------------------------------------------------------
+def pull_pack(pool: ko.HostPool, ids, L, layout=0):
+    C, T, H, D, e = pool.C, pool.T, pool.H, pool.D, pool.e
+    n = len(ids)
+    out = np.zeros(n * L * C * T * H * D * e, dtype=np.uint8)
+    for o in range(out.size):
+        b = o % e; r = o // e
+        d = r % D; r //= D
+        h = r % H; r //= H
+        t = r % T; r //= T
+        if layout == 0:
+            c = r % C; r //= C
+            l = r % L; p = r // L
+        else:
+            p = r % n; r //= n
+            c = r % C; l = r // C
+        out[o] = pool.slabs[l * C + c][int(ids[p]) * pool.page_stride_bytes
+                                      + ((t * H + h) * D + d) * e + b]
+    return out
+
+
+def pull_unpack(src, dst_ids, pool: ko.HostPool, Ts, n_tokens, L):
+    """Returns the expected slabs: for every byte of every destination slab decide where it
+    comes from (page-first source only)."""
+    C, Td, H, D, e = pool.C, pool.T, pool.H, pool.D, pool.e
+    row = Td * H * D * e
+    where = {int(g): q for q, g in enumerate(dst_ids)}
+    src = np.ascontiguousarray(src).view(np.uint8).reshape(-1)
+    out = [s.copy() for s in pool.slabs]
+    for lc in range(L * C):
+        l, c = divmod(lc, C)
+        for o in range(out[lc].size):
+            g, within = divmod(o, pool.page_stride_bytes)
+            if g not in where or within >= row:
+                continue  # untouched page, or stride padding
+            b = within % e; r = within // e
+            d = r % D; r //= D
+            h = r % H; u = r // H
+            j = where[g] * Td + u
+            if j >= n_tokens:
+                out[lc][o] = 0
+            else:
+                p, t = divmod(j, Ts)
+                out[lc][o] = src[(((((p * L + l) * C + c) * Ts + t) * H + h) * D + d) * e + b]
+    return out
+
+
+tiny_dims = st.tuples(st.integers(1, 3), st.integers(1, 2), st.integers(1, 6), st.integers(1, 4),
+                      st.integers(1, 2), st.integers(1, 3), st.sampled_from([1, 2, 4]))
+
+
+@settings(max_examples=40, deadline=None, suppress_health_check=list(HealthCheck))
+@given(dims=tiny_dims, pad=st.sampled_from([0, 4]), seed=st.integers(0, 2 ** 16),
+       layout=st.sampled_from([0, 1]))
+def test_pack_push_equals_pull(dims, pad, seed, layout):
+    L, C, P, T, H, D, e = dims
+    rng = np.random.default_rng(seed)
+    pool = pool_from_array(rand_array(rng, L, C, P, T, H, D, e), pad=pad)
+    ids = rng.integers(0, P, size=rng.integers(0, P + 2))
+    want = pull_pack(pool, ids, L, layout)
+    assert np.array_equal(ko.pack(pool, ids, layout=layout), want)
+    assert np.array_equal(ko.pack_py(pool, ids, layout=layout), want)
+
+
+@settings(max_examples=40, deadline=None, suppress_health_check=list(HealthCheck))
+@given(dims=tiny_dims, Ts=st.integers(1, 5), pad=st.sampled_from([0, 4]),
+       seed=st.integers(0, 2 ** 16), data=st.data())
+def test_unpack_push_equals_pull(dims, Ts, pad, seed, data):
+    L, C, P, Td, H, D, e = dims
+    rng = np.random.default_rng(seed)
+    n_tokens = data.draw(st.integers(0, P * Td))
+    n_dst, n_src = -(-n_tokens // Td), -(-n_tokens // Ts)
+    src = rng.integers(0, 256, size=n_src * L * C * Ts * H * D * e, dtype=np.uint8)
+    dst_ids = rng.permutation(P)[:n_dst]
+    base = pool_from_array(rand_array(rng, L, C, P, Td, H, D, e), pad=pad)
+    want = pull_unpack(src, dst_ids, base, Ts, n_tokens, L)
+    for unpack in (ko.unpack, ko.unpack_py):
+        pool = base.copy()
+        unpack(src, dst_ids, pool, Ts=Ts, n_tokens=n_tokens)
+        for a, b in zip(pool.slabs, want):
+            assert np.array_equal(a, b)
+
+
+# ---------------------------------------------------------------------------------------------
+# 4. invariants (BASELINE.json:north_star): round trip, bijectivity, untouched bytes, pad count
+# ---------------------------------------------------------------------------------------------
+def tagged_array(L, C, P, T, H, D):
+    n = L * C * P * T * H * D
+    return (np.arange(1, n + 1, dtype=np.uint32)).reshape(L, C, P, T, H, D)  # tag 0 = "unwritten"
+
+
+def test_pack_is_a_bijection_onto_touched_elements():
+    A = tagged_array(3, 2, 12, 4, 2, 3)
+    ids = np.random.default_rng(5).permutation(12)[:7]
+    buf = ko.pack(pool_from_array(A), ids).view(np.uint32)
+    assert buf.size == A[:, :, ids].size
+    assert np.all(buf != 0), "some buffer element was never written"
+    assert len(np.unique(buf)) == buf.size, "some pool element was copied twice"
+    assert set(buf.tolist()) == set(A[:, :, ids].reshape(-1).tolist())
+
+
+@pytest.mark.parametrize("Ts,Td,ntok", [(4, 4, 28), (2, 8, 50), (8, 2, 13), (3, 4, 17)])
+def test_unpack_writes_each_touched_element_once_and_nothing_else(Ts, Td, ntok):
+    L, C, H, D, P = 2, 2, 2, 3, 20
+    n_src, n_dst = -(-ntok // Ts), -(-ntok // Td)
+    src = np.arange(1, n_src * L * C * Ts * H * D + 1, dtype=np.uint32)
+    SENT = 0xFFFFFFFF
+    pool = pool_from_array(np.full((L, C, P, Td, H, D), SENT, dtype=np.uint32), pad=16, pad_fill=0x5A)
+    dst_ids = np.random.default_rng(6).permutation(P)[:n_dst]
+    ko.unpack(src, dst_ids, pool, Ts=Ts, n_tokens=ntok)
+    B = array_from_pool(pool)
+    touched = B[:, :, dst_ids].reshape(-1)
+    data = touched[touched != 0]
+    assert np.all(data != SENT), "a slot of a touched page was left unwritten"
+    assert len(np.unique(data)) == data.size == ntok * L * C * H * D
+    # valid source elements = tokens < ntok of every (page, layer, kv)
+    S = src.reshape(n_src, L, C, Ts, H, D).transpose(1, 2, 0, 3, 4, 5).reshape(L, C, n_src * Ts, H, D)
+    assert set(data.tolist()) == set(S[:, :, :ntok].reshape(-1).tolist())
+    # zero-pad count: (n_dst*Td - n_tokens) * L*C*H*D elements
+    assert int((touched == 0).sum()) == (n_dst * Td - ntok) * L * C * H * D
+    # untouched pages and stride padding byte-identical
+    mask = np.ones(P, bool); mask[dst_ids] = False
+    assert np.all(B[:, :, mask] == SENT)
+    for s in pool.slabs:
+        assert np.all(s.reshape(P, -1)[:, pool.row_bytes:] == 0x5A)
+
+
+@pytest.mark.parametrize("shape", SHAPES[1:])
+def test_round_trip_identity(shape):
+    L, C, P, T, H, D, e = shape
+    rng = np.random.default_rng(7)
+    A = rand_array(rng, *shape)
+    Bfill = rand_array(rng, *shape)
+    n = P // 2
+    ids = rng.permutation(P)[:n]
+    ids2 = rng.permutation(P)[:n]
+    poolB = pool_from_array(Bfill)
+    buf = ko.pack(pool_from_array(A), ids)
+    ko.unpack(buf, ids2, poolB, Ts=T, n_tokens=n * T)
+    B = array_from_pool(poolB)
+    assert np.array_equal(B[:, :, ids2], A[:, :, ids])
+    mask = np.ones(P, bool); mask[ids2] = False
+    assert np.array_equal(B[:, :, mask], Bfill[:, :, mask])
+    # and packing B at ids2 gives the same buffer back
+    assert np.array_equal(ko.pack(poolB, ids2), buf)
+
+
+def test_bit_patterns_survive():
+    """bf16 NaN payloads, -0, subnormals, inf: copy is bitwise."""
+    pats = np.array([0x7FC1, 0xFFFF, 0x8000, 0x0001, 0x7F80, 0xFF80, 0x0000, 0x7F81], dtype=np.uint16)
+    A = np.resize(pats, (1, 2, 3, 2, 2, 4)).astype(np.uint16)
+    buf = ko.pack(pool_from_array(A), [2, 0]).view(np.uint16)
+    assert np.array_equal(buf, A[:, :, [2, 0]].transpose(2, 0, 1, 3, 4, 5).reshape(-1))
+
+
+def test_offsets_beyond_4GiB():
+    """SURVEY.md 8(c) reading 18: one slab of 262,145 pages x 16 KiB; ids=[262144, 0] must return
+    the last page first.  The slab is calloc-backed; only two pages are ever touched."""
+    P, T, H, D, e = 262145, 16, 4, 128, 2
+    row = T * H * D * e
+    slab = np.zeros(P * row, dtype=np.uint8)
+    slab[:row] = 0x11
+    slab[(P - 1) * row:] = 0xEE
+    pool = ko.HostPool([slab], 1, 1, P, T, H, D, e, row)
+    buf = ko.pack(pool, [P - 1, 0])
+    assert np.all(buf[:row] == 0xEE) and np.all(buf[row:] == 0x11)
+    ko.unpack(buf, [P - 2, 1], pool, Ts=T, n_tokens=2 * T)
+    assert np.all(slab[(P - 2) * row:(P - 1) * row] == 0xEE) and np.all(slab[row:2 * row] == 0x11)
+    assert not slab[2 * row:3 * row].any()
+
+
+# ---------------------------------------------------------------------------------------------
+# 5. batched, threads, errors, CoW
+# ---------------------------------------------------------------------------------------------
+def test_batched_equals_per_request_and_threads_change_nothing():
+    rng = np.random.default_rng(8)
+    A = rand_array(rng, 3, 2, 40, 4, 2, 4, 2)
+    pool = pool_from_array(A)
+    off = np.array([0, 5, 5, 12, 20])
+    ids = rng.permutation(40)[:20]
+    bufs = ko.pack_batched(pool, ids, off, threads=3)
+    for r in range(4):
+        want = np.take(A, ids[off[r]:off[r + 1]], axis=2).transpose(2, 0, 1, 3, 4, 5).reshape(-1)
+        assert np.array_equal(bufs[r].view(np.uint16), want)
+        assert np.array_equal(bufs[r], ko.pack(pool, ids[off[r]:off[r + 1]], threads=1))
+    # batched re-paging unpack == per-request unpack
+    Td = 8
+    ntok = np.array([5 * 4, 0, 7 * 4 - 3, 8 * 4 - 1])
+    nd = -(-ntok // Td)
+    doff = np.concatenate([[0], np.cumsum(nd)])
+    dids = rng.permutation(30)[:doff[-1]]
+    base = pool_from_array(rand_array(rng, 3, 2, 30, Td, 2, 4, 2))
+    p1, p2 = base.copy(), base.copy()
+    ko.unpack_batched(bufs, dids, doff, ntok, p1, Ts=4, threads=4)
+    for r in range(4):
+        ko.unpack(bufs[r], dids[doff[r]:doff[r + 1]], p2, Ts=4, n_tokens=int(ntok[r]))
+    for a, b in zip(p1.slabs, p2.slabs):
+        assert np.array_equal(a, b)
+
+
+def test_errors():
+    pool = pool_from_array(w1_array())
+    for pack in (ko.pack, ko.pack_py):
+        with pytest.raises(IndexError):
+            pack(pool, [4])
+        with pytest.raises(IndexError):
+            pack(pool, [-1])
+    buf = ko.pack(pool, [0, 1])
+    for unpack in (ko.unpack, ko.unpack_py):
+        with pytest.raises(ValueError):
+            unpack(buf, [1, 1], pool.copy(), Ts=2, n_tokens=4)  # duplicate destination
+        with pytest.raises(ValueError):
+            unpack(buf, [1], pool.copy(), Ts=2, n_tokens=4)  # wrong page count
+        with pytest.raises(IndexError):
+            unpack(buf, [1, 9], pool.copy(), Ts=2, n_tokens=4)
+
+
+def test_empty_calls_touch_nothing():
+    pool = pool_from_array(w1_array())
+    before = [s.copy() for s in pool.slabs]
+    assert ko.pack(pool, []).size == 0
+    ko.unpack(np.zeros(0, np.uint8), [], pool, Ts=2, n_tokens=0)
+    for a, b in zip(pool.slabs, before):
+        assert np.array_equal(a, b)
+
+
+def test_cow_append_is_slice_assignment():
+    """copy the retained partial page into a writable slot, append there."""
+    rng = np.random.default_rng(9)
+    L, C, P, T, H, D = 3, 2, 6, 8, 2, 4
+    A = rand_array(rng, L, C, P, T, H, D, 2)
+    pool = pool_from_array(A, pad=32)
+    n_old, n_app = 3, 4
+    app = rng.integers(0, 65536, size=(L, C, n_app, H, D), dtype=np.uint64).astype(np.uint16)
+    ko.cow_append(pool, old_id=4, new_id=1, n_old=n_old, app=app, n_app=n_app)
+    B = array_from_pool(pool)
+    want = A.copy()
+    want[:, :, 1, :n_old] = A[:, :, 4, :n_old]
+    want[:, :, 1, n_old:n_old + n_app] = app
+    assert np.array_equal(B, want)  # old page, other pages and slots >= n_old+n_app untouched
+    with pytest.raises(ValueError):
+        ko.cow_append(pool, 4, 1, 6, app, 4)  # overflow of the page
+    with pytest.raises(ValueError):
+        ko.cow_append(pool, 2, 2, 1, app, 1)  # in place is not copy-on-write
