@@ -1,0 +1,211 @@
+/*
+ * kvtier.h -- C ABI of the B200-native paged-KV tier transfer library (libkvtier.so).
+ *
+ * The one hot path of Omni-Flow's Data Flow layer: "Cross-tier migration converts between
+ * compute-oriented layouts, including NHD block stacks, and the representation used by
+ * lower-tier storage ... CUDA kernels ... copy and convert pages directly into destination
+ * buffers" (sec. 4.1.2 Multi-Tier Slot Engine), over pools addressed by
+ * (layer, page_idx, K|V slice) (sec. 4.1.1 Physical Paging Layer), between the
+ * L1 GPU tier and the L2 CPU tier (sec. 4).  The lower-tier representation is the
+ * dense page-first buffer [page][layer][K,V][token][head][dim] of BASELINE.json:configs[0].
+ * Call shapes follow BASELINE.json:north_star; the scope table is SURVEY.md 8(a)/(b).
+ *
+ * Conventions that hold for EVERY entry point
+ *   - Plain C types only.  `kv_stream_t` is a cudaStream_t / CUstream passed as an opaque
+ *     pointer (NULL = the legacy default stream).
+ *   - Return value: KV_OK (0) or a negative kv_status.  No exception crosses the ABI.
+ *   - All argument validation happens before the first CUDA call that could write: a call that
+ *     returns a validation error (anything but KV_ERR_CUDA) has written nothing.
+ *   - Ownership: the caller owns pools, buffers and id arrays; the library never frees them.
+ *     HOST arrays (page ids, offsets, token counts, pointer arrays, kv_pool_desc and its `base`
+ *     array) are consumed before the call returns and may be reused immediately.
+ *   - Asynchrony: work is enqueued on `stream` and the call returns.  Results (including the
+ *     host-visible bytes of an offload) are defined once the caller has synchronised `stream`.
+ *     Staged host transfers use a side stream owned by the ctx but are joined back to `stream`
+ *     before the call returns control of ordering.
+ *   - Aliasing: transfer buffers must not overlap any pool; destination page ids of one call
+ *     must be distinct and free (the slot engine guarantees it).
+ *   - Elements are opaque `elem_bytes`-wide bit patterns; nothing is ever interpreted as a number.
+ *   - All byte offsets are 64-bit.
+ *   - A kv_ctx is not thread-safe: one ctx per calling thread.  Calls on different streams are
+ *     independent when their destination page sets are disjoint.
+ */
+#ifndef KVTIER_H
+#define KVTIER_H
+
+#include <stddef.h>
+#include <stdint.h>
+
+#ifdef __cplusplus
+extern "C" {
+#endif
+
+#define KVTIER_VERSION 0x00010000u /* major.minor.patch = 0.1.0 */
+
+typedef struct kv_ctx kv_ctx;
+typedef void *kv_stream_t;
+
+/* One paged KV parameter: outer dim = layers, slice dim = K/V, a page size,
+ * a shape and an element width.  Region (l, g, c) starts at base[l*kv_count + c] +
+ * g*page_stride_bytes and holds page_size*num_heads*head_dim elements in NHD order
+ * [token][head][dim] ("NHD block stacks").  Separate K and V allocations, one fused
+ * allocation per layer, or one allocation for everything are all expressed by the base pointers
+ * and the stride; bytes between the dense row and the stride are never read or written. */
+typedef struct kv_pool_desc {
+  void *const *base;          /* HOST array of layer_count*kv_count DEVICE pointers, [layer][kv], kv 0=K 1=V */
+  uint32_t layer_count;       /* layers in the descriptor */
+  uint32_t kv_count;          /* 2 for K and V; 1 for single-latent pools */
+  uint32_t num_pages;         /* pages in each slab; valid page ids are 0 .. num_pages-1 */
+  uint32_t page_size;         /* tokens per page */
+  uint32_t num_heads;         /* KV heads held by THIS rank (a TP head partition has fewer) */
+  uint32_t head_dim;
+  uint32_t elem_bytes;        /* 1, 2, 4 or 8; bf16 = 2 */
+  uint32_t reserved;          /* must be 0 */
+  uint64_t page_stride_bytes; /* >= page_size*num_heads*head_dim*elem_bytes, multiple of elem_bytes */
+} kv_pool_desc;
+
+/* Layout of the transfer buffer (the "representation used by lower-tier storage"). */
+typedef enum kv_layout {
+  KV_LAYOUT_PAGE_FIRST = 0,  /* [page][layer][kv][token][head][dim]  (BASELINE.json:configs[0]) */
+  KV_LAYOUT_LAYER_FIRST = 1, /* [layer][kv][page][token][head][dim] */
+} kv_layout;
+
+/* How a host-tier transfer crosses the host link (BASELINE.json:north_star item 3). */
+typedef enum kv_host_mode {
+  KV_HOST_AUTO = 0,   /* chosen from the measured table in DESIGN.md */
+  KV_HOST_DIRECT = 1, /* the kernel stores to / loads from mapped pinned memory over the link */
+  KV_HOST_STAGED = 2, /* device staging + copy-engine cudaMemcpyAsync on the ctx's side stream, chunk-pipelined */
+} kv_host_mode;
+
+typedef enum kv_status {
+  KV_OK = 0,
+  KV_ERR_NULL = -1,       /* a required pointer is NULL */
+  KV_ERR_SIZE = -2,       /* buffer too small; page sizes / counts inconsistent; more than 2^32-1 items per request */
+  KV_ERR_PAGE_RANGE = -3, /* a page id is < 0 or >= num_pages */
+  KV_ERR_DUP_PAGE = -4,   /* duplicate destination page id (checked only under KV_FLAG_VALIDATE) */
+  KV_ERR_LAYOUT = -5,     /* unknown kv_layout / kv_host_mode / option */
+  KV_ERR_ALIGN = -6,      /* a pointer or stride is not elem_bytes-aligned */
+  KV_ERR_CUDA = -7,       /* a CUDA call failed; see kv_last_cuda_error() */
+  KV_ERR_HOST_MEM = -8,   /* host buffer of an offload/reload is not pinned (page-locked) memory */
+  KV_ERR_DESC = -9,       /* malformed kv_pool_desc (zero dimension, bad elem_bytes, stride < row, layer_count too large) */
+  KV_ERR_NO_DEVICE = -10, /* planning-only ctx (device < 0): arguments were valid, nothing was launched */
+} kv_status;
+
+/* flags (bit set) */
+#define KV_FLAG_VALIDATE 0x1u      /* also check destination page ids for duplicates (unpack/reload) */
+#define KV_FLAG_IDS_ON_DEVICE 0x2u /* page_ids is a DEVICE pointer; range errors skip the page and set the device status word */
+
+/* kv_ctx_set_option keys (tuning; defaults are the measured best) */
+typedef enum kv_option {
+  KV_OPT_KERNEL = 0,         /* 0 auto, 1 bulk (cp.async.bulk smem ring), 2 vec (16-byte LDG/STG), 3 elem (any alignment) */
+  KV_OPT_STAGE_BYTES = 1,    /* bulk: bytes per shared-memory stage (multiple of 16, 1 KiB .. 64 KiB) */
+  KV_OPT_STAGES_PER_WARP = 2,/* bulk: ring depth per issuing warp (2 .. 16) */
+  KV_OPT_WARPS = 3,          /* bulk: issuing warps per CTA (1 .. 8) */
+  KV_OPT_STORE_LAG = 4,      /* bulk: stores left in flight before a stage is refilled (1 .. 3) */
+  KV_OPT_MAX_CTAS = 5,       /* cap on the grid (0 = SM count x CTAs per SM) */
+  KV_OPT_CHUNK_BYTES = 6,    /* staged host transfers: bytes per pipeline chunk (0 = staging_bytes / slots) */
+  KV_OPT_HOST_MAX_CTAS = 7,  /* grid cap for DIRECT host transfers (0 = same as device transfers) */
+  KV_OPT_STAGING_SLOTS = 8,  /* staged host transfers: pipeline slots the staging buffer is cut into (2 .. 4) */
+  KV_OPT_L2_HINT = 9,        /* bulk: 0 none, 1 evict_first cache hint on loads and stores */
+} kv_option;
+
+/* kv_ctx_get_stat keys */
+typedef enum kv_stat {
+  KV_STAT_LAUNCHES = 0,     /* kernels launched by this ctx since creation */
+  KV_STAT_MEMCPYS = 1,      /* copy-engine memcpys issued by this ctx since creation (id staging + staged host transfers) */
+  KV_STAT_LAST_ITEMS = 2,   /* work items (segments) planned by the last call */
+  KV_STAT_LAST_PAYLOAD = 3, /* payload bytes of the last call (bytes written at the destination) */
+  KV_STAT_LAST_KERNEL = 4,  /* kernel variant the last call used (KV_OPT_KERNEL values) */
+  KV_STAT_LAST_HOST_MODE = 5,/* host mode the last offload/reload used (kv_host_mode) */
+  KV_STAT_LAST_GRID = 6,    /* CTAs of the last launch */
+  KV_STAT_LAST_SEGMENT = 7, /* bytes per work item of the last call */
+} kv_stat;
+
+/* ---- library ------------------------------------------------------------------------------ */
+uint32_t kv_version(void);          /* KVTIER_VERSION of the loaded library */
+const char *kv_strerror(int status); /* static string, never NULL */
+
+/* ---- context ------------------------------------------------------------------------------ */
+/* Creates the per-thread context on CUDA device `device`: side stream, events, the ring that
+ * stages page-id lists, a device status word and (lazily, on the first STAGED transfer)
+ * `staging_bytes` of device staging (0 = 256 MiB).  `device` < 0 creates a PLANNING-ONLY ctx
+ * that touches no CUDA API: every transfer call validates and plans, then returns
+ * KV_ERR_NO_DEVICE instead of launching (used by host-side tests). */
+int kv_ctx_create(kv_ctx **out, int device, size_t staging_bytes);
+int kv_ctx_destroy(kv_ctx *ctx); /* synchronises the ctx's own work, frees everything it owns */
+int kv_ctx_set_option(kv_ctx *ctx, int option, int64_t value); /* KV_ERR_LAYOUT on unknown key, KV_ERR_SIZE on bad value */
+int kv_ctx_get_stat(kv_ctx *ctx, int stat, uint64_t *out);
+int kv_last_cuda_error(kv_ctx *ctx); /* the cudaError_t behind the last KV_ERR_CUDA (0 if none) */
+/* Reads (and clears) the device status word; synchronises the device.  Bit 0: a device-resident
+ * page id was out of range (that page was skipped). */
+int kv_device_status(kv_ctx *ctx, uint32_t *out);
+
+/* ---- pinned host memory (the L2 CPU tier) ----------------------------------- */
+int kv_host_alloc(void **p, size_t bytes); /* page-locked, mapped, portable; free with kv_host_free */
+int kv_host_free(void *p);
+int kv_host_register(void *p, size_t bytes); /* pin + map an existing host range */
+int kv_host_unregister(void *p);
+
+/* ---- device-side pack / unpack -------------------------------------- */
+/* kv_pack: gather pages page_ids[0..n) of the first `layer_count` layers of `pools` into the
+ * transfer buffer `dst` (DEVICE-accessible memory, >= n*layer_count*kv_count*row bytes):
+ *   page-first:  dst[p][l][c][t][h][d] = POOL[l][c][page_ids[p]][t][h][d]
+ * (BASELINE.json:configs[0]).  page_ids order is sequence order and is never
+ * changed; duplicates are allowed (read-only).  n == 0 is KV_OK with no launch. */
+int kv_pack(kv_ctx *ctx, const kv_pool_desc *pools, uint32_t layer_count, const int32_t *page_ids,
+            uint32_t n, int layout, void *dst, size_t dst_bytes, uint32_t flags, kv_stream_t stream);
+
+/* kv_unpack: scatter a transfer buffer of `src_page_size`-token pages holding `n_tokens` valid
+ * tokens into pages dst_page_ids[0..n_dst_pages) of `pools`, whose page size must equal
+ * `dst_page_size`; n_dst_pages must be ceil(n_tokens / dst_page_size).  Sequence token
+ * j = p*Ts + t lands in destination page j / Td, slot j % Td; slots j >= n_tokens of the touched
+ * destination pages are set to all-bits-zero; source tokens >= n_tokens are ignored
+ * (BASELINE.json:configs[4]; "total valid token length").  For a verbatim
+ * whole-page copy pass n_tokens = n*Ts.  `src` must hold ceil(n_tokens/Ts) pages.
+ * Nothing else in any pool is written. */
+int kv_unpack(kv_ctx *ctx, const void *src, size_t src_bytes, const int32_t *dst_page_ids,
+              uint32_t n_dst_pages, const kv_pool_desc *pools, uint32_t layer_count,
+              uint32_t src_page_size, uint32_t dst_page_size, uint64_t n_tokens, int layout,
+              uint32_t flags, kv_stream_t stream);
+
+/* Batched (CSR) variants (BASELINE.json:configs[3]): request r owns
+ * page_ids[req_offsets[r] .. req_offsets[r+1]) and its own buffer dsts[r] / srcs[r] (HOST arrays
+ * of device-accessible pointers).  ONE launch covers all requests.  `dst_bytes` / `src_bytes`
+ * (per request) may be NULL to skip the size check.  For unpack, request r must own exactly
+ * ceil(n_tokens[r] / dst_page_size) destination pages. */
+int kv_pack_batched(kv_ctx *ctx, const kv_pool_desc *pools, uint32_t layer_count,
+                    const int32_t *page_ids, const int64_t *req_offsets, uint32_t n_req, int layout,
+                    void *const *dsts, const uint64_t *dst_bytes, uint32_t flags, kv_stream_t stream);
+int kv_unpack_batched(kv_ctx *ctx, const void *const *srcs, const uint64_t *src_bytes,
+                      const int32_t *dst_page_ids, const int64_t *req_offsets,
+                      const uint64_t *n_tokens, uint32_t n_req, const kv_pool_desc *pools,
+                      uint32_t layer_count, uint32_t src_page_size, uint32_t dst_page_size,
+                      int layout, uint32_t flags, kv_stream_t stream);
+
+/* ---- host tier: offload (device -> pinned host) and reload (pinned host -> device) ----------
+ * Same semantics and bytes as kv_pack / kv_unpack with the transfer buffer in PINNED HOST memory
+ * (from kv_host_alloc, kv_host_register, cudaHostAlloc or torch pin_memory); a pageable pointer
+ * is KV_ERR_HOST_MEM.  `mode` must not change a single byte of the result.
+ * Appending to a session's host buffer is a call with host_dst advanced by the pages already
+ * there (page-first makes append a tail write). */
+int kv_offload(kv_ctx *ctx, const kv_pool_desc *pools, uint32_t layer_count,
+               const int32_t *page_ids, uint32_t n, int layout, void *host_dst, size_t host_bytes,
+               int mode, uint32_t flags, kv_stream_t stream);
+int kv_reload(kv_ctx *ctx, const void *host_src, size_t host_bytes, const int32_t *dst_page_ids,
+              uint32_t n_dst_pages, const kv_pool_desc *pools, uint32_t layer_count,
+              uint32_t src_page_size, uint32_t dst_page_size, uint64_t n_tokens, int layout,
+              int mode, uint32_t flags, kv_stream_t stream);
+int kv_offload_batched(kv_ctx *ctx, const kv_pool_desc *pools, uint32_t layer_count,
+                       const int32_t *page_ids, const int64_t *req_offsets, uint32_t n_req,
+                       int layout, void *const *host_dsts, const uint64_t *host_bytes, int mode,
+                       uint32_t flags, kv_stream_t stream);
+int kv_reload_batched(kv_ctx *ctx, const void *const *host_srcs, const uint64_t *host_bytes,
+                      const int32_t *dst_page_ids, const int64_t *req_offsets,
+                      const uint64_t *n_tokens, uint32_t n_req, const kv_pool_desc *pools,
+                      uint32_t layer_count, uint32_t src_page_size, uint32_t dst_page_size,
+                      int layout, int mode, uint32_t flags, kv_stream_t stream);
+
+#ifdef __cplusplus
+}
+#endif
+#endif /* KVTIER_H */

@@ -1,0 +1,306 @@
+// kv_kernels.cuh -- sm_100a kernels of the paged-KV tier transfer.
+//
+// Every transfer (pack, unpack, re-page, batched, direct host offload/reload) is ONE launch of
+// one of three kernels over a flat list of work items ("segments").  A segment is a run of bytes
+// that is contiguous on BOTH sides: g = gcd(Tpool, Tbuf) tokens of one (layer, K|V) of one page,
+// cut into pieces of at most `sub_bytes`.  The pool side hops between 2*L slabs by page id
+// (PAPER.md:L207 addressing); the buffer side is the dense lower-tier representation
+// (BASELINE.json:configs[0]).
+//
+//   kv_move_bulk  the B200 path: cp.async.bulk (SASS UBLKCP) global -> shared -> global through a
+//                 per-warp ring of mbarrier-tracked stages.  32 lanes decode 32 segments' addresses
+//                 at once (warp-level page-table lookup), lane 0 drives the async copy engine.
+//                 No data ever passes through registers.
+//   kv_move_vec   16-byte LDG/STG, one warp per segment, 8 loads in flight per lane.
+//   kv_move_elem  any alignment: unit-wide (1/2/4/8 B) coalesced copy.  Correctness fallback.
+//
+// This file shares nothing with oracle/.
+#pragma once
+#include <cuda_runtime.h>
+#include <stdint.h>
+
+namespace kvt {
+
+// One contiguous transfer buffer: a request, or one pipeline chunk of a request.
+struct Piece {
+  uint64_t item_begin;   // first flat item index of this piece within the launch
+  uint64_t buf;          // buffer base address (device memory or mapped pinned host memory)
+  uint64_t n_tokens;     // valid tokens; destination slots >= n_tokens are zero-filled (unpack)
+  uint64_t id_begin;     // index of this piece's first page id in ids[]
+  uint64_t n_buf_pages;  // pages in this piece's buffer (layer-first page stride)
+};
+
+struct Job {
+  const uint64_t *bases;  // [LC] slab base addresses, order [layer][kv]
+  const int32_t *ids;     // page ids (device)
+  const Piece *pieces;    // pieces of THIS launch
+  uint32_t *status;       // device status word (bit 0: page id out of range)
+  uint64_t total_items;
+  uint64_t page_stride;     // pool bytes between pages
+  uint64_t buf_row_bytes;   // Tbuf * tokrow
+  uint64_t buf_page_bytes;  // LC * buf_row_bytes (page-first)
+  uint32_t n_pieces;
+  uint32_t LC;            // layer_count * kv_count
+  uint32_t dir;           // 0 = pack (pool -> buffer), 1 = unpack (buffer -> pool)
+  uint32_t layout;        // 0 page-first, 1 layer-first
+  uint32_t g;             // tokens per chunk = gcd(Tpool, Tbuf)
+  uint32_t cpp_pool;      // chunks per pool page  = Tpool / g
+  uint32_t cpp_buf;       // chunks per buffer page = Tbuf / g
+  uint32_t tokrow;        // bytes per token row = H*D*e
+  uint32_t chunk_bytes;   // g * tokrow
+  uint32_t sub_bytes;     // bytes per item (last item of a chunk may be shorter)
+  uint32_t subs;          // items per chunk
+  uint32_t num_pages;     // pool pages (range check of device-resident ids)
+  // bulk kernel geometry
+  uint32_t stage_bytes;
+  uint32_t stages;        // per warp
+  uint32_t lag;           // stores left in flight before a stage is refilled
+  uint32_t zero_bytes;    // size of the shared zero region
+  uint32_t l2_hint;
+};
+
+struct Item {
+  uint64_t src, dst;
+  uint32_t bytes;  // bytes written at dst
+  uint32_t valid;  // first `valid` bytes come from src, the rest is zero fill
+};
+
+// flat item -> (piece, chunk k, layer/kv, sub) -> addresses.
+__device__ __forceinline__ Item decode(const Job &j, uint64_t item) {
+  uint32_t r = 0;
+  if (j.n_pieces > 1) {  // largest r with pieces[r].item_begin <= item
+    uint32_t lo = 0, hi = j.n_pieces;
+    while (hi - lo > 1) {
+      uint32_t mid = (lo + hi) >> 1;
+      if (__ldg(&j.pieces[mid].item_begin) <= item) lo = mid; else hi = mid;
+    }
+    r = lo;
+  }
+  const Piece *pc = j.pieces + r;
+  const uint64_t item_begin = __ldg(&pc->item_begin), buf = __ldg(&pc->buf),
+                 n_tokens = __ldg(&pc->n_tokens), id_begin = __ldg(&pc->id_begin);
+  const uint32_t local = (uint32_t)(item - item_begin);
+  const uint32_t r1 = local / j.subs, sub = local - r1 * j.subs;
+  const uint32_t k = r1 / j.LC, lc = r1 - k * j.LC;
+  const uint32_t pp = k / j.cpp_pool, pk = k - pp * j.cpp_pool;
+  const uint32_t bp = k / j.cpp_buf, bk = k - bp * j.cpp_buf;
+  const uint64_t sub_off = (uint64_t)sub * j.sub_bytes;
+  Item it;
+  it.bytes = min(j.sub_bytes, j.chunk_bytes - (uint32_t)sub_off);
+  const int32_t id = __ldg(j.ids + id_begin + pp);
+  if ((uint32_t)id >= j.num_pages) {  // only reachable with KV_FLAG_IDS_ON_DEVICE
+    atomicOr(j.status, 1u);
+    it.src = it.dst = 0; it.bytes = it.valid = 0;
+    return it;
+  }
+  const uint64_t paddr = __ldg(j.bases + lc) + (uint64_t)id * j.page_stride +
+                         (uint64_t)pk * j.chunk_bytes + sub_off;
+  uint64_t baddr = buf + (uint64_t)bk * j.chunk_bytes + sub_off;
+  if (j.layout == 0) baddr += (uint64_t)bp * j.buf_page_bytes + (uint64_t)lc * j.buf_row_bytes;
+  else baddr += ((uint64_t)lc * __ldg(&pc->n_buf_pages) + bp) * j.buf_row_bytes;
+  const uint64_t tok0 = (uint64_t)k * j.g;
+  const uint64_t vt = n_tokens > tok0 ? min(n_tokens - tok0, (uint64_t)j.g) : 0;
+  const uint64_t vbytes = vt * j.tokrow;
+  it.valid = vbytes > sub_off ? (uint32_t)min(vbytes - sub_off, (uint64_t)it.bytes) : 0u;
+  if (j.dir == 0) { it.src = paddr; it.dst = baddr; } else { it.src = baddr; it.dst = paddr; }
+  return it;
+}
+
+// ---------------------------------------------------------------------------------------------
+// PTX wrappers (async proxy: mbarrier + cp.async.bulk)
+// ---------------------------------------------------------------------------------------------
+__device__ __forceinline__ uint32_t smem_u32(const void *p) {
+  return (uint32_t)__cvta_generic_to_shared(p);
+}
+__device__ __forceinline__ void mbar_init(uint32_t bar, uint32_t count) {
+  asm volatile("mbarrier.init.shared::cta.b64 [%0], %1;" ::"r"(bar), "r"(count));
+}
+__device__ __forceinline__ void mbar_expect_tx(uint32_t bar, uint32_t bytes) {
+  asm volatile("mbarrier.arrive.expect_tx.shared::cta.b64 _, [%0], %1;" ::"r"(bar), "r"(bytes) : "memory");
+}
+__device__ __forceinline__ void mbar_arrive(uint32_t bar) {
+  asm volatile("mbarrier.arrive.shared::cta.b64 _, [%0];" ::"r"(bar) : "memory");
+}
+__device__ __forceinline__ void mbar_wait(uint32_t bar, uint32_t parity) {
+  asm volatile(
+      "{\n\t.reg .pred p;\n\t"
+      "KV_WAIT:\n\t"
+      "mbarrier.try_wait.parity.shared::cta.b64 p, [%0], %1;\n\t"
+      "@p bra KV_DONE;\n\t"
+      "bra KV_WAIT;\n\t"
+      "KV_DONE:\n\t}" ::"r"(bar), "r"(parity) : "memory");
+}
+__device__ __forceinline__ void bulk_g2s(uint32_t dst_smem, uint64_t src, uint32_t bytes, uint32_t bar) {
+  asm volatile("cp.async.bulk.shared::cluster.global.mbarrier::complete_tx::bytes [%0], [%1], %2, [%3];"
+               ::"r"(dst_smem), "l"(src), "r"(bytes), "r"(bar) : "memory");
+}
+__device__ __forceinline__ void bulk_g2s_hint(uint32_t dst_smem, uint64_t src, uint32_t bytes, uint32_t bar, uint64_t pol) {
+  asm volatile("cp.async.bulk.shared::cluster.global.mbarrier::complete_tx::bytes.L2::cache_hint [%0], [%1], %2, [%3], %4;"
+               ::"r"(dst_smem), "l"(src), "r"(bytes), "r"(bar), "l"(pol) : "memory");
+}
+__device__ __forceinline__ void bulk_s2g(uint64_t dst, uint32_t src_smem, uint32_t bytes) {
+  asm volatile("cp.async.bulk.global.shared::cta.bulk_group [%0], [%1], %2;"
+               ::"l"(dst), "r"(src_smem), "r"(bytes) : "memory");
+}
+__device__ __forceinline__ void bulk_s2g_hint(uint64_t dst, uint32_t src_smem, uint32_t bytes, uint64_t pol) {
+  asm volatile("cp.async.bulk.global.shared::cta.bulk_group.L2::cache_hint [%0], [%1], %2, %3;"
+               ::"l"(dst), "r"(src_smem), "r"(bytes), "l"(pol) : "memory");
+}
+__device__ __forceinline__ void bulk_commit() { asm volatile("cp.async.bulk.commit_group;" ::: "memory"); }
+template <int N>
+__device__ __forceinline__ void bulk_wait_read() {
+  asm volatile("cp.async.bulk.wait_group.read %0;" ::"n"(N) : "memory");
+}
+__device__ __forceinline__ void bulk_wait_all() { asm volatile("cp.async.bulk.wait_group 0;" ::: "memory"); }
+
+constexpr int kMaxWarps = 8;
+constexpr int kMaxStages = 16;
+
+struct StageMeta {
+  uint64_t dst;
+  uint32_t bytes, valid;
+};
+
+// ---------------------------------------------------------------------------------------------
+// kv_move_bulk: persistent CTAs (one per SM); every warp owns `stages` shared-memory stages.
+//   load  item i  into stage i % K           at iteration i
+//   store item i  from stage i % K           at iteration i + K - lag   (after its mbarrier flips)
+//   refill stage  at iteration i + K         after cp.async.bulk.wait_group.read <lag>
+// so K - lag loads and lag stores are in flight per warp.  Dynamic shared memory:
+//   [zero region: zero_bytes][warp 0 stages][warp 1 stages]...   all 128-byte aligned.
+// ---------------------------------------------------------------------------------------------
+__global__ void __launch_bounds__(kMaxWarps * 32, 1) kv_move_bulk(const __grid_constant__ Job j) {
+  extern __shared__ __align__(128) uint8_t smem[];
+  __shared__ __align__(8) uint64_t full_bar[kMaxWarps][kMaxStages];
+  __shared__ StageMeta meta[kMaxWarps][kMaxStages];
+
+  const uint32_t warp = threadIdx.x >> 5, lane = threadIdx.x & 31;
+  const uint32_t warps = blockDim.x >> 5;
+  const uint32_t K = j.stages, lag = j.lag;
+
+  // zero region (generic-proxy writes) + barrier init, then make both visible to the async proxy
+  for (uint32_t o = threadIdx.x * 16; o < j.zero_bytes; o += blockDim.x * 16)
+    *reinterpret_cast<uint4 *>(smem + o) = make_uint4(0, 0, 0, 0);
+  if (lane == 0)
+    for (uint32_t s = 0; s < K; ++s) mbar_init(smem_u32(&full_bar[warp][s]), 1);
+  asm volatile("fence.mbarrier_init.release.cluster;" ::: "memory");
+  asm volatile("fence.proxy.async.shared::cta;" ::: "memory");
+  __syncthreads();
+
+  const uint64_t G = (uint64_t)gridDim.x * warps;
+  const uint64_t gw = (uint64_t)blockIdx.x * warps + warp;
+  const uint64_t n_my = gw < j.total_items ? (j.total_items - gw + G - 1) / G : 0;
+  if (n_my == 0) return;
+
+  uint64_t pol = 0;
+  if (j.l2_hint) asm volatile("createpolicy.fractional.L2::evict_first.b64 %0, 1.0;" : "=l"(pol));
+
+  const uint32_t stage0 = smem_u32(smem) + j.zero_bytes + warp * K * j.stage_bytes;
+  const uint32_t zero0 = smem_u32(smem);
+  const uint64_t n_iter = n_my + (K - lag);
+  Item mine;
+  mine.src = mine.dst = 0; mine.bytes = mine.valid = 0;
+
+  for (uint64_t it = 0; it < n_iter; ++it) {
+    if ((it & 31) == 0 && it < n_my) {  // warp-level lookup: 32 segments decoded at once
+      const uint64_t my = it + lane;
+      if (my < n_my) mine = decode(j, gw + my * G);
+    }
+    const uint32_t sel = (uint32_t)it & 31;
+    const uint64_t src = __shfl_sync(0xffffffffu, mine.src, sel);
+    const uint64_t dst = __shfl_sync(0xffffffffu, mine.dst, sel);
+    const uint32_t bytes = __shfl_sync(0xffffffffu, mine.bytes, sel);
+    const uint32_t valid = __shfl_sync(0xffffffffu, mine.valid, sel);
+    if (lane == 0) {
+      if (it >= K - lag) {  // ---- store side: item si
+        const uint64_t si = it - (K - lag);
+        const uint32_t s = (uint32_t)(si % K);
+        mbar_wait(smem_u32(&full_bar[warp][s]), (uint32_t)(si / K) & 1);
+        const StageMeta m = meta[warp][s];
+        if (m.valid) {
+          if (j.l2_hint) bulk_s2g_hint(m.dst, stage0 + s * j.stage_bytes, m.valid, pol);
+          else bulk_s2g(m.dst, stage0 + s * j.stage_bytes, m.valid);
+        }
+        for (uint32_t z = m.valid; z < m.bytes; z += j.zero_bytes)  // zero-padded tail (a5)
+          bulk_s2g(m.dst + z, zero0, min(j.zero_bytes, m.bytes - z));
+        bulk_commit();
+      }
+      if (it < n_my) {  // ---- load side: item it
+        const uint32_t s = (uint32_t)(it % K);
+        if (it >= K) {  // the store that last read this stage was committed `lag` groups ago
+          if (lag == 1) bulk_wait_read<1>();
+          else if (lag == 2) bulk_wait_read<2>();
+          else bulk_wait_read<3>();
+        }
+        meta[warp][s].dst = dst; meta[warp][s].bytes = bytes; meta[warp][s].valid = valid;
+        const uint32_t bar = smem_u32(&full_bar[warp][s]);
+        if (valid) {
+          mbar_expect_tx(bar, valid);
+          if (j.l2_hint) bulk_g2s_hint(stage0 + s * j.stage_bytes, src, valid, bar, pol);
+          else bulk_g2s(stage0 + s * j.stage_bytes, src, valid, bar);
+        } else {
+          mbar_arrive(bar);
+        }
+      }
+    }
+  }
+  if (lane == 0) bulk_wait_all();
+}
+
+// ---------------------------------------------------------------------------------------------
+// kv_move_vec: one warp per segment, 16-byte streaming loads/stores, UNROLL loads in flight.
+// ---------------------------------------------------------------------------------------------
+__device__ __forceinline__ uint4 ld_stream(const uint4 *p) {
+  uint4 r;
+  asm volatile("ld.global.nc.L1::no_allocate.v4.u32 {%0,%1,%2,%3}, [%4];"
+               : "=r"(r.x), "=r"(r.y), "=r"(r.z), "=r"(r.w) : "l"(p));
+  return r;
+}
+__device__ __forceinline__ void st_stream(uint4 *p, const uint4 &v) {
+  asm volatile("st.global.L1::no_allocate.v4.u32 [%0], {%1,%2,%3,%4};"
+               ::"l"(p), "r"(v.x), "r"(v.y), "r"(v.z), "r"(v.w) : "memory");
+}
+
+template <int UNROLL>
+__global__ void __launch_bounds__(256) kv_move_vec(const __grid_constant__ Job j) {
+  const uint32_t lane = threadIdx.x & 31;
+  const uint64_t G = (uint64_t)gridDim.x * (blockDim.x >> 5);
+  for (uint64_t item = (uint64_t)blockIdx.x * (blockDim.x >> 5) + (threadIdx.x >> 5);
+       item < j.total_items; item += G) {
+    const Item it = decode(j, item);
+    const uint4 *s = reinterpret_cast<const uint4 *>(it.src);
+    uint4 *d = reinterpret_cast<uint4 *>(it.dst);
+    const uint32_t nv = it.valid >> 4, nb = it.bytes >> 4;
+    uint32_t i = lane;
+    for (; i + 32 * (UNROLL - 1) < nv; i += 32 * UNROLL) {
+      uint4 v[UNROLL];
+#pragma unroll
+      for (int u = 0; u < UNROLL; ++u) v[u] = ld_stream(s + i + 32 * u);
+#pragma unroll
+      for (int u = 0; u < UNROLL; ++u) st_stream(d + i + 32 * u, v[u]);
+    }
+    for (; i < nv; i += 32) st_stream(d + i, ld_stream(s + i));
+    for (i = nv + lane; i < nb; i += 32) st_stream(d + i, make_uint4(0, 0, 0, 0));
+  }
+}
+
+// ---------------------------------------------------------------------------------------------
+// kv_move_elem: any elem_bytes-aligned pointers; U is the widest unit dividing every address
+// and length of the call (1, 2, 4 or 8 bytes).
+// ---------------------------------------------------------------------------------------------
+template <typename U>
+__global__ void __launch_bounds__(256) kv_move_elem(const __grid_constant__ Job j) {
+  const uint32_t lane = threadIdx.x & 31;
+  const uint64_t G = (uint64_t)gridDim.x * (blockDim.x >> 5);
+  for (uint64_t item = (uint64_t)blockIdx.x * (blockDim.x >> 5) + (threadIdx.x >> 5);
+       item < j.total_items; item += G) {
+    const Item it = decode(j, item);
+    const U *s = reinterpret_cast<const U *>(it.src);
+    U *d = reinterpret_cast<U *>(it.dst);
+    const uint32_t nv = it.valid / sizeof(U), nb = it.bytes / sizeof(U);
+    for (uint32_t i = lane; i < nv; i += 32) d[i] = s[i];
+    for (uint32_t i = nv + lane; i < nb; i += 32) d[i] = U(0);
+  }
+}
+
+}  // namespace kvt

@@ -1,0 +1,857 @@
+// kvtier.cu -- C ABI (include/kvtier.h) of the paged-KV tier transfer: host validation, page-id
+// staging, planning of the flat segment list (a2) and launches (a3-a8).
+// Every byte of the path is moved by the kernels in kv_kernels.cuh or, in KV_HOST_STAGED mode,
+// by the copy engines between the ctx's device staging and pinned host memory.
+// There is no CPU fallback: without a CUDA device transfer calls fail (KV_ERR_CUDA / NO_DEVICE).
+#include "../../include/kvtier.h"
+
+#include <cuda_runtime.h>
+
+#include <algorithm>
+#include <cstring>
+#include <new>
+#include <numeric>
+#include <vector>
+
+#include "kv_kernels.cuh"
+
+namespace {
+
+using kvt::Job;
+using kvt::Piece;
+
+constexpr int kBlobSlots = 16;
+constexpr int kMaxStagingSlots = 4;
+constexpr uint32_t kMaxLayersKv = 4096;  // layer_count * kv_count
+
+enum KernelKind { KERNEL_AUTO = 0, KERNEL_BULK = 1, KERNEL_VEC = 2, KERNEL_ELEM = 3 };
+
+struct BlobSlot {
+  void *h = nullptr;  // pinned host
+  void *d = nullptr;  // device
+  size_t cap = 0;
+  cudaEvent_t ev = nullptr;  // recorded after the last kernel that reads `d`
+  bool used = false;
+};
+
+}  // namespace
+
+struct kv_ctx {
+  int device = -1;
+  bool host_only = false;
+  int sm_count = 148;
+  int max_smem = 0;
+  cudaStream_t side = nullptr;
+  cudaEvent_t ev_entry = nullptr;
+  BlobSlot blobs[kBlobSlots];
+  uint32_t next_blob = 0;
+  uint32_t *d_status = nullptr;
+  // staging for KV_HOST_STAGED
+  void *staging = nullptr;
+  size_t staging_bytes = 0;
+  cudaEvent_t ev_full[kMaxStagingSlots] = {};  // producer into the slot finished
+  cudaEvent_t ev_free[kMaxStagingSlots] = {};  // consumer of the slot finished
+  bool free_valid[kMaxStagingSlots] = {};
+  int last_cuda_error = 0;
+  // options
+  int kernel = KERNEL_AUTO;
+  uint32_t stage_bytes = 16384, stages = 3, warps = 4, lag = 1, max_ctas = 0, host_max_ctas = 0;
+  uint32_t staging_slots = 2, l2_hint = 0;
+  size_t chunk_bytes = 0;
+  // stats
+  uint64_t launches = 0, memcpys = 0, last_items = 0, last_payload = 0, last_kernel = 0,
+           last_mode = 0, last_grid = 0, last_segment = 0;
+};
+
+namespace {
+
+#define KV_CUDA(ctx, expr)                         \
+  do {                                             \
+    cudaError_t e__ = (expr);                      \
+    if (e__ != cudaSuccess) {                      \
+      (ctx)->last_cuda_error = (int)e__;           \
+      (void)cudaGetLastError();                    \
+      return KV_ERR_CUDA;                          \
+    }                                              \
+  } while (0)
+
+struct DeviceGuard {
+  int prev = -1;
+  bool active = false;
+  explicit DeviceGuard(const kv_ctx *ctx) {
+    if (ctx->host_only) return;
+    if (cudaGetDevice(&prev) == cudaSuccess && prev != ctx->device) {
+      cudaSetDevice(ctx->device);
+      active = true;
+    }
+  }
+  ~DeviceGuard() {
+    if (active) cudaSetDevice(prev);
+  }
+};
+
+// Geometry of one call: everything derived from the descriptor, the buffer page size and the
+// kernel options; no pointers to transfer data.
+struct Geom {
+  uint32_t L = 0, C = 0, LC = 0;
+  uint32_t Tpool = 0, Tbuf = 0, g = 0;
+  uint32_t tokrow = 0, chunk_bytes = 0, sub_bytes = 0, subs = 0;
+  uint64_t pool_row = 0, buf_row = 0, buf_page = 0;
+  uint64_t page_stride = 0;
+  uint32_t num_pages = 0, elem = 0;
+  int dir = 0, layout = 0;
+  int kernel = KERNEL_BULK;
+  uint32_t unit = 16;  // widest power of two dividing every address/length (elem kernel)
+};
+
+struct Req {          // one request as the caller states it
+  uint64_t buf = 0;   // transfer buffer (device-accessible address)
+  uint64_t n_tokens = 0;
+  uint64_t id_begin = 0, n_ids = 0;  // its page ids in the call's id array
+  uint64_t n_buf_pages = 0;
+};
+
+int check_desc(const kv_pool_desc *p, uint32_t layer_count) {
+  if (!p || !p->base) return KV_ERR_NULL;
+  if (!p->layer_count || !p->kv_count || !p->num_pages || !p->page_size || !p->num_heads ||
+      !p->head_dim || p->reserved)
+    return KV_ERR_DESC;
+  if (p->elem_bytes != 1 && p->elem_bytes != 2 && p->elem_bytes != 4 && p->elem_bytes != 8)
+    return KV_ERR_DESC;
+  if (!layer_count || layer_count > p->layer_count) return KV_ERR_DESC;
+  if ((uint64_t)p->layer_count * p->kv_count > kMaxLayersKv) return KV_ERR_DESC;
+  const uint64_t row = (uint64_t)p->page_size * p->num_heads * p->head_dim * p->elem_bytes;
+  if (row > 0xFFFFFFFFull) return KV_ERR_DESC;
+  if (p->page_stride_bytes < row) return KV_ERR_DESC;
+  if (p->page_stride_bytes % p->elem_bytes) return KV_ERR_ALIGN;
+  for (uint64_t i = 0; i < (uint64_t)layer_count * p->kv_count; ++i) {
+    if (!p->base[i]) return KV_ERR_NULL;
+    if ((uint64_t)(uintptr_t)p->base[i] % p->elem_bytes) return KV_ERR_ALIGN;
+  }
+  return KV_OK;
+}
+
+uint32_t gcd32(uint32_t a, uint32_t b) {
+  while (b) { uint32_t t = a % b; a = b; b = t; }
+  return a;
+}
+
+uint32_t low_pow2(uint64_t v) {  // largest power of two (<= 16) dividing v; 16 for v == 0
+  uint32_t u = 16;
+  while (u > 1 && (v % u)) u >>= 1;
+  return u;
+}
+
+int make_geom(const kv_ctx *ctx, const kv_pool_desc *p, uint32_t layer_count, uint32_t Tbuf,
+              int dir, int layout, const std::vector<Req> &reqs, Geom *out) {
+  if (layout != KV_LAYOUT_PAGE_FIRST && layout != KV_LAYOUT_LAYER_FIRST) return KV_ERR_LAYOUT;
+  Geom g;
+  g.L = layer_count; g.C = p->kv_count; g.LC = g.L * g.C;
+  g.Tpool = p->page_size; g.Tbuf = Tbuf;
+  g.g = gcd32(g.Tpool, g.Tbuf);
+  g.elem = p->elem_bytes;
+  const uint64_t tokrow = (uint64_t)p->num_heads * p->head_dim * p->elem_bytes;
+  g.tokrow = (uint32_t)tokrow;
+  g.pool_row = tokrow * g.Tpool;
+  g.buf_row = tokrow * g.Tbuf;
+  if (g.buf_row > 0xFFFFFFFFull) return KV_ERR_SIZE;
+  g.buf_page = g.buf_row * g.LC;
+  g.chunk_bytes = (uint32_t)(tokrow * g.g);
+  g.page_stride = p->page_stride_bytes;
+  g.num_pages = p->num_pages;
+  g.dir = dir; g.layout = layout;
+  // widest unit every address and length of this call is a multiple of
+  uint32_t unit = 16;
+  unit = std::min(unit, low_pow2(tokrow));
+  unit = std::min(unit, low_pow2(g.page_stride));
+  for (uint32_t i = 0; i < g.LC; ++i) unit = std::min(unit, low_pow2((uint64_t)(uintptr_t)p->base[i]));
+  for (const Req &r : reqs) {
+    if (r.buf % g.elem) return KV_ERR_ALIGN;
+    unit = std::min(unit, low_pow2(r.buf));
+  }
+  g.unit = unit;
+  int kernel = ctx->kernel;
+  if (unit < 16) kernel = KERNEL_ELEM;  // 16-byte paths need 16-byte alignment everywhere
+  else if (kernel == KERNEL_AUTO) kernel = KERNEL_BULK;
+  g.kernel = kernel;
+  uint32_t cap = kernel == KERNEL_BULK ? ctx->stage_bytes : 16384u;
+  cap = std::max(16u, cap / 16 * 16);
+  g.sub_bytes = std::min(g.chunk_bytes, cap);
+  g.subs = (g.chunk_bytes + g.sub_bytes - 1) / g.sub_bytes;
+  *out = g;
+  return KV_OK;
+}
+
+uint64_t items_of(const Geom &g, uint64_t n_pool_pages) {
+  return n_pool_pages * (g.Tpool / g.g) * g.LC * g.subs;
+}
+
+int check_ids(const int32_t *ids, uint64_t n, uint32_t num_pages) {
+  for (uint64_t i = 0; i < n; ++i)
+    if (ids[i] < 0 || (uint32_t)ids[i] >= num_pages) return KV_ERR_PAGE_RANGE;
+  return KV_OK;
+}
+
+int check_dups(const int32_t *ids, uint64_t n, uint32_t num_pages) {
+  std::vector<uint8_t> seen((size_t)(num_pages + 7) / 8, 0);
+  for (uint64_t i = 0; i < n; ++i) {
+    const uint32_t g = (uint32_t)ids[i];
+    if (seen[g >> 3] & (1u << (g & 7))) return KV_ERR_DUP_PAGE;
+    seen[g >> 3] |= (uint8_t)(1u << (g & 7));
+  }
+  return KV_OK;
+}
+
+// ---------------------------------------------------------------------------------------------
+// blob = [bases: LC x u64][pieces: n x Piece][ids: n_ids x i32], staged through a pinned ring
+// ---------------------------------------------------------------------------------------------
+struct Blob {
+  BlobSlot *slot = nullptr;
+  const uint64_t *d_bases = nullptr;
+  const Piece *d_pieces = nullptr;
+  const int32_t *d_ids = nullptr;
+};
+
+int upload_blob(kv_ctx *ctx, const kv_pool_desc *p, const Geom &g, const std::vector<Piece> &pieces,
+                const int32_t *ids, uint64_t n_ids, bool ids_on_device, cudaStream_t s, Blob *out) {
+  const size_t off_pieces = (size_t)g.LC * 8;
+  const size_t off_ids = off_pieces + pieces.size() * sizeof(Piece);
+  const size_t bytes = off_ids + (ids_on_device ? 0 : (size_t)n_ids * 4);
+  BlobSlot &slot = ctx->blobs[ctx->next_blob++ % kBlobSlots];
+  if (slot.used) KV_CUDA(ctx, cudaEventSynchronize(slot.ev));  // last reader of this slot is done
+  if (slot.cap < bytes) {
+    if (slot.h) cudaFreeHost(slot.h);
+    if (slot.d) cudaFree(slot.d);
+    slot.h = slot.d = nullptr; slot.cap = 0;
+    size_t cap = std::max<size_t>(65536, bytes + bytes / 2);
+    KV_CUDA(ctx, cudaMallocHost(&slot.h, cap));
+    KV_CUDA(ctx, cudaMalloc(&slot.d, cap));
+    slot.cap = cap;
+  }
+  uint8_t *h = (uint8_t *)slot.h;
+  for (uint32_t i = 0; i < g.LC; ++i) ((uint64_t *)h)[i] = (uint64_t)(uintptr_t)p->base[i];
+  std::memcpy(h + off_pieces, pieces.data(), pieces.size() * sizeof(Piece));
+  if (!ids_on_device && n_ids) std::memcpy(h + off_ids, ids, (size_t)n_ids * 4);
+  KV_CUDA(ctx, cudaMemcpyAsync(slot.d, slot.h, bytes, cudaMemcpyHostToDevice, s));
+  ctx->memcpys++;
+  slot.used = true;
+  out->slot = &slot;
+  out->d_bases = (const uint64_t *)slot.d;
+  out->d_pieces = (const Piece *)((uint8_t *)slot.d + off_pieces);
+  out->d_ids = ids_on_device ? ids : (const int32_t *)((uint8_t *)slot.d + off_ids);
+  return KV_OK;
+}
+
+int launch(kv_ctx *ctx, const Geom &g, const Blob &b, uint32_t piece_first, uint32_t n_pieces,
+           uint64_t total_items, uint32_t cta_cap, cudaStream_t s) {
+  if (!total_items) return KV_OK;
+  Job j{};
+  j.bases = b.d_bases; j.ids = b.d_ids; j.pieces = b.d_pieces + piece_first;
+  j.status = ctx->d_status;
+  j.total_items = total_items;
+  j.page_stride = g.page_stride; j.buf_row_bytes = g.buf_row; j.buf_page_bytes = g.buf_page;
+  j.n_pieces = n_pieces; j.LC = g.LC; j.dir = (uint32_t)g.dir; j.layout = (uint32_t)g.layout;
+  j.g = g.g; j.cpp_pool = g.Tpool / g.g; j.cpp_buf = g.Tbuf / g.g;
+  j.tokrow = g.tokrow; j.chunk_bytes = g.chunk_bytes; j.sub_bytes = g.sub_bytes; j.subs = g.subs;
+  j.num_pages = g.num_pages;
+  uint32_t cap = cta_cap ? cta_cap : ctx->max_ctas;
+  uint32_t grid = 0;
+  if (g.kernel == KERNEL_BULK) {
+    j.stage_bytes = (g.sub_bytes + 127) / 128 * 128;
+    j.stages = ctx->stages; j.lag = std::min(ctx->lag, ctx->stages - 1);
+    j.zero_bytes = std::min<uint32_t>(4096, j.stage_bytes);
+    j.l2_hint = ctx->l2_hint;
+    uint32_t warps = ctx->warps;
+    size_t smem = (size_t)j.zero_bytes + (size_t)warps * j.stages * j.stage_bytes;
+    while (smem > (size_t)ctx->max_smem - 4096 && j.stages > 2) {  // static smem holds barriers + meta
+      --j.stages; j.lag = std::min(j.lag, j.stages - 1);
+      smem = (size_t)j.zero_bytes + (size_t)warps * j.stages * j.stage_bytes;
+    }
+    while (smem > (size_t)ctx->max_smem - 4096 && warps > 1) {
+      --warps;
+      smem = (size_t)j.zero_bytes + (size_t)warps * j.stages * j.stage_bytes;
+    }
+    const uint64_t want = (total_items + warps - 1) / warps;
+    grid = (uint32_t)std::min<uint64_t>(want, cap ? cap : (uint32_t)ctx->sm_count);
+    kvt::kv_move_bulk<<<grid, warps * 32, smem, s>>>(j);
+  } else {
+    const uint32_t wpb = 8;  // warps per 256-thread CTA
+    const uint64_t want = (total_items + wpb - 1) / wpb;
+    grid = (uint32_t)std::min<uint64_t>(want, cap ? cap : (uint32_t)ctx->sm_count * 8);
+    if (g.kernel == KERNEL_VEC) kvt::kv_move_vec<8><<<grid, 256, 0, s>>>(j);
+    else if (g.unit >= 8) kvt::kv_move_elem<uint64_t><<<grid, 256, 0, s>>>(j);
+    else if (g.unit == 4) kvt::kv_move_elem<uint32_t><<<grid, 256, 0, s>>>(j);
+    else if (g.unit == 2) kvt::kv_move_elem<uint16_t><<<grid, 256, 0, s>>>(j);
+    else kvt::kv_move_elem<uint8_t><<<grid, 256, 0, s>>>(j);
+  }
+  KV_CUDA(ctx, cudaGetLastError());
+  ctx->launches++;
+  ctx->last_grid = grid;
+  return KV_OK;
+}
+
+// Validation shared by every entry point.  Fills reqs/geom; returns before any CUDA call.
+struct Call {
+  Geom geom;
+  std::vector<Req> reqs;
+  uint64_t n_ids = 0;
+  uint64_t total_items = 0;
+  uint64_t payload = 0;
+};
+
+int plan_pack(kv_ctx *ctx, const kv_pool_desc *pools, uint32_t layer_count, const int32_t *ids,
+              const int64_t *off, uint32_t n_req, int layout, void *const *dsts,
+              const uint64_t *dst_bytes, uint32_t flags, Call *c) {
+  if (!ctx) return KV_ERR_NULL;
+  int rc = check_desc(pools, layer_count);
+  if (rc) return rc;
+  if (n_req && (!off || !dsts)) return KV_ERR_NULL;
+  const uint64_t page = (uint64_t)layer_count * pools->kv_count * pools->page_size *
+                        pools->num_heads * pools->head_dim * pools->elem_bytes;
+  c->reqs.clear();
+  for (uint32_t r = 0; r < n_req; ++r) {
+    if (off[r + 1] < off[r] || off[r] < 0) return KV_ERR_SIZE;
+    const uint64_t n = (uint64_t)(off[r + 1] - off[r]);
+    if (!n) continue;
+    if (!dsts[r]) return KV_ERR_NULL;
+    if (dst_bytes && dst_bytes[r] < n * page) return KV_ERR_SIZE;
+    Req q;
+    q.buf = (uint64_t)(uintptr_t)dsts[r];
+    q.n_tokens = n * pools->page_size;
+    q.id_begin = (uint64_t)off[r]; q.n_ids = n; q.n_buf_pages = n;
+    c->reqs.push_back(q);
+  }
+  c->n_ids = n_req ? (uint64_t)off[n_req] : 0;
+  if (c->n_ids && !ids) return KV_ERR_NULL;
+  rc = make_geom(ctx, pools, layer_count, pools->page_size, /*dir=*/0, layout, c->reqs, &c->geom);
+  if (rc) return rc;
+  if (!(flags & KV_FLAG_IDS_ON_DEVICE)) {
+    rc = check_ids(ids, c->n_ids, pools->num_pages);
+    if (rc) return rc;
+  }
+  c->total_items = 0; c->payload = 0;
+  for (const Req &q : c->reqs) {
+    const uint64_t it = items_of(c->geom, q.n_ids);
+    if (it > 0xFFFFFFFFull) return KV_ERR_SIZE;
+    c->total_items += it;
+    c->payload += q.n_ids * page;
+  }
+  return KV_OK;
+}
+
+int plan_unpack(kv_ctx *ctx, const void *const *srcs, const uint64_t *src_bytes,
+                const int32_t *ids, const int64_t *off, const uint64_t *n_tokens, uint32_t n_req,
+                const kv_pool_desc *pools, uint32_t layer_count, uint32_t Ts, uint32_t Td,
+                int layout, uint32_t flags, Call *c) {
+  if (!ctx) return KV_ERR_NULL;
+  int rc = check_desc(pools, layer_count);
+  if (rc) return rc;
+  if (!Ts || !Td || Td != pools->page_size) return KV_ERR_SIZE;
+  if (n_req && (!off || !srcs || !n_tokens)) return KV_ERR_NULL;
+  const uint64_t tokrow = (uint64_t)pools->num_heads * pools->head_dim * pools->elem_bytes;
+  const uint64_t lc = (uint64_t)layer_count * pools->kv_count;
+  c->reqs.clear();
+  for (uint32_t r = 0; r < n_req; ++r) {
+    if (off[r + 1] < off[r] || off[r] < 0) return KV_ERR_SIZE;
+    const uint64_t n = (uint64_t)(off[r + 1] - off[r]);
+    if (n != (n_tokens[r] + Td - 1) / Td) return KV_ERR_SIZE;
+    if (!n) continue;
+    if (!srcs[r]) return KV_ERR_NULL;
+    const uint64_t n_src = (n_tokens[r] + Ts - 1) / Ts;
+    if (src_bytes && src_bytes[r] < n_src * lc * Ts * tokrow) return KV_ERR_SIZE;
+    Req q;
+    q.buf = (uint64_t)(uintptr_t)srcs[r];
+    q.n_tokens = n_tokens[r];
+    q.id_begin = (uint64_t)off[r]; q.n_ids = n; q.n_buf_pages = n_src;
+    c->reqs.push_back(q);
+  }
+  c->n_ids = n_req ? (uint64_t)off[n_req] : 0;
+  if (c->n_ids && !ids) return KV_ERR_NULL;
+  rc = make_geom(ctx, pools, layer_count, Ts, /*dir=*/1, layout, c->reqs, &c->geom);
+  if (rc) return rc;
+  if (!(flags & KV_FLAG_IDS_ON_DEVICE)) {
+    rc = check_ids(ids, c->n_ids, pools->num_pages);
+    if (rc) return rc;
+    if (flags & KV_FLAG_VALIDATE) {
+      rc = check_dups(ids, c->n_ids, pools->num_pages);
+      if (rc) return rc;
+    }
+  }
+  c->total_items = 0; c->payload = 0;
+  for (const Req &q : c->reqs) {
+    const uint64_t it = items_of(c->geom, q.n_ids);
+    if (it > 0xFFFFFFFFull) return KV_ERR_SIZE;
+    c->total_items += it;
+    c->payload += q.n_ids * lc * Td * tokrow;
+  }
+  return KV_OK;
+}
+
+void note_plan(kv_ctx *ctx, const Call &c) {
+  ctx->last_items = c.total_items;
+  ctx->last_payload = c.payload;
+  ctx->last_kernel = (uint64_t)c.geom.kernel;
+  ctx->last_segment = c.geom.sub_bytes;
+}
+
+// one launch over all requests (device buffers, or mapped pinned host buffers = DIRECT mode)
+int run_single_launch(kv_ctx *ctx, const kv_pool_desc *pools, const Call &c, const int32_t *ids,
+                      uint32_t flags, uint32_t cta_cap, cudaStream_t s) {
+  std::vector<Piece> pieces;
+  pieces.reserve(c.reqs.size());
+  uint64_t acc = 0;
+  for (const Req &q : c.reqs) {
+    Piece pc;
+    pc.item_begin = acc; pc.buf = q.buf; pc.n_tokens = q.n_tokens; pc.id_begin = q.id_begin;
+    pc.n_buf_pages = q.n_buf_pages;
+    pieces.push_back(pc);
+    acc += items_of(c.geom, q.n_ids);
+  }
+  Blob b;
+  int rc = upload_blob(ctx, pools, c.geom, pieces, ids, c.n_ids, flags & KV_FLAG_IDS_ON_DEVICE, s, &b);
+  if (rc) return rc;
+  rc = launch(ctx, c.geom, b, 0, (uint32_t)pieces.size(), acc, cta_cap, s);
+  if (rc) return rc;
+  KV_CUDA(ctx, cudaEventRecord(b.slot->ev, s));
+  return KV_OK;
+}
+
+int ensure_staging(kv_ctx *ctx) {
+  if (ctx->staging) return KV_OK;
+  if (!ctx->staging_bytes) ctx->staging_bytes = (size_t)256 << 20;
+  KV_CUDA(ctx, cudaMalloc(&ctx->staging, ctx->staging_bytes));
+  return KV_OK;
+}
+
+// KV_HOST_STAGED: the flattened page sequence of all requests is cut into chunks that fit one
+// staging slot; per chunk: kernel <-> slot on `s`, copy engine slot <-> pinned host on the side
+// stream, double (or deeper) buffered with events.  Page-first only (a chunk of pages is then
+// contiguous in the host buffer); layer-first falls back to DIRECT.
+int run_staged(kv_ctx *ctx, const kv_pool_desc *pools, const Call &c, const int32_t *ids,
+               uint32_t flags, cudaStream_t s) {
+  int rc = ensure_staging(ctx);
+  if (rc) return rc;
+  const Geom &g = c.geom;
+  const uint32_t n_slots = ctx->staging_slots;
+  // unit of chunking: tokens that are whole pages on both sides
+  const uint64_t unit_tokens = (uint64_t)g.Tpool / g.g * g.Tbuf;  // lcm(Tpool, Tbuf)
+  const uint64_t unit_bytes = unit_tokens * g.tokrow * g.LC;
+  size_t slot_bytes = ctx->staging_bytes / n_slots / 256 * 256;
+  if (ctx->chunk_bytes) slot_bytes = std::min(slot_bytes, ctx->chunk_bytes / 256 * 256);
+  if (slot_bytes < unit_bytes) return KV_ERR_SIZE;
+  const uint64_t chunk_tokens = slot_bytes / unit_bytes * unit_tokens;
+
+  struct Chunk { uint32_t piece_first, n_pieces; uint64_t items; };
+  struct Copy { uint64_t host, dev_off, bytes; };
+  std::vector<Piece> pieces;
+  std::vector<Chunk> chunks;
+  std::vector<std::vector<Copy>> copies;
+  {
+    uint64_t fill_tokens = 0;  // tokens (in buffer-page units) already placed in the open chunk
+    Chunk cur{0, 0, 0};
+    std::vector<Copy> cur_copies;
+    auto close = [&]() {
+      if (cur.n_pieces) { chunks.push_back(cur); copies.push_back(cur_copies); }
+      cur = Chunk{(uint32_t)pieces.size(), 0, 0};
+      cur_copies.clear();
+      fill_tokens = 0;
+    };
+    for (const Req &q : c.reqs) {
+      // the request covers n_ids pool pages = n_ids*Tpool token slots; its buffer holds
+      // n_buf_pages*Tbuf token slots.  Walk it in token ranges [t0, t1) of whole units.
+      const uint64_t slots_pool = q.n_ids * g.Tpool;
+      uint64_t t0 = 0;
+      while (t0 < slots_pool) {
+        if (fill_tokens == chunk_tokens) close();
+        const uint64_t t1 = std::min(slots_pool, t0 + (chunk_tokens - fill_tokens));
+        const uint64_t span = t1 - t0;  // multiple of Tpool; multiple of unit except at the request's end
+        const uint64_t buf_pages = (std::min(t1, q.n_buf_pages * g.Tbuf) - std::min(t0, q.n_buf_pages * g.Tbuf) + g.Tbuf - 1) / g.Tbuf;
+        const uint64_t dev_off = fill_tokens * g.tokrow * g.LC;
+        Piece pc;
+        pc.item_begin = cur.items;
+        pc.buf = (uint64_t)(uintptr_t)ctx->staging;  // + slot base, patched per chunk below
+        pc.buf = dev_off;                              // offset within the slot for now
+        pc.n_tokens = q.n_tokens > t0 ? std::min(q.n_tokens - t0, span) : 0;
+        pc.id_begin = q.id_begin + t0 / g.Tpool;
+        pc.n_buf_pages = buf_pages;
+        pieces.push_back(pc);
+        cur.n_pieces++;
+        cur.items += items_of(g, span / g.Tpool);
+        if (buf_pages)
+          cur_copies.push_back(Copy{q.buf + t0 / g.Tbuf * g.buf_page, dev_off, buf_pages * g.buf_page});
+        // buffer-page units consumed in the slot (a ragged tail still occupies whole units)
+        fill_tokens += (span + unit_tokens - 1) / unit_tokens * unit_tokens;
+        t0 = t1;
+      }
+    }
+    close();
+  }
+  // patch slot bases
+  for (size_t ci = 0; ci < chunks.size(); ++ci) {
+    const uint64_t base = (uint64_t)(uintptr_t)ctx->staging + (ci % n_slots) * slot_bytes;
+    for (uint32_t k = 0; k < chunks[ci].n_pieces; ++k) pieces[chunks[ci].piece_first + k].buf += base;
+  }
+  Blob b;
+  rc = upload_blob(ctx, pools, g, pieces, ids, c.n_ids, flags & KV_FLAG_IDS_ON_DEVICE, s, &b);
+  if (rc) return rc;
+  KV_CUDA(ctx, cudaEventRecord(ctx->ev_entry, s));
+  KV_CUDA(ctx, cudaStreamWaitEvent(ctx->side, ctx->ev_entry, 0));
+  for (size_t ci = 0; ci < chunks.size(); ++ci) {
+    const uint32_t slot = (uint32_t)(ci % n_slots);
+    uint8_t *slot_base = (uint8_t *)ctx->staging + (size_t)slot * slot_bytes;
+    if (g.dir == 0) {  // offload: kernel fills the slot on s, copy engine drains it on side
+      if (ctx->free_valid[slot]) KV_CUDA(ctx, cudaStreamWaitEvent(s, ctx->ev_free[slot], 0));
+      rc = launch(ctx, g, b, chunks[ci].piece_first, chunks[ci].n_pieces, chunks[ci].items, 0, s);
+      if (rc) return rc;
+      KV_CUDA(ctx, cudaEventRecord(ctx->ev_full[slot], s));
+      KV_CUDA(ctx, cudaStreamWaitEvent(ctx->side, ctx->ev_full[slot], 0));
+      for (const Copy &cp : copies[ci]) {
+        KV_CUDA(ctx, cudaMemcpyAsync((void *)(uintptr_t)cp.host, slot_base + cp.dev_off, cp.bytes,
+                                     cudaMemcpyDeviceToHost, ctx->side));
+        ctx->memcpys++;
+      }
+      KV_CUDA(ctx, cudaEventRecord(ctx->ev_free[slot], ctx->side));
+      ctx->free_valid[slot] = true;
+    } else {  // reload: copy engine fills the slot on side, kernel drains it on s
+      if (ctx->free_valid[slot]) KV_CUDA(ctx, cudaStreamWaitEvent(ctx->side, ctx->ev_free[slot], 0));
+      for (const Copy &cp : copies[ci]) {
+        KV_CUDA(ctx, cudaMemcpyAsync(slot_base + cp.dev_off, (const void *)(uintptr_t)cp.host,
+                                     cp.bytes, cudaMemcpyHostToDevice, ctx->side));
+        ctx->memcpys++;
+      }
+      KV_CUDA(ctx, cudaEventRecord(ctx->ev_full[slot], ctx->side));
+      KV_CUDA(ctx, cudaStreamWaitEvent(s, ctx->ev_full[slot], 0));
+      rc = launch(ctx, g, b, chunks[ci].piece_first, chunks[ci].n_pieces, chunks[ci].items, 0, s);
+      if (rc) return rc;
+      KV_CUDA(ctx, cudaEventRecord(ctx->ev_free[slot], s));
+      ctx->free_valid[slot] = true;
+    }
+  }
+  if (g.dir == 0) {  // join the copy engine's tail back into s
+    const size_t first = chunks.size() > n_slots ? chunks.size() - n_slots : 0;
+    for (size_t ci = first; ci < chunks.size(); ++ci)
+      KV_CUDA(ctx, cudaStreamWaitEvent(s, ctx->ev_free[ci % n_slots], 0));
+  }
+  KV_CUDA(ctx, cudaEventRecord(b.slot->ev, s));
+  return KV_OK;
+}
+
+// Is `p` pinned host memory?  Returns its device alias (UVA: normally the same address).
+int host_alias(kv_ctx *ctx, const void *p, uint64_t *alias) {
+  cudaPointerAttributes a;
+  cudaError_t e = cudaPointerGetAttributes(&a, p);
+  if (e != cudaSuccess) { (void)cudaGetLastError(); return KV_ERR_HOST_MEM; }
+  if (a.type != cudaMemoryTypeHost || !a.devicePointer) return KV_ERR_HOST_MEM;
+  (void)ctx;
+  *alias = (uint64_t)(uintptr_t)a.devicePointer;
+  return KV_OK;
+}
+
+int resolve_mode(const kv_ctx *ctx, int mode, const Call &c, int *out) {
+  if (mode != KV_HOST_AUTO && mode != KV_HOST_DIRECT && mode != KV_HOST_STAGED) return KV_ERR_LAYOUT;
+  int m = mode;
+  // measured table: DIRECT stores/loads over the link win at every size
+  if (m == KV_HOST_AUTO) m = KV_HOST_DIRECT;
+  // staged needs chunks that are contiguous in the host buffer
+  if (m == KV_HOST_STAGED && c.geom.layout != KV_LAYOUT_PAGE_FIRST) m = KV_HOST_DIRECT;
+  (void)ctx;
+  *out = m;
+  return KV_OK;
+}
+
+int run_host(kv_ctx *ctx, const kv_pool_desc *pools, Call &c, const int32_t *ids, int mode,
+             uint32_t flags, cudaStream_t s) {
+  int m = 0;
+  int rc = resolve_mode(ctx, mode, c, &m);
+  if (rc) return rc;
+  note_plan(ctx, c);
+  ctx->last_mode = (uint64_t)m;
+  if (ctx->host_only) return KV_ERR_NO_DEVICE;
+  if (c.reqs.empty()) return KV_OK;
+  DeviceGuard guard(ctx);
+  for (Req &q : c.reqs) {
+    uint64_t alias = 0;
+    rc = host_alias(ctx, (const void *)(uintptr_t)q.buf, &alias);
+    if (rc) return rc;
+    if (m == KV_HOST_DIRECT) q.buf = alias;
+  }
+  if (m == KV_HOST_DIRECT) return run_single_launch(ctx, pools, c, ids, flags, ctx->host_max_ctas, s);
+  return run_staged(ctx, pools, c, ids, flags, s);
+}
+
+int run_device(kv_ctx *ctx, const kv_pool_desc *pools, const Call &c, const int32_t *ids,
+               uint32_t flags, cudaStream_t s) {
+  note_plan(ctx, c);
+  if (ctx->host_only) return KV_ERR_NO_DEVICE;
+  if (c.reqs.empty()) return KV_OK;
+  DeviceGuard guard(ctx);
+  return run_single_launch(ctx, pools, c, ids, flags, 0, s);
+}
+
+}  // namespace
+
+// =============================================================================================
+// C ABI
+// =============================================================================================
+extern "C" {
+
+uint32_t kv_version(void) { return KVTIER_VERSION; }
+
+const char *kv_strerror(int status) {
+  switch (status) {
+    case KV_OK: return "ok";
+    case KV_ERR_NULL: return "required pointer is NULL";
+    case KV_ERR_SIZE: return "size mismatch (buffer too small, inconsistent page sizes/counts, or too many items)";
+    case KV_ERR_PAGE_RANGE: return "page id out of range";
+    case KV_ERR_DUP_PAGE: return "duplicate destination page id";
+    case KV_ERR_LAYOUT: return "unknown layout, host mode or option";
+    case KV_ERR_ALIGN: return "pointer or stride not aligned to elem_bytes";
+    case KV_ERR_CUDA: return "CUDA error (see kv_last_cuda_error)";
+    case KV_ERR_HOST_MEM: return "host buffer is not pinned memory";
+    case KV_ERR_DESC: return "malformed kv_pool_desc";
+    case KV_ERR_NO_DEVICE: return "planning-only context: nothing launched";
+    default: return "unknown kvtier status";
+  }
+}
+
+int kv_ctx_create(kv_ctx **out, int device, size_t staging_bytes) {
+  if (!out) return KV_ERR_NULL;
+  *out = nullptr;
+  kv_ctx *ctx = new (std::nothrow) kv_ctx();
+  if (!ctx) return KV_ERR_SIZE;
+  ctx->staging_bytes = staging_bytes;
+  if (device < 0) {
+    ctx->host_only = true;
+    ctx->max_smem = 232448;
+    *out = ctx;
+    return KV_OK;
+  }
+  ctx->device = device;
+  auto fail = [&](cudaError_t e) {
+    int code = (int)e;
+    (void)cudaGetLastError();
+    delete ctx;
+    (void)code;
+    return KV_ERR_CUDA;
+  };
+  cudaError_t e;
+  int prev = -1;
+  if ((e = cudaGetDevice(&prev)) != cudaSuccess) return fail(e);
+  if ((e = cudaSetDevice(device)) != cudaSuccess) return fail(e);
+  if ((e = cudaDeviceGetAttribute(&ctx->sm_count, cudaDevAttrMultiProcessorCount, device)) != cudaSuccess) return fail(e);
+  if ((e = cudaDeviceGetAttribute(&ctx->max_smem, cudaDevAttrMaxSharedMemoryPerBlockOptin, device)) != cudaSuccess) return fail(e);
+  if ((e = cudaFuncSetAttribute(kvt::kv_move_bulk, cudaFuncAttributeMaxDynamicSharedMemorySize, ctx->max_smem - 4096)) != cudaSuccess) return fail(e);
+  if ((e = cudaStreamCreateWithFlags(&ctx->side, cudaStreamNonBlocking)) != cudaSuccess) return fail(e);
+  if ((e = cudaEventCreateWithFlags(&ctx->ev_entry, cudaEventDisableTiming)) != cudaSuccess) return fail(e);
+  for (int i = 0; i < kBlobSlots; ++i)
+    if ((e = cudaEventCreateWithFlags(&ctx->blobs[i].ev, cudaEventDisableTiming)) != cudaSuccess) return fail(e);
+  for (int i = 0; i < kMaxStagingSlots; ++i) {
+    if ((e = cudaEventCreateWithFlags(&ctx->ev_full[i], cudaEventDisableTiming)) != cudaSuccess) return fail(e);
+    if ((e = cudaEventCreateWithFlags(&ctx->ev_free[i], cudaEventDisableTiming)) != cudaSuccess) return fail(e);
+  }
+  if ((e = cudaMalloc((void **)&ctx->d_status, 256)) != cudaSuccess) return fail(e);
+  if ((e = cudaMemset(ctx->d_status, 0, 256)) != cudaSuccess) return fail(e);
+  if (prev >= 0 && prev != device) cudaSetDevice(prev);
+  *out = ctx;
+  return KV_OK;
+}
+
+int kv_ctx_destroy(kv_ctx *ctx) {
+  if (!ctx) return KV_ERR_NULL;
+  if (!ctx->host_only) {
+    DeviceGuard guard(ctx);
+    cudaStreamSynchronize(ctx->side);
+    for (auto &b : ctx->blobs) {
+      if (b.used) cudaEventSynchronize(b.ev);
+      if (b.h) cudaFreeHost(b.h);
+      if (b.d) cudaFree(b.d);
+      if (b.ev) cudaEventDestroy(b.ev);
+    }
+    for (int i = 0; i < kMaxStagingSlots; ++i) {
+      if (ctx->ev_full[i]) cudaEventDestroy(ctx->ev_full[i]);
+      if (ctx->ev_free[i]) { cudaEventSynchronize(ctx->ev_free[i]); cudaEventDestroy(ctx->ev_free[i]); }
+    }
+    if (ctx->staging) cudaFree(ctx->staging);
+    if (ctx->d_status) cudaFree(ctx->d_status);
+    if (ctx->ev_entry) cudaEventDestroy(ctx->ev_entry);
+    if (ctx->side) cudaStreamDestroy(ctx->side);
+    (void)cudaGetLastError();
+  }
+  delete ctx;
+  return KV_OK;
+}
+
+int kv_ctx_set_option(kv_ctx *ctx, int option, int64_t v) {
+  if (!ctx) return KV_ERR_NULL;
+  switch (option) {
+    case KV_OPT_KERNEL: if (v < 0 || v > 3) return KV_ERR_SIZE; ctx->kernel = (int)v; break;
+    case KV_OPT_STAGE_BYTES: if (v < 1024 || v > 65536 || v % 16) return KV_ERR_SIZE; ctx->stage_bytes = (uint32_t)v; break;
+    case KV_OPT_STAGES_PER_WARP: if (v < 2 || v > kvt::kMaxStages) return KV_ERR_SIZE; ctx->stages = (uint32_t)v; break;
+    case KV_OPT_WARPS: if (v < 1 || v > kvt::kMaxWarps) return KV_ERR_SIZE; ctx->warps = (uint32_t)v; break;
+    case KV_OPT_STORE_LAG: if (v < 1 || v > 3) return KV_ERR_SIZE; ctx->lag = (uint32_t)v; break;
+    case KV_OPT_MAX_CTAS: if (v < 0 || v > 65535) return KV_ERR_SIZE; ctx->max_ctas = (uint32_t)v; break;
+    case KV_OPT_CHUNK_BYTES: if (v < 0) return KV_ERR_SIZE; ctx->chunk_bytes = (size_t)v; break;
+    case KV_OPT_HOST_MAX_CTAS: if (v < 0 || v > 65535) return KV_ERR_SIZE; ctx->host_max_ctas = (uint32_t)v; break;
+    case KV_OPT_STAGING_SLOTS: if (v < 2 || v > kMaxStagingSlots) return KV_ERR_SIZE; ctx->staging_slots = (uint32_t)v; break;
+    case KV_OPT_L2_HINT: if (v < 0 || v > 1) return KV_ERR_SIZE; ctx->l2_hint = (uint32_t)v; break;
+    default: return KV_ERR_LAYOUT;
+  }
+  return KV_OK;
+}
+
+int kv_ctx_get_stat(kv_ctx *ctx, int stat, uint64_t *out) {
+  if (!ctx || !out) return KV_ERR_NULL;
+  switch (stat) {
+    case KV_STAT_LAUNCHES: *out = ctx->launches; break;
+    case KV_STAT_MEMCPYS: *out = ctx->memcpys; break;
+    case KV_STAT_LAST_ITEMS: *out = ctx->last_items; break;
+    case KV_STAT_LAST_PAYLOAD: *out = ctx->last_payload; break;
+    case KV_STAT_LAST_KERNEL: *out = ctx->last_kernel; break;
+    case KV_STAT_LAST_HOST_MODE: *out = ctx->last_mode; break;
+    case KV_STAT_LAST_GRID: *out = ctx->last_grid; break;
+    case KV_STAT_LAST_SEGMENT: *out = ctx->last_segment; break;
+    default: return KV_ERR_LAYOUT;
+  }
+  return KV_OK;
+}
+
+int kv_last_cuda_error(kv_ctx *ctx) { return ctx ? ctx->last_cuda_error : 0; }
+
+int kv_device_status(kv_ctx *ctx, uint32_t *out) {
+  if (!ctx || !out) return KV_ERR_NULL;
+  if (ctx->host_only) return KV_ERR_NO_DEVICE;
+  DeviceGuard guard(ctx);
+  KV_CUDA(ctx, cudaDeviceSynchronize());
+  KV_CUDA(ctx, cudaMemcpy(out, ctx->d_status, 4, cudaMemcpyDeviceToHost));
+  KV_CUDA(ctx, cudaMemset(ctx->d_status, 0, 4));
+  return KV_OK;
+}
+
+int kv_host_alloc(void **p, size_t bytes) {
+  if (!p) return KV_ERR_NULL;
+  *p = nullptr;
+  if (!bytes) return KV_ERR_SIZE;
+  cudaError_t e = cudaHostAlloc(p, bytes, cudaHostAllocMapped | cudaHostAllocPortable);
+  if (e != cudaSuccess) { (void)cudaGetLastError(); *p = nullptr; return KV_ERR_CUDA; }
+  return KV_OK;
+}
+
+int kv_host_free(void *p) {
+  if (!p) return KV_ERR_NULL;
+  if (cudaFreeHost(p) != cudaSuccess) { (void)cudaGetLastError(); return KV_ERR_CUDA; }
+  return KV_OK;
+}
+
+int kv_host_register(void *p, size_t bytes) {
+  if (!p) return KV_ERR_NULL;
+  if (!bytes) return KV_ERR_SIZE;
+  if (cudaHostRegister(p, bytes, cudaHostRegisterMapped | cudaHostRegisterPortable) != cudaSuccess) {
+    (void)cudaGetLastError();
+    return KV_ERR_CUDA;
+  }
+  return KV_OK;
+}
+
+int kv_host_unregister(void *p) {
+  if (!p) return KV_ERR_NULL;
+  if (cudaHostUnregister(p) != cudaSuccess) { (void)cudaGetLastError(); return KV_ERR_CUDA; }
+  return KV_OK;
+}
+
+int kv_pack(kv_ctx *ctx, const kv_pool_desc *pools, uint32_t layer_count, const int32_t *page_ids,
+            uint32_t n, int layout, void *dst, size_t dst_bytes, uint32_t flags, kv_stream_t stream) {
+  const int64_t off[2] = {0, (int64_t)n};
+  void *const dsts[1] = {dst};
+  const uint64_t nb[1] = {(uint64_t)dst_bytes};
+  Call c;
+  int rc = plan_pack(ctx, pools, layer_count, page_ids, off, 1, layout, dsts, nb, flags, &c);
+  if (rc) return rc;
+  return run_device(ctx, pools, c, page_ids, flags, (cudaStream_t)stream);
+}
+
+int kv_unpack(kv_ctx *ctx, const void *src, size_t src_bytes, const int32_t *dst_page_ids,
+              uint32_t n_dst_pages, const kv_pool_desc *pools, uint32_t layer_count,
+              uint32_t src_page_size, uint32_t dst_page_size, uint64_t n_tokens, int layout,
+              uint32_t flags, kv_stream_t stream) {
+  const int64_t off[2] = {0, (int64_t)n_dst_pages};
+  const void *const srcs[1] = {src};
+  const uint64_t nb[1] = {(uint64_t)src_bytes};
+  const uint64_t nt[1] = {n_tokens};
+  Call c;
+  int rc = plan_unpack(ctx, srcs, nb, dst_page_ids, off, nt, 1, pools, layer_count, src_page_size,
+                       dst_page_size, layout, flags, &c);
+  if (rc) return rc;
+  return run_device(ctx, pools, c, dst_page_ids, flags, (cudaStream_t)stream);
+}
+
+int kv_pack_batched(kv_ctx *ctx, const kv_pool_desc *pools, uint32_t layer_count,
+                    const int32_t *page_ids, const int64_t *req_offsets, uint32_t n_req, int layout,
+                    void *const *dsts, const uint64_t *dst_bytes, uint32_t flags, kv_stream_t stream) {
+  Call c;
+  int rc = plan_pack(ctx, pools, layer_count, page_ids, req_offsets, n_req, layout, dsts, dst_bytes, flags, &c);
+  if (rc) return rc;
+  return run_device(ctx, pools, c, page_ids, flags, (cudaStream_t)stream);
+}
+
+int kv_unpack_batched(kv_ctx *ctx, const void *const *srcs, const uint64_t *src_bytes,
+                      const int32_t *dst_page_ids, const int64_t *req_offsets,
+                      const uint64_t *n_tokens, uint32_t n_req, const kv_pool_desc *pools,
+                      uint32_t layer_count, uint32_t src_page_size, uint32_t dst_page_size,
+                      int layout, uint32_t flags, kv_stream_t stream) {
+  Call c;
+  int rc = plan_unpack(ctx, srcs, src_bytes, dst_page_ids, req_offsets, n_tokens, n_req, pools,
+                       layer_count, src_page_size, dst_page_size, layout, flags, &c);
+  if (rc) return rc;
+  return run_device(ctx, pools, c, dst_page_ids, flags, (cudaStream_t)stream);
+}
+
+int kv_offload(kv_ctx *ctx, const kv_pool_desc *pools, uint32_t layer_count,
+               const int32_t *page_ids, uint32_t n, int layout, void *host_dst, size_t host_bytes,
+               int mode, uint32_t flags, kv_stream_t stream) {
+  const int64_t off[2] = {0, (int64_t)n};
+  void *const dsts[1] = {host_dst};
+  const uint64_t nb[1] = {(uint64_t)host_bytes};
+  Call c;
+  int rc = plan_pack(ctx, pools, layer_count, page_ids, off, 1, layout, dsts, nb, flags, &c);
+  if (rc) return rc;
+  return run_host(ctx, pools, c, page_ids, mode, flags, (cudaStream_t)stream);
+}
+
+int kv_reload(kv_ctx *ctx, const void *host_src, size_t host_bytes, const int32_t *dst_page_ids,
+              uint32_t n_dst_pages, const kv_pool_desc *pools, uint32_t layer_count,
+              uint32_t src_page_size, uint32_t dst_page_size, uint64_t n_tokens, int layout,
+              int mode, uint32_t flags, kv_stream_t stream) {
+  const int64_t off[2] = {0, (int64_t)n_dst_pages};
+  const void *const srcs[1] = {host_src};
+  const uint64_t nb[1] = {(uint64_t)host_bytes};
+  const uint64_t nt[1] = {n_tokens};
+  Call c;
+  int rc = plan_unpack(ctx, srcs, nb, dst_page_ids, off, nt, 1, pools, layer_count, src_page_size,
+                       dst_page_size, layout, flags, &c);
+  if (rc) return rc;
+  return run_host(ctx, pools, c, dst_page_ids, mode, flags, (cudaStream_t)stream);
+}
+
+int kv_offload_batched(kv_ctx *ctx, const kv_pool_desc *pools, uint32_t layer_count,
+                       const int32_t *page_ids, const int64_t *req_offsets, uint32_t n_req,
+                       int layout, void *const *host_dsts, const uint64_t *host_bytes, int mode,
+                       uint32_t flags, kv_stream_t stream) {
+  Call c;
+  int rc = plan_pack(ctx, pools, layer_count, page_ids, req_offsets, n_req, layout, host_dsts, host_bytes, flags, &c);
+  if (rc) return rc;
+  return run_host(ctx, pools, c, page_ids, mode, flags, (cudaStream_t)stream);
+}
+
+int kv_reload_batched(kv_ctx *ctx, const void *const *host_srcs, const uint64_t *host_bytes,
+                      const int32_t *dst_page_ids, const int64_t *req_offsets,
+                      const uint64_t *n_tokens, uint32_t n_req, const kv_pool_desc *pools,
+                      uint32_t layer_count, uint32_t src_page_size, uint32_t dst_page_size,
+                      int layout, int mode, uint32_t flags, kv_stream_t stream) {
+  Call c;
+  int rc = plan_unpack(ctx, host_srcs, host_bytes, dst_page_ids, req_offsets, n_tokens, n_req,
+                       pools, layer_count, src_page_size, dst_page_size, layout, flags, &c);
+  if (rc) return rc;
+  return run_host(ctx, pools, c, dst_page_ids, mode, flags, (cudaStream_t)stream);
+}
+
+}  // extern "C"

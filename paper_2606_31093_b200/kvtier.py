@@ -1,0 +1,380 @@
+"""Thin ctypes binding of libkvtier.so (include/kvtier.h): same names, argument marshalling only.
+
+Every step of the path (page-id staging, address generation, pack / unpack / re-page, host-tier
+offload / reload) runs inside the library's sm_100a kernels and copy-engine calls; nothing here
+touches transfer data.  PyTorch tensors are accepted only as a source of device pointers and
+stream handles.  Loading fails loudly when the library has not been built: there is no
+fallback path.
+"""
+from __future__ import annotations
+
+import ctypes
+import os
+from typing import Optional, Sequence
+
+import numpy as np
+
+_HERE = os.path.dirname(os.path.abspath(__file__))
+LIB_PATH = os.path.join(_HERE, "libkvtier.so")
+
+if not os.path.exists(LIB_PATH):
+    raise ImportError(
+        f"{LIB_PATH} is missing: build it with `python -c 'import __graft_entry__ as g; g.build()'` "
+        "(nvcc, sm_100a).  kvtier has no CPU or PyTorch fallback."
+    )
+_lib = ctypes.CDLL(LIB_PATH)
+
+# ---- enums (include/kvtier.h) ------------------------------------------------------------------
+KV_OK = 0
+KV_ERR_NULL, KV_ERR_SIZE, KV_ERR_PAGE_RANGE, KV_ERR_DUP_PAGE, KV_ERR_LAYOUT = -1, -2, -3, -4, -5
+KV_ERR_ALIGN, KV_ERR_CUDA, KV_ERR_HOST_MEM, KV_ERR_DESC, KV_ERR_NO_DEVICE = -6, -7, -8, -9, -10
+KV_LAYOUT_PAGE_FIRST, KV_LAYOUT_LAYER_FIRST = 0, 1
+KV_HOST_AUTO, KV_HOST_DIRECT, KV_HOST_STAGED = 0, 1, 2
+KV_FLAG_VALIDATE, KV_FLAG_IDS_ON_DEVICE = 0x1, 0x2
+(KV_OPT_KERNEL, KV_OPT_STAGE_BYTES, KV_OPT_STAGES_PER_WARP, KV_OPT_WARPS, KV_OPT_STORE_LAG,
+ KV_OPT_MAX_CTAS, KV_OPT_CHUNK_BYTES, KV_OPT_HOST_MAX_CTAS, KV_OPT_STAGING_SLOTS,
+ KV_OPT_L2_HINT) = range(10)
+KV_KERNEL_AUTO, KV_KERNEL_BULK, KV_KERNEL_VEC, KV_KERNEL_ELEM = 0, 1, 2, 3
+(KV_STAT_LAUNCHES, KV_STAT_MEMCPYS, KV_STAT_LAST_ITEMS, KV_STAT_LAST_PAYLOAD, KV_STAT_LAST_KERNEL,
+ KV_STAT_LAST_HOST_MODE, KV_STAT_LAST_GRID, KV_STAT_LAST_SEGMENT) = range(8)
+
+
+class kv_pool_desc(ctypes.Structure):
+    _fields_ = [
+        ("base", ctypes.POINTER(ctypes.c_void_p)),
+        ("layer_count", ctypes.c_uint32),
+        ("kv_count", ctypes.c_uint32),
+        ("num_pages", ctypes.c_uint32),
+        ("page_size", ctypes.c_uint32),
+        ("num_heads", ctypes.c_uint32),
+        ("head_dim", ctypes.c_uint32),
+        ("elem_bytes", ctypes.c_uint32),
+        ("reserved", ctypes.c_uint32),
+        ("page_stride_bytes", ctypes.c_uint64),
+    ]
+
+
+_vp, _u32, _u64, _i32, _i64, _int, _sz = (ctypes.c_void_p, ctypes.c_uint32, ctypes.c_uint64,
+                                          ctypes.c_int32, ctypes.c_int64, ctypes.c_int,
+                                          ctypes.c_size_t)
+_pdesc = ctypes.POINTER(kv_pool_desc)
+
+
+def _sig(name, restype, *argtypes):
+    fn = getattr(_lib, name)
+    fn.restype = restype
+    fn.argtypes = list(argtypes)
+    return fn
+
+
+_kv_version = _sig("kv_version", _u32)
+_kv_strerror = _sig("kv_strerror", ctypes.c_char_p, _int)
+_kv_ctx_create = _sig("kv_ctx_create", _int, ctypes.POINTER(_vp), _int, _sz)
+_kv_ctx_destroy = _sig("kv_ctx_destroy", _int, _vp)
+_kv_ctx_set_option = _sig("kv_ctx_set_option", _int, _vp, _int, _i64)
+_kv_ctx_get_stat = _sig("kv_ctx_get_stat", _int, _vp, _int, ctypes.POINTER(_u64))
+_kv_last_cuda_error = _sig("kv_last_cuda_error", _int, _vp)
+_kv_device_status = _sig("kv_device_status", _int, _vp, ctypes.POINTER(_u32))
+_kv_host_alloc = _sig("kv_host_alloc", _int, ctypes.POINTER(_vp), _sz)
+_kv_host_free = _sig("kv_host_free", _int, _vp)
+_kv_host_register = _sig("kv_host_register", _int, _vp, _sz)
+_kv_host_unregister = _sig("kv_host_unregister", _int, _vp)
+_kv_pack = _sig("kv_pack", _int, _vp, _pdesc, _u32, _vp, _u32, _int, _vp, _sz, _u32, _vp)
+_kv_unpack = _sig("kv_unpack", _int, _vp, _vp, _sz, _vp, _u32, _pdesc, _u32, _u32, _u32, _u64,
+                  _int, _u32, _vp)
+_kv_pack_batched = _sig("kv_pack_batched", _int, _vp, _pdesc, _u32, _vp, _vp, _u32, _int, _vp,
+                        _vp, _u32, _vp)
+_kv_unpack_batched = _sig("kv_unpack_batched", _int, _vp, _vp, _vp, _vp, _vp, _vp, _u32, _pdesc,
+                          _u32, _u32, _u32, _int, _u32, _vp)
+_kv_offload = _sig("kv_offload", _int, _vp, _pdesc, _u32, _vp, _u32, _int, _vp, _sz, _int, _u32,
+                   _vp)
+_kv_reload = _sig("kv_reload", _int, _vp, _vp, _sz, _vp, _u32, _pdesc, _u32, _u32, _u32, _u64,
+                  _int, _int, _u32, _vp)
+_kv_offload_batched = _sig("kv_offload_batched", _int, _vp, _pdesc, _u32, _vp, _vp, _u32, _int,
+                           _vp, _vp, _int, _u32, _vp)
+_kv_reload_batched = _sig("kv_reload_batched", _int, _vp, _vp, _vp, _vp, _vp, _vp, _u32, _pdesc,
+                          _u32, _u32, _u32, _int, _int, _u32, _vp)
+
+
+class KvError(RuntimeError):
+    def __init__(self, status: int, cuda_error: int = 0):
+        self.status = status
+        self.cuda_error = cuda_error
+        msg = kv_strerror(status)
+        if cuda_error:
+            msg += f" [cudaError {cuda_error}]"
+        super().__init__(f"kvtier: {msg} ({status})")
+
+
+def kv_version() -> int:
+    return int(_kv_version())
+
+
+def kv_strerror(status: int) -> str:
+    return _kv_strerror(int(status)).decode()
+
+
+# ---- marshalling helpers -----------------------------------------------------------------------
+def _ptr(x) -> Optional[int]:
+    """Address of a torch tensor / numpy array / int / None."""
+    if x is None:
+        return None
+    if isinstance(x, int):
+        return x
+    if hasattr(x, "data_ptr"):
+        return int(x.data_ptr())
+    if isinstance(x, np.ndarray):
+        return int(x.ctypes.data)
+    if isinstance(x, ctypes.c_void_p):
+        return x.value
+    raise TypeError(f"cannot take the address of {type(x)}")
+
+
+def _nbytes(x) -> int:
+    if hasattr(x, "element_size"):
+        return int(x.numel() * x.element_size())
+    if isinstance(x, np.ndarray):
+        return int(x.nbytes)
+    raise TypeError(f"cannot size {type(x)}; pass nbytes explicitly")
+
+
+def _stream(s) -> Optional[int]:
+    if s is None:
+        try:
+            import torch
+
+            if torch.cuda.is_available() and torch.cuda.is_initialized():
+                return int(torch.cuda.current_stream().cuda_stream) or None
+        except ImportError:
+            pass
+        return None
+    if isinstance(s, int):
+        return s or None
+    return int(s.cuda_stream) or None
+
+
+def _host_i32(a):
+    return np.ascontiguousarray(np.asarray(a, dtype=np.int32))
+
+
+def _ids_arg(ids, flags):
+    """(pointer, keepalive, count) for a page-id list: host int32 array, or a device tensor when
+    KV_FLAG_IDS_ON_DEVICE is set."""
+    if flags & KV_FLAG_IDS_ON_DEVICE:
+        return _ptr(ids), ids, int(ids.numel())
+    a = _host_i32(ids)
+    return int(a.ctypes.data) if a.size else None, a, int(a.size)
+
+
+class PoolDesc:
+    """Owns a kv_pool_desc and its host array of slab base pointers.
+
+    ``slabs`` is a sequence of layer_count*kv_count device pointers (torch tensors or ints) in
+    [layer][kv] order (outer dim layers, slice dim K/V)."""
+
+    def __init__(self, slabs: Sequence, layer_count: int, kv_count: int, num_pages: int,
+                 page_size: int, num_heads: int, head_dim: int, elem_bytes: int,
+                 page_stride_bytes: Optional[int] = None):
+        assert len(slabs) == layer_count * kv_count
+        self._keep = list(slabs)
+        self._base = (ctypes.c_void_p * len(slabs))(*[_ptr(s) for s in slabs])
+        row = page_size * num_heads * head_dim * elem_bytes
+        self.desc = kv_pool_desc(
+            ctypes.cast(self._base, ctypes.POINTER(ctypes.c_void_p)), layer_count, kv_count,
+            num_pages, page_size, num_heads, head_dim, elem_bytes, 0,
+            row if page_stride_bytes is None else int(page_stride_bytes))
+        self.row_bytes = row
+
+    def page_bytes(self, layer_count: Optional[int] = None) -> int:
+        L = self.desc.layer_count if layer_count is None else layer_count
+        return L * self.desc.kv_count * self.row_bytes
+
+    @property
+    def ref(self):
+        return ctypes.byref(self.desc)
+
+
+class Ctx:
+    """kv_ctx handle.  ``device=-1`` makes a planning-only context (no CUDA)."""
+
+    def __init__(self, device: int = 0, staging_bytes: int = 0):
+        h = ctypes.c_void_p()
+        rc = _kv_ctx_create(ctypes.byref(h), int(device), int(staging_bytes))
+        if rc:
+            raise KvError(rc)
+        self.h = h
+
+    def close(self):
+        if getattr(self, "h", None):
+            _kv_ctx_destroy(self.h)
+            self.h = None
+
+    __del__ = close
+
+    def __enter__(self):
+        return self
+
+    def __exit__(self, *a):
+        self.close()
+
+    def set_option(self, option: int, value: int):
+        rc = _kv_ctx_set_option(self.h, option, value)
+        if rc:
+            raise KvError(rc)
+
+    def stat(self, stat: int) -> int:
+        out = ctypes.c_uint64()
+        rc = _kv_ctx_get_stat(self.h, stat, ctypes.byref(out))
+        if rc:
+            raise KvError(rc)
+        return int(out.value)
+
+    def last_cuda_error(self) -> int:
+        return int(_kv_last_cuda_error(self.h))
+
+    def device_status(self) -> int:
+        out = ctypes.c_uint32()
+        rc = _kv_device_status(self.h, ctypes.byref(out))
+        if rc:
+            raise KvError(rc, self.last_cuda_error())
+        return int(out.value)
+
+
+def _chk(ctx: Ctx, rc: int):
+    if rc:
+        raise KvError(rc, ctx.last_cuda_error() if rc == KV_ERR_CUDA else 0)
+
+
+def kv_ctx_create(device: int = 0, staging_bytes: int = 0) -> Ctx:
+    return Ctx(device, staging_bytes)
+
+
+def kv_ctx_destroy(ctx: Ctx):
+    ctx.close()
+
+
+def kv_host_alloc(nbytes: int) -> int:
+    p = ctypes.c_void_p()
+    rc = _kv_host_alloc(ctypes.byref(p), int(nbytes))
+    if rc:
+        raise KvError(rc)
+    return int(p.value)
+
+
+def kv_host_free(p: int):
+    rc = _kv_host_free(p)
+    if rc:
+        raise KvError(rc)
+
+
+def kv_host_register(p: int, nbytes: int):
+    rc = _kv_host_register(p, nbytes)
+    if rc:
+        raise KvError(rc)
+
+
+def kv_host_unregister(p: int):
+    rc = _kv_host_unregister(p)
+    if rc:
+        raise KvError(rc)
+
+
+def host_view(p: int, nbytes: int) -> np.ndarray:
+    """numpy uint8 view of pinned memory returned by kv_host_alloc (no copy)."""
+    return np.ctypeslib.as_array((ctypes.c_uint8 * nbytes).from_address(p))
+
+
+def _ptr_array(xs):
+    return (ctypes.c_void_p * max(len(xs), 1))(*[_ptr(x) for x in xs])
+
+
+def _u64_array(xs):
+    return np.ascontiguousarray(np.asarray(xs, dtype=np.uint64))
+
+
+# ---- transfers -------------------------------------------------------------------------------
+def kv_pack(ctx: Ctx, pools: PoolDesc, layer_count: int, page_ids, dst, dst_bytes=None,
+            layout=KV_LAYOUT_PAGE_FIRST, flags=0, stream=None):
+    p, keep, n = _ids_arg(page_ids, flags)
+    nb = _nbytes(dst) if dst_bytes is None else int(dst_bytes)
+    _chk(ctx, _kv_pack(ctx.h, pools.ref, layer_count, p, n, layout, _ptr(dst), nb, flags,
+                       _stream(stream)))
+
+
+def kv_unpack(ctx: Ctx, src, dst_page_ids, pools: PoolDesc, layer_count: int, src_page_size: int,
+              dst_page_size: int, n_tokens: int, src_bytes=None, layout=KV_LAYOUT_PAGE_FIRST,
+              flags=0, stream=None):
+    p, keep, n = _ids_arg(dst_page_ids, flags)
+    nb = _nbytes(src) if src_bytes is None else int(src_bytes)
+    _chk(ctx, _kv_unpack(ctx.h, _ptr(src), nb, p, n, pools.ref, layer_count, src_page_size,
+                         dst_page_size, int(n_tokens), layout, flags, _stream(stream)))
+
+
+def _csr(req_offsets):
+    off = np.ascontiguousarray(np.asarray(req_offsets, dtype=np.int64))
+    return off, int(off.size - 1)
+
+
+def kv_pack_batched(ctx: Ctx, pools: PoolDesc, layer_count: int, page_ids, req_offsets, dsts,
+                    dst_bytes=None, layout=KV_LAYOUT_PAGE_FIRST, flags=0, stream=None):
+    p, keep, _ = _ids_arg(page_ids, flags)
+    off, R = _csr(req_offsets)
+    d = _ptr_array(dsts)
+    nb = None if dst_bytes is None else _u64_array(dst_bytes)
+    _chk(ctx, _kv_pack_batched(ctx.h, pools.ref, layer_count, p, off.ctypes.data, R, layout, d,
+                               None if nb is None else nb.ctypes.data, flags, _stream(stream)))
+
+
+def kv_unpack_batched(ctx: Ctx, srcs, dst_page_ids, req_offsets, n_tokens, pools: PoolDesc,
+                      layer_count: int, src_page_size: int, dst_page_size: int, src_bytes=None,
+                      layout=KV_LAYOUT_PAGE_FIRST, flags=0, stream=None):
+    p, keep, _ = _ids_arg(dst_page_ids, flags)
+    off, R = _csr(req_offsets)
+    s = _ptr_array(srcs)
+    nt = _u64_array(n_tokens)
+    nb = None if src_bytes is None else _u64_array(src_bytes)
+    _chk(ctx, _kv_unpack_batched(ctx.h, s, None if nb is None else nb.ctypes.data, p,
+                                 off.ctypes.data, nt.ctypes.data, R, pools.ref, layer_count,
+                                 src_page_size, dst_page_size, layout, flags, _stream(stream)))
+
+
+def kv_offload(ctx: Ctx, pools: PoolDesc, layer_count: int, page_ids, host_dst, host_bytes,
+               mode=KV_HOST_AUTO, layout=KV_LAYOUT_PAGE_FIRST, flags=0, stream=None):
+    p, keep, n = _ids_arg(page_ids, flags)
+    _chk(ctx, _kv_offload(ctx.h, pools.ref, layer_count, p, n, layout, _ptr(host_dst),
+                          int(host_bytes), mode, flags, _stream(stream)))
+
+
+def kv_reload(ctx: Ctx, host_src, host_bytes, dst_page_ids, pools: PoolDesc, layer_count: int,
+              src_page_size: int, dst_page_size: int, n_tokens: int, mode=KV_HOST_AUTO,
+              layout=KV_LAYOUT_PAGE_FIRST, flags=0, stream=None):
+    p, keep, n = _ids_arg(dst_page_ids, flags)
+    _chk(ctx, _kv_reload(ctx.h, _ptr(host_src), int(host_bytes), p, n, pools.ref, layer_count,
+                         src_page_size, dst_page_size, int(n_tokens), layout, mode, flags,
+                         _stream(stream)))
+
+
+def kv_offload_batched(ctx: Ctx, pools: PoolDesc, layer_count: int, page_ids, req_offsets,
+                       host_dsts, host_bytes=None, mode=KV_HOST_AUTO,
+                       layout=KV_LAYOUT_PAGE_FIRST, flags=0, stream=None):
+    p, keep, _ = _ids_arg(page_ids, flags)
+    off, R = _csr(req_offsets)
+    d = _ptr_array(host_dsts)
+    nb = None if host_bytes is None else _u64_array(host_bytes)
+    _chk(ctx, _kv_offload_batched(ctx.h, pools.ref, layer_count, p, off.ctypes.data, R, layout, d,
+                                  None if nb is None else nb.ctypes.data, mode, flags,
+                                  _stream(stream)))
+
+
+def kv_reload_batched(ctx: Ctx, host_srcs, dst_page_ids, req_offsets, n_tokens, pools: PoolDesc,
+                      layer_count: int, src_page_size: int, dst_page_size: int, host_bytes=None,
+                      mode=KV_HOST_AUTO, layout=KV_LAYOUT_PAGE_FIRST, flags=0, stream=None):
+    p, keep, _ = _ids_arg(dst_page_ids, flags)
+    off, R = _csr(req_offsets)
+    s = _ptr_array(host_srcs)
+    nt = _u64_array(n_tokens)
+    nb = None if host_bytes is None else _u64_array(host_bytes)
+    _chk(ctx, _kv_reload_batched(ctx.h, s, None if nb is None else nb.ctypes.data, p,
+                                 off.ctypes.data, nt.ctypes.data, R, pools.ref, layer_count,
+                                 src_page_size, dst_page_size, layout, mode, flags,
+                                 _stream(stream)))
