@@ -205,7 +205,7 @@ class Ctx:
         self.h = h
 
     def close(self):
-        if getattr(self, "h", None):
+        if getattr(self, "h", None) and _kv_ctx_destroy is not None:
             _kv_ctx_destroy(self.h)
             self.h = None
 
