@@ -194,29 +194,19 @@ def run_ours(args):
     from paper_2606_31093_b200 import kvtier as kv
     from paper_2606_31093_b200 import workloads as W
 
-    world = int(os.environ.get("WORLD_SIZE", "1"))
-    rank = int(os.environ.get("RANK", "0"))
-    local = int(os.environ.get("LOCAL_RANK", "0"))
+    from paper_2606_31093_b200.replicas import Replicas
+
     if not torch.cuda.is_available():
         raise SystemExit("bench.py: no CUDA device; kvtier has no CPU path (use --impl reference for the oracle)")
-    torch.cuda.set_device(local)
-    dist = None
-    if world > 1:
-        import torch.distributed as dist
-
-        dist.init_process_group("nccl", device_id=torch.device("cuda", local))
+    torch.cuda.set_device(int(os.environ.get("LOCAL_RANK", "0")))
+    rep = Replicas("nccl")
+    world, rank, local = rep.world, rep.rank, rep.local_rank
+    max_over_ranks = rep.max_over_ranks
 
     def barrier():
-        if dist is not None:
-            dist.barrier()
         torch.cuda.synchronize()
-
-    def max_over_ranks(x: float) -> float:
-        if dist is None:
-            return x
-        t = torch.tensor([x], dtype=torch.float64, device="cuda")
-        dist.all_reduce(t, op=dist.ReduceOp.MAX)
-        return float(t.item())
+        rep.barrier()
+        torch.cuda.synchronize()
 
     shape = W.QWEN3_OMNI.with_(P=args.pool_pages)
     P, n = shape.P, -(-args.prefix_tokens // shape.T)
@@ -347,8 +337,7 @@ def run_ours(args):
     if rank == 0:
         print(json.dumps(line))
     ctx.close()
-    if dist is not None:
-        dist.destroy_process_group()
+    rep.close()
 
 
 def main():

@@ -72,7 +72,7 @@ typedef enum kv_layout {
 
 /* How a host-tier transfer crosses the host link (BASELINE.json:north_star item 3). */
 typedef enum kv_host_mode {
-  KV_HOST_AUTO = 0,   /* chosen from the measured table in DESIGN.md */
+  KV_HOST_AUTO = 0,   /* chosen from the measured table in DESIGN.md: STAGED from 16 MiB of payload (page-first), else DIRECT */
   KV_HOST_DIRECT = 1, /* the kernel stores to / loads from mapped pinned memory over the link */
   KV_HOST_STAGED = 2, /* device staging + copy-engine cudaMemcpyAsync on the ctx's side stream, chunk-pipelined */
 } kv_host_mode;
@@ -107,6 +107,8 @@ typedef enum kv_option {
   KV_OPT_HOST_MAX_CTAS = 7,  /* grid cap for DIRECT host transfers (0 = same as device transfers) */
   KV_OPT_STAGING_SLOTS = 8,  /* staged host transfers: pipeline slots the staging buffer is cut into (2 .. 4) */
   KV_OPT_L2_HINT = 9,        /* bulk: 0 none, 1 evict_first cache hint on loads and stores */
+  KV_OPT_INLINE_TABLES = 10, /* 1 (default): page ids / slab bases ride in the kernel parameters when they fit (<= 31 KiB);
+                                0: always stage them through the ctx's pinned ring with one H2D copy */
 } kv_option;
 
 /* kv_ctx_get_stat keys */
@@ -128,7 +130,7 @@ const char *kv_strerror(int status); /* static string, never NULL */
 /* ---- context ------------------------------------------------------------------------------ */
 /* Creates the per-thread context on CUDA device `device`: side stream, events, the ring that
  * stages page-id lists, a device status word and (lazily, on the first STAGED transfer)
- * `staging_bytes` of device staging (0 = 256 MiB).  `device` < 0 creates a PLANNING-ONLY ctx
+ * `staging_bytes` of device staging (0 = 128 MiB = two 64 MiB pipeline slots).  `device` < 0 creates a PLANNING-ONLY ctx
  * that touches no CUDA API: every transfer call validates and plans, then returns
  * KV_ERR_NO_DEVICE instead of launching (used by host-side tests). */
 int kv_ctx_create(kv_ctx **out, int device, size_t staging_bytes);

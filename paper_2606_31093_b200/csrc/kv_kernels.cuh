@@ -57,7 +57,42 @@ struct Job {
   uint32_t lag;           // stores left in flight before a stage is refilled
   uint32_t zero_bytes;    // size of the shared zero region
   uint32_t l2_hint;
+  // inline tables (JobT<N>, N > 0): byte offsets into the kernel-parameter blob
+  uint32_t off_pieces, off_ids;
 };
+
+// The lookup tables of a launch: slab bases, page ids, pieces.  They live either in device memory
+// (staged through the ctx's pinned ring, JobT<0>) or, for calls whose tables fit, INSIDE the kernel
+// parameters (JobT<N>): one launch, no H2D copy, tables read through the constant bank.
+struct Tables {
+  const uint64_t *bases;
+  const int32_t *ids;
+  const Piece *pieces;
+};
+template <int N>
+struct JobT {
+  Job j;
+  alignas(8) uint8_t blob[N];  // [bases: LC x u64][pieces][ids]
+};
+template <>
+struct JobT<0> {
+  Job j;
+};
+template <int N>
+__device__ __forceinline__ Tables tables_of(const JobT<N> &p) {
+  if constexpr (N == 0) {
+    return Tables{p.j.bases, p.j.ids, p.j.pieces};
+  } else {  // j.ids != nullptr: device-resident ids supplied by the caller
+    return Tables{reinterpret_cast<const uint64_t *>(p.blob),
+                  p.j.ids ? p.j.ids : reinterpret_cast<const int32_t *>(p.blob + p.j.off_ids),
+                  reinterpret_cast<const Piece *>(p.blob + p.j.off_pieces)};
+  }
+}
+template <bool kGlobal, typename T>
+__device__ __forceinline__ T ldt(const T *p) {
+  if constexpr (kGlobal) return __ldg(p);
+  else return *p;
+}
 
 struct Item {
   uint64_t src, dst;
@@ -66,19 +101,20 @@ struct Item {
 };
 
 // flat item -> (piece, chunk k, layer/kv, sub) -> addresses.
-__device__ __forceinline__ Item decode(const Job &j, uint64_t item) {
+template <bool kGlobal>
+__device__ __forceinline__ Item decode(const Job &j, const Tables &tb, uint64_t item) {
   uint32_t r = 0;
   if (j.n_pieces > 1) {  // largest r with pieces[r].item_begin <= item
     uint32_t lo = 0, hi = j.n_pieces;
     while (hi - lo > 1) {
       uint32_t mid = (lo + hi) >> 1;
-      if (__ldg(&j.pieces[mid].item_begin) <= item) lo = mid; else hi = mid;
+      if (ldt<kGlobal>(&tb.pieces[mid].item_begin) <= item) lo = mid; else hi = mid;
     }
     r = lo;
   }
-  const Piece *pc = j.pieces + r;
-  const uint64_t item_begin = __ldg(&pc->item_begin), buf = __ldg(&pc->buf),
-                 n_tokens = __ldg(&pc->n_tokens), id_begin = __ldg(&pc->id_begin);
+  const Piece *pc = tb.pieces + r;
+  const uint64_t item_begin = ldt<kGlobal>(&pc->item_begin), buf = ldt<kGlobal>(&pc->buf),
+                 n_tokens = ldt<kGlobal>(&pc->n_tokens), id_begin = ldt<kGlobal>(&pc->id_begin);
   const uint32_t local = (uint32_t)(item - item_begin);
   const uint32_t r1 = local / j.subs, sub = local - r1 * j.subs;
   const uint32_t k = r1 / j.LC, lc = r1 - k * j.LC;
@@ -87,17 +123,18 @@ __device__ __forceinline__ Item decode(const Job &j, uint64_t item) {
   const uint64_t sub_off = (uint64_t)sub * j.sub_bytes;
   Item it;
   it.bytes = min(j.sub_bytes, j.chunk_bytes - (uint32_t)sub_off);
-  const int32_t id = __ldg(j.ids + id_begin + pp);
+  // caller-supplied device ids are global memory even when the other tables are inline
+  const int32_t id = (kGlobal || j.ids) ? __ldg(tb.ids + id_begin + pp) : tb.ids[id_begin + pp];
   if ((uint32_t)id >= j.num_pages) {  // only reachable with KV_FLAG_IDS_ON_DEVICE
     atomicOr(j.status, 1u);
     it.src = it.dst = 0; it.bytes = it.valid = 0;
     return it;
   }
-  const uint64_t paddr = __ldg(j.bases + lc) + (uint64_t)id * j.page_stride +
+  const uint64_t paddr = ldt<kGlobal>(tb.bases + lc) + (uint64_t)id * j.page_stride +
                          (uint64_t)pk * j.chunk_bytes + sub_off;
   uint64_t baddr = buf + (uint64_t)bk * j.chunk_bytes + sub_off;
   if (j.layout == 0) baddr += (uint64_t)bp * j.buf_page_bytes + (uint64_t)lc * j.buf_row_bytes;
-  else baddr += ((uint64_t)lc * __ldg(&pc->n_buf_pages) + bp) * j.buf_row_bytes;
+  else baddr += ((uint64_t)lc * ldt<kGlobal>(&pc->n_buf_pages) + bp) * j.buf_row_bytes;
   const uint64_t tok0 = (uint64_t)k * j.g;
   const uint64_t vt = n_tokens > tok0 ? min(n_tokens - tok0, (uint64_t)j.g) : 0;
   const uint64_t vbytes = vt * j.tokrow;
@@ -169,7 +206,10 @@ struct StageMeta {
 // so K - lag loads and lag stores are in flight per warp.  Dynamic shared memory:
 //   [zero region: zero_bytes][warp 0 stages][warp 1 stages]...   all 128-byte aligned.
 // ---------------------------------------------------------------------------------------------
-__global__ void __launch_bounds__(kMaxWarps * 32, 1) kv_move_bulk(const __grid_constant__ Job j) {
+template <int N>
+__global__ void __launch_bounds__(kMaxWarps * 32, 1) kv_move_bulk(const __grid_constant__ JobT<N> p) {
+  const Job &j = p.j;
+  const Tables tb = tables_of(p);
   extern __shared__ __align__(128) uint8_t smem[];
   __shared__ __align__(8) uint64_t full_bar[kMaxWarps][kMaxStages];
   __shared__ StageMeta meta[kMaxWarps][kMaxStages];
@@ -204,7 +244,7 @@ __global__ void __launch_bounds__(kMaxWarps * 32, 1) kv_move_bulk(const __grid_c
   for (uint64_t it = 0; it < n_iter; ++it) {
     if ((it & 31) == 0 && it < n_my) {  // warp-level lookup: 32 segments decoded at once
       const uint64_t my = it + lane;
-      if (my < n_my) mine = decode(j, gw + my * G);
+      if (my < n_my) mine = decode<N == 0>(j, tb, gw + my * G);
     }
     const uint32_t sel = (uint32_t)it & 31;
     const uint64_t src = __shfl_sync(0xffffffffu, mine.src, sel);
@@ -261,13 +301,15 @@ __device__ __forceinline__ void st_stream(uint4 *p, const uint4 &v) {
                ::"l"(p), "r"(v.x), "r"(v.y), "r"(v.z), "r"(v.w) : "memory");
 }
 
-template <int UNROLL>
-__global__ void __launch_bounds__(256) kv_move_vec(const __grid_constant__ Job j) {
+template <int UNROLL, int N>
+__global__ void __launch_bounds__(256) kv_move_vec(const __grid_constant__ JobT<N> p) {
+  const Job &j = p.j;
+  const Tables tb = tables_of(p);
   const uint32_t lane = threadIdx.x & 31;
   const uint64_t G = (uint64_t)gridDim.x * (blockDim.x >> 5);
   for (uint64_t item = (uint64_t)blockIdx.x * (blockDim.x >> 5) + (threadIdx.x >> 5);
        item < j.total_items; item += G) {
-    const Item it = decode(j, item);
+    const Item it = decode<N == 0>(j, tb, item);
     const uint4 *s = reinterpret_cast<const uint4 *>(it.src);
     uint4 *d = reinterpret_cast<uint4 *>(it.dst);
     const uint32_t nv = it.valid >> 4, nb = it.bytes >> 4;
@@ -289,12 +331,14 @@ __global__ void __launch_bounds__(256) kv_move_vec(const __grid_constant__ Job j
 // and length of the call (1, 2, 4 or 8 bytes).
 // ---------------------------------------------------------------------------------------------
 template <typename U>
-__global__ void __launch_bounds__(256) kv_move_elem(const __grid_constant__ Job j) {
+__global__ void __launch_bounds__(256) kv_move_elem(const __grid_constant__ JobT<0> p) {
+  const Job &j = p.j;
+  const Tables tb = tables_of(p);
   const uint32_t lane = threadIdx.x & 31;
   const uint64_t G = (uint64_t)gridDim.x * (blockDim.x >> 5);
   for (uint64_t item = (uint64_t)blockIdx.x * (blockDim.x >> 5) + (threadIdx.x >> 5);
        item < j.total_items; item += G) {
-    const Item it = decode(j, item);
+    const Item it = decode<true>(j, tb, item);
     const U *s = reinterpret_cast<const U *>(it.src);
     U *d = reinterpret_cast<U *>(it.dst);
     const uint32_t nv = it.valid / sizeof(U), nb = it.bytes / sizeof(U);

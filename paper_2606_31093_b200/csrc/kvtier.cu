@@ -23,6 +23,7 @@ using kvt::Piece;
 constexpr int kBlobSlots = 16;
 constexpr int kMaxStagingSlots = 4;
 constexpr uint32_t kMaxLayersKv = 4096;  // layer_count * kv_count
+constexpr uint64_t kAutoStagedMinBytes = 16ull << 20;
 
 enum KernelKind { KERNEL_AUTO = 0, KERNEL_BULK = 1, KERNEL_VEC = 2, KERNEL_ELEM = 3 };
 
@@ -55,8 +56,8 @@ struct kv_ctx {
   int last_cuda_error = 0;
   // options
   int kernel = KERNEL_AUTO;
-  uint32_t stage_bytes = 16384, stages = 3, warps = 4, lag = 1, max_ctas = 0, host_max_ctas = 0;
-  uint32_t staging_slots = 2, l2_hint = 0;
+  uint32_t stage_bytes = 16384, stages = 4, warps = 2, lag = 2, max_ctas = 0, host_max_ctas = 0;
+  uint32_t staging_slots = 2, l2_hint = 0, inline_tables = 1;
   size_t chunk_bytes = 0;
   // stats
   uint64_t launches = 0, memcpys = 0, last_items = 0, last_payload = 0, last_kernel = 0,
@@ -205,18 +206,35 @@ int check_dups(const int32_t *ids, uint64_t n, uint32_t num_pages) {
 // ---------------------------------------------------------------------------------------------
 // blob = [bases: LC x u64][pieces: n x Piece][ids: n_ids x i32], staged through a pinned ring
 // ---------------------------------------------------------------------------------------------
+struct HostBlob {
+  std::vector<uint8_t> bytes;
+  size_t off_pieces = 0, off_ids = 0;
+};
+
+void build_blob(const kv_pool_desc *p, const Geom &g, const std::vector<Piece> &pieces,
+                const int32_t *ids, uint64_t n_ids, bool ids_on_device, HostBlob *hb) {
+  hb->off_pieces = (size_t)g.LC * 8;
+  hb->off_ids = hb->off_pieces + pieces.size() * sizeof(Piece);
+  hb->bytes.resize(hb->off_ids + (ids_on_device ? 0 : (size_t)n_ids * 4));
+  uint8_t *h = hb->bytes.data();
+  for (uint32_t i = 0; i < g.LC; ++i) ((uint64_t *)h)[i] = (uint64_t)(uintptr_t)p->base[i];
+  std::memcpy(h + hb->off_pieces, pieces.data(), pieces.size() * sizeof(Piece));
+  if (!ids_on_device && n_ids) std::memcpy(h + hb->off_ids, ids, (size_t)n_ids * 4);
+}
+
+// Tables of a launch: either resident in device memory (slot of the pinned ring) or carried
+// inside the kernel parameters (inline; no copy, no slot).
 struct Blob {
   BlobSlot *slot = nullptr;
   const uint64_t *d_bases = nullptr;
   const Piece *d_pieces = nullptr;
-  const int32_t *d_ids = nullptr;
+  const int32_t *d_ids = nullptr;  // also set for caller-supplied device ids in inline mode
+  const HostBlob *inl = nullptr;   // non-null: inline tables
 };
 
-int upload_blob(kv_ctx *ctx, const kv_pool_desc *p, const Geom &g, const std::vector<Piece> &pieces,
-                const int32_t *ids, uint64_t n_ids, bool ids_on_device, cudaStream_t s, Blob *out) {
-  const size_t off_pieces = (size_t)g.LC * 8;
-  const size_t off_ids = off_pieces + pieces.size() * sizeof(Piece);
-  const size_t bytes = off_ids + (ids_on_device ? 0 : (size_t)n_ids * 4);
+int upload_blob(kv_ctx *ctx, const HostBlob &hb, const int32_t *ids, bool ids_on_device,
+                cudaStream_t s, Blob *out) {
+  const size_t bytes = hb.bytes.size();
   BlobSlot &slot = ctx->blobs[ctx->next_blob++ % kBlobSlots];
   if (slot.used) KV_CUDA(ctx, cudaEventSynchronize(slot.ev));  // last reader of this slot is done
   if (slot.cap < bytes) {
@@ -228,25 +246,41 @@ int upload_blob(kv_ctx *ctx, const kv_pool_desc *p, const Geom &g, const std::ve
     KV_CUDA(ctx, cudaMalloc(&slot.d, cap));
     slot.cap = cap;
   }
-  uint8_t *h = (uint8_t *)slot.h;
-  for (uint32_t i = 0; i < g.LC; ++i) ((uint64_t *)h)[i] = (uint64_t)(uintptr_t)p->base[i];
-  std::memcpy(h + off_pieces, pieces.data(), pieces.size() * sizeof(Piece));
-  if (!ids_on_device && n_ids) std::memcpy(h + off_ids, ids, (size_t)n_ids * 4);
+  std::memcpy(slot.h, hb.bytes.data(), bytes);
   KV_CUDA(ctx, cudaMemcpyAsync(slot.d, slot.h, bytes, cudaMemcpyHostToDevice, s));
   ctx->memcpys++;
   slot.used = true;
   out->slot = &slot;
   out->d_bases = (const uint64_t *)slot.d;
-  out->d_pieces = (const Piece *)((uint8_t *)slot.d + off_pieces);
-  out->d_ids = ids_on_device ? ids : (const int32_t *)((uint8_t *)slot.d + off_ids);
+  out->d_pieces = (const Piece *)((uint8_t *)slot.d + hb.off_pieces);
+  out->d_ids = ids_on_device ? ids : (const int32_t *)((uint8_t *)slot.d + hb.off_ids);
   return KV_OK;
+}
+
+constexpr int kInlineSmall = 3840;   // whole parameter block stays under the classic 4 KiB
+constexpr int kInlineLarge = 31744;  // CUDA 12.1+ large kernel parameters (<= 32,764 B)
+
+template <int N>
+void launch_bulk(const Job &j, const HostBlob *hb, uint32_t grid, uint32_t block, size_t smem, cudaStream_t s) {
+  static thread_local kvt::JobT<N> p;
+  p.j = j;
+  if constexpr (N > 0) std::memcpy(p.blob, hb->bytes.data(), hb->bytes.size());
+  kvt::kv_move_bulk<N><<<grid, block, smem, s>>>(p);
+}
+template <int N>
+void launch_vec(const Job &j, const HostBlob *hb, uint32_t grid, cudaStream_t s) {
+  static thread_local kvt::JobT<N> p;
+  p.j = j;
+  if constexpr (N > 0) std::memcpy(p.blob, hb->bytes.data(), hb->bytes.size());
+  kvt::kv_move_vec<8, N><<<grid, 256, 0, s>>>(p);
 }
 
 int launch(kv_ctx *ctx, const Geom &g, const Blob &b, uint32_t piece_first, uint32_t n_pieces,
            uint64_t total_items, uint32_t cta_cap, cudaStream_t s) {
   if (!total_items) return KV_OK;
   Job j{};
-  j.bases = b.d_bases; j.ids = b.d_ids; j.pieces = b.d_pieces + piece_first;
+  j.bases = b.d_bases; j.ids = b.d_ids; j.pieces = b.d_pieces ? b.d_pieces + piece_first : nullptr;
+  if (b.inl) { j.off_pieces = (uint32_t)b.inl->off_pieces; j.off_ids = (uint32_t)b.inl->off_ids; }
   j.status = ctx->d_status;
   j.total_items = total_items;
   j.page_stride = g.page_stride; j.buf_row_bytes = g.buf_row; j.buf_page_bytes = g.buf_page;
@@ -273,16 +307,24 @@ int launch(kv_ctx *ctx, const Geom &g, const Blob &b, uint32_t piece_first, uint
     }
     const uint64_t want = (total_items + warps - 1) / warps;
     grid = (uint32_t)std::min<uint64_t>(want, cap ? cap : (uint32_t)ctx->sm_count);
-    kvt::kv_move_bulk<<<grid, warps * 32, smem, s>>>(j);
+    if (!b.inl) launch_bulk<0>(j, nullptr, grid, warps * 32, smem, s);
+    else if (b.inl->bytes.size() <= kInlineSmall) launch_bulk<kInlineSmall>(j, b.inl, grid, warps * 32, smem, s);
+    else launch_bulk<kInlineLarge>(j, b.inl, grid, warps * 32, smem, s);
   } else {
     const uint32_t wpb = 8;  // warps per 256-thread CTA
     const uint64_t want = (total_items + wpb - 1) / wpb;
     grid = (uint32_t)std::min<uint64_t>(want, cap ? cap : (uint32_t)ctx->sm_count * 8);
-    if (g.kernel == KERNEL_VEC) kvt::kv_move_vec<8><<<grid, 256, 0, s>>>(j);
-    else if (g.unit >= 8) kvt::kv_move_elem<uint64_t><<<grid, 256, 0, s>>>(j);
-    else if (g.unit == 4) kvt::kv_move_elem<uint32_t><<<grid, 256, 0, s>>>(j);
-    else if (g.unit == 2) kvt::kv_move_elem<uint16_t><<<grid, 256, 0, s>>>(j);
-    else kvt::kv_move_elem<uint8_t><<<grid, 256, 0, s>>>(j);
+    kvt::JobT<0> p0;
+    p0.j = j;
+    if (g.kernel == KERNEL_VEC) {
+      if (!b.inl) launch_vec<0>(j, nullptr, grid, s);
+      else if (b.inl->bytes.size() <= kInlineSmall) launch_vec<kInlineSmall>(j, b.inl, grid, s);
+      else launch_vec<kInlineLarge>(j, b.inl, grid, s);
+    }
+    else if (g.unit >= 8) kvt::kv_move_elem<uint64_t><<<grid, 256, 0, s>>>(p0);
+    else if (g.unit == 4) kvt::kv_move_elem<uint32_t><<<grid, 256, 0, s>>>(p0);
+    else if (g.unit == 2) kvt::kv_move_elem<uint16_t><<<grid, 256, 0, s>>>(p0);
+    else kvt::kv_move_elem<uint8_t><<<grid, 256, 0, s>>>(p0);
   }
   KV_CUDA(ctx, cudaGetLastError());
   ctx->launches++;
@@ -407,8 +449,16 @@ int run_single_launch(kv_ctx *ctx, const kv_pool_desc *pools, const Call &c, con
     pieces.push_back(pc);
     acc += items_of(c.geom, q.n_ids);
   }
+  const bool dev_ids = flags & KV_FLAG_IDS_ON_DEVICE;
+  HostBlob hb;
+  build_blob(pools, c.geom, pieces, ids, c.n_ids, dev_ids, &hb);
   Blob b;
-  int rc = upload_blob(ctx, pools, c.geom, pieces, ids, c.n_ids, flags & KV_FLAG_IDS_ON_DEVICE, s, &b);
+  if (ctx->inline_tables && c.geom.kernel != KERNEL_ELEM && hb.bytes.size() <= (size_t)kInlineLarge) {
+    b.inl = &hb;  // tables travel inside the kernel parameters: one launch, no copy
+    b.d_ids = dev_ids ? ids : nullptr;
+    return launch(ctx, c.geom, b, 0, (uint32_t)pieces.size(), acc, cta_cap, s);
+  }
+  int rc = upload_blob(ctx, hb, ids, dev_ids, s, &b);
   if (rc) return rc;
   rc = launch(ctx, c.geom, b, 0, (uint32_t)pieces.size(), acc, cta_cap, s);
   if (rc) return rc;
@@ -418,7 +468,7 @@ int run_single_launch(kv_ctx *ctx, const kv_pool_desc *pools, const Call &c, con
 
 int ensure_staging(kv_ctx *ctx) {
   if (ctx->staging) return KV_OK;
-  if (!ctx->staging_bytes) ctx->staging_bytes = (size_t)256 << 20;
+  if (!ctx->staging_bytes) ctx->staging_bytes = (size_t)128 << 20;
   KV_CUDA(ctx, cudaMalloc(&ctx->staging, ctx->staging_bytes));
   return KV_OK;
 }
@@ -491,8 +541,10 @@ int run_staged(kv_ctx *ctx, const kv_pool_desc *pools, const Call &c, const int3
     const uint64_t base = (uint64_t)(uintptr_t)ctx->staging + (ci % n_slots) * slot_bytes;
     for (uint32_t k = 0; k < chunks[ci].n_pieces; ++k) pieces[chunks[ci].piece_first + k].buf += base;
   }
+  HostBlob hb;
+  build_blob(pools, g, pieces, ids, c.n_ids, flags & KV_FLAG_IDS_ON_DEVICE, &hb);
   Blob b;
-  rc = upload_blob(ctx, pools, g, pieces, ids, c.n_ids, flags & KV_FLAG_IDS_ON_DEVICE, s, &b);
+  rc = upload_blob(ctx, hb, ids, flags & KV_FLAG_IDS_ON_DEVICE, s, &b);
   if (rc) return rc;
   KV_CUDA(ctx, cudaEventRecord(ctx->ev_entry, s));
   KV_CUDA(ctx, cudaStreamWaitEvent(ctx->side, ctx->ev_entry, 0));
@@ -550,8 +602,10 @@ int host_alias(kv_ctx *ctx, const void *p, uint64_t *alias) {
 int resolve_mode(const kv_ctx *ctx, int mode, const Call &c, int *out) {
   if (mode != KV_HOST_AUTO && mode != KV_HOST_DIRECT && mode != KV_HOST_STAGED) return KV_ERR_LAYOUT;
   int m = mode;
-  // measured table: DIRECT stores/loads over the link win at every size
-  if (m == KV_HOST_AUTO) m = KV_HOST_DIRECT;
+  // Measured on B200 / PCIe Gen5 x16: the copy engines reach 98-99 % of the
+  // cudaMemcpy peak, SM-issued stores/loads over the link 92 % (128-byte TLP payloads); below
+  // ~16 MiB both are latency-bound and equal, and DIRECT is one launch with no staging traffic.
+  if (m == KV_HOST_AUTO) m = c.payload >= kAutoStagedMinBytes ? KV_HOST_STAGED : KV_HOST_DIRECT;
   // staged needs chunks that are contiguous in the host buffer
   if (m == KV_HOST_STAGED && c.geom.layout != KV_LAYOUT_PAGE_FIRST) m = KV_HOST_DIRECT;
   (void)ctx;
@@ -566,8 +620,8 @@ int run_host(kv_ctx *ctx, const kv_pool_desc *pools, Call &c, const int32_t *ids
   if (rc) return rc;
   note_plan(ctx, c);
   ctx->last_mode = (uint64_t)m;
+  if (c.reqs.empty()) return KV_OK;  // n == 0: nothing to do, no launch
   if (ctx->host_only) return KV_ERR_NO_DEVICE;
-  if (c.reqs.empty()) return KV_OK;
   DeviceGuard guard(ctx);
   for (Req &q : c.reqs) {
     uint64_t alias = 0;
@@ -582,8 +636,8 @@ int run_host(kv_ctx *ctx, const kv_pool_desc *pools, Call &c, const int32_t *ids
 int run_device(kv_ctx *ctx, const kv_pool_desc *pools, const Call &c, const int32_t *ids,
                uint32_t flags, cudaStream_t s) {
   note_plan(ctx, c);
+  if (c.reqs.empty()) return KV_OK;  // n == 0: nothing to do, no launch
   if (ctx->host_only) return KV_ERR_NO_DEVICE;
-  if (c.reqs.empty()) return KV_OK;
   DeviceGuard guard(ctx);
   return run_single_launch(ctx, pools, c, ids, flags, 0, s);
 }
@@ -628,10 +682,9 @@ int kv_ctx_create(kv_ctx **out, int device, size_t staging_bytes) {
   }
   ctx->device = device;
   auto fail = [&](cudaError_t e) {
-    int code = (int)e;
+    (void)e;
     (void)cudaGetLastError();
     delete ctx;
-    (void)code;
     return KV_ERR_CUDA;
   };
   cudaError_t e;
@@ -640,7 +693,9 @@ int kv_ctx_create(kv_ctx **out, int device, size_t staging_bytes) {
   if ((e = cudaSetDevice(device)) != cudaSuccess) return fail(e);
   if ((e = cudaDeviceGetAttribute(&ctx->sm_count, cudaDevAttrMultiProcessorCount, device)) != cudaSuccess) return fail(e);
   if ((e = cudaDeviceGetAttribute(&ctx->max_smem, cudaDevAttrMaxSharedMemoryPerBlockOptin, device)) != cudaSuccess) return fail(e);
-  if ((e = cudaFuncSetAttribute(kvt::kv_move_bulk, cudaFuncAttributeMaxDynamicSharedMemorySize, ctx->max_smem - 4096)) != cudaSuccess) return fail(e);
+  if ((e = cudaFuncSetAttribute(kvt::kv_move_bulk<0>, cudaFuncAttributeMaxDynamicSharedMemorySize, ctx->max_smem - 4096)) != cudaSuccess) return fail(e);
+  if ((e = cudaFuncSetAttribute(kvt::kv_move_bulk<kInlineSmall>, cudaFuncAttributeMaxDynamicSharedMemorySize, ctx->max_smem - 4096)) != cudaSuccess) return fail(e);
+  if ((e = cudaFuncSetAttribute(kvt::kv_move_bulk<kInlineLarge>, cudaFuncAttributeMaxDynamicSharedMemorySize, ctx->max_smem - 4096)) != cudaSuccess) return fail(e);
   if ((e = cudaStreamCreateWithFlags(&ctx->side, cudaStreamNonBlocking)) != cudaSuccess) return fail(e);
   if ((e = cudaEventCreateWithFlags(&ctx->ev_entry, cudaEventDisableTiming)) != cudaSuccess) return fail(e);
   for (int i = 0; i < kBlobSlots; ++i)
@@ -694,6 +749,7 @@ int kv_ctx_set_option(kv_ctx *ctx, int option, int64_t v) {
     case KV_OPT_HOST_MAX_CTAS: if (v < 0 || v > 65535) return KV_ERR_SIZE; ctx->host_max_ctas = (uint32_t)v; break;
     case KV_OPT_STAGING_SLOTS: if (v < 2 || v > kMaxStagingSlots) return KV_ERR_SIZE; ctx->staging_slots = (uint32_t)v; break;
     case KV_OPT_L2_HINT: if (v < 0 || v > 1) return KV_ERR_SIZE; ctx->l2_hint = (uint32_t)v; break;
+    case KV_OPT_INLINE_TABLES: if (v < 0 || v > 1) return KV_ERR_SIZE; ctx->inline_tables = (uint32_t)v; break;
     default: return KV_ERR_LAYOUT;
   }
   return KV_OK;

@@ -1,0 +1,178 @@
+"""CPU-only checks of the C ABI: the library loads, exports every symbol include/kvtier.h
+declares, and its host logic (validation order, planning) is right -- through a planning-only
+context (device = -1) that touches no CUDA API.  No compute call is made here."""
+import ctypes
+import os
+import re
+
+import numpy as np
+import pytest
+
+ROOT = os.path.dirname(os.path.dirname(os.path.abspath(__file__)))
+
+from paper_2606_31093_b200 import kvtier as kv  # noqa: E402
+from paper_2606_31093_b200 import workloads as W  # noqa: E402
+
+
+def declared_symbols():
+    src = open(os.path.join(ROOT, "include", "kvtier.h")).read()
+    src = re.sub(r"/\*.*?\*/", "", src, flags=re.S)
+    names = re.findall(r"\b(kv_[a-z_0-9]+)\s*\(", src)
+    return sorted(set(names))
+
+
+def test_library_exports_every_declared_symbol():
+    lib = ctypes.CDLL(kv.LIB_PATH)
+    names = declared_symbols()
+    assert len(names) >= 20 and "kv_pack" in names and "kv_reload_batched" in names
+    for n in names:
+        assert hasattr(lib, n), f"{n} declared in include/kvtier.h but not exported"
+
+
+def test_binding_has_the_same_names():
+    skip = {"kv_ctx_set_option", "kv_ctx_get_stat", "kv_last_cuda_error", "kv_device_status"}  # Ctx methods
+    for n in declared_symbols():
+        if n not in skip:
+            assert hasattr(kv, n), f"binding lacks {n}"
+
+
+def test_version_and_strerror():
+    assert kv.kv_version() == 0x00010000
+    seen = set()
+    for code in range(0, -11, -1):
+        msg = kv.kv_strerror(code)
+        assert msg and msg not in seen
+        seen.add(msg)
+    assert "unknown" in kv.kv_strerror(-99)
+
+
+def fake_pool(shape, stride=None, base0=0x7000_0000_0000, align=0):
+    slab = shape.P * (stride or shape.row_bytes)
+    bases = [base0 + align + i * ((slab + 4095) // 4096 * 4096) for i in range(shape.L * shape.C)]
+    return kv.PoolDesc(bases, shape.L, shape.C, shape.P, shape.T, shape.H, shape.D, shape.e, stride)
+
+
+BUF = 0x7100_0000_0000
+
+
+def status_of(fn):
+    with pytest.raises(kv.KvError) as ei:
+        fn()
+    return ei.value.status
+
+
+@pytest.fixture()
+def ctx():
+    c = kv.Ctx(-1)
+    yield c
+    c.close()
+
+
+def test_planning_ctx_never_launches(ctx):
+    s = W.QWEN3_OMNI
+    d = fake_pool(s)
+    case = W.prefix_case(0)
+    n = len(case.src_ids)
+    assert n == 512
+    assert status_of(lambda: kv.kv_pack(ctx, d, s.L, case.src_ids, BUF, dst_bytes=n * s.page_bytes)) == kv.KV_ERR_NO_DEVICE
+    # 512 pages x 48 layers x 2 = 49,152 segments of one 16 KiB row
+    assert ctx.stat(kv.KV_STAT_LAST_ITEMS) == 49152
+    assert ctx.stat(kv.KV_STAT_LAST_PAYLOAD) == 768 << 20
+    assert ctx.stat(kv.KV_STAT_LAST_SEGMENT) == 16384
+    assert ctx.stat(kv.KV_STAT_LAST_KERNEL) == kv.KV_KERNEL_BULK
+    assert ctx.stat(kv.KV_STAT_LAUNCHES) == 0 and ctx.stat(kv.KV_STAT_MEMCPYS) == 0
+
+
+def test_plan_repage_16_to_64(ctx):
+    """BASELINE.json:configs[4]: 2,048 tokens -> 32 pages of 64; segment = min(Ts,Td) tokens."""
+    c5 = W.crossrole_case(0)
+    d = fake_pool(c5.dst_shape)
+    s = c5.dst_shape
+    srcs = [BUF + r * (1 << 32) for r in range(32)]
+    assert status_of(lambda: kv.kv_unpack_batched(ctx, srcs, c5.dst_ids, c5.dst_offsets, c5.n_tokens, d, s.L, 16, 64)) == kv.KV_ERR_NO_DEVICE
+    assert ctx.stat(kv.KV_STAT_LAST_ITEMS) == 32 * 32 * 4 * 96
+    assert ctx.stat(kv.KV_STAT_LAST_SEGMENT) == 16384
+    assert ctx.stat(kv.KV_STAT_LAST_PAYLOAD) == 32 * 32 * s.page_bytes == 6 << 30
+    # neither page size divides the other: segment = gcd(16, 24) = 8 tokens = 8 KiB
+    d24 = fake_pool(s.with_(T=24))
+    assert status_of(lambda: kv.kv_unpack(ctx, BUF, np.arange(2), d24, s.L, 16, 24, 48, src_bytes=1 << 40)) == kv.KV_ERR_NO_DEVICE
+    assert ctx.stat(kv.KV_STAT_LAST_SEGMENT) == 8 * 1024
+    assert ctx.stat(kv.KV_STAT_LAST_ITEMS) == 2 * 3 * 96
+
+
+def test_plan_splits_rows_longer_than_a_stage(ctx):
+    s = W.QWEN3_OMNI.with_(T=64)
+    d = fake_pool(s)
+    assert status_of(lambda: kv.kv_pack(ctx, d, s.L, [1, 2, 3], BUF, dst_bytes=1 << 40)) == kv.KV_ERR_NO_DEVICE
+    assert ctx.stat(kv.KV_STAT_LAST_SEGMENT) == 16384  # 64 KiB row cut into 4 stage-sized pieces
+    assert ctx.stat(kv.KV_STAT_LAST_ITEMS) == 3 * 96 * 4
+    ctx.set_option(kv.KV_OPT_STAGE_BYTES, 32768)
+    assert status_of(lambda: kv.kv_pack(ctx, d, s.L, [1, 2, 3], BUF, dst_bytes=1 << 40)) == kv.KV_ERR_NO_DEVICE
+    assert ctx.stat(kv.KV_STAT_LAST_ITEMS) == 3 * 96 * 2
+
+
+def test_misalignment_selects_elem_kernel_never_rejects(ctx):
+    s = W.TINY
+    for d, buf in [(fake_pool(s, align=2), BUF), (fake_pool(s), BUF + 6), (fake_pool(s, stride=s.row_bytes + 2), BUF)]:
+        assert status_of(lambda: kv.kv_pack(ctx, d, s.L, [0], buf, dst_bytes=1 << 30)) == kv.KV_ERR_NO_DEVICE
+        assert ctx.stat(kv.KV_STAT_LAST_KERNEL) == kv.KV_KERNEL_ELEM
+    # but elem_bytes alignment is required (SURVEY.md 8(b) KV_ERR_ALIGN)
+    assert status_of(lambda: kv.kv_pack(ctx, fake_pool(s), s.L, [0], BUF + 1, dst_bytes=1 << 30)) == kv.KV_ERR_ALIGN
+    assert status_of(lambda: kv.kv_pack(ctx, fake_pool(s, align=1), s.L, [0], BUF, dst_bytes=1 << 30)) == kv.KV_ERR_ALIGN
+
+
+def test_validation_errors(ctx):
+    s = W.TINY
+    d = fake_pool(s)
+    pg = s.page_bytes
+    E = kv
+    assert status_of(lambda: kv.kv_pack(ctx, d, s.L, [0, 256], BUF, dst_bytes=2 * pg)) == E.KV_ERR_PAGE_RANGE
+    assert status_of(lambda: kv.kv_pack(ctx, d, s.L, [0, -1], BUF, dst_bytes=2 * pg)) == E.KV_ERR_PAGE_RANGE
+    assert status_of(lambda: kv.kv_pack(ctx, d, s.L, [0, 1], BUF, dst_bytes=2 * pg - 1)) == E.KV_ERR_SIZE
+    assert status_of(lambda: kv.kv_pack(ctx, d, s.L, [0, 1], None, dst_bytes=2 * pg)) == E.KV_ERR_NULL
+    assert status_of(lambda: kv.kv_pack(ctx, d, 0, [0], BUF, dst_bytes=pg)) == E.KV_ERR_DESC
+    assert status_of(lambda: kv.kv_pack(ctx, d, s.L + 1, [0], BUF, dst_bytes=pg)) == E.KV_ERR_DESC
+    assert status_of(lambda: kv.kv_pack(ctx, d, s.L, [0], BUF, dst_bytes=pg, layout=2)) == E.KV_ERR_LAYOUT
+    # unpack: page count must be ceil(n_tokens / Td); Td must be the pool's page size
+    assert status_of(lambda: kv.kv_unpack(ctx, BUF, [0, 1], d, s.L, 16, 16, 33, src_bytes=1 << 30)) == E.KV_ERR_SIZE
+    assert status_of(lambda: kv.kv_unpack(ctx, BUF, [0, 1], d, s.L, 16, 32, 64, src_bytes=1 << 30)) == E.KV_ERR_SIZE
+    assert status_of(lambda: kv.kv_unpack(ctx, BUF, [0, 1], d, s.L, 16, 16, 32, src_bytes=2 * pg - 1)) == E.KV_ERR_SIZE
+    assert status_of(lambda: kv.kv_unpack(ctx, BUF, [3, 3], d, s.L, 16, 16, 32, src_bytes=2 * pg, flags=kv.KV_FLAG_VALIDATE)) == E.KV_ERR_DUP_PAGE
+    assert status_of(lambda: kv.kv_unpack(ctx, BUF, [3, 3], d, s.L, 16, 16, 32, src_bytes=2 * pg)) == E.KV_ERR_NO_DEVICE  # unchecked without the flag
+    assert status_of(lambda: kv.kv_offload(ctx, d, s.L, [0], BUF, pg, mode=3)) == E.KV_ERR_LAYOUT
+    # malformed descriptors
+    bad = fake_pool(s)
+    bad.desc.elem_bytes = 3
+    assert status_of(lambda: kv.kv_pack(ctx, bad, s.L, [0], BUF, dst_bytes=1 << 30)) == E.KV_ERR_DESC
+    bad = fake_pool(s)
+    bad.desc.page_stride_bytes = s.row_bytes - 2
+    assert status_of(lambda: kv.kv_pack(ctx, bad, s.L, [0], BUF, dst_bytes=1 << 30)) == E.KV_ERR_DESC
+    # batched: offsets must be non-decreasing
+    assert status_of(lambda: kv.kv_pack_batched(ctx, d, s.L, [0, 1, 2], [0, 2, 1], [BUF, BUF + (1 << 30)])) == E.KV_ERR_SIZE
+    # options
+    with pytest.raises(kv.KvError):
+        ctx.set_option(kv.KV_OPT_STAGE_BYTES, 1000)
+    with pytest.raises(kv.KvError):
+        ctx.set_option(99, 0)
+
+
+def test_empty_calls_are_ok_even_without_a_device(ctx):
+    """n == 0 / n_req == 0 -> KV_OK, no launch."""
+    s = W.TINY
+    d = fake_pool(s)
+    kv.kv_pack(ctx, d, s.L, [], BUF, dst_bytes=0)
+    kv.kv_unpack(ctx, BUF, [], d, s.L, 16, 16, 0, src_bytes=0)
+    kv.kv_pack_batched(ctx, d, s.L, [], [0], [])
+    kv.kv_pack_batched(ctx, d, s.L, [], [0, 0, 0], [BUF, BUF])
+    assert ctx.stat(kv.KV_STAT_LAST_ITEMS) == 0
+
+
+def test_auto_host_mode_policy(ctx):
+    s = W.QWEN3_OMNI
+    d = fake_pool(s)
+    for n, want in [(4, kv.KV_HOST_DIRECT), (10, kv.KV_HOST_DIRECT), (11, kv.KV_HOST_STAGED), (512, kv.KV_HOST_STAGED)]:
+        assert status_of(lambda: kv.kv_offload(ctx, d, s.L, np.arange(n), BUF, n * s.page_bytes)) == kv.KV_ERR_NO_DEVICE
+        assert ctx.stat(kv.KV_STAT_LAST_HOST_MODE) == want, n
+    # layer-first buffers are not chunk-contiguous: staged falls back to direct
+    assert status_of(lambda: kv.kv_offload(ctx, d, s.L, np.arange(512), BUF, 512 * s.page_bytes, mode=kv.KV_HOST_STAGED, layout=1)) == kv.KV_ERR_NO_DEVICE
+    assert ctx.stat(kv.KV_STAT_LAST_HOST_MODE) == kv.KV_HOST_DIRECT
