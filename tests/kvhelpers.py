@@ -37,3 +37,39 @@ def assert_pool_equal(tens, pool):
             bad = np.flatnonzero(got != s)
             raise AssertionError(f"slab {i}: {bad.size} bytes differ, first at {bad[0]} "
                                  f"(page {bad[0] // pool.page_stride_bytes})")
+
+
+# ---------------------------------------------------------------------------------------------
+# full-scale helpers: pools that live only on the device (96 GiB >> what we want in host RAM)
+# ---------------------------------------------------------------------------------------------
+def device_pool(torch, kvtier, shape, seed, fill="randn"):
+    """2*L slabs of [P][T][H][D] bf16 filled on the device with a seeded torch generator
+    (BASELINE.json:configs[1]: normal(0,1) values).  Returns (slabs as uint8 views, PoolDesc)."""
+    gen = torch.Generator(device="cuda").manual_seed(seed)
+    slabs = []
+    for _ in range(shape.L * shape.C):
+        t = torch.empty(shape.P * shape.T * shape.H * shape.D, dtype=torch.bfloat16, device="cuda")
+        if fill == "randn":
+            t.normal_(generator=gen)
+        else:
+            t.view(torch.int16).random_(-32768, 32767, generator=gen)
+        slabs.append(t.view(torch.uint8))
+    desc = kvtier.PoolDesc(slabs, shape.L, shape.C, shape.P, shape.T, shape.H, shape.D, shape.e)
+    return slabs, desc
+
+
+def snapshot_pages(torch, slabs, ids, shape, layer_count=None):
+    """Copy ONLY the pages `ids` of every slab to the host with torch indexing (shares nothing
+    with the library) as a compact HostPool whose page k is device page ids[k]."""
+    L = shape.L if layer_count is None else layer_count
+    row = shape.row_bytes
+    idx = torch.as_tensor(np.asarray(ids, dtype=np.int64), device="cuda")
+    out = []
+    for s in slabs[:L * shape.C]:
+        out.append(s.view(shape.P, row).index_select(0, idx).cpu().numpy().reshape(-1))
+    return ko.HostPool(out, L, shape.C, len(ids), shape.T, shape.H, shape.D, shape.e, row)
+
+
+def page_checksums(torch, slabs, shape):
+    """Per-page wrap-around 64-bit sums of every slab: [LC][P] int64 on the device."""
+    return torch.stack([s.view(torch.int64).view(shape.P, -1).sum(dim=1) for s in slabs])
