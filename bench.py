@@ -333,7 +333,7 @@ def run_ours(args):
     if args.report and rank == 0:
         from paper_2606_31093_b200 import report
 
-        line["report"] = report.run(ctx, desc, shape, slabs, args.seed)
+        line["report"] = report.run(ctx, desc, shape, [t.view(torch.uint8) for t in slabs], args.seed, hbm_peak=peak)
     if rank == 0:
         print(json.dumps(line))
     ctx.close()

@@ -109,6 +109,8 @@ typedef enum kv_option {
   KV_OPT_L2_HINT = 9,        /* bulk: 0 none, 1 evict_first cache hint on loads and stores */
   KV_OPT_INLINE_TABLES = 10, /* 1 (default): page ids / slab bases ride in the kernel parameters when they fit (<= 31 KiB);
                                 0: always stage them through the ctx's pinned ring with one H2D copy */
+  KV_OPT_DYNAMIC = 11,       /* bulk: 1 (default) large launches claim segments from a device counter (guided chunks);
+                                0: static round-robin only */
 } kv_option;
 
 /* kv_ctx_get_stat keys */

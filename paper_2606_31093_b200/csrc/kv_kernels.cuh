@@ -59,6 +59,11 @@ struct Job {
   uint32_t l2_hint;
   // inline tables (JobT<N>, N > 0): byte offsets into the kernel-parameter blob
   uint32_t off_pieces, off_ids;
+  // dynamic work distribution of kv_move_bulk (nullptr = static round-robin)
+  unsigned long long *sched;  // global claim counter (items beyond the static first blocks)
+  uint32_t *sched_done;       // warps finished; the last one resets both counters to 0
+  uint32_t first_batch;       // B0: static items per warp before claiming starts
+  uint32_t pad_;
 };
 
 // The lookup tables of a launch: slab bases, page ids, pieces.  They live either in device memory
@@ -229,31 +234,84 @@ __global__ void __launch_bounds__(kMaxWarps * 32, 1) kv_move_bulk(const __grid_c
 
   const uint64_t G = (uint64_t)gridDim.x * warps;
   const uint64_t gw = (uint64_t)blockIdx.x * warps + warp;
-  const uint64_t n_my = gw < j.total_items ? (j.total_items - gw + G - 1) / G : 0;
-  if (n_my == 0) return;
+  // Work distribution.
+  //   static  (j.sched == nullptr): this warp's my-th item is gw + my*G.
+  //   dynamic (large launches): the first B0 items of every warp are the static block
+  //           [gw*B0, gw*B0+B0); the rest is claimed from a global counter in guided chunks
+  //           (remaining / 2G, clamped to 1..32), each claim issued one batch ahead so its
+  //           latency hides behind the batch in flight.  SMs that run fast take more segments,
+  //           so the launch ends when the work does, not when the slowest SM does.
+  const bool dyn = j.sched != nullptr;
+  const uint32_t B0 = j.first_batch;
+  const uint64_t dyn_base = G * B0;
+  const uint64_t dyn_total = dyn ? j.total_items - dyn_base : 0;
+  const uint64_t n_my = dyn ? 0 : (gw < j.total_items ? (j.total_items - gw + G - 1) / G : 0);
+  if (!dyn && n_my == 0) return;
 
   uint64_t pol = 0;
   if (j.l2_hint) asm volatile("createpolicy.fractional.L2::evict_first.b64 %0, 1.0;" : "=l"(pol));
 
   const uint32_t stage0 = smem_u32(smem) + j.zero_bytes + warp * K * j.stage_bytes;
   const uint32_t zero0 = smem_u32(smem);
-  const uint64_t n_iter = n_my + (K - lag);
+  const uint32_t depth = K - lag;
   Item mine;
   mine.src = mine.dst = 0; mine.bytes = mine.valid = 0;
 
-  for (uint64_t it = 0; it < n_iter; ++it) {
-    if ((it & 31) == 0 && it < n_my) {  // warp-level lookup: 32 segments decoded at once
-      const uint64_t my = it + lane;
-      if (my < n_my) mine = decode<N == 0>(j, tb, gw + my * G);
+  unsigned long long pre_start = 0;  // lane 0: result of the claim issued one batch ahead
+  uint32_t pre_count = 0;            // warp-uniform: size of that claim (0 = none outstanding)
+  auto guided = [&](uint64_t claimed) -> uint32_t {
+    const uint64_t rem = dyn_total > claimed ? dyn_total - claimed : 0;
+    return (uint32_t)min((uint64_t)32, max((uint64_t)1, rem / (2 * G)));
+  };
+  if (dyn) {
+    pre_count = guided(0);
+    if (lane == 0) pre_start = atomicAdd(j.sched, (unsigned long long)pre_count);
+  }
+
+  uint64_t n_known = 0;      // items of this warp claimed so far
+  uint64_t batch_first = 0;  // my-index of the first item of the batch held in `mine`
+  bool exhausted = false;
+  for (uint64_t it = 0;; ++it) {
+    if (it == n_known && !exhausted) {  // ---- next batch: warp-level lookup, <= 32 segments at once
+      uint64_t first_item = 0, stride = 1;
+      uint32_t cnt = 0;
+      if (!dyn) {
+        cnt = (uint32_t)min((uint64_t)32, n_my - n_known);
+        first_item = gw + n_known * G;
+        stride = G;
+      } else if (n_known == 0) {
+        cnt = B0;
+        first_item = gw * B0;
+      } else if (pre_count) {
+        const uint64_t st = __shfl_sync(0xffffffffu, pre_start, 0);
+        if (st < dyn_total) {
+          cnt = (uint32_t)min((uint64_t)pre_count, dyn_total - st);
+          first_item = dyn_base + st;
+          const uint64_t claimed = st + pre_count;
+          pre_count = claimed < dyn_total ? guided(claimed) : 0;
+          if (pre_count && lane == 0) pre_start = atomicAdd(j.sched, (unsigned long long)pre_count);
+        } else {
+          pre_count = 0;
+        }
+      }
+      if (cnt == 0) {
+        exhausted = true;
+      } else {
+        if (lane < cnt) mine = decode<N == 0>(j, tb, first_item + lane * stride);
+        batch_first = n_known;
+        n_known += cnt;
+      }
     }
-    const uint32_t sel = (uint32_t)it & 31;
+    const bool have = it < n_known;
+    if (!have && it >= n_known + depth) break;
+    const uint32_t sel = (uint32_t)(it - batch_first) & 31;
     const uint64_t src = __shfl_sync(0xffffffffu, mine.src, sel);
     const uint64_t dst = __shfl_sync(0xffffffffu, mine.dst, sel);
     const uint32_t bytes = __shfl_sync(0xffffffffu, mine.bytes, sel);
     const uint32_t valid = __shfl_sync(0xffffffffu, mine.valid, sel);
     if (lane == 0) {
-      if (it >= K - lag) {  // ---- store side: item si
-        const uint64_t si = it - (K - lag);
+      if (it >= depth && it - depth < n_known) {  // ---- store side: item si
+        const uint64_t si = it - depth;
         const uint32_t s = (uint32_t)(si % K);
         mbar_wait(smem_u32(&full_bar[warp][s]), (uint32_t)(si / K) & 1);
         const StageMeta m = meta[warp][s];
@@ -265,7 +323,7 @@ __global__ void __launch_bounds__(kMaxWarps * 32, 1) kv_move_bulk(const __grid_c
           bulk_s2g(m.dst + z, zero0, min(j.zero_bytes, m.bytes - z));
         bulk_commit();
       }
-      if (it < n_my) {  // ---- load side: item it
+      if (have) {  // ---- load side: item it
         const uint32_t s = (uint32_t)(it % K);
         if (it >= K) {  // the store that last read this stage was committed `lag` groups ago
           if (lag == 1) bulk_wait_read<1>();
@@ -282,6 +340,14 @@ __global__ void __launch_bounds__(kMaxWarps * 32, 1) kv_move_bulk(const __grid_c
           mbar_arrive(bar);
         }
       }
+    }
+  }
+  if (dyn && lane == 0) {  // last warp out re-arms the counters for the next launch
+    __threadfence();
+    if (atomicAdd(j.sched_done, 1u) == (uint32_t)G - 1) {
+      *j.sched = 0ull;
+      *j.sched_done = 0u;
+      __threadfence();
     }
   }
   if (lane == 0) bulk_wait_all();

@@ -24,6 +24,7 @@ constexpr int kBlobSlots = 16;
 constexpr int kMaxStagingSlots = 4;
 constexpr uint32_t kMaxLayersKv = 4096;  // layer_count * kv_count
 constexpr uint64_t kAutoStagedMinBytes = 16ull << 20;
+constexpr uint32_t kSchedSlots = 256;  // claim counters, handed out round-robin per launch
 
 enum KernelKind { KERNEL_AUTO = 0, KERNEL_BULK = 1, KERNEL_VEC = 2, KERNEL_ELEM = 3 };
 
@@ -57,7 +58,8 @@ struct kv_ctx {
   // options
   int kernel = KERNEL_AUTO;
   uint32_t stage_bytes = 16384, stages = 4, warps = 2, lag = 2, max_ctas = 0, host_max_ctas = 0;
-  uint32_t staging_slots = 2, l2_hint = 0, inline_tables = 1;
+  uint32_t staging_slots = 2, l2_hint = 0, inline_tables = 1, dynamic = 1;
+  uint32_t next_sched = 0;
   size_t chunk_bytes = 0;
   // stats
   uint64_t launches = 0, memcpys = 0, last_items = 0, last_payload = 0, last_kernel = 0,
@@ -307,6 +309,13 @@ int launch(kv_ctx *ctx, const Geom &g, const Blob &b, uint32_t piece_first, uint
     }
     const uint64_t want = (total_items + warps - 1) / warps;
     grid = (uint32_t)std::min<uint64_t>(want, cap ? cap : (uint32_t)ctx->sm_count);
+    const uint64_t G = (uint64_t)grid * warps;
+    if (ctx->dynamic && total_items >= 8 * G) {  // enough work for claiming to pay
+      uint8_t *slot = (uint8_t *)ctx->d_status + 256 + (size_t)(ctx->next_sched++ % kSchedSlots) * 16;
+      j.sched = (unsigned long long *)slot;
+      j.sched_done = (uint32_t *)(slot + 8);
+      j.first_batch = (uint32_t)std::min<uint64_t>(32, total_items / (4 * G));
+    }
     if (!b.inl) launch_bulk<0>(j, nullptr, grid, warps * 32, smem, s);
     else if (b.inl->bytes.size() <= kInlineSmall) launch_bulk<kInlineSmall>(j, b.inl, grid, warps * 32, smem, s);
     else launch_bulk<kInlineLarge>(j, b.inl, grid, warps * 32, smem, s);
@@ -704,8 +713,8 @@ int kv_ctx_create(kv_ctx **out, int device, size_t staging_bytes) {
     if ((e = cudaEventCreateWithFlags(&ctx->ev_full[i], cudaEventDisableTiming)) != cudaSuccess) return fail(e);
     if ((e = cudaEventCreateWithFlags(&ctx->ev_free[i], cudaEventDisableTiming)) != cudaSuccess) return fail(e);
   }
-  if ((e = cudaMalloc((void **)&ctx->d_status, 256)) != cudaSuccess) return fail(e);
-  if ((e = cudaMemset(ctx->d_status, 0, 256)) != cudaSuccess) return fail(e);
+  if ((e = cudaMalloc((void **)&ctx->d_status, 256 + kSchedSlots * 16)) != cudaSuccess) return fail(e);
+  if ((e = cudaMemset(ctx->d_status, 0, 256 + kSchedSlots * 16)) != cudaSuccess) return fail(e);
   if (prev >= 0 && prev != device) cudaSetDevice(prev);
   *out = ctx;
   return KV_OK;
@@ -750,6 +759,7 @@ int kv_ctx_set_option(kv_ctx *ctx, int option, int64_t v) {
     case KV_OPT_STAGING_SLOTS: if (v < 2 || v > kMaxStagingSlots) return KV_ERR_SIZE; ctx->staging_slots = (uint32_t)v; break;
     case KV_OPT_L2_HINT: if (v < 0 || v > 1) return KV_ERR_SIZE; ctx->l2_hint = (uint32_t)v; break;
     case KV_OPT_INLINE_TABLES: if (v < 0 || v > 1) return KV_ERR_SIZE; ctx->inline_tables = (uint32_t)v; break;
+    case KV_OPT_DYNAMIC: if (v < 0 || v > 1) return KV_ERR_SIZE; ctx->dynamic = (uint32_t)v; break;
     default: return KV_ERR_LAYOUT;
   }
   return KV_OK;
