@@ -39,9 +39,10 @@ sys.path.insert(0, ROOT)
 
 METRIC = "kv_pack_unpack_GBps"
 UNIT = "GB/s"
-# dram__bytes_read.sum + dram__bytes_write.sum of one kv_move_bulk pack launch at this workload,
-# from the `ncu --set full` capture summarised in profiles/ (None until captured).
-NCU_TRAFFIC_BYTES_PER_LAUNCH = None
+# dram__bytes_read.sum + dram__bytes_write.sum of one kv_move_bulk launch at this workload (mean of 4
+# launches), from the `ncu --set full` capture summarised in profiles/r01_kv_move_bulk_full.md:
+# 805.4 MB read + 759.3 MB written (the last ~46 MB of the destination is still dirty in L2 at exit).
+NCU_TRAFFIC_BYTES_PER_LAUNCH = 1564.6e6
 
 
 def parse():
@@ -307,7 +308,7 @@ def run_ours(args):
             "reload_link_GBps": payload / (rel_ms * 1e-3) / 1e9, "reload_ms": rel_ms,
             "host_mode": host_mode,
         },
-        "e2e": {"value": e2e_value, "unit": UNIT, "h2d_bytes_per_step": payload + 2 * (4 * n + 8 * shape.L * shape.C + 40),
+        "e2e": {"value": e2e_value, "unit": UNIT, "h2d_bytes_per_step": payload + 2 * (4 * n + 8 * shape.L * shape.C + 40 * 12),
                 "d2h_bytes_per_step": payload, "steps": Ke,
                 "what": "kv_offload (pool->pinned host) + kv_reload (pinned host->pool) + stream sync per step, through the C ABI",
                 "link_GBps_payload": world * 2 * payload * Ke / (e2e_ms * 1e-3) / 1e9},
@@ -316,7 +317,7 @@ def run_ours(args):
                      "peak": peak, "unit": "GB/s", "frac": achieved / peak,
                      "traffic": NCU_TRAFFIC_BYTES_PER_LAUNCH, "algorithmic_bytes": 2 * payload,
                      "peak_source": peak_src,
-                     "timing": "CUDA events on the launch stream around each kv_pack call (includes its 2.5 KB page-id H2D copy)"},
+                     "timing": "mean over the K timed steps of CUDA events on the launch stream around each kv_pack call (one launch; page ids ride in the kernel parameters)"},
         "clocks": clocks.summary(),
     }
 
