@@ -203,3 +203,97 @@ int kvo_cow_append(void *const *base, uint32_t L, uint32_t C, uint32_t num_pages
           }
   return KVO_OK;
 }
+
+/* Batched copy-on-write append (SURVEY.md 8(f) NEXT-1 "batched over sessions"):
+ * kvo_cow_append once per session s, in order, with its own (old_ids[s], new_ids[s], n_old[s],
+ * n_app[s], apps[s]).  All arguments are checked for every session before anything is written.
+ * new_ids must be distinct and must not appear among old_ids (caller checks, like unpack). */
+int kvo_cow_append_batched(void *const *base, uint32_t L, uint32_t C, uint32_t num_pages,
+                           uint32_t T, uint32_t H, uint32_t D, uint32_t e,
+                           uint64_t page_stride_bytes, const int32_t *old_ids,
+                           const int32_t *new_ids, const uint32_t *n_old, const uint32_t *n_app,
+                           const void *const *apps, uint32_t S) {
+  if (S && (!old_ids || !new_ids || !n_old || !n_app || !apps)) return KVO_ERR_ARG;
+  for (uint32_t s = 0; s < S; ++s) {
+    if ((uint64_t)n_old[s] + n_app[s] > T || old_ids[s] == new_ids[s]) return KVO_ERR_ARG;
+    if (old_ids[s] < 0 || new_ids[s] < 0 || (uint32_t)old_ids[s] >= num_pages ||
+        (uint32_t)new_ids[s] >= num_pages)
+      return KVO_ERR_PAGE_RANGE;
+    if (!apps[s] && n_app[s]) return KVO_ERR_ARG;
+  }
+  for (uint32_t s = 0; s < S; ++s) {
+    int rc = kvo_cow_append(base, L, C, num_pages, T, H, D, e, page_stride_bytes, old_ids[s],
+                            new_ids[s], n_old[s], apps[s], n_app[s]);
+    if (rc) return rc;
+  }
+  return KVO_OK;
+}
+
+/* O-repage, pool -> pool (SURVEY.md 8(c) reading 11 "fused pool->pool is an optional extra";
+ * 8(f) NEXT-2; PAPER.md:L298 cross-role reuse; BASELINE.json:configs[4] "sequence order preserved,
+ * tail page partially filled and zero-padded"): the transfer buffer of O-pack/O-unpack is skipped,
+ *   n_src = ceil(n_tokens / Ts), n_dst = ceil(n_tokens / Td)
+ *   for q,l,c,u,h,d:  j = q*Td + u
+ *     DST[l][c][dst_ids[q]][u][h][d] = (j < n_tokens) ? SRC[l][c][src_ids[j / Ts]][j % Ts][h][d] : 0
+ * Source and destination pools have the same L, C, H, D, e; page sizes Ts / Td, page counts and
+ * strides are their own.  Nothing else in the destination pool is written; SRC is never written. */
+int kvo_repage(const void *const *src_base, uint32_t src_num_pages, uint64_t src_stride_bytes,
+               uint32_t Ts, const int32_t *src_ids, uint64_t n_src, void *const *dst_base,
+               uint32_t dst_num_pages, uint64_t dst_stride_bytes, uint32_t Td,
+               const int32_t *dst_ids, uint64_t n_dst, uint32_t L, uint32_t C, uint32_t H,
+               uint32_t D, uint32_t e, uint64_t n_tokens, int threads) {
+  if (!src_base || !dst_base || !L || !C || !Ts || !Td || !H || !D || !e) return KVO_ERR_ARG;
+  if (n_src != (n_tokens + Ts - 1) / Ts || n_dst != (n_tokens + Td - 1) / Td) return KVO_ERR_ARG;
+  if ((!src_ids || !dst_ids) && n_tokens) return KVO_ERR_ARG;
+  if (!kvo_ids_in_range(src_ids, n_src, src_num_pages)) return KVO_ERR_PAGE_RANGE;
+  if (!kvo_ids_in_range(dst_ids, n_dst, dst_num_pages)) return KVO_ERR_PAGE_RANGE;
+#pragma omp parallel for num_threads(threads) if (threads > 1) schedule(static)
+  for (int64_t q = 0; q < (int64_t)n_dst; ++q)
+    for (uint64_t l = 0; l < L; ++l)
+      for (uint64_t c = 0; c < C; ++c)
+        for (uint64_t u = 0; u < Td; ++u)
+          for (uint64_t h = 0; h < H; ++h)
+            for (uint64_t d = 0; d < D; ++d) {
+              uint64_t j = (uint64_t)q * Td + u; /* sequence position, order preserved */
+              uint8_t *dst = (uint8_t *)dst_base[l * C + c] +
+                             (uint64_t)dst_ids[q] * dst_stride_bytes + ((u * H + h) * D + d) * e;
+              if (j < n_tokens) {
+                const uint8_t *src = (const uint8_t *)src_base[l * C + c] +
+                                     (uint64_t)src_ids[j / Ts] * src_stride_bytes +
+                                     (((j % Ts) * H + h) * D + d) * e;
+                kvo_copy_elem(dst, src, e);
+              } else {
+                kvo_zero_elem(dst, e);
+              }
+            }
+  return KVO_OK;
+}
+
+/* Batched O-repage: request r re-pages src_ids[src_off[r] .. src_off[r+1]) into
+ * dst_ids[dst_off[r] .. dst_off[r+1]) with its own n_tokens[r]. */
+int kvo_repage_batched(const void *const *src_base, uint32_t src_num_pages,
+                       uint64_t src_stride_bytes, uint32_t Ts, const int32_t *src_ids,
+                       const int64_t *src_off, void *const *dst_base, uint32_t dst_num_pages,
+                       uint64_t dst_stride_bytes, uint32_t Td, const int32_t *dst_ids,
+                       const int64_t *dst_off, const uint64_t *n_tokens, uint32_t R, uint32_t L,
+                       uint32_t C, uint32_t H, uint32_t D, uint32_t e, int threads) {
+  if (R && (!src_off || !dst_off || !n_tokens)) return KVO_ERR_ARG;
+  if (!Ts || !Td) return KVO_ERR_ARG;
+  for (uint32_t r = 0; r < R; ++r) {
+    if (src_off[r + 1] < src_off[r] || dst_off[r + 1] < dst_off[r]) return KVO_ERR_ARG;
+    if ((uint64_t)(src_off[r + 1] - src_off[r]) != (n_tokens[r] + Ts - 1) / Ts) return KVO_ERR_ARG;
+    if ((uint64_t)(dst_off[r + 1] - dst_off[r]) != (n_tokens[r] + Td - 1) / Td) return KVO_ERR_ARG;
+    if (!kvo_ids_in_range(src_ids + src_off[r], (uint64_t)(src_off[r + 1] - src_off[r]), src_num_pages))
+      return KVO_ERR_PAGE_RANGE;
+    if (!kvo_ids_in_range(dst_ids + dst_off[r], (uint64_t)(dst_off[r + 1] - dst_off[r]), dst_num_pages))
+      return KVO_ERR_PAGE_RANGE;
+  }
+  for (uint32_t r = 0; r < R; ++r) {
+    int rc = kvo_repage(src_base, src_num_pages, src_stride_bytes, Ts, src_ids + src_off[r],
+                        (uint64_t)(src_off[r + 1] - src_off[r]), dst_base, dst_num_pages,
+                        dst_stride_bytes, Td, dst_ids + dst_off[r],
+                        (uint64_t)(dst_off[r + 1] - dst_off[r]), L, C, H, D, e, n_tokens[r], threads);
+    if (rc) return rc;
+  }
+  return KVO_OK;
+}

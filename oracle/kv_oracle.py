@@ -10,7 +10,7 @@ BASELINE.json:configs[4] re-paging with a zero-padded tail):
 
 * ``*_py``  -- the definition as literal Python loops over (page, layer, K/V, token, head, dim);
                only for tiny cases.
-* ``pack`` / ``unpack`` / ``*_batched`` / ``cow_append`` -- the same loops compiled from
+* ``pack`` / ``unpack`` / ``repage`` / ``*_batched`` / ``cow_append`` -- the same loops compiled from
                ``kv_oracle.c`` (plain C, gcc -O2), called through ctypes.  This is the oracle
                used for parity at scale and the one ``bench.py`` times as ``cpu_baseline``.
 
@@ -228,6 +228,90 @@ def cow_append(pool: HostPool, old_id: int, new_id: int, n_old: int, app: np.nda
                                 ctypes.c_int32(old_id), ctypes.c_int32(new_id),
                                 ctypes.c_uint32(n_old), app.ctypes.data_as(ctypes.c_void_p),
                                 ctypes.c_uint32(n_app))
+    _check(rc)
+
+
+def cow_append_batched(pool: HostPool, old_ids, new_ids, n_old, n_app, apps: Sequence[np.ndarray],
+                       layer_count: int | None = None) -> None:
+    """Batched copy-on-write append, in place.
+    ``apps[s]`` is session s's dense [layer][K,V][token][head][dim] block of n_app[s] tokens."""
+    L = pool.L if layer_count is None else int(layer_count)
+    old_ids, new_ids = _ids(old_ids), _ids(new_ids)
+    n_old = np.ascontiguousarray(np.asarray(n_old, dtype=np.uint32))
+    n_app = np.ascontiguousarray(np.asarray(n_app, dtype=np.uint32))
+    S = len(old_ids)
+    assert len(new_ids) == S and len(n_old) == S and len(n_app) == S and len(apps) == S
+    _assert_distinct(new_ids)
+    if np.intersect1d(old_ids, new_ids).size:
+        raise ValueError("oracle: a new page id is also an old page id")
+    keep = [np.ascontiguousarray(a).view(np.uint8).reshape(-1) for a in apps]
+    tokrow = pool.H * pool.D * pool.e
+    ptrs = (ctypes.c_void_p * max(S, 1))()
+    for s in range(S):
+        if keep[s].size < L * pool.C * int(n_app[s]) * tokrow:
+            raise ValueError("oracle: append buffer too small")
+        ptrs[s] = keep[s].ctypes.data if keep[s].size else None
+    rc = _load().kvo_cow_append_batched(pool._ptrs(), ctypes.c_uint32(L), ctypes.c_uint32(pool.C),
+                                        ctypes.c_uint32(pool.num_pages), ctypes.c_uint32(pool.T),
+                                        ctypes.c_uint32(pool.H), ctypes.c_uint32(pool.D),
+                                        ctypes.c_uint32(pool.e),
+                                        ctypes.c_uint64(pool.page_stride_bytes),
+                                        old_ids.ctypes.data_as(ctypes.c_void_p),
+                                        new_ids.ctypes.data_as(ctypes.c_void_p),
+                                        n_old.ctypes.data_as(ctypes.c_void_p),
+                                        n_app.ctypes.data_as(ctypes.c_void_p), ptrs,
+                                        ctypes.c_uint32(S))
+    _check(rc)
+
+
+def _same_geometry(src: HostPool, dst: HostPool, L: int):
+    if (src.C, src.H, src.D, src.e) != (dst.C, dst.H, dst.D, dst.e) or L > src.L or L > dst.L:
+        raise ValueError("oracle: source and destination pools differ in C/H/D/e or have too few layers")
+
+
+def repage(src: HostPool, src_ids, dst: HostPool, dst_ids, n_tokens: int,
+           layer_count: int | None = None, threads: int = 1) -> None:
+    """O-repage pool -> pool (SURVEY.md 8(c) reading 11, 8(f) NEXT-2), into ``dst`` in place."""
+    L = min(src.L, dst.L) if layer_count is None else int(layer_count)
+    _same_geometry(src, dst, L)
+    src_ids, dst_ids = _ids(src_ids), _ids(dst_ids)
+    _assert_distinct(dst_ids)
+    rc = _load().kvo_repage(src._ptrs(), ctypes.c_uint32(src.num_pages),
+                            ctypes.c_uint64(src.page_stride_bytes), ctypes.c_uint32(src.T),
+                            src_ids.ctypes.data_as(ctypes.c_void_p), ctypes.c_uint64(len(src_ids)),
+                            dst._ptrs(), ctypes.c_uint32(dst.num_pages),
+                            ctypes.c_uint64(dst.page_stride_bytes), ctypes.c_uint32(dst.T),
+                            dst_ids.ctypes.data_as(ctypes.c_void_p), ctypes.c_uint64(len(dst_ids)),
+                            ctypes.c_uint32(L), ctypes.c_uint32(src.C), ctypes.c_uint32(src.H),
+                            ctypes.c_uint32(src.D), ctypes.c_uint32(src.e),
+                            ctypes.c_uint64(int(n_tokens)), ctypes.c_int(threads))
+    _check(rc)
+
+
+def repage_batched(src: HostPool, src_ids, src_off, dst: HostPool, dst_ids, dst_off, n_tokens,
+                   layer_count: int | None = None, threads: int = 1) -> None:
+    """Batched O-repage pool -> pool, into ``dst`` in place."""
+    L = min(src.L, dst.L) if layer_count is None else int(layer_count)
+    _same_geometry(src, dst, L)
+    src_ids, dst_ids = _ids(src_ids), _ids(dst_ids)
+    _assert_distinct(dst_ids)
+    src_off = np.ascontiguousarray(np.asarray(src_off, dtype=np.int64))
+    dst_off = np.ascontiguousarray(np.asarray(dst_off, dtype=np.int64))
+    ntok = np.ascontiguousarray(np.asarray(n_tokens, dtype=np.uint64))
+    R = len(ntok)
+    assert len(src_off) == R + 1 and len(dst_off) == R + 1
+    rc = _load().kvo_repage_batched(src._ptrs(), ctypes.c_uint32(src.num_pages),
+                                    ctypes.c_uint64(src.page_stride_bytes), ctypes.c_uint32(src.T),
+                                    src_ids.ctypes.data_as(ctypes.c_void_p),
+                                    src_off.ctypes.data_as(ctypes.c_void_p), dst._ptrs(),
+                                    ctypes.c_uint32(dst.num_pages),
+                                    ctypes.c_uint64(dst.page_stride_bytes), ctypes.c_uint32(dst.T),
+                                    dst_ids.ctypes.data_as(ctypes.c_void_p),
+                                    dst_off.ctypes.data_as(ctypes.c_void_p),
+                                    ntok.ctypes.data_as(ctypes.c_void_p), ctypes.c_uint32(R),
+                                    ctypes.c_uint32(L), ctypes.c_uint32(src.C),
+                                    ctypes.c_uint32(src.H), ctypes.c_uint32(src.D),
+                                    ctypes.c_uint32(src.e), ctypes.c_int(threads))
     _check(rc)
 
 

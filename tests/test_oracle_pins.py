@@ -416,3 +416,136 @@ def test_cow_append_is_slice_assignment():
         ko.cow_append(pool, 4, 1, 6, app, 4)  # overflow of the page
     with pytest.raises(ValueError):
         ko.cow_append(pool, 2, 2, 1, app, 1)  # in place is not copy-on-write
+
+
+def w4_pool():
+    L, C, P, T, H, D = 2, 2, 3, 4, 1, 2
+    A = np.zeros((L, C, P, T, H, D), dtype=np.uint16)
+    for l in range(L):
+        for c in range(C):
+            for g in range(P):
+                for t in range(T):
+                    for d in range(D):
+                        A[l, c, g, t, 0, d] = 1000 * (2 * l + c) + 8 * g + 2 * t + d
+    app = np.zeros((L, C, 2, H, D), dtype=np.uint16)
+    for l in range(L):
+        for c in range(C):
+            for t in range(2):
+                for d in range(D):
+                    app[l, c, t, 0, d] = 500 + 100 * (2 * l + c) + 2 * t + d
+    return A, app
+
+
+def test_W4_cow_append_hand_computed(golden):
+    A, app = w4_pool()
+    for batched in (False, True):
+        pool = pool_from_array(A)
+        if batched:
+            ko.cow_append_batched(pool, [1], [2], [1], [2], [app])
+        else:
+            ko.cow_append(pool, old_id=1, new_id=2, n_old=1, app=app, n_app=2)
+        got = np.concatenate([s.view(np.uint16) for s in pool.slabs]).tolist()
+        assert got == golden("W4_cow_append.txt")
+
+
+def test_cow_append_batched_is_slice_assignment_per_session():
+    """PAPER.md:L238, batched over sessions: every session's new page = its old page's first n_old
+    tokens followed by its append block; old pages, other pages and later slots untouched."""
+    rng = np.random.default_rng(19)
+    L, C, P, T, H, D = 3, 2, 24, 8, 2, 4
+    A = rand_array(rng, L, C, P, T, H, D, 2)
+    pool = pool_from_array(A, pad=16)
+    perm = rng.permutation(P)
+    S = 7
+    old, new = perm[:S], perm[S:2 * S]
+    n_old = np.array([0, 3, 7, 8, 1, 5, 0])
+    n_app = np.array([8, 4, 1, 0, 0, 2, 0])  # fresh page, mid, exactly full, pure copy, ..., no-op
+    apps = [rng.integers(0, 65536, size=(L, C, int(a), H, D), dtype=np.uint64).astype(np.uint16)
+            for a in n_app]
+    ko.cow_append_batched(pool, old, new, n_old, n_app, apps)
+    want = A.copy()
+    for s in range(S):
+        want[:, :, new[s], :n_old[s]] = A[:, :, old[s], :n_old[s]]
+        want[:, :, new[s], n_old[s]:n_old[s] + n_app[s]] = apps[s]
+    assert np.array_equal(array_from_pool(pool), want)
+    for s in pool.slabs:  # stride padding untouched
+        assert np.all(s.reshape(P, -1)[:, T * H * D * 2:] == 0xA5)
+    with pytest.raises(ValueError):
+        ko.cow_append_batched(pool, [1, 2], [3, 3], [1, 1], [1, 1], apps[:2])  # duplicate new page
+    with pytest.raises(ValueError):
+        ko.cow_append_batched(pool, [1, 2], [2, 3], [1, 1], [1, 1], apps[:2])  # new page is an old page
+    with pytest.raises(IndexError):
+        ko.cow_append_batched(pool, [1], [P], [1], [1], apps[:1])
+    # layer subset: only the first layer_count layers are touched
+    pool2 = pool_from_array(A)
+    ko.cow_append_batched(pool2, old[:2], new[:2], n_old[:2], n_app[:2],
+                          [a[:2] for a in apps[:2]], layer_count=2)
+    B = array_from_pool(pool2)
+    assert np.array_equal(B[2], A[2]) and not np.array_equal(B[:2], A[:2])
+
+
+# ---------------------------------------------------------------------------------------------
+# 6. fused pool -> pool re-paging (SURVEY.md 8(c) reading 11, 8(f) NEXT-2)
+# ---------------------------------------------------------------------------------------------
+def test_W3_repage_pool_to_pool_hand_computed(golden):
+    src = pool_from_array(w1_array())
+    dst = pool_from_array(np.full((2, 2, 3, 4, 1, 2), 7777, dtype=np.uint16))
+    ko.repage(src, [1, 2, 0], dst, [0, 2], n_tokens=5)
+    got = np.concatenate([s.view(np.uint16) for s in dst.slabs]).tolist()
+    assert got == golden("W3_repage_pool_to_pool.txt")
+    # W2's values again, reached without the buffer: src_ids=[3,0], n_tokens=3, dst_ids=[2]
+    dst = pool_from_array(np.full((2, 2, 3, 4, 1, 2), 7777, dtype=np.uint16))
+    ko.repage(src, [3, 0], dst, [2], n_tokens=3)
+    got = np.concatenate([s.view(np.uint16) for s in dst.slabs]).tolist()
+    assert got == golden("W2_repage_padded_tail.txt")
+
+
+@pytest.mark.parametrize("Ts,Td,ntok", [(4, 16, 61), (16, 4, 64), (3, 5, 31), (8, 8, 40), (2, 7, 1)])
+def test_repage_is_numpy_token_stream_reshape(Ts, Td, ntok):
+    """Library-routine pin: gather source pages with take, flatten the token axis, cut to n_tokens,
+    zero-fill to whole destination pages, reshape, scatter by fancy-index assignment."""
+    rng = np.random.default_rng(23)
+    L, C, H, D, e = 2, 2, 3, 4, 2
+    n_src, n_dst = -(-ntok // Ts), -(-ntok // Td)
+    A = rand_array(rng, L, C, n_src + 5, Ts, H, D, e)
+    B0 = rand_array(rng, L, C, n_dst + 4, Td, H, D, e)
+    src_ids = rng.permutation(n_src + 5)[:n_src]
+    dst_ids = rng.permutation(n_dst + 4)[:n_dst]
+    src, dst = pool_from_array(A, pad=8), pool_from_array(B0, pad=24)
+    ko.repage(src, src_ids, dst, dst_ids, n_tokens=ntok, threads=3)
+    stream = np.take(A, src_ids, axis=2).reshape(L, C, n_src * Ts, H, D)[:, :, :ntok]
+    padded = np.zeros((L, C, n_dst * Td, H, D), dtype=A.dtype)
+    padded[:, :, :ntok] = stream
+    want = B0.copy()
+    want[:, :, dst_ids] = padded.reshape(L, C, n_dst, Td, H, D)
+    assert np.array_equal(array_from_pool(dst), want)
+    assert np.array_equal(array_from_pool(src), A)  # the source pool is never written
+    for s in dst.slabs:  # stride padding untouched
+        assert np.all(s.reshape(n_dst + 4, -1)[:, Td * H * D * e:] == 0xA5)
+
+
+def test_repage_equals_pack_then_unpack_and_batched_equals_per_request():
+    rng = np.random.default_rng(29)
+    L, C, H, D, e, Ts, Td = 3, 2, 2, 4, 2, 4, 16
+    A = rand_array(rng, L, C, 64, Ts, H, D, e)
+    B0 = rand_array(rng, L, C, 20, Td, H, D, e)
+    src = pool_from_array(A)
+    ntok = np.array([37, 0, 64, 5])
+    ns, nd = -(-ntok // Ts), -(-ntok // Td)
+    soff, doff = np.concatenate([[0], np.cumsum(ns)]), np.concatenate([[0], np.cumsum(nd)])
+    sids = rng.permutation(64)[:soff[-1]]
+    dids = rng.permutation(20)[:doff[-1]]
+    d1, d2, d3 = (pool_from_array(B0) for _ in range(3))
+    ko.repage_batched(src, sids, soff, d1, dids, doff, ntok, threads=2)
+    for r in range(4):
+        a, b = slice(soff[r], soff[r + 1]), slice(doff[r], doff[r + 1])
+        ko.repage(src, sids[a], d2, dids[b], n_tokens=int(ntok[r]))
+        ko.unpack(ko.pack(src, sids[a]), dids[b], d3, Ts=Ts, n_tokens=int(ntok[r]))
+    for x, y, z in zip(d1.slabs, d2.slabs, d3.slabs):
+        assert np.array_equal(x, y) and np.array_equal(x, z)
+    with pytest.raises(ValueError):
+        ko.repage(src, sids[:2], d1, [1, 1], n_tokens=8)  # wrong destination count / duplicates
+    with pytest.raises(IndexError):
+        ko.repage(src, [64], d1, [1], n_tokens=4)
+    with pytest.raises(ValueError):
+        ko.repage(src, [1], pool_from_array(rand_array(rng, L, C, 4, Td, H, D + 1, e)), [1], n_tokens=4)
