@@ -186,6 +186,51 @@ int kv_unpack_batched(kv_ctx *ctx, const void *const *srcs, const uint64_t *src_
                       uint32_t layer_count, uint32_t src_page_size, uint32_t dst_page_size,
                       int layout, uint32_t flags, kv_stream_t stream);
 
+/* ---- fused pool -> pool re-paging (8(c) reading 11) ------------------
+ * kv_repage: kv_pack followed by kv_unpack without the transfer buffer, for cross-role reuse on one
+ * device (a diffusion role reuses the LLM role's conditioning KV;
+ * BASELINE.json:configs[4]: destination page size differs).  With Ts = src_pools->page_size and
+ * Td = dst_pools->page_size, sequence token j of the request lives in source page
+ * src_page_ids[j / Ts], slot j % Ts, and lands in destination page dst_page_ids[j / Td], slot j % Td;
+ * slots j >= n_tokens of the touched destination pages are all-bits-zero; source tokens >= n_tokens
+ * are ignored.  n_src_pages must be ceil(n_tokens/Ts) and n_dst_pages ceil(n_tokens/Td).  The two
+ * descriptors must agree in kv_count, num_heads, head_dim and elem_bytes (KV_ERR_DESC otherwise);
+ * page counts, page sizes and strides are their own; `layer_count` layers of both are used.  Ts == Td
+ * makes it a page migration inside or between pools.  The source pool is never written; destination
+ * pages must be distinct and must not be source pages.  HBM traffic is 2 x payload instead of the
+ * 4 x of pack + unpack.  KV_FLAG_IDS_ON_DEVICE is not supported here (KV_ERR_LAYOUT). */
+int kv_repage(kv_ctx *ctx, const kv_pool_desc *src_pools, const int32_t *src_page_ids,
+              uint32_t n_src_pages, const kv_pool_desc *dst_pools, const int32_t *dst_page_ids,
+              uint32_t n_dst_pages, uint32_t layer_count, uint64_t n_tokens, uint32_t flags,
+              kv_stream_t stream);
+/* Batched: request r re-pages src_page_ids[src_offsets[r] .. src_offsets[r+1]) into
+ * dst_page_ids[dst_offsets[r] .. dst_offsets[r+1]) with n_tokens[r] valid tokens.  ONE launch. */
+int kv_repage_batched(kv_ctx *ctx, const kv_pool_desc *src_pools, const int32_t *src_page_ids,
+                      const int64_t *src_offsets, const kv_pool_desc *dst_pools,
+                      const int32_t *dst_page_ids, const int64_t *dst_offsets,
+                      const uint64_t *n_tokens, uint32_t n_req, uint32_t layer_count, uint32_t flags,
+                      kv_stream_t stream);
+
+/* ---- copy-on-write partial-page append ----------------
+ * "When incremental data extends a retained partial page, the system copies its existing contents
+ * into a writable slot and appends the new data there.  The updated page is published under a new
+ * page ID, preserving the old published identity" (sec. 4.1.4).  For every (layer, K|V):
+ *   NEW[new_id][t] = OLD[old_id][t]        for t <  n_old
+ *                  = app[l][c][t - n_old]  for n_old <= t < n_old + n_app
+ *   slots t >= n_old + n_app of the new page, the old page and every other page are not written.
+ * `app` is DEVICE-accessible memory (device, or mapped pinned host), dense
+ * [layer][K,V][token][head][dim] with n_app tokens and `layer_count` layers; it may be NULL when
+ * n_app == 0 (a plain page copy).  n_old + n_app <= page_size and old_id != new_id (KV_ERR_SIZE).
+ * The batched call covers all sessions in ONE launch; new ids must be distinct and must not be any
+ * session's old id (checked under KV_FLAG_VALIDATE -> KV_ERR_DUP_PAGE).  Host id lists only. */
+int kv_cow_append(kv_ctx *ctx, const kv_pool_desc *pools, uint32_t layer_count, int32_t old_id,
+                  int32_t new_id, uint32_t n_old, const void *app, uint32_t n_app, uint32_t flags,
+                  kv_stream_t stream);
+int kv_cow_append_batched(kv_ctx *ctx, const kv_pool_desc *pools, uint32_t layer_count,
+                          const int32_t *old_ids, const int32_t *new_ids, const uint32_t *n_old,
+                          const uint32_t *n_app, const void *const *apps, uint32_t n_sessions,
+                          uint32_t flags, kv_stream_t stream);
+
 /* ---- host tier: offload (device -> pinned host) and reload (pinned host -> device) ----------
  * Same semantics and bytes as kv_pack / kv_unpack with the transfer buffer in PINNED HOST memory
  * (from kv_host_alloc, kv_host_register, cudaHostAlloc or torch pin_memory); a pageable pointer

@@ -22,6 +22,9 @@
 namespace kvt {
 
 // One contiguous transfer buffer: a request, or one pipeline chunk of a request.
+//   dir 2 (pool -> pool): `buf` is the index of the request's first SOURCE page id in ids[].
+//   dir 3 (copy-on-write append, one piece per session): `buf` = append block address,
+//         n_tokens = n_old | n_app << 32, id_begin = old page id | new page id << 32.
 struct Piece {
   uint64_t item_begin;   // first flat item index of this piece within the launch
   uint64_t buf;          // buffer base address (device memory or mapped pinned host memory)
@@ -41,7 +44,8 @@ struct Job {
   uint64_t buf_page_bytes;  // LC * buf_row_bytes (page-first)
   uint32_t n_pieces;
   uint32_t LC;            // layer_count * kv_count
-  uint32_t dir;           // 0 = pack (pool -> buffer), 1 = unpack (buffer -> pool)
+  uint32_t dir;           // 0 pack (pool -> buffer), 1 unpack (buffer -> pool), 2 re-page (pool -> pool),
+                          // 3 copy-on-write append (old page + append block -> new page)
   uint32_t layout;        // 0 page-first, 1 layer-first
   uint32_t g;             // tokens per chunk = gcd(Tpool, Tbuf)
   uint32_t cpp_pool;      // chunks per pool page  = Tpool / g
@@ -63,7 +67,8 @@ struct Job {
   unsigned long long *sched;  // global claim counter (items beyond the static first blocks)
   uint32_t *sched_done;       // warps finished; the last one resets both counters to 0
   uint32_t first_batch;       // B0: static items per warp before claiming starts
-  uint32_t pad_;
+  uint32_t src_num_pages;     // dir 2: pages of the SOURCE pool (range check of device-resident ids)
+  uint64_t src_page_stride;   // dir 2: source pool bytes between pages; its slab bases are bases[LC..2LC)
 };
 
 // The lookup tables of a launch: slab bases, page ids, pieces.  They live either in device memory
@@ -121,6 +126,26 @@ __device__ __forceinline__ Item decode(const Job &j, const Tables &tb, uint64_t 
   const uint64_t item_begin = ldt<kGlobal>(&pc->item_begin), buf = ldt<kGlobal>(&pc->buf),
                  n_tokens = ldt<kGlobal>(&pc->n_tokens), id_begin = ldt<kGlobal>(&pc->id_begin);
   const uint32_t local = (uint32_t)(item - item_begin);
+  if (j.dir == 3) {  // copy-on-write append: per (layer,kv) s0 items copy the old
+                     // page's first n_old tokens, s1 items append the session's new rows behind them
+    const uint32_t n_old = (uint32_t)n_tokens, n_app = (uint32_t)(n_tokens >> 32);
+    const uint32_t b_old = n_old * j.tokrow, b_app = n_app * j.tokrow;
+    const uint32_t s0 = (b_old + j.sub_bytes - 1) / j.sub_bytes, s1 = (b_app + j.sub_bytes - 1) / j.sub_bytes;
+    const uint32_t lc = local / (s0 + s1), k = local - lc * (s0 + s1);
+    const uint64_t slab = ldt<kGlobal>(tb.bases + lc);
+    const uint64_t old_pg = slab + (id_begin & 0xffffffffull) * j.page_stride;
+    const uint64_t new_pg = slab + (id_begin >> 32) * j.page_stride;
+    Item it;
+    if (k < s0) {
+      const uint32_t o = k * j.sub_bytes;
+      it.src = old_pg + o; it.dst = new_pg + o; it.bytes = min(j.sub_bytes, b_old - o);
+    } else {
+      const uint32_t o = (k - s0) * j.sub_bytes;
+      it.src = buf + (uint64_t)lc * b_app + o; it.dst = new_pg + b_old + o; it.bytes = min(j.sub_bytes, b_app - o);
+    }
+    it.valid = it.bytes;
+    return it;
+  }
   const uint32_t r1 = local / j.subs, sub = local - r1 * j.subs;
   const uint32_t k = r1 / j.LC, lc = r1 - k * j.LC;
   const uint32_t pp = k / j.cpp_pool, pk = k - pp * j.cpp_pool;
@@ -137,11 +162,25 @@ __device__ __forceinline__ Item decode(const Job &j, const Tables &tb, uint64_t 
   }
   const uint64_t paddr = ldt<kGlobal>(tb.bases + lc) + (uint64_t)id * j.page_stride +
                          (uint64_t)pk * j.chunk_bytes + sub_off;
-  uint64_t baddr = buf + (uint64_t)bk * j.chunk_bytes + sub_off;
-  if (j.layout == 0) baddr += (uint64_t)bp * j.buf_page_bytes + (uint64_t)lc * j.buf_row_bytes;
-  else baddr += ((uint64_t)lc * ldt<kGlobal>(&pc->n_buf_pages) + bp) * j.buf_row_bytes;
   const uint64_t tok0 = (uint64_t)k * j.g;
   const uint64_t vt = n_tokens > tok0 ? min(n_tokens - tok0, (uint64_t)j.g) : 0;
+  uint64_t baddr;
+  if (j.dir == 2 && vt == 0) {  // wholly zero-padded chunk: there is no source page to look up
+    baddr = 0;
+  } else if (j.dir == 2) {  // pool -> pool: the "buffer" side is page src_ids[bp] of the source pool
+    const int32_t sid = (kGlobal || j.ids) ? __ldg(tb.ids + buf + bp) : tb.ids[buf + bp];
+    if ((uint32_t)sid >= j.src_num_pages) {
+      atomicOr(j.status, 1u);
+      it.src = it.dst = 0; it.bytes = it.valid = 0;
+      return it;
+    }
+    baddr = ldt<kGlobal>(tb.bases + j.LC + lc) + (uint64_t)sid * j.src_page_stride +
+            (uint64_t)bk * j.chunk_bytes + sub_off;
+  } else {
+    baddr = buf + (uint64_t)bk * j.chunk_bytes + sub_off;
+    if (j.layout == 0) baddr += (uint64_t)bp * j.buf_page_bytes + (uint64_t)lc * j.buf_row_bytes;
+    else baddr += ((uint64_t)lc * ldt<kGlobal>(&pc->n_buf_pages) + bp) * j.buf_row_bytes;
+  }
   const uint64_t vbytes = vt * j.tokrow;
   it.valid = vbytes > sub_off ? (uint32_t)min(vbytes - sub_off, (uint64_t)it.bytes) : 0u;
   if (j.dir == 0) { it.src = paddr; it.dst = baddr; } else { it.src = baddr; it.dst = paddr; }

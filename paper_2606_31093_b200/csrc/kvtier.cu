@@ -105,6 +105,8 @@ struct Geom {
   int dir = 0, layout = 0;
   int kernel = KERNEL_BULK;
   uint32_t unit = 16;  // widest power of two dividing every address/length (elem kernel)
+  // dir 2 (pool -> pool): the source pool; its bases follow the destination's in the tables
+  const kv_pool_desc *src_pool = nullptr;
 };
 
 struct Req {          // one request as the caller states it
@@ -112,6 +114,7 @@ struct Req {          // one request as the caller states it
   uint64_t n_tokens = 0;
   uint64_t id_begin = 0, n_ids = 0;  // its page ids in the call's id array
   uint64_t n_buf_pages = 0;
+  uint64_t items = 0;  // work items of this request (filled by the planners)
 };
 
 int check_desc(const kv_pool_desc *p, uint32_t layer_count) {
@@ -146,7 +149,8 @@ uint32_t low_pow2(uint64_t v) {  // largest power of two (<= 16) dividing v; 16 
 }
 
 int make_geom(const kv_ctx *ctx, const kv_pool_desc *p, uint32_t layer_count, uint32_t Tbuf,
-              int dir, int layout, const std::vector<Req> &reqs, Geom *out) {
+              int dir, int layout, const std::vector<Req> &reqs, Geom *out,
+              const kv_pool_desc *src_pool = nullptr) {
   if (layout != KV_LAYOUT_PAGE_FIRST && layout != KV_LAYOUT_LAYER_FIRST) return KV_ERR_LAYOUT;
   Geom g;
   g.L = layer_count; g.C = p->kv_count; g.LC = g.L * g.C;
@@ -168,9 +172,15 @@ int make_geom(const kv_ctx *ctx, const kv_pool_desc *p, uint32_t layer_count, ui
   unit = std::min(unit, low_pow2(tokrow));
   unit = std::min(unit, low_pow2(g.page_stride));
   for (uint32_t i = 0; i < g.LC; ++i) unit = std::min(unit, low_pow2((uint64_t)(uintptr_t)p->base[i]));
-  for (const Req &r : reqs) {
-    if (r.buf % g.elem) return KV_ERR_ALIGN;
-    unit = std::min(unit, low_pow2(r.buf));
+  if (dir != 2)  // dir 2 keeps an id index in Req::buf, not an address
+    for (const Req &r : reqs) {
+      if (r.buf % g.elem) return KV_ERR_ALIGN;
+      unit = std::min(unit, low_pow2(r.buf));
+    }
+  if (src_pool) {
+    g.src_pool = src_pool;
+    unit = std::min(unit, low_pow2(src_pool->page_stride_bytes));
+    for (uint32_t i = 0; i < g.LC; ++i) unit = std::min(unit, low_pow2((uint64_t)(uintptr_t)src_pool->base[i]));
   }
   g.unit = unit;
   int kernel = ctx->kernel;
@@ -215,11 +225,13 @@ struct HostBlob {
 
 void build_blob(const kv_pool_desc *p, const Geom &g, const std::vector<Piece> &pieces,
                 const int32_t *ids, uint64_t n_ids, bool ids_on_device, HostBlob *hb) {
-  hb->off_pieces = (size_t)g.LC * 8;
+  hb->off_pieces = (size_t)g.LC * 8 * (g.src_pool ? 2 : 1);
   hb->off_ids = hb->off_pieces + pieces.size() * sizeof(Piece);
   hb->bytes.resize(hb->off_ids + (ids_on_device ? 0 : (size_t)n_ids * 4));
   uint8_t *h = hb->bytes.data();
   for (uint32_t i = 0; i < g.LC; ++i) ((uint64_t *)h)[i] = (uint64_t)(uintptr_t)p->base[i];
+  if (g.src_pool)
+    for (uint32_t i = 0; i < g.LC; ++i) ((uint64_t *)h)[g.LC + i] = (uint64_t)(uintptr_t)g.src_pool->base[i];
   std::memcpy(h + hb->off_pieces, pieces.data(), pieces.size() * sizeof(Piece));
   if (!ids_on_device && n_ids) std::memcpy(h + hb->off_ids, ids, (size_t)n_ids * 4);
 }
@@ -290,6 +302,7 @@ int launch(kv_ctx *ctx, const Geom &g, const Blob &b, uint32_t piece_first, uint
   j.g = g.g; j.cpp_pool = g.Tpool / g.g; j.cpp_buf = g.Tbuf / g.g;
   j.tokrow = g.tokrow; j.chunk_bytes = g.chunk_bytes; j.sub_bytes = g.sub_bytes; j.subs = g.subs;
   j.num_pages = g.num_pages;
+  if (g.src_pool) { j.src_num_pages = g.src_pool->num_pages; j.src_page_stride = g.src_pool->page_stride_bytes; }
   uint32_t cap = cta_cap ? cta_cap : ctx->max_ctas;
   uint32_t grid = 0;
   if (g.kernel == KERNEL_BULK) {
@@ -381,10 +394,10 @@ int plan_pack(kv_ctx *ctx, const kv_pool_desc *pools, uint32_t layer_count, cons
     if (rc) return rc;
   }
   c->total_items = 0; c->payload = 0;
-  for (const Req &q : c->reqs) {
-    const uint64_t it = items_of(c->geom, q.n_ids);
-    if (it > 0xFFFFFFFFull) return KV_ERR_SIZE;
-    c->total_items += it;
+  for (Req &q : c->reqs) {
+    q.items = items_of(c->geom, q.n_ids);
+    if (q.items > 0xFFFFFFFFull) return KV_ERR_SIZE;
+    c->total_items += q.items;
     c->payload += q.n_ids * page;
   }
   return KV_OK;
@@ -429,11 +442,121 @@ int plan_unpack(kv_ctx *ctx, const void *const *srcs, const uint64_t *src_bytes,
     }
   }
   c->total_items = 0; c->payload = 0;
-  for (const Req &q : c->reqs) {
-    const uint64_t it = items_of(c->geom, q.n_ids);
-    if (it > 0xFFFFFFFFull) return KV_ERR_SIZE;
-    c->total_items += it;
+  for (Req &q : c->reqs) {
+    q.items = items_of(c->geom, q.n_ids);
+    if (q.items > 0xFFFFFFFFull) return KV_ERR_SIZE;
+    c->total_items += q.items;
     c->payload += q.n_ids * lc * Td * tokrow;
+  }
+  return KV_OK;
+}
+
+// kv_repage[_batched]: destination pool `dp` (page size Td), source pool `sp` (page size Ts);
+// the combined id array is [all destination ids][all source ids] and Req::buf indexes into it.
+int plan_repage(kv_ctx *ctx, const kv_pool_desc *sp, const int32_t *src_ids, const int64_t *src_off,
+                const kv_pool_desc *dp, const int32_t *dst_ids, const int64_t *dst_off,
+                const uint64_t *n_tokens, uint32_t n_req, uint32_t layer_count, uint32_t flags,
+                Call *c, std::vector<int32_t> *all_ids) {
+  if (!ctx) return KV_ERR_NULL;
+  int rc = check_desc(dp, layer_count);
+  if (rc) return rc;
+  rc = check_desc(sp, layer_count);
+  if (rc) return rc;
+  if (flags & KV_FLAG_IDS_ON_DEVICE) return KV_ERR_LAYOUT;  // host id lists only on this entry
+  if (sp->kv_count != dp->kv_count || sp->num_heads != dp->num_heads || sp->head_dim != dp->head_dim ||
+      sp->elem_bytes != dp->elem_bytes)
+    return KV_ERR_DESC;
+  if (n_req && (!src_off || !dst_off || !n_tokens)) return KV_ERR_NULL;
+  const uint32_t Ts = sp->page_size, Td = dp->page_size;
+  const uint64_t tokrow = (uint64_t)dp->num_heads * dp->head_dim * dp->elem_bytes;
+  const uint64_t lc = (uint64_t)layer_count * dp->kv_count;
+  const uint64_t n_dst_total = n_req ? (uint64_t)dst_off[n_req] : 0;
+  c->reqs.clear();
+  for (uint32_t r = 0; r < n_req; ++r) {
+    if (dst_off[r + 1] < dst_off[r] || dst_off[r] < 0 || src_off[r + 1] < src_off[r] || src_off[r] < 0)
+      return KV_ERR_SIZE;
+    const uint64_t nd = (uint64_t)(dst_off[r + 1] - dst_off[r]), ns = (uint64_t)(src_off[r + 1] - src_off[r]);
+    if (nd != (n_tokens[r] + Td - 1) / Td || ns != (n_tokens[r] + Ts - 1) / Ts) return KV_ERR_SIZE;
+    if (!nd) continue;
+    Req q;
+    q.buf = n_dst_total + (uint64_t)src_off[r];  // index of its first source id in the combined array
+    q.n_tokens = n_tokens[r];
+    q.id_begin = (uint64_t)dst_off[r]; q.n_ids = nd; q.n_buf_pages = ns;
+    c->reqs.push_back(q);
+  }
+  const uint64_t n_src_total = n_req ? (uint64_t)src_off[n_req] : 0;
+  c->n_ids = n_dst_total + n_src_total;
+  if ((n_dst_total && !dst_ids) || (n_src_total && !src_ids)) return KV_ERR_NULL;
+  rc = make_geom(ctx, dp, layer_count, Ts, /*dir=*/2, KV_LAYOUT_PAGE_FIRST, c->reqs, &c->geom, sp);
+  if (rc) return rc;
+  rc = check_ids(dst_ids, n_dst_total, dp->num_pages);
+  if (rc) return rc;
+  rc = check_ids(src_ids, n_src_total, sp->num_pages);
+  if (rc) return rc;
+  if (flags & KV_FLAG_VALIDATE) {
+    rc = check_dups(dst_ids, n_dst_total, dp->num_pages);
+    if (rc) return rc;
+  }
+  all_ids->resize((size_t)c->n_ids);
+  if (n_dst_total) std::memcpy(all_ids->data(), dst_ids, (size_t)n_dst_total * 4);
+  if (n_src_total) std::memcpy(all_ids->data() + n_dst_total, src_ids, (size_t)n_src_total * 4);
+  c->total_items = 0; c->payload = 0;
+  for (Req &q : c->reqs) {
+    q.items = items_of(c->geom, q.n_ids);
+    if (q.items > 0xFFFFFFFFull) return KV_ERR_SIZE;
+    c->total_items += q.items;
+    c->payload += q.n_ids * lc * Td * tokrow;
+  }
+  return KV_OK;
+}
+
+// kv_cow_append[_batched]: one Req per session with something to move.
+int plan_cow(kv_ctx *ctx, const kv_pool_desc *pools, uint32_t layer_count, const int32_t *old_ids,
+             const int32_t *new_ids, const uint32_t *n_old, const uint32_t *n_app,
+             const void *const *apps, uint32_t n_sessions, uint32_t flags, Call *c) {
+  if (!ctx) return KV_ERR_NULL;
+  int rc = check_desc(pools, layer_count);
+  if (rc) return rc;
+  if (flags & KV_FLAG_IDS_ON_DEVICE) return KV_ERR_LAYOUT;
+  if (n_sessions && (!old_ids || !new_ids || !n_old || !n_app || !apps)) return KV_ERR_NULL;
+  const uint64_t tokrow = (uint64_t)pools->num_heads * pools->head_dim * pools->elem_bytes;
+  const uint64_t lc = (uint64_t)layer_count * pools->kv_count;
+  c->reqs.clear();
+  for (uint32_t s = 0; s < n_sessions; ++s) {
+    if ((uint64_t)n_old[s] + n_app[s] > pools->page_size || old_ids[s] == new_ids[s]) return KV_ERR_SIZE;
+    if (old_ids[s] < 0 || new_ids[s] < 0 || (uint32_t)old_ids[s] >= pools->num_pages ||
+        (uint32_t)new_ids[s] >= pools->num_pages)
+      return KV_ERR_PAGE_RANGE;
+    if (n_app[s] && !apps[s]) return KV_ERR_NULL;
+    if (!n_old[s] && !n_app[s]) continue;
+    Req q;
+    q.buf = (uint64_t)(uintptr_t)apps[s];
+    q.n_tokens = (uint64_t)n_old[s] | ((uint64_t)n_app[s] << 32);
+    q.id_begin = (uint64_t)(uint32_t)old_ids[s] | ((uint64_t)(uint32_t)new_ids[s] << 32);
+    c->reqs.push_back(q);
+  }
+  if (flags & KV_FLAG_VALIDATE) {  // new pages distinct, and none of them is some session's old page
+    std::vector<uint8_t> is_new((size_t)(pools->num_pages + 7) / 8, 0);
+    for (uint32_t s = 0; s < n_sessions; ++s) {
+      const uint32_t g = (uint32_t)new_ids[s];
+      if (is_new[g >> 3] & (1u << (g & 7))) return KV_ERR_DUP_PAGE;
+      is_new[g >> 3] |= (uint8_t)(1u << (g & 7));
+    }
+    for (uint32_t s = 0; s < n_sessions; ++s) {
+      const uint32_t g = (uint32_t)old_ids[s];
+      if (is_new[g >> 3] & (1u << (g & 7))) return KV_ERR_DUP_PAGE;
+    }
+  }
+  c->n_ids = 0;
+  rc = make_geom(ctx, pools, layer_count, pools->page_size, /*dir=*/3, KV_LAYOUT_PAGE_FIRST, c->reqs, &c->geom);
+  if (rc) return rc;
+  c->total_items = 0; c->payload = 0;
+  const uint64_t sub = c->geom.sub_bytes;
+  for (Req &q : c->reqs) {
+    const uint64_t b_old = (q.n_tokens & 0xffffffffull) * tokrow, b_app = (q.n_tokens >> 32) * tokrow;
+    q.items = lc * ((b_old + sub - 1) / sub + (b_app + sub - 1) / sub);
+    c->total_items += q.items;
+    c->payload += lc * (b_old + b_app);
   }
   return KV_OK;
 }
@@ -456,7 +579,7 @@ int run_single_launch(kv_ctx *ctx, const kv_pool_desc *pools, const Call &c, con
     pc.item_begin = acc; pc.buf = q.buf; pc.n_tokens = q.n_tokens; pc.id_begin = q.id_begin;
     pc.n_buf_pages = q.n_buf_pages;
     pieces.push_back(pc);
-    acc += items_of(c.geom, q.n_ids);
+    acc += q.items;
   }
   const bool dev_ids = flags & KV_FLAG_IDS_ON_DEVICE;
   HostBlob hb;
@@ -869,6 +992,48 @@ int kv_unpack_batched(kv_ctx *ctx, const void *const *srcs, const uint64_t *src_
                        layer_count, src_page_size, dst_page_size, layout, flags, &c);
   if (rc) return rc;
   return run_device(ctx, pools, c, dst_page_ids, flags, (cudaStream_t)stream);
+}
+
+int kv_repage_batched(kv_ctx *ctx, const kv_pool_desc *src_pools, const int32_t *src_page_ids,
+                      const int64_t *src_offsets, const kv_pool_desc *dst_pools,
+                      const int32_t *dst_page_ids, const int64_t *dst_offsets,
+                      const uint64_t *n_tokens, uint32_t n_req, uint32_t layer_count, uint32_t flags,
+                      kv_stream_t stream) {
+  Call c;
+  std::vector<int32_t> ids;
+  int rc = plan_repage(ctx, src_pools, src_page_ids, src_offsets, dst_pools, dst_page_ids,
+                       dst_offsets, n_tokens, n_req, layer_count, flags, &c, &ids);
+  if (rc) return rc;
+  return run_device(ctx, dst_pools, c, ids.data(), flags, (cudaStream_t)stream);
+}
+
+int kv_repage(kv_ctx *ctx, const kv_pool_desc *src_pools, const int32_t *src_page_ids,
+              uint32_t n_src_pages, const kv_pool_desc *dst_pools, const int32_t *dst_page_ids,
+              uint32_t n_dst_pages, uint32_t layer_count, uint64_t n_tokens, uint32_t flags,
+              kv_stream_t stream) {
+  const int64_t soff[2] = {0, (int64_t)n_src_pages}, doff[2] = {0, (int64_t)n_dst_pages};
+  const uint64_t nt[1] = {n_tokens};
+  return kv_repage_batched(ctx, src_pools, src_page_ids, soff, dst_pools, dst_page_ids, doff, nt, 1,
+                           layer_count, flags, stream);
+}
+
+int kv_cow_append_batched(kv_ctx *ctx, const kv_pool_desc *pools, uint32_t layer_count,
+                          const int32_t *old_ids, const int32_t *new_ids, const uint32_t *n_old,
+                          const uint32_t *n_app, const void *const *apps, uint32_t n_sessions,
+                          uint32_t flags, kv_stream_t stream) {
+  Call c;
+  int rc = plan_cow(ctx, pools, layer_count, old_ids, new_ids, n_old, n_app, apps, n_sessions, flags, &c);
+  if (rc) return rc;
+  return run_device(ctx, pools, c, nullptr, flags, (cudaStream_t)stream);
+}
+
+int kv_cow_append(kv_ctx *ctx, const kv_pool_desc *pools, uint32_t layer_count, int32_t old_id,
+                  int32_t new_id, uint32_t n_old, const void *app, uint32_t n_app, uint32_t flags,
+                  kv_stream_t stream) {
+  const int32_t o[1] = {old_id}, n[1] = {new_id};
+  const uint32_t no[1] = {n_old}, na[1] = {n_app};
+  const void *const ap[1] = {app};
+  return kv_cow_append_batched(ctx, pools, layer_count, o, n, no, na, ap, 1, flags, stream);
 }
 
 int kv_offload(kv_ctx *ctx, const kv_pool_desc *pools, uint32_t layer_count,

@@ -94,6 +94,12 @@ _kv_offload_batched = _sig("kv_offload_batched", _int, _vp, _pdesc, _u32, _vp, _
                            _vp, _vp, _int, _u32, _vp)
 _kv_reload_batched = _sig("kv_reload_batched", _int, _vp, _vp, _vp, _vp, _vp, _vp, _u32, _pdesc,
                           _u32, _u32, _u32, _int, _int, _u32, _vp)
+_kv_repage = _sig("kv_repage", _int, _vp, _pdesc, _vp, _u32, _pdesc, _vp, _u32, _u32, _u64, _u32, _vp)
+_kv_repage_batched = _sig("kv_repage_batched", _int, _vp, _pdesc, _vp, _vp, _pdesc, _vp, _vp, _vp,
+                          _u32, _u32, _u32, _vp)
+_kv_cow_append = _sig("kv_cow_append", _int, _vp, _pdesc, _u32, _i32, _i32, _u32, _vp, _u32, _u32, _vp)
+_kv_cow_append_batched = _sig("kv_cow_append_batched", _int, _vp, _pdesc, _u32, _vp, _vp, _vp, _vp,
+                              _vp, _u32, _u32, _vp)
 
 
 class KvError(RuntimeError):
@@ -378,3 +384,43 @@ def kv_reload_batched(ctx: Ctx, host_srcs, dst_page_ids, req_offsets, n_tokens, 
                                  off.ctypes.data, nt.ctypes.data, R, pools.ref, layer_count,
                                  src_page_size, dst_page_size, layout, mode, flags,
                                  _stream(stream)))
+
+
+def kv_repage(ctx: Ctx, src_pools: PoolDesc, src_page_ids, dst_pools: PoolDesc, dst_page_ids,
+              layer_count: int, n_tokens: int, flags=0, stream=None):
+    sp, skeep, ns = _ids_arg(src_page_ids, 0)
+    dp, dkeep, nd = _ids_arg(dst_page_ids, 0)
+    _chk(ctx, _kv_repage(ctx.h, src_pools.ref, sp, ns, dst_pools.ref, dp, nd, layer_count,
+                         int(n_tokens), flags, _stream(stream)))
+
+
+def kv_repage_batched(ctx: Ctx, src_pools: PoolDesc, src_page_ids, src_offsets, dst_pools: PoolDesc,
+                      dst_page_ids, dst_offsets, n_tokens, layer_count: int, flags=0, stream=None):
+    sp, skeep, _ = _ids_arg(src_page_ids, 0)
+    dp, dkeep, _ = _ids_arg(dst_page_ids, 0)
+    soff, R = _csr(src_offsets)
+    doff, R2 = _csr(dst_offsets)
+    assert R == R2
+    nt = _u64_array(n_tokens)
+    _chk(ctx, _kv_repage_batched(ctx.h, src_pools.ref, sp, soff.ctypes.data, dst_pools.ref, dp,
+                                 doff.ctypes.data, nt.ctypes.data, R, layer_count, flags,
+                                 _stream(stream)))
+
+
+def kv_cow_append(ctx: Ctx, pools: PoolDesc, layer_count: int, old_id: int, new_id: int, n_old: int,
+                  app, n_app: int, flags=0, stream=None):
+    _chk(ctx, _kv_cow_append(ctx.h, pools.ref, layer_count, int(old_id), int(new_id), int(n_old),
+                             _ptr(app), int(n_app), flags, _stream(stream)))
+
+
+def kv_cow_append_batched(ctx: Ctx, pools: PoolDesc, layer_count: int, old_ids, new_ids, n_old,
+                          n_app, apps, flags=0, stream=None):
+    o, n = _host_i32(old_ids), _host_i32(new_ids)
+    no = np.ascontiguousarray(np.asarray(n_old, dtype=np.uint32))
+    na = np.ascontiguousarray(np.asarray(n_app, dtype=np.uint32))
+    S = int(o.size)
+    assert n.size == S and no.size == S and na.size == S and len(apps) == S
+    a = _ptr_array(apps)
+    _chk(ctx, _kv_cow_append_batched(ctx.h, pools.ref, layer_count, o.ctypes.data if S else None,
+                                     n.ctypes.data if S else None, no.ctypes.data if S else None,
+                                     na.ctypes.data if S else None, a, S, flags, _stream(stream)))

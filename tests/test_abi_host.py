@@ -176,3 +176,33 @@ def test_auto_host_mode_policy(ctx):
     # layer-first buffers are not chunk-contiguous: staged falls back to direct
     assert status_of(lambda: kv.kv_offload(ctx, d, s.L, np.arange(512), BUF, 512 * s.page_bytes, mode=kv.KV_HOST_STAGED, layout=1)) == kv.KV_ERR_NO_DEVICE
     assert ctx.stat(kv.KV_STAT_LAST_HOST_MODE) == kv.KV_HOST_DIRECT
+
+
+def test_plan_fused_repage_and_cow(ctx):
+    """SURVEY.md 8(f) NEXT-2 / NEXT-1 planning: segment counts and payloads, validation before launch."""
+    c5 = W.crossrole_case(0)
+    src, dst = fake_pool(c5.src_shape), fake_pool(c5.dst_shape, base0=0x7800_0000_0000)
+    L = c5.dst_shape.L
+    f = lambda **kw: kv.kv_repage_batched(ctx, src, c5.src_ids, c5.src_offsets, dst, c5.dst_ids,
+                                          c5.dst_offsets, c5.n_tokens, L, **kw)
+    assert status_of(f) == kv.KV_ERR_NO_DEVICE
+    assert ctx.stat(kv.KV_STAT_LAST_ITEMS) == 32 * 32 * 4 * 96  # 16 KiB segments, 4 per 64-token row
+    assert ctx.stat(kv.KV_STAT_LAST_PAYLOAD) == 6 << 30
+    assert ctx.stat(kv.KV_STAT_LAST_KERNEL) == kv.KV_KERNEL_BULK
+    assert status_of(lambda: f(flags=kv.KV_FLAG_IDS_ON_DEVICE)) == kv.KV_ERR_LAYOUT
+    bad = c5.dst_ids.copy(); bad[5] = bad[4]
+    assert status_of(lambda: kv.kv_repage_batched(ctx, src, c5.src_ids, c5.src_offsets, dst, bad, c5.dst_offsets,
+                                                  c5.n_tokens, L, flags=kv.KV_FLAG_VALIDATE)) == kv.KV_ERR_DUP_PAGE
+    nt = np.array(c5.n_tokens).copy(); nt[0] += 1
+    assert status_of(lambda: kv.kv_repage_batched(ctx, src, c5.src_ids, c5.src_offsets, dst, c5.dst_ids,
+                                                  c5.dst_offsets, nt, L)) == kv.KV_ERR_SIZE
+    # copy-on-write append on the Qwen3-Omni shape: 5 old tokens + 7 new ones, 96 (layer,kv) rows
+    s = W.QWEN3_OMNI
+    d = fake_pool(s)
+    assert status_of(lambda: kv.kv_cow_append(ctx, d, s.L, 7, 9, 5, BUF, 7)) == kv.KV_ERR_NO_DEVICE
+    assert ctx.stat(kv.KV_STAT_LAST_ITEMS) == 96 * 2
+    assert ctx.stat(kv.KV_STAT_LAST_PAYLOAD) == 96 * 12 * 1024
+    assert status_of(lambda: kv.kv_cow_append(ctx, d, s.L, 7, 9, 10, BUF, 7)) == kv.KV_ERR_SIZE
+    assert status_of(lambda: kv.kv_cow_append(ctx, d, s.L, 7, 7, 1, BUF, 1)) == kv.KV_ERR_SIZE
+    assert status_of(lambda: kv.kv_cow_append(ctx, d, s.L, 7, s.P, 1, BUF, 1)) == kv.KV_ERR_PAGE_RANGE
+    kv.kv_cow_append(ctx, d, s.L, 7, 9, 0, None, 0)  # nothing to do: KV_OK, even without a device

@@ -1,0 +1,202 @@
+"""GPU parity for the SURVEY.md 8(f) rows built on top of the hot path: fused pool -> pool
+re-paging (NEXT-2, kv_repage) and copy-on-write partial-page append (NEXT-1, kv_cow_append,
+PAPER.md:L238), byte for byte against the CPU oracle on the same seeded inputs."""
+import numpy as np
+import pytest
+
+torch = pytest.importorskip("torch")
+pytestmark = pytest.mark.gpu
+
+from oracle import kv_oracle as ko  # noqa: E402
+from tests.kvhelpers import assert_pool_equal, host_pool, to_device  # noqa: E402
+
+
+@pytest.fixture(scope="module")
+def kv():
+    if not torch.cuda.is_available():
+        pytest.skip("no CUDA device")
+    from paper_2606_31093_b200 import kvtier
+    return kvtier
+
+
+@pytest.fixture()
+def ctx(kv):
+    c = kv.Ctx(0, staging_bytes=8 << 20)
+    yield c
+    torch.cuda.synchronize()
+    c.close()
+
+
+KERNELS = {"bulk": 1, "vec": 2, "elem": 3}
+
+
+@pytest.mark.parametrize("kernel", KERNELS)
+@pytest.mark.parametrize("Ts,Td,ntok,pad", [(16, 64, 2048, 0), (16, 64, 2048 - 37, 0), (64, 16, 1000, 0),
+                                            (16, 24, 500, 0), (3, 5, 77, 0), (16, 16, 16 * 9, 256),
+                                            (8, 64, 1, 0), (16, 64, 65, 0)])
+def test_repage_pool_to_pool(kv, ctx, kernel, Ts, Td, ntok, pad):
+    L, C, H, D, e = 3, 2, 4, 128, 2
+    rng = np.random.default_rng(Ts * 977 + Td * 31 + ntok)
+    ctx.set_option(kv.KV_OPT_KERNEL, KERNELS[kernel])
+    n_src, n_dst = -(-ntok // Ts), -(-ntok // Td)
+    A = host_pool(rng, L, C, n_src + 9, Ts, H, D, e, pad)
+    B = host_pool(rng, L, C, n_dst + 7, Td, H, D, e, pad)
+    tA, dA = to_device(A, kv, torch)
+    tB, dB = to_device(B, kv, torch)
+    sids = rng.permutation(n_src + 9)[:n_src].astype(np.int32)
+    dids = rng.permutation(n_dst + 7)[:n_dst].astype(np.int32)
+    launches = ctx.stat(kv.KV_STAT_LAUNCHES)
+    kv.kv_repage(ctx, dA, sids, dB, dids, L, ntok, flags=kv.KV_FLAG_VALIDATE)
+    assert ctx.stat(kv.KV_STAT_LAUNCHES) == launches + 1  # fused: one launch, no buffer
+    ko.repage(A, sids, B, dids, n_tokens=ntok)
+    assert_pool_equal(tB, B)  # touched pages equal; untouched pages and stride padding identical
+    assert_pool_equal(tA, A)  # the source pool is never written
+    assert ctx.stat(kv.KV_STAT_LAST_KERNEL) == KERNELS[kernel]
+
+
+def test_repage_batched_and_page_migration_inside_one_pool(kv, ctx):
+    L, C, H, D, e, Ts, Td = 4, 2, 2, 64, 2, 16, 64
+    rng = np.random.default_rng(41)
+    A = host_pool(rng, L, C, 400, Ts, H, D, e)
+    B = host_pool(rng, L, C, 120, Td, H, D, e)
+    tA, dA = to_device(A, kv, torch)
+    tB, dB = to_device(B, kv, torch)
+    ntok = np.array([2048, 0, 2048 - 61, 17, 64, 1000])
+    ns, nd = -(-ntok // Ts), -(-ntok // Td)
+    soff = np.concatenate([[0], np.cumsum(ns)]).astype(np.int64)
+    doff = np.concatenate([[0], np.cumsum(nd)]).astype(np.int64)
+    sids = rng.permutation(400)[:soff[-1]].astype(np.int32)
+    dids = rng.permutation(120)[:doff[-1]].astype(np.int32)
+    kv.kv_repage_batched(ctx, dA, sids, soff, dB, dids, doff, ntok, L)
+    ko.repage_batched(A, sids, soff, B, dids, doff, ntok)
+    assert_pool_equal(tB, B)
+    # layer subset
+    kv.kv_repage_batched(ctx, dA, sids[::-1].copy()[-int(soff[1]):], soff[:2], dB, dids[:int(doff[1])], doff[:2], ntok[:1], 2)
+    ko.repage_batched(A, sids[::-1].copy()[-int(soff[1]):], soff[:2], B, dids[:int(doff[1])], doff[:2], ntok[:1], layer_count=2)
+    assert_pool_equal(tB, B)
+    # Ts == Td inside ONE pool: a page migration (defragmentation); disjoint source/destination ids
+    perm = rng.permutation(400).astype(np.int32)
+    src, dst = perm[:50], perm[50:100]
+    A2 = A.copy()
+    kv.kv_repage(ctx, dA, src, dA, dst, L, 50 * Ts)
+    ko.repage(A, src, A2, dst, n_tokens=50 * Ts)
+    assert_pool_equal(tA, A2)
+
+
+def test_repage_errors_write_nothing(kv, ctx):
+    L, C, H, D, e = 2, 2, 2, 64, 2
+    rng = np.random.default_rng(43)
+    A = host_pool(rng, L, C, 20, 16, H, D, e)
+    B = host_pool(rng, L, C, 10, 64, H, D, e)
+    Bh = host_pool(rng, L, C, 10, 64, H + 1, D, e)
+    tA, dA = to_device(A, kv, torch)
+    tB, dB = to_device(B, kv, torch)
+    _, dBh = to_device(Bh, kv, torch)
+    s8 = np.arange(8, dtype=np.int32)
+
+    def status(fn):
+        try:
+            fn()
+        except kv.KvError as ex:
+            return ex.status
+        return 0
+
+    assert status(lambda: kv.kv_repage(ctx, dA, s8, dB, [1, 2, 3], L, 128)) == kv.KV_ERR_SIZE
+    assert status(lambda: kv.kv_repage(ctx, dA, s8[:7], dB, [1, 2], L, 128)) == kv.KV_ERR_SIZE
+    assert status(lambda: kv.kv_repage(ctx, dA, [0, 1, 2, 3, 4, 5, 6, 20], dB, [1, 2], L, 128)) == kv.KV_ERR_PAGE_RANGE
+    assert status(lambda: kv.kv_repage(ctx, dA, s8, dB, [1, 10], L, 128)) == kv.KV_ERR_PAGE_RANGE
+    assert status(lambda: kv.kv_repage(ctx, dA, s8, dB, [1, 1], L, 128, flags=kv.KV_FLAG_VALIDATE)) == kv.KV_ERR_DUP_PAGE
+    assert status(lambda: kv.kv_repage(ctx, dA, s8, dBh, [1, 2], L, 128)) == kv.KV_ERR_DESC
+    assert status(lambda: kv.kv_repage(ctx, dA, s8, dB, [1, 2], L + 1, 128)) == kv.KV_ERR_DESC
+    assert status(lambda: kv.kv_repage(ctx, dA, s8, dB, [1, 2], L, 128, flags=kv.KV_FLAG_IDS_ON_DEVICE)) == kv.KV_ERR_LAYOUT
+    kv.kv_repage(ctx, dA, [], dB, [], L, 0)  # empty: KV_OK, no launch
+    torch.cuda.synchronize()
+    assert_pool_equal(tB, B)
+    assert_pool_equal(tA, A)
+
+
+# ------------------------------------------------------------------------------------------------
+# copy-on-write partial-page append
+# ------------------------------------------------------------------------------------------------
+COW_SHAPES = [  # L, C, P, T, H, D, e, pad
+    (4, 2, 64, 16, 2, 64, 2, 0),     # Tiny-like
+    (3, 2, 40, 16, 4, 128, 2, 0),    # Qwen3-Omni row
+    (2, 2, 24, 64, 4, 128, 2, 0),    # 64 KiB rows: parts longer than one stage
+    (2, 1, 30, 5, 3, 24, 2, 0),      # odd sizes (tokrow 144 B)
+    (2, 2, 30, 16, 2, 64, 2, 256),   # padded stride
+    (2, 2, 30, 8, 1, 5, 1, 0),       # 5-byte token rows: elem path with unit 1
+]
+
+
+@pytest.mark.parametrize("kernel", KERNELS)
+@pytest.mark.parametrize("shape", COW_SHAPES)
+def test_cow_append_batched(kv, ctx, kernel, shape):
+    L, C, P, T, H, D, e, pad = shape
+    rng = np.random.default_rng(abs(hash(shape)) % 2**31)
+    ctx.set_option(kv.KV_OPT_KERNEL, KERNELS[kernel])
+    A = host_pool(rng, L, C, P, T, H, D, e, pad)
+    tA, dA = to_device(A, kv, torch)
+    S = 9
+    perm = rng.permutation(P).astype(np.int32)
+    old, new = perm[:S], perm[S:2 * S]
+    n_old = rng.integers(0, T + 1, size=S)
+    n_app = np.array([rng.integers(0, T - o + 1) for o in n_old])
+    n_old[0], n_app[0] = 0, T      # a fresh page filled by the append alone
+    n_old[1], n_app[1] = T, 0      # a plain page copy
+    n_old[2], n_app[2] = 0, 0      # nothing to do for this session
+    n_old[3], n_app[3] = T - 1, 1  # exactly full after the append
+    apps = [rng.integers(0, 256, size=L * C * int(a) * H * D * e, dtype=np.uint8) for a in n_app]
+    dev_apps = [torch.from_numpy(a).cuda() if a.size else None for a in apps]
+    launches = ctx.stat(kv.KV_STAT_LAUNCHES)
+    kv.kv_cow_append_batched(ctx, dA, L, old, new, n_old, n_app, dev_apps, flags=kv.KV_FLAG_VALIDATE)
+    assert ctx.stat(kv.KV_STAT_LAUNCHES) == launches + 1  # all sessions in one launch
+    ko.cow_append_batched(A, old, new, n_old, n_app, apps)
+    assert_pool_equal(tA, A)  # new pages equal; old pages, other pages, later slots, padding identical
+    want_kernel = KERNELS[kernel] if (H * D * e) % 16 == 0 else KERNELS["elem"]
+    assert ctx.stat(kv.KV_STAT_LAST_KERNEL) == want_kernel
+
+
+def test_cow_append_single_layer_subset_and_host_append_block(kv, ctx):
+    L, C, P, T, H, D, e = 4, 2, 32, 16, 2, 64, 2
+    rng = np.random.default_rng(47)
+    A = host_pool(rng, L, C, P, T, H, D, e)
+    tA, dA = to_device(A, kv, torch)
+    n_old, n_app, Lsub = 5, 7, 3
+    app = rng.integers(0, 256, size=Lsub * C * n_app * H * D * e, dtype=np.uint8)
+    hp = kv.kv_host_alloc(app.size)  # the new rows may sit in mapped pinned host memory
+    try:
+        kv.host_view(hp, app.size)[:] = app
+        kv.kv_cow_append(ctx, dA, Lsub, 3, 9, n_old, hp, n_app)
+        torch.cuda.synchronize()
+    finally:
+        kv.kv_host_free(hp)
+    ko.cow_append(A, 3, 9, n_old, app, n_app, layer_count=Lsub)
+    assert_pool_equal(tA, A)
+
+
+def test_cow_errors_write_nothing(kv, ctx):
+    L, C, P, T, H, D, e = 2, 2, 16, 16, 2, 64, 2
+    rng = np.random.default_rng(53)
+    A = host_pool(rng, L, C, P, T, H, D, e)
+    tA, dA = to_device(A, kv, torch)
+    app = torch.zeros(L * C * T * H * D * e, dtype=torch.uint8, device="cuda")
+
+    def status(fn):
+        try:
+            fn()
+        except kv.KvError as ex:
+            return ex.status
+        return 0
+
+    assert status(lambda: kv.kv_cow_append(ctx, dA, L, 1, 2, 10, app, 7)) == kv.KV_ERR_SIZE      # overflows the page
+    assert status(lambda: kv.kv_cow_append(ctx, dA, L, 2, 2, 1, app, 1)) == kv.KV_ERR_SIZE       # in place is not CoW
+    assert status(lambda: kv.kv_cow_append(ctx, dA, L, 1, P, 1, app, 1)) == kv.KV_ERR_PAGE_RANGE
+    assert status(lambda: kv.kv_cow_append(ctx, dA, L, -1, 2, 1, app, 1)) == kv.KV_ERR_PAGE_RANGE
+    assert status(lambda: kv.kv_cow_append(ctx, dA, L, 1, 2, 1, None, 1)) == kv.KV_ERR_NULL
+    assert status(lambda: kv.kv_cow_append_batched(ctx, dA, L, [1, 3], [2, 2], [1, 1], [1, 1], [app, app],
+                                                   flags=kv.KV_FLAG_VALIDATE)) == kv.KV_ERR_DUP_PAGE
+    assert status(lambda: kv.kv_cow_append_batched(ctx, dA, L, [1, 2], [2, 3], [1, 1], [1, 1], [app, app],
+                                                   flags=kv.KV_FLAG_VALIDATE)) == kv.KV_ERR_DUP_PAGE
+    kv.kv_cow_append_batched(ctx, dA, L, [], [], [], [], [])  # empty: KV_OK, no launch
+    torch.cuda.synchronize()
+    assert_pool_equal(tA, A)
