@@ -27,6 +27,10 @@
  *     must be distinct and free (the slot engine guarantees it).
  *   - Elements are opaque `elem_bytes`-wide bit patterns; nothing is ever interpreted as a number.
  *   - All byte offsets are 64-bit.
+ *   - CUDA graphs: every transfer whose tables fit the kernel parameters is ONE kernel node and may be
+ *     captured (cudaStreamBeginCapture on `stream`); page ids passed as host arrays are baked into the
+ *     node, ids passed with KV_FLAG_IDS_ON_DEVICE are re-read from device memory at every replay.
+ *     Host-tier calls captured with KV_HOST_AUTO use DIRECT.  Otherwise: KV_ERR_CAPTURE.
  *   - A kv_ctx is not thread-safe: one ctx per calling thread.  Calls on different streams are
  *     independent when their destination page sets are disjoint.
  */
@@ -89,6 +93,9 @@ typedef enum kv_status {
   KV_ERR_HOST_MEM = -8,   /* host buffer of an offload/reload is not pinned (page-locked) memory */
   KV_ERR_DESC = -9,       /* malformed kv_pool_desc (zero dimension, bad elem_bytes, stride < row, layer_count too large) */
   KV_ERR_NO_DEVICE = -10, /* planning-only ctx (device < 0): arguments were valid, nothing was launched */
+  KV_ERR_CAPTURE = -11,   /* `stream` is capturing a CUDA graph and this call is not replayable: its tables exceed
+                             the kernel parameters (~31 KiB: about 7,500 page ids), the element-wise fallback kernel
+                             is needed, or mode is KV_HOST_STAGED.  Nothing was enqueued. */
 } kv_status;
 
 /* flags (bit set) */

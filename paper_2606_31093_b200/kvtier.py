@@ -28,6 +28,7 @@ _lib = ctypes.CDLL(LIB_PATH)
 KV_OK = 0
 KV_ERR_NULL, KV_ERR_SIZE, KV_ERR_PAGE_RANGE, KV_ERR_DUP_PAGE, KV_ERR_LAYOUT = -1, -2, -3, -4, -5
 KV_ERR_ALIGN, KV_ERR_CUDA, KV_ERR_HOST_MEM, KV_ERR_DESC, KV_ERR_NO_DEVICE = -6, -7, -8, -9, -10
+KV_ERR_CAPTURE = -11
 KV_LAYOUT_PAGE_FIRST, KV_LAYOUT_LAYER_FIRST = 0, 1
 KV_HOST_AUTO, KV_HOST_DIRECT, KV_HOST_STAGED = 0, 1, 2
 KV_FLAG_VALIDATE, KV_FLAG_IDS_ON_DEVICE = 0x1, 0x2
@@ -144,15 +145,21 @@ def _nbytes(x) -> int:
     raise TypeError(f"cannot size {type(x)}; pass nbytes explicitly")
 
 
-def _stream(s) -> Optional[int]:
-    if s is None:
-        try:
-            import torch
+_torch = None
 
-            if torch.cuda.is_available() and torch.cuda.is_initialized():
-                return int(torch.cuda.current_stream().cuda_stream) or None
-        except ImportError:
-            pass
+
+def _stream(s) -> Optional[int]:
+    """cudaStream_t of `s` (torch stream / int / None = torch's current stream, else the default)."""
+    global _torch
+    if s is None:
+        if _torch is None:
+            try:
+                import torch
+            except ImportError:
+                return None
+            _torch = torch
+        if _torch.cuda.is_initialized():
+            return int(_torch.cuda.current_stream().cuda_stream) or None
         return None
     if isinstance(s, int):
         return s or None

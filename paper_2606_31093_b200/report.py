@@ -21,6 +21,10 @@ from . import workloads as W
 
 
 def _events(torch, fn, reps, warm, flush=None):
+    """Median / best duration in us of `fn` between two CUDA events on the current stream.
+    `flush` = (w, r): write 512 MiB then read another 512 MiB before every timed call, so the 126 MB
+    L2 is cold AND clean -- a write-only flush leaves up to an L2's worth of dirty lines whose
+    write-back (~20 us of DRAM time) would be billed to the timed call."""
     stream = torch.cuda.current_stream()
     for _ in range(warm):
         fn()
@@ -28,7 +32,8 @@ def _events(torch, fn, reps, warm, flush=None):
     ts = []
     for _ in range(reps):
         if flush is not None:
-            flush.fill_(1)
+            flush[0].fill_(1)
+            flush[1].view(torch.int64).sum()
         a, b = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
         a.record(stream)
         fn()
@@ -43,7 +48,8 @@ def run(ctx, desc, shape, slabs, seed=0, out_dir="gpurun_out", hbm_peak=None):
 
     rng = np.random.default_rng(seed + 77)
     recs = []
-    flush = torch.empty(512 << 20, dtype=torch.uint8, device="cuda")
+    flush = (torch.empty(512 << 20, dtype=torch.uint8, device="cuda"),
+             torch.zeros(512 << 20, dtype=torch.uint8, device="cuda"))
 
     # ---- peaks measured in this run -----------------------------------------------------------
     N = 1 << 30
@@ -215,7 +221,21 @@ def run(ctx, desc, shape, slabs, seed=0, out_dir="gpurun_out", hbm_peak=None):
             rec(name, "unpack_batched re-page 16->64", "device", wr, rd + wr, int(c5.dst_offsets[-1]),
                 lambda: kv.kv_unpack_batched(ctx, bufs5, c5.dst_ids, c5.dst_offsets, c5.n_tokens, d_dst, L, 16, 64),
                 reps=10)
+            rec(name, "repage_batched fused pool->pool 16->64", "device", wr, rd + wr, int(c5.dst_offsets[-1]),
+                lambda: kv.kv_repage_batched(ctx, d_src, c5.src_ids, c5.src_offsets, d_dst, c5.dst_ids,
+                                             c5.dst_offsets, c5.n_tokens, L), reps=10)
             del big5, bufs5
+
+        # ---- NEXT-1: copy-on-write tail-page append, 64 sessions in one launch -------
+        S = 64
+        perm = rng.permutation(shape.P).astype(np.int32)
+        n_old = rng.integers(0, T, size=S)
+        n_app = np.array([rng.integers(1, T - o + 1) for o in n_old])
+        apps = [torch.empty(int(a) * shape.tok_bytes, dtype=torch.uint8, device="cuda") for a in n_app]
+        plc = int((n_old + n_app).sum()) * shape.tok_bytes
+        rec("3 session", "cow_append_batched (64 sessions' tail pages)", "device", plc, 2 * plc, S,
+            lambda: kv.kv_cow_append_batched(ctx, desc, L, perm[:S], perm[S:2 * S], n_old, n_app, apps), reps=20)
+        del apps
 
         # ---- transfer-size sweep 1 MiB .. 8 GiB (layer_count = 32 => 1 MiB pages) --------------------
         Ls = 32
@@ -238,6 +258,8 @@ def run(ctx, desc, shape, slabs, seed=0, out_dir="gpurun_out", hbm_peak=None):
             row_["unpack_GBps"], row_["unpack_us"] = 2 * pls / m / 1e3, m
             m, bst = _events(torch, lambda: kv.kv_unpack(ctx, bufS, dst64, d_dst, Ls, 16, 64, npg * 16), reps, 2, fl_)
             row_["repage_GBps"], row_["repage_us"] = (pls + nd * Ls * shape.C * 4 * row) / m / 1e3, m
+            m, bst = _events(torch, lambda: kv.kv_repage(ctx, d_src, ids_s, d_dst, dst64, Ls, npg * 16), reps, 2, fl_)
+            row_["repage_fused_GBps"], row_["repage_fused_us"] = (pls + nd * Ls * shape.C * 4 * row) / m / 1e3, m
             reps_h = 7 if pls <= (1 << 30) else 3
             m, bst = _events(torch, lambda: kv.kv_offload(ctx, desc, Ls, ids, hp, pls), reps_h, 1)
             row_["offload_GBps"], row_["offload_us"], row_["offload_mode"] = pls / m / 1e3, m, ctx.stat(kv.KV_STAT_LAST_HOST_MODE)

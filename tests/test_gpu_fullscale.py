@@ -252,6 +252,57 @@ def test_config5_cross_role_repage(kv, ctx, pool, ragged):
         ko.unpack(want, np.arange(len(dids)), exp, Ts=16, n_tokens=int(c5.n_tokens[r]), threads=THREADS)
         for x, y in zip(got.slabs, exp.slabs):
             assert np.array_equal(x, y), f"request {r}: re-paged pages != oracle"
+    # fused pool -> pool re-paging (kv_repage_batched) into OTHER free
+    # destination pages: one launch, no transfer buffer, same bytes as the oracle's O-repage
+    free = np.setdiff1d(np.arange(s_dst.P, dtype=np.int32), c5.dst_ids)
+    dids2 = np.random.default_rng(5).permutation(free)[:len(c5.dst_ids)].astype(np.int32)
+    before = page_checksums(torch, dst_slabs, s_dst)
+    launches = ctx.stat(kv.KV_STAT_LAUNCHES)
+    kv.kv_repage_batched(ctx, d_src, c5.src_ids, c5.src_offsets, d_dst, dids2, c5.dst_offsets, c5.n_tokens, s_dst.L)
+    assert ctx.stat(kv.KV_STAT_LAUNCHES) == launches + 1 and ctx.stat(kv.KV_STAT_LAST_GRID) == 148
+    torch.cuda.synchronize()
+    assert_untouched(before, page_checksums(torch, dst_slabs, s_dst), dids2, s_dst.P)
+    for r in range(0, R, 5):
+        ids = c5.src_ids[c5.src_offsets[r]:c5.src_offsets[r + 1]]
+        mini = snapshot_pages(torch, src_slabs, ids, s_src)
+        dd = dids2[c5.dst_offsets[r]:c5.dst_offsets[r + 1]]
+        got = snapshot_pages(torch, dst_slabs, dd, s_dst)
+        exp = ko.HostPool([np.full_like(s, 0x5A) for s in got.slabs], s_dst.L, s_dst.C, len(dd), 64,
+                          s_dst.H, s_dst.D, s_dst.e, s_dst.row_bytes)
+        ko.repage(mini, np.arange(len(ids)), exp, np.arange(len(dd)), n_tokens=int(c5.n_tokens[r]), threads=THREADS)
+        for x, y in zip(got.slabs, exp.slabs):
+            assert np.array_equal(x, y), f"request {r}: fused re-page != oracle"
+    # and it equals what pack + unpack produced, for ALL requests (device-side compare)
+    a = torch.as_tensor(c5.dst_ids.astype(np.int64), device="cuda")
+    b2 = torch.as_tensor(dids2.astype(np.int64), device="cuda")
+    for s in dst_slabs[::5]:
+        v = s.view(s_dst.P, s_dst.row_bytes)
+        assert torch.equal(v.index_select(0, a), v.index_select(0, b2))
+
+
+def test_cow_tail_pages_of_64_sessions(kv, ctx, pool):
+    """PAPER.md:L238 at the Qwen3-Omni shape: 64 sessions each extend a retained partial tail page
+    (copy n_old tokens into a fresh page, append n_app new tokens) in ONE launch."""
+    shape, slabs, desc = pool
+    rng = np.random.default_rng(64)
+    S = 64
+    perm = rng.permutation(shape.P).astype(np.int32)
+    old, new = perm[:S], perm[S:2 * S]
+    n_old = rng.integers(0, shape.T, size=S)
+    n_app = np.array([rng.integers(0, shape.T - o + 1) for o in n_old])
+    apps_h = [rng.integers(0, 256, size=shape.L * shape.C * int(a) * shape.H * shape.D * shape.e, dtype=np.uint8) for a in n_app]
+    apps = [torch.from_numpy(a).cuda() if a.size else None for a in apps_h]
+    touched = np.concatenate([old, new])
+    mini = snapshot_pages(torch, slabs, touched, shape)
+    before = page_checksums(torch, slabs, shape)
+    kv.kv_cow_append_batched(ctx, desc, shape.L, old, new, n_old, n_app, apps, flags=kv.KV_FLAG_VALIDATE)
+    torch.cuda.synchronize()
+    assert ctx.stat(kv.KV_STAT_LAST_KERNEL) == kv.KV_KERNEL_BULK
+    assert_untouched(before, page_checksums(torch, slabs, shape), new, shape.P)
+    ko.cow_append_batched(mini, np.arange(S), np.arange(S, 2 * S), n_old, n_app, apps_h)
+    got = snapshot_pages(torch, slabs, touched, shape)
+    for x, y in zip(got.slabs, mini.slabs):
+        assert np.array_equal(x, y), "batched CoW append != oracle"
 
 
 @pytest.mark.parametrize("n", [1, 2, 64, 683, 8192])

@@ -200,3 +200,87 @@ def test_cow_errors_write_nothing(kv, ctx):
     kv.kv_cow_append_batched(ctx, dA, L, [], [], [], [], [])  # empty: KV_OK, no launch
     torch.cuda.synchronize()
     assert_pool_equal(tA, A)
+
+
+# ------------------------------------------------------------------------------------------------
+# CUDA graphs: a transfer is one kernel node; device-resident ids are re-read at every replay
+# ------------------------------------------------------------------------------------------------
+def test_cuda_graph_capture_and_replay_with_device_ids(kv, ctx):
+    L, C, P, T, H, D, e = 4, 2, 256, 16, 2, 64, 2
+    rng = np.random.default_rng(61)
+    A = host_pool(rng, L, C, P, T, H, D, e)
+    B = host_pool(rng, L, C, P, T, H, D, e)
+    tA, dA = to_device(A, kv, torch)
+    tB, dB = to_device(B, kv, torch)
+    n = 37
+    d_src = torch.zeros(n, dtype=torch.int32, device="cuda")
+    d_dst = torch.zeros(n, dtype=torch.int32, device="cuda")
+    buf = torch.zeros(n * dA.page_bytes(), dtype=torch.uint8, device="cuda")
+    side = torch.cuda.Stream()
+    g = torch.cuda.CUDAGraph()
+    launches = ctx.stat(kv.KV_STAT_LAUNCHES)
+    hp = kv.kv_host_alloc(buf.numel())
+    with torch.cuda.graph(g, stream=side):
+        kv.kv_pack(ctx, dA, L, d_src, buf, flags=kv.KV_FLAG_IDS_ON_DEVICE, stream=side)
+        kv.kv_unpack(ctx, buf, d_dst, dB, L, T, T, n * T, flags=kv.KV_FLAG_IDS_ON_DEVICE, stream=side)
+        # not replayable: staged host mode -> refused, nothing enqueued
+        with pytest.raises(kv.KvError) as ei:
+            kv.kv_offload(ctx, dA, L, np.arange(n), hp, buf.numel(), mode=kv.KV_HOST_STAGED, stream=side)
+        assert ei.value.status == kv.KV_ERR_CAPTURE
+    kv.kv_host_free(hp)
+    assert ctx.stat(kv.KV_STAT_LAUNCHES) == launches + 2
+    for rep in range(3):  # new page ids per replay, no host work besides the id upload
+        src = rng.choice(P, n, replace=False).astype(np.int32)
+        dst = rng.permutation(P)[:n].astype(np.int32)
+        d_src.copy_(torch.from_numpy(src))
+        d_dst.copy_(torch.from_numpy(dst))
+        torch.cuda.synchronize()
+        g.replay()
+        torch.cuda.synchronize()
+        want = ko.pack(A, src)
+        assert np.array_equal(buf.cpu().numpy(), want), f"replay {rep}: pack != oracle"
+        ko.unpack(want, dst, B, Ts=T, n_tokens=n * T)
+        assert_pool_equal(tB, B)
+    assert ctx.device_status() == 0
+
+
+def test_cuda_graph_large_transfer_host_ids_and_direct_offload(kv, ctx):
+    """Large captured transfers use the static work distribution; host ids are baked into the node;
+    KV_HOST_AUTO captured = DIRECT (one kernel storing to mapped pinned memory)."""
+    L, C, P, T, H, D, e = 6, 2, 512, 16, 4, 128, 2
+    rng = np.random.default_rng(67)
+    A = host_pool(rng, L, C, P, T, H, D, e)
+    tA, dA = to_device(A, kv, torch)
+    n = 400  # 400 * 12 = 4,800 segments >= 8 per warp: dynamic claiming when launched live
+    ids = rng.choice(P, n, replace=False).astype(np.int32)
+    nbytes = n * dA.page_bytes()
+    buf = torch.zeros(nbytes, dtype=torch.uint8, device="cuda")
+    hp = kv.kv_host_alloc(nbytes)
+    try:
+        side = torch.cuda.Stream()
+        g = torch.cuda.CUDAGraph()
+        with torch.cuda.graph(g, stream=side):
+            kv.kv_pack(ctx, dA, L, ids, buf, stream=side)
+            kv.kv_offload(ctx, dA, L, ids, hp, nbytes, stream=side)  # AUTO would be STAGED (75 MiB) live
+        assert ctx.stat(kv.KV_STAT_LAST_HOST_MODE) == kv.KV_HOST_DIRECT
+        want = ko.pack(A, ids)
+        for rep in range(2):
+            buf.zero_()
+            kv.host_view(hp, nbytes)[:] = 0
+            torch.cuda.synchronize()
+            g.replay()
+            torch.cuda.synchronize()
+            assert np.array_equal(buf.cpu().numpy(), want)
+            assert np.array_equal(kv.host_view(hp, nbytes), want)
+        # too many ids for the kernel parameters -> cannot be captured
+        big_ids = rng.integers(0, P, size=9000).astype(np.int32)
+        big = torch.empty(16, dtype=torch.uint8, device="cuda")
+        g2 = torch.cuda.CUDAGraph()
+        with torch.cuda.graph(g2, stream=side):
+            kv.kv_pack(ctx, dA, L, ids[:4], buf, stream=side)
+            with pytest.raises(kv.KvError) as ei:
+                kv.kv_pack(ctx, dA, L, big_ids, big, dst_bytes=1 << 40, stream=side)
+            assert ei.value.status == kv.KV_ERR_CAPTURE
+    finally:
+        torch.cuda.synchronize()
+        kv.kv_host_free(hp)
