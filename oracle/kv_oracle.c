@@ -14,6 +14,11 @@
  *                       POOL[l][c][g][t][h][d] = *(elem*)(base[l*C+c] + g*page_stride_bytes
  *                                                         + ((t*H + h)*D + d)*e)
  *                     in-page order NHD = [token][head][dim] ("NHD block stacks").
+ *   HND pools         PAPER.md:L214 "compute-oriented layouts, INCLUDING NHD block stacks" (so
+ *                     others exist); SURVEY.md 8(f) NEXT-2 "HND pools".  `order` 1 stores a page
+ *                     as [head][token][dim]:
+ *                       POOL[l][c][g][t][h][d] at in-page element ((h*T + t)*D + d)
+ *                     The transfer buffer and the CoW append block stay NHD.
  *   lower-tier layout BASELINE.json:configs[0]: page-first [page][layer][K,V][token][head][dim],
  *                     dense.  (reading R1.)
  *   O-pack            PAPER.md:L214 (sec. 4.1.2) "copy and convert pages directly into
@@ -50,6 +55,14 @@ static inline void kvo_zero_elem(uint8_t *dst, uint32_t e) {
   for (uint32_t b = 0; b < e; ++b) dst[b] = 0;
 }
 
+/* In-page element index of POOL[..][t][h][d] (T = page size of THAT pool).
+ *   order 0, NHD: (t*H + h)*D + d        order 1, HND: (h*T + t)*D + d */
+static inline uint64_t kvo_in_page(int order, uint64_t t, uint64_t T, uint64_t h, uint64_t H,
+                                   uint64_t d, uint64_t D) {
+  if (order == 0) return (t * H + h) * D + d;
+  return (h * T + t) * D + d;
+}
+
 static int kvo_ids_in_range(const int32_t *ids, uint64_t n, uint32_t num_pages) {
   for (uint64_t i = 0; i < n; ++i)
     if (ids[i] < 0 || (uint32_t)ids[i] >= num_pages) return 0;
@@ -69,10 +82,10 @@ static inline uint64_t kvo_buf_index(int layout, uint64_t p, uint64_t n, uint64_
 
 /* O-pack: buf[p][l][c][t][h][d] = POOL[l][c][ids[p]][t][h][d] */
 int kvo_pack(const void *const *base, uint32_t L, uint32_t C, uint32_t num_pages, uint32_t T,
-             uint32_t H, uint32_t D, uint32_t e, uint64_t page_stride_bytes, const int32_t *ids,
-             uint64_t n, int layout, void *buf, int threads) {
+             uint32_t H, uint32_t D, uint32_t e, uint64_t page_stride_bytes, int order,
+             const int32_t *ids, uint64_t n, int layout, void *buf, int threads) {
   if (!base || (!ids && n) || (!buf && n) || !L || !C || !T || !H || !D || !e) return KVO_ERR_ARG;
-  if (layout != 0 && layout != 1) return KVO_ERR_ARG;
+  if ((layout != 0 && layout != 1) || (order != 0 && order != 1)) return KVO_ERR_ARG;
   if (!kvo_ids_in_range(ids, n, num_pages)) return KVO_ERR_PAGE_RANGE;
   uint8_t *out = (uint8_t *)buf;
 #pragma omp parallel for num_threads(threads) if (threads > 1) schedule(static)
@@ -83,7 +96,8 @@ int kvo_pack(const void *const *base, uint32_t L, uint32_t C, uint32_t num_pages
           for (uint64_t h = 0; h < H; ++h)
             for (uint64_t d = 0; d < D; ++d) {
               const uint8_t *src = (const uint8_t *)base[l * C + c] +
-                                   (uint64_t)ids[p] * page_stride_bytes + ((t * H + h) * D + d) * e;
+                                   (uint64_t)ids[p] * page_stride_bytes +
+                                   kvo_in_page(order, t, T, h, H, d, D) * e;
               uint64_t o = kvo_buf_index(layout, (uint64_t)p, n, l, L, c, C, t, T, h, H, d, D);
               kvo_copy_elem(out + o * e, src, e);
             }
@@ -99,10 +113,10 @@ int kvo_pack(const void *const *base, uint32_t L, uint32_t C, uint32_t num_pages
  */
 int kvo_unpack(const void *src, const int32_t *dst_ids, uint64_t n_dst, void *const *base,
                uint32_t L, uint32_t C, uint32_t num_pages, uint32_t H, uint32_t D, uint32_t e,
-               uint64_t page_stride_bytes, uint32_t Ts, uint32_t Td, uint64_t n_tokens, int layout,
-               int threads) {
+               uint64_t page_stride_bytes, int order, uint32_t Ts, uint32_t Td, uint64_t n_tokens,
+               int layout, int threads) {
   if (!base || !L || !C || !Ts || !Td || !H || !D || !e) return KVO_ERR_ARG;
-  if (layout != 0 && layout != 1) return KVO_ERR_ARG;
+  if ((layout != 0 && layout != 1) || (order != 0 && order != 1)) return KVO_ERR_ARG;
   if (n_dst != (n_tokens + Td - 1) / Td) return KVO_ERR_ARG;
   if ((!src || !dst_ids) && n_dst) return KVO_ERR_ARG;
   if (!kvo_ids_in_range(dst_ids, n_dst, num_pages)) return KVO_ERR_PAGE_RANGE;
@@ -117,7 +131,8 @@ int kvo_unpack(const void *src, const int32_t *dst_ids, uint64_t n_dst, void *co
             for (uint64_t d = 0; d < D; ++d) {
               uint64_t j = (uint64_t)q * Td + u; /* sequence position, order preserved */
               uint8_t *dst = (uint8_t *)base[l * C + c] +
-                             (uint64_t)dst_ids[q] * page_stride_bytes + ((u * H + h) * D + d) * e;
+                             (uint64_t)dst_ids[q] * page_stride_bytes +
+                             kvo_in_page(order, u, Td, h, H, d, D) * e;
               if (j < n_tokens) {
                 uint64_t o = kvo_buf_index(layout, j / Ts, n_src, l, L, c, C, j % Ts, Ts, h, H, d, D);
                 kvo_copy_elem(dst, in + o * e, e);
@@ -132,7 +147,7 @@ int kvo_unpack(const void *src, const int32_t *dst_ids, uint64_t n_dst, void *co
  * ids[off[r] .. off[r+1]) into its own buffer dsts[r]. */
 int kvo_pack_batched(const void *const *base, uint32_t L, uint32_t C, uint32_t num_pages,
                      uint32_t T, uint32_t H, uint32_t D, uint32_t e, uint64_t page_stride_bytes,
-                     const int32_t *ids, const int64_t *off, uint32_t R, int layout,
+                     int order, const int32_t *ids, const int64_t *off, uint32_t R, int layout,
                      void *const *dsts, int threads) {
   if (R && (!off || !dsts)) return KVO_ERR_ARG;
   for (uint32_t r = 0; r < R; ++r) {
@@ -141,7 +156,7 @@ int kvo_pack_batched(const void *const *base, uint32_t L, uint32_t C, uint32_t n
       return KVO_ERR_PAGE_RANGE;
   }
   for (uint32_t r = 0; r < R; ++r) {
-    int rc = kvo_pack(base, L, C, num_pages, T, H, D, e, page_stride_bytes, ids + off[r],
+    int rc = kvo_pack(base, L, C, num_pages, T, H, D, e, page_stride_bytes, order, ids + off[r],
                       (uint64_t)(off[r + 1] - off[r]), layout, dsts[r], threads);
     if (rc) return rc;
   }
@@ -153,7 +168,7 @@ int kvo_pack_batched(const void *const *base, uint32_t L, uint32_t C, uint32_t n
 int kvo_unpack_batched(const void *const *srcs, const int32_t *dst_ids, const int64_t *off,
                        const uint64_t *n_tokens, uint32_t R, void *const *base, uint32_t L,
                        uint32_t C, uint32_t num_pages, uint32_t H, uint32_t D, uint32_t e,
-                       uint64_t page_stride_bytes, uint32_t Ts, uint32_t Td, int layout,
+                       uint64_t page_stride_bytes, int order, uint32_t Ts, uint32_t Td, int layout,
                        int threads) {
   if (R && (!off || !srcs || !n_tokens)) return KVO_ERR_ARG;
   if (!Td) return KVO_ERR_ARG;
@@ -165,7 +180,8 @@ int kvo_unpack_batched(const void *const *srcs, const int32_t *dst_ids, const in
   }
   for (uint32_t r = 0; r < R; ++r) {
     int rc = kvo_unpack(srcs[r], dst_ids + off[r], (uint64_t)(off[r + 1] - off[r]), base, L, C,
-                        num_pages, H, D, e, page_stride_bytes, Ts, Td, n_tokens[r], layout, threads);
+                        num_pages, H, D, e, page_stride_bytes, order, Ts, Td, n_tokens[r], layout,
+                        threads);
     if (rc) return rc;
   }
   return KVO_OK;
@@ -180,9 +196,9 @@ int kvo_unpack_batched(const void *const *srcs, const int32_t *dst_ids, const in
  * `app` is dense [layer][K,V][token][head][dim] with n_app tokens.  OLD page is never written.
  */
 int kvo_cow_append(void *const *base, uint32_t L, uint32_t C, uint32_t num_pages, uint32_t T,
-                   uint32_t H, uint32_t D, uint32_t e, uint64_t page_stride_bytes, int32_t old_id,
-                   int32_t new_id, uint32_t n_old, const void *app, uint32_t n_app) {
-  if (!base || !L || !C || !T || !H || !D || !e) return KVO_ERR_ARG;
+                   uint32_t H, uint32_t D, uint32_t e, uint64_t page_stride_bytes, int order,
+                   int32_t old_id, int32_t new_id, uint32_t n_old, const void *app, uint32_t n_app) {
+  if (!base || !L || !C || !T || !H || !D || !e || (order != 0 && order != 1)) return KVO_ERR_ARG;
   if ((uint64_t)n_old + n_app > T || old_id == new_id) return KVO_ERR_ARG;
   if (old_id < 0 || new_id < 0 || (uint32_t)old_id >= num_pages || (uint32_t)new_id >= num_pages)
     return KVO_ERR_PAGE_RANGE;
@@ -193,9 +209,10 @@ int kvo_cow_append(void *const *base, uint32_t L, uint32_t C, uint32_t num_pages
         for (uint64_t h = 0; h < H; ++h)
           for (uint64_t d = 0; d < D; ++d) {
             uint8_t *slab = (uint8_t *)base[l * C + c];
-            uint8_t *dst = slab + (uint64_t)new_id * page_stride_bytes + ((t * H + h) * D + d) * e;
+            uint64_t in_page = kvo_in_page(order, t, T, h, H, d, D) * e;
+            uint8_t *dst = slab + (uint64_t)new_id * page_stride_bytes + in_page;
             if (t < n_old) {
-              kvo_copy_elem(dst, slab + (uint64_t)old_id * page_stride_bytes + ((t * H + h) * D + d) * e, e);
+              kvo_copy_elem(dst, slab + (uint64_t)old_id * page_stride_bytes + in_page, e);
             } else {
               uint64_t o = ((((l * C + c) * n_app) + (t - n_old)) * H + h) * D + d;
               kvo_copy_elem(dst, (const uint8_t *)app + o * e, e);
@@ -210,7 +227,7 @@ int kvo_cow_append(void *const *base, uint32_t L, uint32_t C, uint32_t num_pages
  * new_ids must be distinct and must not appear among old_ids (caller checks, like unpack). */
 int kvo_cow_append_batched(void *const *base, uint32_t L, uint32_t C, uint32_t num_pages,
                            uint32_t T, uint32_t H, uint32_t D, uint32_t e,
-                           uint64_t page_stride_bytes, const int32_t *old_ids,
+                           uint64_t page_stride_bytes, int order, const int32_t *old_ids,
                            const int32_t *new_ids, const uint32_t *n_old, const uint32_t *n_app,
                            const void *const *apps, uint32_t S) {
   if (S && (!old_ids || !new_ids || !n_old || !n_app || !apps)) return KVO_ERR_ARG;
@@ -222,7 +239,7 @@ int kvo_cow_append_batched(void *const *base, uint32_t L, uint32_t C, uint32_t n
     if (!apps[s] && n_app[s]) return KVO_ERR_ARG;
   }
   for (uint32_t s = 0; s < S; ++s) {
-    int rc = kvo_cow_append(base, L, C, num_pages, T, H, D, e, page_stride_bytes, old_ids[s],
+    int rc = kvo_cow_append(base, L, C, num_pages, T, H, D, e, page_stride_bytes, order, old_ids[s],
                             new_ids[s], n_old[s], apps[s], n_app[s]);
     if (rc) return rc;
   }
@@ -238,11 +255,12 @@ int kvo_cow_append_batched(void *const *base, uint32_t L, uint32_t C, uint32_t n
  * Source and destination pools have the same L, C, H, D, e; page sizes Ts / Td, page counts and
  * strides are their own.  Nothing else in the destination pool is written; SRC is never written. */
 int kvo_repage(const void *const *src_base, uint32_t src_num_pages, uint64_t src_stride_bytes,
-               uint32_t Ts, const int32_t *src_ids, uint64_t n_src, void *const *dst_base,
-               uint32_t dst_num_pages, uint64_t dst_stride_bytes, uint32_t Td,
-               const int32_t *dst_ids, uint64_t n_dst, uint32_t L, uint32_t C, uint32_t H,
-               uint32_t D, uint32_t e, uint64_t n_tokens, int threads) {
+               int src_order, uint32_t Ts, const int32_t *src_ids, uint64_t n_src,
+               void *const *dst_base, uint32_t dst_num_pages, uint64_t dst_stride_bytes,
+               int dst_order, uint32_t Td, const int32_t *dst_ids, uint64_t n_dst, uint32_t L,
+               uint32_t C, uint32_t H, uint32_t D, uint32_t e, uint64_t n_tokens, int threads) {
   if (!src_base || !dst_base || !L || !C || !Ts || !Td || !H || !D || !e) return KVO_ERR_ARG;
+  if ((src_order != 0 && src_order != 1) || (dst_order != 0 && dst_order != 1)) return KVO_ERR_ARG;
   if (n_src != (n_tokens + Ts - 1) / Ts || n_dst != (n_tokens + Td - 1) / Td) return KVO_ERR_ARG;
   if ((!src_ids || !dst_ids) && n_tokens) return KVO_ERR_ARG;
   if (!kvo_ids_in_range(src_ids, n_src, src_num_pages)) return KVO_ERR_PAGE_RANGE;
@@ -256,11 +274,12 @@ int kvo_repage(const void *const *src_base, uint32_t src_num_pages, uint64_t src
             for (uint64_t d = 0; d < D; ++d) {
               uint64_t j = (uint64_t)q * Td + u; /* sequence position, order preserved */
               uint8_t *dst = (uint8_t *)dst_base[l * C + c] +
-                             (uint64_t)dst_ids[q] * dst_stride_bytes + ((u * H + h) * D + d) * e;
+                             (uint64_t)dst_ids[q] * dst_stride_bytes +
+                             kvo_in_page(dst_order, u, Td, h, H, d, D) * e;
               if (j < n_tokens) {
                 const uint8_t *src = (const uint8_t *)src_base[l * C + c] +
                                      (uint64_t)src_ids[j / Ts] * src_stride_bytes +
-                                     (((j % Ts) * H + h) * D + d) * e;
+                                     kvo_in_page(src_order, j % Ts, Ts, h, H, d, D) * e;
                 kvo_copy_elem(dst, src, e);
               } else {
                 kvo_zero_elem(dst, e);
@@ -272,9 +291,10 @@ int kvo_repage(const void *const *src_base, uint32_t src_num_pages, uint64_t src
 /* Batched O-repage: request r re-pages src_ids[src_off[r] .. src_off[r+1]) into
  * dst_ids[dst_off[r] .. dst_off[r+1]) with its own n_tokens[r]. */
 int kvo_repage_batched(const void *const *src_base, uint32_t src_num_pages,
-                       uint64_t src_stride_bytes, uint32_t Ts, const int32_t *src_ids,
-                       const int64_t *src_off, void *const *dst_base, uint32_t dst_num_pages,
-                       uint64_t dst_stride_bytes, uint32_t Td, const int32_t *dst_ids,
+                       uint64_t src_stride_bytes, int src_order, uint32_t Ts,
+                       const int32_t *src_ids, const int64_t *src_off, void *const *dst_base,
+                       uint32_t dst_num_pages, uint64_t dst_stride_bytes, int dst_order,
+                       uint32_t Td, const int32_t *dst_ids,
                        const int64_t *dst_off, const uint64_t *n_tokens, uint32_t R, uint32_t L,
                        uint32_t C, uint32_t H, uint32_t D, uint32_t e, int threads) {
   if (R && (!src_off || !dst_off || !n_tokens)) return KVO_ERR_ARG;
@@ -289,9 +309,9 @@ int kvo_repage_batched(const void *const *src_base, uint32_t src_num_pages,
       return KVO_ERR_PAGE_RANGE;
   }
   for (uint32_t r = 0; r < R; ++r) {
-    int rc = kvo_repage(src_base, src_num_pages, src_stride_bytes, Ts, src_ids + src_off[r],
-                        (uint64_t)(src_off[r + 1] - src_off[r]), dst_base, dst_num_pages,
-                        dst_stride_bytes, Td, dst_ids + dst_off[r],
+    int rc = kvo_repage(src_base, src_num_pages, src_stride_bytes, src_order, Ts,
+                        src_ids + src_off[r], (uint64_t)(src_off[r + 1] - src_off[r]), dst_base,
+                        dst_num_pages, dst_stride_bytes, dst_order, Td, dst_ids + dst_off[r],
                         (uint64_t)(dst_off[r + 1] - dst_off[r]), L, C, H, D, e, n_tokens[r], threads);
     if (rc) return rc;
   }

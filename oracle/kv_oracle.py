@@ -34,6 +34,8 @@ _LIB = os.path.join(_HERE, "libkvoracle.so")
 
 PAGE_FIRST = 0
 LAYER_FIRST = 1
+NHD = 0  # in-page order [token][head][dim] ("NHD block stacks")
+HND = 1  # in-page order [head][token][dim]
 
 
 def build(force: bool = False) -> str:
@@ -70,6 +72,7 @@ class HostPool:
     D: int
     e: int
     page_stride_bytes: int
+    order: int = 0  # in-page order: 0 NHD [token][head][dim], 1 HND [head][token][dim]
 
     @property
     def row_bytes(self) -> int:
@@ -80,16 +83,16 @@ class HostPool:
         return self.L * self.C * self.row_bytes
 
     @staticmethod
-    def empty(L, C, num_pages, T, H, D, e, page_stride_bytes=None, fill=0) -> "HostPool":
+    def empty(L, C, num_pages, T, H, D, e, page_stride_bytes=None, fill=0, order=0) -> "HostPool":
         row = T * H * D * e
         stride = row if page_stride_bytes is None else int(page_stride_bytes)
         assert stride >= row
         slabs = [np.full(num_pages * stride, fill, dtype=np.uint8) for _ in range(L * C)]
-        return HostPool(slabs, L, C, num_pages, T, H, D, e, stride)
+        return HostPool(slabs, L, C, num_pages, T, H, D, e, stride, order)
 
     def copy(self) -> "HostPool":
         return HostPool([s.copy() for s in self.slabs], self.L, self.C, self.num_pages, self.T,
-                        self.H, self.D, self.e, self.page_stride_bytes)
+                        self.H, self.D, self.e, self.page_stride_bytes, self.order)
 
     def _ptrs(self):
         arr = (ctypes.c_void_p * (self.L * self.C))()
@@ -131,7 +134,7 @@ def pack(pool: HostPool, ids, layer_count: int | None = None, layout: int = PAGE
     rc = _load().kvo_pack(pool._ptrs(), ctypes.c_uint32(L), ctypes.c_uint32(pool.C),
                           ctypes.c_uint32(pool.num_pages), ctypes.c_uint32(pool.T),
                           ctypes.c_uint32(pool.H), ctypes.c_uint32(pool.D), ctypes.c_uint32(pool.e),
-                          ctypes.c_uint64(pool.page_stride_bytes),
+                          ctypes.c_uint64(pool.page_stride_bytes), ctypes.c_int(pool.order),
                           ids.ctypes.data_as(ctypes.c_void_p), ctypes.c_uint64(n),
                           ctypes.c_int(layout), buf.ctypes.data_as(ctypes.c_void_p),
                           ctypes.c_int(threads))
@@ -155,8 +158,8 @@ def unpack(src: np.ndarray, dst_ids, pool: HostPool, Ts: int, n_tokens: int,
                             pool._ptrs(), ctypes.c_uint32(L), ctypes.c_uint32(pool.C),
                             ctypes.c_uint32(pool.num_pages), ctypes.c_uint32(pool.H),
                             ctypes.c_uint32(pool.D), ctypes.c_uint32(pool.e),
-                            ctypes.c_uint64(pool.page_stride_bytes), ctypes.c_uint32(Ts),
-                            ctypes.c_uint32(pool.T), ctypes.c_uint64(int(n_tokens)),
+                            ctypes.c_uint64(pool.page_stride_bytes), ctypes.c_int(pool.order),
+                            ctypes.c_uint32(Ts), ctypes.c_uint32(pool.T), ctypes.c_uint64(int(n_tokens)),
                             ctypes.c_int(layout), ctypes.c_int(threads))
     _check(rc)
 
@@ -177,7 +180,7 @@ def pack_batched(pool: HostPool, ids, off, layer_count: int | None = None,
                                   ctypes.c_uint32(pool.num_pages), ctypes.c_uint32(pool.T),
                                   ctypes.c_uint32(pool.H), ctypes.c_uint32(pool.D),
                                   ctypes.c_uint32(pool.e), ctypes.c_uint64(pool.page_stride_bytes),
-                                  ids.ctypes.data_as(ctypes.c_void_p),
+                                  ctypes.c_int(pool.order), ids.ctypes.data_as(ctypes.c_void_p),
                                   off.ctypes.data_as(ctypes.c_void_p), ctypes.c_uint32(R),
                                   ctypes.c_int(layout), dsts, ctypes.c_int(threads))
     _check(rc)
@@ -208,8 +211,8 @@ def unpack_batched(srcs: Sequence[np.ndarray], dst_ids, off, n_tokens, pool: Hos
                                     pool._ptrs(), ctypes.c_uint32(L), ctypes.c_uint32(pool.C),
                                     ctypes.c_uint32(pool.num_pages), ctypes.c_uint32(pool.H),
                                     ctypes.c_uint32(pool.D), ctypes.c_uint32(pool.e),
-                                    ctypes.c_uint64(pool.page_stride_bytes), ctypes.c_uint32(Ts),
-                                    ctypes.c_uint32(pool.T), ctypes.c_int(layout),
+                                    ctypes.c_uint64(pool.page_stride_bytes), ctypes.c_int(pool.order),
+                                    ctypes.c_uint32(Ts), ctypes.c_uint32(pool.T), ctypes.c_int(layout),
                                     ctypes.c_int(threads))
     _check(rc)
 
@@ -225,7 +228,7 @@ def cow_append(pool: HostPool, old_id: int, new_id: int, n_old: int, app: np.nda
                                 ctypes.c_uint32(pool.num_pages), ctypes.c_uint32(pool.T),
                                 ctypes.c_uint32(pool.H), ctypes.c_uint32(pool.D),
                                 ctypes.c_uint32(pool.e), ctypes.c_uint64(pool.page_stride_bytes),
-                                ctypes.c_int32(old_id), ctypes.c_int32(new_id),
+                                ctypes.c_int(pool.order), ctypes.c_int32(old_id), ctypes.c_int32(new_id),
                                 ctypes.c_uint32(n_old), app.ctypes.data_as(ctypes.c_void_p),
                                 ctypes.c_uint32(n_app))
     _check(rc)
@@ -256,6 +259,7 @@ def cow_append_batched(pool: HostPool, old_ids, new_ids, n_old, n_app, apps: Seq
                                         ctypes.c_uint32(pool.H), ctypes.c_uint32(pool.D),
                                         ctypes.c_uint32(pool.e),
                                         ctypes.c_uint64(pool.page_stride_bytes),
+                                        ctypes.c_int(pool.order),
                                         old_ids.ctypes.data_as(ctypes.c_void_p),
                                         new_ids.ctypes.data_as(ctypes.c_void_p),
                                         n_old.ctypes.data_as(ctypes.c_void_p),
@@ -277,10 +281,12 @@ def repage(src: HostPool, src_ids, dst: HostPool, dst_ids, n_tokens: int,
     src_ids, dst_ids = _ids(src_ids), _ids(dst_ids)
     _assert_distinct(dst_ids)
     rc = _load().kvo_repage(src._ptrs(), ctypes.c_uint32(src.num_pages),
-                            ctypes.c_uint64(src.page_stride_bytes), ctypes.c_uint32(src.T),
+                            ctypes.c_uint64(src.page_stride_bytes), ctypes.c_int(src.order),
+                            ctypes.c_uint32(src.T),
                             src_ids.ctypes.data_as(ctypes.c_void_p), ctypes.c_uint64(len(src_ids)),
                             dst._ptrs(), ctypes.c_uint32(dst.num_pages),
-                            ctypes.c_uint64(dst.page_stride_bytes), ctypes.c_uint32(dst.T),
+                            ctypes.c_uint64(dst.page_stride_bytes), ctypes.c_int(dst.order),
+                            ctypes.c_uint32(dst.T),
                             dst_ids.ctypes.data_as(ctypes.c_void_p), ctypes.c_uint64(len(dst_ids)),
                             ctypes.c_uint32(L), ctypes.c_uint32(src.C), ctypes.c_uint32(src.H),
                             ctypes.c_uint32(src.D), ctypes.c_uint32(src.e),
@@ -301,11 +307,13 @@ def repage_batched(src: HostPool, src_ids, src_off, dst: HostPool, dst_ids, dst_
     R = len(ntok)
     assert len(src_off) == R + 1 and len(dst_off) == R + 1
     rc = _load().kvo_repage_batched(src._ptrs(), ctypes.c_uint32(src.num_pages),
-                                    ctypes.c_uint64(src.page_stride_bytes), ctypes.c_uint32(src.T),
+                                    ctypes.c_uint64(src.page_stride_bytes), ctypes.c_int(src.order),
+                                    ctypes.c_uint32(src.T),
                                     src_ids.ctypes.data_as(ctypes.c_void_p),
                                     src_off.ctypes.data_as(ctypes.c_void_p), dst._ptrs(),
                                     ctypes.c_uint32(dst.num_pages),
-                                    ctypes.c_uint64(dst.page_stride_bytes), ctypes.c_uint32(dst.T),
+                                    ctypes.c_uint64(dst.page_stride_bytes), ctypes.c_int(dst.order),
+                                    ctypes.c_uint32(dst.T),
                                     dst_ids.ctypes.data_as(ctypes.c_void_p),
                                     dst_off.ctypes.data_as(ctypes.c_void_p),
                                     ntok.ctypes.data_as(ctypes.c_void_p), ctypes.c_uint32(R),
@@ -319,8 +327,10 @@ def repage_batched(src: HostPool, src_ids, src_off, dst: HostPool, dst_ids, dst_
 # the definitions as literal Python loops (tiny cases only)
 # ----------------------------------------------------------------------------------------------
 def _pool_off(pool: HostPool, g, t, h, d) -> int:
-    # PAPER.md:L207 region (layer, page_idx, K|V) + NHD in-page order
-    return g * pool.page_stride_bytes + ((t * pool.H + h) * pool.D + d) * pool.e
+    # PAPER.md:L207 region (layer, page_idx, K|V) + in-page order: NHD or HND
+    if pool.order == NHD:
+        return g * pool.page_stride_bytes + ((t * pool.H + h) * pool.D + d) * pool.e
+    return g * pool.page_stride_bytes + ((h * pool.T + t) * pool.D + d) * pool.e
 
 
 def _buf_index(layout, p, n, l, L, c, C, t, T, h, H, d, D) -> int:

@@ -24,28 +24,34 @@ DT = {1: np.uint8, 2: np.uint16, 4: np.uint32}
 # ---------------------------------------------------------------------------------------------
 # helpers: pools as a stacked numpy array A[L,C,P,T,H,D] (dense stride) <-> HostPool
 # ---------------------------------------------------------------------------------------------
-def pool_from_array(A: np.ndarray, pad: int = 0, pad_fill: int = 0xA5) -> ko.HostPool:
+def pool_from_array(A: np.ndarray, pad: int = 0, pad_fill: int = 0xA5, order: int = 0) -> ko.HostPool:
+    """A is the LOGICAL pool A[L,C,P,T,H,D]; order 1 (HND) stores every page as [H][T][D]."""
     L, C, P, T, H, D = A.shape
     e = A.dtype.itemsize
     row = T * H * D * e
     stride = row + pad
+    phys = A if order == 0 else np.ascontiguousarray(A.transpose(0, 1, 2, 4, 3, 5))
     slabs = []
     for l in range(L):
         for c in range(C):
             s = np.full((P, stride), pad_fill, dtype=np.uint8)
-            s[:, :row] = A[l, c].reshape(P, -1).view(np.uint8)
+            s[:, :row] = np.ascontiguousarray(phys[l, c]).reshape(P, -1).view(np.uint8)
             slabs.append(s.reshape(-1))
-    return ko.HostPool(slabs, L, C, P, T, H, D, e, stride)
+    return ko.HostPool(slabs, L, C, P, T, H, D, e, stride, order)
 
 
 def array_from_pool(pool: ko.HostPool) -> np.ndarray:
+    """The LOGICAL pool A[L,C,P,T,H,D], whatever the in-page order."""
     row = pool.row_bytes
     out = np.empty((pool.L, pool.C, pool.num_pages, pool.T, pool.H, pool.D), dtype=DT[pool.e])
     for l in range(pool.L):
         for c in range(pool.C):
             s = pool.slabs[l * pool.C + c].reshape(pool.num_pages, pool.page_stride_bytes)[:, :row]
-            out[l, c] = np.ascontiguousarray(s).view(DT[pool.e]).reshape(pool.num_pages, pool.T,
-                                                                        pool.H, pool.D)
+            v = np.ascontiguousarray(s).view(DT[pool.e])
+            if pool.order == 0:
+                out[l, c] = v.reshape(pool.num_pages, pool.T, pool.H, pool.D)
+            else:
+                out[l, c] = v.reshape(pool.num_pages, pool.H, pool.T, pool.D).transpose(0, 2, 1, 3)
     return out
 
 
@@ -549,3 +555,88 @@ def test_repage_equals_pack_then_unpack_and_batched_equals_per_request():
         ko.repage(src, [64], d1, [1], n_tokens=4)
     with pytest.raises(ValueError):
         ko.repage(src, [1], pool_from_array(rand_array(rng, L, C, 4, Td, H, D + 1, e)), [1], n_tokens=4)
+
+
+# ---------------------------------------------------------------------------------------------
+# 7. HND pools: in-page order [head][token][dim] ("including")
+# ---------------------------------------------------------------------------------------------
+def w5_pool():
+    """Slab c is the word sequence 1000*c + i, i = physical word index; pages are HND."""
+    L, C, P, T, H, D = 1, 2, 3, 2, 2, 2
+    slabs = [(1000 * c + np.arange(P * T * H * D)).astype(np.uint16).view(np.uint8) for c in range(C)]
+    return ko.HostPool(slabs, L, C, P, T, H, D, 2, T * H * D * 2, ko.HND)
+
+
+@pytest.mark.parametrize("impl", IMPLS)
+def test_W5_hnd_pool_hand_computed(impl, golden):
+    pack, unpack = IMPLS[impl]
+    buf = pack(w5_pool(), [2, 0])
+    assert buf.view(np.uint16).tolist() == golden("W5_hnd_pack.txt")
+    # the inverse: unpacking that buffer into pages [1, 2] of a zeroed HND pool puts page 2's
+    # physical words into page 1 and page 0's into page 2
+    dst = w5_pool()
+    for s in dst.slabs:
+        s[:] = 0
+    unpack(buf, [1, 2], dst, Ts=2, n_tokens=4)
+    for c in range(2):
+        w = dst.slabs[c].view(np.uint16)
+        assert w[:8].tolist() == [0] * 8
+        assert w[8:16].tolist() == [1000 * c + 16 + i for i in range(8)]
+        assert w[16:24].tolist() == [1000 * c + i for i in range(8)]
+
+
+@pytest.mark.parametrize("shape", SHAPES)
+@pytest.mark.parametrize("pad", [0, 8])
+def test_hnd_pack_unpack_are_numpy_take_transpose(shape, pad):
+    L, C, P, T, H, D, e = shape
+    rng = np.random.default_rng(31)
+    A = rand_array(rng, L, C, P, T, H, D, e)
+    pool = pool_from_array(A, pad=pad, order=ko.HND)
+    ids = rng.permutation(P)[:max(1, P // 2)]
+    want = np.take(A, ids, axis=2).transpose(2, 0, 1, 3, 4, 5).reshape(-1)
+    for f in (ko.pack, ko.pack_py) if P * T * H * D <= 4096 else (ko.pack,):
+        assert np.array_equal(f(pool, ids).view(DT[e]), want)
+    # unpack into an HND pool == fancy-index assignment on the logical array
+    B0 = rand_array(rng, L, C, P, T, H, D, e)
+    dst_ids = rng.permutation(P)[:len(ids)]
+    dst = pool_from_array(B0, pad=pad, order=ko.HND)
+    ko.unpack(want.view(np.uint8), dst_ids, dst, Ts=T, n_tokens=len(ids) * T)
+    wantB = B0.copy()
+    wantB[:, :, dst_ids] = np.take(A, ids, axis=2)
+    assert np.array_equal(array_from_pool(dst), wantB)
+    for s in dst.slabs:
+        assert np.all(s.reshape(P, -1)[:, T * H * D * e:] == 0xA5)
+
+
+@pytest.mark.parametrize("so,do", [(0, 1), (1, 0), (1, 1)])
+@pytest.mark.parametrize("Ts,Td,ntok", [(4, 16, 61), (16, 4, 64), (3, 5, 31)])
+def test_hnd_repage_and_cow(so, do, Ts, Td, ntok):
+    rng = np.random.default_rng(37)
+    L, C, H, D, e = 2, 2, 3, 4, 2
+    n_src, n_dst = -(-ntok // Ts), -(-ntok // Td)
+    A = rand_array(rng, L, C, n_src + 5, Ts, H, D, e)
+    B0 = rand_array(rng, L, C, n_dst + 4, Td, H, D, e)
+    src_ids = rng.permutation(n_src + 5)[:n_src]
+    dst_ids = rng.permutation(n_dst + 4)[:n_dst]
+    src, dst = pool_from_array(A, pad=8, order=so), pool_from_array(B0, order=do)
+    ko.repage(src, src_ids, dst, dst_ids, n_tokens=ntok)
+    stream = np.take(A, src_ids, axis=2).reshape(L, C, n_src * Ts, H, D)[:, :, :ntok]
+    padded = np.zeros((L, C, n_dst * Td, H, D), dtype=A.dtype)
+    padded[:, :, :ntok] = stream
+    want = B0.copy()
+    want[:, :, dst_ids] = padded.reshape(L, C, n_dst, Td, H, D)
+    assert np.array_equal(array_from_pool(dst), want)
+    # the same through the NHD buffer
+    dst2 = pool_from_array(B0, order=do)
+    ko.unpack(ko.pack(src, src_ids), dst_ids, dst2, Ts=Ts, n_tokens=ntok)
+    assert np.array_equal(array_from_pool(dst2), want)
+    # copy-on-write append in an HND pool: slice assignment on the logical array
+    if Td >= 4:
+        pool = pool_from_array(B0, order=ko.HND)
+        n_old, n_app = 1, Td - 2
+        app = rng.integers(0, 65536, size=(L, C, n_app, H, D), dtype=np.uint64).astype(np.uint16)
+        ko.cow_append(pool, 0, 1, n_old, app, n_app)
+        w = B0.copy()
+        w[:, :, 1, :n_old] = B0[:, :, 0, :n_old]
+        w[:, :, 1, n_old:n_old + n_app] = app
+        assert np.array_equal(array_from_pool(pool), w)
