@@ -51,10 +51,15 @@ typedef void *kv_stream_t;
 
 /* One paged KV parameter: outer dim = layers, slice dim = K/V, a page size,
  * a shape and an element width.  Region (l, g, c) starts at base[l*kv_count + c] +
- * g*page_stride_bytes and holds page_size*num_heads*head_dim elements in NHD order
- * [token][head][dim] ("NHD block stacks").  Separate K and V allocations, one fused
- * allocation per layer, or one allocation for everything are all expressed by the base pointers
- * and the stride; bytes between the dense row and the stride are never read or written. */
+ * g*page_stride_bytes and holds page_size*num_heads*head_dim elements, in-page order `order`:
+ * KV_ORDER_NHD [token][head][dim] ("NHD block stacks") or KV_ORDER_HND
+ * [head][token][dim] ("compute-oriented layouts, INCLUDING NHD block stacks" -- NHD
+ * is one of several).  The transfer buffer and the copy-on-write append block
+ * are always NHD, so a transfer to or from an HND pool is a real transposition of [token] and [head].
+ * Separate K and V allocations, one fused allocation per layer, or one allocation for everything are
+ * all expressed by the base pointers and the stride; bytes between the dense row and the stride are
+ * never read or written. */
+typedef enum kv_order { KV_ORDER_NHD = 0, KV_ORDER_HND = 1 } kv_order;
 typedef struct kv_pool_desc {
   void *const *base;          /* HOST array of layer_count*kv_count DEVICE pointers, [layer][kv], kv 0=K 1=V */
   uint32_t layer_count;       /* layers in the descriptor */
@@ -64,7 +69,7 @@ typedef struct kv_pool_desc {
   uint32_t num_heads;         /* KV heads held by THIS rank (a TP head partition has fewer) */
   uint32_t head_dim;
   uint32_t elem_bytes;        /* 1, 2, 4 or 8; bf16 = 2 */
-  uint32_t reserved;          /* must be 0 */
+  uint32_t order;             /* kv_order: in-page order of THIS pool (0 = NHD) */
   uint64_t page_stride_bytes; /* >= page_size*num_heads*head_dim*elem_bytes, multiple of elem_bytes */
 } kv_pool_desc;
 
@@ -91,7 +96,7 @@ typedef enum kv_status {
   KV_ERR_ALIGN = -6,      /* a pointer or stride is not elem_bytes-aligned */
   KV_ERR_CUDA = -7,       /* a CUDA call failed; see kv_last_cuda_error() */
   KV_ERR_HOST_MEM = -8,   /* host buffer of an offload/reload is not pinned (page-locked) memory */
-  KV_ERR_DESC = -9,       /* malformed kv_pool_desc (zero dimension, bad elem_bytes, stride < row, layer_count too large) */
+  KV_ERR_DESC = -9,       /* malformed kv_pool_desc (zero dimension, bad elem_bytes or order, stride < row, layer_count too large) */
   KV_ERR_NO_DEVICE = -10, /* planning-only ctx (device < 0): arguments were valid, nothing was launched */
   KV_ERR_CAPTURE = -11,   /* `stream` is capturing a CUDA graph and this call is not replayable: its tables exceed
                              the kernel parameters (~31 KiB: about 7,500 page ids), the element-wise fallback kernel

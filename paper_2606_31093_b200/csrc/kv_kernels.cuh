@@ -69,6 +69,15 @@ struct Job {
   uint32_t first_batch;       // B0: static items per warp before claiming starts
   uint32_t src_num_pages;     // dir 2: pages of the SOURCE pool (range check of device-resident ids)
   uint64_t src_page_stride;   // dir 2: source pool bytes between pages; its slab bases are bases[LC..2LC)
+  // transposing transfers (an HND pool on either side; kTrans kernels only).  A side is either
+  // contiguous in the item's NHD-linear order or "strided": row r = t*H + h of the chunk (one
+  // head_dim row of `drow` bytes) sits at side_base + t*ts + h*hs.
+  uint32_t drow;              // head_dim * elem_bytes
+  uint32_t H;                 // num_heads
+  uint32_t pool_hnd;          // the (destination) pool is HND
+  uint32_t src_hnd;           // dir 2: the source pool is HND
+  uint64_t p_ts, p_hs;        // strides of the pool side when it is HND (ts = drow, hs = Tpool*drow)
+  uint64_t q_ts, q_hs;        // dir 2: strides of the source pool when it is HND
 };
 
 // The lookup tables of a launch: slab bases, page ids, pieces.  They live either in device memory
@@ -108,10 +117,15 @@ struct Item {
   uint64_t src, dst;
   uint32_t bytes;  // bytes written at dst
   uint32_t valid;  // first `valid` bytes come from src, the rest is zero fill
+  // kTrans only: bit 0 = src strided, bit 1 = dst strided.  A strided side's address is the base of
+  // the CHUNK (token 0, head 0) and the item covers rows [r0, r0 + bytes/drow) of it; a contiguous
+  // side's address already points at the item's first byte.
+  uint32_t mode;
+  uint32_t r0;
 };
 
 // flat item -> (piece, chunk k, layer/kv, sub) -> addresses.
-template <bool kGlobal>
+template <bool kGlobal, bool kTrans = false>
 __device__ __forceinline__ Item decode(const Job &j, const Tables &tb, uint64_t item) {
   uint32_t r = 0;
   if (j.n_pieces > 1) {  // largest r with pieces[r].item_begin <= item
@@ -136,12 +150,19 @@ __device__ __forceinline__ Item decode(const Job &j, const Tables &tb, uint64_t 
     const uint64_t old_pg = slab + (id_begin & 0xffffffffull) * j.page_stride;
     const uint64_t new_pg = slab + (id_begin >> 32) * j.page_stride;
     Item it;
+    it.mode = 0; it.r0 = 0;
     if (k < s0) {
       const uint32_t o = k * j.sub_bytes;
       it.src = old_pg + o; it.dst = new_pg + o; it.bytes = min(j.sub_bytes, b_old - o);
+      if (kTrans && j.pool_hnd) {  // rows of the first n_old tokens, same place in both pages
+        it.src = old_pg; it.dst = new_pg; it.mode = 3; it.r0 = o / j.drow;
+      }
     } else {
       const uint32_t o = (k - s0) * j.sub_bytes;
       it.src = buf + (uint64_t)lc * b_app + o; it.dst = new_pg + b_old + o; it.bytes = min(j.sub_bytes, b_app - o);
+      if (kTrans && j.pool_hnd) {  // NHD append block -> token slots n_old.. of every head's run
+        it.dst = new_pg + (uint64_t)n_old * j.p_ts; it.mode = 2; it.r0 = o / j.drow;
+      }
     }
     it.valid = it.bytes;
     return it;
@@ -152,6 +173,7 @@ __device__ __forceinline__ Item decode(const Job &j, const Tables &tb, uint64_t 
   const uint32_t bp = k / j.cpp_buf, bk = k - bp * j.cpp_buf;
   const uint64_t sub_off = (uint64_t)sub * j.sub_bytes;
   Item it;
+  it.mode = 0; it.r0 = 0;
   it.bytes = min(j.sub_bytes, j.chunk_bytes - (uint32_t)sub_off);
   // caller-supplied device ids are global memory even when the other tables are inline
   const int32_t id = (kGlobal || j.ids) ? __ldg(tb.ids + id_begin + pp) : tb.ids[id_begin + pp];
@@ -160,8 +182,10 @@ __device__ __forceinline__ Item decode(const Job &j, const Tables &tb, uint64_t 
     it.src = it.dst = 0; it.bytes = it.valid = 0;
     return it;
   }
-  const uint64_t paddr = ldt<kGlobal>(tb.bases + lc) + (uint64_t)id * j.page_stride +
-                         (uint64_t)pk * j.chunk_bytes + sub_off;
+  uint64_t paddr = ldt<kGlobal>(tb.bases + lc) + (uint64_t)id * j.page_stride;
+  uint32_t pmode = 0, bmode = 0;  // is the pool / buffer side strided?
+  if (kTrans && j.pool_hnd) { paddr += (uint64_t)pk * j.g * j.p_ts; pmode = 1; }
+  else paddr += (uint64_t)pk * j.chunk_bytes + sub_off;
   const uint64_t tok0 = (uint64_t)k * j.g;
   const uint64_t vt = n_tokens > tok0 ? min(n_tokens - tok0, (uint64_t)j.g) : 0;
   uint64_t baddr;
@@ -174,8 +198,9 @@ __device__ __forceinline__ Item decode(const Job &j, const Tables &tb, uint64_t 
       it.src = it.dst = 0; it.bytes = it.valid = 0;
       return it;
     }
-    baddr = ldt<kGlobal>(tb.bases + j.LC + lc) + (uint64_t)sid * j.src_page_stride +
-            (uint64_t)bk * j.chunk_bytes + sub_off;
+    baddr = ldt<kGlobal>(tb.bases + j.LC + lc) + (uint64_t)sid * j.src_page_stride;
+    if (kTrans && j.src_hnd) { baddr += (uint64_t)bk * j.g * j.q_ts; bmode = 1; }
+    else baddr += (uint64_t)bk * j.chunk_bytes + sub_off;
   } else {
     baddr = buf + (uint64_t)bk * j.chunk_bytes + sub_off;
     if (j.layout == 0) baddr += (uint64_t)bp * j.buf_page_bytes + (uint64_t)lc * j.buf_row_bytes;
@@ -184,7 +209,21 @@ __device__ __forceinline__ Item decode(const Job &j, const Tables &tb, uint64_t 
   const uint64_t vbytes = vt * j.tokrow;
   it.valid = vbytes > sub_off ? (uint32_t)min(vbytes - sub_off, (uint64_t)it.bytes) : 0u;
   if (j.dir == 0) { it.src = paddr; it.dst = baddr; } else { it.src = baddr; it.dst = paddr; }
+  if (kTrans) {
+    it.mode = j.dir == 0 ? (pmode | bmode << 1) : (bmode | pmode << 1);
+    it.r0 = (uint32_t)(sub_off / j.drow);
+  }
   return it;
+}
+
+// Strides of a strided side (kTrans).  Source side: the pool for pack and copy-on-write, the source
+// pool for pool -> pool; destination side: always the pool.
+struct Strides { uint64_t s_ts, s_hs, d_ts, d_hs; };
+__device__ __forceinline__ Strides strides_of(const Job &j) {
+  Strides s;
+  s.s_ts = j.dir == 2 ? j.q_ts : j.p_ts; s.s_hs = j.dir == 2 ? j.q_hs : j.p_hs;
+  s.d_ts = j.p_ts; s.d_hs = j.p_hs;
+  return s;
 }
 
 // ---------------------------------------------------------------------------------------------
@@ -233,6 +272,40 @@ __device__ __forceinline__ void bulk_wait_read() {
   asm volatile("cp.async.bulk.wait_group.read %0;" ::"n"(N) : "memory");
 }
 __device__ __forceinline__ void bulk_wait_all() { asm volatile("cp.async.bulk.wait_group 0;" ::: "memory"); }
+// 16-byte asynchronous global -> shared copy (SASS LDGSTS), L2 only; completion is reported to an
+// mbarrier by cp_async_arrive (the arrival is pre-counted in the barrier's init count: .noinc).
+__device__ __forceinline__ void cp_async16(uint32_t dst_smem, uint64_t src) {
+  asm volatile("cp.async.cg.shared.global [%0], [%1], 16;" ::"r"(dst_smem), "l"(src) : "memory");
+}
+__device__ __forceinline__ void cp_async_arrive(uint32_t bar) {
+  asm volatile("cp.async.mbarrier.arrive.noinc.shared::cta.b64 [%0];" ::"r"(bar) : "memory");
+}
+__device__ __forceinline__ uint4 lds128(uint32_t addr) {
+  uint4 r;
+  asm volatile("ld.shared.v4.u32 {%0,%1,%2,%3}, [%4];" : "=r"(r.x), "=r"(r.y), "=r"(r.z), "=r"(r.w) : "r"(addr));
+  return r;
+}
+
+__device__ __forceinline__ uint4 ld_stream(const uint4 *p) {
+  uint4 r;
+  asm volatile("ld.global.nc.L1::no_allocate.v4.u32 {%0,%1,%2,%3}, [%4];"
+               : "=r"(r.x), "=r"(r.y), "=r"(r.z), "=r"(r.w) : "l"(p));
+  return r;
+}
+__device__ __forceinline__ void st_stream(uint4 *p, const uint4 &v) {
+  asm volatile("st.global.L1::no_allocate.v4.u32 [%0], {%1,%2,%3,%4};"
+               ::"l"(p), "r"(v.x), "r"(v.y), "r"(v.z), "r"(v.w) : "memory");
+}
+
+// Address of the u-th unit (U bytes) of a kTrans item on one side.
+template <uint32_t U>
+__device__ __forceinline__ uint64_t trans_addr(uint64_t base, bool strided, uint32_t r0, uint32_t u,
+                                               uint32_t upr, uint32_t H, uint64_t ts, uint64_t hs) {
+  if (!strided) return base + (uint64_t)u * U;
+  const uint32_t rr = u / upr, dd = u - rr * upr;
+  const uint32_t row = r0 + rr, t = row / H, h = row - t * H;
+  return base + t * ts + h * hs + (uint64_t)dd * U;
+}
 
 constexpr int kMaxWarps = 8;
 constexpr int kMaxStages = 16;
@@ -240,6 +313,7 @@ constexpr int kMaxStages = 16;
 struct StageMeta {
   uint64_t dst;
   uint32_t bytes, valid;
+  uint32_t mode, r0;  // kTrans only
 };
 
 // ---------------------------------------------------------------------------------------------
@@ -250,7 +324,15 @@ struct StageMeta {
 // so K - lag loads and lag stores are in flight per warp.  Dynamic shared memory:
 //   [zero region: zero_bytes][warp 0 stages][warp 1 stages]...   all 128-byte aligned.
 // ---------------------------------------------------------------------------------------------
-template <int N>
+//
+// kTrans (an HND pool on either side): a stage holds the item in NHD-linear order and every lane of
+// the warp works.  A contiguous side moves it with one bulk copy as above.  A strided SOURCE is
+// gathered row by row with 16-byte cp.async (SASS LDGSTS) by all 32 lanes, each lane's arrival on the
+// stage's mbarrier (count 32) firing when its own copies have landed; the stage then leaves with one
+// bulk store after a fence.proxy.async.  A strided DESTINATION is written with LDS.128 + STG.128.
+// (Per-row bulk copies of head_dim*elem_bytes = 256 B were measured first: 3.1-4.3 TB/s, bound by the
+// rate at which one SM retires small bulk copies.)
+template <int N, bool kTrans>
 __global__ void __launch_bounds__(kMaxWarps * 32, 1) kv_move_bulk(const __grid_constant__ JobT<N> p) {
   const Job &j = p.j;
   const Tables tb = tables_of(p);
@@ -266,7 +348,7 @@ __global__ void __launch_bounds__(kMaxWarps * 32, 1) kv_move_bulk(const __grid_c
   for (uint32_t o = threadIdx.x * 16; o < j.zero_bytes; o += blockDim.x * 16)
     *reinterpret_cast<uint4 *>(smem + o) = make_uint4(0, 0, 0, 0);
   if (lane == 0)
-    for (uint32_t s = 0; s < K; ++s) mbar_init(smem_u32(&full_bar[warp][s]), 1);
+    for (uint32_t s = 0; s < K; ++s) mbar_init(smem_u32(&full_bar[warp][s]), kTrans ? 32 : 1);
   asm volatile("fence.mbarrier_init.release.cluster;" ::: "memory");
   asm volatile("fence.proxy.async.shared::cta;" ::: "memory");
   __syncthreads();
@@ -336,7 +418,7 @@ __global__ void __launch_bounds__(kMaxWarps * 32, 1) kv_move_bulk(const __grid_c
       if (cnt == 0) {
         exhausted = true;
       } else {
-        if (lane < cnt) mine = decode<N == 0>(j, tb, first_item + lane * stride);
+        if (lane < cnt) mine = decode<N == 0, kTrans>(j, tb, first_item + lane * stride);
         batch_first = n_known;
         n_known += cnt;
       }
@@ -348,6 +430,71 @@ __global__ void __launch_bounds__(kMaxWarps * 32, 1) kv_move_bulk(const __grid_c
     const uint64_t dst = __shfl_sync(0xffffffffu, mine.dst, sel);
     const uint32_t bytes = __shfl_sync(0xffffffffu, mine.bytes, sel);
     const uint32_t valid = __shfl_sync(0xffffffffu, mine.valid, sel);
+    if constexpr (kTrans) {
+      const uint32_t mode = __shfl_sync(0xffffffffu, mine.mode, sel);
+      const uint32_t r0 = __shfl_sync(0xffffffffu, mine.r0, sel);
+      const Strides st = strides_of(j);
+      const uint32_t upr = j.drow >> 4;  // 16-byte units per head_dim row
+      if (it >= depth && it - depth < n_known) {  // ---- store side: item si
+        const uint64_t si = it - depth;
+        const uint32_t s = (uint32_t)(si % K);
+        mbar_wait(smem_u32(&full_bar[warp][s]), (uint32_t)(si / K) & 1);
+        const StageMeta m = meta[warp][s];
+        const uint32_t sbase = stage0 + s * j.stage_bytes;
+        if (m.mode & 2) {  // strided destination: LDS.128 from the stage, STG.128 to the row's place
+          const uint32_t nb = m.bytes >> 4, nv = m.valid >> 4;
+          for (uint32_t u0 = lane; u0 < nb; u0 += 128) {
+            uint4 v[4];
+#pragma unroll
+            for (int q = 0; q < 4; ++q) {
+              const uint32_t u = u0 + 32 * q;
+              v[q] = make_uint4(0, 0, 0, 0);
+              if (u < nv) v[q] = lds128(sbase + (u << 4));
+            }
+#pragma unroll
+            for (int q = 0; q < 4; ++q) {
+              const uint32_t u = u0 + 32 * q;
+              if (u < nb)
+                st_stream(reinterpret_cast<uint4 *>(trans_addr<16>(m.dst, true, m.r0, u, upr, j.H, st.d_ts, st.d_hs)), v[q]);
+            }
+          }
+        } else if (lane == 0) {
+          asm volatile("fence.proxy.async.shared::cta;" ::: "memory");  // rows gathered by cp.async -> bulk store
+          if (m.valid) bulk_s2g(m.dst, sbase, m.valid);
+          for (uint32_t z = m.valid; z < m.bytes; z += j.zero_bytes)
+            bulk_s2g(m.dst + z, zero0, min(j.zero_bytes, m.bytes - z));
+        }
+        bulk_commit();  // every lane, every item: the per-thread group counts stay in step
+      }
+      if (have) {  // ---- load side: item it
+        const uint32_t s = (uint32_t)(it % K);
+        if (it >= K) {
+          if (lag == 1) bulk_wait_read<1>();
+          else if (lag == 2) bulk_wait_read<2>();
+          else bulk_wait_read<3>();
+        }
+        __syncwarp();  // every lane has finished reading this stage (bulk store or LDS)
+        const uint32_t bar = smem_u32(&full_bar[warp][s]);
+        const uint32_t sbase = stage0 + s * j.stage_bytes;
+        if (lane == 0) {
+          StageMeta &m = meta[warp][s];
+          m.dst = dst; m.bytes = bytes; m.valid = valid; m.mode = mode; m.r0 = r0;
+        }
+        if (mode & 1) {  // strided source: 16-byte cp.async (LDGSTS) gathers the rows in NHD order;
+                         // each lane's arrival fires when its own copies have landed
+          const uint32_t nv = valid >> 4;
+          for (uint32_t u = lane; u < nv; u += 32)
+            cp_async16(sbase + (u << 4), trans_addr<16>(src, true, r0, u, upr, j.H, st.s_ts, st.s_hs));
+          cp_async_arrive(bar);
+        } else if (lane == 0 && valid) {
+          mbar_expect_tx(bar, valid);
+          bulk_g2s(sbase, src, valid, bar);
+        } else {
+          mbar_arrive(bar);
+        }
+      }
+      __syncwarp();  // meta[] written by lane 0 is read by every lane `depth` iterations later
+    } else
     if (lane == 0) {
       if (it >= depth && it - depth < n_known) {  // ---- store side: item si
         const uint64_t si = it - depth;
@@ -389,24 +536,13 @@ __global__ void __launch_bounds__(kMaxWarps * 32, 1) kv_move_bulk(const __grid_c
       __threadfence();
     }
   }
-  if (lane == 0) bulk_wait_all();
+  if (lane == 0 || kTrans) bulk_wait_all();
 }
 
 // ---------------------------------------------------------------------------------------------
 // kv_move_vec: one warp per segment, 16-byte streaming loads/stores, UNROLL loads in flight.
 // ---------------------------------------------------------------------------------------------
-__device__ __forceinline__ uint4 ld_stream(const uint4 *p) {
-  uint4 r;
-  asm volatile("ld.global.nc.L1::no_allocate.v4.u32 {%0,%1,%2,%3}, [%4];"
-               : "=r"(r.x), "=r"(r.y), "=r"(r.z), "=r"(r.w) : "l"(p));
-  return r;
-}
-__device__ __forceinline__ void st_stream(uint4 *p, const uint4 &v) {
-  asm volatile("st.global.L1::no_allocate.v4.u32 [%0], {%1,%2,%3,%4};"
-               ::"l"(p), "r"(v.x), "r"(v.y), "r"(v.z), "r"(v.w) : "memory");
-}
-
-template <int UNROLL, int N>
+template <int UNROLL, int N, bool kTrans>
 __global__ void __launch_bounds__(256) kv_move_vec(const __grid_constant__ JobT<N> p) {
   const Job &j = p.j;
   const Tables tb = tables_of(p);
@@ -414,10 +550,36 @@ __global__ void __launch_bounds__(256) kv_move_vec(const __grid_constant__ JobT<
   const uint64_t G = (uint64_t)gridDim.x * (blockDim.x >> 5);
   for (uint64_t item = (uint64_t)blockIdx.x * (blockDim.x >> 5) + (threadIdx.x >> 5);
        item < j.total_items; item += G) {
-    const Item it = decode<N == 0>(j, tb, item);
+    const Item it = decode<N == 0, kTrans>(j, tb, item);
     const uint4 *s = reinterpret_cast<const uint4 *>(it.src);
     uint4 *d = reinterpret_cast<uint4 *>(it.dst);
     const uint32_t nv = it.valid >> 4, nb = it.bytes >> 4;
+    if constexpr (kTrans) {
+      if (it.mode) {  // [token] x [head] transposition in 16-byte units of head_dim rows
+        const Strides st = strides_of(j);
+        const uint32_t upr = j.drow >> 4;
+        for (uint32_t i0 = lane; i0 < nb; i0 += 32 * UNROLL) {
+          uint4 v[UNROLL];
+#pragma unroll
+          for (int u = 0; u < UNROLL; ++u) {
+            const uint32_t i = i0 + 32 * u;
+            v[u] = make_uint4(0, 0, 0, 0);
+            if (i < nv)
+              v[u] = ld_stream(reinterpret_cast<const uint4 *>(
+                  trans_addr<16>(it.src, it.mode & 1, it.r0, i, upr, j.H, st.s_ts, st.s_hs)));
+          }
+#pragma unroll
+          for (int u = 0; u < UNROLL; ++u) {
+            const uint32_t i = i0 + 32 * u;
+            if (i < nb)
+              st_stream(reinterpret_cast<uint4 *>(
+                            trans_addr<16>(it.dst, it.mode & 2, it.r0, i, upr, j.H, st.d_ts, st.d_hs)),
+                        v[u]);
+          }
+        }
+        continue;
+      }
+    }
     uint32_t i = lane;
     for (; i + 32 * (UNROLL - 1) < nv; i += 32 * UNROLL) {
       uint4 v[UNROLL];
@@ -435,7 +597,7 @@ __global__ void __launch_bounds__(256) kv_move_vec(const __grid_constant__ JobT<
 // kv_move_elem: any elem_bytes-aligned pointers; U is the widest unit dividing every address
 // and length of the call (1, 2, 4 or 8 bytes).
 // ---------------------------------------------------------------------------------------------
-template <typename U>
+template <typename U, bool kTrans>
 __global__ void __launch_bounds__(256) kv_move_elem(const __grid_constant__ JobT<0> p) {
   const Job &j = p.j;
   const Tables tb = tables_of(p);
@@ -443,10 +605,25 @@ __global__ void __launch_bounds__(256) kv_move_elem(const __grid_constant__ JobT
   const uint64_t G = (uint64_t)gridDim.x * (blockDim.x >> 5);
   for (uint64_t item = (uint64_t)blockIdx.x * (blockDim.x >> 5) + (threadIdx.x >> 5);
        item < j.total_items; item += G) {
-    const Item it = decode<true>(j, tb, item);
+    const Item it = decode<true, kTrans>(j, tb, item);
     const U *s = reinterpret_cast<const U *>(it.src);
     U *d = reinterpret_cast<U *>(it.dst);
     const uint32_t nv = it.valid / sizeof(U), nb = it.bytes / sizeof(U);
+    if constexpr (kTrans) {
+      if (it.mode) {
+        const Strides st = strides_of(j);
+        const uint32_t upr = j.drow / sizeof(U);
+        for (uint32_t i = lane; i < nb; i += 32) {
+          U v = U(0);
+          if (i < nv)
+            v = *reinterpret_cast<const U *>(
+                trans_addr<sizeof(U)>(it.src, it.mode & 1, it.r0, i, upr, j.H, st.s_ts, st.s_hs));
+          *reinterpret_cast<U *>(
+              trans_addr<sizeof(U)>(it.dst, it.mode & 2, it.r0, i, upr, j.H, st.d_ts, st.d_hs)) = v;
+        }
+        continue;
+      }
+    }
     for (uint32_t i = lane; i < nv; i += 32) d[i] = s[i];
     for (uint32_t i = nv + lane; i < nb; i += 32) d[i] = U(0);
   }

@@ -58,6 +58,9 @@ struct kv_ctx {
   // options
   int kernel = KERNEL_AUTO;
   uint32_t stage_bytes = 16384, stages = 4, warps = 2, lag = 2, max_ctas = 0, host_max_ctas = 0;
+  // bulk geometry of transposing transfers (an HND pool): rows are gathered with 16-byte cp.async by all
+  // lanes, which wants more, shallower issuing warps (measured: 8 x 4 x 4 KiB)
+  uint32_t t_stage_bytes = 4096, t_stages = 4, t_warps = 8;
   uint32_t staging_slots = 2, l2_hint = 0, inline_tables = 1, dynamic = 1;
   uint32_t next_sched = 0;
   size_t chunk_bytes = 0;
@@ -107,6 +110,9 @@ struct Geom {
   uint32_t unit = 16;  // widest power of two dividing every address/length (elem kernel)
   // dir 2 (pool -> pool): the source pool; its bases follow the destination's in the tables
   const kv_pool_desc *src_pool = nullptr;
+  // an HND pool on either side makes the transfer a [token] x [head] transposition (kTrans kernels)
+  bool trans = false;
+  uint32_t drow = 0, H = 0, pool_hnd = 0, src_hnd = 0;
 };
 
 struct Req {          // one request as the caller states it
@@ -120,7 +126,7 @@ struct Req {          // one request as the caller states it
 int check_desc(const kv_pool_desc *p, uint32_t layer_count) {
   if (!p || !p->base) return KV_ERR_NULL;
   if (!p->layer_count || !p->kv_count || !p->num_pages || !p->page_size || !p->num_heads ||
-      !p->head_dim || p->reserved)
+      !p->head_dim || p->order > KV_ORDER_HND)
     return KV_ERR_DESC;
   if (p->elem_bytes != 1 && p->elem_bytes != 2 && p->elem_bytes != 4 && p->elem_bytes != 8)
     return KV_ERR_DESC;
@@ -191,22 +197,37 @@ int make_geom(const kv_ctx *ctx, const kv_pool_desc *p, uint32_t layer_count, ui
     unit = std::min(unit, low_pow2(src_pool->page_stride_bytes));
     for (uint32_t i = 0; i < g.LC; ++i) unit = std::min(unit, low_pow2((uint64_t)(uintptr_t)src_pool->base[i]));
   }
+  g.H = p->num_heads;
+  g.drow = p->head_dim * p->elem_bytes;
+  // With one head, or one token per page, [token][head] and [head][token] are the same bytes.
+  auto is_hnd = [](const kv_pool_desc *q) { return q->order == KV_ORDER_HND && q->num_heads > 1 && q->page_size > 1; };
+  g.pool_hnd = is_hnd(p); g.src_hnd = src_pool && is_hnd(src_pool);
+  g.trans = g.pool_hnd || g.src_hnd;
+  if (g.trans) unit = std::min(unit, low_pow2(g.drow));  // rows are moved one by one
   g.unit = unit;
   int kernel = ctx->kernel;
   if (unit < 16) kernel = KERNEL_ELEM;  // 16-byte paths need 16-byte alignment everywhere
-  else if (kernel == KERNEL_AUTO) kernel = KERNEL_BULK;
-  g.kernel = kernel;
-  uint32_t cap = kernel == KERNEL_BULK ? ctx->stage_bytes : 16384u;
+  else if (kernel == KERNEL_AUTO) {
+    // Measured on B200: a strided DESTINATION is fastest with 16-byte STG from many
+    // warps (vec, 5.5 TB/s); a strided source alone is fastest gathered by cp.async into the bulk ring
+    // and stored with one bulk copy (5.8 TB/s); everything contiguous is the bulk path (6.3 TB/s).
+    const bool dst_strided = g.pool_hnd && dir != 0;
+    kernel = dst_strided ? KERNEL_VEC : KERNEL_BULK;
+  }
+  uint32_t cap = kernel == KERNEL_BULK ? (g.trans ? ctx->t_stage_bytes : ctx->stage_bytes) : 16384u;
   cap = std::max(16u, cap / 16 * 16);
+  if (g.trans && kernel == KERNEL_BULK && g.drow > cap) kernel = KERNEL_VEC;  // a row must fit one stage
+  g.kernel = kernel;
   g.sub_bytes = std::min(g.chunk_bytes, cap);
+  if (g.trans) g.sub_bytes = std::min(g.chunk_bytes, std::max(g.drow, cap / g.drow * g.drow));  // whole rows
   if (kernel == KERNEL_BULK && dir != 3) {
     // Launch-bound calls: with fewer segments than issuing warps most SMs would idle while a few
     // move 16 KiB each; cutting segments down to >= 4 KiB spreads a small transfer over the chip
     // (measured on B200, 1 MiB pack back to back: 6.1 -> 5.0 us per call).
     uint64_t chunks = 0;
     for (const Req &r : reqs) chunks += r.n_ids * (g.Tpool / g.g) * g.LC;
-    const uint64_t lanes = (uint64_t)ctx->sm_count * ctx->warps;
-    while (g.sub_bytes >= 8192 && g.sub_bytes % 32 == 0 &&
+    const uint64_t lanes = (uint64_t)ctx->sm_count * (g.trans ? ctx->t_warps : ctx->warps);
+    while (g.sub_bytes >= 8192 && g.sub_bytes % 32 == 0 && (!g.trans || (g.sub_bytes / 2) % g.drow == 0) &&
            chunks * ((g.chunk_bytes + g.sub_bytes - 1) / g.sub_bytes) * 2 <= lanes)
       g.sub_bytes /= 2;
   }
@@ -295,18 +316,25 @@ constexpr int kInlineSmall = 3840;   // whole parameter block stays under the cl
 constexpr int kInlineLarge = 31744;  // CUDA 12.1+ large kernel parameters (<= 32,764 B)
 
 template <int N>
-void launch_bulk(const Job &j, const HostBlob *hb, uint32_t grid, uint32_t block, size_t smem, cudaStream_t s) {
+void launch_bulk(const Job &j, const HostBlob *hb, bool trans, uint32_t grid, uint32_t block, size_t smem, cudaStream_t s) {
   static thread_local kvt::JobT<N> p;
   p.j = j;
   if constexpr (N > 0) std::memcpy(p.blob, hb->bytes.data(), hb->bytes.size());
-  kvt::kv_move_bulk<N><<<grid, block, smem, s>>>(p);
+  if (trans) kvt::kv_move_bulk<N, true><<<grid, block, smem, s>>>(p);
+  else kvt::kv_move_bulk<N, false><<<grid, block, smem, s>>>(p);
 }
 template <int N>
-void launch_vec(const Job &j, const HostBlob *hb, uint32_t grid, cudaStream_t s) {
+void launch_vec(const Job &j, const HostBlob *hb, bool trans, uint32_t grid, cudaStream_t s) {
   static thread_local kvt::JobT<N> p;
   p.j = j;
   if constexpr (N > 0) std::memcpy(p.blob, hb->bytes.data(), hb->bytes.size());
-  kvt::kv_move_vec<8, N><<<grid, 256, 0, s>>>(p);
+  if (trans) kvt::kv_move_vec<8, N, true><<<grid, 256, 0, s>>>(p);
+  else kvt::kv_move_vec<8, N, false><<<grid, 256, 0, s>>>(p);
+}
+template <typename U>
+void launch_elem(const kvt::JobT<0> &p, bool trans, uint32_t grid, cudaStream_t s) {
+  if (trans) kvt::kv_move_elem<U, true><<<grid, 256, 0, s>>>(p);
+  else kvt::kv_move_elem<U, false><<<grid, 256, 0, s>>>(p);
 }
 
 int launch(kv_ctx *ctx, const Geom &g, const Blob &b, uint32_t piece_first, uint32_t n_pieces,
@@ -323,14 +351,21 @@ int launch(kv_ctx *ctx, const Geom &g, const Blob &b, uint32_t piece_first, uint
   j.tokrow = g.tokrow; j.chunk_bytes = g.chunk_bytes; j.sub_bytes = g.sub_bytes; j.subs = g.subs;
   j.num_pages = g.num_pages;
   if (g.src_pool) { j.src_num_pages = g.src_pool->num_pages; j.src_page_stride = g.src_pool->page_stride_bytes; }
+  j.drow = g.drow; j.H = g.H;
+  if (g.trans) {
+    // the pool of this geometry is the destination pool of dir 2 and "the" pool otherwise; g.Tpool is its page size
+    j.pool_hnd = g.pool_hnd; j.src_hnd = g.src_hnd;
+    j.p_ts = g.drow; j.p_hs = (uint64_t)g.Tpool * g.drow;
+    j.q_ts = g.drow; j.q_hs = (uint64_t)g.Tbuf * g.drow;  // dir 2: Tbuf is the source pool's page size
+  }
   uint32_t cap = cta_cap ? cta_cap : ctx->max_ctas;
   uint32_t grid = 0;
   if (g.kernel == KERNEL_BULK) {
     j.stage_bytes = (g.sub_bytes + 127) / 128 * 128;
-    j.stages = ctx->stages; j.lag = std::min(ctx->lag, ctx->stages - 1);
+    j.stages = g.trans ? ctx->t_stages : ctx->stages; j.lag = std::min(ctx->lag, j.stages - 1);
     j.zero_bytes = std::min<uint32_t>(4096, j.stage_bytes);
     j.l2_hint = ctx->l2_hint;
-    uint32_t warps = ctx->warps;
+    uint32_t warps = g.trans ? ctx->t_warps : ctx->warps;
     size_t smem = (size_t)j.zero_bytes + (size_t)warps * j.stages * j.stage_bytes;
     while (smem > (size_t)ctx->max_smem - 4096 && j.stages > 2) {  // static smem holds barriers + meta
       --j.stages; j.lag = std::min(j.lag, j.stages - 1);
@@ -349,9 +384,9 @@ int launch(kv_ctx *ctx, const Geom &g, const Blob &b, uint32_t piece_first, uint
       j.sched_done = (uint32_t *)(slot + 8);
       j.first_batch = (uint32_t)std::min<uint64_t>(32, total_items / (4 * G));
     }
-    if (!b.inl) launch_bulk<0>(j, nullptr, grid, warps * 32, smem, s);
-    else if (b.inl->bytes.size() <= kInlineSmall) launch_bulk<kInlineSmall>(j, b.inl, grid, warps * 32, smem, s);
-    else launch_bulk<kInlineLarge>(j, b.inl, grid, warps * 32, smem, s);
+    if (!b.inl) launch_bulk<0>(j, nullptr, g.trans, grid, warps * 32, smem, s);
+    else if (b.inl->bytes.size() <= kInlineSmall) launch_bulk<kInlineSmall>(j, b.inl, g.trans, grid, warps * 32, smem, s);
+    else launch_bulk<kInlineLarge>(j, b.inl, g.trans, grid, warps * 32, smem, s);
   } else {
     const uint32_t wpb = 8;  // warps per 256-thread CTA
     const uint64_t want = (total_items + wpb - 1) / wpb;
@@ -359,14 +394,14 @@ int launch(kv_ctx *ctx, const Geom &g, const Blob &b, uint32_t piece_first, uint
     kvt::JobT<0> p0;
     p0.j = j;
     if (g.kernel == KERNEL_VEC) {
-      if (!b.inl) launch_vec<0>(j, nullptr, grid, s);
-      else if (b.inl->bytes.size() <= kInlineSmall) launch_vec<kInlineSmall>(j, b.inl, grid, s);
-      else launch_vec<kInlineLarge>(j, b.inl, grid, s);
+      if (!b.inl) launch_vec<0>(j, nullptr, g.trans, grid, s);
+      else if (b.inl->bytes.size() <= kInlineSmall) launch_vec<kInlineSmall>(j, b.inl, g.trans, grid, s);
+      else launch_vec<kInlineLarge>(j, b.inl, g.trans, grid, s);
     }
-    else if (g.unit >= 8) kvt::kv_move_elem<uint64_t><<<grid, 256, 0, s>>>(p0);
-    else if (g.unit == 4) kvt::kv_move_elem<uint32_t><<<grid, 256, 0, s>>>(p0);
-    else if (g.unit == 2) kvt::kv_move_elem<uint16_t><<<grid, 256, 0, s>>>(p0);
-    else kvt::kv_move_elem<uint8_t><<<grid, 256, 0, s>>>(p0);
+    else if (g.unit >= 8) launch_elem<uint64_t>(p0, g.trans, grid, s);
+    else if (g.unit == 4) launch_elem<uint32_t>(p0, g.trans, grid, s);
+    else if (g.unit == 2) launch_elem<uint16_t>(p0, g.trans, grid, s);
+    else launch_elem<uint8_t>(p0, g.trans, grid, s);
   }
   KV_CUDA(ctx, cudaGetLastError());
   ctx->launches++;
@@ -852,9 +887,11 @@ int kv_ctx_create(kv_ctx **out, int device, size_t staging_bytes) {
   if ((e = cudaSetDevice(device)) != cudaSuccess) return fail(e);
   if ((e = cudaDeviceGetAttribute(&ctx->sm_count, cudaDevAttrMultiProcessorCount, device)) != cudaSuccess) return fail(e);
   if ((e = cudaDeviceGetAttribute(&ctx->max_smem, cudaDevAttrMaxSharedMemoryPerBlockOptin, device)) != cudaSuccess) return fail(e);
-  if ((e = cudaFuncSetAttribute(kvt::kv_move_bulk<0>, cudaFuncAttributeMaxDynamicSharedMemorySize, ctx->max_smem - 4096)) != cudaSuccess) return fail(e);
-  if ((e = cudaFuncSetAttribute(kvt::kv_move_bulk<kInlineSmall>, cudaFuncAttributeMaxDynamicSharedMemorySize, ctx->max_smem - 4096)) != cudaSuccess) return fail(e);
-  if ((e = cudaFuncSetAttribute(kvt::kv_move_bulk<kInlineLarge>, cudaFuncAttributeMaxDynamicSharedMemorySize, ctx->max_smem - 4096)) != cudaSuccess) return fail(e);
+  const void *bulk_kernels[] = {(const void *)kvt::kv_move_bulk<0, false>, (const void *)kvt::kv_move_bulk<kInlineSmall, false>,
+                                (const void *)kvt::kv_move_bulk<kInlineLarge, false>, (const void *)kvt::kv_move_bulk<0, true>,
+                                (const void *)kvt::kv_move_bulk<kInlineSmall, true>, (const void *)kvt::kv_move_bulk<kInlineLarge, true>};
+  for (const void *k : bulk_kernels)
+    if ((e = cudaFuncSetAttribute(k, cudaFuncAttributeMaxDynamicSharedMemorySize, ctx->max_smem - 4096)) != cudaSuccess) return fail(e);
   if ((e = cudaStreamCreateWithFlags(&ctx->side, cudaStreamNonBlocking)) != cudaSuccess) return fail(e);
   if ((e = cudaEventCreateWithFlags(&ctx->ev_entry, cudaEventDisableTiming)) != cudaSuccess) return fail(e);
   for (int i = 0; i < kBlobSlots; ++i)
@@ -899,9 +936,9 @@ int kv_ctx_set_option(kv_ctx *ctx, int option, int64_t v) {
   if (!ctx) return KV_ERR_NULL;
   switch (option) {
     case KV_OPT_KERNEL: if (v < 0 || v > 3) return KV_ERR_SIZE; ctx->kernel = (int)v; break;
-    case KV_OPT_STAGE_BYTES: if (v < 1024 || v > 65536 || v % 16) return KV_ERR_SIZE; ctx->stage_bytes = (uint32_t)v; break;
-    case KV_OPT_STAGES_PER_WARP: if (v < 2 || v > kvt::kMaxStages) return KV_ERR_SIZE; ctx->stages = (uint32_t)v; break;
-    case KV_OPT_WARPS: if (v < 1 || v > kvt::kMaxWarps) return KV_ERR_SIZE; ctx->warps = (uint32_t)v; break;
+    case KV_OPT_STAGE_BYTES: if (v < 1024 || v > 65536 || v % 16) return KV_ERR_SIZE; ctx->stage_bytes = ctx->t_stage_bytes = (uint32_t)v; break;
+    case KV_OPT_STAGES_PER_WARP: if (v < 2 || v > kvt::kMaxStages) return KV_ERR_SIZE; ctx->stages = ctx->t_stages = (uint32_t)v; break;
+    case KV_OPT_WARPS: if (v < 1 || v > kvt::kMaxWarps) return KV_ERR_SIZE; ctx->warps = ctx->t_warps = (uint32_t)v; break;
     case KV_OPT_STORE_LAG: if (v < 1 || v > 3) return KV_ERR_SIZE; ctx->lag = (uint32_t)v; break;
     case KV_OPT_MAX_CTAS: if (v < 0 || v > 65535) return KV_ERR_SIZE; ctx->max_ctas = (uint32_t)v; break;
     case KV_OPT_CHUNK_BYTES: if (v < 0) return KV_ERR_SIZE; ctx->chunk_bytes = (size_t)v; break;

@@ -31,6 +31,7 @@ KV_ERR_ALIGN, KV_ERR_CUDA, KV_ERR_HOST_MEM, KV_ERR_DESC, KV_ERR_NO_DEVICE = -6, 
 KV_ERR_CAPTURE = -11
 KV_LAYOUT_PAGE_FIRST, KV_LAYOUT_LAYER_FIRST = 0, 1
 KV_HOST_AUTO, KV_HOST_DIRECT, KV_HOST_STAGED = 0, 1, 2
+KV_ORDER_NHD, KV_ORDER_HND = 0, 1
 KV_FLAG_VALIDATE, KV_FLAG_IDS_ON_DEVICE = 0x1, 0x2
 (KV_OPT_KERNEL, KV_OPT_STAGE_BYTES, KV_OPT_STAGES_PER_WARP, KV_OPT_WARPS, KV_OPT_STORE_LAG,
  KV_OPT_MAX_CTAS, KV_OPT_CHUNK_BYTES, KV_OPT_HOST_MAX_CTAS, KV_OPT_STAGING_SLOTS,
@@ -50,7 +51,7 @@ class kv_pool_desc(ctypes.Structure):
         ("num_heads", ctypes.c_uint32),
         ("head_dim", ctypes.c_uint32),
         ("elem_bytes", ctypes.c_uint32),
-        ("reserved", ctypes.c_uint32),
+        ("order", ctypes.c_uint32),
         ("page_stride_bytes", ctypes.c_uint64),
     ]
 
@@ -183,18 +184,19 @@ class PoolDesc:
     """Owns a kv_pool_desc and its host array of slab base pointers.
 
     ``slabs`` is a sequence of layer_count*kv_count device pointers (torch tensors or ints) in
-    [layer][kv] order (outer dim layers, slice dim K/V)."""
+    [layer][kv] order (outer dim layers, slice dim K/V); ``order`` is the in-page
+    order of the pool, KV_ORDER_NHD [token][head][dim] or KV_ORDER_HND [head][token][dim]."""
 
     def __init__(self, slabs: Sequence, layer_count: int, kv_count: int, num_pages: int,
                  page_size: int, num_heads: int, head_dim: int, elem_bytes: int,
-                 page_stride_bytes: Optional[int] = None):
+                 page_stride_bytes: Optional[int] = None, order: int = KV_ORDER_NHD):
         assert len(slabs) == layer_count * kv_count
         self._keep = list(slabs)
         self._base = (ctypes.c_void_p * len(slabs))(*[_ptr(s) for s in slabs])
         row = page_size * num_heads * head_dim * elem_bytes
         self.desc = kv_pool_desc(
             ctypes.cast(self._base, ctypes.POINTER(ctypes.c_void_p)), layer_count, kv_count,
-            num_pages, page_size, num_heads, head_dim, elem_bytes, 0,
+            num_pages, page_size, num_heads, head_dim, elem_bytes, int(order),
             row if page_stride_bytes is None else int(page_stride_bytes))
         self.row_bytes = row
 

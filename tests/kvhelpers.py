@@ -6,12 +6,12 @@ import numpy as np
 from oracle import kv_oracle as ko
 
 
-def host_pool(rng, L, C, P, T, H, D, e, pad=0):
+def host_pool(rng, L, C, P, T, H, D, e, pad=0, order=0):
     """Random-byte HostPool (random 8-bit patterns => random 16/32-bit patterns)."""
     row = T * H * D * e
     stride = row + pad
     slabs = [rng.integers(0, 256, size=P * stride, dtype=np.uint8) for _ in range(L * C)]
-    return ko.HostPool(slabs, L, C, P, T, H, D, e, stride)
+    return ko.HostPool(slabs, L, C, P, T, H, D, e, stride, order)
 
 
 def to_device(pool, kvtier, torch, offset_bytes=0):
@@ -25,7 +25,7 @@ def to_device(pool, kvtier, torch, offset_bytes=0):
         tens.append(v)
         bases.append(v.data_ptr())
     desc = kvtier.PoolDesc(bases, pool.L, pool.C, pool.num_pages, pool.T, pool.H, pool.D, pool.e,
-                           pool.page_stride_bytes)
+                           pool.page_stride_bytes, pool.order)
     desc._tensors = tens
     return tens, desc
 

@@ -206,3 +206,43 @@ def test_plan_fused_repage_and_cow(ctx):
     assert status_of(lambda: kv.kv_cow_append(ctx, d, s.L, 7, 7, 1, BUF, 1)) == kv.KV_ERR_SIZE
     assert status_of(lambda: kv.kv_cow_append(ctx, d, s.L, 7, s.P, 1, BUF, 1)) == kv.KV_ERR_PAGE_RANGE
     kv.kv_cow_append(ctx, d, s.L, 7, 9, 0, None, 0)  # nothing to do: KV_OK, even without a device
+
+
+def test_plan_hnd_pools(ctx):
+    """SURVEY.md 8(f) NEXT-2, HND pools: kernel and segment chosen per direction (DESIGN.md "HND pools");
+    a malformed order is KV_ERR_DESC; degenerate HND (one head) plans as a plain copy."""
+    s = W.QWEN3_OMNI
+
+    def pool(order, shape=s, **kw):
+        d = fake_pool(shape, **kw)
+        d.desc.order = order
+        return d
+
+    hnd = pool(kv.KV_ORDER_HND)
+    # pack out of an HND pool: strided source -> bulk ring with 4 KiB stages (16 head_dim rows each)
+    assert status_of(lambda: kv.kv_pack(ctx, hnd, s.L, [1, 2, 3], BUF, dst_bytes=1 << 40)) == kv.KV_ERR_NO_DEVICE
+    assert ctx.stat(kv.KV_STAT_LAST_KERNEL) == kv.KV_KERNEL_BULK
+    assert ctx.stat(kv.KV_STAT_LAST_SEGMENT) == 4096
+    assert ctx.stat(kv.KV_STAT_LAST_ITEMS) == 3 * 96 * 4
+    assert ctx.stat(kv.KV_STAT_LAST_PAYLOAD) == 3 * s.page_bytes
+    # unpack into an HND pool: strided destination -> vec kernel, whole 16 KiB rows
+    assert status_of(lambda: kv.kv_unpack(ctx, BUF, [1, 2, 3], hnd, s.L, 16, 16, 48, src_bytes=1 << 40)) == kv.KV_ERR_NO_DEVICE
+    assert ctx.stat(kv.KV_STAT_LAST_KERNEL) == kv.KV_KERNEL_VEC
+    assert ctx.stat(kv.KV_STAT_LAST_SEGMENT) == 16384
+    # pool -> pool: HND -> NHD is a strided source, NHD -> HND a strided destination
+    nhd64 = pool(kv.KV_ORDER_NHD, s.with_(T=64, P=64), base0=0x7800_0000_0000)
+    hnd64 = pool(kv.KV_ORDER_HND, s.with_(T=64, P=64), base0=0x7800_0000_0000)
+    assert status_of(lambda: kv.kv_repage(ctx, hnd, np.arange(8), nhd64, [0, 1], s.L, 128)) == kv.KV_ERR_NO_DEVICE
+    assert ctx.stat(kv.KV_STAT_LAST_KERNEL) == kv.KV_KERNEL_BULK
+    assert status_of(lambda: kv.kv_repage(ctx, pool(0), np.arange(8), hnd64, [0, 1], s.L, 128)) == kv.KV_ERR_NO_DEVICE
+    assert ctx.stat(kv.KV_STAT_LAST_KERNEL) == kv.KV_KERNEL_VEC
+    # head_dim rows that are not multiples of 16 bytes: element-wise kernel, never rejected
+    odd = pool(kv.KV_ORDER_HND, s.with_(D=20))
+    assert status_of(lambda: kv.kv_pack(ctx, odd, s.L, [1], BUF, dst_bytes=1 << 40)) == kv.KV_ERR_NO_DEVICE
+    assert ctx.stat(kv.KV_STAT_LAST_KERNEL) == kv.KV_KERNEL_ELEM
+    # one head: [token][head] == [head][token]; planned as the contiguous copy it is
+    one = pool(kv.KV_ORDER_HND, s.with_(H=1))
+    assert status_of(lambda: kv.kv_unpack(ctx, BUF, [1], one, s.L, 16, 16, 16, src_bytes=1 << 40)) == kv.KV_ERR_NO_DEVICE
+    assert ctx.stat(kv.KV_STAT_LAST_KERNEL) == kv.KV_KERNEL_BULK
+    assert ctx.stat(kv.KV_STAT_LAST_SEGMENT) == 4096  # the whole 4 KiB row
+    assert status_of(lambda: kv.kv_pack(ctx, pool(2), s.L, [1], BUF, dst_bytes=1 << 40)) == kv.KV_ERR_DESC
