@@ -288,3 +288,46 @@ def run(ctx, desc, shape, slabs, seed=0, out_dir="gpurun_out", hbm_peak=None):
             "summary": [{k: r[k] for k in ("config", "op", "mode", "GBps", "pct_of_measured_hbm_peak", "pct_of_link_peak", "verified") if k in r}
                         for r in recs if "GBps" in r],
             "file": os.path.join(out_dir, "report.json")}
+
+
+def markdown(rep: dict) -> str:
+    """Summary tables of a report.json (what profiles/*_report_summary.md holds)."""
+    pk = rep["peaks"]
+    out = [f"Peaks measured in the same run: D2D copy {pk['hbm_copy_GBps_this_run']:.0f} GB/s (read+write), pinned H2D "
+           f"{pk['h2d_GBps']:.1f} GB/s, D2H {pk['d2h_GBps']:.1f} GB/s; denominator for HBM fractions: "
+           f"{pk['hbm_peak_GBps']:.1f} GB/s (MEASURED_PEAKS.json). GPU: {rep.get('gpu')}; host cores: {rep.get('cores')}.", "",
+           "| config | op | mode | payload MiB | median us | GB/s | % of peak | verified |",
+           "|---|---|---|---:|---:|---:|---:|---|"]
+    for r in rep["records"]:
+        if "time_us_median" in r:
+            pct = (f"{r['pct_of_measured_hbm_peak']:.1f} (HBM)" if "pct_of_measured_hbm_peak" in r
+                   else f"{r['pct_of_link_peak']:.1f} (link)")
+            out.append(f"| {r['config']} | {r['op']} | {r['mode']} | {r['payload_bytes'] / 2**20:.1f} | "
+                       f"{r['time_us_median']:.1f} | {r['GBps']:.1f} | {pct} | {r.get('verified', '')} |")
+        elif "time_us_total" in r:
+            out.append(f"| {r['config']} | {r['op']} | {r['mode']} | {r['payload_bytes'] / 2**20:.0f} | "
+                       f"{r['time_us_total']:.0f} (total) | reload {r['reload_GBps']:.1f} / offload {r['offload_GBps']:.1f} | "
+                       f"{r['pct_of_link_peak_reload']:.1f} (link, reload) | turn 50: {r['turn50_reload_pages']} pages in "
+                       f"{r['turn50_reload_us'] / 1e3:.1f} ms |")
+    for r in rep["records"]:
+        if "rows" not in r:
+            continue
+        out += ["", f"{r['config']}: {r['op']} (isolated calls; L2 flushed clean below 256 MiB):", "",
+                "| MiB | pack us | pack GB/s | % HBM | unpack GB/s | re-page 16->64 GB/s | fused re-page GB/s | offload GB/s (mode) | % link | reload GB/s | % link |",
+                "|---:|---:|---:|---:|---:|---:|---:|---:|---:|---:|---:|"]
+        for w in r["rows"]:
+            mode = {1: "direct", 2: "staged"}.get(w.get("offload_mode"), "?")
+            out.append(f"| {w['MiB']} | {w['pack_us']:.1f} | {w['pack_GBps']:.0f} | {w['pack_pct_hbm_peak']:.1f} | "
+                       f"{w['unpack_GBps']:.0f} | {w['repage_GBps']:.0f} | {w.get('repage_fused_GBps', 0):.0f} | "
+                       f"{w['offload_GBps']:.1f} ({mode}) | {w['offload_pct_link_peak']:.1f} | {w['reload_GBps']:.1f} | "
+                       f"{w['reload_pct_link_peak']:.1f} |")
+        out += ["", f"Smallest size reaching 80 % of the HBM peak (pack, isolated call): "
+                    f"{r.get('smallest_MiB_reaching_80pct_hbm_pack')} MiB."]
+    return "\n".join(out) + "\n"
+
+
+if __name__ == "__main__":  # python -m paper_2606_31093_b200.report gpurun_out/report.json
+    import sys
+
+    with open(sys.argv[1]) as f:
+        sys.stdout.write(markdown(json.load(f)))
