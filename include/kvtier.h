@@ -123,6 +123,9 @@ typedef enum kv_option {
                                 0: always stage them through the ctx's pinned ring with one H2D copy */
   KV_OPT_DYNAMIC = 11,       /* bulk: 1 (default) large launches claim segments from a device counter (guided chunks);
                                 0: static round-robin only */
+  KV_OPT_TENSOR_MAPS = 12,   /* HND pools: 1 (default) whole-token boxes move with cp.async.bulk.tensor through per-slab
+                                tensor maps (cached per pool in the ctx; the copy engine transposes [head][token]);
+                                0: row-gather / 16-byte store paths only */
 } kv_option;
 
 /* kv_ctx_get_stat keys */
@@ -135,6 +138,7 @@ typedef enum kv_stat {
   KV_STAT_LAST_HOST_MODE = 5,/* host mode the last offload/reload used (kv_host_mode) */
   KV_STAT_LAST_GRID = 6,    /* CTAs of the last launch */
   KV_STAT_LAST_SEGMENT = 7, /* bytes per work item of the last call */
+  KV_STAT_LAST_TENSOR_MAPS = 8, /* 1 if the last call's launches used tensor maps for an HND pool side */
 } kv_stat;
 
 /* ---- library ------------------------------------------------------------------------------ */

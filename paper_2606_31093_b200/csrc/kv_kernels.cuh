@@ -78,6 +78,14 @@ struct Job {
   uint32_t src_hnd;           // dir 2: the source pool is HND
   uint64_t p_ts, p_hs;        // strides of the pool side when it is HND (ts = drow, hs = Tpool*drow)
   uint64_t q_ts, q_hs;        // dir 2: strides of the source pool when it is HND
+  // TMA tensor maps of HND pools (one 128-byte CUtensorMap per slab, device memory): the slab is the
+  // rank-4 tensor (dim, head, token, page) with strides (1, T*drow, drow, page_stride) -- token and
+  // head swapped against memory order -- so ONE cp.async.bulk.tensor with the box (drow, H, tb, 1)
+  // moves tb whole tokens between the HND page and an NHD-linear shared-memory stage: the copy
+  // engine does the [head][token] <-> [token][head] transposition.
+  const uint8_t *maps_pool;   // nullptr: the pool side does not use tensor copies
+  const uint8_t *maps_src;    // dir 2: the source pool's maps
+  uint32_t tb;                // tokens per box; a "full" item has bytes == valid == tb * tokrow
 };
 
 // The lookup tables of a launch: slab bases, page ids, pieces.  They live either in device memory
@@ -122,6 +130,8 @@ struct Item {
   // side's address already points at the item's first byte.
   uint32_t mode;
   uint32_t r0;
+  // kTrans only: slab index and (page, first token) of a strided side, the coordinates of a tensor copy
+  uint32_t lc, s_pg, s_t, d_pg, d_t;
 };
 
 // flat item -> (piece, chunk k, layer/kv, sub) -> addresses.
@@ -151,6 +161,7 @@ __device__ __forceinline__ Item decode(const Job &j, const Tables &tb, uint64_t 
     const uint64_t new_pg = slab + (id_begin >> 32) * j.page_stride;
     Item it;
     it.mode = 0; it.r0 = 0;
+    it.lc = lc; it.s_pg = it.s_t = it.d_pg = it.d_t = 0;
     if (k < s0) {
       const uint32_t o = k * j.sub_bytes;
       it.src = old_pg + o; it.dst = new_pg + o; it.bytes = min(j.sub_bytes, b_old - o);
@@ -174,6 +185,7 @@ __device__ __forceinline__ Item decode(const Job &j, const Tables &tb, uint64_t 
   const uint64_t sub_off = (uint64_t)sub * j.sub_bytes;
   Item it;
   it.mode = 0; it.r0 = 0;
+  it.lc = lc; it.s_pg = it.s_t = it.d_pg = it.d_t = 0;
   it.bytes = min(j.sub_bytes, j.chunk_bytes - (uint32_t)sub_off);
   // caller-supplied device ids are global memory even when the other tables are inline
   const int32_t id = (kGlobal || j.ids) ? __ldg(tb.ids + id_begin + pp) : tb.ids[id_begin + pp];
@@ -199,6 +211,7 @@ __device__ __forceinline__ Item decode(const Job &j, const Tables &tb, uint64_t 
       return it;
     }
     baddr = ldt<kGlobal>(tb.bases + j.LC + lc) + (uint64_t)sid * j.src_page_stride;
+    if (kTrans) { it.s_pg = (uint32_t)sid; it.s_t = bk * j.g + (uint32_t)(sub_off / j.tokrow); }
     if (kTrans && j.src_hnd) { baddr += (uint64_t)bk * j.g * j.q_ts; bmode = 1; }
     else baddr += (uint64_t)bk * j.chunk_bytes + sub_off;
   } else {
@@ -212,6 +225,8 @@ __device__ __forceinline__ Item decode(const Job &j, const Tables &tb, uint64_t 
   if (kTrans) {
     it.mode = j.dir == 0 ? (pmode | bmode << 1) : (bmode | pmode << 1);
     it.r0 = (uint32_t)(sub_off / j.drow);
+    const uint32_t pt = pk * j.g + (uint32_t)(sub_off / j.tokrow);
+    if (j.dir == 0) { it.s_pg = (uint32_t)id; it.s_t = pt; } else { it.d_pg = (uint32_t)id; it.d_t = pt; }
   }
   return it;
 }
@@ -266,6 +281,15 @@ __device__ __forceinline__ void bulk_s2g_hint(uint64_t dst, uint32_t src_smem, u
   asm volatile("cp.async.bulk.global.shared::cta.bulk_group.L2::cache_hint [%0], [%1], %2, %3;"
                ::"l"(dst), "r"(src_smem), "r"(bytes), "l"(pol) : "memory");
 }
+// Tensor copies (SASS UTMALDG / UTMASTG) of the rank-4 box at coordinates (0, 0, token, page).
+__device__ __forceinline__ void tensor_g2s(uint32_t dst_smem, const void *map, uint32_t t, uint32_t pg, uint32_t bar) {
+  asm volatile("cp.async.bulk.tensor.4d.shared::cluster.global.tile.mbarrier::complete_tx::bytes [%0], [%1, {%2, %3, %4, %5}], [%6];"
+               ::"r"(dst_smem), "l"(map), "r"(0), "r"(0), "r"(t), "r"(pg), "r"(bar) : "memory");
+}
+__device__ __forceinline__ void tensor_s2g(const void *map, uint32_t t, uint32_t pg, uint32_t src_smem) {
+  asm volatile("cp.async.bulk.tensor.4d.global.shared::cta.tile.bulk_group [%0, {%1, %2, %3, %4}], [%5];"
+               ::"l"(map), "r"(0), "r"(0), "r"(t), "r"(pg), "r"(src_smem) : "memory");
+}
 __device__ __forceinline__ void bulk_commit() { asm volatile("cp.async.bulk.commit_group;" ::: "memory"); }
 template <int N>
 __device__ __forceinline__ void bulk_wait_read() {
@@ -314,6 +338,7 @@ struct StageMeta {
   uint64_t dst;
   uint32_t bytes, valid;
   uint32_t mode, r0;  // kTrans only
+  uint32_t lc, d_pg, d_t;
 };
 
 // ---------------------------------------------------------------------------------------------
@@ -433,15 +458,28 @@ __global__ void __launch_bounds__(kMaxWarps * 32, 1) kv_move_bulk(const __grid_c
     if constexpr (kTrans) {
       const uint32_t mode = __shfl_sync(0xffffffffu, mine.mode, sel);
       const uint32_t r0 = __shfl_sync(0xffffffffu, mine.r0, sel);
+      const uint32_t lc = __shfl_sync(0xffffffffu, mine.lc, sel);
+      const uint32_t s_pg = __shfl_sync(0xffffffffu, mine.s_pg, sel), s_t = __shfl_sync(0xffffffffu, mine.s_t, sel);
+      const uint32_t d_pg = __shfl_sync(0xffffffffu, mine.d_pg, sel), d_t = __shfl_sync(0xffffffffu, mine.d_t, sel);
       const Strides st = strides_of(j);
       const uint32_t upr = j.drow >> 4;  // 16-byte units per head_dim row
+      // tensor copies serve whole boxes only; ragged tails (and copy-on-write rows) take the lane paths
+      const uint32_t box_bytes = j.tb * j.tokrow;
+      const uint8_t *maps_s = j.dir == 2 ? j.maps_src : (j.dir == 0 ? j.maps_pool : nullptr);
+      const uint8_t *maps_d = (j.dir == 1 || j.dir == 2) ? j.maps_pool : nullptr;
       if (it >= depth && it - depth < n_known) {  // ---- store side: item si
         const uint64_t si = it - depth;
         const uint32_t s = (uint32_t)(si % K);
         mbar_wait(smem_u32(&full_bar[warp][s]), (uint32_t)(si / K) & 1);
         const StageMeta m = meta[warp][s];
         const uint32_t sbase = stage0 + s * j.stage_bytes;
-        if (m.mode & 2) {  // strided destination: LDS.128 from the stage, STG.128 to the row's place
+        if ((m.mode & 2) && maps_d && m.bytes == box_bytes && m.valid == box_bytes) {
+          // strided destination, whole box: one tensor store scatters the NHD stage into the HND page
+          if (lane == 0) {
+            asm volatile("fence.proxy.async.shared::cta;" ::: "memory");
+            tensor_s2g(maps_d + (size_t)m.lc * 128, m.d_t, m.d_pg, sbase);
+          }
+        } else if (m.mode & 2) {  // strided destination: LDS.128 from the stage, STG.128 to the row's place
           const uint32_t nb = m.bytes >> 4, nv = m.valid >> 4;
           for (uint32_t u0 = lane; u0 < nb; u0 += 128) {
             uint4 v[4];
@@ -479,8 +517,17 @@ __global__ void __launch_bounds__(kMaxWarps * 32, 1) kv_move_bulk(const __grid_c
         if (lane == 0) {
           StageMeta &m = meta[warp][s];
           m.dst = dst; m.bytes = bytes; m.valid = valid; m.mode = mode; m.r0 = r0;
+          m.lc = lc; m.d_pg = d_pg; m.d_t = d_t;
         }
-        if (mode & 1) {  // strided source: 16-byte cp.async (LDGSTS) gathers the rows in NHD order;
+        if ((mode & 1) && maps_s && bytes == box_bytes && valid == box_bytes) {
+          // strided source, whole box: one tensor load gathers the HND page's rows in NHD order
+          if (lane == 0) {
+            mbar_expect_tx(bar, box_bytes);
+            tensor_g2s(sbase, maps_s + (size_t)lc * 128, s_t, s_pg, bar);
+          } else {
+            mbar_arrive(bar);
+          }
+        } else if (mode & 1) {  // strided source: 16-byte cp.async (LDGSTS) gathers the rows in NHD order;
                          // each lane's arrival fires when its own copies have landed
           const uint32_t nv = valid >> 4;
           for (uint32_t u = lane; u < nv; u += 32)

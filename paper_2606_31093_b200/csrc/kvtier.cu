@@ -5,6 +5,7 @@
 // There is no CPU fallback: without a CUDA device transfer calls fail (KV_ERR_CUDA / NO_DEVICE).
 #include "../../include/kvtier.h"
 
+#include <cuda.h>  // CUtensorMap types only; the encoder is fetched through cudaGetDriverEntryPoint
 #include <cuda_runtime.h>
 
 #include <algorithm>
@@ -25,8 +26,20 @@ constexpr int kMaxStagingSlots = 4;
 constexpr uint32_t kMaxLayersKv = 4096;  // layer_count * kv_count
 constexpr uint64_t kAutoStagedMinBytes = 16ull << 20;
 constexpr uint32_t kSchedSlots = 256;  // claim counters, handed out round-robin per launch
+constexpr int kStaticSmemReserve = 8192;  // static shared memory of kv_move_bulk (barriers + stage metadata, 6 KiB) rounded up
 
 enum KernelKind { KERNEL_AUTO = 0, KERNEL_BULK = 1, KERNEL_VEC = 2, KERNEL_ELEM = 3 };
+
+// Tensor maps of one HND pool for one box size (kv_kernels.cuh "TMA tensor maps"): built once per
+// (pool, box) and kept in device memory for the life of the ctx.
+struct MapSet {
+  std::vector<uint64_t> key;  // slab bases + every descriptor field the maps depend on + box tokens
+  void *d = nullptr;          // device array of LC CUtensorMap
+};
+constexpr size_t kMaxMapSets = 64;
+typedef CUresult (*EncodeTiledFn)(CUtensorMap *, CUtensorMapDataType, cuuint32_t, void *, const cuuint64_t *,
+                                  const cuuint64_t *, const cuuint32_t *, const cuuint32_t *, CUtensorMapInterleave,
+                                  CUtensorMapSwizzle, CUtensorMapL2promotion, CUtensorMapFloatOOBfill);
 
 struct BlobSlot {
   void *h = nullptr;  // pinned host
@@ -61,8 +74,12 @@ struct kv_ctx {
   // bulk geometry of transposing transfers (an HND pool): rows are gathered with 16-byte cp.async by all
   // lanes, which wants more, shallower issuing warps (measured: 8 x 4 x 4 KiB)
   uint32_t t_stage_bytes = 4096, t_stages = 4, t_warps = 8;
-  uint32_t staging_slots = 2, l2_hint = 0, inline_tables = 1, dynamic = 1;
+  uint32_t staging_slots = 2, l2_hint = 0, inline_tables = 1, dynamic = 1, tensor_maps = 1;
   uint32_t next_sched = 0;
+  EncodeTiledFn encode_tiled = nullptr;  // cuTensorMapEncodeTiled, nullptr if the driver has none
+  std::vector<MapSet> map_sets;
+  cudaStream_t cur_stream = nullptr;     // stream of the entry point being served (capture check while planning)
+  uint64_t last_tma = 0;
   size_t chunk_bytes = 0;
   // stats
   uint64_t launches = 0, memcpys = 0, last_items = 0, last_payload = 0, last_kernel = 0,
@@ -110,9 +127,13 @@ struct Geom {
   uint32_t unit = 16;  // widest power of two dividing every address/length (elem kernel)
   // dir 2 (pool -> pool): the source pool; its bases follow the destination's in the tables
   const kv_pool_desc *src_pool = nullptr;
+  const kv_pool_desc *dst_pool = nullptr;  // the pool of the call (destination pool of dir 2)
   // an HND pool on either side makes the transfer a [token] x [head] transposition (kTrans kernels)
   bool trans = false;
   uint32_t drow = 0, H = 0, pool_hnd = 0, src_hnd = 0;
+  // HND sides served by tensor copies: box of `tb` whole tokens, element width `tma_es` bytes
+  bool tma = false;
+  uint32_t tb = 0, tma_es = 0;
 };
 
 struct Req {          // one request as the caller states it
@@ -163,12 +184,93 @@ uint32_t low_pow2(uint64_t v) {  // largest power of two (<= 16) dividing v; 16 
   return u;
 }
 
+// ---- tensor maps of HND pools ----------------------------------------------------------------
+void map_key(const kv_pool_desc *p, uint32_t layer_count, uint32_t tb, uint32_t es, std::vector<uint64_t> *k) {
+  const uint32_t LC = layer_count * p->kv_count;
+  k->clear();
+  k->reserve(LC + 8);
+  const uint64_t f[8] = {LC, p->num_pages, p->page_size, p->num_heads, (uint64_t)p->head_dim * p->elem_bytes,
+                         p->page_stride_bytes, tb, es};
+  k->insert(k->end(), f, f + 8);
+  for (uint32_t i = 0; i < LC; ++i) k->push_back((uint64_t)(uintptr_t)p->base[i]);
+}
+
+const MapSet *find_maps(const kv_ctx *ctx, const std::vector<uint64_t> &key) {
+  for (const MapSet &m : ctx->map_sets)
+    if (m.key == key) return &m;
+  return nullptr;
+}
+
+// Smallest element width that keeps the innermost box dimension within the 256-element limit.
+uint32_t tma_elem_bytes(uint32_t drow) {
+  for (uint32_t es : {1u, 2u, 4u, 8u})
+    if (drow % es == 0 && drow / es <= 256) return es;
+  return 0;
+}
+
+// Device array of LC tensor maps for pool `p` (slab = tensor (dim, head, token, page), box (drow, H, tb, 1)).
+// Built on first use: LC encoder calls + one blocking copy; never during stream capture (the caller checks).
+int get_maps(kv_ctx *ctx, const kv_pool_desc *p, uint32_t layer_count, uint32_t tb, uint32_t es, const uint8_t **out) {
+  std::vector<uint64_t> key;
+  map_key(p, layer_count, tb, es, &key);
+  if (const MapSet *m = find_maps(ctx, key)) { *out = (const uint8_t *)m->d; return KV_OK; }
+  const uint32_t LC = layer_count * p->kv_count;
+  const uint32_t drow = p->head_dim * p->elem_bytes;
+  static const CUtensorMapDataType kTypes[9] = {CU_TENSOR_MAP_DATA_TYPE_UINT8, CU_TENSOR_MAP_DATA_TYPE_UINT8,
+      CU_TENSOR_MAP_DATA_TYPE_UINT16, CU_TENSOR_MAP_DATA_TYPE_UINT16, CU_TENSOR_MAP_DATA_TYPE_UINT32,
+      CU_TENSOR_MAP_DATA_TYPE_UINT32, CU_TENSOR_MAP_DATA_TYPE_UINT32, CU_TENSOR_MAP_DATA_TYPE_UINT32,
+      CU_TENSOR_MAP_DATA_TYPE_UINT64};
+  std::vector<CUtensorMap> maps(LC);
+  const cuuint64_t dims[4] = {drow / es, p->num_heads, p->page_size, p->num_pages};
+  const cuuint64_t strides[3] = {(cuuint64_t)p->page_size * drow, drow, p->page_stride_bytes};
+  const cuuint32_t box[4] = {drow / es, p->num_heads, tb, 1};
+  const cuuint32_t ones[4] = {1, 1, 1, 1};
+  for (uint32_t i = 0; i < LC; ++i) {
+    CUresult r = ctx->encode_tiled(&maps[i], kTypes[es], 4, p->base[i], dims, strides, box, ones,
+                                   CU_TENSOR_MAP_INTERLEAVE_NONE, CU_TENSOR_MAP_SWIZZLE_NONE,
+                                   CU_TENSOR_MAP_L2_PROMOTION_L2_256B, CU_TENSOR_MAP_FLOAT_OOB_FILL_NONE);
+    if (r != CUDA_SUCCESS) { ctx->last_cuda_error = (int)r; return KV_ERR_CUDA; }
+  }
+  if (ctx->map_sets.size() >= kMaxMapSets) {  // rare: drop everything once nothing can still be reading it
+    KV_CUDA(ctx, cudaDeviceSynchronize());
+    for (MapSet &m : ctx->map_sets) cudaFree(m.d);
+    ctx->map_sets.clear();
+  }
+  MapSet ms;
+  ms.key = key;
+  KV_CUDA(ctx, cudaMalloc(&ms.d, (size_t)LC * sizeof(CUtensorMap)));
+  cudaError_t e = cudaMemcpy(ms.d, maps.data(), (size_t)LC * sizeof(CUtensorMap), cudaMemcpyHostToDevice);
+  if (e != cudaSuccess) { cudaFree(ms.d); ctx->last_cuda_error = (int)e; (void)cudaGetLastError(); return KV_ERR_CUDA; }
+  ctx->map_sets.push_back(ms);
+  *out = (const uint8_t *)ms.d;
+  return KV_OK;
+}
+
+// Can the HND side(s) of this geometry move by tensor copies?  (Planning only: no CUDA calls except
+// the capture query.)  While `cur_stream` is being captured, only maps already in the cache may be used.
+bool tma_eligible(const kv_ctx *ctx, const kv_pool_desc *p, const kv_pool_desc *src_pool, uint32_t layer_count,
+                  uint32_t gtok, uint64_t tokrow, uint32_t drow, uint32_t cap, uint32_t *tb_out, uint32_t *es_out) {
+  if (!ctx->tensor_maps || !ctx->encode_tiled) return false;
+  const uint32_t es = tma_elem_bytes(drow);
+  if (!es || (drow % 16) || p->num_heads > 256 || tokrow > cap) return false;
+  uint32_t tb = (uint32_t)std::min<uint64_t>(std::min<uint64_t>(gtok, 256), cap / tokrow);
+  while (tb > 1 && gtok % tb) --tb;  // boxes tile the chunk exactly
+  auto side_ok = [&](const kv_pool_desc *q) {
+    return q->page_stride_bytes % 16 == 0 && q->page_stride_bytes < (1ull << 40) &&
+           (uint64_t)q->page_size * drow < (1ull << 40);
+  };
+  if (!side_ok(p) || (src_pool && !side_ok(src_pool))) return false;
+  *tb_out = tb; *es_out = es;
+  return true;
+}
+
 int make_geom(const kv_ctx *ctx, const kv_pool_desc *p, uint32_t layer_count, uint32_t Tbuf,
               int dir, int layout, const std::vector<Req> &reqs, Geom *out,
               const kv_pool_desc *src_pool = nullptr) {
   if (layout != KV_LAYOUT_PAGE_FIRST && layout != KV_LAYOUT_LAYER_FIRST) return KV_ERR_LAYOUT;
   Geom g;
   g.L = layer_count; g.C = p->kv_count; g.LC = g.L * g.C;
+  g.dst_pool = p;
   g.Tpool = p->page_size; g.Tbuf = Tbuf;
   g.g = gcd32(g.Tpool, g.Tbuf);
   g.elem = p->elem_bytes;
@@ -207,29 +309,48 @@ int make_geom(const kv_ctx *ctx, const kv_pool_desc *p, uint32_t layer_count, ui
   g.unit = unit;
   int kernel = ctx->kernel;
   if (unit < 16) kernel = KERNEL_ELEM;  // 16-byte paths need 16-byte alignment everywhere
-  else if (kernel == KERNEL_AUTO) {
-    // Measured on B200: a strided DESTINATION is fastest with 16-byte STG from many
-    // warps (vec, 5.5 TB/s); a strided source alone is fastest gathered by cp.async into the bulk ring
-    // and stored with one bulk copy (5.8 TB/s); everything contiguous is the bulk path (6.3 TB/s).
+  if (g.trans && dir != 3 && kernel != KERNEL_ELEM && kernel != KERNEL_VEC) {
+    // HND sides by tensor copies: the bulk ring with its contiguous-path geometry, one box per item
+    uint32_t tb = 0, es = 0;
+    const uint32_t cap16 = std::max(16u, ctx->stage_bytes / 16 * 16);
+    if (tma_eligible(ctx, p, g.src_hnd ? src_pool : nullptr, layer_count, g.g, tokrow, g.drow, cap16, &tb, &es)) {
+      bool cached_or_free = true;
+      if (!ctx->host_only && capturing(ctx->cur_stream)) {
+        std::vector<uint64_t> key;
+        if (g.pool_hnd) { map_key(p, layer_count, tb, es, &key); cached_or_free = find_maps(ctx, key) != nullptr; }
+        if (cached_or_free && g.src_hnd) { map_key(src_pool, layer_count, tb, es, &key); cached_or_free = find_maps(ctx, key) != nullptr; }
+      }
+      if (cached_or_free) { g.tma = true; g.tb = tb; g.tma_es = es; kernel = KERNEL_BULK; }
+    }
+  }
+  if (kernel == KERNEL_AUTO) {
+    // Measured on B200 for the paths without tensor maps: a strided DESTINATION is
+    // fastest with 16-byte STG from many warps (vec, 5.5 TB/s); a strided source alone is fastest gathered by
+    // cp.async into the bulk ring and stored with one bulk copy (5.8 TB/s); everything contiguous is the
+    // bulk path (6.3 TB/s).
     const bool dst_strided = g.pool_hnd && dir != 0;
     kernel = dst_strided ? KERNEL_VEC : KERNEL_BULK;
   }
-  uint32_t cap = kernel == KERNEL_BULK ? (g.trans ? ctx->t_stage_bytes : ctx->stage_bytes) : 16384u;
+  uint32_t cap = kernel == KERNEL_BULK ? (g.trans && !g.tma ? ctx->t_stage_bytes : ctx->stage_bytes) : 16384u;
   cap = std::max(16u, cap / 16 * 16);
   if (g.trans && kernel == KERNEL_BULK && g.drow > cap) kernel = KERNEL_VEC;  // a row must fit one stage
   g.kernel = kernel;
   g.sub_bytes = std::min(g.chunk_bytes, cap);
   if (g.trans) g.sub_bytes = std::min(g.chunk_bytes, std::max(g.drow, cap / g.drow * g.drow));  // whole rows
+  if (g.tma) g.sub_bytes = g.tb * g.tokrow;  // whole tokens: one box
   if (kernel == KERNEL_BULK && dir != 3) {
     // Launch-bound calls: with fewer segments than issuing warps most SMs would idle while a few
     // move 16 KiB each; cutting segments down to >= 4 KiB spreads a small transfer over the chip
     // (measured on B200, 1 MiB pack back to back: 6.1 -> 5.0 us per call).
     uint64_t chunks = 0;
     for (const Req &r : reqs) chunks += r.n_ids * (g.Tpool / g.g) * g.LC;
-    const uint64_t lanes = (uint64_t)ctx->sm_count * (g.trans ? ctx->t_warps : ctx->warps);
+    const uint64_t lanes = (uint64_t)ctx->sm_count * (g.trans && !g.tma ? ctx->t_warps : ctx->warps);
     while (g.sub_bytes >= 8192 && g.sub_bytes % 32 == 0 && (!g.trans || (g.sub_bytes / 2) % g.drow == 0) &&
-           chunks * ((g.chunk_bytes + g.sub_bytes - 1) / g.sub_bytes) * 2 <= lanes)
+           (!g.tma || g.tb % 2 == 0) &&
+           chunks * ((g.chunk_bytes + g.sub_bytes - 1) / g.sub_bytes) * 2 <= lanes) {
       g.sub_bytes /= 2;
+      if (g.tma) g.tb /= 2;
+    }
   }
   g.subs = (g.chunk_bytes + g.sub_bytes - 1) / g.sub_bytes;
   *out = g;
@@ -358,20 +479,34 @@ int launch(kv_ctx *ctx, const Geom &g, const Blob &b, uint32_t piece_first, uint
     j.p_ts = g.drow; j.p_hs = (uint64_t)g.Tpool * g.drow;
     j.q_ts = g.drow; j.q_hs = (uint64_t)g.Tbuf * g.drow;  // dir 2: Tbuf is the source pool's page size
   }
+  ctx->last_tma = 0;
+  if (g.tma && g.kernel == KERNEL_BULK) {
+    j.tb = g.tb;
+    if (g.pool_hnd) {
+      int rc = get_maps(ctx, g.dst_pool, g.L, g.tb, g.tma_es, &j.maps_pool);
+      if (rc) return rc;
+    }
+    if (g.src_hnd) {
+      int rc = get_maps(ctx, g.src_pool, g.L, g.tb, g.tma_es, &j.maps_src);
+      if (rc) return rc;
+    }
+    ctx->last_tma = 1;
+  }
   uint32_t cap = cta_cap ? cta_cap : ctx->max_ctas;
   uint32_t grid = 0;
   if (g.kernel == KERNEL_BULK) {
+    const bool lane_geom = g.trans && !g.tma;  // row gathers by all lanes want more, shallower warps
     j.stage_bytes = (g.sub_bytes + 127) / 128 * 128;
-    j.stages = g.trans ? ctx->t_stages : ctx->stages; j.lag = std::min(ctx->lag, j.stages - 1);
+    j.stages = lane_geom ? ctx->t_stages : ctx->stages; j.lag = std::min(ctx->lag, j.stages - 1);
     j.zero_bytes = std::min<uint32_t>(4096, j.stage_bytes);
     j.l2_hint = ctx->l2_hint;
-    uint32_t warps = g.trans ? ctx->t_warps : ctx->warps;
+    uint32_t warps = lane_geom ? ctx->t_warps : ctx->warps;
     size_t smem = (size_t)j.zero_bytes + (size_t)warps * j.stages * j.stage_bytes;
-    while (smem > (size_t)ctx->max_smem - 4096 && j.stages > 2) {  // static smem holds barriers + meta
+    while (smem > (size_t)ctx->max_smem - kStaticSmemReserve && j.stages > 2) {  // static smem holds barriers + meta
       --j.stages; j.lag = std::min(j.lag, j.stages - 1);
       smem = (size_t)j.zero_bytes + (size_t)warps * j.stages * j.stage_bytes;
     }
-    while (smem > (size_t)ctx->max_smem - 4096 && warps > 1) {
+    while (smem > (size_t)ctx->max_smem - kStaticSmemReserve && warps > 1) {
       --warps;
       smem = (size_t)j.zero_bytes + (size_t)warps * j.stages * j.stage_bytes;
     }
@@ -891,7 +1026,16 @@ int kv_ctx_create(kv_ctx **out, int device, size_t staging_bytes) {
                                 (const void *)kvt::kv_move_bulk<kInlineLarge, false>, (const void *)kvt::kv_move_bulk<0, true>,
                                 (const void *)kvt::kv_move_bulk<kInlineSmall, true>, (const void *)kvt::kv_move_bulk<kInlineLarge, true>};
   for (const void *k : bulk_kernels)
-    if ((e = cudaFuncSetAttribute(k, cudaFuncAttributeMaxDynamicSharedMemorySize, ctx->max_smem - 4096)) != cudaSuccess) return fail(e);
+    if ((e = cudaFuncSetAttribute(k, cudaFuncAttributeMaxDynamicSharedMemorySize, ctx->max_smem - kStaticSmemReserve)) != cudaSuccess) return fail(e);
+  {  // cuTensorMapEncodeTiled without linking libcuda; absent -> HND pools keep to the lane paths
+    void *fn = nullptr;
+    cudaDriverEntryPointQueryResult qr = cudaDriverEntryPointSymbolNotFound;
+    if (cudaGetDriverEntryPoint("cuTensorMapEncodeTiled", &fn, cudaEnableDefault, &qr) == cudaSuccess &&
+        qr == cudaDriverEntryPointSuccess)
+      ctx->encode_tiled = (EncodeTiledFn)fn;
+    else
+      (void)cudaGetLastError();
+  }
   if ((e = cudaStreamCreateWithFlags(&ctx->side, cudaStreamNonBlocking)) != cudaSuccess) return fail(e);
   if ((e = cudaEventCreateWithFlags(&ctx->ev_entry, cudaEventDisableTiming)) != cudaSuccess) return fail(e);
   for (int i = 0; i < kBlobSlots; ++i)
@@ -923,6 +1067,7 @@ int kv_ctx_destroy(kv_ctx *ctx) {
       if (ctx->ev_free[i]) { cudaEventSynchronize(ctx->ev_free[i]); cudaEventDestroy(ctx->ev_free[i]); }
     }
     if (ctx->staging) cudaFree(ctx->staging);
+    for (MapSet &m : ctx->map_sets) cudaFree(m.d);
     if (ctx->d_status) cudaFree(ctx->d_status);
     if (ctx->ev_entry) cudaEventDestroy(ctx->ev_entry);
     if (ctx->side) cudaStreamDestroy(ctx->side);
@@ -947,6 +1092,7 @@ int kv_ctx_set_option(kv_ctx *ctx, int option, int64_t v) {
     case KV_OPT_L2_HINT: if (v < 0 || v > 1) return KV_ERR_SIZE; ctx->l2_hint = (uint32_t)v; break;
     case KV_OPT_INLINE_TABLES: if (v < 0 || v > 1) return KV_ERR_SIZE; ctx->inline_tables = (uint32_t)v; break;
     case KV_OPT_DYNAMIC: if (v < 0 || v > 1) return KV_ERR_SIZE; ctx->dynamic = (uint32_t)v; break;
+    case KV_OPT_TENSOR_MAPS: if (v < 0 || v > 1) return KV_ERR_SIZE; ctx->tensor_maps = (uint32_t)v; break;
     default: return KV_ERR_LAYOUT;
   }
   return KV_OK;
@@ -963,6 +1109,7 @@ int kv_ctx_get_stat(kv_ctx *ctx, int stat, uint64_t *out) {
     case KV_STAT_LAST_HOST_MODE: *out = ctx->last_mode; break;
     case KV_STAT_LAST_GRID: *out = ctx->last_grid; break;
     case KV_STAT_LAST_SEGMENT: *out = ctx->last_segment; break;
+    case KV_STAT_LAST_TENSOR_MAPS: *out = ctx->last_tma; break;
     default: return KV_ERR_LAYOUT;
   }
   return KV_OK;
@@ -1016,6 +1163,7 @@ int kv_pack(kv_ctx *ctx, const kv_pool_desc *pools, uint32_t layer_count, const 
   const int64_t off[2] = {0, (int64_t)n};
   void *const dsts[1] = {dst};
   const uint64_t nb[1] = {(uint64_t)dst_bytes};
+  if (ctx) ctx->cur_stream = (cudaStream_t)stream;
   Call c;
   int rc = plan_pack(ctx, pools, layer_count, page_ids, off, 1, layout, dsts, nb, flags, &c);
   if (rc) return rc;
@@ -1030,6 +1178,7 @@ int kv_unpack(kv_ctx *ctx, const void *src, size_t src_bytes, const int32_t *dst
   const void *const srcs[1] = {src};
   const uint64_t nb[1] = {(uint64_t)src_bytes};
   const uint64_t nt[1] = {n_tokens};
+  if (ctx) ctx->cur_stream = (cudaStream_t)stream;
   Call c;
   int rc = plan_unpack(ctx, srcs, nb, dst_page_ids, off, nt, 1, pools, layer_count, src_page_size,
                        dst_page_size, layout, flags, &c);
@@ -1040,6 +1189,7 @@ int kv_unpack(kv_ctx *ctx, const void *src, size_t src_bytes, const int32_t *dst
 int kv_pack_batched(kv_ctx *ctx, const kv_pool_desc *pools, uint32_t layer_count,
                     const int32_t *page_ids, const int64_t *req_offsets, uint32_t n_req, int layout,
                     void *const *dsts, const uint64_t *dst_bytes, uint32_t flags, kv_stream_t stream) {
+  if (ctx) ctx->cur_stream = (cudaStream_t)stream;
   Call c;
   int rc = plan_pack(ctx, pools, layer_count, page_ids, req_offsets, n_req, layout, dsts, dst_bytes, flags, &c);
   if (rc) return rc;
@@ -1051,6 +1201,7 @@ int kv_unpack_batched(kv_ctx *ctx, const void *const *srcs, const uint64_t *src_
                       const uint64_t *n_tokens, uint32_t n_req, const kv_pool_desc *pools,
                       uint32_t layer_count, uint32_t src_page_size, uint32_t dst_page_size,
                       int layout, uint32_t flags, kv_stream_t stream) {
+  if (ctx) ctx->cur_stream = (cudaStream_t)stream;
   Call c;
   int rc = plan_unpack(ctx, srcs, src_bytes, dst_page_ids, req_offsets, n_tokens, n_req, pools,
                        layer_count, src_page_size, dst_page_size, layout, flags, &c);
@@ -1063,6 +1214,7 @@ int kv_repage_batched(kv_ctx *ctx, const kv_pool_desc *src_pools, const int32_t 
                       const int32_t *dst_page_ids, const int64_t *dst_offsets,
                       const uint64_t *n_tokens, uint32_t n_req, uint32_t layer_count, uint32_t flags,
                       kv_stream_t stream) {
+  if (ctx) ctx->cur_stream = (cudaStream_t)stream;
   Call c;
   std::vector<int32_t> ids;
   int rc = plan_repage(ctx, src_pools, src_page_ids, src_offsets, dst_pools, dst_page_ids,
@@ -1085,6 +1237,7 @@ int kv_cow_append_batched(kv_ctx *ctx, const kv_pool_desc *pools, uint32_t layer
                           const int32_t *old_ids, const int32_t *new_ids, const uint32_t *n_old,
                           const uint32_t *n_app, const void *const *apps, uint32_t n_sessions,
                           uint32_t flags, kv_stream_t stream) {
+  if (ctx) ctx->cur_stream = (cudaStream_t)stream;
   Call c;
   int rc = plan_cow(ctx, pools, layer_count, old_ids, new_ids, n_old, n_app, apps, n_sessions, flags, &c);
   if (rc) return rc;
@@ -1106,6 +1259,7 @@ int kv_offload(kv_ctx *ctx, const kv_pool_desc *pools, uint32_t layer_count,
   const int64_t off[2] = {0, (int64_t)n};
   void *const dsts[1] = {host_dst};
   const uint64_t nb[1] = {(uint64_t)host_bytes};
+  if (ctx) ctx->cur_stream = (cudaStream_t)stream;
   Call c;
   int rc = plan_pack(ctx, pools, layer_count, page_ids, off, 1, layout, dsts, nb, flags, &c);
   if (rc) return rc;
@@ -1120,6 +1274,7 @@ int kv_reload(kv_ctx *ctx, const void *host_src, size_t host_bytes, const int32_
   const void *const srcs[1] = {host_src};
   const uint64_t nb[1] = {(uint64_t)host_bytes};
   const uint64_t nt[1] = {n_tokens};
+  if (ctx) ctx->cur_stream = (cudaStream_t)stream;
   Call c;
   int rc = plan_unpack(ctx, srcs, nb, dst_page_ids, off, nt, 1, pools, layer_count, src_page_size,
                        dst_page_size, layout, flags, &c);
@@ -1131,6 +1286,7 @@ int kv_offload_batched(kv_ctx *ctx, const kv_pool_desc *pools, uint32_t layer_co
                        const int32_t *page_ids, const int64_t *req_offsets, uint32_t n_req,
                        int layout, void *const *host_dsts, const uint64_t *host_bytes, int mode,
                        uint32_t flags, kv_stream_t stream) {
+  if (ctx) ctx->cur_stream = (cudaStream_t)stream;
   Call c;
   int rc = plan_pack(ctx, pools, layer_count, page_ids, req_offsets, n_req, layout, host_dsts, host_bytes, flags, &c);
   if (rc) return rc;
@@ -1142,6 +1298,7 @@ int kv_reload_batched(kv_ctx *ctx, const void *const *host_srcs, const uint64_t 
                       const uint64_t *n_tokens, uint32_t n_req, const kv_pool_desc *pools,
                       uint32_t layer_count, uint32_t src_page_size, uint32_t dst_page_size,
                       int layout, int mode, uint32_t flags, kv_stream_t stream) {
+  if (ctx) ctx->cur_stream = (cudaStream_t)stream;
   Call c;
   int rc = plan_unpack(ctx, host_srcs, host_bytes, dst_page_ids, req_offsets, n_tokens, n_req,
                        pools, layer_count, src_page_size, dst_page_size, layout, flags, &c);

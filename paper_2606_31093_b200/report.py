@@ -116,6 +116,18 @@ def run(ctx, desc, shape, slabs, seed=0, out_dir="gpurun_out", hbm_peak=None):
     rec("2 prefix", "unpack", "device", pl, 2 * pl, n,
         lambda: kv.kv_unpack(ctx, buf, c2.dst_ids, desc, L, T, T, n * T), reps=20, warm=3,
         check=lambda: scatter_ok(buf, c2.dst_ids))
+    # ---- NEXT-2: the same prefix on an HND pool ([head][token][dim] pages; the buffer stays NHD, so the
+    # transfer transposes).  Same slabs, HND descriptor: timing only (parity: tests/test_gpu_hnd.py).
+    desc_h = kv.PoolDesc(slabs, L, shape.C, shape.P, T, shape.H, shape.D, shape.e, order=kv.KV_ORDER_HND)
+    for tm, label in ((1, "tensor maps (cp.async.bulk.tensor)"), (0, "lane paths (cp.async gather / STG.128)")):
+        ctx.set_option(kv.KV_OPT_TENSOR_MAPS, tm)
+        rec("2 prefix, HND pool", "pack", label, pl, 2 * pl, n,
+            lambda: kv.kv_pack(ctx, desc_h, L, c2.src_ids, buf), reps=20, warm=3)
+        rec("2 prefix, HND pool", "unpack", label, pl, 2 * pl, n,
+            lambda: kv.kv_unpack(ctx, buf, c2.dst_ids, desc_h, L, T, T, n * T), reps=20, warm=3)
+        rec("2 prefix, HND pool", "repage HND->HND pool", label, pl, 2 * pl, n,
+            lambda: kv.kv_repage(ctx, desc_h, c2.src_ids, desc_h, c2.dst_ids, L, n * T), reps=20, warm=3)
+    ctx.set_option(kv.KV_OPT_TENSOR_MAPS, 1)
     host_total = 0
     hp = None
     try:

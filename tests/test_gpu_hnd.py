@@ -20,9 +20,13 @@ def kv():
     return kvtier
 
 
-@pytest.fixture()
-def ctx(kv):
+@pytest.fixture(params=[1, 0], ids=["tensormaps", "lanes"])
+def ctx(kv, request):
+    """Every case runs twice: HND sides moved by cp.async.bulk.tensor through per-slab tensor maps
+    (the default), and by the lane paths (cp.async row gather / 16-byte stores) alone."""
     c = kv.Ctx(0, staging_bytes=8 << 20)
+    c.set_option(kv.KV_OPT_TENSOR_MAPS, request.param)
+    c.tensor_maps = request.param
     yield c
     torch.cuda.synchronize()
     c.close()
@@ -191,11 +195,48 @@ def test_hnd_degenerate_orders_are_plain_copies(kv, ctx):
         assert np.array_equal(buf.cpu().numpy(), ko.pack(A, ids))
 
 
+def test_auto_with_tensor_maps_is_one_bulk_kernel(kv, ctx):
+    """AUTO with tensor maps (the default): every direction of an HND transfer is the bulk ring, whole-token
+    boxes moved by cp.async.bulk.tensor; the second call on the same pool reuses the cached maps."""
+    if not ctx.tensor_maps:
+        pytest.skip("tensor maps switched off in this parametrisation")
+    L, C, P, T, H, D, e, n = 3, 2, 64, 16, 4, 128, 2, 20
+    rng = np.random.default_rng(83)
+    A = host_pool(rng, L, C, P, T, H, D, e, order=HND)
+    N = host_pool(rng, L, C, P, T, H, D, e, order=ko.NHD)
+    tA, dA = to_device(A, kv, torch)
+    tN, dN = to_device(N, kv, torch)
+    ids = rng.choice(P, n, replace=False).astype(np.int32)
+    buf = torch.zeros(n * dA.page_bytes(), dtype=torch.uint8, device="cuda")
+    for _ in range(2):
+        kv.kv_pack(ctx, dA, L, ids, buf)
+        assert ctx.stat(kv.KV_STAT_LAST_KERNEL) == KERNELS["bulk"]
+        assert ctx.stat(kv.KV_STAT_LAST_TENSOR_MAPS) == 1
+        assert ctx.stat(kv.KV_STAT_LAST_SEGMENT) == 8192  # 120 rows of 16 KiB split once to cover the chip
+    want = ko.pack(A, ids)
+    assert np.array_equal(buf.cpu().numpy(), want)
+    kv.kv_unpack(ctx, buf, ids[::-1].copy(), dA, L, T, T, n * T)
+    assert ctx.stat(kv.KV_STAT_LAST_KERNEL) == KERNELS["bulk"] and ctx.stat(kv.KV_STAT_LAST_TENSOR_MAPS) == 1
+    ko.unpack(want, ids[::-1].copy(), A, Ts=T, n_tokens=n * T)
+    assert_pool_equal(tA, A)
+    kv.kv_repage(ctx, dA, ids, dN, ids, L, n * T)
+    assert ctx.stat(kv.KV_STAT_LAST_KERNEL) == KERNELS["bulk"] and ctx.stat(kv.KV_STAT_LAST_TENSOR_MAPS) == 1
+    ko.repage(A, ids, N, ids, n_tokens=n * T)
+    assert_pool_equal(tN, N)
+    kv.kv_repage(ctx, dN, ids, dA, ids, L, n * T)
+    assert ctx.stat(kv.KV_STAT_LAST_KERNEL) == KERNELS["bulk"] and ctx.stat(kv.KV_STAT_LAST_TENSOR_MAPS) == 1
+    ko.repage(N, ids, A, ids, n_tokens=n * T)
+    assert_pool_equal(tA, A)
+    kv.kv_pack(ctx, dN, L, ids, buf)  # NHD pool: nothing to transpose, no maps
+    assert ctx.stat(kv.KV_STAT_LAST_TENSOR_MAPS) == 0
+
+
 def test_auto_kernel_choice_per_direction(kv, ctx):
-    """AUTO (DESIGN.md "HND pools"): strided source only -> bulk ring (cp.async gather + bulk store);
-    strided destination -> vec (16-byte STG from many warps); NHD <-> NHD stays on the bulk path."""
+    """AUTO without tensor maps: strided source only -> bulk ring (cp.async gather +
+    bulk store); strided destination -> vec (16-byte STG from many warps); NHD <-> NHD stays on the bulk path."""
     L, C, P, T, H, D, e, n = 3, 2, 64, 16, 4, 128, 2, 20
     rng = np.random.default_rng(79)
+    ctx.set_option(kv.KV_OPT_TENSOR_MAPS, 0)
     A = host_pool(rng, L, C, P, T, H, D, e, order=HND)
     N = host_pool(rng, L, C, P, T, H, D, e, order=ko.NHD)
     tA, dA = to_device(A, kv, torch)
