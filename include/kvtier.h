@@ -160,6 +160,23 @@ int kv_last_cuda_error(kv_ctx *ctx); /* the cudaError_t behind the last KV_ERR_C
  * page id was out of range (that page was skipped). */
 int kv_device_status(kv_ctx *ctx, uint32_t *out);
 
+/* ---- peer GPU as a tier --------------------------------------------- */
+/* The single-box analogue of the provider-issued batched write of PAPER.md:L236 ("the consumer supplies
+ * destination-buffer descriptors, and the provider issues batched RDMA writes"): after kv_peer_enable, any
+ * pool slab or transfer buffer of a call may live on `peer_device`; the SAME kernels then load from / store
+ * to it over NVLink (UVA addresses, one-sided, no collective, no copy on the peer).  The push direction
+ * (kv_unpack / kv_repage from local memory into a peer pool: posted stores) is the fast one.
+ * Errors: KV_ERR_SIZE if peer_device is the ctx's own device or negative; KV_ERR_CUDA if the device does
+ * not exist, has no peer path to the ctx's device (cudaDeviceCanAccessPeer = 0) or enabling fails;
+ * KV_ERR_NO_DEVICE on a planning-only ctx.  Enabling twice is KV_OK.  The mapping lasts for the process. */
+int kv_peer_enable(kv_ctx *ctx, int peer_device);
+/* kv_signal: enqueue on `stream` a release-ordered, system-scope store of `value` to the 8-byte-aligned
+ * word `flag` (device memory of the ctx's device or of an enabled peer, or mapped pinned host memory).
+ * Stream order puts it after every transfer enqueued on `stream` before it, so a consumer on the peer GPU
+ * (or the host) that reads `flag` == value with an acquire load may read the transferred pages: the
+ * availability notification of PAPER.md:L234, without a host round trip.  Capturable. */
+int kv_signal(kv_ctx *ctx, uint64_t *flag, uint64_t value, kv_stream_t stream);
+
 /* ---- pinned host memory (the L2 CPU tier) ----------------------------------- */
 int kv_host_alloc(void **p, size_t bytes); /* page-locked, mapped, portable; free with kv_host_free */
 int kv_host_free(void *p);
