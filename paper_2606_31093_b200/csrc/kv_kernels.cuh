@@ -676,4 +676,14 @@ __global__ void __launch_bounds__(256) kv_move_elem(const __grid_constant__ JobT
   }
 }
 
+// ---------------------------------------------------------------------------------------------
+// kv_signal: the availability flag that follows a transfer in stream order (kvtier.h kv_signal).
+// fence.sc.sys orders every write this GPU performed before the launch (the previous kernels of the
+// stream have completed) ahead of the flag for observers anywhere in the system: a peer GPU or the host.
+// ---------------------------------------------------------------------------------------------
+__global__ void kv_signal_kernel(uint64_t *flag, uint64_t value) {
+  __threadfence_system();
+  asm volatile("st.release.sys.global.u64 [%0], %1;" ::"l"(flag), "l"(value) : "memory");
+}
+
 }  // namespace kvt

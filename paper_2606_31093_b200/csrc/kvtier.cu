@@ -1127,6 +1127,39 @@ int kv_device_status(kv_ctx *ctx, uint32_t *out) {
   return KV_OK;
 }
 
+int kv_peer_enable(kv_ctx *ctx, int peer_device) {
+  if (!ctx) return KV_ERR_NULL;
+  if (ctx->host_only) return KV_ERR_NO_DEVICE;
+  if (peer_device < 0 || peer_device == ctx->device) return KV_ERR_SIZE;
+  DeviceGuard guard(ctx);
+  int can = 0;
+  KV_CUDA(ctx, cudaDeviceCanAccessPeer(&can, ctx->device, peer_device));
+  if (!can) { ctx->last_cuda_error = (int)cudaErrorPeerAccessUnsupported; return KV_ERR_CUDA; }
+  cudaError_t e = cudaDeviceEnablePeerAccess(peer_device, 0);
+  if (e == cudaErrorPeerAccessAlreadyEnabled) { (void)cudaGetLastError(); e = cudaSuccess; }
+  KV_CUDA(ctx, e);
+  return KV_OK;
+}
+
+int kv_signal(kv_ctx *ctx, uint64_t *flag, uint64_t value, kv_stream_t stream) {
+  if (!ctx || !flag) return KV_ERR_NULL;
+  if ((uint64_t)(uintptr_t)flag % 8) return KV_ERR_ALIGN;
+  if (ctx->host_only) return KV_ERR_NO_DEVICE;
+  DeviceGuard guard(ctx);
+  uint64_t *dev = flag;
+  cudaPointerAttributes a;
+  if (cudaPointerGetAttributes(&a, flag) != cudaSuccess) { (void)cudaGetLastError(); return KV_ERR_HOST_MEM; }
+  if (a.type == cudaMemoryTypeUnregistered) return KV_ERR_HOST_MEM;  // pageable host memory
+  if (a.type == cudaMemoryTypeHost) {
+    if (!a.devicePointer) return KV_ERR_HOST_MEM;
+    dev = (uint64_t *)a.devicePointer;
+  }
+  kvt::kv_signal_kernel<<<1, 1, 0, (cudaStream_t)stream>>>(dev, value);
+  KV_CUDA(ctx, cudaGetLastError());
+  ctx->launches++;
+  return KV_OK;
+}
+
 int kv_host_alloc(void **p, size_t bytes) {
   if (!p) return KV_ERR_NULL;
   *p = nullptr;

@@ -77,6 +77,8 @@ _kv_ctx_set_option = _sig("kv_ctx_set_option", _int, _vp, _int, _i64)
 _kv_ctx_get_stat = _sig("kv_ctx_get_stat", _int, _vp, _int, ctypes.POINTER(_u64))
 _kv_last_cuda_error = _sig("kv_last_cuda_error", _int, _vp)
 _kv_device_status = _sig("kv_device_status", _int, _vp, ctypes.POINTER(_u32))
+_kv_peer_enable = _sig("kv_peer_enable", _int, _vp, _int)
+_kv_signal = _sig("kv_signal", _int, _vp, _vp, _u64, _vp)
 _kv_host_alloc = _sig("kv_host_alloc", _int, ctypes.POINTER(_vp), _sz)
 _kv_host_free = _sig("kv_host_free", _int, _vp)
 _kv_host_register = _sig("kv_host_register", _int, _vp, _sz)
@@ -266,6 +268,17 @@ def kv_ctx_create(device: int = 0, staging_bytes: int = 0) -> Ctx:
 
 def kv_ctx_destroy(ctx: Ctx):
     ctx.close()
+
+
+def kv_peer_enable(ctx: Ctx, peer_device: int):
+    """Map `peer_device`'s memory into the ctx's device (NVLink P2P); pools/buffers may then live there."""
+    _chk(ctx, _kv_peer_enable(ctx.h, int(peer_device)))
+
+
+def kv_signal(ctx: Ctx, flag, value: int, stream=None):
+    """Release-ordered system-scope store of `value` to the 8-byte word `flag` (tensor or address), after
+    every transfer already enqueued on the stream."""
+    _chk(ctx, _kv_signal(ctx.h, _ptr(flag), int(value), _stream(stream)))
 
 
 def kv_host_alloc(nbytes: int) -> int:

@@ -246,3 +246,22 @@ def test_plan_hnd_pools(ctx):
     assert ctx.stat(kv.KV_STAT_LAST_KERNEL) == kv.KV_KERNEL_BULK
     assert ctx.stat(kv.KV_STAT_LAST_SEGMENT) == 4096  # the whole 4 KiB row
     assert status_of(lambda: kv.kv_pack(ctx, pool(2), s.L, [1], BUF, dst_bytes=1 << 40)) == kv.KV_ERR_DESC
+
+
+def test_peer_and_signal_argument_errors(ctx):
+    """SURVEY.md 8(f) NEXT-3 entries on a planning-only ctx: argument errors come first, then
+    KV_ERR_NO_DEVICE (nothing is launched, no CUDA call is made)."""
+    with pytest.raises(kv.KvError) as ei:
+        kv.kv_peer_enable(ctx, 1)
+    assert ei.value.status == kv.KV_ERR_NO_DEVICE
+    word = np.zeros(2, dtype=np.uint64)
+    with pytest.raises(kv.KvError) as ei:
+        kv.kv_signal(ctx, None, 1, stream=0)
+    assert ei.value.status == kv.KV_ERR_NULL
+    with pytest.raises(kv.KvError) as ei:
+        kv.kv_signal(ctx, int(word.ctypes.data) + 4, 1, stream=0)
+    assert ei.value.status == kv.KV_ERR_ALIGN
+    with pytest.raises(kv.KvError) as ei:
+        kv.kv_signal(ctx, word, 1, stream=0)
+    assert ei.value.status == kv.KV_ERR_NO_DEVICE
+    assert word[0] == 0

@@ -284,3 +284,113 @@ def test_cuda_graph_large_transfer_host_ids_and_direct_offload(kv, ctx):
     finally:
         torch.cuda.synchronize()
         kv.kv_host_free(hp)
+
+
+# ------------------------------------------------------------------------------------------------
+# availability flag after a transfer, peer mapping (one GPU here: the flag and
+# error paths; the data path of a peer pool is the same kernels on UVA addresses)
+# ------------------------------------------------------------------------------------------------
+def test_signal_follows_the_transfer_in_stream_order(kv, ctx):
+    L, C, P, T, H, D, e = 4, 2, 256, 16, 4, 128, 2
+    rng = np.random.default_rng(89)
+    A = host_pool(rng, L, C, P, T, H, D, e)
+    B = host_pool(rng, L, C, P, T, H, D, e)
+    tA, dA = to_device(A, kv, torch)
+    tB, dB = to_device(B, kv, torch)
+    n = 200
+    src = rng.choice(P, n, replace=False).astype(np.int32)
+    dst = rng.permutation(P)[:n].astype(np.int32)
+    buf = torch.zeros(n * dA.page_bytes(), dtype=torch.uint8, device="cuda")
+    dflag = torch.zeros(1, dtype=torch.int64, device="cuda")
+    hflag_p = kv.kv_host_alloc(64)
+    hflag = kv.host_view(hflag_p, 64).view(np.uint64)
+    hflag[:] = 0
+    try:
+        side = torch.cuda.Stream()
+        kv.kv_pack(ctx, dA, L, src, buf, stream=side)
+        kv.kv_unpack(ctx, buf, dst, dB, L, T, T, n * T, stream=side)
+        kv.kv_signal(ctx, dflag, 0x1234_5678_9ABC_DEF0, stream=side)
+        kv.kv_signal(ctx, hflag_p, 7, stream=side)
+        import time
+        t0 = time.time()
+        while hflag[0] != 7:  # the host polls the mapped word: no stream synchronisation
+            assert time.time() - t0 < 10, "flag never arrived"
+        # the flag was stored after the transfer's kernels completed: a copy on ANOTHER stream, started
+        # only now, already sees every unpacked page
+        other = torch.cuda.Stream()
+        with torch.cuda.stream(other):
+            snap = [t.clone() for t in tB]
+        other.synchronize()
+        ko.unpack(ko.pack(A, src), dst, B, Ts=T, n_tokens=n * T)
+        assert_pool_equal(snap, B)
+        side.synchronize()
+        assert int(dflag.item()) == 0x1234_5678_9ABC_DEF0
+        pageable = np.zeros(1, dtype=np.uint64)
+        with pytest.raises(kv.KvError) as ei:
+            kv.kv_signal(ctx, pageable, 1)
+        assert ei.value.status == kv.KV_ERR_HOST_MEM
+    finally:
+        torch.cuda.synchronize()
+        kv.kv_host_free(hflag_p)
+
+
+def test_peer_enable_errors_on_this_box(kv, ctx):
+    with pytest.raises(kv.KvError) as ei:
+        kv.kv_peer_enable(ctx, 0)  # the ctx's own device
+    assert ei.value.status == kv.KV_ERR_SIZE
+    with pytest.raises(kv.KvError) as ei:
+        kv.kv_peer_enable(ctx, -1)
+    assert ei.value.status == kv.KV_ERR_SIZE
+    n = torch.cuda.device_count()
+    with pytest.raises(kv.KvError) as ei:
+        kv.kv_peer_enable(ctx, n)  # no such device
+    assert ei.value.status == kv.KV_ERR_CUDA
+    if n > 1 and torch.cuda.can_device_access_peer(0, 1):  # exercised only where a second GPU is visible
+        kv.kv_peer_enable(ctx, 1)
+        kv.kv_peer_enable(ctx, 1)  # twice is fine
+        L, C, P, T, H, D, e = 2, 2, 64, 16, 4, 128, 2
+        rng = np.random.default_rng(97)
+        A = host_pool(rng, L, C, P, T, H, D, e)
+        B = host_pool(rng, L, C, P, T, H, D, e)
+        tA, dA = to_device(A, kv, torch)
+        tB = [torch.from_numpy(x).to("cuda:1") for x in B.slabs]
+        dB = kv.PoolDesc(tB, L, C, P, T, H, D, e)
+        ids = rng.choice(P, 20, replace=False).astype(np.int32)
+        buf = torch.zeros(20 * dA.page_bytes(), dtype=torch.uint8, device="cuda:0")
+        kv.kv_pack(ctx, dA, L, ids, buf)
+        kv.kv_unpack(ctx, buf, ids, dB, L, T, T, 20 * T)  # push into the peer's pool over NVLink
+        torch.cuda.synchronize(0)
+        ko.unpack(ko.pack(A, ids), ids, B, Ts=T, n_tokens=20 * T)
+        assert_pool_equal(tB, B)
+
+
+def test_cuda_graph_capture_of_hnd_transfer_uses_cached_tensor_maps(kv, ctx):
+    """Tensor maps are built (device allocation + blocking copy) on a pool's first use, which a capturing
+    stream cannot do: a first-ever captured HND call takes the lane paths, a warmed-up one the maps."""
+    L, C, P, T, H, D, e = 3, 2, 128, 16, 4, 128, 2
+    rng = np.random.default_rng(101)
+    A = host_pool(rng, L, C, P, T, H, D, e, order=ko.HND)
+    tA, dA = to_device(A, kv, torch)
+    n = 60
+    ids = rng.choice(P, n, replace=False).astype(np.int32)
+    buf = torch.zeros(n * dA.page_bytes(), dtype=torch.uint8, device="cuda")
+    want = ko.pack(A, ids)
+    side = torch.cuda.Stream()
+    g = torch.cuda.CUDAGraph()
+    with torch.cuda.graph(g, stream=side):
+        kv.kv_pack(ctx, dA, L, ids, buf, stream=side)
+    assert ctx.stat(kv.KV_STAT_LAST_TENSOR_MAPS) == 0
+    g.replay()
+    torch.cuda.synchronize()
+    assert np.array_equal(buf.cpu().numpy(), want)
+    kv.kv_pack(ctx, dA, L, ids, buf)  # live call builds and caches the maps
+    assert ctx.stat(kv.KV_STAT_LAST_TENSOR_MAPS) == 1
+    torch.cuda.synchronize()
+    g2 = torch.cuda.CUDAGraph()
+    with torch.cuda.graph(g2, stream=side):
+        kv.kv_pack(ctx, dA, L, ids, buf, stream=side)
+    assert ctx.stat(kv.KV_STAT_LAST_TENSOR_MAPS) == 1
+    buf.zero_()
+    g2.replay()
+    torch.cuda.synchronize()
+    assert np.array_equal(buf.cpu().numpy(), want)
