@@ -222,3 +222,49 @@ def sweep_sizes_pages(max_bytes: int = 8 << 30) -> List[int]:
         out.append(n)
         n *= 2
     return out
+
+
+# --------------------------------------------------------------------------------------------
+# content identities for chained paged hashing
+# --------------------------------------------------------------------------------------------
+VOCAB = 151_936  # text token ids are drawn below this (a Qwen-sized vocabulary; only the range matters)
+
+
+@dataclass
+class IdentityBatch:
+    ident: np.ndarray        # uint64[total tokens]: one content identity per token position
+    tok_offsets: np.ndarray  # int64[S+1] CSR over sessions
+    shared_prefix: np.ndarray  # int64[S]: tokens each session shares with session 0 (0 for session 0)
+
+
+def identity_batch(seed: int = 0, lens=None, n_sessions: int = 64, lo: int = 512, hi: int = 16384,
+                   share: float = 0.5) -> IdentityBatch:
+    """One 64-bit identity per token: a text position carries its token id, every position of an image /
+    audio placeholder span carries that item's (random 64-bit) content hash id.  Span structure as in
+    config 3 (spans of 256-1,024 positions, half the mass text).  With probability `share` a session
+    starts with a copy of a random-length prefix of session 0 (cross-session reuse: equal page-aligned
+    prefixes must get equal page ids); the copy length is recorded, not consumed by the hash."""
+    rng = np.random.default_rng(seed)
+    if lens is None:
+        lens = np.floor(np.exp(rng.uniform(math.log(lo), math.log(hi), size=n_sessions))).astype(np.int64)
+    lens = np.asarray(lens, dtype=np.int64)
+    off = np.zeros(len(lens) + 1, dtype=np.int64)
+    np.cumsum(lens, out=off[1:])
+    ident = np.zeros(int(off[-1]), dtype=np.uint64)
+    shared = np.zeros(len(lens), dtype=np.int64)
+    for s, n in enumerate(lens):
+        a = ident[off[s]:off[s + 1]]
+        pos = 0
+        while pos < n:
+            if rng.random() < 0.5:  # a multimodal item
+                ln = min(int(rng.integers(256, 1025)), int(n) - pos)
+                a[pos:pos + ln] = rng.integers(0, 2**64, dtype=np.uint64)
+            else:
+                ln = min(int(rng.integers(8, 513)), int(n) - pos)
+                a[pos:pos + ln] = rng.integers(0, VOCAB, size=ln).astype(np.uint64)
+            pos += ln
+        if s > 0 and rng.random() < share:
+            k = int(rng.integers(1, min(int(n), int(lens[0])) + 1))
+            a[:k] = ident[off[0]:off[0] + k]
+            shared[s] = k
+    return IdentityBatch(ident, off, shared)
