@@ -177,6 +177,31 @@ int kv_peer_enable(kv_ctx *ctx, int peer_device);
  * availability notification of PAPER.md:L234, without a host round trip.  Capturable. */
 int kv_signal(kv_ctx *ctx, uint64_t *flag, uint64_t value, kv_stream_t stream);
 
+/* ---- chained paged hashing ------------------------------------------ */
+/* "each page ID hashes its predecessor together with the current page's content
+ * identities, thereby representing the complete page-aligned prefix" -- the 64-bit ids under which KV pages
+ * are published and looked up (not the int32 pool slots the transfers take).  The paper names no hash;
+ * this library fixes (readings H1-H4): one 64-bit content identity per token position; 64-bit
+ * FNV-1a, byte-serial, little-endian encodings;
+ *     digest_k = FNV1a(identities of page k, 8*page_size bytes)
+ *     id_k     = FNV1a(LE64(id_{k-1}) || LE64(digest_k)),   id_{-1} = roots[s] (KV_CHAIN_ROOT if roots == NULL)
+ * and only whole pages get ids: session s yields floor(len_s / page_size) of them.
+ *   ident         DEVICE uint64[tok_offsets[n_sessions]], 8-byte aligned; session s owns
+ *                 [tok_offsets[s], tok_offsets[s+1])
+ *   tok_offsets   HOST int64[n_sessions+1], non-negative, non-decreasing (consumed before return)
+ *   roots         HOST uint64[n_sessions] or NULL
+ *   out           DEVICE uint64[out_capacity]; ids of session s start at page_offsets[s] (sessions back to back)
+ *   page_offsets  HOST int64[n_sessions+1], written by the call (may be NULL)
+ * Two launches on `stream` (per-page digests in parallel, then one warp per session along the chain);
+ * results are defined after the caller synchronises `stream`.  Errors: KV_ERR_NULL, KV_ERR_SIZE (page_size
+ * 0, bad offsets, out_capacity too small), KV_ERR_ALIGN, KV_ERR_CAPTURE (not capturable), KV_ERR_NO_DEVICE
+ * (planning-only ctx; page_offsets are still written), KV_ERR_CUDA.  n_sessions == 0 or no whole page:
+ * KV_OK, nothing launched. */
+#define KV_CHAIN_ROOT 0xcbf29ce484222325ull
+int kv_chain_hash(kv_ctx *ctx, const uint64_t *ident, const int64_t *tok_offsets, uint32_t n_sessions,
+                  uint32_t page_size, const uint64_t *roots, uint64_t *out, size_t out_capacity,
+                  int64_t *page_offsets, kv_stream_t stream);
+
 /* ---- pinned host memory (the L2 CPU tier) ----------------------------------- */
 int kv_host_alloc(void **p, size_t bytes); /* page-locked, mapped, portable; free with kv_host_free */
 int kv_host_free(void *p);

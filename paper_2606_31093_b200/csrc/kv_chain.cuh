@@ -1,0 +1,86 @@
+// kv_chain.cuh -- chained paged hashing on the GPU (kvtier.h
+// kv_chain_hash).  id_k = FNV1a64(LE64(id_{k-1}) || LE64(digest_k)), digest_k = FNV1a64 of the 8*T
+// little-endian bytes of page k's T content identities; id_{-1} = the session's root.
+//
+// The work splits where the dependence does:
+//   kv_chain_digest  one THREAD per page, all pages of all sessions at once: 8*T dependent
+//                    xor/multiply steps per page, no dependence between pages -- the parallel 8/9ths.
+//   kv_chain_link    one WARP per session: the chain proper, 16 dependent steps per page.  The 32 lanes
+//                    fetch 32 digests with one coalesced load, every lane then walks the same 32 links
+//                    (digest handed round by shuffle), lane i keeps link i, and the 32 ids leave with
+//                    one coalesced store.  Serial along the chain, parallel across sessions -- as the
+//                    definition is.
+// Both are bound by the latency of dependent integer multiplies, not by memory (8 B read per token
+// against 98,304 B of KV the same token owns).  Shares nothing with oracle/.
+#pragma once
+#include <cuda_runtime.h>
+#include <stdint.h>
+
+namespace kvt {
+
+constexpr uint64_t kFnvBasis = 0xcbf29ce484222325ull;
+constexpr uint64_t kFnvPrime = 0x100000001b3ull;
+
+// eight byte-serial FNV-1a steps over the little-endian bytes of w
+__device__ __forceinline__ uint64_t fnv1a_word(uint64_t h, uint64_t w) {
+#pragma unroll
+  for (int b = 0; b < 8; ++b) {
+    h ^= (w >> (8 * b)) & 0xffull;
+    h *= kFnvPrime;
+  }
+  return h;
+}
+
+struct ChainJob {
+  const uint64_t *ident;     // device: identities of all sessions
+  uint64_t *out;             // device: digests (after kv_chain_digest), then ids (after kv_chain_link)
+  const int64_t *tok_off;    // device [S+1]
+  const int64_t *page_off;   // device [S+1]
+  const uint64_t *roots;     // device [S] or nullptr
+  uint64_t default_root;
+  uint64_t total_pages;
+  uint32_t n_sessions;
+  uint32_t T;
+};
+
+__global__ void __launch_bounds__(128) kv_chain_digest(const ChainJob j) {
+  const uint64_t p = (uint64_t)blockIdx.x * blockDim.x + threadIdx.x;
+  if (p >= j.total_pages) return;
+  uint32_t lo = 0, hi = j.n_sessions;  // largest s with page_off[s] <= p
+  while (hi - lo > 1) {
+    const uint32_t mid = (lo + hi) >> 1;
+    if ((uint64_t)__ldg(j.page_off + mid) <= p) lo = mid; else hi = mid;
+  }
+  const uint64_t k = p - (uint64_t)__ldg(j.page_off + lo);
+  const uint64_t *src = j.ident + (uint64_t)__ldg(j.tok_off + lo) + k * j.T;
+  uint64_t h = kFnvBasis;
+  uint32_t t = 0;
+  for (; t + 4 <= j.T; t += 4) {  // four loads in flight ahead of the dependent arithmetic
+    const uint64_t w0 = __ldg(src + t), w1 = __ldg(src + t + 1), w2 = __ldg(src + t + 2), w3 = __ldg(src + t + 3);
+    h = fnv1a_word(fnv1a_word(fnv1a_word(fnv1a_word(h, w0), w1), w2), w3);
+  }
+  for (; t < j.T; ++t) h = fnv1a_word(h, __ldg(src + t));
+  j.out[p] = h;
+}
+
+__global__ void __launch_bounds__(32) kv_chain_link(const ChainJob j) {
+  const uint32_t s = blockIdx.x, lane = threadIdx.x;
+  if (s >= j.n_sessions) return;
+  const uint64_t p0 = (uint64_t)__ldg(j.page_off + s), p1 = (uint64_t)__ldg(j.page_off + s + 1);
+  uint64_t prev = j.roots ? __ldg(j.roots + s) : j.default_root;
+  uint64_t next_d = p0 + lane < p1 ? j.out[p0 + lane] : 0;
+  for (uint64_t base = p0; base < p1; base += 32) {
+    const uint64_t d = next_d;
+    if (base + 32 + lane < p1) next_d = j.out[base + 32 + lane];  // prefetch the next 32 digests
+    const uint32_t n = (uint32_t)min((uint64_t)32, p1 - base);
+    uint64_t mine = 0;
+    for (uint32_t i = 0; i < n; ++i) {  // every lane walks the same links: no divergence, no broadcast of ids
+      const uint64_t di = __shfl_sync(0xffffffffu, d, i);
+      prev = fnv1a_word(fnv1a_word(kFnvBasis, prev), di);
+      if (i == lane) mine = prev;
+    }
+    if (lane < n) j.out[base + lane] = mine;
+  }
+}
+
+}  // namespace kvt

@@ -14,6 +14,7 @@
 #include <numeric>
 #include <vector>
 
+#include "kv_chain.cuh"
 #include "kv_kernels.cuh"
 
 namespace {
@@ -1157,6 +1158,56 @@ int kv_signal(kv_ctx *ctx, uint64_t *flag, uint64_t value, kv_stream_t stream) {
   kvt::kv_signal_kernel<<<1, 1, 0, (cudaStream_t)stream>>>(dev, value);
   KV_CUDA(ctx, cudaGetLastError());
   ctx->launches++;
+  return KV_OK;
+}
+
+int kv_chain_hash(kv_ctx *ctx, const uint64_t *ident, const int64_t *tok_offsets, uint32_t n_sessions,
+                  uint32_t page_size, const uint64_t *roots, uint64_t *out, size_t out_capacity,
+                  int64_t *page_offsets, kv_stream_t stream) {
+  if (!ctx) return KV_ERR_NULL;
+  if (!page_size) return KV_ERR_SIZE;
+  if (n_sessions && !tok_offsets) return KV_ERR_NULL;
+  std::vector<int64_t> poff((size_t)n_sessions + 1, 0);
+  for (uint32_t s = 0; s < n_sessions; ++s) {
+    if (tok_offsets[s] < 0 || tok_offsets[s + 1] < tok_offsets[s]) return KV_ERR_SIZE;
+    poff[s + 1] = poff[s] + (tok_offsets[s + 1] - tok_offsets[s]) / (int64_t)page_size;
+  }
+  const uint64_t total = (uint64_t)poff[n_sessions];
+  if (total > out_capacity) return KV_ERR_SIZE;
+  if (page_offsets) std::memcpy(page_offsets, poff.data(), poff.size() * sizeof(int64_t));
+  ctx->last_items = total;
+  if (!total) return KV_OK;
+  if (!ident || !out) return KV_ERR_NULL;
+  if (((uint64_t)(uintptr_t)ident | (uint64_t)(uintptr_t)out) % 8) return KV_ERR_ALIGN;
+  if (ctx->host_only) return KV_ERR_NO_DEVICE;
+  cudaStream_t s = (cudaStream_t)stream;
+  DeviceGuard guard(ctx);
+  if (capturing(s)) return KV_ERR_CAPTURE;
+  // tables: [tok_off: S+1][page_off: S+1][roots: S], staged through the pinned ring
+  HostBlob hb;
+  const size_t n1 = (size_t)n_sessions + 1;
+  hb.bytes.resize((2 * n1 + (roots ? n_sessions : 0)) * 8);
+  std::memcpy(hb.bytes.data(), tok_offsets, n1 * 8);
+  std::memcpy(hb.bytes.data() + n1 * 8, poff.data(), n1 * 8);
+  if (roots) std::memcpy(hb.bytes.data() + 2 * n1 * 8, roots, (size_t)n_sessions * 8);
+  Blob b;
+  int rc = upload_blob(ctx, hb, nullptr, true, s, &b);
+  if (rc) return rc;
+  kvt::ChainJob j{};
+  j.ident = ident; j.out = out;
+  j.tok_off = (const int64_t *)b.slot->d;
+  j.page_off = j.tok_off + n1;
+  j.roots = roots ? (const uint64_t *)(j.page_off + n1) : nullptr;
+  j.default_root = KV_CHAIN_ROOT;
+  j.total_pages = total; j.n_sessions = n_sessions; j.T = page_size;
+  const uint64_t blocks = (total + 127) / 128;
+  if (blocks > 0x7fffffffull) return KV_ERR_SIZE;
+  kvt::kv_chain_digest<<<(uint32_t)blocks, 128, 0, s>>>(j);
+  KV_CUDA(ctx, cudaGetLastError());
+  kvt::kv_chain_link<<<n_sessions, 32, 0, s>>>(j);
+  KV_CUDA(ctx, cudaGetLastError());
+  ctx->launches += 2;
+  KV_CUDA(ctx, cudaEventRecord(b.slot->ev, s));
   return KV_OK;
 }
 

@@ -79,6 +79,7 @@ _kv_last_cuda_error = _sig("kv_last_cuda_error", _int, _vp)
 _kv_device_status = _sig("kv_device_status", _int, _vp, ctypes.POINTER(_u32))
 _kv_peer_enable = _sig("kv_peer_enable", _int, _vp, _int)
 _kv_signal = _sig("kv_signal", _int, _vp, _vp, _u64, _vp)
+_kv_chain_hash = _sig("kv_chain_hash", _int, _vp, _vp, _vp, _u32, _u32, _vp, _vp, _sz, _vp, _vp)
 _kv_host_alloc = _sig("kv_host_alloc", _int, ctypes.POINTER(_vp), _sz)
 _kv_host_free = _sig("kv_host_free", _int, _vp)
 _kv_host_register = _sig("kv_host_register", _int, _vp, _sz)
@@ -279,6 +280,25 @@ def kv_signal(ctx: Ctx, flag, value: int, stream=None):
     """Release-ordered system-scope store of `value` to the 8-byte word `flag` (tensor or address), after
     every transfer already enqueued on the stream."""
     _chk(ctx, _kv_signal(ctx.h, _ptr(flag), int(value), _stream(stream)))
+
+
+KV_CHAIN_ROOT = 0xCBF29CE484222325
+
+
+def kv_chain_hash(ctx: Ctx, ident, tok_offsets, page_size: int, out, roots=None, out_capacity=None,
+                  stream=None) -> np.ndarray:
+    """Chained page ids of all sessions into the device tensor `out`; returns the page
+    offsets (int64[S+1]).  `ident` / `out` are device tensors (or addresses), offsets / roots host arrays."""
+    off = np.ascontiguousarray(np.asarray(tok_offsets, dtype=np.int64))
+    S = max(int(off.size) - 1, 0)
+    poff = np.zeros(S + 1, dtype=np.int64)
+    r = None if roots is None else _u64_array(roots)
+    cap = (int(out.numel()) if hasattr(out, "numel") else 0) if out_capacity is None else int(out_capacity)
+    rc = _kv_chain_hash(ctx.h, _ptr(ident), int(off.ctypes.data) if off.size else None, S, int(page_size),
+                        None if r is None else int(r.ctypes.data), _ptr(out), cap, int(poff.ctypes.data),
+                        _stream(stream))
+    _chk(ctx, rc)
+    return poff
 
 
 def kv_host_alloc(nbytes: int) -> int:

@@ -265,3 +265,32 @@ def test_peer_and_signal_argument_errors(ctx):
         kv.kv_signal(ctx, word, 1, stream=0)
     assert ei.value.status == kv.KV_ERR_NO_DEVICE
     assert word[0] == 0
+
+
+def test_chain_hash_planning_and_errors(ctx):
+    """kv_chain_hash on a planning-only ctx: offsets are validated and page offsets written (H4: whole
+    pages only), then KV_ERR_NO_DEVICE; nothing is dereferenced on the device side."""
+    ident, out = 0x1000, 0x2000  # never touched without a device
+    with pytest.raises(kv.KvError) as ei:
+        kv.kv_chain_hash(ctx, ident, [0, 40, 40, 75], 16, out, out_capacity=4)
+    assert ei.value.status == kv.KV_ERR_NO_DEVICE
+    assert ctx.stat(kv.KV_STAT_LAST_ITEMS) == 4  # 2 + 0 + 2 whole pages
+    with pytest.raises(kv.KvError) as ei:
+        kv.kv_chain_hash(ctx, ident, [0, 40, 40, 75], 16, out, out_capacity=3)
+    assert ei.value.status == kv.KV_ERR_SIZE
+    for bad in ([0, 5, 3], [-1, 4]):
+        with pytest.raises(kv.KvError) as ei:
+            kv.kv_chain_hash(ctx, ident, bad, 1, out, out_capacity=100)
+        assert ei.value.status == kv.KV_ERR_SIZE
+    with pytest.raises(kv.KvError) as ei:
+        kv.kv_chain_hash(ctx, ident, [0, 16], 0, out, out_capacity=1)
+    assert ei.value.status == kv.KV_ERR_SIZE
+    with pytest.raises(kv.KvError) as ei:
+        kv.kv_chain_hash(ctx, ident + 4, [0, 16], 16, out, out_capacity=1)
+    assert ei.value.status == kv.KV_ERR_ALIGN
+    with pytest.raises(kv.KvError) as ei:
+        kv.kv_chain_hash(ctx, None, [0, 16], 16, out, out_capacity=1)
+    assert ei.value.status == kv.KV_ERR_NULL
+    # nothing to hash: KV_OK even without a device
+    assert kv.kv_chain_hash(ctx, None, [0, 15, 15], 16, None, out_capacity=0).tolist() == [0, 0, 0]
+    assert kv.kv_chain_hash(ctx, None, [0], 16, None, out_capacity=0).tolist() == [0]

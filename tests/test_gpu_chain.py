@@ -1,0 +1,103 @@
+"""GPU parity of kv_chain_hash (PAPER.md:L276 chained paged hashing) against
+oracle/chain_oracle: 64-bit ids, bit-exact, on the same seeded identity batches."""
+import numpy as np
+import pytest
+
+torch = pytest.importorskip("torch")
+pytestmark = pytest.mark.gpu
+
+from oracle import chain_oracle as co  # noqa: E402
+from paper_2606_31093_b200 import workloads as W  # noqa: E402
+
+
+@pytest.fixture(scope="module")
+def kv():
+    if not torch.cuda.is_available():
+        pytest.skip("no CUDA device")
+    from paper_2606_31093_b200 import kvtier
+    return kvtier
+
+
+@pytest.fixture()
+def ctx(kv):
+    c = kv.Ctx(0)
+    yield c
+    torch.cuda.synchronize()
+    c.close()
+
+
+def run(kv, ctx, ident, off, T, roots=None, slack=3):
+    d_ident = torch.from_numpy(np.ascontiguousarray(ident).view(np.int64)).cuda()
+    n = int((np.diff(off) // T).sum())
+    out = torch.full((n + slack,), -1, dtype=torch.int64, device="cuda")
+    poff = kv.kv_chain_hash(ctx, d_ident, off, T, out, roots=roots)
+    torch.cuda.synchronize()
+    got = out.cpu().numpy().view(np.uint64)
+    assert (got[n:] == np.uint64(2**64 - 1)).all(), "wrote past the last id"
+    return got[:n], poff
+
+
+@pytest.mark.parametrize("T", [16, 64, 1, 5, 33])
+@pytest.mark.parametrize("seed,S,lo,hi", [(0, 64, 512, 16384), (1, 7, 1, 300), (2, 200, 16, 700)])
+def test_chain_hash_equals_oracle(kv, ctx, T, seed, S, lo, hi):
+    wb = W.identity_batch(seed=seed, n_sessions=S, lo=lo, hi=hi)
+    want, wpoff = co.chain_batched(wb.ident, wb.tok_offsets, T)
+    got, poff = run(kv, ctx, wb.ident, wb.tok_offsets, T)
+    assert np.array_equal(poff, wpoff)
+    assert np.array_equal(got, want)
+    roots = np.random.default_rng(seed).integers(0, 2**64, size=S, dtype=np.uint64)
+    want_r, _ = co.chain_batched(wb.ident, wb.tok_offsets, T, roots)
+    got_r, _ = run(kv, ctx, wb.ident, wb.tok_offsets, T, roots=roots)
+    assert np.array_equal(got_r, want_r)
+    assert not np.array_equal(got_r, got) or got.size == 0
+
+
+def test_config3_session_and_config4_batch_shapes(kv, ctx):
+    """The paper-shaped inputs: one 50-turn session's 46k-token history (2,875 ids, one long chain) and
+    the 64-request batch of config 4 (288,990 tokens, 18,059 whole pages)."""
+    turns = W.session_turns(seed=0)
+    one = W.identity_batch(seed=3, lens=[turns[-1].cum_tokens])
+    got, poff = run(kv, ctx, one.ident, one.tok_offsets, 16)
+    assert poff.tolist() == [0, turns[-1].cum_tokens // 16]
+    assert np.array_equal(got, co.chain(one.ident, 16))
+    c4 = W.batch_case(seed=0)
+    wb = W.identity_batch(seed=4, lens=c4.lens)
+    got, poff = run(kv, ctx, wb.ident, wb.tok_offsets, 16)
+    want, wpoff = co.chain_batched(wb.ident, wb.tok_offsets, 16, threads=8)
+    assert np.array_equal(poff, wpoff) and np.array_equal(got, want)
+    # cross-session reuse: sessions that copied a prefix of session 0 share its leading ids
+    for s in np.nonzero(wb.shared_prefix)[0]:
+        k = min(int(wb.shared_prefix[s]) // 16, int(poff[1] - poff[0]), int(poff[s + 1] - poff[s]))
+        assert np.array_equal(got[poff[s]:poff[s] + k], got[:k])
+
+
+def test_empty_sessions_tails_and_offsets_not_at_zero(kv, ctx):
+    rng = np.random.default_rng(9)
+    ident = rng.integers(0, 2**64, size=500, dtype=np.uint64)
+    off = np.array([7, 7, 22, 23, 23, 300, 500], dtype=np.int64)  # first session starts at token 7
+    want, wpoff = co.chain_batched(ident, off, 16)
+    got, poff = run(kv, ctx, ident, off, 16)
+    assert np.array_equal(poff, wpoff) and np.array_equal(got, want)
+    assert poff.tolist() == [0, 0, 0, 0, 0, 17, 29]
+    # the worked value of tests/test_chain_oracle_pins.py (identity 0x61, T = 1, root 0)
+    got, _ = run(kv, ctx, np.array([0x61], dtype=np.uint64), [0, 1], 1, roots=[0])
+    assert got.tolist() == co.chain_py([0x61], 1, root=0)
+
+
+def test_errors_write_nothing_and_capture_is_refused(kv, ctx):
+    ident = torch.zeros(64, dtype=torch.int64, device="cuda")
+    out = torch.full((4,), -1, dtype=torch.int64, device="cuda")
+    with pytest.raises(kv.KvError) as ei:
+        kv.kv_chain_hash(ctx, ident, [0, 64], 8, out, out_capacity=4)  # needs 8 ids
+    assert ei.value.status == kv.KV_ERR_SIZE
+    torch.cuda.synchronize()
+    assert (out == -1).all()
+    side = torch.cuda.Stream()
+    g = torch.cuda.CUDAGraph()
+    with torch.cuda.graph(g, stream=side):
+        with pytest.raises(kv.KvError) as ei:
+            kv.kv_chain_hash(ctx, ident, [0, 64], 16, out, stream=side)
+        assert ei.value.status == kv.KV_ERR_CAPTURE
+        ident.add_(0)  # a graph needs at least one node
+    torch.cuda.synchronize()
+    assert (out == -1).all()
