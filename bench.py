@@ -335,6 +335,31 @@ def run_ours(args):
         from paper_2606_31093_b200 import report
 
         line["report"] = report.run(ctx, desc, shape, [t.view(torch.uint8) for t in slabs], args.seed, hbm_peak=peak)
+        # the oracle of the NEXT-4 row timed beside the GPU records (cpu_baseline leg: the one place bench.py runs oracle/)
+        from oracle import chain_oracle as co
+
+        cores = len(os.sched_getaffinity(0))
+        turns = W.session_turns(args.seed)
+        chain_oracle = {}
+        for name, wb in (("config 3: one 50-turn session history (a single chain)", W.identity_batch(args.seed + 3, lens=[turns[-1].cum_tokens])),
+                         ("config 4: 64 requests, log-uniform 512-16,384 tokens", W.identity_batch(args.seed + 4, lens=W.batch_case(args.seed).lens)),
+                         ("4,096 sessions, log-uniform 512-16,384 tokens", W.identity_batch(args.seed + 5, n_sessions=4096))):
+            ts = {}
+            for th in (1, cores):
+                best = 1e30
+                for _ in range(3):
+                    t0 = time.perf_counter()
+                    co.chain_batched(wb.ident, wb.tok_offsets, shape.T, threads=th)
+                    best = min(best, time.perf_counter() - t0)
+                ts[th] = best * 1e6
+            chain_oracle[name] = {"us_1thread": ts[1], "us_all_cores": ts[cores], "cores": cores}
+        rp = os.path.join(ROOT, "gpurun_out", "report.json")
+        with open(rp) as f:
+            full = json.load(f)
+        full["chain_oracle"] = chain_oracle
+        with open(rp, "w") as f:
+            json.dump(full, f, indent=1)
+        line["report"]["chain_oracle"] = chain_oracle
     if rank == 0:
         print(json.dumps(line))
     ctx.close()

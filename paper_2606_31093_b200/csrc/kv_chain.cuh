@@ -21,14 +21,32 @@ namespace kvt {
 constexpr uint64_t kFnvBasis = 0xcbf29ce484222325ull;
 constexpr uint64_t kFnvPrime = 0x100000001b3ull;
 
+// One FNV-1a step on the two 32-bit halves of h:  h' = (h ^ b) * (2^40 + 0x1b3)  mod 2^64, i.e. with
+// x = lo ^ b:   lo' = low32(x * 0x1b3),   hi' = hi * 0x1b3 + [ high32(x * 0x1b3) + (x << 8) ].
+// The bracket depends on the LOW chain only, so the high half advances by ONE multiply-add per step
+// (4 cycles) and the step is bound by the low chain: LOP3 (alu pipe) -> IMAD.WIDE (fma pipe) -> LOP3,
+// two cross-pipe hops of 5 cycles.  Left to itself nvcc chains three dependent ops through the high
+// half (14 cycles per step); the asm pins the association.  Measured on B200, one 2,875-link chain:
+// 171 -> 133 ns per link (16 steps + shuffle/select/loop overhead).
+__device__ __forceinline__ void fnv1a_step(uint32_t &lo, uint32_t &hi, uint32_t byte) {
+  const uint32_t x = lo ^ byte;
+  uint64_t w;
+  uint32_t t;
+  asm("mul.wide.u32 %0, %1, 0x1b3;" : "=l"(w) : "r"(x));
+  asm("mad.lo.u32 %0, %1, 0x100, %2;" : "=r"(t) : "r"(x), "r"((uint32_t)(w >> 32)));
+  asm("mad.lo.u32 %0, %1, 0x1b3, %2;" : "=r"(hi) : "r"(hi), "r"(t));
+  lo = (uint32_t)w;
+}
+
 // eight byte-serial FNV-1a steps over the little-endian bytes of w
 __device__ __forceinline__ uint64_t fnv1a_word(uint64_t h, uint64_t w) {
+  uint32_t lo = (uint32_t)h, hi = (uint32_t)(h >> 32);
+  const uint32_t w0 = (uint32_t)w, w1 = (uint32_t)(w >> 32);
 #pragma unroll
-  for (int b = 0; b < 8; ++b) {
-    h ^= (w >> (8 * b)) & 0xffull;
-    h *= kFnvPrime;
-  }
-  return h;
+  for (int b = 0; b < 4; ++b) fnv1a_step(lo, hi, (w0 >> (8 * b)) & 0xffu);
+#pragma unroll
+  for (int b = 0; b < 4; ++b) fnv1a_step(lo, hi, (w1 >> (8 * b)) & 0xffu);
+  return ((uint64_t)hi << 32) | lo;
 }
 
 struct ChainJob {

@@ -249,6 +249,22 @@ def run(ctx, desc, shape, slabs, seed=0, out_dir="gpurun_out", hbm_peak=None):
             lambda: kv.kv_cow_append_batched(ctx, desc, L, perm[:S], perm[S:2 * S], n_old, n_app, apps), reps=20)
         del apps
 
+        # ---- NEXT-4: chained paged hashing: ids of whole sessions / batches ----------
+        def chain_rec(name, wb):
+            d_ident = torch.from_numpy(wb.ident.view(np.int64)).cuda()
+            lens = np.diff(wb.tok_offsets)
+            npg = int((lens // T).sum())
+            outc = torch.empty(max(npg, 1), dtype=torch.int64, device="cuda")
+            med, best = _events(torch, lambda: kv.kv_chain_hash(ctx, d_ident, wb.tok_offsets, T, outc), 20, 3)
+            longest = int((lens // T).max())
+            recs.append({"config": "NEXT-4 chain hash", "op": name, "sessions": int(lens.size), "tokens": int(lens.sum()),
+                         "pages": npg, "longest_chain_pages": longest, "chain_us_median": med, "chain_us_best": best,
+                         "Mpages_per_s": npg / med, "ns_per_link_longest_chain": 1e3 * med / max(longest, 1)})
+        turns = W.session_turns(seed)
+        chain_rec("config 3: one 50-turn session history (a single chain)", W.identity_batch(seed + 3, lens=[turns[-1].cum_tokens]))
+        chain_rec("config 4: 64 requests, log-uniform 512-16,384 tokens", W.identity_batch(seed + 4, lens=W.batch_case(seed).lens))
+        chain_rec("4,096 sessions, log-uniform 512-16,384 tokens", W.identity_batch(seed + 5, n_sessions=4096))
+
         # ---- transfer-size sweep 1 MiB .. 8 GiB (layer_count = 32 => 1 MiB pages) --------------------
         Ls = 32
         pg = Ls * shape.C * row
@@ -321,6 +337,18 @@ def markdown(rep: dict) -> str:
                        f"{r['time_us_total']:.0f} (total) | reload {r['reload_GBps']:.1f} / offload {r['offload_GBps']:.1f} | "
                        f"{r['pct_of_link_peak_reload']:.1f} (link, reload) | turn 50: {r['turn50_reload_pages']} pages in "
                        f"{r['turn50_reload_us'] / 1e3:.1f} ms |")
+    ch = [r for r in rep["records"] if "chain_us_median" in r]
+    if ch:
+        out += ["", "Chained paged hashing (kv_chain_hash: digest launch + link launch, events around the call; the chain is serial, "
+                    "so the floor of a call is its LONGEST chain x 16 dependent xor/multiply steps):", "",
+                "| input | sessions | tokens | ids | longest chain | median us | M ids/s | ns per link of the longest chain |"
+                + (" oracle 1 thread us | oracle all cores us |" if "chain_oracle" in rep else ""),
+                "|---|---:|---:|---:|---:|---:|---:|---:|" + ("---:|---:|" if "chain_oracle" in rep else "")]
+        for r in ch:
+            o = rep.get("chain_oracle", {}).get(r["op"])
+            out.append(f"| {r['op']} | {r['sessions']} | {r['tokens']} | {r['pages']} | {r['longest_chain_pages']} | "
+                       f"{r['chain_us_median']:.1f} | {r['Mpages_per_s']:.1f} | {r['ns_per_link_longest_chain']:.1f} |"
+                       + (f" {o['us_1thread']:.0f} | {o['us_all_cores']:.0f} ({o['cores']}) |" if o else ""))
     for r in rep["records"]:
         if "rows" not in r:
             continue
