@@ -56,6 +56,8 @@ def parse():
     ap.add_argument("--e2e-steps", type=int, default=0, help="steps of the host-tier leg (0 = min(steps, 20))")
     ap.add_argument("--no-cpu-baseline", action="store_true")
     ap.add_argument("--report", action="store_true", help="also time every BASELINE.json config -> gpurun_out/report.json")
+    ap.add_argument("--pool-order", default="nhd", choices=["nhd", "hnd"],
+                    help="in-page order of the pool (BASELINE.json configs are NHD; hnd = the NEXT-2 transposing transfers)")
     ap.add_argument("--seed", type=int, default=0)
     return ap.parse_args()
 
@@ -222,7 +224,8 @@ def run_ours(args):
         t = torch.empty(P * shape.T * shape.H * shape.D, dtype=torch.bfloat16, device="cuda")
         t.normal_(generator=gen)
         slabs.append(t)
-    desc = kv.PoolDesc(slabs, shape.L, shape.C, P, shape.T, shape.H, shape.D, shape.e)
+    desc = kv.PoolDesc(slabs, shape.L, shape.C, P, shape.T, shape.H, shape.D, shape.e,
+                       order=kv.KV_ORDER_HND if args.pool_order == "hnd" else kv.KV_ORDER_NHD)
     bufs = [torch.empty(payload, dtype=torch.uint8, device="cuda") for _ in range(2)]
     rng = np.random.default_rng(args.seed + 1000 * rank)
     total = Wm + max(K, Ke) + 1
@@ -296,7 +299,7 @@ def run_ours(args):
             "workload": "configs[1] single-request prefix offload: pack 512 fragmented pages (8,192 tokens) "
                         "to a device buffer + unpack a buffer into 512 other pages",
             "layers": shape.L, "kv_heads": shape.H, "head_dim": shape.D, "page_size": shape.T,
-            "pool_pages": P, "pool_GiB": round(shape.L * shape.C * P * shape.row_bytes / 2**30, 1),
+            "pool_order": args.pool_order, "pool_pages": P, "pool_GiB": round(shape.L * shape.C * P * shape.row_bytes / 2**30, 1),
             "payload_MiB": payload / 2**20, "pages_per_step": n, "parallelism": "replicas only",
             "l2": "inputs larger than L2 (768 MiB per op, fresh page ids per step; unpack reads the buffer packed one step earlier)",
             "bytes_convention": "GB/s = (bytes read + bytes written) / time = 2*payload per op",
@@ -313,9 +316,10 @@ def run_ours(args):
                 "what": "kv_offload (pool->pinned host) + kv_reload (pinned host->pool) + stream sync per step, through the C ABI",
                 "link_GBps_payload": world * 2 * payload * Ke / (e2e_ms * 1e-3) / 1e9},
         "gpu_launches": launches,
-        "roofline": {"bound": "hbm", "kernel": "kv_move_bulk (kv_pack launch)", "achieved": achieved,
+        "roofline": {"bound": "hbm", "kernel": "kv_move_bulk (kv_pack launch)" if args.pool_order == "nhd"
+                     else "kv_move_bulk<kTrans> with tensor maps (kv_pack launch, HND pool)", "achieved": achieved,
                      "peak": peak, "unit": "GB/s", "frac": achieved / peak,
-                     "traffic": NCU_TRAFFIC_BYTES_PER_LAUNCH, "algorithmic_bytes": 2 * payload,
+                     "traffic": NCU_TRAFFIC_BYTES_PER_LAUNCH if args.pool_order == "nhd" and n == 512 else None, "algorithmic_bytes": 2 * payload,
                      "peak_source": peak_src,
                      "timing": "mean over the K timed steps of CUDA events on the launch stream around each kv_pack call (one launch; page ids ride in the kernel parameters)"},
         "clocks": clocks.summary(),
