@@ -26,6 +26,7 @@ constexpr int kBlobSlots = 16;
 constexpr int kMaxStagingSlots = 4;
 constexpr uint32_t kMaxLayersKv = 4096;  // layer_count * kv_count
 constexpr uint64_t kAutoStagedMinBytes = 16ull << 20;
+constexpr uint64_t kAutoVecMinBytes = 40ull << 20, kAutoVecMaxBytes = 384ull << 20;  // AUTO: vec kernel in between
 constexpr uint32_t kSchedSlots = 256;  // claim counters, handed out round-robin per launch
 constexpr int kStaticSmemReserve = 8192;  // static shared memory of kv_move_bulk (barriers + stage metadata, 6 KiB) rounded up
 
@@ -331,6 +332,15 @@ int make_geom(const kv_ctx *ctx, const kv_pool_desc *p, uint32_t layer_count, ui
     // bulk path (6.3 TB/s).
     const bool dst_strided = g.pool_hnd && dir != 0;
     kernel = dst_strided ? KERNEL_VEC : KERNEL_BULK;
+    // Mid-sized contiguous transfers are latency-bound: 14 MB in flight through 296 issuing warps ramps slower
+    // than 16-byte loads from 1,184 CTAs' worth of warps.  Measured on B200, isolated calls on a cold L2
+    // (DESIGN.md "Kernels"): 48 MiB 23.6 -> 18.5 us, 64 MiB 27.7 -> 23.6, 192 MiB 68.6 -> 64.6; equal at
+    // <= 32 MiB (launch-bound) and 128 MiB; bulk ahead again from 512 MiB (171 vs 177 us).
+    if (!g.trans && dir != 3) {
+      uint64_t bytes = 0;
+      for (const Req &r : reqs) bytes += r.n_ids * g.pool_row * g.LC;
+      if (bytes >= kAutoVecMinBytes && bytes < kAutoVecMaxBytes) kernel = KERNEL_VEC;
+    }
   }
   uint32_t cap = kernel == KERNEL_BULK ? (g.trans && !g.tma ? ctx->t_stage_bytes : ctx->stage_bytes) : 16384u;
   cap = std::max(16u, cap / 16 * 16);

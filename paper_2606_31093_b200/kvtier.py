@@ -130,12 +130,15 @@ def _ptr(x) -> Optional[int]:
     """Address of a torch tensor / numpy array / int / None."""
     if x is None:
         return None
-    if isinstance(x, int):
+    if type(x) is int:
         return x
-    if hasattr(x, "data_ptr"):
-        return int(x.data_ptr())
+    dp = getattr(x, "data_ptr", None)
+    if dp is not None:
+        return dp()
     if isinstance(x, np.ndarray):
-        return int(x.ctypes.data)
+        return x.__array_interface__["data"][0]
+    if isinstance(x, int):
+        return int(x)
     if isinstance(x, ctypes.c_void_p):
         return x.value
     raise TypeError(f"cannot take the address of {type(x)}")
@@ -143,18 +146,19 @@ def _ptr(x) -> Optional[int]:
 
 def _nbytes(x) -> int:
     if hasattr(x, "element_size"):
-        return int(x.numel() * x.element_size())
+        return x.numel() * x.element_size()
     if isinstance(x, np.ndarray):
         return int(x.nbytes)
     raise TypeError(f"cannot size {type(x)}; pass nbytes explicitly")
 
 
 _torch = None
+_raw_stream = None  # torch._C._cuda_getCurrentRawStream: the current stream's handle without building a Stream object
 
 
 def _stream(s) -> Optional[int]:
     """cudaStream_t of `s` (torch stream / int / None = torch's current stream, else the default)."""
-    global _torch
+    global _torch, _raw_stream
     if s is None:
         if _torch is None:
             try:
@@ -162,7 +166,10 @@ def _stream(s) -> Optional[int]:
             except ImportError:
                 return None
             _torch = torch
+            _raw_stream = getattr(torch._C, "_cuda_getCurrentRawStream", None)
         if _torch.cuda.is_initialized():
+            if _raw_stream is not None:
+                return _raw_stream(_torch.cuda.current_device()) or None
             return int(_torch.cuda.current_stream().cuda_stream) or None
         return None
     if isinstance(s, int):
@@ -170,7 +177,12 @@ def _stream(s) -> Optional[int]:
     return int(s.cuda_stream) or None
 
 
+_I32 = np.dtype(np.int32)
+
+
 def _host_i32(a):
+    if type(a) is np.ndarray and a.dtype == _I32 and a.flags.c_contiguous:
+        return a  # the common case: no copy, no new array object
     return np.ascontiguousarray(np.asarray(a, dtype=np.int32))
 
 
@@ -180,7 +192,8 @@ def _ids_arg(ids, flags):
     if flags & KV_FLAG_IDS_ON_DEVICE:
         return _ptr(ids), ids, int(ids.numel())
     a = _host_i32(ids)
-    return int(a.ctypes.data) if a.size else None, a, int(a.size)
+    n = a.size
+    return (a.__array_interface__["data"][0] if n else None), a, n
 
 
 class PoolDesc:
@@ -202,14 +215,11 @@ class PoolDesc:
             num_pages, page_size, num_heads, head_dim, elem_bytes, int(order),
             row if page_stride_bytes is None else int(page_stride_bytes))
         self.row_bytes = row
+        self.ref = ctypes.byref(self.desc)  # built once: every transfer call passes it
 
     def page_bytes(self, layer_count: Optional[int] = None) -> int:
         L = self.desc.layer_count if layer_count is None else layer_count
         return L * self.desc.kv_count * self.row_bytes
-
-    @property
-    def ref(self):
-        return ctypes.byref(self.desc)
 
 
 class Ctx:
