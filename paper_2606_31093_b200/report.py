@@ -146,6 +146,40 @@ def run(ctx, desc, shape, slabs, seed=0, out_dir="gpurun_out", hbm_peak=None):
         torch.cuda.synchronize()
         recs[-1]["verified"] = bool(scatter_ok(buf, c2.dst_ids))
 
+        # both directions of the link at once: offload on one stream (ctx), reload of ANOTHER buffer on a
+        # second stream (ctx2) -- eviction of one session while another is restored.  Peak = two plain
+        # cudaMemcpyAsync of the same sizes on the same two streams.
+        ctx2 = kv.Ctx(torch.cuda.current_device())
+        sa, sb = torch.cuda.Stream(), torch.cuda.Stream()
+        dev2 = torch.empty(pl, dtype=torch.uint8, device="cuda")
+        hA = torch.from_numpy(kv.host_view(hp, 2 * pl))
+
+        def both(f, g):
+            sa.wait_stream(torch.cuda.current_stream())
+            sb.wait_stream(torch.cuda.current_stream())
+            f()
+            g()
+            torch.cuda.current_stream().wait_stream(sa)
+            torch.cuda.current_stream().wait_stream(sb)
+
+        def mc_a():
+            with torch.cuda.stream(sa):
+                hA[:pl].copy_(buf, non_blocking=True)
+
+        def mc_b():
+            with torch.cuda.stream(sb):
+                dev2.copy_(hA[pl:], non_blocking=True)
+
+        _, t = _events(torch, lambda: both(mc_a, mc_b), 7, 2)
+        peaks["duplex_memcpy_GBps"] = duplex = 2 * pl / t / 1e3
+        rec("2 prefix", "offload and reload at once (two ctxs, two streams)", "auto", 2 * pl, 2 * pl, 2 * n,
+            lambda: both(lambda: kv.kv_offload(ctx, desc, L, c2.src_ids, hp, pl, stream=sa),
+                         lambda: kv.kv_reload(ctx2, hp + pl, pl, c2.dst_ids, desc, L, T, T, n * T, stream=sb)),
+            reps=7, link=duplex)
+        torch.cuda.synchronize()
+        ctx2.close()
+        del dev2, hA
+
         # ---- config 3: 50-turn session ------------------------------------------------------------
         turns = W.session_turns(seed, T=T)
         fl = W.FreeList(shape.P, np.random.default_rng(seed))
@@ -322,7 +356,7 @@ def markdown(rep: dict) -> str:
     """Summary tables of a report.json (what profiles/*_report_summary.md holds)."""
     pk = rep["peaks"]
     out = [f"Peaks measured in the same run: D2D copy {pk['hbm_copy_GBps_this_run']:.0f} GB/s (read+write), pinned H2D "
-           f"{pk['h2d_GBps']:.1f} GB/s, D2H {pk['d2h_GBps']:.1f} GB/s; denominator for HBM fractions: "
+           f"{pk['h2d_GBps']:.1f} GB/s, D2H {pk['d2h_GBps']:.1f} GB/s, both at once {pk.get('duplex_memcpy_GBps', 0):.1f} GB/s; denominator for HBM fractions: "
            f"{pk['hbm_peak_GBps']:.1f} GB/s (MEASURED_PEAKS.json). GPU: {rep.get('gpu')}; host cores: {rep.get('cores')}.", "",
            "| config | op | mode | payload MiB | median us | GB/s | % of peak | verified |",
            "|---|---|---|---:|---:|---:|---:|---|"]

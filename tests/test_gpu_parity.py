@@ -324,3 +324,44 @@ def test_medium_qwen_shape_parity(kv, ctx):
     kv.kv_unpack(ctx, buf, dst, dA, s.L, s.T, s.T, 300 * s.T)
     ko.unpack(want, dst, A, Ts=s.T, n_tokens=300 * s.T, threads=8)
     assert_pool_equal(tA, A)
+
+
+@pytest.mark.parametrize("mode", ["direct", "staged"])
+def test_offload_and_reload_at_once_on_two_contexts(kv, ctx, mode):
+    """The schedule bench.py's e2e leg times: one ctx offloads on one stream while a second ctx reloads
+    another buffer into other pages of the SAME pool on a second stream (reading R21: calls on
+    different streams are independent if their destination pages are disjoint; one ctx per stream).
+    Several rounds back to back, no synchronisation in between beyond each stream's own order."""
+    m = {"direct": kv.KV_HOST_DIRECT, "staged": kv.KV_HOST_STAGED}[mode]
+    L, C, P, T, H, D, e = 6, 2, 768, 16, 4, 128, 2   # page = 192 KiB
+    rng = np.random.default_rng(141)
+    A = host_pool(rng, L, C, P, T, H, D, e)
+    tA, dA = to_device(A, kv, torch)
+    n, rounds = 90, 4
+    page = dA.page_bytes()
+    perm = rng.permutation(P).astype(np.int32)
+    src = [perm[r * n:(r + 1) * n] for r in range(rounds)]                 # pages offloaded in round r
+    dst = [perm[(rounds + r) * n:(rounds + r + 1) * n] for r in range(rounds - 1)]  # pages restored in round r+1
+    hps = [kv.kv_host_alloc(n * page) for _ in range(rounds)]
+    ctx2 = kv.Ctx(0, staging_bytes=8 << 20)
+    s_off, s_rel = torch.cuda.Stream(), torch.cuda.Stream()
+    done = [torch.cuda.Event() for _ in range(rounds)]
+    try:
+        for r in range(rounds):
+            kv.kv_offload(ctx, dA, L, src[r], hps[r], n * page, mode=m, stream=s_off)
+            done[r].record(s_off)
+            if r:  # restore what round r-1 offloaded, into fresh pages, while round r's offload runs
+                s_rel.wait_event(done[r - 1])
+                kv.kv_reload(ctx2, hps[r - 1], n * page, dst[r - 1], dA, L, T, T, n * T, mode=m, stream=s_rel)
+        torch.cuda.synchronize()
+        for r in range(rounds):
+            want = ko.pack(A, src[r])
+            assert np.array_equal(kv.host_view(hps[r], n * page), want), f"round {r}: offloaded bytes"
+        for r in range(rounds - 1):
+            ko.unpack(ko.pack(A, src[r]), dst[r], A, Ts=T, n_tokens=n * T)
+        assert_pool_equal(tA, A)
+    finally:
+        torch.cuda.synchronize()
+        ctx2.close()
+        for hp in hps:
+            kv.kv_host_free(hp)
