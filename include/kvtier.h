@@ -126,6 +126,9 @@ typedef enum kv_option {
   KV_OPT_TENSOR_MAPS = 12,   /* HND pools: 1 (default) whole-token boxes move with cp.async.bulk.tensor through per-slab
                                 tensor maps (cached per pool in the ctx; the copy engine transposes [head][token]);
                                 0: row-gather / 16-byte store paths only */
+  KV_OPT_PDL = 13,           /* bulk: 1 (default) = launch with programmatic stream serialization: the grid may become resident
+                                and run its prologue while the previous kernel of the stream drains; it touches no
+                                global memory before that kernel has completed (griddepcontrol.wait) */
 } kv_option;
 
 /* kv_ctx_get_stat keys */

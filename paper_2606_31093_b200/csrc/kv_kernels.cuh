@@ -377,6 +377,11 @@ __global__ void __launch_bounds__(kMaxWarps * 32, 1) kv_move_bulk(const __grid_c
   asm volatile("fence.mbarrier_init.release.cluster;" ::: "memory");
   asm volatile("fence.proxy.async.shared::cta;" ::: "memory");
   __syncthreads();
+  // Programmatic dependent launch (KV_OPT_PDL): let the next kernel of the stream become resident now, and
+  // touch no global memory until the previous one has completed and flushed.  Both are no-ops for a
+  // launch without the attribute.
+  asm volatile("griddepcontrol.launch_dependents;" ::: "memory");
+  asm volatile("griddepcontrol.wait;" ::: "memory");
 
   const uint64_t G = (uint64_t)gridDim.x * warps;
   const uint64_t gw = (uint64_t)blockIdx.x * warps + warp;

@@ -76,7 +76,7 @@ struct kv_ctx {
   // bulk geometry of transposing transfers (an HND pool): rows are gathered with 16-byte cp.async by all
   // lanes, which wants more, shallower issuing warps (measured: 8 x 4 x 4 KiB)
   uint32_t t_stage_bytes = 4096, t_stages = 4, t_warps = 8;
-  uint32_t staging_slots = 2, l2_hint = 0, inline_tables = 1, dynamic = 1, tensor_maps = 1;
+  uint32_t staging_slots = 2, l2_hint = 0, inline_tables = 1, dynamic = 1, tensor_maps = 1, pdl = 1;
   uint32_t next_sched = 0;
   EncodeTiledFn encode_tiled = nullptr;  // cuTensorMapEncodeTiled, nullptr if the driver has none
   std::vector<MapSet> map_sets;
@@ -455,12 +455,22 @@ constexpr int kInlineSmall = 3840;   // whole parameter block stays under the cl
 constexpr int kInlineLarge = 31744;  // CUDA 12.1+ large kernel parameters (<= 32,764 B)
 
 template <int N>
-void launch_bulk(const Job &j, const HostBlob *hb, bool trans, uint32_t grid, uint32_t block, size_t smem, cudaStream_t s) {
+void launch_bulk(const Job &j, const HostBlob *hb, bool trans, uint32_t grid, uint32_t block, size_t smem,
+                 cudaStream_t s, bool pdl) {
   static thread_local kvt::JobT<N> p;
   p.j = j;
   if constexpr (N > 0) std::memcpy(p.blob, hb->bytes.data(), hb->bytes.size());
-  if (trans) kvt::kv_move_bulk<N, true><<<grid, block, smem, s>>>(p);
-  else kvt::kv_move_bulk<N, false><<<grid, block, smem, s>>>(p);
+  // Programmatic dependent launch: this grid may become resident while the previous kernel of the stream
+  // is still draining (its CTAs leave half of each SM's shared memory free); it runs its prologue and then
+  // blocks in griddepcontrol.wait until that kernel has completed and flushed.
+  cudaLaunchAttribute attr[1];
+  attr[0].id = cudaLaunchAttributeProgrammaticStreamSerialization;
+  attr[0].val.programmaticStreamSerializationAllowed = 1;
+  cudaLaunchConfig_t cfg = {};
+  cfg.gridDim = dim3(grid); cfg.blockDim = dim3(block); cfg.dynamicSmemBytes = smem; cfg.stream = s;
+  cfg.attrs = attr; cfg.numAttrs = pdl ? 1 : 0;
+  if (trans) (void)cudaLaunchKernelEx(&cfg, kvt::kv_move_bulk<N, true>, p);
+  else (void)cudaLaunchKernelEx(&cfg, kvt::kv_move_bulk<N, false>, p);
 }
 template <int N>
 void launch_vec(const Job &j, const HostBlob *hb, bool trans, uint32_t grid, cudaStream_t s) {
@@ -537,9 +547,10 @@ int launch(kv_ctx *ctx, const Geom &g, const Blob &b, uint32_t piece_first, uint
       j.sched_done = (uint32_t *)(slot + 8);
       j.first_batch = (uint32_t)std::min<uint64_t>(32, total_items / (4 * G));
     }
-    if (!b.inl) launch_bulk<0>(j, nullptr, g.trans, grid, warps * 32, smem, s);
-    else if (b.inl->bytes.size() <= kInlineSmall) launch_bulk<kInlineSmall>(j, b.inl, g.trans, grid, warps * 32, smem, s);
-    else launch_bulk<kInlineLarge>(j, b.inl, g.trans, grid, warps * 32, smem, s);
+    const bool pdl = ctx->pdl && !capturing(s);
+    if (!b.inl) launch_bulk<0>(j, nullptr, g.trans, grid, warps * 32, smem, s, pdl);
+    else if (b.inl->bytes.size() <= kInlineSmall) launch_bulk<kInlineSmall>(j, b.inl, g.trans, grid, warps * 32, smem, s, pdl);
+    else launch_bulk<kInlineLarge>(j, b.inl, g.trans, grid, warps * 32, smem, s, pdl);
   } else {
     const uint32_t wpb = 8;  // warps per 256-thread CTA
     const uint64_t want = (total_items + wpb - 1) / wpb;
@@ -1111,6 +1122,7 @@ int kv_ctx_set_option(kv_ctx *ctx, int option, int64_t v) {
     case KV_OPT_INLINE_TABLES: if (v < 0 || v > 1) return KV_ERR_SIZE; ctx->inline_tables = (uint32_t)v; break;
     case KV_OPT_DYNAMIC: if (v < 0 || v > 1) return KV_ERR_SIZE; ctx->dynamic = (uint32_t)v; break;
     case KV_OPT_TENSOR_MAPS: if (v < 0 || v > 1) return KV_ERR_SIZE; ctx->tensor_maps = (uint32_t)v; break;
+    case KV_OPT_PDL: if (v < 0 || v > 1) return KV_ERR_SIZE; ctx->pdl = (uint32_t)v; break;
     default: return KV_ERR_LAYOUT;
   }
   return KV_OK;

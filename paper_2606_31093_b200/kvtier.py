@@ -35,7 +35,7 @@ KV_ORDER_NHD, KV_ORDER_HND = 0, 1
 KV_FLAG_VALIDATE, KV_FLAG_IDS_ON_DEVICE = 0x1, 0x2
 (KV_OPT_KERNEL, KV_OPT_STAGE_BYTES, KV_OPT_STAGES_PER_WARP, KV_OPT_WARPS, KV_OPT_STORE_LAG,
  KV_OPT_MAX_CTAS, KV_OPT_CHUNK_BYTES, KV_OPT_HOST_MAX_CTAS, KV_OPT_STAGING_SLOTS,
- KV_OPT_L2_HINT, KV_OPT_INLINE_TABLES, KV_OPT_DYNAMIC, KV_OPT_TENSOR_MAPS) = range(13)
+ KV_OPT_L2_HINT, KV_OPT_INLINE_TABLES, KV_OPT_DYNAMIC, KV_OPT_TENSOR_MAPS, KV_OPT_PDL) = range(14)
 KV_KERNEL_AUTO, KV_KERNEL_BULK, KV_KERNEL_VEC, KV_KERNEL_ELEM = 0, 1, 2, 3
 (KV_STAT_LAUNCHES, KV_STAT_MEMCPYS, KV_STAT_LAST_ITEMS, KV_STAT_LAST_PAYLOAD, KV_STAT_LAST_KERNEL,
  KV_STAT_LAST_HOST_MODE, KV_STAT_LAST_GRID, KV_STAT_LAST_SEGMENT, KV_STAT_LAST_TENSOR_MAPS) = range(9)
