@@ -394,3 +394,92 @@ def test_cuda_graph_capture_of_hnd_transfer_uses_cached_tensor_maps(kv, ctx):
     g2.replay()
     torch.cuda.synchronize()
     assert np.array_equal(buf.cpu().numpy(), want)
+
+
+# ------------------------------------------------------------------------------------------------
+# SURVEY.md 8(c) reading 18 on the device: id * page_stride beyond 2^32 inside ONE slab
+# ------------------------------------------------------------------------------------------------
+@pytest.mark.parametrize("kernel", [1, 2, 3])
+def test_page_offsets_beyond_4_gib_in_one_slab(kv, ctx, kernel):
+    """One (layer, K) slab of 262,145 pages x 16 KiB = 4 GiB + 16 KiB: ids [262144, 0, 262143, 131072] must
+    come back in that order (the oracle's pin, tests/test_oracle_pins.py, on the device), and unpacking
+    into the far end must touch only those pages.  Expected bytes come from the slab's closed-form fill
+    (64-bit word i holds i * 0x9E3779B97F4A7C15 mod 2^64), nothing from the library."""
+    free, _ = torch.cuda.mem_get_info()
+    if free < 10 << 30:
+        pytest.skip("needs 10 GiB of free device memory")
+    P, T, H, D, e = 262145, 16, 4, 128, 2
+    row = T * H * D * e
+    wpp = row // 8  # 64-bit words per page
+    ctx.set_option(kv.KV_OPT_KERNEL, kernel)
+    slab = torch.arange(P * wpp, dtype=torch.int64, device="cuda")
+    slab.mul_(-7046029254386353131)  # 0x9E3779B97F4A7C15 as a signed 64-bit value; wraps mod 2^64
+    desc = kv.PoolDesc([slab], 1, 1, P, T, H, D, e)
+
+    def page_words(g):
+        i = np.arange(g * wpp, (g + 1) * wpp, dtype=np.uint64)
+        return i * np.uint64(0x9E3779B97F4A7C15)
+
+    ids = np.array([262144, 0, 262143, 131072], dtype=np.int32)
+    buf = torch.zeros(len(ids) * row, dtype=torch.uint8, device="cuda")
+    kv.kv_pack(ctx, desc, 1, ids, buf)
+    torch.cuda.synchronize()
+    got = buf.cpu().numpy().view(np.uint64).reshape(len(ids), wpp)
+    for p, g in enumerate(ids):
+        assert np.array_equal(got[p], page_words(int(g))), f"buffer page {p} is not pool page {g}"
+    # scatter the buffer into four other pages, two of them past the 4 GiB line
+    dst = np.array([262142, 1, 200000, 262141], dtype=np.int32)
+    kv.kv_unpack(ctx, buf, dst, desc, 1, T, T, len(ids) * T, flags=kv.KV_FLAG_VALIDATE)
+    torch.cuda.synchronize()
+    view = slab.view(P, wpp)
+    for p, g in enumerate(dst):
+        assert np.array_equal(view[int(g)].cpu().numpy().view(np.uint64), page_words(int(ids[p])))
+    for g in (262143, 262144, 262140, 0, 2, 199999, 200001):  # neighbours untouched
+        assert np.array_equal(view[g].cpu().numpy().view(np.uint64), page_words(g))
+    # every other page: 64-bit checksum per page against the closed form, on the device
+    sums = view.sum(dim=1)
+    i0 = torch.arange(P, dtype=torch.int64, device="cuda") * wpp
+    want = (i0 * wpp + wpp * (wpp - 1) // 2) * (-7046029254386353131)
+    mask = torch.ones(P, dtype=torch.bool, device="cuda")
+    mask[torch.as_tensor(dst.astype(np.int64), device="cuda")] = False
+    assert torch.equal(sums[mask], want[mask]), "a page outside the destination set changed"
+    del slab, view, sums, i0, want
+    torch.cuda.empty_cache()
+
+
+@pytest.mark.parametrize("tensor_maps", [1, 0])
+def test_hnd_page_offsets_beyond_4_gib(kv, ctx, tensor_maps):
+    """The same slab read as an HND pool: the tensor-map path addresses page 262,144 through the map's
+    page coordinate (stride 16 KiB, 4 GiB from the base), the lane paths through 64-bit arithmetic."""
+    free, _ = torch.cuda.mem_get_info()
+    if free < 10 << 30:
+        pytest.skip("needs 10 GiB of free device memory")
+    P, T, H, D, e = 262145, 16, 4, 128, 2
+    row = T * H * D * e
+    wpp, wpr = row // 8, D * e // 8
+    ctx.set_option(kv.KV_OPT_TENSOR_MAPS, tensor_maps)
+    slab = torch.arange(P * wpp, dtype=torch.int64, device="cuda")
+    slab.mul_(-7046029254386353131)
+    desc = kv.PoolDesc([slab], 1, 1, P, T, H, D, e, order=kv.KV_ORDER_HND)
+
+    def nhd_words(g):  # the HND page g re-ordered to [token][head][dim]
+        i = np.arange(g * wpp, (g + 1) * wpp, dtype=np.uint64) * np.uint64(0x9E3779B97F4A7C15)
+        return i.reshape(H, T, wpr).transpose(1, 0, 2).reshape(-1)
+
+    ids = np.array([262144, 0, 262143, 131072], dtype=np.int32)
+    buf = torch.zeros(len(ids) * row, dtype=torch.uint8, device="cuda")
+    kv.kv_pack(ctx, desc, 1, ids, buf)
+    torch.cuda.synchronize()
+    assert ctx.stat(kv.KV_STAT_LAST_TENSOR_MAPS) == tensor_maps
+    got = buf.cpu().numpy().view(np.uint64).reshape(len(ids), wpp)
+    for p, g in enumerate(ids):
+        assert np.array_equal(got[p], nhd_words(int(g))), f"buffer page {p} is not pool page {g} transposed"
+    dst = np.array([262142, 1, 200000, 262141], dtype=np.int32)
+    kv.kv_unpack(ctx, buf, dst, desc, 1, T, T, len(ids) * T)
+    torch.cuda.synchronize()
+    view = slab.view(P, wpp)
+    for p, g in enumerate(dst):  # HND -> NHD buffer -> HND page: the source page's words, in place
+        src = np.arange(int(ids[p]) * wpp, (int(ids[p]) + 1) * wpp, dtype=np.uint64) * np.uint64(0x9E3779B97F4A7C15)
+        assert np.array_equal(view[int(g)].cpu().numpy().view(np.uint64), src)
+    del slab, view
+    torch.cuda.empty_cache()
