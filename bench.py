@@ -58,6 +58,8 @@ def parse():
     ap.add_argument("--report", action="store_true", help="also time every BASELINE.json config -> gpurun_out/report.json")
     ap.add_argument("--pool-order", default="nhd", choices=["nhd", "hnd"],
                     help="in-page order of the pool (BASELINE.json configs are NHD; hnd = the NEXT-2 transposing transfers)")
+    ap.add_argument("--host-mode", default="auto", choices=["auto", "direct", "staged"],
+                    help="kv_host_mode of the host-tier legs (auto = the library's measured choice)")
     ap.add_argument("--seed", type=int, default=0)
     return ap.parse_args()
 
@@ -269,20 +271,21 @@ def run_ours(args):
         #           hp[(i + 1) & 1], written one step earlier -- the schedule of the device leg, and of a
         #           server that evicts one session while it restores another; both PCIe directions carry
         #           payload at once
+        hm = {"auto": kv.KV_HOST_AUTO, "direct": kv.KV_HOST_DIRECT, "staged": kv.KV_HOST_STAGED}[args.host_mode]
         hp = [kv.kv_host_alloc(payload) for _ in range(2)]
         Ks = min(Ke, 5)
-        kv.kv_offload(ctx, desc, shape.L, src_ids[-1], hp[1], payload)  # the buffer the first duplex step reloads
+        kv.kv_offload(ctx, desc, shape.L, src_ids[-1], hp[1], payload, mode=hm)  # the buffer the first duplex step reloads
         for i in range(min(Wm, 2)):
-            kv.kv_offload(ctx, desc, shape.L, src_ids[i], hp[0], payload)
-            kv.kv_reload(ctx, hp[0], payload, dst_ids[i], desc, shape.L, shape.T, shape.T, n * shape.T)
+            kv.kv_offload(ctx, desc, shape.L, src_ids[i], hp[0], payload, mode=hm)
+            kv.kv_reload(ctx, hp[0], payload, dst_ids[i], desc, shape.L, shape.T, shape.T, n * shape.T, mode=hm)
             stream.synchronize()
         barrier()
         eo = [torch.cuda.Event(enable_timing=True) for _ in range(2 * Ks + 1)]
         eo[0].record(stream)
         for i in range(Ks):
-            kv.kv_offload(ctx, desc, shape.L, src_ids[Wm + i], hp[0], payload)
+            kv.kv_offload(ctx, desc, shape.L, src_ids[Wm + i], hp[0], payload, mode=hm)
             eo[2 * i + 1].record(stream)
-            kv.kv_reload(ctx, hp[0], payload, dst_ids[Wm + i], desc, shape.L, shape.T, shape.T, n * shape.T)
+            kv.kv_reload(ctx, hp[0], payload, dst_ids[Wm + i], desc, shape.L, shape.T, shape.T, n * shape.T, mode=hm)
             eo[2 * i + 2].record(stream)
             stream.synchronize()
         barrier()
@@ -295,9 +298,9 @@ def run_ours(args):
         s_off, s_rel = torch.cuda.Stream(), torch.cuda.Stream()
 
         def duplex_step(i):
-            kv.kv_offload(ctx, desc, shape.L, src_ids[i], hp[i & 1], payload, stream=s_off)
+            kv.kv_offload(ctx, desc, shape.L, src_ids[i], hp[i & 1], payload, mode=hm, stream=s_off)
             kv.kv_reload(ctx2, hp[(i + 1) & 1], payload, dst_ids[i], desc, shape.L, shape.T, shape.T, n * shape.T,
-                         stream=s_rel)
+                         mode=hm, stream=s_rel)
             s_off.synchronize()  # the host reads the step's result here
             s_rel.synchronize()
 
