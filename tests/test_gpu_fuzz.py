@@ -1,0 +1,97 @@
+"""Seeded random cases of every transfer against the CPU oracle, byte for byte: random shapes, page
+sizes on both sides, in-page orders, buffer layouts, strides with padding, ragged token counts, CSR
+batches with empty requests, every kernel choice (AUTO / bulk / vec / elem), tensor maps on and off.
+The directed cases live in test_gpu_parity / test_gpu_next / test_gpu_hnd; this file is the net under
+them: each seed draws one configuration and runs pack -> unpack (re-paged) -> fused re-page ->
+copy-on-write append on it."""
+import numpy as np
+import pytest
+
+torch = pytest.importorskip("torch")
+pytestmark = pytest.mark.gpu
+
+from oracle import kv_oracle as ko  # noqa: E402
+from tests.kvhelpers import assert_pool_equal, host_pool, to_device  # noqa: E402
+
+
+@pytest.fixture(scope="module")
+def kv():
+    if not torch.cuda.is_available():
+        pytest.skip("no CUDA device")
+    from paper_2606_31093_b200 import kvtier
+    return kvtier
+
+
+def draw(rng):
+    e = int(rng.choice([1, 2, 2, 2, 4, 8]))
+    D = int(rng.choice([8, 16, 24, 64, 128, 128, 256, 40]))
+    H = int(rng.choice([1, 2, 3, 4, 4, 8]))
+    Ts = int(rng.choice([1, 2, 4, 8, 16, 16, 16, 32, 64, 5, 12]))
+    Td = int(rng.choice([Ts, Ts, 16, 64, 4, 8, 32, 7, 24]))
+    L = int(rng.integers(1, 5))
+    C = int(rng.choice([1, 2, 2]))
+    pad_unit = int(rng.choice([0, 0, e, 16, 256]))
+    return dict(e=e, D=D, H=H, Ts=Ts, Td=Td, L=L, C=C, pad=pad_unit,
+                order_s=int(rng.integers(0, 2)), order_d=int(rng.integers(0, 2)),
+                layout=int(rng.integers(0, 2)), kernel=int(rng.choice([0, 0, 1, 2, 3])),
+                tensor_maps=int(rng.integers(0, 2)), R=int(rng.integers(1, 5)))
+
+
+@pytest.mark.parametrize("seed", range(300))
+def test_random_configuration(kv, seed):
+    rng = np.random.default_rng(10_000 + seed)
+    c = draw(rng)
+    e, D, H, Ts, Td, L, C = c["e"], c["D"], c["H"], c["Ts"], c["Td"], c["L"], c["C"]
+    ctx = kv.Ctx(0, staging_bytes=4 << 20)
+    try:
+        ctx.set_option(kv.KV_OPT_KERNEL, c["kernel"])
+        ctx.set_option(kv.KV_OPT_TENSOR_MAPS, c["tensor_maps"])
+        # requests: token counts, some empty, ragged against both page sizes
+        ntok = [int(rng.choice([0, 1, Ts, Td, Ts * 3 + 1, int(rng.integers(1, 400))])) for _ in range(c["R"])]
+        ns = [-(-t // Ts) for t in ntok]
+        nd = [-(-t // Td) for t in ntok]
+        Ps, Pd = sum(ns) + 5, sum(nd) + 6
+        A = host_pool(rng, L, C, Ps, Ts, H, D, e, c["pad"], order=c["order_s"])
+        B = host_pool(rng, L, C, Pd, Td, H, D, e, c["pad"], order=c["order_d"])
+        B2 = ko.HostPool([s.copy() for s in B.slabs], L, C, Pd, Td, H, D, e, B.page_stride_bytes, c["order_d"])
+        tA, dA = to_device(A, kv, torch)
+        tB, dB = to_device(B, kv, torch)
+        tB2, dB2 = to_device(B2, kv, torch)
+        soff = np.concatenate([[0], np.cumsum(ns)]).astype(np.int64)
+        doff = np.concatenate([[0], np.cumsum(nd)]).astype(np.int64)
+        sids = rng.permutation(Ps)[:soff[-1]].astype(np.int32)
+        dids = rng.permutation(Pd)[:doff[-1]].astype(np.int32)
+        page_s = L * C * Ts * H * D * e
+        # 1. batched pack (whole source pages) into per-request buffers
+        bufs = [torch.full((max(n * page_s, 16),), 0xAB, dtype=torch.uint8, device="cuda") for n in ns]
+        kv.kv_pack_batched(ctx, dA, L, sids, soff, bufs, [n * page_s for n in ns], layout=c["layout"])
+        want = ko.pack_batched(A, sids, soff, layout=c["layout"])
+        for r, n in enumerate(ns):
+            assert np.array_equal(bufs[r].cpu().numpy()[:n * page_s], want[r]), f"{c}: pack, request {r}"
+        assert_pool_equal(tA, A)
+        # 2. batched unpack with re-paging Ts -> Td and ragged tails
+        kv.kv_unpack_batched(ctx, bufs, dids, doff, ntok, dB, L, Ts, Td, layout=c["layout"],
+                             flags=kv.KV_FLAG_VALIDATE)
+        ko.unpack_batched(want, dids, doff, ntok, B, Ts=Ts, layout=c["layout"])
+        assert_pool_equal(tB, B)
+        # 3. the same movement fused pool -> pool
+        kv.kv_repage_batched(ctx, dA, sids, soff, dB2, dids, doff, ntok, L, flags=kv.KV_FLAG_VALIDATE)
+        ko.repage_batched(A, sids, soff, B2, dids, doff, ntok)
+        assert_pool_equal(tB2, B2)
+        assert_pool_equal(tA, A)
+        # 4. copy-on-write append on the destination pool
+        S = int(rng.integers(1, 4))
+        if Pd >= 2 * S:
+            perm = rng.permutation(Pd).astype(np.int32)
+            old, new = perm[:S], perm[S:2 * S]
+            n_old = rng.integers(0, Td + 1, size=S)
+            n_app = np.array([rng.integers(0, Td - o + 1) for o in n_old])
+            apps = [rng.integers(0, 256, size=L * C * int(a) * H * D * e, dtype=np.uint8) for a in n_app]
+            dev = [torch.from_numpy(a).cuda() if a.size else None for a in apps]
+            kv.kv_cow_append_batched(ctx, dB, L, old, new, n_old, n_app, dev, flags=kv.KV_FLAG_VALIDATE)
+            ko.cow_append_batched(B, old, new, n_old, n_app, apps)
+            assert_pool_equal(tB, B)
+        torch.cuda.synchronize()
+    finally:
+        torch.cuda.synchronize()
+        ctx.close()
