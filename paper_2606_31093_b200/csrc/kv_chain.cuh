@@ -24,10 +24,12 @@ constexpr uint64_t kFnvPrime = 0x100000001b3ull;
 // One FNV-1a step on the two 32-bit halves of h:  h' = (h ^ b) * (2^40 + 0x1b3)  mod 2^64, i.e. with
 // x = lo ^ b:   lo' = low32(x * 0x1b3),   hi' = hi * 0x1b3 + [ high32(x * 0x1b3) + (x << 8) ].
 // The bracket depends on the LOW chain only, so the high half advances by ONE multiply-add per step
-// (4 cycles) and the step is bound by the low chain: LOP3 (alu pipe) -> IMAD.WIDE (fma pipe) -> LOP3,
-// two cross-pipe hops of 5 cycles.  Left to itself nvcc chains three dependent ops through the high
-// half (14 cycles per step); the asm pins the association.  Measured on B200, one 2,875-link chain:
-// 171 -> 133 ns per link (16 steps + shuffle/select/loop overhead).
+// and the step is bound by the low chain: LOP3 (alu pipe) -> IMAD (fma pipe) -> LOP3.  A bare chain of
+// exactly that pair measures 15.7 cycles per step on B200 (one warp, clock64 around 1.6 M dependent
+// steps; it is the same with IMAD.WIDE or with a 32-bit IMAD on the chain), i.e. 251 cycles = 128 ns per
+// 16-step link at 1,965 MHz: the floor.  Left to itself nvcc chains three dependent ops through the
+// high half (171 ns per link); with the association pinned by the asm below a 2,875-link chain runs at
+// 131 ns per link.
 __device__ __forceinline__ void fnv1a_step(uint32_t &lo, uint32_t &hi, uint32_t byte) {
   const uint32_t x = lo ^ byte;
   uint64_t w;
@@ -92,10 +94,12 @@ __global__ void __launch_bounds__(32) kv_chain_link(const ChainJob j) {
     if (base + 32 + lane < p1) next_d = j.out[base + 32 + lane];  // prefetch the next 32 digests
     const uint32_t n = (uint32_t)min((uint64_t)32, p1 - base);
     uint64_t mine = 0;
+    uint64_t di = __shfl_sync(0xffffffffu, d, 0);
     for (uint32_t i = 0; i < n; ++i) {  // every lane walks the same links: no divergence, no broadcast of ids
-      const uint64_t di = __shfl_sync(0xffffffffu, d, i);
+      const uint64_t dn = __shfl_sync(0xffffffffu, d, (i + 1) & 31);  // next link's digest, off the chain
       prev = fnv1a_word(fnv1a_word(kFnvBasis, prev), di);
       if (i == lane) mine = prev;
+      di = dn;
     }
     if (lane < n) j.out[base + lane] = mine;
   }
