@@ -259,7 +259,8 @@ int kv_unpack_batched(kv_ctx *ctx, const void *const *srcs, const uint64_t *src_
  * page counts, page sizes and strides are their own; `layer_count` layers of both are used.  Ts == Td
  * makes it a page migration inside or between pools.  The source pool is never written; destination
  * pages must be distinct and must not be source pages.  HBM traffic is 2 x payload instead of the
- * 4 x of pack + unpack.  KV_FLAG_IDS_ON_DEVICE is not supported here (KV_ERR_LAYOUT). */
+ * 4 x of pack + unpack.  With KV_FLAG_IDS_ON_DEVICE both id lists are DEVICE arrays (offsets and token counts
+ * stay on the host); an out-of-range id of either list skips its piece and sets the device status word. */
 int kv_repage(kv_ctx *ctx, const kv_pool_desc *src_pools, const int32_t *src_page_ids,
               uint32_t n_src_pages, const kv_pool_desc *dst_pools, const int32_t *dst_page_ids,
               uint32_t n_dst_pages, uint32_t layer_count, uint64_t n_tokens, uint32_t flags,

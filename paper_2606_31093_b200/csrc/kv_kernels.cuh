@@ -86,6 +86,9 @@ struct Job {
   const uint8_t *maps_pool;   // nullptr: the pool side does not use tensor copies
   const uint8_t *maps_src;    // dir 2: the source pool's maps
   uint32_t tb;                // tokens per box; a "full" item has bytes == valid == tb * tokrow
+  // dir 2 with KV_FLAG_IDS_ON_DEVICE: the caller's device array of SOURCE page ids (then `ids` is the
+  // caller's destination array and Piece::buf indexes this one); nullptr: both lists sit in `ids`
+  const int32_t *src_ids;
 };
 
 // The lookup tables of a launch: slab bases, page ids, pieces.  They live either in device memory
@@ -204,7 +207,8 @@ __device__ __forceinline__ Item decode(const Job &j, const Tables &tb, uint64_t 
   if (j.dir == 2 && vt == 0) {  // wholly zero-padded chunk: there is no source page to look up
     baddr = 0;
   } else if (j.dir == 2) {  // pool -> pool: the "buffer" side is page src_ids[bp] of the source pool
-    const int32_t sid = (kGlobal || j.ids) ? __ldg(tb.ids + buf + bp) : tb.ids[buf + bp];
+    const int32_t sid = j.src_ids ? __ldg(j.src_ids + buf + bp)
+                                  : ((kGlobal || j.ids) ? __ldg(tb.ids + buf + bp) : tb.ids[buf + bp]);
     if ((uint32_t)sid >= j.src_num_pages) {
       atomicOr(j.status, 1u);
       it.src = it.dst = 0; it.bytes = it.valid = 0;

@@ -130,6 +130,7 @@ struct Geom {
   // dir 2 (pool -> pool): the source pool; its bases follow the destination's in the tables
   const kv_pool_desc *src_pool = nullptr;
   const kv_pool_desc *dst_pool = nullptr;  // the pool of the call (destination pool of dir 2)
+  const int32_t *dev_src_ids = nullptr;    // dir 2 with device-resident ids: the source list
   // an HND pool on either side makes the transfer a [token] x [head] transposition (kTrans kernels)
   bool trans = false;
   uint32_t drow = 0, H = 0, pool_hnd = 0, src_hnd = 0;
@@ -500,6 +501,7 @@ int launch(kv_ctx *ctx, const Geom &g, const Blob &b, uint32_t piece_first, uint
   j.tokrow = g.tokrow; j.chunk_bytes = g.chunk_bytes; j.sub_bytes = g.sub_bytes; j.subs = g.subs;
   j.num_pages = g.num_pages;
   if (g.src_pool) { j.src_num_pages = g.src_pool->num_pages; j.src_page_stride = g.src_pool->page_stride_bytes; }
+  j.src_ids = g.dev_src_ids;
   j.drow = g.drow; j.H = g.H;
   if (g.trans) {
     // the pool of this geometry is the destination pool of dir 2 and "the" pool otherwise; g.Tpool is its page size
@@ -681,7 +683,7 @@ int plan_repage(kv_ctx *ctx, const kv_pool_desc *sp, const int32_t *src_ids, con
   if (rc) return rc;
   rc = check_desc(sp, layer_count);
   if (rc) return rc;
-  if (flags & KV_FLAG_IDS_ON_DEVICE) return KV_ERR_LAYOUT;  // host id lists only on this entry
+  const bool dev_ids = flags & KV_FLAG_IDS_ON_DEVICE;
   if (sp->kv_count != dp->kv_count || sp->num_heads != dp->num_heads || sp->head_dim != dp->head_dim ||
       sp->elem_bytes != dp->elem_bytes)
     return KV_ERR_DESC;
@@ -698,7 +700,8 @@ int plan_repage(kv_ctx *ctx, const kv_pool_desc *sp, const int32_t *src_ids, con
     if (nd != (n_tokens[r] + Td - 1) / Td || ns != (n_tokens[r] + Ts - 1) / Ts) return KV_ERR_SIZE;
     if (!nd) continue;
     Req q;
-    q.buf = n_dst_total + (uint64_t)src_off[r];  // index of its first source id in the combined array
+    // index of its first source id: in the combined host array, or in the caller's device array
+    q.buf = (dev_ids ? 0 : n_dst_total) + (uint64_t)src_off[r];
     q.n_tokens = n_tokens[r];
     q.id_begin = (uint64_t)dst_off[r]; q.n_ids = nd; q.n_buf_pages = ns;
     c->reqs.push_back(q);
@@ -708,17 +711,21 @@ int plan_repage(kv_ctx *ctx, const kv_pool_desc *sp, const int32_t *src_ids, con
   if ((n_dst_total && !dst_ids) || (n_src_total && !src_ids)) return KV_ERR_NULL;
   rc = make_geom(ctx, dp, layer_count, Ts, /*dir=*/2, KV_LAYOUT_PAGE_FIRST, c->reqs, &c->geom, sp);
   if (rc) return rc;
-  rc = check_ids(dst_ids, n_dst_total, dp->num_pages);
-  if (rc) return rc;
-  rc = check_ids(src_ids, n_src_total, sp->num_pages);
-  if (rc) return rc;
-  if (flags & KV_FLAG_VALIDATE) {
-    rc = check_dups(dst_ids, n_dst_total, dp->num_pages);
+  if (dev_ids) {  // nothing to validate on the host: out-of-range ids skip their page and set the status word
+    c->geom.dev_src_ids = src_ids;
+  } else {
+    rc = check_ids(dst_ids, n_dst_total, dp->num_pages);
     if (rc) return rc;
+    rc = check_ids(src_ids, n_src_total, sp->num_pages);
+    if (rc) return rc;
+    if (flags & KV_FLAG_VALIDATE) {
+      rc = check_dups(dst_ids, n_dst_total, dp->num_pages);
+      if (rc) return rc;
+    }
+    all_ids->resize((size_t)c->n_ids);
+    if (n_dst_total) std::memcpy(all_ids->data(), dst_ids, (size_t)n_dst_total * 4);
+    if (n_src_total) std::memcpy(all_ids->data() + n_dst_total, src_ids, (size_t)n_src_total * 4);
   }
-  all_ids->resize((size_t)c->n_ids);
-  if (n_dst_total) std::memcpy(all_ids->data(), dst_ids, (size_t)n_dst_total * 4);
-  if (n_src_total) std::memcpy(all_ids->data() + n_dst_total, src_ids, (size_t)n_src_total * 4);
   c->total_items = 0; c->payload = 0;
   for (Req &q : c->reqs) {
     q.items = items_of(c->geom, q.n_ids);
@@ -1333,7 +1340,8 @@ int kv_repage_batched(kv_ctx *ctx, const kv_pool_desc *src_pools, const int32_t 
   int rc = plan_repage(ctx, src_pools, src_page_ids, src_offsets, dst_pools, dst_page_ids,
                        dst_offsets, n_tokens, n_req, layer_count, flags, &c, &ids);
   if (rc) return rc;
-  return run_device(ctx, dst_pools, c, ids.data(), flags, (cudaStream_t)stream);
+  return run_device(ctx, dst_pools, c, (flags & KV_FLAG_IDS_ON_DEVICE) ? dst_page_ids : ids.data(), flags,
+                    (cudaStream_t)stream);
 }
 
 int kv_repage(kv_ctx *ctx, const kv_pool_desc *src_pools, const int32_t *src_page_ids,

@@ -440,16 +440,16 @@ def kv_reload_batched(ctx: Ctx, host_srcs, dst_page_ids, req_offsets, n_tokens, 
 
 def kv_repage(ctx: Ctx, src_pools: PoolDesc, src_page_ids, dst_pools: PoolDesc, dst_page_ids,
               layer_count: int, n_tokens: int, flags=0, stream=None):
-    sp, skeep, ns = _ids_arg(src_page_ids, 0)
-    dp, dkeep, nd = _ids_arg(dst_page_ids, 0)
+    sp, skeep, ns = _ids_arg(src_page_ids, flags)
+    dp, dkeep, nd = _ids_arg(dst_page_ids, flags)
     _chk(ctx, _kv_repage(ctx.h, src_pools.ref, sp, ns, dst_pools.ref, dp, nd, layer_count,
                          int(n_tokens), flags, _stream(stream)))
 
 
 def kv_repage_batched(ctx: Ctx, src_pools: PoolDesc, src_page_ids, src_offsets, dst_pools: PoolDesc,
                       dst_page_ids, dst_offsets, n_tokens, layer_count: int, flags=0, stream=None):
-    sp, skeep, _ = _ids_arg(src_page_ids, 0)
-    dp, dkeep, _ = _ids_arg(dst_page_ids, 0)
+    sp, skeep, _ = _ids_arg(src_page_ids, flags)
+    dp, dkeep, _ = _ids_arg(dst_page_ids, flags)
     soff, R = _csr(src_offsets)
     doff, R2 = _csr(dst_offsets)
     assert R == R2

@@ -189,7 +189,13 @@ def test_plan_fused_repage_and_cow(ctx):
     assert ctx.stat(kv.KV_STAT_LAST_ITEMS) == 32 * 32 * 4 * 96  # 16 KiB segments, 4 per 64-token row
     assert ctx.stat(kv.KV_STAT_LAST_PAYLOAD) == 6 << 30
     assert ctx.stat(kv.KV_STAT_LAST_KERNEL) == kv.KV_KERNEL_BULK
-    assert status_of(lambda: f(flags=kv.KV_FLAG_IDS_ON_DEVICE)) == kv.KV_ERR_LAYOUT
+    # device-resident id lists: nothing is validated on the host (the arrays are never dereferenced here)
+    import torch
+    fd = lambda: kv.kv_repage_batched(ctx, src, torch.from_numpy(c5.src_ids), c5.src_offsets, dst,
+                                      torch.from_numpy(c5.dst_ids), c5.dst_offsets, c5.n_tokens, L,
+                                      flags=kv.KV_FLAG_IDS_ON_DEVICE)
+    assert status_of(fd) == kv.KV_ERR_NO_DEVICE
+    assert ctx.stat(kv.KV_STAT_LAST_ITEMS) == 32 * 32 * 4 * 96
     bad = c5.dst_ids.copy(); bad[5] = bad[4]
     assert status_of(lambda: kv.kv_repage_batched(ctx, src, c5.src_ids, c5.src_offsets, dst, bad, c5.dst_offsets,
                                                   c5.n_tokens, L, flags=kv.KV_FLAG_VALIDATE)) == kv.KV_ERR_DUP_PAGE

@@ -108,7 +108,6 @@ def test_repage_errors_write_nothing(kv, ctx):
     assert status(lambda: kv.kv_repage(ctx, dA, s8, dB, [1, 1], L, 128, flags=kv.KV_FLAG_VALIDATE)) == kv.KV_ERR_DUP_PAGE
     assert status(lambda: kv.kv_repage(ctx, dA, s8, dBh, [1, 2], L, 128)) == kv.KV_ERR_DESC
     assert status(lambda: kv.kv_repage(ctx, dA, s8, dB, [1, 2], L + 1, 128)) == kv.KV_ERR_DESC
-    assert status(lambda: kv.kv_repage(ctx, dA, s8, dB, [1, 2], L, 128, flags=kv.KV_FLAG_IDS_ON_DEVICE)) == kv.KV_ERR_LAYOUT
     kv.kv_repage(ctx, dA, [], dB, [], L, 0)  # empty: KV_OK, no launch
     torch.cuda.synchronize()
     assert_pool_equal(tB, B)
@@ -483,3 +482,38 @@ def test_hnd_page_offsets_beyond_4_gib(kv, ctx, tensor_maps):
         assert np.array_equal(view[int(g)].cpu().numpy().view(np.uint64), src)
     del slab, view
     torch.cuda.empty_cache()
+
+
+@pytest.mark.parametrize("orders", [(0, 0), (1, 0), (0, 1)])
+def test_repage_with_device_resident_ids(kv, ctx, orders):
+    """kv_repage_batched with KV_FLAG_IDS_ON_DEVICE: both id lists are device arrays (say, written by a
+    GPU-side slot allocator); an out-of-range id of either list skips its piece and raises the status word."""
+    L, C, H, D, e, Ts, Td = 3, 2, 4, 128, 2, 16, 64
+    rng = np.random.default_rng(131 + orders[0] * 2 + orders[1])
+    ntok = [2048 - 37, 0, 100, 64]
+    ns, nd = [-(-t // Ts) for t in ntok], [-(-t // Td) for t in ntok]
+    A = host_pool(rng, L, C, sum(ns) + 9, Ts, H, D, e, order=orders[0])
+    B = host_pool(rng, L, C, sum(nd) + 7, Td, H, D, e, order=orders[1])
+    tA, dA = to_device(A, kv, torch)
+    tB, dB = to_device(B, kv, torch)
+    soff = np.concatenate([[0], np.cumsum(ns)]).astype(np.int64)
+    doff = np.concatenate([[0], np.cumsum(nd)]).astype(np.int64)
+    sids = rng.permutation(sum(ns) + 9)[:soff[-1]].astype(np.int32)
+    dids = rng.permutation(sum(nd) + 7)[:doff[-1]].astype(np.int32)
+    d_s, d_d = torch.from_numpy(sids).cuda(), torch.from_numpy(dids).cuda()
+    kv.kv_repage_batched(ctx, dA, d_s, soff, dB, d_d, doff, ntok, L, flags=kv.KV_FLAG_IDS_ON_DEVICE)
+    torch.cuda.synchronize()
+    ko.repage_batched(A, sids, soff, B, dids, doff, ntok)
+    assert_pool_equal(tB, B)
+    assert_pool_equal(tA, A)
+    assert ctx.device_status() == 0
+    # a bad SOURCE id: the pieces that would read it are skipped, everything else is as the oracle says
+    bad = sids.copy()
+    bad[3] = A.num_pages + 5
+    d_s.copy_(torch.from_numpy(bad))
+    kv.kv_repage_batched(ctx, dA, d_s, soff, dB, d_d, doff, ntok, L, flags=kv.KV_FLAG_IDS_ON_DEVICE)
+    assert ctx.device_status() == 1
+    assert ctx.device_status() == 0  # reading clears it
+    # the single-request entry takes device tensors too
+    one_s, one_d = d_s[:0], d_d[:0]
+    kv.kv_repage(ctx, dA, one_s, dB, one_d, L, 0, flags=kv.KV_FLAG_IDS_ON_DEVICE)  # empty: KV_OK
