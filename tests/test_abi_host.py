@@ -300,3 +300,18 @@ def test_chain_hash_planning_and_errors(ctx):
     # nothing to hash: KV_OK even without a device
     assert kv.kv_chain_hash(ctx, None, [0, 15, 15], 16, None, out_capacity=0).tolist() == [0, 0, 0]
     assert kv.kv_chain_hash(ctx, None, [0], 16, None, out_capacity=0).tolist() == [0]
+
+
+def test_header_is_c_and_links_from_c(tmp_path):
+    """include/kvtier.h compiles as C99 with -Wall -Wextra -Werror -pedantic and a plain-C program drives the
+    library through it (planning-only ctx: validation, planning and errors, no CUDA call)."""
+    import subprocess
+    root = os.path.dirname(os.path.dirname(os.path.abspath(__file__)))
+    pkg = os.path.join(root, "paper_2606_31093_b200")
+    exe = str(tmp_path / "abi_smoke")
+    subprocess.check_call(["gcc", "-std=c99", "-Wall", "-Wextra", "-Werror", "-pedantic", "-I", os.path.join(root, "include"),
+                           os.path.join(root, "tests", "c", "abi_smoke.c"), "-o", exe, "-L", pkg, "-l:libkvtier.so",
+                           "-Wl,-rpath," + pkg])
+    out = subprocess.run([exe], capture_output=True, text=True)
+    assert out.returncode == 0, out.stderr
+    assert "abi_smoke ok" in out.stdout
