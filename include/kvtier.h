@@ -306,6 +306,30 @@ int kv_reload(kv_ctx *ctx, const void *host_src, size_t host_bytes, const int32_
               uint32_t n_dst_pages, const kv_pool_desc *pools, uint32_t layer_count,
               uint32_t src_page_size, uint32_t dst_page_size, uint64_t n_tokens, int layout,
               int mode, uint32_t flags, kv_stream_t stream);
+/* kv_reload_layerwise[_batched]: kv_reload of a LAYER-FIRST host buffer [layer][K,V][page][token][head][dim]
+ * that publishes its progress per layer ("layer-first buffer ... enables per-layer
+ * streaming reload overlapped with prefill").  Arguments as kv_reload[_batched]; the layout is
+ * KV_LAYOUT_LAYER_FIRST by definition.  `layer_flags` is an 8-byte-aligned array of `layer_count` words in
+ * device memory or mapped pinned host memory: once every page of layer l (all requests) is in the pool,
+ * layer_flags[l] = flag_value is stored with release semantics at system scope, in stream order -- a consumer
+ * (the prefill kernel of layer l on another stream, or the host) that acquires the flag may read the layer.
+ * Flags are stored in ascending layer order.  KV_HOST_STAGED (AUTO's choice from 16 MiB) streams the buffer
+ * through the ctx's staging in chunks of whole layers (a layer wider than a staging slot is cut by page
+ * ranges), copy engine and scatter kernel pipelined, so layer 0 is usable after ~1/layer_count of the
+ * transfer; KV_HOST_DIRECT is one launch over all layers followed by all flags.  n_req == 0 or no pages:
+ * the flags are still stored.  Errors as kv_reload, plus KV_ERR_NULL / KV_ERR_ALIGN / KV_ERR_HOST_MEM for
+ * `layer_flags`. */
+int kv_reload_layerwise(kv_ctx *ctx, const void *host_src, size_t host_bytes, const int32_t *dst_page_ids,
+                        uint32_t n_dst_pages, const kv_pool_desc *pools, uint32_t layer_count,
+                        uint32_t src_page_size, uint32_t dst_page_size, uint64_t n_tokens,
+                        uint64_t *layer_flags, uint64_t flag_value, int mode, uint32_t flags,
+                        kv_stream_t stream);
+int kv_reload_layerwise_batched(kv_ctx *ctx, const void *const *host_srcs, const uint64_t *host_bytes,
+                                const int32_t *dst_page_ids, const int64_t *req_offsets,
+                                const uint64_t *n_tokens, uint32_t n_req, const kv_pool_desc *pools,
+                                uint32_t layer_count, uint32_t src_page_size, uint32_t dst_page_size,
+                                uint64_t *layer_flags, uint64_t flag_value, int mode, uint32_t flags,
+                                kv_stream_t stream);
 int kv_offload_batched(kv_ctx *ctx, const kv_pool_desc *pools, uint32_t layer_count,
                        const int32_t *page_ids, const int64_t *req_offsets, uint32_t n_req,
                        int layout, void *const *host_dsts, const uint64_t *host_bytes, int mode,

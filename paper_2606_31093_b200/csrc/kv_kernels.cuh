@@ -695,4 +695,11 @@ __global__ void kv_signal_kernel(uint64_t *flag, uint64_t value) {
   asm volatile("st.release.sys.global.u64 [%0], %1;" ::"l"(flag), "l"(value) : "memory");
 }
 
+// n <= 32 consecutive flags at once (kv_reload_layerwise: the layers whose pages have just landed)
+__global__ void kv_signal_range(uint64_t *flags, uint32_t n, uint64_t value) {
+  __threadfence_system();
+  for (uint32_t i = threadIdx.x; i < n; i += blockDim.x)
+    asm volatile("st.release.sys.global.u64 [%0], %1;" ::"l"(flags + i), "l"(value) : "memory");
+}
+
 }  // namespace kvt

@@ -487,16 +487,19 @@ void launch_elem(const kvt::JobT<0> &p, bool trans, uint32_t grid, cudaStream_t 
   else kvt::kv_move_elem<U, false><<<grid, 256, 0, s>>>(p);
 }
 
+// lc0 / lc_count: the launch covers slabs [lc0, lc0 + lc_count) of the call only (layer-range chunks of the
+// layer-first staged pipeline; tables in device memory); lc_count == 0: all of them.
 int launch(kv_ctx *ctx, const Geom &g, const Blob &b, uint32_t piece_first, uint32_t n_pieces,
-           uint64_t total_items, uint32_t cta_cap, cudaStream_t s) {
+           uint64_t total_items, uint32_t cta_cap, cudaStream_t s, uint32_t lc0 = 0, uint32_t lc_count = 0) {
   if (!total_items) return KV_OK;
   Job j{};
-  j.bases = b.d_bases; j.ids = b.d_ids; j.pieces = b.d_pieces ? b.d_pieces + piece_first : nullptr;
+  j.bases = b.d_bases ? b.d_bases + lc0 : nullptr; j.ids = b.d_ids;
+  j.pieces = b.d_pieces ? b.d_pieces + piece_first : nullptr;
   if (b.inl) { j.off_pieces = (uint32_t)b.inl->off_pieces; j.off_ids = (uint32_t)b.inl->off_ids; }
   j.status = ctx->d_status;
   j.total_items = total_items;
   j.page_stride = g.page_stride; j.buf_row_bytes = g.buf_row; j.buf_page_bytes = g.buf_page;
-  j.n_pieces = n_pieces; j.LC = g.LC; j.dir = (uint32_t)g.dir; j.layout = (uint32_t)g.layout;
+  j.n_pieces = n_pieces; j.LC = lc_count ? lc_count : g.LC; j.dir = (uint32_t)g.dir; j.layout = (uint32_t)g.layout;
   j.g = g.g; j.cpp_pool = g.Tpool / g.g; j.cpp_buf = g.Tbuf / g.g;
   j.tokrow = g.tokrow; j.chunk_bytes = g.chunk_bytes; j.sub_bytes = g.sub_bytes; j.subs = g.subs;
   j.num_pages = g.num_pages;
@@ -520,6 +523,7 @@ int launch(kv_ctx *ctx, const Geom &g, const Blob &b, uint32_t piece_first, uint
       int rc = get_maps(ctx, g.src_pool, g.L, g.tb, g.tma_es, &j.maps_src);
       if (rc) return rc;
     }
+    if (j.maps_pool) j.maps_pool += (size_t)lc0 * sizeof(CUtensorMap);
     ctx->last_tma = 1;
   }
   uint32_t cap = cta_cap ? cta_cap : ctx->max_ctas;
@@ -836,32 +840,89 @@ int ensure_staging(kv_ctx *ctx) {
 // staging slot; per chunk: kernel <-> slot on `s`, copy engine slot <-> pinned host on the side
 // stream, double (or deeper) buffered with events.  Page-first only (a chunk of pages is then
 // contiguous in the host buffer); layer-first falls back to DIRECT.
+// Layer flags of kv_reload_layerwise: after the pages of layers [l0, l0 + n) have landed in the pool,
+// flags[l] = value is stored (release, system scope) in stream order.
+struct LayerFlags { uint64_t *flags = nullptr; uint64_t value = 0; };
+
 int run_staged(kv_ctx *ctx, const kv_pool_desc *pools, const Call &c, const int32_t *ids,
-               uint32_t flags, cudaStream_t s) {
+               uint32_t flags, cudaStream_t s, LayerFlags lf = LayerFlags()) {
   int rc = ensure_staging(ctx);
   if (rc) return rc;
   const Geom &g = c.geom;
   const uint32_t n_slots = ctx->staging_slots;
   // unit of chunking: tokens that are whole pages on both sides
   const uint64_t unit_tokens = (uint64_t)g.Tpool / g.g * g.Tbuf;  // lcm(Tpool, Tbuf)
-  const uint64_t unit_bytes = unit_tokens * g.tokrow * g.LC;
+  const bool layer_first = g.layout == KV_LAYOUT_LAYER_FIRST;
+  const uint64_t unit_bytes = unit_tokens * g.tokrow * (layer_first ? g.C : g.LC);
   size_t slot_bytes = ctx->staging_bytes / n_slots / 256 * 256;
   if (ctx->chunk_bytes) slot_bytes = std::min(slot_bytes, ctx->chunk_bytes / 256 * 256);
   if (slot_bytes < unit_bytes) return KV_ERR_SIZE;
   const uint64_t chunk_tokens = slot_bytes / unit_bytes * unit_tokens;
 
-  struct Chunk { uint32_t piece_first, n_pieces; uint64_t items; };
+  // A chunk = what one staging slot holds: pieces for the kernel, copies for the copy engine.  Page-first:
+  // a run of whole pages, all layers (contiguous in the host buffer).  Layer-first: a range of layers
+  // [l0, l0 + nl) of one or more page ranges; every (layer, K|V) of a page range is one contiguous host run.
+  struct Chunk { uint32_t piece_first, n_pieces; uint64_t items; uint32_t l0, nl, sig_n; };
   struct Copy { uint64_t host, dev_off, bytes; };
   std::vector<Piece> pieces;
   std::vector<Chunk> chunks;
   std::vector<std::vector<Copy>> copies;
-  {
+  if (layer_first) {
+    const uint64_t row = g.buf_row;  // bytes of one buffer page of one (layer, K|V)
+    uint64_t widest = 1;
+    for (const Req &q : c.reqs) widest = std::max<uint64_t>(widest, q.n_buf_pages);
+    // as many layers per chunk as the widest request allows; a request wider than a slot is cut by page ranges
+    const uint32_t kl = (uint32_t)std::min<uint64_t>(g.L, std::max<uint64_t>(1, slot_bytes / (widest * g.C * row)));
+    const uint64_t unit_pool_pages = unit_tokens / g.Tpool;
+    for (uint32_t l0 = 0; l0 < g.L; l0 += kl) {
+      const uint32_t nl = std::min(kl, g.L - l0);
+      const uint64_t per_buf_page = (uint64_t)nl * g.C * row;  // slot bytes one buffer page costs in this layer range
+      const uint64_t max_pool_pages = slot_bytes / per_buf_page * g.Tbuf / g.Tpool / unit_pool_pages * unit_pool_pages;
+      if (!max_pool_pages) return KV_ERR_SIZE;
+      Chunk cur{(uint32_t)pieces.size(), 0, 0, l0, nl, 0};
+      std::vector<Copy> cur_copies;
+      uint64_t fill = 0;
+      auto close = [&]() {
+        if (cur.n_pieces) { chunks.push_back(cur); copies.push_back(cur_copies); }
+        cur = Chunk{(uint32_t)pieces.size(), 0, 0, l0, nl, 0};
+        cur_copies.clear();
+        fill = 0;
+      };
+      for (const Req &q : c.reqs) {
+        for (uint64_t q0 = 0; q0 < q.n_ids; q0 += max_pool_pages) {
+          const uint64_t q1 = std::min(q.n_ids, q0 + max_pool_pages);
+          const uint64_t t0 = q0 * g.Tpool, t1 = q1 * g.Tpool;
+          const uint64_t b0 = std::min(t0 / g.Tbuf, q.n_buf_pages);
+          const uint64_t b1 = std::min((t1 + g.Tbuf - 1) / g.Tbuf, q.n_buf_pages);
+          const uint64_t nb = b1 - b0, region = nb * per_buf_page;
+          if (fill + region > slot_bytes) close();
+          Piece pc;
+          pc.item_begin = cur.items;
+          pc.buf = fill;  // offset within the slot; the slot base is added below
+          pc.n_tokens = q.n_tokens > t0 ? std::min(q.n_tokens - t0, t1 - t0) : 0;
+          pc.id_begin = q.id_begin + q0;
+          pc.n_buf_pages = nb;
+          pieces.push_back(pc);
+          cur.n_pieces++;
+          cur.items += (q1 - q0) * (g.Tpool / g.g) * nl * g.C * g.subs;
+          if (nb)
+            for (uint32_t l = 0; l < nl; ++l)
+              for (uint32_t kc = 0; kc < g.C; ++kc)
+                cur_copies.push_back(Copy{q.buf + (((uint64_t)(l0 + l) * g.C + kc) * q.n_buf_pages + b0) * row,
+                                          fill + ((uint64_t)l * g.C + kc) * nb * row, nb * row});
+          fill += (region + 255) / 256 * 256;
+        }
+      }
+      close();
+      if (!chunks.empty()) chunks.back().sig_n = nl;  // layers [l0, l0 + nl) are complete after this chunk
+    }
+  } else {
     uint64_t fill_tokens = 0;  // tokens (in buffer-page units) already placed in the open chunk
-    Chunk cur{0, 0, 0};
+    Chunk cur{0, 0, 0, 0, g.L, 0};
     std::vector<Copy> cur_copies;
     auto close = [&]() {
       if (cur.n_pieces) { chunks.push_back(cur); copies.push_back(cur_copies); }
-      cur = Chunk{(uint32_t)pieces.size(), 0, 0};
+      cur = Chunk{(uint32_t)pieces.size(), 0, 0, 0, g.L, 0};
       cur_copies.clear();
       fill_tokens = 0;
     };
@@ -912,7 +973,8 @@ int run_staged(kv_ctx *ctx, const kv_pool_desc *pools, const Call &c, const int3
     uint8_t *slot_base = (uint8_t *)ctx->staging + (size_t)slot * slot_bytes;
     if (g.dir == 0) {  // offload: kernel fills the slot on s, copy engine drains it on side
       if (ctx->free_valid[slot]) KV_CUDA(ctx, cudaStreamWaitEvent(s, ctx->ev_free[slot], 0));
-      rc = launch(ctx, g, b, chunks[ci].piece_first, chunks[ci].n_pieces, chunks[ci].items, 0, s);
+      rc = launch(ctx, g, b, chunks[ci].piece_first, chunks[ci].n_pieces, chunks[ci].items, 0, s,
+                  chunks[ci].l0 * g.C, chunks[ci].nl * g.C);
       if (rc) return rc;
       KV_CUDA(ctx, cudaEventRecord(ctx->ev_full[slot], s));
       KV_CUDA(ctx, cudaStreamWaitEvent(ctx->side, ctx->ev_full[slot], 0));
@@ -932,8 +994,14 @@ int run_staged(kv_ctx *ctx, const kv_pool_desc *pools, const Call &c, const int3
       }
       KV_CUDA(ctx, cudaEventRecord(ctx->ev_full[slot], ctx->side));
       KV_CUDA(ctx, cudaStreamWaitEvent(s, ctx->ev_full[slot], 0));
-      rc = launch(ctx, g, b, chunks[ci].piece_first, chunks[ci].n_pieces, chunks[ci].items, 0, s);
+      rc = launch(ctx, g, b, chunks[ci].piece_first, chunks[ci].n_pieces, chunks[ci].items, 0, s,
+                  chunks[ci].l0 * g.C, chunks[ci].nl * g.C);
       if (rc) return rc;
+      if (lf.flags && chunks[ci].sig_n) {  // these layers' pages are in the pool: publish
+        kvt::kv_signal_range<<<1, 32, 0, s>>>(lf.flags + chunks[ci].l0, chunks[ci].sig_n, lf.value);  // strides over > 32
+        KV_CUDA(ctx, cudaGetLastError());
+        ctx->launches++;
+      }
       KV_CUDA(ctx, cudaEventRecord(ctx->ev_free[slot], s));
       ctx->free_valid[slot] = true;
     }
@@ -965,15 +1033,27 @@ int resolve_mode(const kv_ctx *ctx, int mode, const Call &c, int *out) {
   // cudaMemcpy peak, SM-issued stores/loads over the link 92 % (128-byte TLP payloads); below
   // ~16 MiB both are latency-bound and equal, and DIRECT is one launch with no staging traffic.
   if (m == KV_HOST_AUTO) m = c.payload >= kAutoStagedMinBytes ? KV_HOST_STAGED : KV_HOST_DIRECT;
-  // staged needs chunks that are contiguous in the host buffer
-  if (m == KV_HOST_STAGED && c.geom.layout != KV_LAYOUT_PAGE_FIRST) m = KV_HOST_DIRECT;
   (void)ctx;
   *out = m;
   return KV_OK;
 }
 
+// Device alias of a flag word (device memory, or mapped pinned host memory).
+int flag_alias(const void *p, uint64_t **out) {
+  cudaPointerAttributes a;
+  if (cudaPointerGetAttributes(&a, p) != cudaSuccess) { (void)cudaGetLastError(); return KV_ERR_HOST_MEM; }
+  if (a.type == cudaMemoryTypeUnregistered) return KV_ERR_HOST_MEM;
+  if (a.type == cudaMemoryTypeHost) {
+    if (!a.devicePointer) return KV_ERR_HOST_MEM;
+    *out = (uint64_t *)a.devicePointer;
+  } else {
+    *out = (uint64_t *)p;
+  }
+  return KV_OK;
+}
+
 int run_host(kv_ctx *ctx, const kv_pool_desc *pools, Call &c, const int32_t *ids, int mode,
-             uint32_t flags, cudaStream_t s) {
+             uint32_t flags, cudaStream_t s, LayerFlags lf = LayerFlags()) {
   int m = 0;
   int rc = resolve_mode(ctx, mode, c, &m);
   if (rc) return rc;
@@ -993,8 +1073,21 @@ int run_host(kv_ctx *ctx, const kv_pool_desc *pools, Call &c, const int32_t *ids
     if (rc) return rc;
     if (m == KV_HOST_DIRECT) q.buf = alias;
   }
-  if (m == KV_HOST_DIRECT) return run_single_launch(ctx, pools, c, ids, flags, ctx->host_max_ctas, s);
-  return run_staged(ctx, pools, c, ids, flags, s);
+  if (lf.flags) {
+    rc = flag_alias(lf.flags, &lf.flags);
+    if (rc) return rc;
+  }
+  if (m == KV_HOST_DIRECT) {  // one launch moves every layer: the flags follow it together
+    rc = run_single_launch(ctx, pools, c, ids, flags, ctx->host_max_ctas, s);
+    if (rc || !lf.flags) return rc;
+    for (uint32_t l0 = 0; l0 < c.geom.L; l0 += 32) {
+      kvt::kv_signal_range<<<1, 32, 0, s>>>(lf.flags + l0, std::min(32u, c.geom.L - l0), lf.value);
+      KV_CUDA(ctx, cudaGetLastError());
+      ctx->launches++;
+    }
+    return KV_OK;
+  }
+  return run_staged(ctx, pools, c, ids, flags, s, lf);
 }
 
 int run_device(kv_ctx *ctx, const kv_pool_desc *pools, const Call &c, const int32_t *ids,
@@ -1401,6 +1494,49 @@ int kv_reload(kv_ctx *ctx, const void *host_src, size_t host_bytes, const int32_
                        dst_page_size, layout, flags, &c);
   if (rc) return rc;
   return run_host(ctx, pools, c, dst_page_ids, mode, flags, (cudaStream_t)stream);
+}
+
+int kv_reload_layerwise_batched(kv_ctx *ctx, const void *const *host_srcs, const uint64_t *host_bytes,
+                                const int32_t *dst_page_ids, const int64_t *req_offsets,
+                                const uint64_t *n_tokens, uint32_t n_req, const kv_pool_desc *pools,
+                                uint32_t layer_count, uint32_t src_page_size, uint32_t dst_page_size,
+                                uint64_t *layer_flags, uint64_t flag_value, int mode, uint32_t flags,
+                                kv_stream_t stream) {
+  if (ctx) ctx->cur_stream = (cudaStream_t)stream;
+  if (!layer_flags) return KV_ERR_NULL;
+  if ((uint64_t)(uintptr_t)layer_flags % 8) return KV_ERR_ALIGN;
+  Call c;
+  int rc = plan_unpack(ctx, host_srcs, host_bytes, dst_page_ids, req_offsets, n_tokens, n_req, pools,
+                       layer_count, src_page_size, dst_page_size, KV_LAYOUT_LAYER_FIRST, flags, &c);
+  if (rc) return rc;
+  LayerFlags lf;
+  lf.flags = layer_flags; lf.value = flag_value;
+  if (c.reqs.empty() && !ctx->host_only) {  // nothing to move: every layer is trivially complete
+    int m = 0;
+    rc = resolve_mode(ctx, mode, c, &m);
+    if (rc) return rc;
+    DeviceGuard guard(ctx);
+    rc = flag_alias(lf.flags, &lf.flags);
+    if (rc) return rc;
+    kvt::kv_signal_range<<<1, 32, 0, (cudaStream_t)stream>>>(lf.flags, layer_count, flag_value);
+    KV_CUDA(ctx, cudaGetLastError());
+    ctx->launches++;
+    return KV_OK;
+  }
+  return run_host(ctx, pools, c, dst_page_ids, mode, flags, (cudaStream_t)stream, lf);
+}
+
+int kv_reload_layerwise(kv_ctx *ctx, const void *host_src, size_t host_bytes, const int32_t *dst_page_ids,
+                        uint32_t n_dst_pages, const kv_pool_desc *pools, uint32_t layer_count,
+                        uint32_t src_page_size, uint32_t dst_page_size, uint64_t n_tokens,
+                        uint64_t *layer_flags, uint64_t flag_value, int mode, uint32_t flags,
+                        kv_stream_t stream) {
+  const int64_t off[2] = {0, (int64_t)n_dst_pages};
+  const void *const srcs[1] = {host_src};
+  const uint64_t nb[1] = {(uint64_t)host_bytes};
+  const uint64_t nt[1] = {n_tokens};
+  return kv_reload_layerwise_batched(ctx, srcs, nb, dst_page_ids, off, nt, 1, pools, layer_count, src_page_size,
+                                     dst_page_size, layer_flags, flag_value, mode, flags, stream);
 }
 
 int kv_offload_batched(kv_ctx *ctx, const kv_pool_desc *pools, uint32_t layer_count,

@@ -99,6 +99,10 @@ _kv_offload_batched = _sig("kv_offload_batched", _int, _vp, _pdesc, _u32, _vp, _
                            _vp, _vp, _int, _u32, _vp)
 _kv_reload_batched = _sig("kv_reload_batched", _int, _vp, _vp, _vp, _vp, _vp, _vp, _u32, _pdesc,
                           _u32, _u32, _u32, _int, _int, _u32, _vp)
+_kv_reload_layerwise = _sig("kv_reload_layerwise", _int, _vp, _vp, _sz, _vp, _u32, _pdesc, _u32, _u32, _u32, _u64,
+                            _vp, _u64, _int, _u32, _vp)
+_kv_reload_layerwise_batched = _sig("kv_reload_layerwise_batched", _int, _vp, _vp, _vp, _vp, _vp, _vp, _u32, _pdesc,
+                                    _u32, _u32, _u32, _vp, _u64, _int, _u32, _vp)
 _kv_repage = _sig("kv_repage", _int, _vp, _pdesc, _vp, _u32, _pdesc, _vp, _u32, _u32, _u64, _u32, _vp)
 _kv_repage_batched = _sig("kv_repage_batched", _int, _vp, _pdesc, _vp, _vp, _pdesc, _vp, _vp, _vp,
                           _u32, _u32, _u32, _vp)
@@ -436,6 +440,30 @@ def kv_reload_batched(ctx: Ctx, host_srcs, dst_page_ids, req_offsets, n_tokens, 
                                  off.ctypes.data, nt.ctypes.data, R, pools.ref, layer_count,
                                  src_page_size, dst_page_size, layout, mode, flags,
                                  _stream(stream)))
+
+
+def kv_reload_layerwise(ctx: Ctx, host_src, host_bytes, dst_page_ids, pools: PoolDesc, layer_count: int,
+                        src_page_size: int, dst_page_size: int, n_tokens: int, layer_flags, flag_value: int,
+                        mode=KV_HOST_AUTO, flags=0, stream=None):
+    """Layer-first host buffer -> pool, layer_flags[l] = flag_value stored as each layer lands."""
+    p, keep, n = _ids_arg(dst_page_ids, flags)
+    _chk(ctx, _kv_reload_layerwise(ctx.h, _ptr(host_src), int(host_bytes), p, n, pools.ref, layer_count,
+                                   src_page_size, dst_page_size, int(n_tokens), _ptr(layer_flags),
+                                   int(flag_value), mode, flags, _stream(stream)))
+
+
+def kv_reload_layerwise_batched(ctx: Ctx, host_srcs, dst_page_ids, req_offsets, n_tokens, pools: PoolDesc,
+                                layer_count: int, src_page_size: int, dst_page_size: int, layer_flags,
+                                flag_value: int, host_bytes=None, mode=KV_HOST_AUTO, flags=0, stream=None):
+    p, keep, _ = _ids_arg(dst_page_ids, flags)
+    off, R = _csr(req_offsets)
+    s = _ptr_array(host_srcs)
+    nt = _u64_array(n_tokens)
+    nb = None if host_bytes is None else _u64_array(host_bytes)
+    _chk(ctx, _kv_reload_layerwise_batched(ctx.h, s, None if nb is None else nb.ctypes.data, p,
+                                           off.ctypes.data, nt.ctypes.data, R, pools.ref, layer_count,
+                                           src_page_size, dst_page_size, _ptr(layer_flags), int(flag_value),
+                                           mode, flags, _stream(stream)))
 
 
 def kv_repage(ctx: Ctx, src_pools: PoolDesc, src_page_ids, dst_pools: PoolDesc, dst_page_ids,

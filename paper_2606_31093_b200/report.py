@@ -146,6 +146,37 @@ def run(ctx, desc, shape, slabs, seed=0, out_dir="gpurun_out", hbm_peak=None):
         torch.cuda.synchronize()
         recs[-1]["verified"] = bool(scatter_ok(buf, c2.dst_ids))
 
+        # layer-first host buffer (NEXT-2): staged in chunks of whole layers; layer-by-layer reload with flags
+        for mode, name in ((kv.KV_HOST_DIRECT, "direct"), (kv.KV_HOST_STAGED, "staged")):
+            rec("2 prefix, layer-first buffer", "offload", name, pl, pl, n,
+                lambda: kv.kv_offload(ctx, desc, L, c2.src_ids, hp, pl, mode=mode, layout=kv.KV_LAYOUT_LAYER_FIRST),
+                reps=7, link=d2h)
+            rec("2 prefix, layer-first buffer", "reload", name, pl, pl, n,
+                lambda: kv.kv_reload(ctx, hp, pl, c2.dst_ids, desc, L, T, T, n * T, mode=mode,
+                                     layout=kv.KV_LAYOUT_LAYER_FIRST), reps=7, link=h2d)
+        flp = kv.kv_host_alloc(L * 8)
+        fh = kv.host_view(flp, L * 8).view(np.uint64)
+        for mode, name in ((kv.KV_HOST_DIRECT, "direct"), (kv.KV_HOST_STAGED, "staged")):
+            first, last = [], []
+            for it in range(5):
+                fh[:] = 0
+                torch.cuda.synchronize()
+                t0 = time.perf_counter()
+                kv.kv_reload_layerwise(ctx, hp, pl, c2.dst_ids, desc, L, T, T, n * T, flp, 1, mode=mode)
+                while fh[0] != 1:
+                    pass
+                t1 = time.perf_counter()
+                while fh[L - 1] != 1:
+                    pass
+                t2 = time.perf_counter()
+                first.append((t1 - t0) * 1e6)
+                last.append((t2 - t0) * 1e6)
+            recs.append({"config": "2 prefix, layer-first buffer", "op": "reload_layerwise", "mode": name,
+                         "payload_bytes": int(pl), "first_layer_us": float(np.median(first)),
+                         "last_layer_us": float(np.median(last)), "GBps": pl / float(np.median(last)) / 1e3,
+                         "timing": "host wall clock from the call to the flag seen in mapped pinned memory"})
+        kv.kv_host_free(flp)
+
         # both directions of the link at once: offload on one stream (ctx), reload of ANOTHER buffer on a
         # second stream (ctx2) -- eviction of one session while another is restored.  Peak = two plain
         # cudaMemcpyAsync of the same sizes on the same two streams.
@@ -371,6 +402,13 @@ def markdown(rep: dict) -> str:
                        f"{r['time_us_total']:.0f} (total) | reload {r['reload_GBps']:.1f} / offload {r['offload_GBps']:.1f} | "
                        f"{r['pct_of_link_peak_reload']:.1f} (link, reload) | turn 50: {r['turn50_reload_pages']} pages in "
                        f"{r['turn50_reload_us'] / 1e3:.1f} ms |")
+    lw = [r for r in rep["records"] if "first_layer_us" in r]
+    if lw:
+        out += ["", "Layer-by-layer reload of a layer-first host buffer (kv_reload_layerwise, 768 MiB, 48 layers; host wall clock from the "
+                    "call to the flag seen in mapped pinned memory):", "",
+                "| mode | first layer usable after us | last layer after us | GB/s |", "|---|---:|---:|---:|"]
+        for r in lw:
+            out.append(f"| {r['mode']} | {r['first_layer_us']:.0f} | {r['last_layer_us']:.0f} | {r['GBps']:.1f} |")
     ch = [r for r in rep["records"] if "chain_us_median" in r]
     if ch:
         out += ["", "Chained paged hashing (kv_chain_hash: digest launch + link launch, events around the call; the chain is serial, "

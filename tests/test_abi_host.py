@@ -173,9 +173,17 @@ def test_auto_host_mode_policy(ctx):
     for n, want in [(4, kv.KV_HOST_DIRECT), (10, kv.KV_HOST_DIRECT), (11, kv.KV_HOST_STAGED), (512, kv.KV_HOST_STAGED)]:
         assert status_of(lambda: kv.kv_offload(ctx, d, s.L, np.arange(n), BUF, n * s.page_bytes)) == kv.KV_ERR_NO_DEVICE
         assert ctx.stat(kv.KV_STAT_LAST_HOST_MODE) == want, n
-    # layer-first buffers are not chunk-contiguous: staged falls back to direct
+    # layer-first buffers stage too (chunks of whole layers: each (layer, K|V) run of pages is contiguous)
     assert status_of(lambda: kv.kv_offload(ctx, d, s.L, np.arange(512), BUF, 512 * s.page_bytes, mode=kv.KV_HOST_STAGED, layout=1)) == kv.KV_ERR_NO_DEVICE
-    assert ctx.stat(kv.KV_STAT_LAST_HOST_MODE) == kv.KV_HOST_DIRECT
+    assert ctx.stat(kv.KV_STAT_LAST_HOST_MODE) == kv.KV_HOST_STAGED
+    assert status_of(lambda: kv.kv_offload(ctx, d, s.L, np.arange(512), BUF, 512 * s.page_bytes, layout=1)) == kv.KV_ERR_NO_DEVICE
+    assert ctx.stat(kv.KV_STAT_LAST_HOST_MODE) == kv.KV_HOST_STAGED
+    # layerwise reload: flag array checked before anything else
+    flags8 = 0x9000
+    f = lambda fl: kv.kv_reload_layerwise(ctx, BUF, 512 * s.page_bytes, np.arange(512), d, s.L, 16, 16, 512 * 16, fl, 1)
+    assert status_of(lambda: f(flags8)) == kv.KV_ERR_NO_DEVICE
+    assert status_of(lambda: f(None)) == kv.KV_ERR_NULL
+    assert status_of(lambda: f(flags8 + 4)) == kv.KV_ERR_ALIGN
 
 
 def test_plan_fused_repage_and_cow(ctx):

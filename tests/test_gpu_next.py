@@ -517,3 +517,110 @@ def test_repage_with_device_resident_ids(kv, ctx, orders):
     # the single-request entry takes device tensors too
     one_s, one_d = d_s[:0], d_d[:0]
     kv.kv_repage(ctx, dA, one_s, dB, one_d, L, 0, flags=kv.KV_FLAG_IDS_ON_DEVICE)  # empty: KV_OK
+
+
+# ------------------------------------------------------------------------------------------------
+# layer-first host buffers through the staged pipeline, and the layer-by-layer reload
+# ------------------------------------------------------------------------------------------------
+@pytest.mark.parametrize("order", [0, 1])
+@pytest.mark.parametrize("staging_mib,Ts,Td", [(8, 16, 16), (2, 16, 16), (1, 16, 64), (2, 64, 16), (8, 16, 24)])
+def test_layer_first_host_tier_staged_equals_direct_equals_oracle(kv, order, staging_mib, Ts, Td):
+    """KV_HOST_STAGED with a layer-first buffer: chunks of whole layers (8 MiB staging), layers cut by page
+    ranges (1-2 MiB staging: one layer of the widest request does not fit a slot), re-paging, batched with
+    an empty request, NHD and HND pools.  Host bytes and pool bytes equal the oracle's in both modes."""
+    L, C, H, D, e = 5, 2, 4, 128, 2
+    rng = np.random.default_rng(151 + staging_mib + Ts + Td + order)
+    ctx = kv.Ctx(0, staging_bytes=staging_mib << 20)
+    counts_tok = [Ts * 90 - 7, 0, Ts * 3, 1, Ts * 41]
+    ns = [-(-t // Ts) for t in counts_tok]
+    nd = [-(-t // Td) for t in counts_tok]
+    A = host_pool(rng, L, C, sum(ns) + 11, Ts, H, D, e, order=order)
+    B = host_pool(rng, L, C, sum(nd) + 13, Td, H, D, e, order=order)
+    tA, dA = to_device(A, kv, torch)
+    soff = np.concatenate([[0], np.cumsum(ns)]).astype(np.int64)
+    doff = np.concatenate([[0], np.cumsum(nd)]).astype(np.int64)
+    sids = rng.permutation(sum(ns) + 11)[:soff[-1]].astype(np.int32)
+    dids = rng.permutation(sum(nd) + 13)[:doff[-1]].astype(np.int32)
+    page_s = dA.page_bytes()
+    hps = [kv.kv_host_alloc(max(n * page_s, 16)) for n in ns]
+    try:
+        want = ko.pack_batched(A, sids, soff, layout=ko.LAYER_FIRST)
+        for m in (kv.KV_HOST_STAGED, kv.KV_HOST_DIRECT):
+            for hp, n in zip(hps, ns):
+                kv.host_view(hp, max(n * page_s, 16))[:] = 0x5A
+            kv.kv_offload_batched(ctx, dA, L, sids, soff, hps, [n * page_s for n in ns], mode=m,
+                                  layout=kv.KV_LAYOUT_LAYER_FIRST)
+            torch.cuda.synchronize()
+            assert ctx.stat(kv.KV_STAT_LAST_HOST_MODE) == m
+            for r, n in enumerate(ns):
+                assert np.array_equal(kv.host_view(hps[r], n * page_s)[:n * page_s], want[r]), f"mode {m} request {r}"
+            Bm = ko.HostPool([s.copy() for s in B.slabs], L, C, B.num_pages, Td, H, D, e, B.page_stride_bytes, order)
+            tB, dB = to_device(Bm, kv, torch)
+            kv.kv_reload_batched(ctx, hps, dids, doff, counts_tok, dB, L, Ts, Td,
+                                 host_bytes=[n * page_s for n in ns], mode=m, layout=kv.KV_LAYOUT_LAYER_FIRST,
+                                 flags=kv.KV_FLAG_VALIDATE)
+            torch.cuda.synchronize()
+            ko.unpack_batched(want, dids, doff, counts_tok, Bm, Ts=Ts, layout=ko.LAYER_FIRST)
+            assert_pool_equal(tB, Bm)
+    finally:
+        torch.cuda.synchronize()
+        ctx.close()
+        for hp in hps:
+            kv.kv_host_free(hp)
+
+
+@pytest.mark.parametrize("mode", ["staged", "direct"])
+def test_reload_layerwise_publishes_layers_in_order(kv, mode):
+    """kv_reload_layerwise: flag l is stored only after layer l's pages are in the pool, and (staged) long
+    before the whole transfer ends.  A second stream waits for each flag ON THE DEVICE and snapshots that
+    layer at once; every snapshot must already equal the oracle's layer."""
+    m = {"staged": kv.KV_HOST_STAGED, "direct": kv.KV_HOST_DIRECT}[mode]
+    L, C, P, T, H, D, e = 12, 2, 700, 16, 4, 128, 2   # 1 MiB... per (layer, K|V): 600 pages x 16 KiB = 9.4 MiB
+    rng = np.random.default_rng(157)
+    ctx = kv.Ctx(0, staging_bytes=48 << 20)   # 24 MiB slots: one layer (18.75 MiB) per chunk
+    B = host_pool(rng, L, C, P, T, H, D, e)
+    tB, dB = to_device(B, kv, torch)
+    n = 600
+    dst = rng.permutation(P)[:n].astype(np.int32)
+    nbytes = n * dB.page_bytes()
+    hp = kv.kv_host_alloc(nbytes)
+    fl_p = kv.kv_host_alloc(L * 8)
+    try:
+        src = rng.integers(0, 256, size=nbytes, dtype=np.uint8)
+        kv.host_view(hp, nbytes)[:] = src
+        flags_h = kv.host_view(fl_p, L * 8).view(np.uint64)
+        flags_h[:] = 0
+        ko.unpack(src, dst, B, Ts=T, n_tokens=n * T, layout=ko.LAYER_FIRST)  # B is now the expected pool
+        side = torch.cuda.Stream()
+        main = torch.cuda.Stream()
+        seen_order = []
+        kv.kv_reload_layerwise(ctx, hp, nbytes, dst, dB, L, T, T, n * T, fl_p, 42, mode=m, stream=main)
+        assert ctx.stat(kv.KV_STAT_LAST_HOST_MODE) == m
+        snaps = []
+        import time
+        t0 = time.time()
+        for l in range(L):  # the host polls the mapped flags; the snapshot of layer l starts the moment flag l is seen
+            while flags_h[l] != 42:
+                assert time.time() - t0 < 20, f"flag {l} never arrived"
+            seen_order.append([int(x) for x in flags_h])
+            with torch.cuda.stream(side):
+                snaps.append([tB[l * C + c].clone() for c in range(C)])
+        side.synchronize()
+        main.synchronize()
+        for l in range(L):
+            assert all(x == 42 for x in seen_order[l][:l + 1]), "flags are stored in ascending layer order"
+            for c in range(C):
+                assert np.array_equal(snaps[l][c].cpu().numpy(), B.slabs[l * C + c]), f"layer {l} was published early"
+        if mode == "staged":  # streaming: when flag 0 was seen the last layers had not been published yet
+            assert seen_order[0][L - 1] == 0
+        assert_pool_equal(tB, B)
+        # no pages: the flags are still stored
+        flags_h[:] = 0
+        kv.kv_reload_layerwise(ctx, hp, 0, [], dB, L, T, T, 0, fl_p, 7, mode=m, stream=main)
+        main.synchronize()
+        assert (flags_h == 7).all()
+    finally:
+        torch.cuda.synchronize()
+        ctx.close()
+        kv.kv_host_free(hp)
+        kv.kv_host_free(fl_p)
