@@ -3,7 +3,7 @@ sizes on both sides, in-page orders, buffer layouts, strides with padding, ragge
 batches with empty requests, every kernel choice (AUTO / bulk / vec / elem), tensor maps on and off.
 The directed cases live in test_gpu_parity / test_gpu_next / test_gpu_hnd; this file is the net under
 them: each seed draws one configuration and runs pack -> unpack (re-paged) -> fused re-page ->
-copy-on-write append on it."""
+copy-on-write append -> host-tier offload / re-paging reload (random mode and pipeline chunk size) on it."""
 import numpy as np
 import pytest
 
@@ -91,6 +91,34 @@ def test_random_configuration(kv, seed):
             kv.kv_cow_append_batched(ctx, dB, L, old, new, n_old, n_app, dev, flags=kv.KV_FLAG_VALIDATE)
             ko.cow_append_batched(B, old, new, n_old, n_app, apps)
             assert_pool_equal(tB, B)
+        # 5. the host tier on the same requests: offload A's pages, reload them re-paged into a fresh copy
+        #    of the destination pool; random mode, random pipeline chunk size (multi-chunk, layer ranges,
+        #    page ranges); a chunk smaller than one lcm(Ts, Td) unit is refused with KV_ERR_SIZE -> direct
+        B3 = ko.HostPool([s_.copy() for s_ in B2.slabs], L, C, Pd, Td, H, D, e, B.page_stride_bytes, c["order_d"])
+        ko.unpack_batched(want, dids, doff, ntok, B3, Ts=Ts, layout=c["layout"])
+        tB3, dB3 = to_device(B2, kv, torch)
+        mode = int(rng.choice([kv.KV_HOST_DIRECT, kv.KV_HOST_STAGED, kv.KV_HOST_STAGED]))
+        ctx.set_option(kv.KV_OPT_CHUNK_BYTES, int(rng.choice([0, 64 << 10, 256 << 10, 1 << 20])))
+        hps = [kv.kv_host_alloc(max(n * page_s, 16)) for n in ns]
+        try:
+            def both(m):
+                kv.kv_offload_batched(ctx, dA, L, sids, soff, hps, [n * page_s for n in ns], mode=m, layout=c["layout"])
+                torch.cuda.synchronize()
+                for r, n in enumerate(ns):
+                    assert np.array_equal(kv.host_view(hps[r], max(n * page_s, 16))[:n * page_s], want[r]), f"{c}: offload {m}, request {r}"
+                kv.kv_reload_batched(ctx, hps, dids, doff, ntok, dB3, L, Ts, Td, host_bytes=[n * page_s for n in ns],
+                                     mode=m, layout=c["layout"])
+                torch.cuda.synchronize()
+            try:
+                both(mode)
+            except kv.KvError as ex:
+                assert ex.status == kv.KV_ERR_SIZE and mode == kv.KV_HOST_STAGED, f"{c}: {ex}"
+                both(kv.KV_HOST_DIRECT)
+            assert_pool_equal(tB3, B3)
+        finally:
+            torch.cuda.synchronize()
+            for hp in hps:
+                kv.kv_host_free(hp)
         torch.cuda.synchronize()
     finally:
         torch.cuda.synchronize()
