@@ -1,0 +1,105 @@
+// kv_host_state.h -- the ctx: constants, staging ring, tensor-map cache, options, statistics
+// Part of the host side of libkvtier.so; included by kvtier.cu only (one translation unit).
+// Shares nothing with oracle/.
+#pragma once
+
+namespace {
+
+using kvt::Job;
+using kvt::Piece;
+
+constexpr int kBlobSlots = 16;
+constexpr int kMaxStagingSlots = 4;
+constexpr uint32_t kMaxLayersKv = 4096;  // layer_count * kv_count
+constexpr uint64_t kAutoStagedMinBytes = 16ull << 20;
+constexpr uint64_t kAutoVecMinBytes = 40ull << 20, kAutoVecMaxBytes = 384ull << 20;  // AUTO: vec kernel in between
+constexpr uint32_t kSchedSlots = 256;  // claim counters, handed out round-robin per launch
+constexpr int kStaticSmemReserve = 8192;  // static shared memory of kv_move_bulk (barriers + stage metadata, 6 KiB) rounded up
+
+enum KernelKind { KERNEL_AUTO = 0, KERNEL_BULK = 1, KERNEL_VEC = 2, KERNEL_ELEM = 3 };
+
+// Tensor maps of one HND pool for one box size (kv_kernels.cuh "TMA tensor maps"): built once per
+// (pool, box) and kept in device memory for the life of the ctx.
+struct MapSet {
+  std::vector<uint64_t> key;  // slab bases + every descriptor field the maps depend on + box tokens
+  void *d = nullptr;          // device array of LC CUtensorMap
+};
+constexpr size_t kMaxMapSets = 64;
+typedef CUresult (*EncodeTiledFn)(CUtensorMap *, CUtensorMapDataType, cuuint32_t, void *, const cuuint64_t *,
+                                  const cuuint64_t *, const cuuint32_t *, const cuuint32_t *, CUtensorMapInterleave,
+                                  CUtensorMapSwizzle, CUtensorMapL2promotion, CUtensorMapFloatOOBfill);
+
+struct BlobSlot {
+  void *h = nullptr;  // pinned host
+  void *d = nullptr;  // device
+  size_t cap = 0;
+  cudaEvent_t ev = nullptr;  // recorded after the last kernel that reads `d`
+  bool used = false;
+};
+
+}  // namespace
+
+struct kv_ctx {
+  int device = -1;
+  bool host_only = false;
+  int sm_count = 148;
+  int max_smem = 0;
+  cudaStream_t side = nullptr;
+  cudaEvent_t ev_entry = nullptr;
+  BlobSlot blobs[kBlobSlots];
+  uint32_t next_blob = 0;
+  uint32_t *d_status = nullptr;
+  // staging for KV_HOST_STAGED
+  void *staging = nullptr;
+  size_t staging_bytes = 0;
+  cudaEvent_t ev_full[kMaxStagingSlots] = {};  // producer into the slot finished
+  cudaEvent_t ev_free[kMaxStagingSlots] = {};  // consumer of the slot finished
+  bool free_valid[kMaxStagingSlots] = {};
+  int last_cuda_error = 0;
+  // options
+  int kernel = KERNEL_AUTO;
+  uint32_t stage_bytes = 16384, stages = 4, warps = 2, lag = 2, max_ctas = 0, host_max_ctas = 0;
+  // bulk geometry of transposing transfers (an HND pool): rows are gathered with 16-byte cp.async by all
+  // lanes, which wants more, shallower issuing warps (measured: 8 x 4 x 4 KiB)
+  uint32_t t_stage_bytes = 4096, t_stages = 4, t_warps = 8;
+  uint32_t staging_slots = 2, l2_hint = 0, inline_tables = 1, dynamic = 1, tensor_maps = 1, pdl = 1;
+  uint32_t next_sched = 0;
+  EncodeTiledFn encode_tiled = nullptr;  // cuTensorMapEncodeTiled, nullptr if the driver has none
+  std::vector<MapSet> map_sets;
+  cudaStream_t cur_stream = nullptr;     // stream of the entry point being served (capture check while planning)
+  uint64_t last_tma = 0;
+  size_t chunk_bytes = 0;
+  // stats
+  uint64_t launches = 0, memcpys = 0, last_items = 0, last_payload = 0, last_kernel = 0,
+           last_mode = 0, last_grid = 0, last_segment = 0;
+};
+
+namespace {
+
+#define KV_CUDA(ctx, expr)                         \
+  do {                                             \
+    cudaError_t e__ = (expr);                      \
+    if (e__ != cudaSuccess) {                      \
+      (ctx)->last_cuda_error = (int)e__;           \
+      (void)cudaGetLastError();                    \
+      return KV_ERR_CUDA;                          \
+    }                                              \
+  } while (0)
+
+struct DeviceGuard {
+  int prev = -1;
+  bool active = false;
+  explicit DeviceGuard(const kv_ctx *ctx) {
+    if (ctx->host_only) return;
+    if (cudaGetDevice(&prev) == cudaSuccess && prev != ctx->device) {
+      cudaSetDevice(ctx->device);
+      active = true;
+    }
+  }
+  ~DeviceGuard() {
+    if (active) cudaSetDevice(prev);
+  }
+};
+
+
+}  // namespace

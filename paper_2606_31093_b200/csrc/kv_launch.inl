@@ -1,0 +1,191 @@
+// kv_launch.inl -- lookup tables of a launch (inline in the kernel parameters, or staged through the pinned ring) and the launches themselves
+// Part of the host side of libkvtier.so; included by kvtier.cu only (one translation unit).
+// Shares nothing with oracle/.
+#pragma once
+
+namespace {
+
+// ---------------------------------------------------------------------------------------------
+// blob = [bases: LC x u64][pieces: n x Piece][ids: n_ids x i32], staged through a pinned ring
+// ---------------------------------------------------------------------------------------------
+struct HostBlob {
+  std::vector<uint8_t> bytes;
+  size_t off_pieces = 0, off_ids = 0;
+};
+
+void build_blob(const kv_pool_desc *p, const Geom &g, const std::vector<Piece> &pieces,
+                const int32_t *ids, uint64_t n_ids, bool ids_on_device, HostBlob *hb) {
+  hb->off_pieces = (size_t)g.LC * 8 * (g.src_pool ? 2 : 1);
+  hb->off_ids = hb->off_pieces + pieces.size() * sizeof(Piece);
+  hb->bytes.resize(hb->off_ids + (ids_on_device ? 0 : (size_t)n_ids * 4));
+  uint8_t *h = hb->bytes.data();
+  for (uint32_t i = 0; i < g.LC; ++i) ((uint64_t *)h)[i] = (uint64_t)(uintptr_t)p->base[i];
+  if (g.src_pool)
+    for (uint32_t i = 0; i < g.LC; ++i) ((uint64_t *)h)[g.LC + i] = (uint64_t)(uintptr_t)g.src_pool->base[i];
+  std::memcpy(h + hb->off_pieces, pieces.data(), pieces.size() * sizeof(Piece));
+  if (!ids_on_device && n_ids) std::memcpy(h + hb->off_ids, ids, (size_t)n_ids * 4);
+}
+
+// Tables of a launch: either resident in device memory (slot of the pinned ring) or carried
+// inside the kernel parameters (inline; no copy, no slot).
+struct Blob {
+  BlobSlot *slot = nullptr;
+  const uint64_t *d_bases = nullptr;
+  const Piece *d_pieces = nullptr;
+  const int32_t *d_ids = nullptr;  // also set for caller-supplied device ids in inline mode
+  const HostBlob *inl = nullptr;   // non-null: inline tables
+};
+
+int upload_blob(kv_ctx *ctx, const HostBlob &hb, const int32_t *ids, bool ids_on_device,
+                cudaStream_t s, Blob *out) {
+  const size_t bytes = hb.bytes.size();
+  BlobSlot &slot = ctx->blobs[ctx->next_blob++ % kBlobSlots];
+  if (slot.used) KV_CUDA(ctx, cudaEventSynchronize(slot.ev));  // last reader of this slot is done
+  if (slot.cap < bytes) {
+    if (slot.h) cudaFreeHost(slot.h);
+    if (slot.d) cudaFree(slot.d);
+    slot.h = slot.d = nullptr; slot.cap = 0;
+    size_t cap = std::max<size_t>(65536, bytes + bytes / 2);
+    KV_CUDA(ctx, cudaMallocHost(&slot.h, cap));
+    KV_CUDA(ctx, cudaMalloc(&slot.d, cap));
+    slot.cap = cap;
+  }
+  std::memcpy(slot.h, hb.bytes.data(), bytes);
+  KV_CUDA(ctx, cudaMemcpyAsync(slot.d, slot.h, bytes, cudaMemcpyHostToDevice, s));
+  ctx->memcpys++;
+  slot.used = true;
+  out->slot = &slot;
+  out->d_bases = (const uint64_t *)slot.d;
+  out->d_pieces = (const Piece *)((uint8_t *)slot.d + hb.off_pieces);
+  out->d_ids = ids_on_device ? ids : (const int32_t *)((uint8_t *)slot.d + hb.off_ids);
+  return KV_OK;
+}
+
+constexpr int kInlineSmall = 3840;   // whole parameter block stays under the classic 4 KiB
+constexpr int kInlineLarge = 31744;  // CUDA 12.1+ large kernel parameters (<= 32,764 B)
+
+template <int N>
+void launch_bulk(const Job &j, const HostBlob *hb, bool trans, uint32_t grid, uint32_t block, size_t smem,
+                 cudaStream_t s, bool pdl) {
+  static thread_local kvt::JobT<N> p;
+  p.j = j;
+  if constexpr (N > 0) std::memcpy(p.blob, hb->bytes.data(), hb->bytes.size());
+  // Programmatic dependent launch: this grid may become resident while the previous kernel of the stream
+  // is still draining (its CTAs leave half of each SM's shared memory free); it runs its prologue and then
+  // blocks in griddepcontrol.wait until that kernel has completed and flushed.
+  cudaLaunchAttribute attr[1];
+  attr[0].id = cudaLaunchAttributeProgrammaticStreamSerialization;
+  attr[0].val.programmaticStreamSerializationAllowed = 1;
+  cudaLaunchConfig_t cfg = {};
+  cfg.gridDim = dim3(grid); cfg.blockDim = dim3(block); cfg.dynamicSmemBytes = smem; cfg.stream = s;
+  cfg.attrs = attr; cfg.numAttrs = pdl ? 1 : 0;
+  if (trans) (void)cudaLaunchKernelEx(&cfg, kvt::kv_move_bulk<N, true>, p);
+  else (void)cudaLaunchKernelEx(&cfg, kvt::kv_move_bulk<N, false>, p);
+}
+template <int N>
+void launch_vec(const Job &j, const HostBlob *hb, bool trans, uint32_t grid, cudaStream_t s) {
+  static thread_local kvt::JobT<N> p;
+  p.j = j;
+  if constexpr (N > 0) std::memcpy(p.blob, hb->bytes.data(), hb->bytes.size());
+  if (trans) kvt::kv_move_vec<8, N, true><<<grid, 256, 0, s>>>(p);
+  else kvt::kv_move_vec<8, N, false><<<grid, 256, 0, s>>>(p);
+}
+template <typename U>
+void launch_elem(const kvt::JobT<0> &p, bool trans, uint32_t grid, cudaStream_t s) {
+  if (trans) kvt::kv_move_elem<U, true><<<grid, 256, 0, s>>>(p);
+  else kvt::kv_move_elem<U, false><<<grid, 256, 0, s>>>(p);
+}
+
+// lc0 / lc_count: the launch covers slabs [lc0, lc0 + lc_count) of the call only (layer-range chunks of the
+// layer-first staged pipeline; tables in device memory); lc_count == 0: all of them.
+int launch(kv_ctx *ctx, const Geom &g, const Blob &b, uint32_t piece_first, uint32_t n_pieces,
+           uint64_t total_items, uint32_t cta_cap, cudaStream_t s, uint32_t lc0 = 0, uint32_t lc_count = 0) {
+  if (!total_items) return KV_OK;
+  Job j{};
+  j.bases = b.d_bases ? b.d_bases + lc0 : nullptr; j.ids = b.d_ids;
+  j.pieces = b.d_pieces ? b.d_pieces + piece_first : nullptr;
+  if (b.inl) { j.off_pieces = (uint32_t)b.inl->off_pieces; j.off_ids = (uint32_t)b.inl->off_ids; }
+  j.status = ctx->d_status;
+  j.total_items = total_items;
+  j.page_stride = g.page_stride; j.buf_row_bytes = g.buf_row; j.buf_page_bytes = g.buf_page;
+  j.n_pieces = n_pieces; j.LC = lc_count ? lc_count : g.LC; j.dir = (uint32_t)g.dir; j.layout = (uint32_t)g.layout;
+  j.g = g.g; j.cpp_pool = g.Tpool / g.g; j.cpp_buf = g.Tbuf / g.g;
+  j.tokrow = g.tokrow; j.chunk_bytes = g.chunk_bytes; j.sub_bytes = g.sub_bytes; j.subs = g.subs;
+  j.num_pages = g.num_pages;
+  if (g.src_pool) { j.src_num_pages = g.src_pool->num_pages; j.src_page_stride = g.src_pool->page_stride_bytes; }
+  j.src_ids = g.dev_src_ids;
+  j.drow = g.drow; j.H = g.H;
+  if (g.trans) {
+    // the pool of this geometry is the destination pool of dir 2 and "the" pool otherwise; g.Tpool is its page size
+    j.pool_hnd = g.pool_hnd; j.src_hnd = g.src_hnd;
+    j.p_ts = g.drow; j.p_hs = (uint64_t)g.Tpool * g.drow;
+    j.q_ts = g.drow; j.q_hs = (uint64_t)g.Tbuf * g.drow;  // dir 2: Tbuf is the source pool's page size
+  }
+  ctx->last_tma = 0;
+  if (g.tma && g.kernel == KERNEL_BULK) {
+    j.tb = g.tb;
+    if (g.pool_hnd) {
+      int rc = get_maps(ctx, g.dst_pool, g.L, g.tb, g.tma_es, &j.maps_pool);
+      if (rc) return rc;
+    }
+    if (g.src_hnd) {
+      int rc = get_maps(ctx, g.src_pool, g.L, g.tb, g.tma_es, &j.maps_src);
+      if (rc) return rc;
+    }
+    if (j.maps_pool) j.maps_pool += (size_t)lc0 * sizeof(CUtensorMap);
+    ctx->last_tma = 1;
+  }
+  uint32_t cap = cta_cap ? cta_cap : ctx->max_ctas;
+  uint32_t grid = 0;
+  if (g.kernel == KERNEL_BULK) {
+    const bool lane_geom = g.trans && !g.tma;  // row gathers by all lanes want more, shallower warps
+    j.stage_bytes = (g.sub_bytes + 127) / 128 * 128;
+    j.stages = lane_geom ? ctx->t_stages : ctx->stages; j.lag = std::min(ctx->lag, j.stages - 1);
+    j.zero_bytes = std::min<uint32_t>(4096, j.stage_bytes);
+    j.l2_hint = ctx->l2_hint;
+    uint32_t warps = lane_geom ? ctx->t_warps : ctx->warps;
+    size_t smem = (size_t)j.zero_bytes + (size_t)warps * j.stages * j.stage_bytes;
+    while (smem > (size_t)ctx->max_smem - kStaticSmemReserve && j.stages > 2) {  // static smem holds barriers + meta
+      --j.stages; j.lag = std::min(j.lag, j.stages - 1);
+      smem = (size_t)j.zero_bytes + (size_t)warps * j.stages * j.stage_bytes;
+    }
+    while (smem > (size_t)ctx->max_smem - kStaticSmemReserve && warps > 1) {
+      --warps;
+      smem = (size_t)j.zero_bytes + (size_t)warps * j.stages * j.stage_bytes;
+    }
+    const uint64_t want = (total_items + warps - 1) / warps;
+    grid = (uint32_t)std::min<uint64_t>(want, cap ? cap : (uint32_t)ctx->sm_count);
+    const uint64_t G = (uint64_t)grid * warps;
+    if (ctx->dynamic && total_items >= 8 * G && !capturing(s)) {  // enough work for claiming to pay
+      uint8_t *slot = (uint8_t *)ctx->d_status + 256 + (size_t)(ctx->next_sched++ % kSchedSlots) * 16;
+      j.sched = (unsigned long long *)slot;
+      j.sched_done = (uint32_t *)(slot + 8);
+      j.first_batch = (uint32_t)std::min<uint64_t>(32, total_items / (4 * G));
+    }
+    const bool pdl = ctx->pdl && !capturing(s);
+    if (!b.inl) launch_bulk<0>(j, nullptr, g.trans, grid, warps * 32, smem, s, pdl);
+    else if (b.inl->bytes.size() <= kInlineSmall) launch_bulk<kInlineSmall>(j, b.inl, g.trans, grid, warps * 32, smem, s, pdl);
+    else launch_bulk<kInlineLarge>(j, b.inl, g.trans, grid, warps * 32, smem, s, pdl);
+  } else {
+    const uint32_t wpb = 8;  // warps per 256-thread CTA
+    const uint64_t want = (total_items + wpb - 1) / wpb;
+    grid = (uint32_t)std::min<uint64_t>(want, cap ? cap : (uint32_t)ctx->sm_count * 8);
+    kvt::JobT<0> p0;
+    p0.j = j;
+    if (g.kernel == KERNEL_VEC) {
+      if (!b.inl) launch_vec<0>(j, nullptr, g.trans, grid, s);
+      else if (b.inl->bytes.size() <= kInlineSmall) launch_vec<kInlineSmall>(j, b.inl, g.trans, grid, s);
+      else launch_vec<kInlineLarge>(j, b.inl, g.trans, grid, s);
+    }
+    else if (g.unit >= 8) launch_elem<uint64_t>(p0, g.trans, grid, s);
+    else if (g.unit == 4) launch_elem<uint32_t>(p0, g.trans, grid, s);
+    else if (g.unit == 2) launch_elem<uint16_t>(p0, g.trans, grid, s);
+    else launch_elem<uint8_t>(p0, g.trans, grid, s);
+  }
+  KV_CUDA(ctx, cudaGetLastError());
+  ctx->launches++;
+  ctx->last_grid = grid;
+  return KV_OK;
+}
+
+}  // namespace

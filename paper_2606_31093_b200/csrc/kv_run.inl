@@ -1,0 +1,309 @@
+// kv_run.inl -- execution: one launch (device / DIRECT host), or the STAGED chunk pipeline between the kernels and the copy engines
+// Part of the host side of libkvtier.so; included by kvtier.cu only (one translation unit).
+// Shares nothing with oracle/.
+#pragma once
+
+namespace {
+
+// one launch over all requests (device buffers, or mapped pinned host buffers = DIRECT mode)
+int run_single_launch(kv_ctx *ctx, const kv_pool_desc *pools, const Call &c, const int32_t *ids,
+                      uint32_t flags, uint32_t cta_cap, cudaStream_t s) {
+  std::vector<Piece> pieces;
+  pieces.reserve(c.reqs.size());
+  uint64_t acc = 0;
+  for (const Req &q : c.reqs) {
+    Piece pc;
+    pc.item_begin = acc; pc.buf = q.buf; pc.n_tokens = q.n_tokens; pc.id_begin = q.id_begin;
+    pc.n_buf_pages = q.n_buf_pages;
+    pieces.push_back(pc);
+    acc += q.items;
+  }
+  const bool dev_ids = flags & KV_FLAG_IDS_ON_DEVICE;
+  HostBlob hb;
+  build_blob(pools, c.geom, pieces, ids, c.n_ids, dev_ids, &hb);
+  Blob b;
+  if (ctx->inline_tables && c.geom.kernel != KERNEL_ELEM && hb.bytes.size() <= (size_t)kInlineLarge) {
+    b.inl = &hb;  // tables travel inside the kernel parameters: one launch, no copy
+    b.d_ids = dev_ids ? ids : nullptr;
+    return launch(ctx, c.geom, b, 0, (uint32_t)pieces.size(), acc, cta_cap, s);
+  }
+  if (capturing(s)) return KV_ERR_CAPTURE;
+  int rc = upload_blob(ctx, hb, ids, dev_ids, s, &b);
+  if (rc) return rc;
+  rc = launch(ctx, c.geom, b, 0, (uint32_t)pieces.size(), acc, cta_cap, s);
+  if (rc) return rc;
+  KV_CUDA(ctx, cudaEventRecord(b.slot->ev, s));
+  return KV_OK;
+}
+
+int ensure_staging(kv_ctx *ctx) {
+  if (ctx->staging) return KV_OK;
+  if (!ctx->staging_bytes) ctx->staging_bytes = (size_t)128 << 20;
+  KV_CUDA(ctx, cudaMalloc(&ctx->staging, ctx->staging_bytes));
+  return KV_OK;
+}
+
+// KV_HOST_STAGED: the flattened page sequence of all requests is cut into chunks that fit one
+// staging slot; per chunk: kernel <-> slot on `s`, copy engine slot <-> pinned host on the side
+// stream, double (or deeper) buffered with events.  Page-first only (a chunk of pages is then
+// contiguous in the host buffer); layer-first falls back to DIRECT.
+// Layer flags of kv_reload_layerwise: after the pages of layers [l0, l0 + n) have landed in the pool,
+// flags[l] = value is stored (release, system scope) in stream order.
+struct LayerFlags { uint64_t *flags = nullptr; uint64_t value = 0; };
+
+int run_staged(kv_ctx *ctx, const kv_pool_desc *pools, const Call &c, const int32_t *ids,
+               uint32_t flags, cudaStream_t s, LayerFlags lf = LayerFlags()) {
+  int rc = ensure_staging(ctx);
+  if (rc) return rc;
+  const Geom &g = c.geom;
+  const uint32_t n_slots = ctx->staging_slots;
+  // unit of chunking: tokens that are whole pages on both sides
+  const uint64_t unit_tokens = (uint64_t)g.Tpool / g.g * g.Tbuf;  // lcm(Tpool, Tbuf)
+  const bool layer_first = g.layout == KV_LAYOUT_LAYER_FIRST;
+  const uint64_t unit_bytes = unit_tokens * g.tokrow * (layer_first ? g.C : g.LC);
+  size_t slot_bytes = ctx->staging_bytes / n_slots / 256 * 256;
+  if (ctx->chunk_bytes) slot_bytes = std::min(slot_bytes, ctx->chunk_bytes / 256 * 256);
+  if (slot_bytes < unit_bytes) return KV_ERR_SIZE;
+  const uint64_t chunk_tokens = slot_bytes / unit_bytes * unit_tokens;
+
+  // A chunk = what one staging slot holds: pieces for the kernel, copies for the copy engine.  Page-first:
+  // a run of whole pages, all layers (contiguous in the host buffer).  Layer-first: a range of layers
+  // [l0, l0 + nl) of one or more page ranges; every (layer, K|V) of a page range is one contiguous host run.
+  struct Chunk { uint32_t piece_first, n_pieces; uint64_t items; uint32_t l0, nl, sig_n; };
+  struct Copy { uint64_t host, dev_off, bytes; };
+  std::vector<Piece> pieces;
+  std::vector<Chunk> chunks;
+  std::vector<std::vector<Copy>> copies;
+  if (layer_first) {
+    const uint64_t row = g.buf_row;  // bytes of one buffer page of one (layer, K|V)
+    uint64_t widest = 1;
+    for (const Req &q : c.reqs) widest = std::max<uint64_t>(widest, q.n_buf_pages);
+    // as many layers per chunk as the widest request allows; a request wider than a slot is cut by page ranges
+    const uint32_t kl = (uint32_t)std::min<uint64_t>(g.L, std::max<uint64_t>(1, slot_bytes / (widest * g.C * row)));
+    const uint64_t unit_pool_pages = unit_tokens / g.Tpool;
+    for (uint32_t l0 = 0; l0 < g.L; l0 += kl) {
+      const uint32_t nl = std::min(kl, g.L - l0);
+      const uint64_t per_buf_page = (uint64_t)nl * g.C * row;  // slot bytes one buffer page costs in this layer range
+      const uint64_t max_pool_pages = slot_bytes / per_buf_page * g.Tbuf / g.Tpool / unit_pool_pages * unit_pool_pages;
+      if (!max_pool_pages) return KV_ERR_SIZE;
+      Chunk cur{(uint32_t)pieces.size(), 0, 0, l0, nl, 0};
+      std::vector<Copy> cur_copies;
+      uint64_t fill = 0;
+      auto close = [&]() {
+        if (cur.n_pieces) { chunks.push_back(cur); copies.push_back(cur_copies); }
+        cur = Chunk{(uint32_t)pieces.size(), 0, 0, l0, nl, 0};
+        cur_copies.clear();
+        fill = 0;
+      };
+      for (const Req &q : c.reqs) {
+        for (uint64_t q0 = 0; q0 < q.n_ids; q0 += max_pool_pages) {
+          const uint64_t q1 = std::min(q.n_ids, q0 + max_pool_pages);
+          const uint64_t t0 = q0 * g.Tpool, t1 = q1 * g.Tpool;
+          const uint64_t b0 = std::min(t0 / g.Tbuf, q.n_buf_pages);
+          const uint64_t b1 = std::min((t1 + g.Tbuf - 1) / g.Tbuf, q.n_buf_pages);
+          const uint64_t nb = b1 - b0, region = nb * per_buf_page;
+          if (fill + region > slot_bytes) close();
+          Piece pc;
+          pc.item_begin = cur.items;
+          pc.buf = fill;  // offset within the slot; the slot base is added below
+          pc.n_tokens = q.n_tokens > t0 ? std::min(q.n_tokens - t0, t1 - t0) : 0;
+          pc.id_begin = q.id_begin + q0;
+          pc.n_buf_pages = nb;
+          pieces.push_back(pc);
+          cur.n_pieces++;
+          cur.items += (q1 - q0) * (g.Tpool / g.g) * nl * g.C * g.subs;
+          if (nb)
+            for (uint32_t l = 0; l < nl; ++l)
+              for (uint32_t kc = 0; kc < g.C; ++kc)
+                cur_copies.push_back(Copy{q.buf + (((uint64_t)(l0 + l) * g.C + kc) * q.n_buf_pages + b0) * row,
+                                          fill + ((uint64_t)l * g.C + kc) * nb * row, nb * row});
+          fill += (region + 255) / 256 * 256;
+        }
+      }
+      close();
+      if (!chunks.empty()) chunks.back().sig_n = nl;  // layers [l0, l0 + nl) are complete after this chunk
+    }
+  } else {
+    uint64_t fill_tokens = 0;  // tokens (in buffer-page units) already placed in the open chunk
+    Chunk cur{0, 0, 0, 0, g.L, 0};
+    std::vector<Copy> cur_copies;
+    auto close = [&]() {
+      if (cur.n_pieces) { chunks.push_back(cur); copies.push_back(cur_copies); }
+      cur = Chunk{(uint32_t)pieces.size(), 0, 0, 0, g.L, 0};
+      cur_copies.clear();
+      fill_tokens = 0;
+    };
+    for (const Req &q : c.reqs) {
+      // the request covers n_ids pool pages = n_ids*Tpool token slots; its buffer holds
+      // n_buf_pages*Tbuf token slots.  Walk it in token ranges [t0, t1) of whole units.
+      const uint64_t slots_pool = q.n_ids * g.Tpool;
+      uint64_t t0 = 0;
+      while (t0 < slots_pool) {
+        if (fill_tokens == chunk_tokens) close();
+        const uint64_t t1 = std::min(slots_pool, t0 + (chunk_tokens - fill_tokens));
+        const uint64_t span = t1 - t0;  // multiple of Tpool; multiple of unit except at the request's end
+        const uint64_t buf_pages = (std::min(t1, q.n_buf_pages * g.Tbuf) - std::min(t0, q.n_buf_pages * g.Tbuf) + g.Tbuf - 1) / g.Tbuf;
+        const uint64_t dev_off = fill_tokens * g.tokrow * g.LC;
+        Piece pc;
+        pc.item_begin = cur.items;
+        pc.buf = (uint64_t)(uintptr_t)ctx->staging;  // + slot base, patched per chunk below
+        pc.buf = dev_off;                              // offset within the slot for now
+        pc.n_tokens = q.n_tokens > t0 ? std::min(q.n_tokens - t0, span) : 0;
+        pc.id_begin = q.id_begin + t0 / g.Tpool;
+        pc.n_buf_pages = buf_pages;
+        pieces.push_back(pc);
+        cur.n_pieces++;
+        cur.items += items_of(g, span / g.Tpool);
+        if (buf_pages)
+          cur_copies.push_back(Copy{q.buf + t0 / g.Tbuf * g.buf_page, dev_off, buf_pages * g.buf_page});
+        // buffer-page units consumed in the slot (a ragged tail still occupies whole units)
+        fill_tokens += (span + unit_tokens - 1) / unit_tokens * unit_tokens;
+        t0 = t1;
+      }
+    }
+    close();
+  }
+  // patch slot bases
+  for (size_t ci = 0; ci < chunks.size(); ++ci) {
+    const uint64_t base = (uint64_t)(uintptr_t)ctx->staging + (ci % n_slots) * slot_bytes;
+    for (uint32_t k = 0; k < chunks[ci].n_pieces; ++k) pieces[chunks[ci].piece_first + k].buf += base;
+  }
+  HostBlob hb;
+  build_blob(pools, g, pieces, ids, c.n_ids, flags & KV_FLAG_IDS_ON_DEVICE, &hb);
+  Blob b;
+  rc = upload_blob(ctx, hb, ids, flags & KV_FLAG_IDS_ON_DEVICE, s, &b);
+  if (rc) return rc;
+  KV_CUDA(ctx, cudaEventRecord(ctx->ev_entry, s));
+  KV_CUDA(ctx, cudaStreamWaitEvent(ctx->side, ctx->ev_entry, 0));
+  for (size_t ci = 0; ci < chunks.size(); ++ci) {
+    const uint32_t slot = (uint32_t)(ci % n_slots);
+    uint8_t *slot_base = (uint8_t *)ctx->staging + (size_t)slot * slot_bytes;
+    if (g.dir == 0) {  // offload: kernel fills the slot on s, copy engine drains it on side
+      if (ctx->free_valid[slot]) KV_CUDA(ctx, cudaStreamWaitEvent(s, ctx->ev_free[slot], 0));
+      rc = launch(ctx, g, b, chunks[ci].piece_first, chunks[ci].n_pieces, chunks[ci].items, 0, s,
+                  chunks[ci].l0 * g.C, chunks[ci].nl * g.C);
+      if (rc) return rc;
+      KV_CUDA(ctx, cudaEventRecord(ctx->ev_full[slot], s));
+      KV_CUDA(ctx, cudaStreamWaitEvent(ctx->side, ctx->ev_full[slot], 0));
+      for (const Copy &cp : copies[ci]) {
+        KV_CUDA(ctx, cudaMemcpyAsync((void *)(uintptr_t)cp.host, slot_base + cp.dev_off, cp.bytes,
+                                     cudaMemcpyDeviceToHost, ctx->side));
+        ctx->memcpys++;
+      }
+      KV_CUDA(ctx, cudaEventRecord(ctx->ev_free[slot], ctx->side));
+      ctx->free_valid[slot] = true;
+    } else {  // reload: copy engine fills the slot on side, kernel drains it on s
+      if (ctx->free_valid[slot]) KV_CUDA(ctx, cudaStreamWaitEvent(ctx->side, ctx->ev_free[slot], 0));
+      for (const Copy &cp : copies[ci]) {
+        KV_CUDA(ctx, cudaMemcpyAsync(slot_base + cp.dev_off, (const void *)(uintptr_t)cp.host,
+                                     cp.bytes, cudaMemcpyHostToDevice, ctx->side));
+        ctx->memcpys++;
+      }
+      KV_CUDA(ctx, cudaEventRecord(ctx->ev_full[slot], ctx->side));
+      KV_CUDA(ctx, cudaStreamWaitEvent(s, ctx->ev_full[slot], 0));
+      rc = launch(ctx, g, b, chunks[ci].piece_first, chunks[ci].n_pieces, chunks[ci].items, 0, s,
+                  chunks[ci].l0 * g.C, chunks[ci].nl * g.C);
+      if (rc) return rc;
+      if (lf.flags && chunks[ci].sig_n) {  // these layers' pages are in the pool: publish
+        kvt::kv_signal_range<<<1, 32, 0, s>>>(lf.flags + chunks[ci].l0, chunks[ci].sig_n, lf.value);  // strides over > 32
+        KV_CUDA(ctx, cudaGetLastError());
+        ctx->launches++;
+      }
+      KV_CUDA(ctx, cudaEventRecord(ctx->ev_free[slot], s));
+      ctx->free_valid[slot] = true;
+    }
+  }
+  if (g.dir == 0) {  // join the copy engine's tail back into s
+    const size_t first = chunks.size() > n_slots ? chunks.size() - n_slots : 0;
+    for (size_t ci = first; ci < chunks.size(); ++ci)
+      KV_CUDA(ctx, cudaStreamWaitEvent(s, ctx->ev_free[ci % n_slots], 0));
+  }
+  KV_CUDA(ctx, cudaEventRecord(b.slot->ev, s));
+  return KV_OK;
+}
+
+// Is `p` pinned host memory?  Returns its device alias (UVA: normally the same address).
+int host_alias(kv_ctx *ctx, const void *p, uint64_t *alias) {
+  cudaPointerAttributes a;
+  cudaError_t e = cudaPointerGetAttributes(&a, p);
+  if (e != cudaSuccess) { (void)cudaGetLastError(); return KV_ERR_HOST_MEM; }
+  if (a.type != cudaMemoryTypeHost || !a.devicePointer) return KV_ERR_HOST_MEM;
+  (void)ctx;
+  *alias = (uint64_t)(uintptr_t)a.devicePointer;
+  return KV_OK;
+}
+
+int resolve_mode(const kv_ctx *ctx, int mode, const Call &c, int *out) {
+  if (mode != KV_HOST_AUTO && mode != KV_HOST_DIRECT && mode != KV_HOST_STAGED) return KV_ERR_LAYOUT;
+  int m = mode;
+  // Measured on B200 / PCIe Gen5 x16: the copy engines reach 98-99 % of the
+  // cudaMemcpy peak, SM-issued stores/loads over the link 92 % (128-byte TLP payloads); below
+  // ~16 MiB both are latency-bound and equal, and DIRECT is one launch with no staging traffic.
+  if (m == KV_HOST_AUTO) m = c.payload >= kAutoStagedMinBytes ? KV_HOST_STAGED : KV_HOST_DIRECT;
+  (void)ctx;
+  *out = m;
+  return KV_OK;
+}
+
+// Device alias of a flag word (device memory, or mapped pinned host memory).
+int flag_alias(const void *p, uint64_t **out) {
+  cudaPointerAttributes a;
+  if (cudaPointerGetAttributes(&a, p) != cudaSuccess) { (void)cudaGetLastError(); return KV_ERR_HOST_MEM; }
+  if (a.type == cudaMemoryTypeUnregistered) return KV_ERR_HOST_MEM;
+  if (a.type == cudaMemoryTypeHost) {
+    if (!a.devicePointer) return KV_ERR_HOST_MEM;
+    *out = (uint64_t *)a.devicePointer;
+  } else {
+    *out = (uint64_t *)p;
+  }
+  return KV_OK;
+}
+
+int run_host(kv_ctx *ctx, const kv_pool_desc *pools, Call &c, const int32_t *ids, int mode,
+             uint32_t flags, cudaStream_t s, LayerFlags lf = LayerFlags()) {
+  int m = 0;
+  int rc = resolve_mode(ctx, mode, c, &m);
+  if (rc) return rc;
+  note_plan(ctx, c);
+  ctx->last_mode = (uint64_t)m;
+  if (c.reqs.empty()) return KV_OK;  // n == 0: nothing to do, no launch
+  if (ctx->host_only) return KV_ERR_NO_DEVICE;
+  DeviceGuard guard(ctx);
+  if (capturing(s)) {  // the chunk pipeline (side stream, staging slots, table upload) is not replayable
+    if (mode == KV_HOST_STAGED) return KV_ERR_CAPTURE;
+    m = KV_HOST_DIRECT;
+    ctx->last_mode = (uint64_t)m;
+  }
+  for (Req &q : c.reqs) {
+    uint64_t alias = 0;
+    rc = host_alias(ctx, (const void *)(uintptr_t)q.buf, &alias);
+    if (rc) return rc;
+    if (m == KV_HOST_DIRECT) q.buf = alias;
+  }
+  if (lf.flags) {
+    rc = flag_alias(lf.flags, &lf.flags);
+    if (rc) return rc;
+  }
+  if (m == KV_HOST_DIRECT) {  // one launch moves every layer: the flags follow it together
+    rc = run_single_launch(ctx, pools, c, ids, flags, ctx->host_max_ctas, s);
+    if (rc || !lf.flags) return rc;
+    for (uint32_t l0 = 0; l0 < c.geom.L; l0 += 32) {
+      kvt::kv_signal_range<<<1, 32, 0, s>>>(lf.flags + l0, std::min(32u, c.geom.L - l0), lf.value);
+      KV_CUDA(ctx, cudaGetLastError());
+      ctx->launches++;
+    }
+    return KV_OK;
+  }
+  return run_staged(ctx, pools, c, ids, flags, s, lf);
+}
+
+int run_device(kv_ctx *ctx, const kv_pool_desc *pools, const Call &c, const int32_t *ids,
+               uint32_t flags, cudaStream_t s) {
+  note_plan(ctx, c);
+  if (c.reqs.empty()) return KV_OK;  // n == 0: nothing to do, no launch
+  if (ctx->host_only) return KV_ERR_NO_DEVICE;
+  DeviceGuard guard(ctx);
+  return run_single_launch(ctx, pools, c, ids, flags, 0, s);
+}
+
+}  // namespace
