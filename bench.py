@@ -260,6 +260,8 @@ def run_ours(args):
             ev[2 * i + 2].record(stream)
         barrier()
         launches = ctx.stat(kv.KV_STAT_LAUNCHES) - l0
+        kern_name = {kv.KV_KERNEL_BULK: "kv_move_bulk", kv.KV_KERNEL_VEC: "kv_move_vec",
+                     kv.KV_KERNEL_ELEM: "kv_move_elem"}.get(ctx.stat(kv.KV_STAT_LAST_KERNEL), "?")
         t_total_ms = max_over_ranks(ev[0].elapsed_time(ev[2 * K]))
         pack_ms = float(np.mean([ev[2 * i].elapsed_time(ev[2 * i + 1]) for i in range(K)]))
         unpack_ms = float(np.mean([ev[2 * i + 1].elapsed_time(ev[2 * i + 2]) for i in range(K)]))
@@ -350,8 +352,8 @@ def run_ours(args):
                 "serial_what": "same two calls on ONE stream, reload reading the buffer the offload just wrote",
                 "link_GBps_payload": world * 2 * payload * Ke / (e2e_ms * 1e-3) / 1e9},
         "gpu_launches": launches,
-        "roofline": {"bound": "hbm", "kernel": "kv_move_bulk (kv_pack launch)" if args.pool_order == "nhd"
-                     else "kv_move_bulk<kTrans> with tensor maps (kv_pack launch, HND pool)", "achieved": achieved,
+        "roofline": {"bound": "hbm", "kernel": f"{kern_name} (kv_pack launch)" if args.pool_order == "nhd"
+                     else f"{kern_name}<kTrans> with tensor maps (kv_pack launch, HND pool)", "achieved": achieved,
                      "peak": peak, "unit": "GB/s", "frac": achieved / peak,
                      "traffic": NCU_TRAFFIC_BYTES_PER_LAUNCH if args.pool_order == "nhd" and n == 512 else None, "algorithmic_bytes": 2 * payload,
                      "peak_source": peak_src,
