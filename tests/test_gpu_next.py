@@ -624,3 +624,42 @@ def test_reload_layerwise_publishes_layers_in_order(kv, mode):
         ctx.close()
         kv.kv_host_free(hp)
         kv.kv_host_free(fl_p)
+
+
+def test_reload_layerwise_errors_and_capture(kv, ctx):
+    """Flag array in pageable memory is refused before anything is enqueued; under stream capture the call is one
+    DIRECT launch plus the flag stores, replayable."""
+    L, C, P, T, H, D, e = 4, 2, 64, 16, 2, 64, 2
+    rng = np.random.default_rng(163)
+    B = host_pool(rng, L, C, P, T, H, D, e)
+    tB, dB = to_device(B, kv, torch)
+    n = 20
+    dst = rng.permutation(P)[:n].astype(np.int32)
+    nbytes = n * dB.page_bytes()
+    hp = kv.kv_host_alloc(nbytes)
+    try:
+        src = rng.integers(0, 256, size=nbytes, dtype=np.uint8)
+        kv.host_view(hp, nbytes)[:] = src
+        pageable = np.zeros(L, dtype=np.uint64)
+        with pytest.raises(kv.KvError) as ei:
+            kv.kv_reload_layerwise(ctx, hp, nbytes, dst, dB, L, T, T, n * T, pageable, 1)
+        assert ei.value.status == kv.KV_ERR_HOST_MEM
+        torch.cuda.synchronize()
+        assert_pool_equal(tB, B)  # nothing moved
+        dflags = torch.zeros(L, dtype=torch.int64, device="cuda")
+        side = torch.cuda.Stream()
+        g = torch.cuda.CUDAGraph()
+        with torch.cuda.graph(g, stream=side):
+            kv.kv_reload_layerwise(ctx, hp, nbytes, dst, dB, L, T, T, n * T, dflags, 9, stream=side)
+        assert ctx.stat(kv.KV_STAT_LAST_HOST_MODE) == kv.KV_HOST_DIRECT
+        ko.unpack(src, dst, B, Ts=T, n_tokens=n * T, layout=ko.LAYER_FIRST)
+        for rep in range(2):
+            dflags.zero_()
+            torch.cuda.synchronize()
+            g.replay()
+            torch.cuda.synchronize()
+            assert (dflags == 9).all()
+            assert_pool_equal(tB, B)
+    finally:
+        torch.cuda.synchronize()
+        kv.kv_host_free(hp)
