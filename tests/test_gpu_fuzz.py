@@ -1,6 +1,7 @@
 """Seeded random cases of every transfer against the CPU oracle, byte for byte: random shapes, page
 sizes on both sides, in-page orders, buffer layouts, strides with padding, ragged token counts, CSR
-batches with empty requests, every kernel choice (AUTO / bulk / vec / elem), tensor maps on and off.
+batches with empty requests, every kernel choice (AUTO / bulk / vec / elem), tensor maps on and off,
+PDL / dynamic claiming / inline tables on and off, stage sizes and warp counts of the bulk ring.
 The directed cases live in test_gpu_parity / test_gpu_next / test_gpu_hnd; this file is the net under
 them: each seed draws one configuration and runs pack -> unpack (re-paged) -> fused re-page ->
 copy-on-write append -> host-tier offload / re-paging reload (random mode and pipeline chunk size) on it."""
@@ -34,7 +35,10 @@ def draw(rng):
     return dict(e=e, D=D, H=H, Ts=Ts, Td=Td, L=L, C=C, pad=pad_unit,
                 order_s=int(rng.integers(0, 2)), order_d=int(rng.integers(0, 2)),
                 layout=int(rng.integers(0, 2)), kernel=int(rng.choice([0, 0, 1, 2, 3])),
-                tensor_maps=int(rng.integers(0, 2)), R=int(rng.integers(1, 5)))
+                tensor_maps=int(rng.integers(0, 2)), R=int(rng.integers(1, 5)),
+                pdl=int(rng.integers(0, 2)), dynamic=int(rng.integers(0, 2)), inline=int(rng.integers(0, 2)),
+                stage=int(rng.choice([16384, 16384, 4096, 1024, 8192])), warps=int(rng.choice([2, 2, 1, 4])),
+                max_ctas=int(rng.choice([0, 0, 1, 3])))  # 1 or 3 CTAs: many segments per warp -> guided claiming
 
 
 @pytest.mark.parametrize("seed", range(300))
@@ -46,6 +50,12 @@ def test_random_configuration(kv, seed):
     try:
         ctx.set_option(kv.KV_OPT_KERNEL, c["kernel"])
         ctx.set_option(kv.KV_OPT_TENSOR_MAPS, c["tensor_maps"])
+        ctx.set_option(kv.KV_OPT_PDL, c["pdl"])
+        ctx.set_option(kv.KV_OPT_DYNAMIC, c["dynamic"])
+        ctx.set_option(kv.KV_OPT_INLINE_TABLES, c["inline"])
+        ctx.set_option(kv.KV_OPT_STAGE_BYTES, c["stage"])
+        ctx.set_option(kv.KV_OPT_WARPS, c["warps"])
+        ctx.set_option(kv.KV_OPT_MAX_CTAS, c["max_ctas"])
         # requests: token counts, some empty, ragged against both page sizes
         ntok = [int(rng.choice([0, 1, Ts, Td, Ts * 3 + 1, int(rng.integers(1, 400))])) for _ in range(c["R"])]
         ns = [-(-t // Ts) for t in ntok]
