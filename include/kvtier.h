@@ -312,7 +312,10 @@ int kv_reload(kv_ctx *ctx, const void *host_src, size_t host_bytes, const int32_
  * KV_LAYOUT_LAYER_FIRST by definition.  `layer_flags` is an 8-byte-aligned array of `layer_count` words in
  * device memory or mapped pinned host memory: once every page of layer l (all requests) is in the pool,
  * layer_flags[l] = flag_value is stored with release semantics at system scope, in stream order -- a consumer
- * (the prefill kernel of layer l on another stream, or the host) that acquires the flag may read the layer.
+ * that acquires the flag may read the layer: the host (which then launches layer l's attention), a kernel on
+ * ANOTHER GPU, or a kernel that checks the flag once and does not spin.  Do NOT park a kernel of the same GPU in a
+ * loop on these flags: nothing guarantees that it and the transfer's kernels run at the same time (measured on
+ * this B200 / driver 580: a spinning kernel on one stream kept a kernel of another stream from starting).
  * Flags are stored in ascending layer order.  KV_HOST_STAGED (AUTO's choice from 16 MiB) streams the buffer
  * through the ctx's staging in chunks of whole layers (a layer wider than a staging slot is cut by page
  * ranges), copy engine and scatter kernel pipelined, so layer 0 is usable after ~1/layer_count of the

@@ -663,3 +663,43 @@ def test_reload_layerwise_errors_and_capture(kv, ctx):
     finally:
         torch.cuda.synchronize()
         kv.kv_host_free(hp)
+
+
+def test_layer_ranges_offload_behind_producer_events(kv, ctx):
+    """Offload that follows the producer layer by layer WITHOUT any device-side waiting: a layer range is
+    just a descriptor whose base array starts at that layer, written to that layer's place in the
+    layer-first host buffer; ordering comes from cudaStreamWaitEvent on the producer's per-layer events.
+    (A kernel or stream operation that waits for a flag another stream raises is not used anywhere in
+    this library: nothing guarantees the two run at the same time.)"""
+    L, C, P, T, H, D, e = 6, 2, 300, 16, 4, 128, 2
+    rng = np.random.default_rng(173)
+    final = host_pool(rng, L, C, P, T, H, D, e)
+    t_final = [torch.from_numpy(x).cuda() for x in final.slabs]
+    t_pool = [torch.full_like(x, 0x11) for x in t_final]  # stale
+    n = 200
+    ids = rng.permutation(P)[:n].astype(np.int32)
+    row = T * H * D * e
+    nbytes = n * L * C * row
+    hp = kv.kv_host_alloc(nbytes)
+    try:
+        s_prod, s_off = torch.cuda.Stream(), torch.cuda.Stream()
+        evs = []
+        with torch.cuda.stream(s_prod):
+            for l in range(L):
+                torch.cuda._sleep(500_000)
+                for c in range(C):
+                    t_pool[l * C + c].copy_(t_final[l * C + c])
+                ev = torch.cuda.Event()
+                ev.record(s_prod)
+                evs.append(ev)
+        for l0 in range(0, L, 2):  # ranges of two layers
+            s_off.wait_event(evs[l0 + 1])
+            sub = kv.PoolDesc(t_pool[l0 * C:(l0 + 2) * C], 2, C, P, T, H, D, e)
+            kv.kv_offload(ctx, sub, 2, ids, hp + l0 * C * n * row, 2 * C * n * row,
+                          layout=kv.KV_LAYOUT_LAYER_FIRST, stream=s_off)
+        s_off.synchronize()
+        want = ko.pack(final, ids, layout=ko.LAYER_FIRST)
+        assert np.array_equal(kv.host_view(hp, nbytes), want)
+    finally:
+        torch.cuda.synchronize()
+        kv.kv_host_free(hp)
