@@ -151,7 +151,7 @@ const char *kv_strerror(int status); /* static string, never NULL */
 /* ---- context ------------------------------------------------------------------------------ */
 /* Creates the per-thread context on CUDA device `device`: side stream, events, the ring that
  * stages page-id lists, a device status word and (lazily, on the first STAGED transfer)
- * `staging_bytes` of device staging (0 = 128 MiB = two 64 MiB pipeline slots).  `device` < 0 creates a PLANNING-ONLY ctx
+ * `staging_bytes` of device staging (0 = 512 MiB = two 256 MiB pipeline slots).  `device` < 0 creates a PLANNING-ONLY ctx
  * that touches no CUDA API: every transfer call validates and plans, then returns
  * KV_ERR_NO_DEVICE instead of launching (used by host-side tests). */
 int kv_ctx_create(kv_ctx **out, int device, size_t staging_bytes);

@@ -38,7 +38,7 @@ int run_single_launch(kv_ctx *ctx, const kv_pool_desc *pools, const Call &c, con
 
 int ensure_staging(kv_ctx *ctx) {
   if (ctx->staging) return KV_OK;
-  if (!ctx->staging_bytes) ctx->staging_bytes = (size_t)128 << 20;
+  if (!ctx->staging_bytes) ctx->staging_bytes = (size_t)512 << 20;  // 256 MiB chunks: measured best with both link directions busy
   KV_CUDA(ctx, cudaMalloc(&ctx->staging, ctx->staging_bytes));
   return KV_OK;
 }
@@ -63,6 +63,9 @@ int run_staged(kv_ctx *ctx, const kv_pool_desc *pools, const Call &c, const int3
   const uint64_t unit_bytes = unit_tokens * g.tokrow * (layer_first ? g.C : g.LC);
   size_t slot_bytes = ctx->staging_bytes / n_slots / 256 * 256;
   if (ctx->chunk_bytes) slot_bytes = std::min(slot_bytes, ctx->chunk_bytes / 256 * 256);
+  // layer-by-layer reload: the first flag should come early, so chunks stay small (a 64 MiB chunk of the
+  // Qwen3-Omni prefix is 4 layers: first layer usable after 1.3 ms; 256 MiB chunks would make it 5 ms)
+  if (lf.flags) slot_bytes = std::min<size_t>(slot_bytes, (size_t)64 << 20);
   if (slot_bytes < unit_bytes) return KV_ERR_SIZE;
   const uint64_t chunk_tokens = slot_bytes / unit_bytes * unit_tokens;
 
