@@ -141,3 +141,18 @@ def test_empty_and_degenerate_sessions():
     assert ids.size == 0 and poff.tolist() == [0]
     with pytest.raises(ValueError):
         co.chain_batched(np.zeros(4, dtype=np.uint64), [0, 3, 2], 1)
+
+
+def test_a_chain_continues_from_its_last_id():
+    """Turn k+1 hashes only its new pages: the ids of [old pages | new pages] equal the old ids followed by a
+    chain over the new pages rooted at the last old id (what `roots` is for; "hashes its
+    predecessor")."""
+    rng = np.random.default_rng(11)
+    T = 16
+    a = rng.integers(0, W.VOCAB, size=T * 50).astype(np.uint64)
+    full = co.chain(a, T)
+    for cut in (1, 17, 49):
+        head = co.chain(a[:cut * T], T)
+        tail = co.chain(a[cut * T:], T, root=int(head[-1]))
+        assert np.array_equal(np.concatenate([head, tail]), full)
+    assert co.chain_py(a[:64].tolist(), T) + co.chain_py(a[64:128].tolist(), T, root=int(full[3])) == full[:8].tolist()

@@ -101,3 +101,24 @@ def test_errors_write_nothing_and_capture_is_refused(kv, ctx):
         ident.add_(0)  # a graph needs at least one node
     torch.cuda.synchronize()
     assert (out == -1).all()
+
+
+def test_incremental_turns_continue_the_chain(kv, ctx):
+    """A 50-turn session hashed turn by turn (each call: only the turn's new whole pages, root = the last id so
+    far) gives the ids of the whole history hashed at once -- and both equal the oracle's."""
+    turns = W.session_turns(seed=0)
+    wb = W.identity_batch(seed=6, lens=[turns[-1].cum_tokens])
+    T = 16
+    want = co.chain(wb.ident, T)
+    got_all, _ = run(kv, ctx, wb.ident, wb.tok_offsets, T)
+    assert np.array_equal(got_all, want)
+    pieces, done, root = [], 0, kv.KV_CHAIN_ROOT
+    for tn in turns:
+        n_pages = tn.cum_tokens // T
+        if n_pages == done:
+            continue
+        seg = wb.ident[done * T:n_pages * T]
+        ids, _ = run(kv, ctx, seg, [0, seg.size], T, roots=[root])
+        pieces.append(ids)
+        root, done = int(ids[-1]), n_pages
+    assert np.array_equal(np.concatenate(pieces), want)
