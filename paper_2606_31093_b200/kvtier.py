@@ -160,8 +160,8 @@ _torch = None
 _raw_stream = None  # torch._C._cuda_getCurrentRawStream: the current stream's handle without building a Stream object
 
 
-def _stream(s) -> Optional[int]:
-    """cudaStream_t of `s` (torch stream / int / None = torch's current stream, else the default)."""
+def _stream(s, device: int = -1) -> Optional[int]:
+    """cudaStream_t of `s` (torch stream / int / None = torch's current stream ON THE CTX'S DEVICE, else the default)."""
     global _torch, _raw_stream
     if s is None:
         if _torch is None:
@@ -173,8 +173,8 @@ def _stream(s) -> Optional[int]:
             _raw_stream = getattr(torch._C, "_cuda_getCurrentRawStream", None)
         if _torch.cuda.is_initialized():
             if _raw_stream is not None:
-                return _raw_stream(_torch.cuda.current_device()) or None
-            return int(_torch.cuda.current_stream().cuda_stream) or None
+                return _raw_stream(device if device >= 0 else _torch.cuda.current_device()) or None
+            return int(_torch.cuda.current_stream(device if device >= 0 else None).cuda_stream) or None
         return None
     if isinstance(s, int):
         return s or None
@@ -235,6 +235,7 @@ class Ctx:
         if rc:
             raise KvError(rc)
         self.h = h
+        self.device = int(device)
 
     def close(self):
         if getattr(self, "h", None) and _kv_ctx_destroy is not None:
@@ -293,7 +294,7 @@ def kv_peer_enable(ctx: Ctx, peer_device: int):
 def kv_signal(ctx: Ctx, flag, value: int, stream=None):
     """Release-ordered system-scope store of `value` to the 8-byte word `flag` (tensor or address), after
     every transfer already enqueued on the stream."""
-    _chk(ctx, _kv_signal(ctx.h, _ptr(flag), int(value), _stream(stream)))
+    _chk(ctx, _kv_signal(ctx.h, _ptr(flag), int(value), _stream(stream, ctx.device)))
 
 
 KV_CHAIN_ROOT = 0xCBF29CE484222325
@@ -310,7 +311,7 @@ def kv_chain_hash(ctx: Ctx, ident, tok_offsets, page_size: int, out, roots=None,
     cap = (int(out.numel()) if hasattr(out, "numel") else 0) if out_capacity is None else int(out_capacity)
     rc = _kv_chain_hash(ctx.h, _ptr(ident), int(off.ctypes.data) if off.size else None, S, int(page_size),
                         None if r is None else int(r.ctypes.data), _ptr(out), cap, int(poff.ctypes.data),
-                        _stream(stream))
+                        _stream(stream, ctx.device))
     _chk(ctx, rc)
     return poff
 
@@ -360,7 +361,7 @@ def kv_pack(ctx: Ctx, pools: PoolDesc, layer_count: int, page_ids, dst, dst_byte
     p, keep, n = _ids_arg(page_ids, flags)
     nb = _nbytes(dst) if dst_bytes is None else int(dst_bytes)
     _chk(ctx, _kv_pack(ctx.h, pools.ref, layer_count, p, n, layout, _ptr(dst), nb, flags,
-                       _stream(stream)))
+                       _stream(stream, ctx.device)))
 
 
 def kv_unpack(ctx: Ctx, src, dst_page_ids, pools: PoolDesc, layer_count: int, src_page_size: int,
@@ -369,7 +370,7 @@ def kv_unpack(ctx: Ctx, src, dst_page_ids, pools: PoolDesc, layer_count: int, sr
     p, keep, n = _ids_arg(dst_page_ids, flags)
     nb = _nbytes(src) if src_bytes is None else int(src_bytes)
     _chk(ctx, _kv_unpack(ctx.h, _ptr(src), nb, p, n, pools.ref, layer_count, src_page_size,
-                         dst_page_size, int(n_tokens), layout, flags, _stream(stream)))
+                         dst_page_size, int(n_tokens), layout, flags, _stream(stream, ctx.device)))
 
 
 def _csr(req_offsets):
@@ -384,7 +385,7 @@ def kv_pack_batched(ctx: Ctx, pools: PoolDesc, layer_count: int, page_ids, req_o
     d = _ptr_array(dsts)
     nb = None if dst_bytes is None else _u64_array(dst_bytes)
     _chk(ctx, _kv_pack_batched(ctx.h, pools.ref, layer_count, p, off.ctypes.data, R, layout, d,
-                               None if nb is None else nb.ctypes.data, flags, _stream(stream)))
+                               None if nb is None else nb.ctypes.data, flags, _stream(stream, ctx.device)))
 
 
 def kv_unpack_batched(ctx: Ctx, srcs, dst_page_ids, req_offsets, n_tokens, pools: PoolDesc,
@@ -397,14 +398,14 @@ def kv_unpack_batched(ctx: Ctx, srcs, dst_page_ids, req_offsets, n_tokens, pools
     nb = None if src_bytes is None else _u64_array(src_bytes)
     _chk(ctx, _kv_unpack_batched(ctx.h, s, None if nb is None else nb.ctypes.data, p,
                                  off.ctypes.data, nt.ctypes.data, R, pools.ref, layer_count,
-                                 src_page_size, dst_page_size, layout, flags, _stream(stream)))
+                                 src_page_size, dst_page_size, layout, flags, _stream(stream, ctx.device)))
 
 
 def kv_offload(ctx: Ctx, pools: PoolDesc, layer_count: int, page_ids, host_dst, host_bytes,
                mode=KV_HOST_AUTO, layout=KV_LAYOUT_PAGE_FIRST, flags=0, stream=None):
     p, keep, n = _ids_arg(page_ids, flags)
     _chk(ctx, _kv_offload(ctx.h, pools.ref, layer_count, p, n, layout, _ptr(host_dst),
-                          int(host_bytes), mode, flags, _stream(stream)))
+                          int(host_bytes), mode, flags, _stream(stream, ctx.device)))
 
 
 def kv_reload(ctx: Ctx, host_src, host_bytes, dst_page_ids, pools: PoolDesc, layer_count: int,
@@ -413,7 +414,7 @@ def kv_reload(ctx: Ctx, host_src, host_bytes, dst_page_ids, pools: PoolDesc, lay
     p, keep, n = _ids_arg(dst_page_ids, flags)
     _chk(ctx, _kv_reload(ctx.h, _ptr(host_src), int(host_bytes), p, n, pools.ref, layer_count,
                          src_page_size, dst_page_size, int(n_tokens), layout, mode, flags,
-                         _stream(stream)))
+                         _stream(stream, ctx.device)))
 
 
 def kv_offload_batched(ctx: Ctx, pools: PoolDesc, layer_count: int, page_ids, req_offsets,
@@ -425,7 +426,7 @@ def kv_offload_batched(ctx: Ctx, pools: PoolDesc, layer_count: int, page_ids, re
     nb = None if host_bytes is None else _u64_array(host_bytes)
     _chk(ctx, _kv_offload_batched(ctx.h, pools.ref, layer_count, p, off.ctypes.data, R, layout, d,
                                   None if nb is None else nb.ctypes.data, mode, flags,
-                                  _stream(stream)))
+                                  _stream(stream, ctx.device)))
 
 
 def kv_reload_batched(ctx: Ctx, host_srcs, dst_page_ids, req_offsets, n_tokens, pools: PoolDesc,
@@ -439,7 +440,7 @@ def kv_reload_batched(ctx: Ctx, host_srcs, dst_page_ids, req_offsets, n_tokens, 
     _chk(ctx, _kv_reload_batched(ctx.h, s, None if nb is None else nb.ctypes.data, p,
                                  off.ctypes.data, nt.ctypes.data, R, pools.ref, layer_count,
                                  src_page_size, dst_page_size, layout, mode, flags,
-                                 _stream(stream)))
+                                 _stream(stream, ctx.device)))
 
 
 def kv_reload_layerwise(ctx: Ctx, host_src, host_bytes, dst_page_ids, pools: PoolDesc, layer_count: int,
@@ -449,7 +450,7 @@ def kv_reload_layerwise(ctx: Ctx, host_src, host_bytes, dst_page_ids, pools: Poo
     p, keep, n = _ids_arg(dst_page_ids, flags)
     _chk(ctx, _kv_reload_layerwise(ctx.h, _ptr(host_src), int(host_bytes), p, n, pools.ref, layer_count,
                                    src_page_size, dst_page_size, int(n_tokens), _ptr(layer_flags),
-                                   int(flag_value), mode, flags, _stream(stream)))
+                                   int(flag_value), mode, flags, _stream(stream, ctx.device)))
 
 
 def kv_reload_layerwise_batched(ctx: Ctx, host_srcs, dst_page_ids, req_offsets, n_tokens, pools: PoolDesc,
@@ -463,7 +464,7 @@ def kv_reload_layerwise_batched(ctx: Ctx, host_srcs, dst_page_ids, req_offsets, 
     _chk(ctx, _kv_reload_layerwise_batched(ctx.h, s, None if nb is None else nb.ctypes.data, p,
                                            off.ctypes.data, nt.ctypes.data, R, pools.ref, layer_count,
                                            src_page_size, dst_page_size, _ptr(layer_flags), int(flag_value),
-                                           mode, flags, _stream(stream)))
+                                           mode, flags, _stream(stream, ctx.device)))
 
 
 def kv_repage(ctx: Ctx, src_pools: PoolDesc, src_page_ids, dst_pools: PoolDesc, dst_page_ids,
@@ -471,7 +472,7 @@ def kv_repage(ctx: Ctx, src_pools: PoolDesc, src_page_ids, dst_pools: PoolDesc, 
     sp, skeep, ns = _ids_arg(src_page_ids, flags)
     dp, dkeep, nd = _ids_arg(dst_page_ids, flags)
     _chk(ctx, _kv_repage(ctx.h, src_pools.ref, sp, ns, dst_pools.ref, dp, nd, layer_count,
-                         int(n_tokens), flags, _stream(stream)))
+                         int(n_tokens), flags, _stream(stream, ctx.device)))
 
 
 def kv_repage_batched(ctx: Ctx, src_pools: PoolDesc, src_page_ids, src_offsets, dst_pools: PoolDesc,
@@ -484,13 +485,13 @@ def kv_repage_batched(ctx: Ctx, src_pools: PoolDesc, src_page_ids, src_offsets, 
     nt = _u64_array(n_tokens)
     _chk(ctx, _kv_repage_batched(ctx.h, src_pools.ref, sp, soff.ctypes.data, dst_pools.ref, dp,
                                  doff.ctypes.data, nt.ctypes.data, R, layer_count, flags,
-                                 _stream(stream)))
+                                 _stream(stream, ctx.device)))
 
 
 def kv_cow_append(ctx: Ctx, pools: PoolDesc, layer_count: int, old_id: int, new_id: int, n_old: int,
                   app, n_app: int, flags=0, stream=None):
     _chk(ctx, _kv_cow_append(ctx.h, pools.ref, layer_count, int(old_id), int(new_id), int(n_old),
-                             _ptr(app), int(n_app), flags, _stream(stream)))
+                             _ptr(app), int(n_app), flags, _stream(stream, ctx.device)))
 
 
 def kv_cow_append_batched(ctx: Ctx, pools: PoolDesc, layer_count: int, old_ids, new_ids, n_old,
@@ -503,4 +504,4 @@ def kv_cow_append_batched(ctx: Ctx, pools: PoolDesc, layer_count: int, old_ids, 
     a = _ptr_array(apps)
     _chk(ctx, _kv_cow_append_batched(ctx.h, pools.ref, layer_count, o.ctypes.data if S else None,
                                      n.ctypes.data if S else None, no.ctypes.data if S else None,
-                                     na.ctypes.data if S else None, a, S, flags, _stream(stream)))
+                                     na.ctypes.data if S else None, a, S, flags, _stream(stream, ctx.device)))
