@@ -12,7 +12,7 @@ constexpr int kBlobSlots = 16;
 constexpr int kMaxStagingSlots = 4;
 constexpr uint32_t kMaxLayersKv = 4096;  // layer_count * kv_count
 constexpr uint64_t kAutoStagedMinBytes = 16ull << 20;
-constexpr uint64_t kAutoVecMinBytes = 40ull << 20, kAutoVecMaxBytes = 384ull << 20;  // AUTO: vec kernel in between
+constexpr uint64_t kAutoVecMinBytes = 40ull << 20, kAutoVecMaxBytes = 288ull << 20;  // AUTO: vec kernel in between
 constexpr uint32_t kSchedSlots = 256;  // claim counters, handed out round-robin per launch
 constexpr int kStaticSmemReserve = 8192;  // static shared memory of kv_move_bulk (barriers + stage metadata, 6 KiB) rounded up
 
