@@ -65,7 +65,9 @@ int run_staged(kv_ctx *ctx, const kv_pool_desc *pools, const Call &c, const int3
   if (ctx->chunk_bytes) slot_bytes = std::min(slot_bytes, ctx->chunk_bytes / 256 * 256);
   // at least three chunks per transfer where that leaves >= 64 MiB each: only the first chunk's kernel (offload)
   // or the last one's (reload) is not hidden behind a copy
-  else slot_bytes = std::min<size_t>(slot_bytes, std::max<size_t>((size_t)64 << 20, (c.payload / 3 + 255) / 256 * 256));
+  // (a third of the payload rounded UP to whole chunking units, so that three chunks do cover it)
+  else slot_bytes = std::min<size_t>(slot_bytes, std::max<size_t>((size_t)64 << 20,
+                                                                  (c.payload / 3 + unit_bytes) / unit_bytes * unit_bytes));
   // layer-by-layer reload: the first flag should come early, so chunks stay small (a 64 MiB chunk of the
   // Qwen3-Omni prefix is 4 layers: first layer usable after 1.3 ms; 256 MiB chunks would make it 5 ms)
   if (lf.flags) slot_bytes = std::min<size_t>(slot_bytes, (size_t)64 << 20);
