@@ -78,7 +78,9 @@ int run_staged(kv_ctx *ctx, const kv_pool_desc *pools, const Call &c, const int3
   // a run of whole pages, all layers (contiguous in the host buffer).  Layer-first: a range of layers
   // [l0, l0 + nl) of one or more page ranges; every (layer, K|V) of a page range is one contiguous host run.
   struct Chunk { uint32_t piece_first, n_pieces; uint64_t items; uint32_t l0, nl, sig_n; };
-  struct Copy { uint64_t host, dev_off, bytes; };
+  // rows > 1: a strided copy of `rows` runs of `bytes` each, host_pitch apart in the host buffer and dense in the
+  // slot (the (layer, K|V) runs of a layer-first page range): ONE 2-D copy-engine transfer instead of `rows`
+  struct Copy { uint64_t host, dev_off, bytes; uint64_t rows = 1, host_pitch = 0; };
   std::vector<Piece> pieces;
   std::vector<Chunk> chunks;
   std::vector<std::vector<Copy>> copies;
@@ -120,11 +122,18 @@ int run_staged(kv_ctx *ctx, const kv_pool_desc *pools, const Call &c, const int3
           pieces.push_back(pc);
           cur.n_pieces++;
           cur.items += (q1 - q0) * (g.Tpool / g.g) * nl * g.C * g.subs;
-          if (nb)
-            for (uint32_t l = 0; l < nl; ++l)
-              for (uint32_t kc = 0; kc < g.C; ++kc)
-                cur_copies.push_back(Copy{q.buf + (((uint64_t)(l0 + l) * g.C + kc) * q.n_buf_pages + b0) * row,
-                                          fill + ((uint64_t)l * g.C + kc) * nb * row, nb * row});
+          if (nb) {
+            const uint64_t pitch = q.n_buf_pages * row;  // host bytes between consecutive (layer, K|V) runs
+            if (pitch <= (1ull << 30)) {
+              cur_copies.push_back(Copy{q.buf + ((uint64_t)l0 * g.C * q.n_buf_pages + b0) * row, fill, nb * row,
+                                        (uint64_t)nl * g.C, pitch});
+            } else {  // beyond the 2-D copy's pitch limit: one copy per run
+              for (uint32_t l = 0; l < nl; ++l)
+                for (uint32_t kc = 0; kc < g.C; ++kc)
+                  cur_copies.push_back(Copy{q.buf + (((uint64_t)(l0 + l) * g.C + kc) * q.n_buf_pages + b0) * row,
+                                            fill + ((uint64_t)l * g.C + kc) * nb * row, nb * row});
+            }
+          }
           fill += (region + 255) / 256 * 256;
         }
       }
@@ -194,8 +203,12 @@ int run_staged(kv_ctx *ctx, const kv_pool_desc *pools, const Call &c, const int3
       KV_CUDA(ctx, cudaEventRecord(ctx->ev_full[slot], s));
       KV_CUDA(ctx, cudaStreamWaitEvent(ctx->side, ctx->ev_full[slot], 0));
       for (const Copy &cp : copies[ci]) {
-        KV_CUDA(ctx, cudaMemcpyAsync((void *)(uintptr_t)cp.host, slot_base + cp.dev_off, cp.bytes,
-                                     cudaMemcpyDeviceToHost, ctx->side));
+        if (cp.rows > 1)
+          KV_CUDA(ctx, cudaMemcpy2DAsync((void *)(uintptr_t)cp.host, cp.host_pitch, slot_base + cp.dev_off, cp.bytes,
+                                         cp.bytes, cp.rows, cudaMemcpyDeviceToHost, ctx->side));
+        else
+          KV_CUDA(ctx, cudaMemcpyAsync((void *)(uintptr_t)cp.host, slot_base + cp.dev_off, cp.bytes,
+                                       cudaMemcpyDeviceToHost, ctx->side));
         ctx->memcpys++;
       }
       KV_CUDA(ctx, cudaEventRecord(ctx->ev_free[slot], ctx->side));
@@ -203,8 +216,12 @@ int run_staged(kv_ctx *ctx, const kv_pool_desc *pools, const Call &c, const int3
     } else {  // reload: copy engine fills the slot on side, kernel drains it on s
       if (ctx->free_valid[slot]) KV_CUDA(ctx, cudaStreamWaitEvent(ctx->side, ctx->ev_free[slot], 0));
       for (const Copy &cp : copies[ci]) {
-        KV_CUDA(ctx, cudaMemcpyAsync(slot_base + cp.dev_off, (const void *)(uintptr_t)cp.host,
-                                     cp.bytes, cudaMemcpyHostToDevice, ctx->side));
+        if (cp.rows > 1)
+          KV_CUDA(ctx, cudaMemcpy2DAsync(slot_base + cp.dev_off, cp.bytes, (const void *)(uintptr_t)cp.host,
+                                         cp.host_pitch, cp.bytes, cp.rows, cudaMemcpyHostToDevice, ctx->side));
+        else
+          KV_CUDA(ctx, cudaMemcpyAsync(slot_base + cp.dev_off, (const void *)(uintptr_t)cp.host,
+                                       cp.bytes, cudaMemcpyHostToDevice, ctx->side));
         ctx->memcpys++;
       }
       KV_CUDA(ctx, cudaEventRecord(ctx->ev_full[slot], ctx->side));
