@@ -204,7 +204,7 @@ def run_ours(args):
     if not torch.cuda.is_available():
         raise SystemExit("bench.py: no CUDA device; kvtier has no CPU path (use --impl reference for the oracle)")
     torch.cuda.set_device(int(os.environ.get("LOCAL_RANK", "0")))
-    rep = Replicas("nccl")
+    rep = Replicas(os.environ.get("KV_BENCH_BACKEND", "nccl"))  # gloo only in the plumbing test (two ranks, one GPU)
     world, rank, local = rep.world, rep.rank, rep.local_rank
     max_over_ranks = rep.max_over_ranks
 

@@ -50,3 +50,32 @@ def test_our_arm_prints_the_contract_line():
     assert line["cpu_baseline"]["kind"] == "oracle" and line["cpu_baseline"]["value"] > 0
     assert set(line["clocks"]) >= {"sm_mhz", "sm_max_mhz", "reasons"}
     assert line["config"]["workload"].startswith("configs[1]")
+
+
+@pytest.mark.gpu
+def test_two_replicas_aggregate_on_rank_zero():
+    """The N > 1 plumbing of our arm (barrier, max over ranks of the device-timed interval, sum of units) with two
+    ranks sharing this box's one GPU over gloo: replicas never wait on one another's kernels, only the hosts
+    meet at barriers.  Rank 0 prints the whole-job line, rank 1 prints nothing."""
+    import socket
+    torch = pytest.importorskip("torch")
+    if not torch.cuda.is_available():
+        pytest.skip("no CUDA device")
+    with socket.socket() as s:
+        s.bind(("127.0.0.1", 0))
+        port = s.getsockname()[1]
+    procs = []
+    for r in range(2):
+        env = dict(os.environ, RANK=str(r), LOCAL_RANK="0", WORLD_SIZE="2", MASTER_ADDR="127.0.0.1",
+                   MASTER_PORT=str(port), KV_BENCH_BACKEND="gloo")
+        procs.append(subprocess.Popen([sys.executable, os.path.join(ROOT, "bench.py"), "--gpus", "2", "--steps", "3",
+                                       "--warmup", "3", "--pool-pages", "2048", "--e2e-steps", "2", "--no-cpu-baseline"],
+                                      env=env, stdout=subprocess.PIPE, stderr=subprocess.PIPE, text=True, cwd=ROOT))
+    outs = [p.communicate(timeout=600) for p in procs]
+    for p, (o, e) in zip(procs, outs):
+        assert p.returncode == 0, e[-2000:]
+    assert outs[1][0].strip() == ""
+    line = json.loads([ln for ln in outs[0][0].strip().splitlines() if ln.startswith("{")][-1])
+    assert line["n_gpus"] == 2 and line["scaling"] == "weak" and line["value"] > 0
+    # whole-job value = 2 replicas' bytes over the slower replica's time
+    assert line["value"] == pytest.approx(2 * 4 * 512 * 1572864 * 3 / (line["ms_per_step"] * 3 * 1e-3) / 1e9, rel=1e-6)
