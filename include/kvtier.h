@@ -284,7 +284,10 @@ int kv_repage_batched(kv_ctx *ctx, const kv_pool_desc *src_pools, const int32_t 
  * [layer][K,V][token][head][dim] with n_app tokens and `layer_count` layers; it may be NULL when
  * n_app == 0 (a plain page copy).  n_old + n_app <= page_size and old_id != new_id (KV_ERR_SIZE).
  * The batched call covers all sessions in ONE launch; new ids must be distinct and must not be any
- * session's old id (checked under KV_FLAG_VALIDATE -> KV_ERR_DUP_PAGE).  Host id lists only. */
+ * session's old id (checked under KV_FLAG_VALIDATE -> KV_ERR_DUP_PAGE).  With KV_FLAG_IDS_ON_DEVICE (batched entry)
+ * old_ids / new_ids are DEVICE arrays of n_sessions ids (n_old, n_app and apps stay on the host); a session whose
+ * ids are out of range or equal is skipped and raises the device status word.  kv_cow_append itself takes its two
+ * ids by value, so the flag has no meaning there and is refused (KV_ERR_LAYOUT). */
 int kv_cow_append(kv_ctx *ctx, const kv_pool_desc *pools, uint32_t layer_count, int32_t old_id,
                   int32_t new_id, uint32_t n_old, const void *app, uint32_t n_app, uint32_t flags,
                   kv_stream_t stream);

@@ -160,11 +160,21 @@ __device__ __forceinline__ Item decode(const Job &j, const Tables &tb, uint64_t 
     const uint32_t s0 = (b_old + j.sub_bytes - 1) / j.sub_bytes, s1 = (b_app + j.sub_bytes - 1) / j.sub_bytes;
     const uint32_t lc = local / (s0 + s1), k = local - lc * (s0 + s1);
     const uint64_t slab = ldt<kGlobal>(tb.bases + lc);
-    const uint64_t old_pg = slab + (id_begin & 0xffffffffull) * j.page_stride;
-    const uint64_t new_pg = slab + (id_begin >> 32) * j.page_stride;
+    uint32_t old_id = (uint32_t)id_begin, new_id = (uint32_t)(id_begin >> 32);
     Item it;
     it.mode = 0; it.r0 = 0;
     it.lc = lc; it.s_pg = it.s_t = it.d_pg = it.d_t = 0;
+    if (j.src_ids) {  // KV_FLAG_IDS_ON_DEVICE: id_begin is the session index into the caller's device arrays
+      old_id = (uint32_t)__ldg(j.ids + id_begin);
+      new_id = (uint32_t)__ldg(j.src_ids + id_begin);
+      if (old_id >= j.num_pages || new_id >= j.num_pages || old_id == new_id) {
+        atomicOr(j.status, 1u);
+        it.src = it.dst = 0; it.bytes = it.valid = 0;
+        return it;
+      }
+    }
+    const uint64_t old_pg = slab + (uint64_t)old_id * j.page_stride;
+    const uint64_t new_pg = slab + (uint64_t)new_id * j.page_stride;
     if (k < s0) {
       const uint32_t o = k * j.sub_bytes;
       it.src = old_pg + o; it.dst = new_pg + o; it.bytes = min(j.sub_bytes, b_old - o);

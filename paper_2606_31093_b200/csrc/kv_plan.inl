@@ -173,25 +173,28 @@ int plan_cow(kv_ctx *ctx, const kv_pool_desc *pools, uint32_t layer_count, const
   if (!ctx) return KV_ERR_NULL;
   int rc = check_desc(pools, layer_count);
   if (rc) return rc;
-  if (flags & KV_FLAG_IDS_ON_DEVICE) return KV_ERR_LAYOUT;
+  const bool dev_ids = flags & KV_FLAG_IDS_ON_DEVICE;  // old_ids / new_ids are device arrays, read by the kernel
   if (n_sessions && (!old_ids || !new_ids || !n_old || !n_app || !apps)) return KV_ERR_NULL;
   const uint64_t tokrow = (uint64_t)pools->num_heads * pools->head_dim * pools->elem_bytes;
   const uint64_t lc = (uint64_t)layer_count * pools->kv_count;
   c->reqs.clear();
   for (uint32_t s = 0; s < n_sessions; ++s) {
-    if ((uint64_t)n_old[s] + n_app[s] > pools->page_size || old_ids[s] == new_ids[s]) return KV_ERR_SIZE;
-    if (old_ids[s] < 0 || new_ids[s] < 0 || (uint32_t)old_ids[s] >= pools->num_pages ||
-        (uint32_t)new_ids[s] >= pools->num_pages)
-      return KV_ERR_PAGE_RANGE;
+    if ((uint64_t)n_old[s] + n_app[s] > pools->page_size) return KV_ERR_SIZE;
+    if (!dev_ids) {
+      if (old_ids[s] == new_ids[s]) return KV_ERR_SIZE;
+      if (old_ids[s] < 0 || new_ids[s] < 0 || (uint32_t)old_ids[s] >= pools->num_pages ||
+          (uint32_t)new_ids[s] >= pools->num_pages)
+        return KV_ERR_PAGE_RANGE;
+    }
     if (n_app[s] && !apps[s]) return KV_ERR_NULL;
     if (!n_old[s] && !n_app[s]) continue;
     Req q;
     q.buf = (uint64_t)(uintptr_t)apps[s];
     q.n_tokens = (uint64_t)n_old[s] | ((uint64_t)n_app[s] << 32);
-    q.id_begin = (uint64_t)(uint32_t)old_ids[s] | ((uint64_t)(uint32_t)new_ids[s] << 32);
+    q.id_begin = dev_ids ? (uint64_t)s : (uint64_t)(uint32_t)old_ids[s] | ((uint64_t)(uint32_t)new_ids[s] << 32);
     c->reqs.push_back(q);
   }
-  if (flags & KV_FLAG_VALIDATE) {  // new pages distinct, and none of them is some session's old page
+  if ((flags & KV_FLAG_VALIDATE) && !dev_ids) {  // new pages distinct, and none of them is some session's old page
     std::vector<uint8_t> is_new((size_t)(pools->num_pages + 7) / 8, 0);
     for (uint32_t s = 0; s < n_sessions; ++s) {
       const uint32_t g = (uint32_t)new_ids[s];
@@ -206,6 +209,7 @@ int plan_cow(kv_ctx *ctx, const kv_pool_desc *pools, uint32_t layer_count, const
   c->n_ids = 0;
   rc = make_geom(ctx, pools, layer_count, pools->page_size, /*dir=*/3, KV_LAYOUT_PAGE_FIRST, c->reqs, &c->geom);
   if (rc) return rc;
+  if (dev_ids) c->geom.dev_src_ids = new_ids;
   c->total_items = 0; c->payload = 0;
   const uint64_t sub = c->geom.sub_bytes;
   for (Req &q : c->reqs) {

@@ -378,12 +378,13 @@ int kv_cow_append_batched(kv_ctx *ctx, const kv_pool_desc *pools, uint32_t layer
   Call c;
   int rc = plan_cow(ctx, pools, layer_count, old_ids, new_ids, n_old, n_app, apps, n_sessions, flags, &c);
   if (rc) return rc;
-  return run_device(ctx, pools, c, nullptr, flags, (cudaStream_t)stream);
+  return run_device(ctx, pools, c, (flags & KV_FLAG_IDS_ON_DEVICE) ? old_ids : nullptr, flags, (cudaStream_t)stream);
 }
 
 int kv_cow_append(kv_ctx *ctx, const kv_pool_desc *pools, uint32_t layer_count, int32_t old_id,
                   int32_t new_id, uint32_t n_old, const void *app, uint32_t n_app, uint32_t flags,
                   kv_stream_t stream) {
+  if (flags & KV_FLAG_IDS_ON_DEVICE) return KV_ERR_LAYOUT;  // the ids are passed by value here
   const int32_t o[1] = {old_id}, n[1] = {new_id};
   const uint32_t no[1] = {n_old}, na[1] = {n_app};
   const void *const ap[1] = {app};

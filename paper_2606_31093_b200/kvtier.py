@@ -496,12 +496,17 @@ def kv_cow_append(ctx: Ctx, pools: PoolDesc, layer_count: int, old_id: int, new_
 
 def kv_cow_append_batched(ctx: Ctx, pools: PoolDesc, layer_count: int, old_ids, new_ids, n_old,
                           n_app, apps, flags=0, stream=None):
-    o, n = _host_i32(old_ids), _host_i32(new_ids)
     no = np.ascontiguousarray(np.asarray(n_old, dtype=np.uint32))
     na = np.ascontiguousarray(np.asarray(n_app, dtype=np.uint32))
-    S = int(o.size)
-    assert n.size == S and no.size == S and na.size == S and len(apps) == S
+    S = int(no.size)
+    if flags & KV_FLAG_IDS_ON_DEVICE:  # device tensors of S int32 ids each
+        op, np_ = _ptr(old_ids), _ptr(new_ids)
+        assert int(old_ids.numel()) == S and int(new_ids.numel()) == S
+    else:
+        o, n = _host_i32(old_ids), _host_i32(new_ids)
+        assert o.size == S and n.size == S
+        op, np_ = (o.ctypes.data if S else None), (n.ctypes.data if S else None)
+    assert na.size == S and len(apps) == S
     a = _ptr_array(apps)
-    _chk(ctx, _kv_cow_append_batched(ctx.h, pools.ref, layer_count, o.ctypes.data if S else None,
-                                     n.ctypes.data if S else None, no.ctypes.data if S else None,
+    _chk(ctx, _kv_cow_append_batched(ctx.h, pools.ref, layer_count, op, np_, no.ctypes.data if S else None,
                                      na.ctypes.data if S else None, a, S, flags, _stream(stream, ctx.device)))

@@ -715,3 +715,37 @@ def test_layer_ranges_offload_behind_producer_events(kv, ctx):
     finally:
         torch.cuda.synchronize()
         kv.kv_host_free(hp)
+
+
+def test_cow_append_with_device_resident_ids(kv, ctx):
+    """kv_cow_append_batched with KV_FLAG_IDS_ON_DEVICE: old / new page ids in device arrays; a bad session
+    (id out of range, or old == new) is skipped and raises the status word, the others are as the oracle says."""
+    L, C, P, T, H, D, e = 3, 2, 64, 16, 4, 128, 2
+    rng = np.random.default_rng(179)
+    A = host_pool(rng, L, C, P, T, H, D, e)
+    tA, dA = to_device(A, kv, torch)
+    S = 7
+    perm = rng.permutation(P).astype(np.int32)
+    old, new = perm[:S].copy(), perm[S:2 * S].copy()
+    n_old = rng.integers(0, T + 1, size=S)
+    n_app = np.array([rng.integers(0, T - o + 1) for o in n_old])
+    n_old[0], n_app[0] = 5, 4
+    apps = [rng.integers(0, 256, size=L * C * int(a) * H * D * e, dtype=np.uint8) for a in n_app]
+    dev = [torch.from_numpy(a).cuda() if a.size else None for a in apps]
+    d_old, d_new = torch.from_numpy(old).cuda(), torch.from_numpy(new).cuda()
+    kv.kv_cow_append_batched(ctx, dA, L, d_old, d_new, n_old, n_app, dev, flags=kv.KV_FLAG_IDS_ON_DEVICE)
+    torch.cuda.synchronize()
+    ko.cow_append_batched(A, old, new, n_old, n_app, apps)
+    assert_pool_equal(tA, A)
+    assert ctx.device_status() == 0
+    # session 0 gets an out-of-range new id, session 1 old == new: both skipped, the rest done again (idempotent)
+    bad_new = new.copy()
+    bad_new[0] = P + 3
+    bad_new[1] = old[1]
+    d_new.copy_(torch.from_numpy(bad_new))
+    kv.kv_cow_append_batched(ctx, dA, L, d_old, d_new, n_old, n_app, dev, flags=kv.KV_FLAG_IDS_ON_DEVICE)
+    assert ctx.device_status() == 1
+    assert_pool_equal(tA, A)
+    with pytest.raises(kv.KvError) as ei:
+        kv.kv_cow_append(ctx, dA, L, 1, 2, 3, None, 0, flags=kv.KV_FLAG_IDS_ON_DEVICE)
+    assert ei.value.status == kv.KV_ERR_LAYOUT
