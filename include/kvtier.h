@@ -197,7 +197,8 @@ int kv_signal(kv_ctx *ctx, uint64_t *flag, uint64_t value, kv_stream_t stream);
  *   page_offsets  HOST int64[n_sessions+1], written by the call (may be NULL)
  * Two launches on `stream` (per-page digests in parallel, then one warp per session along the chain);
  * results are defined after the caller synchronises `stream`.  Errors: KV_ERR_NULL, KV_ERR_SIZE (page_size
- * 0, bad offsets, out_capacity too small), KV_ERR_ALIGN, KV_ERR_CAPTURE (not capturable), KV_ERR_NO_DEVICE
+ * 0, bad offsets, out_capacity too small), KV_ERR_ALIGN, KV_ERR_CAPTURE (more than 128 sessions: the tables do
+ * not fit the kernel parameters; up to 128 the call is two self-contained launches and capturable), KV_ERR_NO_DEVICE
  * (planning-only ctx; page_offsets are still written), KV_ERR_CUDA.  n_sessions == 0 or no whole page:
  * KV_OK, nothing launched. */
 #define KV_CHAIN_ROOT 0xcbf29ce484222325ull

@@ -63,16 +63,41 @@ struct ChainJob {
   uint32_t T;
 };
 
-__global__ void __launch_bounds__(128) kv_chain_digest(const ChainJob j) {
+// Tables of small batches ride inside the kernel parameters (kInline): no staging copy, so the call is two
+// self-contained launches and can be captured into a CUDA graph.  [tok_off: S+1][page_off: S+1][roots: S]
+constexpr int kChainInlineSessions = 128;
+struct ChainJobInline {
+  ChainJob j;
+  int64_t tok_off[kChainInlineSessions + 1];
+  int64_t page_off[kChainInlineSessions + 1];
+  uint64_t roots[kChainInlineSessions];
+};
+template <bool kInline> struct ChainParam { typedef ChainJob type; };
+template <> struct ChainParam<true> { typedef ChainJobInline type; };
+template <bool kInline, typename P>
+__device__ __forceinline__ ChainJob chain_job(const P &p) {
+  if constexpr (kInline) {
+    ChainJob j = p.j;
+    j.tok_off = p.tok_off; j.page_off = p.page_off;
+    if (j.roots) j.roots = p.roots;
+    return j;
+  } else {
+    return p;
+  }
+}
+
+template <bool kInline>
+__global__ void __launch_bounds__(128) kv_chain_digest(const __grid_constant__ typename ChainParam<kInline>::type prm) {
+  const ChainJob j = chain_job<kInline>(prm);
   const uint64_t p = (uint64_t)blockIdx.x * blockDim.x + threadIdx.x;
   if (p >= j.total_pages) return;
   uint32_t lo = 0, hi = j.n_sessions;  // largest s with page_off[s] <= p
   while (hi - lo > 1) {
     const uint32_t mid = (lo + hi) >> 1;
-    if ((uint64_t)__ldg(j.page_off + mid) <= p) lo = mid; else hi = mid;
+    if ((uint64_t)j.page_off[mid] <= p) lo = mid; else hi = mid;
   }
-  const uint64_t k = p - (uint64_t)__ldg(j.page_off + lo);
-  const uint64_t *src = j.ident + (uint64_t)__ldg(j.tok_off + lo) + k * j.T;
+  const uint64_t k = p - (uint64_t)j.page_off[lo];
+  const uint64_t *src = j.ident + (uint64_t)j.tok_off[lo] + k * j.T;
   uint64_t h = kFnvBasis;
   uint32_t t = 0;
   for (; t + 4 <= j.T; t += 4) {  // four loads in flight ahead of the dependent arithmetic
@@ -83,11 +108,13 @@ __global__ void __launch_bounds__(128) kv_chain_digest(const ChainJob j) {
   j.out[p] = h;
 }
 
-__global__ void __launch_bounds__(32) kv_chain_link(const ChainJob j) {
+template <bool kInline>
+__global__ void __launch_bounds__(32) kv_chain_link(const __grid_constant__ typename ChainParam<kInline>::type prm) {
+  const ChainJob j = chain_job<kInline>(prm);
   const uint32_t s = blockIdx.x, lane = threadIdx.x;
   if (s >= j.n_sessions) return;
-  const uint64_t p0 = (uint64_t)__ldg(j.page_off + s), p1 = (uint64_t)__ldg(j.page_off + s + 1);
-  uint64_t prev = j.roots ? __ldg(j.roots + s) : j.default_root;
+  const uint64_t p0 = (uint64_t)j.page_off[s], p1 = (uint64_t)j.page_off[s + 1];
+  uint64_t prev = j.roots ? j.roots[s] : j.default_root;
   uint64_t next_d = p0 + lane < p1 ? j.out[p0 + lane] : 0;
   for (uint64_t base = p0; base < p1; base += 32) {
     const uint64_t d = next_d;

@@ -234,10 +234,30 @@ int kv_chain_hash(kv_ctx *ctx, const uint64_t *ident, const int64_t *tok_offsets
   if (ctx->host_only) return KV_ERR_NO_DEVICE;
   cudaStream_t s = (cudaStream_t)stream;
   DeviceGuard guard(ctx);
-  if (capturing(s)) return KV_ERR_CAPTURE;
-  // tables: [tok_off: S+1][page_off: S+1][roots: S], staged through the pinned ring
-  HostBlob hb;
   const size_t n1 = (size_t)n_sessions + 1;
+  const uint64_t blocks = (total + 127) / 128;
+  if (blocks > 0x7fffffffull) return KV_ERR_SIZE;
+  kvt::ChainJob j{};
+  j.ident = ident; j.out = out;
+  j.default_root = KV_CHAIN_ROOT;
+  j.total_pages = total; j.n_sessions = n_sessions; j.T = page_size;
+  if (n_sessions <= (uint32_t)kvt::kChainInlineSessions) {  // tables inside the kernel parameters: capturable
+    static thread_local kvt::ChainJobInline pi;
+    pi.j = j;
+    pi.j.roots = roots ? pi.roots : nullptr;  // non-null marks "roots present"; the kernel points it at its own copy
+    std::memcpy(pi.tok_off, tok_offsets, n1 * 8);
+    std::memcpy(pi.page_off, poff.data(), n1 * 8);
+    if (roots) std::memcpy(pi.roots, roots, (size_t)n_sessions * 8);
+    kvt::kv_chain_digest<true><<<(uint32_t)blocks, 128, 0, s>>>(pi);
+    KV_CUDA(ctx, cudaGetLastError());
+    kvt::kv_chain_link<true><<<n_sessions, 32, 0, s>>>(pi);
+    KV_CUDA(ctx, cudaGetLastError());
+    ctx->launches += 2;
+    return KV_OK;
+  }
+  if (capturing(s)) return KV_ERR_CAPTURE;
+  // larger batches: [tok_off: S+1][page_off: S+1][roots: S] staged through the pinned ring
+  HostBlob hb;
   hb.bytes.resize((2 * n1 + (roots ? n_sessions : 0)) * 8);
   std::memcpy(hb.bytes.data(), tok_offsets, n1 * 8);
   std::memcpy(hb.bytes.data() + n1 * 8, poff.data(), n1 * 8);
@@ -245,18 +265,12 @@ int kv_chain_hash(kv_ctx *ctx, const uint64_t *ident, const int64_t *tok_offsets
   Blob b;
   int rc = upload_blob(ctx, hb, nullptr, true, s, &b);
   if (rc) return rc;
-  kvt::ChainJob j{};
-  j.ident = ident; j.out = out;
   j.tok_off = (const int64_t *)b.slot->d;
   j.page_off = j.tok_off + n1;
   j.roots = roots ? (const uint64_t *)(j.page_off + n1) : nullptr;
-  j.default_root = KV_CHAIN_ROOT;
-  j.total_pages = total; j.n_sessions = n_sessions; j.T = page_size;
-  const uint64_t blocks = (total + 127) / 128;
-  if (blocks > 0x7fffffffull) return KV_ERR_SIZE;
-  kvt::kv_chain_digest<<<(uint32_t)blocks, 128, 0, s>>>(j);
+  kvt::kv_chain_digest<false><<<(uint32_t)blocks, 128, 0, s>>>(j);
   KV_CUDA(ctx, cudaGetLastError());
-  kvt::kv_chain_link<<<n_sessions, 32, 0, s>>>(j);
+  kvt::kv_chain_link<false><<<n_sessions, 32, 0, s>>>(j);
   KV_CUDA(ctx, cudaGetLastError());
   ctx->launches += 2;
   KV_CUDA(ctx, cudaEventRecord(b.slot->ev, s));

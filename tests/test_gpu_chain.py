@@ -84,7 +84,7 @@ def test_empty_sessions_tails_and_offsets_not_at_zero(kv, ctx):
     assert got.tolist() == co.chain_py([0x61], 1, root=0)
 
 
-def test_errors_write_nothing_and_capture_is_refused(kv, ctx):
+def test_errors_write_nothing_and_capture(kv, ctx):
     ident = torch.zeros(64, dtype=torch.int64, device="cuda")
     out = torch.full((4,), -1, dtype=torch.int64, device="cuda")
     with pytest.raises(kv.KvError) as ei:
@@ -92,15 +92,36 @@ def test_errors_write_nothing_and_capture_is_refused(kv, ctx):
     assert ei.value.status == kv.KV_ERR_SIZE
     torch.cuda.synchronize()
     assert (out == -1).all()
+    # up to 128 sessions the tables ride in the kernel parameters: two self-contained launches, capturable;
+    # identities are re-read at every replay
+    wb = W.identity_batch(seed=8, n_sessions=100, lo=16, hi=300)
+    d_ident = torch.from_numpy(wb.ident.view(np.int64)).cuda()
+    n = int((np.diff(wb.tok_offsets) // 16).sum())
+    outg = torch.zeros(n, dtype=torch.int64, device="cuda")
     side = torch.cuda.Stream()
     g = torch.cuda.CUDAGraph()
     with torch.cuda.graph(g, stream=side):
+        kv.kv_chain_hash(ctx, d_ident, wb.tok_offsets, 16, outg, stream=side)
+    for rep in range(2):
+        g.replay()
+        torch.cuda.synchronize()
+        assert np.array_equal(outg.cpu().numpy().view(np.uint64), co.chain_batched(wb.ident, wb.tok_offsets, 16)[0])
+        wb.ident[::7] ^= np.uint64(rep + 1)  # new identities, same graph
+        d_ident.copy_(torch.from_numpy(wb.ident.view(np.int64)))
+    # more sessions than fit the parameters: refused under capture, nothing enqueued
+    big = W.identity_batch(seed=9, n_sessions=129, lo=16, hi=40)
+    d_big = torch.from_numpy(big.ident.view(np.int64)).cuda()
+    out_big = torch.full((int((np.diff(big.tok_offsets) // 16).sum()),), -1, dtype=torch.int64, device="cuda")
+    g2 = torch.cuda.CUDAGraph()
+    with torch.cuda.graph(g2, stream=side):
         with pytest.raises(kv.KvError) as ei:
-            kv.kv_chain_hash(ctx, ident, [0, 64], 16, out, stream=side)
+            kv.kv_chain_hash(ctx, d_big, big.tok_offsets, 16, out_big, stream=side)
         assert ei.value.status == kv.KV_ERR_CAPTURE
         ident.add_(0)  # a graph needs at least one node
     torch.cuda.synchronize()
-    assert (out == -1).all()
+    assert (out_big == -1).all()
+    got, _ = run(kv, ctx, big.ident, big.tok_offsets, 16)  # live, through the pinned ring
+    assert np.array_equal(got, co.chain_batched(big.ident, big.tok_offsets, 16)[0])
 
 
 def test_incremental_turns_continue_the_chain(kv, ctx):
