@@ -690,8 +690,16 @@ __global__ void __launch_bounds__(256) kv_move_elem(const __grid_constant__ JobT
         continue;
       }
     }
-    for (uint32_t i = lane; i < nv; i += 32) d[i] = s[i];
-    for (uint32_t i = nv + lane; i < nb; i += 32) d[i] = U(0);
+    uint32_t i = lane;
+    for (; i + 32 * 7 < nv; i += 32 * 8) {  // eight loads in flight per lane before the first store
+      U v[8];
+#pragma unroll
+      for (int u = 0; u < 8; ++u) v[u] = s[i + 32 * u];
+#pragma unroll
+      for (int u = 0; u < 8; ++u) d[i + 32 * u] = v[u];
+    }
+    for (; i < nv; i += 32) d[i] = s[i];
+    for (i = nv + lane; i < nb; i += 32) d[i] = U(0);
   }
 }
 
