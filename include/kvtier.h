@@ -81,9 +81,9 @@ typedef enum kv_layout {
 
 /* How a host-tier transfer crosses the host link (BASELINE.json:north_star item 3). */
 typedef enum kv_host_mode {
-  KV_HOST_AUTO = 0,   /* chosen from the measured table in DESIGN.md: STAGED from 16 MiB of payload (page-first), else DIRECT */
+  KV_HOST_AUTO = 0,   /* chosen from the measured table in DESIGN.md: STAGED from 16 MiB of payload (either layout), else DIRECT */
   KV_HOST_DIRECT = 1, /* the kernel stores to / loads from mapped pinned memory over the link */
-  KV_HOST_STAGED = 2, /* device staging + copy-engine cudaMemcpyAsync on the ctx's side stream, chunk-pipelined */
+  KV_HOST_STAGED = 2, /* device staging + copy-engine transfers (1-D, or 2-D for layer-first chunks) on the ctx's side stream, chunk-pipelined */
 } kv_host_mode;
 
 typedef enum kv_status {

@@ -45,8 +45,9 @@ int ensure_staging(kv_ctx *ctx) {
 
 // KV_HOST_STAGED: the flattened page sequence of all requests is cut into chunks that fit one
 // staging slot; per chunk: kernel <-> slot on `s`, copy engine slot <-> pinned host on the side
-// stream, double (or deeper) buffered with events.  Page-first only (a chunk of pages is then
-// contiguous in the host buffer); layer-first falls back to DIRECT.
+// stream, double (or deeper) buffered with events.  Page-first: a chunk is a run of whole pages,
+// contiguous in the host buffer (one copy).  Layer-first: a chunk is a range of whole layers of one or more page
+// ranges; its (layer, K|V) runs are a layer apart in the host buffer and move as ONE 2-D copy.
 // Layer flags of kv_reload_layerwise: after the pages of layers [l0, l0 + n) have landed in the pool,
 // flags[l] = value is stored (release, system scope) in stream order.
 struct LayerFlags { uint64_t *flags = nullptr; uint64_t value = 0; };
