@@ -408,6 +408,15 @@ def run_ours(args):
 
 def main():
     args = parse()
+    if int(os.environ.get("LOCAL_RANK", "0")) == 0:  # fresh checkout: build what is missing (one rank per node)
+        import __graft_entry__
+
+        __graft_entry__.ensure_built()
+    else:  # the other ranks of the node wait for rank 0's build instead of racing it
+        lib = os.path.join(ROOT, "paper_2606_31093_b200", "libkvtier.so")
+        t0 = time.time()
+        while args.impl == "ours" and not os.path.exists(lib) and time.time() - t0 < 300:
+            time.sleep(1.0)
     if args.impl == "reference":
         run_reference(args)
     else:

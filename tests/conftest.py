@@ -10,6 +10,9 @@ if ROOT not in sys.path:
 
 def pytest_configure(config):
     config.addinivalue_line("markers", "gpu: needs a CUDA device (run on the B200 box)")
+    import __graft_entry__
+
+    __graft_entry__.ensure_built()  # fresh checkout: compile libkvtier.so (nvcc, sm_100a) and the oracles (gcc)
 
 
 def read_golden(name):
