@@ -144,6 +144,19 @@ int launch(kv_ctx *ctx, const Geom &g, const Blob &b, uint32_t piece_first, uint
     j.zero_bytes = std::min<uint32_t>(4096, j.stage_bytes);
     j.l2_hint = ctx->l2_hint;
     uint32_t warps = lane_geom ? ctx->t_warps : ctx->warps;
+    if (!lane_geom && ctx->auto_geom && j.stage_bytes < 16384) {
+      // Narrow rows (a tensor-parallel head partition: 1 KV head = 4 KiB rows, 2 heads = 8 KiB): what saturates HBM is
+      // the BYTES in flight per SM (~128 KiB of stages), so smaller stages need more of them.  Measured on B200,
+      // 768 MiB back to back: 4 KiB rows 3.46 TB/s with the 2 x 4 ring, 6.2 with 8 x 4; 8 KiB rows 5.09 -> 6.24 with
+      // 4 x 4.  Launch-sized calls keep the 2-warp ring (more CTAs, each with little to do).
+      const uint32_t total = 131072u / j.stage_bytes;          // stages per SM
+      const uint32_t w = std::min<uint32_t>(kvt::kMaxWarps, std::max<uint32_t>(2, total / 4));
+      if (total_items >= 4ull * ctx->sm_count * w) {
+        warps = w;
+        j.stages = std::min<uint32_t>(kvt::kMaxStages, std::max<uint32_t>(4, total / w));
+        j.lag = std::min(ctx->lag, j.stages - 1);
+      }
+    }
     size_t smem = (size_t)j.zero_bytes + (size_t)warps * j.stages * j.stage_bytes;
     while (smem > (size_t)ctx->max_smem - kStaticSmemReserve && j.stages > 2) {  // static smem holds barriers + meta
       --j.stages; j.lag = std::min(j.lag, j.stages - 1);

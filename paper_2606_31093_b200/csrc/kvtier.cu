@@ -133,9 +133,9 @@ int kv_ctx_set_option(kv_ctx *ctx, int option, int64_t v) {
   if (!ctx) return KV_ERR_NULL;
   switch (option) {
     case KV_OPT_KERNEL: if (v < 0 || v > 3) return KV_ERR_SIZE; ctx->kernel = (int)v; break;
-    case KV_OPT_STAGE_BYTES: if (v < 1024 || v > 65536 || v % 16) return KV_ERR_SIZE; ctx->stage_bytes = ctx->t_stage_bytes = (uint32_t)v; break;
-    case KV_OPT_STAGES_PER_WARP: if (v < 2 || v > kvt::kMaxStages) return KV_ERR_SIZE; ctx->stages = ctx->t_stages = (uint32_t)v; break;
-    case KV_OPT_WARPS: if (v < 1 || v > kvt::kMaxWarps) return KV_ERR_SIZE; ctx->warps = ctx->t_warps = (uint32_t)v; break;
+    case KV_OPT_STAGE_BYTES: if (v < 1024 || v > 65536 || v % 16) return KV_ERR_SIZE; ctx->stage_bytes = ctx->t_stage_bytes = (uint32_t)v; ctx->auto_geom = false; break;
+    case KV_OPT_STAGES_PER_WARP: if (v < 2 || v > kvt::kMaxStages) return KV_ERR_SIZE; ctx->stages = ctx->t_stages = (uint32_t)v; ctx->auto_geom = false; break;
+    case KV_OPT_WARPS: if (v < 1 || v > kvt::kMaxWarps) return KV_ERR_SIZE; ctx->warps = ctx->t_warps = (uint32_t)v; ctx->auto_geom = false; break;
     case KV_OPT_STORE_LAG: if (v < 1 || v > 3) return KV_ERR_SIZE; ctx->lag = (uint32_t)v; break;
     case KV_OPT_MAX_CTAS: if (v < 0 || v > 65535) return KV_ERR_SIZE; ctx->max_ctas = (uint32_t)v; break;
     case KV_OPT_CHUNK_BYTES: if (v < 0) return KV_ERR_SIZE; ctx->chunk_bytes = (size_t)v; break;

@@ -136,6 +136,18 @@ def run(ctx, desc, shape, slabs, seed=0, out_dir="gpurun_out", hbm_peak=None):
         rec("2 prefix, ids in runs", f"unpack, runs of {r_len}", "device", pl, 2 * pl, n,
             lambda: kv.kv_unpack(ctx, buf, ids_r, desc, L, T, T, n * T), reps=20, warm=3)
 
+    # ---- tensor-parallel head partitions ("head partitions"): the same slabs read as pools of 1 and 2
+    # KV heads per rank -> 4 KiB / 8 KiB rows, 4x / 2x the pages for the same 768 MiB (timing only)
+    for Hp in (1, 2):
+        f = shape.H // Hp
+        desc_p = kv.PoolDesc(slabs, L, shape.C, shape.P * f, T, Hp, shape.D, shape.e)
+        ids_p = rng.choice(shape.P * f, n * f, replace=False).astype(np.int32)
+        dst_p = rng.choice(shape.P * f, n * f, replace=False).astype(np.int32)
+        rec(f"2 prefix, {Hp} KV head(s) per rank", f"pack ({4 * Hp} KiB rows)", "device", pl, 2 * pl, n * f,
+            lambda: kv.kv_pack(ctx, desc_p, L, ids_p, buf), reps=20, warm=3)
+        rec(f"2 prefix, {Hp} KV head(s) per rank", f"unpack ({4 * Hp} KiB rows)", "device", pl, 2 * pl, n * f,
+            lambda: kv.kv_unpack(ctx, buf, dst_p, desc_p, L, T, T, n * f * T), reps=20, warm=3)
+
     # ---- NEXT-2: the same prefix on an HND pool ([head][token][dim] pages; the buffer stays NHD, so the
     # transfer transposes).  Same slabs, HND descriptor: timing only (parity: tests/test_gpu_hnd.py).
     desc_h = kv.PoolDesc(slabs, L, shape.C, shape.P, T, shape.H, shape.D, shape.e, order=kv.KV_ORDER_HND)
