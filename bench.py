@@ -275,9 +275,11 @@ def run_ours(args):
         #           payload at once
         hm = {"auto": kv.KV_HOST_AUTO, "direct": kv.KV_HOST_DIRECT, "staged": kv.KV_HOST_STAGED}[args.host_mode]
         hp = [kv.kv_host_alloc(payload) for _ in range(2)]
+        for h in hp:  # touch every page from the CPU once: a fresh VM backs guest memory lazily, and the first DMA
+            kv.host_view(h, payload)[:] = 0  # passes over untouched pinned pages ran at ~40 instead of ~56 GB/s
         Ks = min(Ke, 5)
         kv.kv_offload(ctx, desc, shape.L, src_ids[-1], hp[1], payload, mode=hm)  # the buffer the first duplex step reloads
-        for i in range(min(Wm, 2)):
+        for i in range(Wm):
             kv.kv_offload(ctx, desc, shape.L, src_ids[i], hp[0], payload, mode=hm)
             kv.kv_reload(ctx, hp[0], payload, dst_ids[i], desc, shape.L, shape.T, shape.T, n * shape.T, mode=hm)
             stream.synchronize()
@@ -306,7 +308,7 @@ def run_ours(args):
             s_off.synchronize()  # the host reads the step's result here
             s_rel.synchronize()
 
-        for i in range(min(Wm, 2)):
+        for i in range(Wm):
             duplex_step(i)
         barrier()
         e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
