@@ -64,11 +64,20 @@ int run_staged(kv_ctx *ctx, const kv_pool_desc *pools, const Call &c, const int3
   const uint64_t unit_bytes = unit_tokens * g.tokrow * (layer_first ? g.C : g.LC);
   size_t slot_bytes = ctx->staging_bytes / n_slots / 256 * 256;
   if (ctx->chunk_bytes) slot_bytes = std::min(slot_bytes, ctx->chunk_bytes / 256 * 256);
-  // at least three chunks per transfer where that leaves >= 64 MiB each: only the first chunk's kernel (offload)
-  // or the last one's (reload) is not hidden behind a copy
-  // (a third of the payload rounded UP to whole chunking units, so that three chunks do cover it)
-  else slot_bytes = std::min<size_t>(slot_bytes, std::max<size_t>((size_t)64 << 20,
-                                                                  (c.payload / 3 + unit_bytes) / unit_bytes * unit_bytes));
+  // Equal chunks: at least three per transfer where that leaves >= 64 MiB each (only the first chunk's kernel of an
+  // offload, or the last one's of a reload, is not hidden behind a copy), as many as the slot size demands, and the
+  // payload divided evenly among them in whole chunking units (no two-page leftover chunk at the end).
+  else {
+    const uint64_t cap = slot_bytes / unit_bytes * unit_bytes, min_chunk = (uint64_t)64 << 20;
+    if (cap < unit_bytes) return KV_ERR_SIZE;  // one chunking unit does not fit a staging slot
+    uint64_t n = std::max<uint64_t>(1, std::min<uint64_t>(3, c.payload / min_chunk));
+    uint64_t per = cap;
+    for (;; ++n) {
+      per = ((c.payload + n - 1) / n + unit_bytes - 1) / unit_bytes * unit_bytes;
+      if (per <= cap) break;
+    }
+    slot_bytes = (size_t)std::max<uint64_t>(per, unit_bytes);
+  }
   // layer-by-layer reload: the first flag should come early, so chunks stay small (a 64 MiB chunk of the
   // Qwen3-Omni prefix is 4 layers: first layer usable after 1.3 ms; 256 MiB chunks would make it 5 ms)
   if (lf.flags) slot_bytes = std::min<size_t>(slot_bytes, (size_t)64 << 20);
