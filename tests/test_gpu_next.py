@@ -778,3 +778,50 @@ def test_narrow_rows_of_a_head_partition(kv, ctx, H, order):
     ko.repage(A, src, B, dst[::-1].copy(), n_tokens=n * T)
     assert_pool_equal(tB, B)
     assert_pool_equal(tA, A)
+
+
+def test_four_threads_four_contexts(kv):
+    """'One ctx per calling thread' (kvtier.h): four host threads, each with its own ctx and stream, hammer the same
+    source pool into their own destination pools at once (ctypes drops the GIL inside the library, so the C side
+    really runs concurrently).  Every thread's result equals the oracle's."""
+    import threading
+    L, C, P, T, H, D, e = 4, 2, 128, 16, 4, 128, 2
+    rng = np.random.default_rng(191)
+    A = host_pool(rng, L, C, P, T, H, D, e)
+    tA, dA = to_device(A, kv, torch)
+    n, rounds, nthreads = 48, 25, 4
+    plans = []
+    for t in range(nthreads):
+        r = np.random.default_rng(1000 + t)
+        B = host_pool(r, L, C, P, T, H, D, e, order=t % 2)
+        tB, dB = to_device(B, kv, torch)
+        steps = [(r.choice(P, n, replace=False).astype(np.int32), r.permutation(P)[:n].astype(np.int32)) for _ in range(rounds)]
+        plans.append((B, tB, dB, steps))
+    errors = []
+
+    def worker(t):
+        try:
+            B, tB, dB, steps = plans[t]
+            ctx = kv.Ctx(0, staging_bytes=8 << 20)
+            stream = torch.cuda.Stream()
+            buf = torch.zeros(n * dA.page_bytes(), dtype=torch.uint8, device="cuda")
+            for src, dst in steps:
+                kv.kv_pack(ctx, dA, L, src, buf, stream=stream)
+                kv.kv_unpack(ctx, buf, dst, dB, L, T, T, n * T, stream=stream)
+            stream.synchronize()
+            ctx.close()
+        except Exception as ex:  # noqa: BLE001
+            errors.append((t, repr(ex)))
+
+    threads = [threading.Thread(target=worker, args=(t,)) for t in range(nthreads)]
+    for th in threads:
+        th.start()
+    for th in threads:
+        th.join()
+    assert not errors, errors
+    torch.cuda.synchronize()
+    for B, tB, dB, steps in plans:
+        for src, dst in steps:
+            ko.unpack(ko.pack(A, src), dst, B, Ts=T, n_tokens=n * T)
+        assert_pool_equal(tB, B)
+    assert_pool_equal(tA, A)
