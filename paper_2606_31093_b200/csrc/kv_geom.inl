@@ -232,8 +232,9 @@ int make_geom(const kv_ctx *ctx, const kv_pool_desc *p, uint32_t layer_count, ui
       for (const Req &r : reqs) bytes += r.n_ids * g.pool_row * g.LC;
       if (bytes >= kAutoVecMinBytes && bytes < kAutoVecMaxBytes) kernel = KERNEL_VEC;
       // Segments of 1 KiB or less (one-token pages; re-paging between page sizes with no common divisor): an SM
-      // retires small bulk copies too slowly (about 11 M segments/s: 3.4 TB/s at 1 KiB), one warp per segment with
-      // 16-byte loads does 4.3-5.4 TB/s.  From 2 KiB the bulk ring (re-shaped, kv_launch.inl) is back at 6.2 TB/s.
+      // retires small bulk copies too slowly (about 11 M segments/s: 3.4 TB/s at 1 KiB); kv_move_small (32 segments
+      // decoded per warp at once, copied eight at a time) does 6.05-6.15 TB/s.  From 2 KiB the bulk ring (re-shaped,
+      // kv_launch.inl) is back at 6.2 TB/s.
       if (g.chunk_bytes <= 1024 && bytes >= (8ull << 20)) kernel = KERNEL_VEC;
     } else if (!g.trans) {
       // copy-on-write appends are many short, ragged pieces (about 6 KiB each): one warp per piece with 16-byte

@@ -12,6 +12,7 @@
 //                 at once (warp-level page-table lookup), lane 0 drives the async copy engine.
 //                 No data ever passes through registers.
 //   kv_move_vec   16-byte LDG/STG, one warp per segment, 8 loads in flight per lane.
+//   kv_move_small segments <= 1 KiB: 32 segments decoded per warp, copied eight at a time (16-byte LDG/STG).
 //   kv_move_elem  any alignment: unit-wide (1/2/4/8 B) coalesced copy.  Correctness fallback.
 //
 // This file shares nothing with oracle/.
@@ -670,6 +671,50 @@ __global__ void __launch_bounds__(256) kv_move_vec(const __grid_constant__ JobT<
     }
     for (; i < nv; i += 32) st_stream(d + i, ld_stream(s + i));
     for (i = nv + lane; i < nb; i += 32) st_stream(d + i, make_uint4(0, 0, 0, 0));
+  }
+}
+
+// ---------------------------------------------------------------------------------------------
+// kv_move_small: segments of at most 1 KiB (one-token pages; re-paging between page sizes with no common
+// divisor).  A segment is too short to pay for a warp-wide address computation of its own, so the 32 lanes
+// decode 32 segments at once (as kv_move_bulk does) and the warp then copies them eight at a time: two
+// 16-byte vectors per lane and segment, sixteen loads in flight per lane before the first store.
+// ---------------------------------------------------------------------------------------------
+template <int N>
+__global__ void __launch_bounds__(256) kv_move_small(const __grid_constant__ JobT<N> p) {
+  const Job &j = p.j;
+  const Tables tb = tables_of(p);
+  const uint32_t lane = threadIdx.x & 31;
+  const uint64_t G = (uint64_t)gridDim.x * (blockDim.x >> 5);
+  uint32_t hint = 0;
+  for (uint64_t base = ((uint64_t)blockIdx.x * (blockDim.x >> 5) + (threadIdx.x >> 5)) * 32; base < j.total_items;
+       base += G * 32) {
+    const uint32_t cnt = (uint32_t)min((uint64_t)32, j.total_items - base);
+    Item mine;
+    mine.src = mine.dst = 0; mine.bytes = mine.valid = 0;
+    if (lane < cnt) mine = decode<N == 0, false>(j, tb, base + lane, hint);
+    for (uint32_t k0 = 0; k0 < cnt; k0 += 8) {
+      uint4 v[8][2];
+      uint64_t dst[8];
+      uint32_t nb[8], nv[8];
+#pragma unroll
+      for (int q = 0; q < 8; ++q) {
+        const uint32_t k = min(k0 + q, 31u);
+        const uint64_t src = __shfl_sync(0xffffffffu, mine.src, k);
+        dst[q] = __shfl_sync(0xffffffffu, mine.dst, k);
+        nb[q] = k0 + q < cnt ? __shfl_sync(0xffffffffu, mine.bytes, k) >> 4 : 0;
+        nv[q] = k0 + q < cnt ? __shfl_sync(0xffffffffu, mine.valid, k) >> 4 : 0;
+        const uint4 *sp = reinterpret_cast<const uint4 *>(src);
+        v[q][0] = lane < nv[q] ? ld_stream(sp + lane) : make_uint4(0, 0, 0, 0);
+        v[q][1] = lane + 32 < nv[q] ? ld_stream(sp + lane + 32) : make_uint4(0, 0, 0, 0);
+      }
+#pragma unroll
+      for (int q = 0; q < 8; ++q) {
+        uint4 *dp = reinterpret_cast<uint4 *>(dst[q]);
+        if (lane < nb[q]) st_stream(dp + lane, v[q][0]);
+        if (lane + 32 < nb[q]) st_stream(dp + lane + 32, v[q][1]);
+      }
+    }
   }
 }
 

@@ -90,6 +90,13 @@ void launch_vec(const Job &j, const HostBlob *hb, bool trans, uint32_t grid, cud
   if (trans) kvt::kv_move_vec<8, N, true><<<grid, 256, 0, s>>>(p);
   else kvt::kv_move_vec<8, N, false><<<grid, 256, 0, s>>>(p);
 }
+template <int N>
+void launch_small(const Job &j, const HostBlob *hb, uint32_t grid, cudaStream_t s) {
+  static thread_local kvt::JobT<N> p;
+  p.j = j;
+  if constexpr (N > 0) std::memcpy(p.blob, hb->bytes.data(), hb->bytes.size());
+  kvt::kv_move_small<N><<<grid, 256, 0, s>>>(p);
+}
 template <typename U>
 void launch_elem(const kvt::JobT<0> &p, bool trans, uint32_t grid, cudaStream_t s) {
   if (trans) kvt::kv_move_elem<U, true><<<grid, 256, 0, s>>>(p);
@@ -185,7 +192,13 @@ int launch(kv_ctx *ctx, const Geom &g, const Blob &b, uint32_t piece_first, uint
     grid = (uint32_t)std::min<uint64_t>(want, cap ? cap : (uint32_t)ctx->sm_count * 8);
     kvt::JobT<0> p0;
     p0.j = j;
-    if (g.kernel == KERNEL_VEC) {
+    if (g.kernel == KERNEL_VEC && !g.trans && g.dir != 3 && g.sub_bytes <= 1024) {
+      // segments of <= 1 KiB: 32 of them per warp and pass (kv_move_small)
+      grid = (uint32_t)std::min<uint64_t>((total_items + wpb * 32 - 1) / (wpb * 32), cap ? cap : (uint32_t)ctx->sm_count * 8);
+      if (!b.inl) launch_small<0>(j, nullptr, grid, s);
+      else if (b.inl->bytes.size() <= kInlineSmall) launch_small<kInlineSmall>(j, b.inl, grid, s);
+      else launch_small<kInlineLarge>(j, b.inl, grid, s);
+    } else if (g.kernel == KERNEL_VEC) {
       if (!b.inl) launch_vec<0>(j, nullptr, g.trans, grid, s);
       else if (b.inl->bytes.size() <= kInlineSmall) launch_vec<kInlineSmall>(j, b.inl, g.trans, grid, s);
       else launch_vec<kInlineLarge>(j, b.inl, g.trans, grid, s);
