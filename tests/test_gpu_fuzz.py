@@ -134,3 +134,45 @@ def test_random_configuration(kv, seed):
     finally:
         torch.cuda.synchronize()
         ctx.close()
+
+
+MEDIUM = [  # Ts, Td, H, order_s, order_d, layout, tokens: sizes at which AUTO's rules and the re-shaped ring engage
+    (16, 16, 4, 0, 0, 0, 3000), (16, 16, 1, 0, 0, 0, 9000), (16, 16, 2, 0, 1, 0, 5000), (16, 64, 4, 0, 0, 0, 2048 * 3 - 37),
+    (64, 16, 4, 0, 0, 1, 4000), (16, 24, 4, 0, 0, 0, 3100), (5, 7, 4, 0, 0, 0, 3001), (1, 1, 4, 0, 0, 0, 2500),
+    (16, 16, 4, 1, 1, 0, 3000), (16, 64, 2, 1, 0, 0, 5000), (16, 16, 1, 0, 0, 1, 7000), (7, 5, 2, 0, 0, 0, 4100),
+    (16, 16, 1, 0, 0, 0, 5000), (16, 16, 2, 1, 1, 0, 2400),  # < 40 MiB of narrow rows: the bulk ring, re-shaped
+]
+
+
+@pytest.mark.parametrize("Ts,Td,H,order_s,order_d,layout,ntok", MEDIUM)
+def test_medium_sizes_with_default_options(kv, Ts, Td, H, order_s, order_d, layout, ntok):
+    """Tens of MiB per call with nothing overridden: the sizes at which the automatic choices engage -- the vec kernel
+    from 40 MiB, kv_move_small for segments <= 1 KiB, the ring re-shaped for narrow rows, guided claiming, tensor
+    maps -- through pack -> re-paging unpack -> fused re-page, against the oracle."""
+    L, C, D, e = 12, 2, 128, 2
+    rng = np.random.default_rng(hash((Ts, Td, H, order_s, order_d, layout, ntok)) % 2**31)
+    ctx = kv.Ctx(0)
+    try:
+        ns, nd = -(-ntok // Ts), -(-ntok // Td)
+        A = host_pool(rng, L, C, ns + 7, Ts, H, D, e, order=order_s)
+        B = host_pool(rng, L, C, nd + 9, Td, H, D, e, order=order_d)
+        B2 = ko.HostPool([s.copy() for s in B.slabs], L, C, nd + 9, Td, H, D, e, B.page_stride_bytes, order_d)
+        tA, dA = to_device(A, kv, torch)
+        tB, dB = to_device(B, kv, torch)
+        tB2, dB2 = to_device(B2, kv, torch)
+        sids = rng.permutation(ns + 7)[:ns].astype(np.int32)
+        dids = rng.permutation(nd + 9)[:nd].astype(np.int32)
+        buf = torch.zeros(ns * dA.page_bytes(), dtype=torch.uint8, device="cuda")
+        kv.kv_pack(ctx, dA, L, sids, buf, layout=layout)
+        want = ko.pack(A, sids, layout=layout, threads=8)
+        assert np.array_equal(buf.cpu().numpy(), want), "pack"
+        kv.kv_unpack(ctx, buf, dids, dB, L, Ts, Td, ntok, layout=layout, flags=kv.KV_FLAG_VALIDATE)
+        ko.unpack(want, dids, B, Ts=Ts, n_tokens=ntok, layout=layout, threads=8)
+        assert_pool_equal(tB, B)
+        kv.kv_repage(ctx, dA, sids, dB2, dids, L, ntok)
+        ko.repage(A, sids, B2, dids, n_tokens=ntok, threads=8)
+        assert_pool_equal(tB2, B2)
+        assert_pool_equal(tA, A)
+    finally:
+        torch.cuda.synchronize()
+        ctx.close()
