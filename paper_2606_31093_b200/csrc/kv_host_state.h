@@ -47,6 +47,7 @@ struct kv_ctx {
   cudaStream_t side = nullptr;
   cudaEvent_t ev_entry = nullptr;
   BlobSlot blobs[kBlobSlots];
+  void *blob_arena_h = nullptr, *blob_arena_d = nullptr;  // the slots' backing store: one pinned, one device allocation
   uint32_t next_blob = 0;
   uint32_t *d_status = nullptr;
   // staging for KV_HOST_STAGED

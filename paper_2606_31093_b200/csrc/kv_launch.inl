@@ -42,13 +42,22 @@ int upload_blob(kv_ctx *ctx, const HostBlob &hb, const int32_t *ids, bool ids_on
   BlobSlot &slot = ctx->blobs[ctx->next_blob++ % kBlobSlots];
   if (slot.used) KV_CUDA(ctx, cudaEventSynchronize(slot.ev));  // last reader of this slot is done
   if (slot.cap < bytes) {
-    if (slot.h) cudaFreeHost(slot.h);
-    if (slot.d) cudaFree(slot.d);
-    slot.h = slot.d = nullptr; slot.cap = 0;
-    size_t cap = std::max<size_t>(65536, bytes + bytes / 2);
-    KV_CUDA(ctx, cudaMallocHost(&slot.h, cap));
-    KV_CUDA(ctx, cudaMalloc(&slot.d, cap));
-    slot.cap = cap;
+    // The 16 slots are views into ONE pinned + ONE device arena, (re)allocated together: a slot that grew on its own
+    // cost a cudaFree (a device-wide sync) and a millisecond of cudaMallocHost per slot, i.e. 16 hiccups in a row.
+    for (BlobSlot &o : ctx->blobs)
+      if (o.used) KV_CUDA(ctx, cudaEventSynchronize(o.ev));
+    if (ctx->blob_arena_h) cudaFreeHost(ctx->blob_arena_h);
+    if (ctx->blob_arena_d) cudaFree(ctx->blob_arena_d);
+    ctx->blob_arena_h = ctx->blob_arena_d = nullptr;
+    for (BlobSlot &o : ctx->blobs) { o.h = o.d = nullptr; o.cap = 0; o.used = false; }
+    const size_t cap = (std::max<size_t>((size_t)256 << 10, bytes + bytes / 2) + 255) / 256 * 256;
+    KV_CUDA(ctx, cudaMallocHost(&ctx->blob_arena_h, cap * kBlobSlots));
+    KV_CUDA(ctx, cudaMalloc(&ctx->blob_arena_d, cap * kBlobSlots));
+    for (int i = 0; i < kBlobSlots; ++i) {
+      ctx->blobs[i].h = (uint8_t *)ctx->blob_arena_h + (size_t)i * cap;
+      ctx->blobs[i].d = (uint8_t *)ctx->blob_arena_d + (size_t)i * cap;
+      ctx->blobs[i].cap = cap;
+    }
   }
   std::memcpy(slot.h, hb.bytes.data(), bytes);
   KV_CUDA(ctx, cudaMemcpyAsync(slot.d, slot.h, bytes, cudaMemcpyHostToDevice, s));

@@ -110,14 +110,14 @@ int kv_ctx_destroy(kv_ctx *ctx) {
     cudaStreamSynchronize(ctx->side);
     for (auto &b : ctx->blobs) {
       if (b.used) cudaEventSynchronize(b.ev);
-      if (b.h) cudaFreeHost(b.h);
-      if (b.d) cudaFree(b.d);
       if (b.ev) cudaEventDestroy(b.ev);
     }
     for (int i = 0; i < kMaxStagingSlots; ++i) {
       if (ctx->ev_full[i]) cudaEventDestroy(ctx->ev_full[i]);
       if (ctx->ev_free[i]) { cudaEventSynchronize(ctx->ev_free[i]); cudaEventDestroy(ctx->ev_free[i]); }
     }
+    if (ctx->blob_arena_h) cudaFreeHost(ctx->blob_arena_h);
+    if (ctx->blob_arena_d) cudaFree(ctx->blob_arena_d);
     if (ctx->staging) cudaFree(ctx->staging);
     for (MapSet &m : ctx->map_sets) cudaFree(m.d);
     if (ctx->d_status) cudaFree(ctx->d_status);
