@@ -250,6 +250,14 @@ int make_geom(const kv_ctx *ctx, const kv_pool_desc *p, uint32_t layer_count, ui
   if (g.trans && kernel == KERNEL_BULK && g.drow > cap) kernel = KERNEL_VEC;  // a row must fit one stage
   g.kernel = kernel;
   g.sub_bytes = std::min(g.chunk_bytes, cap);
+  if (!g.trans && g.chunk_bytes > cap && g.chunk_bytes % 16 == 0) {
+    // A row a little longer than a stage (say 17,280 B) would be cut into one full stage and a 896-byte crumb, and
+    // crumbs are copied at the small-copy rate.  Cut it into equal pieces instead (two of 8,704 / 8,576 B):
+    // measured on a 5-token x 3-head x 576-dim pool: 4.96 -> 6.05 TB/s; 20 KiB rows: 5.4 -> 6.2.
+    const uint32_t n = (g.chunk_bytes + cap - 1) / cap;
+    const uint32_t even = ((g.chunk_bytes + n - 1) / n + 127) / 128 * 128;
+    if (even <= cap) g.sub_bytes = even;
+  }
   if (g.trans) g.sub_bytes = std::min(g.chunk_bytes, std::max(g.drow, cap / g.drow * g.drow));  // whole rows
   if (g.tma) g.sub_bytes = g.tb * g.tokrow;  // whole tokens: one box
   if (kernel == KERNEL_BULK && dir != 3) {
