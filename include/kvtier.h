@@ -115,7 +115,8 @@ typedef enum kv_option {
   KV_OPT_WARPS = 3,          /* bulk: issuing warps per CTA (1 .. 8) */
   KV_OPT_STORE_LAG = 4,      /* bulk: stores left in flight before a stage is refilled (1 .. 3) */
   KV_OPT_MAX_CTAS = 5,       /* cap on the grid (0 = SM count x CTAs per SM) */
-  KV_OPT_CHUNK_BYTES = 6,    /* staged host transfers: bytes per pipeline chunk (0 = staging_bytes / slots) */
+  KV_OPT_CHUNK_BYTES = 6,    /* staged host transfers: bytes per pipeline chunk (0 = automatic: equal chunks, at least three per
+                                transfer where that leaves 64 MiB each, at most one staging slot each) */
   KV_OPT_HOST_MAX_CTAS = 7,  /* grid cap for DIRECT host transfers (0 = same as device transfers) */
   KV_OPT_STAGING_SLOTS = 8,  /* staged host transfers: pipeline slots the staging buffer is cut into (2 .. 4) */
   KV_OPT_L2_HINT = 9,        /* bulk: 0 none, 1 evict_first cache hint on loads and stores */
