@@ -112,7 +112,8 @@ typedef enum kv_option {
   KV_OPT_KERNEL = 0,         /* 0 auto, 1 bulk (cp.async.bulk smem ring), 2 vec (16-byte LDG/STG), 3 elem (any alignment) */
   KV_OPT_STAGE_BYTES = 1,    /* bulk: bytes per shared-memory stage (multiple of 16, 1 KiB .. 64 KiB) */
   KV_OPT_STAGES_PER_WARP = 2,/* bulk: ring depth per issuing warp (2 .. 16) */
-  KV_OPT_WARPS = 3,          /* bulk: issuing warps per CTA (1 .. 8) */
+  KV_OPT_WARPS = 3,          /* bulk: issuing warps per CTA (1 .. 8).  Until options 1-3 are set the ring follows the row
+                                width: ~128 KiB of stages per SM (2 x 4 x 16 KiB ... 8 x 16 x 1 KiB); setting any pins it */
   KV_OPT_STORE_LAG = 4,      /* bulk: stores left in flight before a stage is refilled (1 .. 3) */
   KV_OPT_MAX_CTAS = 5,       /* cap on the grid (0 = SM count x CTAs per SM) */
   KV_OPT_CHUNK_BYTES = 6,    /* staged host transfers: bytes per pipeline chunk (0 = automatic: equal chunks, at least three per
