@@ -18,7 +18,14 @@ prefix = 512 fragmented pages (768 MiB), fresh page ids every step.
   cpu_baseline = the oracle (oracle/kv_oracle.c, as it stands) on the box's host cores, on a
               bounded sample of the same workload.
 
-`--impl reference` times the oracle alone (the reference arm of this tier).
+  roofline_host = offload / reload / both-at-once against the pinned cudaMemcpyAsync peaks measured in the SAME run
+              (BASELINE.json:north_star "host-link peak"), per_config = the other configs of BASELINE.json (turn 50 of
+              configs[2], configs[3] 26.5 GiB batched, configs[4] exact + ragged, six sweep points) device-timed with a
+              bit_exact flag each (bench_report.compact), peer = the NEXT-3 push into a pool on another GPU where
+              one is visible.
+
+`--impl reference` times the oracle alone (the reference arm of this tier) on the SAME config: the full 512-page prefix,
+--steps / --warmup honoured (a wall-clock cap, printed, is the only bound).
 `--report` additionally times every config of BASELINE.json and writes gpurun_out/report.json.
 Multi-GPU: the path does not shard with an exchange step -- replicas only:
 under torchrun each rank runs an independent replica; value = sum of units / max time.
@@ -39,10 +46,14 @@ sys.path.insert(0, ROOT)
 
 METRIC = "kv_pack_unpack_GBps"
 UNIT = "GB/s"
-# dram__bytes_read.sum + dram__bytes_write.sum of one kv_move_bulk launch at this workload (mean of 4
-# launches), from the `ncu --set full` capture summarised in profiles/r01_kv_move_bulk_full.md:
-# 805.4 MB read + 759.3 MB written (the last ~46 MB of the destination is still dirty in L2 at exit).
-NCU_TRAFFIC_BYTES_PER_LAUNCH = 1564.6e6
+# dram__bytes_read.sum + dram__bytes_write.sum of one kv_move_bulk launch (mean of 4 launches) from an `ncu --set full`
+# capture of THIS command at THIS workload.  It is a profile figure, not something this run measures: it is emitted only
+# when the run's configuration is the profiled one (512 pages, NHD pool, default kernel options), with the file named
+# beside it; otherwise `traffic` is null.  805.4 MB read + 759.3 MB written (the last ~46 MB written are still dirty in
+# L2 at exit).
+NCU_TRAFFIC = {"bytes_per_launch": 1564.6e6, "profile": "profiles/r01_kv_move_bulk_full.md",
+               "workload": {"pages": 512, "pool_order": "nhd", "kernel": "kv_move_bulk"}}
+REFERENCE_WALL_CAP_S = 150.0  # the reference arm stops adding steps beyond this (and says so); 50 steps need ~8 s
 
 
 def parse():
@@ -55,6 +66,7 @@ def parse():
     ap.add_argument("--prefix-tokens", type=int, default=8192)
     ap.add_argument("--e2e-steps", type=int, default=0, help="steps of the host-tier leg (0 = min(steps, 20))")
     ap.add_argument("--no-cpu-baseline", action="store_true")
+    ap.add_argument("--no-per-config", action="store_true", help="skip per_config / roofline_host / peer (small pools, plumbing tests)")
     ap.add_argument("--report", action="store_true", help="also time every BASELINE.json config -> gpurun_out/report.json")
     ap.add_argument("--pool-order", default="nhd", choices=["nhd", "hnd"],
                     help="in-page order of the pool (BASELINE.json configs are NHD; hnd = the NEXT-2 transposing transfers)")
@@ -133,34 +145,58 @@ class ClockSampler:
 # ------------------------------------------------------------------------------------------------
 # reference arm / cpu_baseline: the oracle on host cores
 # ------------------------------------------------------------------------------------------------
-def oracle_run(shape, pool_pages: int, n_pages: int, steps: int, warmup: int, threads: int, seed: int):
-    """Times oracle pack + unpack (C loops, as they stand) on a host pool.  Returns
-    (GB/s in the (read+written)/time convention, seconds per step)."""
+def bench_config(args, shape):
+    """The `config` object of BOTH arms (the reference arm times the oracle on our arm's config)."""
+    n = -(-args.prefix_tokens // shape.T)
+    return {
+        "workload": "configs[1] single-request prefix offload: pack 512 fragmented pages (8,192 tokens) "
+                    "to a device buffer + unpack a buffer into 512 other pages.  configs[1] is the configuration the metric's "
+                    "80 % bar is hardest on among those that are bandwidth-bound (768 MiB per call; configs[3] 26.5 GiB and "
+                    "configs[4] 6 GiB run at 1.00-1.02 of the same peak and are carried in per_config, configs[0] is launch-bound)",
+        "layers": shape.L, "kv_heads": shape.H, "head_dim": shape.D, "page_size": shape.T,
+        "pool_order": args.pool_order, "pool_pages": args.pool_pages,
+        "pool_GiB": round(shape.L * shape.C * args.pool_pages * shape.row_bytes / 2**30, 1),
+        "payload_MiB": n * shape.page_bytes / 2**20, "pages_per_step": n, "parallelism": "replicas only",
+        "l2": "inputs larger than L2 (768 MiB per op, fresh page ids per step; unpack reads the buffer packed one step earlier)",
+        "bytes_convention": "GB/s = (bytes read + bytes written) / time = 2*payload per op",
+    }
+
+
+def oracle_pool(shape, pool_pages: int, seed: int):
+    """Host-resident pool for the oracle: normal(0,1) bf16 bit patterns (upper 16 bits of float32 normals); one slab is
+    drawn, the others are rotations of it (the copy's speed does not depend on the values)."""
     from oracle import kv_oracle as ko
 
     rng = np.random.default_rng(seed)
     row = shape.row_bytes
-    # normal(0,1) bf16 bit patterns = upper 16 bits of float32 normals
-    def slab():
-        f = rng.standard_normal(pool_pages * row // 2, dtype=np.float32)
-        return (f.view(np.uint32) >> 16).astype(np.uint16).view(np.uint8)
-
-    one = slab()
+    f = rng.standard_normal(pool_pages * row // 2, dtype=np.float32)
+    one = (f.view(np.uint32) >> 16).astype(np.uint16).view(np.uint8)
     slabs = [one] + [np.roll(one, 4096 * (i + 1)) for i in range(shape.L * shape.C - 1)]
-    pool = ko.HostPool(slabs, shape.L, shape.C, pool_pages, shape.T, shape.H, shape.D, shape.e, row)
-    payload = n_pages * shape.page_bytes
+    return ko.HostPool(slabs, shape.L, shape.C, pool_pages, shape.T, shape.H, shape.D, shape.e, row), rng
+
+
+def oracle_run(pool, rng, shape, n_pages: int, steps: int, warmup: int, threads: int, wall_cap_s=None):
+    """Times oracle pack + unpack (C loops, as they stand) of `n_pages` fresh random pages per step.  Returns the
+    per-step seconds of the timed steps (fewer than `steps` only if the wall-clock cap was hit)."""
+    from oracle import kv_oracle as ko
+
     ts = []
+    t_begin = time.perf_counter()
     for s in range(warmup + steps):
-        ids = rng.choice(pool_pages, n_pages, replace=False).astype(np.int32)
-        dst = rng.choice(pool_pages, n_pages, replace=False).astype(np.int32)
+        ids = rng.choice(pool.num_pages, n_pages, replace=False).astype(np.int32)
+        dst = rng.choice(pool.num_pages, n_pages, replace=False).astype(np.int32)
         t0 = time.perf_counter()
         buf = ko.pack(pool, ids, threads=threads)
         ko.unpack(buf, dst, pool, Ts=shape.T, n_tokens=n_pages * shape.T, threads=threads)
         t1 = time.perf_counter()
         if s >= warmup:
             ts.append(t1 - t0)
-    sec = float(np.mean(ts))
-    return 4 * payload / sec / 1e9, sec
+        if wall_cap_s is not None and ts and time.perf_counter() - t_begin > wall_cap_s:
+            break
+    return ts
+
+
+ORACLE_POOL_PAGES = 4096  # BASELINE.md 4: "default 4,096 pages = 6 GiB at 48 L x 4 H x 128 D bf16, T 16"
 
 
 def run_reference(args):
@@ -171,18 +207,22 @@ def run_reference(args):
         return
     shape = W.QWEN3_OMNI
     cores = len(os.sched_getaffinity(0))
-    n_pages = 64  # bounded sample of the 512-page prefix
-    steps, warmup = max(1, min(args.steps, 10)), max(1, min(args.warmup, 2))
-    gbps, sec = oracle_run(shape, 256, n_pages, steps, warmup, cores, args.seed)
-    sample = (f"oracle pack+unpack of {n_pages} of the 512 pages per step on a 256-page host pool "
-              f"(48 L x 4 H x 128 D bf16), {steps} steps, {cores} OpenMP threads over the page loop")
+    n_pages = -(-args.prefix_tokens // shape.T)  # the FULL prefix of our arm's config: 512 pages per step
+    payload = n_pages * shape.page_bytes
+    pool, rng = oracle_pool(shape, ORACLE_POOL_PAGES, args.seed)
+    ts = oracle_run(pool, rng, shape, n_pages, args.steps, args.warmup, cores, wall_cap_s=REFERENCE_WALL_CAP_S)
+    sec = float(np.mean(ts))
+    gbps = 4 * payload / sec / 1e9
+    capped = len(ts) < args.steps
+    sample = (f"oracle pack+unpack of the full {n_pages}-page prefix per step on a {ORACLE_POOL_PAGES}-page host pool "
+              f"({ORACLE_POOL_PAGES * shape.page_bytes / 2**30:.0f} GiB, 48 L x 4 H x 128 D bf16; the pool is host-resident, so its "
+              f"size is bounded by RAM: BASELINE.md 4), {len(ts)} timed steps after {args.warmup} warm-ups, {cores} OpenMP threads "
+              f"over the page loop" + (f"; STOPPED at the {REFERENCE_WALL_CAP_S:.0f} s wall-clock cap before {args.steps} steps" if capped else ""))
     line = {
         "impl": "reference", "metric": METRIC, "value": gbps, "unit": UNIT, "n_gpus": args.gpus,
-        "steps": steps, "warmup": warmup, "ms_per_step": sec * 1e3, "higher_is_better": True,
-        "scaling": "weak", "vs_baseline": None, "dtype": "u16", "data": "synthetic",
-        "config": {"workload": "configs[1] single-request prefix offload (bounded sample)",
-                   "layers": shape.L, "kv_heads": shape.H, "head_dim": shape.D, "page_size": shape.T,
-                   "pages_per_step": n_pages},
+        "steps": len(ts), "warmup": args.warmup, "ms_per_step": sec * 1e3, "higher_is_better": True,
+        "scaling": "weak", "vs_baseline": None, "dtype": "u16 (bf16 bit patterns, bitwise copy)", "data": "synthetic",
+        "config": bench_config(args, shape),
         "cpu_baseline": {"value": gbps, "unit": UNIT, "cores": cores, "kind": "oracle", "sample": sample},
         "e2e": {"value": gbps, "unit": UNIT, "h2d_bytes_per_step": 0, "d2h_bytes_per_step": 0},
         "gpu_launches": 0,
@@ -193,6 +233,76 @@ def run_reference(args):
 # ------------------------------------------------------------------------------------------------
 # our arm
 # ------------------------------------------------------------------------------------------------
+def peer_leg(torch, kv, ctx, shape, local, seed):
+    """the provider pushes pages into a pool on ANOTHER GPU of the box over NVLink
+    (kv_unpack / kv_repage with the destination pool P2P-mapped), no collective; pull = kv_pack from the peer's pool.
+    Runs in ONE process whenever a second, peer-accessible GPU is visible (under torchrun every rank sees all GPUs);
+    reported against a cudaMemcpyPeerAsync peak measured here; results checked with torch indexing on the peer."""
+    ndev = torch.cuda.device_count()
+    if ndev < 2:
+        return {"available": False, "reason": f"{ndev} GPU visible to this process: the two-GPU push stays unmeasured on hardware"}
+    peer = (local + 1) % ndev
+    if not torch.cuda.can_device_access_peer(local, peer):
+        return {"available": False, "reason": f"GPU {local} has no peer path to GPU {peer}"}
+    import bench_report
+
+    kv.kv_peer_enable(ctx, peer)
+    pd = f"cuda:{peer}"
+    sp = shape.with_(P=4096)  # a 6 GiB destination pool on the peer
+    n = 512
+    page, row, L, T = sp.page_bytes, sp.row_bytes, sp.L, sp.T
+    rng = np.random.default_rng(seed + 31 + local)
+    pslabs = [torch.zeros(sp.P * row, dtype=torch.uint8, device=pd) for _ in range(L * sp.C)]
+    pdesc = kv.PoolDesc(pslabs, L, sp.C, sp.P, T, sp.H, sp.D, sp.e)
+    buf = torch.empty(n * page, dtype=torch.uint8, device=f"cuda:{local}")
+    buf.random_(0, 256)
+    back = torch.empty_like(buf)
+    stream = torch.cuda.current_stream()
+    flag = torch.zeros(1, dtype=torch.int64, device=pd)
+
+    def timed(fn, reps=10, warm=3):
+        for _ in range(warm):
+            fn()
+        stream.synchronize()
+        a, b = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+        a.record(stream)
+        for _ in range(reps):
+            fn()
+        b.record(stream)
+        stream.synchronize()
+        return a.elapsed_time(b) * 1e3 / reps  # us
+
+    # peak: plain device-to-device copies over the same link, both directions
+    tmp = torch.empty(n * page, dtype=torch.uint8, device=pd)
+    push_peak = n * page / timed(lambda: tmp.copy_(buf, non_blocking=True)) / 1e3
+    pull_peak = n * page / timed(lambda: back.copy_(tmp, non_blocking=True)) / 1e3
+    del tmp
+    ids = [rng.permutation(sp.P)[:n].astype(np.int32) for _ in range(16)]
+    it = iter(range(10**9))
+    us_push = timed(lambda: kv.kv_unpack(ctx, buf, ids[next(it) % 16], pdesc, L, T, T, n * T))
+    kv.kv_unpack(ctx, buf, ids[0], pdesc, L, T, T, n * T)
+    kv.kv_signal(ctx, flag, 1)  # availability flag in the peer's memory, behind the pages
+    stream.synchronize()
+    with torch.cuda.device(peer):
+        pchk = bench_report.Checker(torch, pslabs, sp)
+        vb = buf.to(pd)
+        ok_push = bool(pchk.unpack_ok(vb, ids[0])) and int(flag.item()) == 1
+    us_pull = timed(lambda: kv.kv_pack(ctx, pdesc, L, ids[next(it) % 16], back))
+    kv.kv_pack(ctx, pdesc, L, ids[3], back)
+    stream.synchronize()
+    with torch.cuda.device(peer):
+        ok_pull = bool(pchk.pack_ok(back.to(pd), ids[3]))
+    return {"available": True, "from_gpu": local, "to_gpu": peer, "payload_MiB": n * page / 2**20,
+            "push": {"op": "kv_unpack: local buffer -> 512 scattered pages of the peer's pool (posted stores)",
+                     "GBps": n * page / us_push / 1e3, "peak": push_peak, "frac": n * page / us_push / 1e3 / push_peak,
+                     "bit_exact": ok_push},
+            "pull": {"op": "kv_pack: 512 scattered pages of the peer's pool -> local buffer (loads over the link)",
+                     "GBps": n * page / us_pull / 1e3, "peak": pull_peak, "frac": n * page / us_pull / 1e3 / pull_peak,
+                     "bit_exact": ok_pull},
+            "peak_how": "cudaMemcpyPeerAsync (torch copy_ between the two devices) of the same 768 MiB, back to back, CUDA events",
+            "unit": "GB/s of payload over NVLink"}
+
+
 def run_ours(args):
     import torch
 
@@ -265,6 +375,15 @@ def run_ours(args):
         t_total_ms = max_over_ranks(ev[0].elapsed_time(ev[2 * K]))
         pack_ms = float(np.mean([ev[2 * i].elapsed_time(ev[2 * i + 1]) for i in range(K)]))
         unpack_ms = float(np.mean([ev[2 * i + 1].elapsed_time(ev[2 * i + 2]) for i in range(K)]))
+        # bit-exactness of the timed region's LAST step, with plain torch indexing (no library code, no oracle): the
+        # buffer just packed == gather of its source pages; the pages just scattered == the buffer they came from
+        import bench_report
+
+        u8 = [t.view(torch.uint8) for t in slabs]
+        chk = bench_report.Checker(torch, u8, shape)
+        hnd = (shape.H, shape.T, shape.D * shape.e) if args.pool_order == "hnd" else None
+        headline_ok = bool(chk.pack_ok(bufs[(K - 1) & 1], src_ids[Wm + K - 1], hnd=hnd)
+                           and chk.unpack_ok(bufs[K & 1], dst_ids[Wm + K - 1], hnd=hnd))
 
         # ---- host-tier legs: every step offloads 512 pages to pinned host memory and reloads 512 pages
         # from it, through the C ABI, host buffers, stream sync per step.
@@ -318,27 +437,53 @@ def run_ours(args):
         e1.record(s_off)  # both streams were synchronised by the last step
         barrier()
         e2e_ms = max_over_ranks(e0.elapsed_time(e1))
+        # the same schedule with the two host syncs per step replaced by cross-stream events (offload i -> reload i+1
+        # reads its buffer; reload i+1 -> offload i+2 overwrites it): what the link does when the host never waits
+        done_off = [torch.cuda.Event() for _ in range(Ke + 1)]
+        done_rel = [torch.cuda.Event() for _ in range(Ke + 1)]
+        e2, e3 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+        s_rel.wait_stream(s_off)
+        e2.record(s_off)
+        for i in range(Ke):
+            if i >= 2:
+                s_off.wait_event(done_rel[i - 1])
+            kv.kv_offload(ctx, desc, shape.L, src_ids[Wm + i], hp[i & 1], payload, mode=hm, stream=s_off)
+            done_off[i].record(s_off)
+            if i >= 1:
+                s_rel.wait_event(done_off[i - 1])
+            kv.kv_reload(ctx2, hp[(i + 1) & 1], payload, dst_ids[Wm + i], desc, shape.L, shape.T, shape.T, n * shape.T,
+                         mode=hm, stream=s_rel)
+            done_rel[i].record(s_rel)
+        s_off.wait_stream(s_rel)
+        e3.record(s_off)
+        barrier()
+        dup_nosync = {"achieved": 2 * payload * Ke / (e2.elapsed_time(e3) * 1e-3) / 1e9,
+                      "what": "the same Ke offload+reload steps with cross-stream events instead of host syncs"}
         ctx2.close()
         for h in hp:
             kv.kv_host_free(h)
+
+        link = per_config = None
+        peer = {"available": False, "reason": "skipped (--no-per-config)"}
+        if not args.no_per_config:
+            link = bench_report.link_peaks(torch)
+            dup_nosync["frac"] = dup_nosync["achieved"] / link["duplex_GBps"]
+            peer = peer_leg(torch, kv, ctx, shape, local, args.seed)
+            if rank == 0 and args.pool_pages >= 65536 and args.pool_order == "nhd":
+                per_config = bench_report.compact(ctx, desc, shape, u8, args.seed, measured_peaks()[0])
 
     peak, peak_src = measured_peaks()
     value = world * 4 * payload * K / (t_total_ms * 1e-3) / 1e9
     e2e_value = world * 4 * payload * Ke / (e2e_ms * 1e-3) / 1e9
     achieved = 2 * payload / (pack_ms * 1e-3) / 1e9
+    profiled = (args.pool_order == NCU_TRAFFIC["workload"]["pool_order"] and n == NCU_TRAFFIC["workload"]["pages"]
+                and kern_name == NCU_TRAFFIC["workload"]["kernel"] and args.pool_pages == 65536)
     line = {
         "metric": METRIC, "value": value, "unit": UNIT, "n_gpus": world, "steps": K, "warmup": Wm,
         "ms_per_step": t_total_ms / K, "higher_is_better": True, "scaling": "weak",
         "vs_baseline": None, "dtype": "u16 (bf16 bit patterns, bitwise copy)", "data": "synthetic",
-        "config": {
-            "workload": "configs[1] single-request prefix offload: pack 512 fragmented pages (8,192 tokens) "
-                        "to a device buffer + unpack a buffer into 512 other pages",
-            "layers": shape.L, "kv_heads": shape.H, "head_dim": shape.D, "page_size": shape.T,
-            "pool_order": args.pool_order, "pool_pages": P, "pool_GiB": round(shape.L * shape.C * P * shape.row_bytes / 2**30, 1),
-            "payload_MiB": payload / 2**20, "pages_per_step": n, "parallelism": "replicas only",
-            "l2": "inputs larger than L2 (768 MiB per op, fresh page ids per step; unpack reads the buffer packed one step earlier)",
-            "bytes_convention": "GB/s = (bytes read + bytes written) / time = 2*payload per op",
-        },
+        "config": bench_config(args, shape),
+        "bit_exact": headline_ok,
         "ops": {
             "pack_GBps": 2 * payload / (pack_ms * 1e-3) / 1e9, "pack_ms": pack_ms,
             "unpack_GBps": 2 * payload / (unpack_ms * 1e-3) / 1e9, "unpack_ms": unpack_ms,
@@ -346,61 +491,91 @@ def run_ours(args):
             "reload_link_GBps": payload / (rel_ms * 1e-3) / 1e9, "reload_ms": rel_ms,
             "host_mode": host_mode,
         },
-        "e2e": {"value": e2e_value, "unit": UNIT, "h2d_bytes_per_step": payload + 2 * (4 * n + 8 * shape.L * shape.C + 40 * 12),
+        "e2e": {"value": e2e_value, "unit": UNIT, "h2d_bytes_per_step": payload + 2 * (4 * n + 8 * shape.L * shape.C + 48 * 12),
                 "d2h_bytes_per_step": payload, "steps": Ke,
+                "link_GBps_payload": world * 2 * payload * Ke / (e2e_ms * 1e-3) / 1e9,
                 "what": "kv_offload (pool->pinned host) on one stream + kv_reload (pinned host->pool, buffer written one step earlier) "
-                        "on another, both through the C ABI, both streams synchronised every step",
+                        "on another, both through the C ABI, both streams synchronised every step.  `value` follows the metric's "
+                        "convention (bytes read + written on each side of the link = 4*payload per step); link_GBps_payload is what "
+                        "crosses the link, both directions summed",
                 "serial_value": world * 4 * payload / (serial_ms * 1e-3) / 1e9,
-                "serial_what": "same two calls on ONE stream, reload reading the buffer the offload just wrote",
-                "link_GBps_payload": world * 2 * payload * Ke / (e2e_ms * 1e-3) / 1e9},
+                "serial_what": "same two calls on ONE stream, reload reading the buffer the offload just wrote"},
         "gpu_launches": launches,
         "roofline": {"bound": "hbm", "kernel": f"{kern_name} (kv_pack launch)" if args.pool_order == "nhd"
                      else f"{kern_name}<kTrans> with tensor maps (kv_pack launch, HND pool)", "achieved": achieved,
                      "peak": peak, "unit": "GB/s", "frac": achieved / peak,
-                     "traffic": NCU_TRAFFIC_BYTES_PER_LAUNCH if args.pool_order == "nhd" and n == 512 else None, "algorithmic_bytes": 2 * payload,
-                     "peak_source": peak_src,
+                     "traffic": NCU_TRAFFIC["bytes_per_launch"] if profiled else None,
+                     "traffic_source": (f"ncu --set full capture of this command at this workload, {NCU_TRAFFIC['profile']} "
+                                        "(a profile figure, not measured by this run)") if profiled else None,
+                     "algorithmic_bytes": 2 * payload, "peak_source": peak_src,
                      "timing": "mean over the K timed steps of CUDA events on the launch stream around each kv_pack call (one launch; page ids ride in the kernel parameters)"},
         "clocks": clocks.summary(),
     }
+    if link is not None:  # host-link roofline: achieved payload GB/s against the pinned cudaMemcpyAsync peaks of THIS run
+        off_g, rel_g = payload / (off_ms * 1e-3) / 1e9, payload / (rel_ms * 1e-3) / 1e9
+        dup_g = 2 * payload * Ke / (e2e_ms * 1e-3) / 1e9  # this rank's link (replicas have a link each)
+        line["roofline_host"] = {
+            "bound": "host link (PCIe)", "unit": "GB/s of payload",
+            "offload": {"achieved": off_g, "peak": link["d2h_GBps"], "frac": off_g / link["d2h_GBps"]},
+            "reload": {"achieved": rel_g, "peak": link["h2d_GBps"], "frac": rel_g / link["h2d_GBps"]},
+            "duplex": {"achieved": dup_g, "peak": link["duplex_GBps"], "frac": dup_g / link["duplex_GBps"],
+                       "what": "the e2e leg (offload and reload at once, host sync every step) against D2H + H2D "
+                               "cudaMemcpyAsync at once"},
+            "duplex_no_host_sync": dup_nosync,
+            "peaks": link, "host_mode": host_mode,
+        }
+        line["e2e"]["frac_of_duplex_memcpy_peak"] = dup_g / link["duplex_GBps"]
+    if per_config is not None:
+        line["per_config"] = per_config
+    line["peer"] = peer
 
     if rank == 0 and not args.no_cpu_baseline:
+        # the oracle as it stands, 4,096-page host pool, same pages per call as the config (512),
+        # 3 warm-ups, median of 10; all cores, and a single thread
         cores = len(os.sched_getaffinity(0))
-        gbps, sec = oracle_run(W.QWEN3_OMNI, 1024, n, steps=6, warmup=1, threads=cores, seed=args.seed)
-        gbps1, _ = oracle_run(W.QWEN3_OMNI, 256, 64, steps=1, warmup=1, threads=1, seed=args.seed)
+        pool_o, rng_o = oracle_pool(W.QWEN3_OMNI, ORACLE_POOL_PAGES, args.seed)
+        ts = oracle_run(pool_o, rng_o, W.QWEN3_OMNI, n, steps=10, warmup=3, threads=cores)
+        ts1 = oracle_run(pool_o, rng_o, W.QWEN3_OMNI, n, steps=3, warmup=1, threads=1)
+        sec, sec1 = float(np.median(ts)), float(np.median(ts1))
         line["cpu_baseline"] = {
-            "value": gbps, "unit": UNIT, "cores": cores, "kind": "oracle",
-            "sample": f"oracle pack+unpack of the full {n}-page prefix on a 1,024-page host pool, 6 steps after 1 warm-up, "
-                      f"{cores} OpenMP threads over the page loop ({sec:.2f} s/step); single thread on a 64-page sample: {gbps1:.2f} GB/s",
-            "single_thread_value": gbps1,
+            "value": 4 * payload / sec / 1e9, "unit": UNIT, "cores": cores, "kind": "oracle",
+            "sample": f"oracle pack+unpack of the full {n}-page prefix per step on a {ORACLE_POOL_PAGES}-page host pool (6 GiB; BASELINE.md 4), "
+                      f"median of 10 steps after 3 warm-ups, {cores} OpenMP threads over the page loop ({sec:.2f} s/step); "
+                      f"single thread, same {n} pages, median of 3 after 1 warm-up: {4 * payload / sec1 / 1e9:.2f} GB/s ({sec1:.2f} s/step)",
+            "single_thread_value": 4 * payload / sec1 / 1e9,
         }
+        del pool_o
     if args.report and rank == 0:
-        from paper_2606_31093_b200 import report
+        import bench_report
 
-        line["report"] = report.run(ctx, desc, shape, [t.view(torch.uint8) for t in slabs], args.seed, hbm_peak=peak)
-        # the oracle of the NEXT-4 row timed beside the GPU records (cpu_baseline leg: the one place bench.py runs oracle/)
+        rep_full = bench_report.run(ctx, desc, shape, [t.view(torch.uint8) for t in slabs], args.seed, hbm_peak=peak)
+        # the oracle of the NEXT-4 row timed beside the GPU records, and the GPU's ids compared with it (cpu_baseline leg:
+        # the one place bench.py runs oracle/)
         from oracle import chain_oracle as co
 
         cores = len(os.sched_getaffinity(0))
         turns = W.session_turns(args.seed)
         chain_oracle = {}
-        for name, wb in (("config 3: one 50-turn session history (a single chain)", W.identity_batch(args.seed + 3, lens=[turns[-1].cum_tokens])),
-                         ("config 4: 64 requests, log-uniform 512-16,384 tokens", W.identity_batch(args.seed + 4, lens=W.batch_case(args.seed).lens)),
-                         ("4,096 sessions, log-uniform 512-16,384 tokens", W.identity_batch(args.seed + 5, n_sessions=4096))):
+        inputs = {"config 3: one 50-turn session history (a single chain)": W.identity_batch(args.seed + 3, lens=[turns[-1].cum_tokens]),
+                  "config 3: one turn's increment (60 pages, a single chain)": W.identity_batch(args.seed + 6, lens=[60 * shape.T]),
+                  "config 4: 64 requests, log-uniform 512-16,384 tokens": W.identity_batch(args.seed + 4, lens=W.batch_case(args.seed).lens),
+                  "4,096 sessions, log-uniform 512-16,384 tokens": W.identity_batch(args.seed + 5, n_sessions=4096)}
+        for r in rep_full["records"]:
+            wb = inputs.get(r.get("op")) if r.get("config") == "NEXT-4 chain hash" else None
+            if wb is None:
+                continue
             ts = {}
             for th in (1, cores):
                 best = 1e30
                 for _ in range(3):
                     t0 = time.perf_counter()
-                    co.chain_batched(wb.ident, wb.tok_offsets, shape.T, threads=th)
+                    want_ids = co.chain_batched(wb.ident, wb.tok_offsets, shape.T, threads=th)[0]
                     best = min(best, time.perf_counter() - t0)
                 ts[th] = best * 1e6
-            chain_oracle[name] = {"us_1thread": ts[1], "us_all_cores": ts[cores], "cores": cores}
-        rp = os.path.join(ROOT, "gpurun_out", "report.json")
-        with open(rp) as f:
-            full = json.load(f)
-        full["chain_oracle"] = chain_oracle
-        with open(rp, "w") as f:
-            json.dump(full, f, indent=1)
+            chain_oracle[r["op"]] = {"us_1thread": ts[1], "us_all_cores": ts[cores], "cores": cores}
+            r["verified"] = bool(np.array_equal(r["_ids"], want_ids))
+        rep_full["chain_oracle"] = chain_oracle
+        line["report"] = bench_report.write(rep_full)
         line["report"]["chain_oracle"] = chain_oracle
     if rank == 0:
         print(json.dumps(line))
@@ -410,15 +585,9 @@ def run_ours(args):
 
 def main():
     args = parse()
-    if int(os.environ.get("LOCAL_RANK", "0")) == 0:  # fresh checkout: build what is missing (one rank per node)
-        import __graft_entry__
+    import __graft_entry__
 
-        __graft_entry__.ensure_built()
-    else:  # the other ranks of the node wait for rank 0's build instead of racing it
-        lib = os.path.join(ROOT, "paper_2606_31093_b200", "libkvtier.so")
-        t0 = time.time()
-        while args.impl == "ours" and not os.path.exists(lib) and time.time() - t0 < 300:
-            time.sleep(1.0)
+    __graft_entry__.ensure_built()  # every rank: mtime-based, serialised by a file lock (one compiles, the others wait)
     if args.impl == "reference":
         run_reference(args)
     else:

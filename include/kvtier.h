@@ -30,9 +30,14 @@
  *   - CUDA graphs: every transfer whose tables fit the kernel parameters is ONE kernel node and may be
  *     captured (cudaStreamBeginCapture on `stream`); page ids passed as host arrays are baked into the
  *     node, ids passed with KV_FLAG_IDS_ON_DEVICE are re-read from device memory at every replay.
- *     Host-tier calls captured with KV_HOST_AUTO use DIRECT.  Otherwise: KV_ERR_CAPTURE.
+ *     STAGED host transfers are capturable too (copy nodes on a forked branch + one kernel node per chunk, each
+ *     with its tables in its parameters) once the ctx's staging exists (KV_OPT_RESERVE_STAGING, or any earlier
+ *     staged call): KV_HOST_AUTO then captures what it would run eagerly; without staging it captures DIRECT.
+ *     A graph holding staged transfers uses the ctx's staging buffer at every replay: replay it on the stream on
+ *     which the ctx's other staged transfers run, or not at the same time as them.  Otherwise: KV_ERR_CAPTURE.
  *   - A kv_ctx is not thread-safe: one ctx per calling thread.  Calls on different streams are
- *     independent when their destination page sets are disjoint.
+ *     independent when their destination page sets are disjoint; staged host transfers of ONE ctx issued on
+ *     different streams share its staging slots and are ordered against one another slot by slot.
  */
 #ifndef KVTIER_H
 #define KVTIER_H
@@ -99,8 +104,9 @@ typedef enum kv_status {
   KV_ERR_DESC = -9,       /* malformed kv_pool_desc (zero dimension, bad elem_bytes or order, stride < row, layer_count too large) */
   KV_ERR_NO_DEVICE = -10, /* planning-only ctx (device < 0): arguments were valid, nothing was launched */
   KV_ERR_CAPTURE = -11,   /* `stream` is capturing a CUDA graph and this call is not replayable: its tables exceed
-                             the kernel parameters (~31 KiB: about 7,500 page ids), the element-wise fallback kernel
-                             is needed, or mode is KV_HOST_STAGED.  Nothing was enqueued. */
+                             the kernel parameters (~31 KiB: about 7,500 page ids per launch), the element-wise
+                             fallback kernel is needed, or mode is KV_HOST_STAGED and the ctx has no staging buffer
+                             yet.  Nothing was enqueued. */
 } kv_status;
 
 /* flags (bit set) */
@@ -131,6 +137,10 @@ typedef enum kv_option {
   KV_OPT_PDL = 13,           /* bulk: 1 (default) = launch with programmatic stream serialization: the grid may become resident
                                 and run its prologue while the previous kernel of the stream drains; it touches no
                                 global memory before that kernel has completed (griddepcontrol.wait) */
+  KV_OPT_RESERVE_STAGING = 14, /* allocate the staging buffer of STAGED host transfers NOW (value = bytes; 0 = the size given
+                                to kv_ctx_create, else 512 MiB) instead of on the first staged call -- required before a
+                                first staged transfer can be captured.  Already allocated: KV_OK if value is 0 or the
+                                same size, else KV_ERR_SIZE. */
 } kv_option;
 
 /* kv_ctx_get_stat keys */
@@ -197,10 +207,11 @@ int kv_signal(kv_ctx *ctx, uint64_t *flag, uint64_t value, kv_stream_t stream);
  *   roots         HOST uint64[n_sessions] or NULL
  *   out           DEVICE uint64[out_capacity]; ids of session s start at page_offsets[s] (sessions back to back)
  *   page_offsets  HOST int64[n_sessions+1], written by the call (may be NULL)
- * Two launches on `stream` (per-page digests in parallel, then one warp per session along the chain);
- * results are defined after the caller synchronises `stream`.  Errors: KV_ERR_NULL, KV_ERR_SIZE (page_size
- * 0, bad offsets, out_capacity too small), KV_ERR_ALIGN, KV_ERR_CAPTURE (more than 128 sessions: the tables do
- * not fit the kernel parameters; up to 128 the call is two self-contained launches and capturable), KV_ERR_NO_DEVICE
+ * Up to 128 sessions: ONE launch on `stream` (a CTA per session digests its pages, then its first warp walks the
+ * chain), tables in the kernel parameters, capturable.  More: two launches (per-page digests of all sessions in
+ * parallel, then one warp per session along the chain) with tables staged through the ctx's pinned ring.
+ * Results are defined after the caller synchronises `stream`.  Errors: KV_ERR_NULL, KV_ERR_SIZE (page_size
+ * 0, bad offsets, out_capacity too small), KV_ERR_ALIGN, KV_ERR_CAPTURE (more than 128 sessions), KV_ERR_NO_DEVICE
  * (planning-only ctx; page_offsets are still written), KV_ERR_CUDA.  n_sessions == 0 or no whole page:
  * KV_OK, nothing launched. */
 #define KV_CHAIN_ROOT 0xcbf29ce484222325ull
@@ -249,6 +260,34 @@ int kv_unpack_batched(kv_ctx *ctx, const void *const *srcs, const uint64_t *src_
                       const uint64_t *n_tokens, uint32_t n_req, const kv_pool_desc *pools,
                       uint32_t layer_count, uint32_t src_page_size, uint32_t dst_page_size,
                       int layout, uint32_t flags, kv_stream_t stream);
+
+/* ---- several independent transfers in ONE launch ----------
+ * A serving turn issues small transfers back to back -- scatter a matched prefix into fresh pages, extend the
+ * retained partial page copy-on-write (the append follows the reload in every turn), gather the
+ * pages that became full -- and below ~100 MiB each of them is bound by launch latency, not by HBM.  kv_submit
+ * runs a list of such operations on ONE pool as one persistent launch: the direction is a property of the piece,
+ * not of the launch.
+ *   KV_OP_PACK        buf[p][l][c][..] = POOL[l][c][page_ids[p]]          (kv_pack; n_pages ids, buf written)
+ *   KV_OP_UNPACK      POOL[l][c][page_ids[q]] = buf[q][l][c][..], slots >= n_tokens zero  (kv_unpack with the buffer's
+ *                     page size equal to the pool's; n_pages must be ceil(n_tokens / page_size))
+ *   KV_OP_COW_APPEND  kv_cow_append with old_id = page_ids[0], new_id = page_ids[1], append block `buf`
+ * The operations of one call are UNORDERED among themselves: no operation may read a page or buffer that another
+ * one writes, and all written pages must be distinct (both checked under KV_FLAG_VALIDATE -> KV_ERR_DUP_PAGE for
+ * pages; buffers are the caller's responsibility).  The result equals the single calls issued in any order.
+ * Errors as the single calls; KV_FLAG_IDS_ON_DEVICE is not supported here (KV_ERR_LAYOUT).  n_ops == 0 or nothing
+ * to move: KV_OK, no launch. */
+typedef enum kv_op_kind { KV_OP_PACK = 0, KV_OP_UNPACK = 1, KV_OP_COW_APPEND = 3 } kv_op_kind;
+typedef struct kv_op {
+  uint32_t kind;           /* kv_op_kind */
+  uint32_t n_pages;        /* PACK: pages gathered; UNPACK: destination pages; COW_APPEND: ignored */
+  const int32_t *page_ids; /* HOST array: PACK source ids / UNPACK destination ids (n_pages of them); COW_APPEND: {old, new} */
+  void *buf;               /* device-accessible: PACK destination buffer; UNPACK source buffer; COW_APPEND append block (NULL if n_app == 0) */
+  uint64_t buf_bytes;      /* PACK / UNPACK: size of buf for the bounds check (0 = unchecked) */
+  uint64_t n_tokens;       /* UNPACK: valid tokens (n_pages * page_size = verbatim whole pages) */
+  uint32_t n_old, n_app;   /* COW_APPEND: tokens kept from the old page, tokens appended; n_old + n_app <= page_size */
+} kv_op;
+int kv_submit(kv_ctx *ctx, const kv_pool_desc *pools, uint32_t layer_count, const kv_op *ops, uint32_t n_ops,
+              int layout, uint32_t flags, kv_stream_t stream);
 
 /* ---- fused pool -> pool re-paging (8(c) reading 11) ------------------
  * kv_repage: kv_pack followed by kv_unpack without the transfer buffer, for cross-role reuse on one

@@ -2,7 +2,8 @@
 // kv_chain_hash).  id_k = FNV1a64(LE64(id_{k-1}) || LE64(digest_k)), digest_k = FNV1a64 of the 8*T
 // little-endian bytes of page k's T content identities; id_{-1} = the session's root.
 //
-// The work splits where the dependence does:
+// The work splits where the dependence does (two launches for large batches; kv_chain_fused does both phases in one
+// launch for up to 128 sessions):
 //   kv_chain_digest  one THREAD per page, all pages of all sessions at once: 8*T dependent
 //                    xor/multiply steps per page, no dependence between pages -- the parallel 8/9ths.
 //   kv_chain_link    one WARP per session: the chain proper, 16 dependent steps per page.  The 32 lanes
@@ -86,33 +87,21 @@ __device__ __forceinline__ ChainJob chain_job(const P &p) {
   }
 }
 
-template <bool kInline>
-__global__ void __launch_bounds__(128) kv_chain_digest(const __grid_constant__ typename ChainParam<kInline>::type prm) {
-  const ChainJob j = chain_job<kInline>(prm);
-  const uint64_t p = (uint64_t)blockIdx.x * blockDim.x + threadIdx.x;
-  if (p >= j.total_pages) return;
-  uint32_t lo = 0, hi = j.n_sessions;  // largest s with page_off[s] <= p
-  while (hi - lo > 1) {
-    const uint32_t mid = (lo + hi) >> 1;
-    if ((uint64_t)j.page_off[mid] <= p) lo = mid; else hi = mid;
-  }
-  const uint64_t k = p - (uint64_t)j.page_off[lo];
-  const uint64_t *src = j.ident + (uint64_t)j.tok_off[lo] + k * j.T;
+// digest of page k of session s (8*T dependent steps; four identity loads in flight ahead of the arithmetic)
+__device__ __forceinline__ uint64_t chain_digest_page(const ChainJob &j, uint32_t s, uint64_t k) {
+  const uint64_t *src = j.ident + (uint64_t)j.tok_off[s] + k * j.T;
   uint64_t h = kFnvBasis;
   uint32_t t = 0;
-  for (; t + 4 <= j.T; t += 4) {  // four loads in flight ahead of the dependent arithmetic
+  for (; t + 4 <= j.T; t += 4) {
     const uint64_t w0 = __ldg(src + t), w1 = __ldg(src + t + 1), w2 = __ldg(src + t + 2), w3 = __ldg(src + t + 3);
     h = fnv1a_word(fnv1a_word(fnv1a_word(fnv1a_word(h, w0), w1), w2), w3);
   }
   for (; t < j.T; ++t) h = fnv1a_word(h, __ldg(src + t));
-  j.out[p] = h;
+  return h;
 }
 
-template <bool kInline>
-__global__ void __launch_bounds__(32) kv_chain_link(const __grid_constant__ typename ChainParam<kInline>::type prm) {
-  const ChainJob j = chain_job<kInline>(prm);
-  const uint32_t s = blockIdx.x, lane = threadIdx.x;
-  if (s >= j.n_sessions) return;
+// the chain of session s, walked by one warp: digests in j.out[p0, p1) are replaced by the ids
+__device__ __forceinline__ void chain_link_session(const ChainJob &j, uint32_t s, uint32_t lane) {
   const uint64_t p0 = (uint64_t)j.page_off[s], p1 = (uint64_t)j.page_off[s + 1];
   uint64_t prev = j.roots ? j.roots[s] : j.default_root;
   uint64_t next_d = p0 + lane < p1 ? j.out[p0 + lane] : 0;
@@ -130,6 +119,41 @@ __global__ void __launch_bounds__(32) kv_chain_link(const __grid_constant__ type
     }
     if (lane < n) j.out[base + lane] = mine;
   }
+}
+
+template <bool kInline>
+__global__ void __launch_bounds__(128) kv_chain_digest(const __grid_constant__ typename ChainParam<kInline>::type prm) {
+  const ChainJob j = chain_job<kInline>(prm);
+  const uint64_t p = (uint64_t)blockIdx.x * blockDim.x + threadIdx.x;
+  if (p >= j.total_pages) return;
+  uint32_t lo = 0, hi = j.n_sessions;  // largest s with page_off[s] <= p
+  while (hi - lo > 1) {
+    const uint32_t mid = (lo + hi) >> 1;
+    if ((uint64_t)j.page_off[mid] <= p) lo = mid; else hi = mid;
+  }
+  j.out[p] = chain_digest_page(j, lo, p - (uint64_t)j.page_off[lo]);
+}
+
+template <bool kInline>
+__global__ void __launch_bounds__(32) kv_chain_link(const __grid_constant__ typename ChainParam<kInline>::type prm) {
+  const ChainJob j = chain_job<kInline>(prm);
+  if (blockIdx.x >= j.n_sessions) return;
+  chain_link_session(j, blockIdx.x, threadIdx.x);
+}
+
+// Batches of up to kChainInlineSessions sessions: ONE launch, one CTA per session.  All threads of the CTA digest the
+// session's pages (one page per thread and pass), the CTA meets, warp 0 walks the chain.  The digest phase of even the
+// longest paper-shaped history (2,875 pages on 1,024 threads: three passes of 128 steps) is ~3 us against the 377 us of
+// its chain, and a turn's incremental hash of a few dozen pages is one launch instead of two.
+template <bool kInline>
+__global__ void __launch_bounds__(1024) kv_chain_fused(const __grid_constant__ typename ChainParam<kInline>::type prm) {
+  const ChainJob j = chain_job<kInline>(prm);
+  const uint32_t s = blockIdx.x;
+  if (s >= j.n_sessions) return;
+  const uint64_t p0 = (uint64_t)j.page_off[s], p1 = (uint64_t)j.page_off[s + 1];
+  for (uint64_t p = p0 + threadIdx.x; p < p1; p += blockDim.x) j.out[p] = chain_digest_page(j, s, p - p0);
+  __syncthreads();  // the digests (global memory) are visible to warp 0
+  if (threadIdx.x < 32) chain_link_session(j, s, threadIdx.x);
 }
 
 }  // namespace kvt

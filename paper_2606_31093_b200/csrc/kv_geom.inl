@@ -35,6 +35,7 @@ struct Req {          // one request as the caller states it
   uint64_t id_begin = 0, n_ids = 0;  // its page ids in the call's id array
   uint64_t n_buf_pages = 0;
   uint64_t items = 0;  // work items of this request (filled by the planners)
+  uint32_t dir = 0;    // kv_submit only: this request's direction (0 pack, 1 unpack, 3 copy-on-write append)
 };
 
 int check_desc(const kv_pool_desc *p, uint32_t layer_count) {
@@ -64,6 +65,12 @@ bool capturing(cudaStream_t s) {
   cudaStreamCaptureStatus st = cudaStreamCaptureStatusNone;
   if (cudaStreamIsCapturing(s, &st) != cudaSuccess) { (void)cudaGetLastError(); return false; }
   return st != cudaStreamCaptureStatusNone;
+}
+// Every entry point that may launch calls this first: one capture query per call, not one per launch.
+void enter(kv_ctx *ctx, kv_stream_t stream) {
+  if (!ctx) return;
+  ctx->cur_stream = (cudaStream_t)stream;
+  ctx->cur_capturing = !ctx->host_only && capturing(ctx->cur_stream);
 }
 
 uint32_t gcd32(uint32_t a, uint32_t b) {
@@ -208,7 +215,7 @@ int make_geom(const kv_ctx *ctx, const kv_pool_desc *p, uint32_t layer_count, ui
     const uint32_t cap16 = std::max(16u, ctx->stage_bytes / 16 * 16);
     if (tma_eligible(ctx, p, g.src_hnd ? src_pool : nullptr, layer_count, g.g, tokrow, g.drow, cap16, &tb, &es)) {
       bool cached_or_free = true;
-      if (!ctx->host_only && capturing(ctx->cur_stream)) {
+      if (!ctx->host_only && ctx->cur_capturing) {
         std::vector<uint64_t> key;
         if (g.pool_hnd) { map_key(p, layer_count, tb, es, &key); cached_or_free = find_maps(ctx, key) != nullptr; }
         if (cached_or_free && g.src_hnd) { map_key(src_pool, layer_count, tb, es, &key); cached_or_free = find_maps(ctx, key) != nullptr; }

@@ -53,9 +53,15 @@ struct kv_ctx {
   // staging for KV_HOST_STAGED
   void *staging = nullptr;
   size_t staging_bytes = 0;
+  // Slot i is ALWAYS the bytes [i * pitch, (i + 1) * pitch) of `staging`, pitch = staging_bytes / staging_slots: a
+  // call whose chunks are smaller uses a prefix of each slot.  The per-slot events therefore guard the same memory for
+  // every call, whatever its chunk size and whichever stream it runs on.
   cudaEvent_t ev_full[kMaxStagingSlots] = {};  // producer into the slot finished
   cudaEvent_t ev_free[kMaxStagingSlots] = {};  // consumer of the slot finished
   bool free_valid[kMaxStagingSlots] = {};
+  // the same roles inside a stream capture: captured records are not real records, so they get events of their own
+  // and never touch the bookkeeping of eager calls
+  cudaEvent_t cap_entry = nullptr, cap_full[kMaxStagingSlots] = {}, cap_free[kMaxStagingSlots] = {};
   int last_cuda_error = 0;
   // options
   int kernel = KERNEL_AUTO;
@@ -68,7 +74,8 @@ struct kv_ctx {
   uint32_t next_sched = 0;
   EncodeTiledFn encode_tiled = nullptr;  // cuTensorMapEncodeTiled, nullptr if the driver has none
   std::vector<MapSet> map_sets;
-  cudaStream_t cur_stream = nullptr;     // stream of the entry point being served (capture check while planning)
+  cudaStream_t cur_stream = nullptr;     // stream of the entry point being served
+  bool cur_capturing = false;            // ... and whether it is being captured (queried once per call)
   uint64_t last_tma = 0;
   size_t chunk_bytes = 0;
   // stats

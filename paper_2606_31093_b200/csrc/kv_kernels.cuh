@@ -26,12 +26,15 @@ namespace kvt {
 //   dir 2 (pool -> pool): `buf` is the index of the request's first SOURCE page id in ids[].
 //   dir 3 (copy-on-write append, one piece per session): `buf` = append block address,
 //         n_tokens = n_old | n_app << 32, id_begin = old page id | new page id << 32.
+//   dir 4 (kv_submit: a mixed launch): every piece carries its own direction (0, 1 or 3) in `dir`.
 struct Piece {
   uint64_t item_begin;   // first flat item index of this piece within the launch
   uint64_t buf;          // buffer base address (device memory or mapped pinned host memory)
   uint64_t n_tokens;     // valid tokens; destination slots >= n_tokens are zero-filled (unpack)
   uint64_t id_begin;     // index of this piece's first page id in ids[]
   uint64_t n_buf_pages;  // pages in this piece's buffer (layer-first page stride)
+  uint32_t dir;          // Job::dir == 4 only: this piece's direction (0 pack, 1 unpack, 3 copy-on-write append)
+  uint32_t pad_;
 };
 
 struct Job {
@@ -46,7 +49,8 @@ struct Job {
   uint32_t n_pieces;
   uint32_t LC;            // layer_count * kv_count
   uint32_t dir;           // 0 pack (pool -> buffer), 1 unpack (buffer -> pool), 2 re-page (pool -> pool),
-                          // 3 copy-on-write append (old page + append block -> new page)
+                          // 3 copy-on-write append (old page + append block -> new page),
+                          // 4 mixed (kv_submit): the direction is a property of the piece (Piece::dir)
   uint32_t layout;        // 0 page-first, 1 layer-first
   uint32_t g;             // tokens per chunk = gcd(Tpool, Tbuf)
   uint32_t cpp_pool;      // chunks per pool page  = Tpool / g
@@ -129,7 +133,8 @@ struct Item {
   uint64_t src, dst;
   uint32_t bytes;  // bytes written at dst
   uint32_t valid;  // first `valid` bytes come from src, the rest is zero fill
-  // kTrans only: bit 0 = src strided, bit 1 = dst strided.  A strided side's address is the base of
+  // kTrans only: bit 0 = src strided, bit 1 = dst strided, bit 2 = never by tensor copies (copy-on-write rows).
+  // A strided side's address is the base of
   // the CHUNK (token 0, head 0) and the item covers rows [r0, r0 + bytes/drow) of it; a contiguous
   // side's address already points at the item's first byte.
   uint32_t mode;
@@ -166,7 +171,8 @@ __device__ __forceinline__ Item decode(const Job &j, const Tables &tb, uint64_t 
   const uint64_t item_begin = ldt<kGlobal>(&pc->item_begin), buf = ldt<kGlobal>(&pc->buf),
                  n_tokens = ldt<kGlobal>(&pc->n_tokens), id_begin = ldt<kGlobal>(&pc->id_begin);
   const uint32_t local = (uint32_t)(item - item_begin);
-  if (j.dir == 3) {  // copy-on-write append: per (layer,kv) s0 items copy the old
+  const uint32_t dir = j.dir == 4 ? ldt<kGlobal>(&pc->dir) : j.dir;
+  if (dir == 3) {  // copy-on-write append: per (layer,kv) s0 items copy the old
                      // page's first n_old tokens, s1 items append the session's new rows behind them
     const uint32_t n_old = (uint32_t)n_tokens, n_app = (uint32_t)(n_tokens >> 32);
     const uint32_t b_old = n_old * j.tokrow, b_app = n_app * j.tokrow;
@@ -192,13 +198,13 @@ __device__ __forceinline__ Item decode(const Job &j, const Tables &tb, uint64_t 
       const uint32_t o = k * j.sub_bytes;
       it.src = old_pg + o; it.dst = new_pg + o; it.bytes = min(j.sub_bytes, b_old - o);
       if (kTrans && j.pool_hnd) {  // rows of the first n_old tokens, same place in both pages
-        it.src = old_pg; it.dst = new_pg; it.mode = 3; it.r0 = o / j.drow;
+        it.src = old_pg; it.dst = new_pg; it.mode = 3 | 4; it.r0 = o / j.drow;
       }
     } else {
       const uint32_t o = (k - s0) * j.sub_bytes;
       it.src = buf + (uint64_t)lc * b_app + o; it.dst = new_pg + b_old + o; it.bytes = min(j.sub_bytes, b_app - o);
       if (kTrans && j.pool_hnd) {  // NHD append block -> token slots n_old.. of every head's run
-        it.dst = new_pg + (uint64_t)n_old * j.p_ts; it.mode = 2; it.r0 = o / j.drow;
+        it.dst = new_pg + (uint64_t)n_old * j.p_ts; it.mode = 2 | 4; it.r0 = o / j.drow;
       }
     }
     it.valid = it.bytes;
@@ -227,9 +233,9 @@ __device__ __forceinline__ Item decode(const Job &j, const Tables &tb, uint64_t 
   const uint64_t tok0 = (uint64_t)k * j.g;
   const uint64_t vt = n_tokens > tok0 ? min(n_tokens - tok0, (uint64_t)j.g) : 0;
   uint64_t baddr;
-  if (j.dir == 2 && vt == 0) {  // wholly zero-padded chunk: there is no source page to look up
+  if (dir == 2 && vt == 0) {  // wholly zero-padded chunk: there is no source page to look up
     baddr = 0;
-  } else if (j.dir == 2) {  // pool -> pool: the "buffer" side is page src_ids[bp] of the source pool
+  } else if (dir == 2) {  // pool -> pool: the "buffer" side is page src_ids[bp] of the source pool
     const int32_t sid = j.src_ids ? __ldg(j.src_ids + buf + bp)
                                   : ((kGlobal || j.ids) ? __ldg(tb.ids + buf + bp) : tb.ids[buf + bp]);
     if ((uint32_t)sid >= j.src_num_pages) {
@@ -248,12 +254,12 @@ __device__ __forceinline__ Item decode(const Job &j, const Tables &tb, uint64_t 
   }
   const uint64_t vbytes = vt * j.tokrow;
   it.valid = vbytes > sub_off ? (uint32_t)min(vbytes - sub_off, (uint64_t)it.bytes) : 0u;
-  if (j.dir == 0) { it.src = paddr; it.dst = baddr; } else { it.src = baddr; it.dst = paddr; }
+  if (dir == 0) { it.src = paddr; it.dst = baddr; } else { it.src = baddr; it.dst = paddr; }
   if (kTrans) {
-    it.mode = j.dir == 0 ? (pmode | bmode << 1) : (bmode | pmode << 1);
+    it.mode = dir == 0 ? (pmode | bmode << 1) : (bmode | pmode << 1);
     it.r0 = (uint32_t)(sub_off / j.drow);
     const uint32_t pt = pk * j.g + (uint32_t)(sub_off / j.tokrow);
-    if (j.dir == 0) { it.s_pg = (uint32_t)id; it.s_t = pt; } else { it.d_pg = (uint32_t)id; it.d_t = pt; }
+    if (dir == 0) { it.s_pg = (uint32_t)id; it.s_t = pt; } else { it.d_pg = (uint32_t)id; it.d_t = pt; }
   }
   return it;
 }
@@ -498,20 +504,23 @@ __global__ void __launch_bounds__(kMaxWarps * 32, 1) kv_move_bulk(const __grid_c
       const uint32_t upr = j.drow >> 4;  // 16-byte units per head_dim row
       // tensor copies serve whole boxes only; ragged tails (and copy-on-write rows) take the lane paths
       const uint32_t box_bytes = j.tb * j.tokrow;
-      const uint8_t *maps_s = j.dir == 2 ? j.maps_src : (j.dir == 0 ? j.maps_pool : nullptr);
-      const uint8_t *maps_d = (j.dir == 1 || j.dir == 2) ? j.maps_pool : nullptr;
+      // (a mixed launch has one pool: whichever side of an item is strided is that pool; bit 2 of the mode keeps
+      // copy-on-write rows on the lane paths)
+      const uint8_t *maps_s = j.dir == 2 ? j.maps_src : ((j.dir == 0 || j.dir == 4) ? j.maps_pool : nullptr);
+      const uint8_t *maps_d = (j.dir == 1 || j.dir == 2 || j.dir == 4) ? j.maps_pool : nullptr;
       if (it >= depth && it - depth < n_known) {  // ---- store side: item si
         const uint64_t si = it - depth;
         const uint32_t s = (uint32_t)(si % K);
         mbar_wait(smem_u32(&full_bar[warp][s]), (uint32_t)(si / K) & 1);
         const StageMeta m = meta[warp][s];
         const uint32_t sbase = stage0 + s * j.stage_bytes;
-        if ((m.mode & 2) && maps_d && m.bytes == box_bytes && m.valid == box_bytes) {
-          // strided destination, whole box: one tensor store scatters the NHD stage into the HND page
-          if (lane == 0) {
-            asm volatile("fence.proxy.async.shared::cta;" ::: "memory");
-            tensor_s2g(maps_d + (size_t)m.lc * 128, m.d_t, m.d_pg, sbase);
-          }
+        if ((m.mode & 6) == 2 && maps_d && m.bytes == box_bytes && m.valid == box_bytes) {
+          // strided destination, whole box: one tensor store scatters the NHD stage into the HND page.
+          // The stage may have been written through the generic proxy (cp.async row gathers by all lanes): every
+          // writing lane fences its own writes into the async proxy before lane 0 issues the store.
+          asm volatile("fence.proxy.async.shared::cta;" ::: "memory");
+          __syncwarp();
+          if (lane == 0) tensor_s2g(maps_d + (size_t)m.lc * 128, m.d_t, m.d_pg, sbase);
         } else if (m.mode & 2) {  // strided destination: LDS.128 from the stage, STG.128 to the row's place
           const uint32_t nb = m.bytes >> 4, nv = m.valid >> 4;
           for (uint32_t u0 = lane; u0 < nb; u0 += 128) {
@@ -529,11 +538,16 @@ __global__ void __launch_bounds__(kMaxWarps * 32, 1) kv_move_bulk(const __grid_c
                 st_stream(reinterpret_cast<uint4 *>(trans_addr<16>(m.dst, true, m.r0, u, upr, j.H, st.d_ts, st.d_hs)), v[q]);
             }
           }
-        } else if (lane == 0) {
-          asm volatile("fence.proxy.async.shared::cta;" ::: "memory");  // rows gathered by cp.async -> bulk store
-          if (m.valid) bulk_s2g(m.dst, sbase, m.valid);
-          for (uint32_t z = m.valid; z < m.bytes; z += j.zero_bytes)
-            bulk_s2g(m.dst + z, zero0, min(j.zero_bytes, m.bytes - z));
+        } else {
+          // rows gathered by cp.async (generic proxy, all 32 lanes) -> bulk store (async proxy): the PTX memory model
+          // wants the WRITING threads' accesses fenced into the async proxy, so every lane fences, then the warp meets
+          asm volatile("fence.proxy.async.shared::cta;" ::: "memory");
+          __syncwarp();
+          if (lane == 0) {
+            if (m.valid) bulk_s2g(m.dst, sbase, m.valid);
+            for (uint32_t z = m.valid; z < m.bytes; z += j.zero_bytes)
+              bulk_s2g(m.dst + z, zero0, min(j.zero_bytes, m.bytes - z));
+          }
         }
         bulk_commit();  // every lane, every item: the per-thread group counts stay in step
       }
@@ -552,7 +566,7 @@ __global__ void __launch_bounds__(kMaxWarps * 32, 1) kv_move_bulk(const __grid_c
           m.dst = dst; m.bytes = bytes; m.valid = valid; m.mode = mode; m.r0 = r0;
           m.lc = lc; m.d_pg = d_pg; m.d_t = d_t;
         }
-        if ((mode & 1) && maps_s && bytes == box_bytes && valid == box_bytes) {
+        if ((mode & 5) == 1 && maps_s && bytes == box_bytes && valid == box_bytes) {
           // strided source, whole box: one tensor load gathers the HND page's rows in NHD order
           if (lane == 0) {
             mbar_expect_tx(bar, box_bytes);

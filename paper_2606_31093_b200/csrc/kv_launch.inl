@@ -13,16 +13,20 @@ struct HostBlob {
   size_t off_pieces = 0, off_ids = 0;
 };
 
-void build_blob(const kv_pool_desc *p, const Geom &g, const std::vector<Piece> &pieces,
-                const int32_t *ids, uint64_t n_ids, bool ids_on_device, HostBlob *hb) {
-  hb->off_pieces = (size_t)g.LC * 8 * (g.src_pool ? 2 : 1);
-  hb->off_ids = hb->off_pieces + pieces.size() * sizeof(Piece);
+// `pieces` / `n_pieces`: the pieces of the launch(es) the blob serves.  lc0 / lc_n: only the slab bases
+// [lc0, lc0 + lc_n) go in (a layer-range chunk of the staged pipeline with tables of its own); lc_n == 0: all.
+void build_blob(const kv_pool_desc *p, const Geom &g, const Piece *pieces, size_t n_pieces,
+                const int32_t *ids, uint64_t n_ids, bool ids_on_device, HostBlob *hb,
+                uint32_t lc0 = 0, uint32_t lc_n = 0) {
+  if (!lc_n) lc_n = g.LC;
+  hb->off_pieces = (size_t)lc_n * 8 * (g.src_pool ? 2 : 1);
+  hb->off_ids = hb->off_pieces + n_pieces * sizeof(Piece);
   hb->bytes.resize(hb->off_ids + (ids_on_device ? 0 : (size_t)n_ids * 4));
   uint8_t *h = hb->bytes.data();
-  for (uint32_t i = 0; i < g.LC; ++i) ((uint64_t *)h)[i] = (uint64_t)(uintptr_t)p->base[i];
+  for (uint32_t i = 0; i < lc_n; ++i) ((uint64_t *)h)[i] = (uint64_t)(uintptr_t)p->base[lc0 + i];
   if (g.src_pool)
-    for (uint32_t i = 0; i < g.LC; ++i) ((uint64_t *)h)[g.LC + i] = (uint64_t)(uintptr_t)g.src_pool->base[i];
-  std::memcpy(h + hb->off_pieces, pieces.data(), pieces.size() * sizeof(Piece));
+    for (uint32_t i = 0; i < lc_n; ++i) ((uint64_t *)h)[lc_n + i] = (uint64_t)(uintptr_t)g.src_pool->base[lc0 + i];
+  if (n_pieces) std::memcpy(h + hb->off_pieces, pieces, n_pieces * sizeof(Piece));
   if (!ids_on_device && n_ids) std::memcpy(h + hb->off_ids, ids, (size_t)n_ids * 4);
 }
 
@@ -62,6 +66,8 @@ int upload_blob(kv_ctx *ctx, const HostBlob &hb, const int32_t *ids, bool ids_on
   std::memcpy(slot.h, hb.bytes.data(), bytes);
   KV_CUDA(ctx, cudaMemcpyAsync(slot.d, slot.h, bytes, cudaMemcpyHostToDevice, s));
   ctx->memcpys++;
+  // From here on the slot is in flight.  Its event must be recorded behind the last reader on EVERY way out of the
+  // caller, failures included: BlobGuard (below) does that.
   slot.used = true;
   out->slot = &slot;
   out->d_bases = (const uint64_t *)slot.d;
@@ -69,6 +75,23 @@ int upload_blob(kv_ctx *ctx, const HostBlob &hb, const int32_t *ids, bool ids_on
   out->d_ids = ids_on_device ? ids : (const int32_t *)((uint8_t *)slot.d + hb.off_ids);
   return KV_OK;
 }
+
+// Records the slot's event on `s` when the caller's scope ends -- after the launches on the way out of a successful
+// call, and equally after a launch / tensor-map failure in between, so that the slot is never reused on the strength
+// of a stale or never-recorded event while its table copy or a kernel reading it may still be pending.
+struct BlobGuard {
+  kv_ctx *ctx; const Blob *b; cudaStream_t s;
+  BlobGuard(kv_ctx *c, const Blob *bl, cudaStream_t st) : ctx(c), b(bl), s(st) {}
+  ~BlobGuard() {
+    if (!b->slot) return;
+    if (cudaEventRecord(b->slot->ev, s) != cudaSuccess) {  // cannot order the slot's reuse behind its readers: drain them
+      (void)cudaGetLastError();
+      cudaStreamSynchronize(s);
+      (void)cudaGetLastError();
+      b->slot->used = false;
+    }
+  }
+};
 
 constexpr int kInlineSmall = 3840;   // whole parameter block stays under the classic 4 KiB
 constexpr int kInlineLarge = 31744;  // CUDA 12.1+ large kernel parameters (<= 32,764 B)
@@ -185,13 +208,13 @@ int launch(kv_ctx *ctx, const Geom &g, const Blob &b, uint32_t piece_first, uint
     const uint64_t want = (total_items + warps - 1) / warps;
     grid = (uint32_t)std::min<uint64_t>(want, cap ? cap : (uint32_t)ctx->sm_count);
     const uint64_t G = (uint64_t)grid * warps;
-    if (ctx->dynamic && total_items >= 8 * G && !capturing(s)) {  // enough work for claiming to pay
+    if (ctx->dynamic && total_items >= 8 * G && !ctx->cur_capturing) {  // enough work for claiming to pay
       uint8_t *slot = (uint8_t *)ctx->d_status + 256 + (size_t)(ctx->next_sched++ % kSchedSlots) * 16;
       j.sched = (unsigned long long *)slot;
       j.sched_done = (uint32_t *)(slot + 8);
       j.first_batch = (uint32_t)std::min<uint64_t>(32, total_items / (4 * G));
     }
-    const bool pdl = ctx->pdl && !capturing(s);
+    const bool pdl = ctx->pdl && !ctx->cur_capturing;
     if (!b.inl) launch_bulk<0>(j, nullptr, g.trans, grid, warps * 32, smem, s, pdl);
     else if (b.inl->bytes.size() <= kInlineSmall) launch_bulk<kInlineSmall>(j, b.inl, g.trans, grid, warps * 32, smem, s, pdl);
     else launch_bulk<kInlineLarge>(j, b.inl, g.trans, grid, warps * 32, smem, s, pdl);

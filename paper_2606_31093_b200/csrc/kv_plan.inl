@@ -221,6 +221,101 @@ int plan_cow(kv_ctx *ctx, const kv_pool_desc *pools, uint32_t layer_count, const
   return KV_OK;
 }
 
+// kv_submit: several independent pack / unpack / copy-on-write operations on one pool -> ONE launch in which the
+// direction is a property of the piece (Job::dir == 4, Piece::dir).  Page ids of all pack / unpack operations are
+// gathered into `all_ids` in operation order.
+int plan_submit(kv_ctx *ctx, const kv_pool_desc *pools, uint32_t layer_count, const kv_op *ops, uint32_t n_ops,
+                int layout, uint32_t flags, Call *c, std::vector<int32_t> *all_ids) {
+  if (!ctx) return KV_ERR_NULL;
+  int rc = check_desc(pools, layer_count);
+  if (rc) return rc;
+  if (flags & KV_FLAG_IDS_ON_DEVICE) return KV_ERR_LAYOUT;
+  if (n_ops && !ops) return KV_ERR_NULL;
+  const uint32_t T = pools->page_size;
+  const uint64_t tokrow = (uint64_t)pools->num_heads * pools->head_dim * pools->elem_bytes;
+  const uint64_t lc = (uint64_t)layer_count * pools->kv_count;
+  const uint64_t page = lc * T * tokrow;
+  c->reqs.clear();
+  all_ids->clear();
+  for (uint32_t i = 0; i < n_ops; ++i) {
+    const kv_op &op = ops[i];
+    Req q;
+    q.dir = op.kind;
+    if (op.kind == KV_OP_PACK || op.kind == KV_OP_UNPACK) {
+      const uint64_t n = op.n_pages;
+      if (op.kind == KV_OP_UNPACK) {
+        if (n != (op.n_tokens + T - 1) / T) return KV_ERR_SIZE;
+      }
+      if (!n) continue;
+      if (!op.page_ids || !op.buf) return KV_ERR_NULL;
+      if (op.buf_bytes && op.buf_bytes < n * page) return KV_ERR_SIZE;
+      rc = check_ids(op.page_ids, n, pools->num_pages);
+      if (rc) return rc;
+      q.buf = (uint64_t)(uintptr_t)op.buf;
+      q.n_tokens = op.kind == KV_OP_PACK ? n * T : op.n_tokens;
+      q.id_begin = all_ids->size(); q.n_ids = n; q.n_buf_pages = n;
+      all_ids->insert(all_ids->end(), op.page_ids, op.page_ids + n);
+    } else if (op.kind == KV_OP_COW_APPEND) {
+      if (!op.page_ids) return KV_ERR_NULL;
+      if ((uint64_t)op.n_old + op.n_app > T) return KV_ERR_SIZE;
+      const int32_t o = op.page_ids[0], nw = op.page_ids[1];
+      if (o == nw) return KV_ERR_SIZE;
+      if (o < 0 || nw < 0 || (uint32_t)o >= pools->num_pages || (uint32_t)nw >= pools->num_pages) return KV_ERR_PAGE_RANGE;
+      if (op.n_app && !op.buf) return KV_ERR_NULL;
+      if (!op.n_old && !op.n_app) continue;
+      q.buf = (uint64_t)(uintptr_t)op.buf;
+      q.n_tokens = (uint64_t)op.n_old | ((uint64_t)op.n_app << 32);
+      q.id_begin = (uint64_t)(uint32_t)o | ((uint64_t)(uint32_t)nw << 32);
+    } else {
+      return KV_ERR_LAYOUT;
+    }
+    c->reqs.push_back(q);
+  }
+  if (flags & KV_FLAG_VALIDATE) {  // written pages distinct; nothing read that the same call writes
+    std::vector<uint8_t> written((size_t)(pools->num_pages + 7) / 8, 0);
+    auto test = [&](uint32_t g) { return (written[g >> 3] >> (g & 7)) & 1u; };
+    for (const Req &q : c->reqs) {
+      if (q.dir == KV_OP_UNPACK) {
+        for (uint64_t k = 0; k < q.n_ids; ++k) {
+          const uint32_t g = (uint32_t)(*all_ids)[q.id_begin + k];
+          if (test(g)) return KV_ERR_DUP_PAGE;
+          written[g >> 3] |= (uint8_t)(1u << (g & 7));
+        }
+      } else if (q.dir == KV_OP_COW_APPEND) {
+        const uint32_t g = (uint32_t)(q.id_begin >> 32);
+        if (test(g)) return KV_ERR_DUP_PAGE;
+        written[g >> 3] |= (uint8_t)(1u << (g & 7));
+      }
+    }
+    for (const Req &q : c->reqs) {
+      if (q.dir == KV_OP_PACK) {
+        for (uint64_t k = 0; k < q.n_ids; ++k)
+          if (test((uint32_t)(*all_ids)[q.id_begin + k])) return KV_ERR_DUP_PAGE;
+      } else if (q.dir == KV_OP_COW_APPEND) {
+        if (test((uint32_t)q.id_begin)) return KV_ERR_DUP_PAGE;
+      }
+    }
+  }
+  c->n_ids = all_ids->size();
+  rc = make_geom(ctx, pools, layer_count, T, /*dir=*/4, layout, c->reqs, &c->geom);
+  if (rc) return rc;
+  c->total_items = 0; c->payload = 0;
+  const uint64_t sub = c->geom.sub_bytes;
+  for (Req &q : c->reqs) {
+    if (q.dir == KV_OP_COW_APPEND) {
+      const uint64_t b_old = (q.n_tokens & 0xffffffffull) * tokrow, b_app = (q.n_tokens >> 32) * tokrow;
+      q.items = lc * ((b_old + sub - 1) / sub + (b_app + sub - 1) / sub);
+      c->payload += lc * (b_old + b_app);
+    } else {
+      q.items = items_of(c->geom, q.n_ids);
+      c->payload += q.n_ids * page;
+    }
+    if (q.items > 0xFFFFFFFFull) return KV_ERR_SIZE;
+    c->total_items += q.items;
+  }
+  return KV_OK;
+}
+
 void note_plan(kv_ctx *ctx, const Call &c) {
   ctx->last_items = c.total_items;
   ctx->last_payload = c.payload;

@@ -12,32 +12,31 @@ int run_single_launch(kv_ctx *ctx, const kv_pool_desc *pools, const Call &c, con
   pieces.reserve(c.reqs.size());
   uint64_t acc = 0;
   for (const Req &q : c.reqs) {
-    Piece pc;
+    Piece pc{};
     pc.item_begin = acc; pc.buf = q.buf; pc.n_tokens = q.n_tokens; pc.id_begin = q.id_begin;
-    pc.n_buf_pages = q.n_buf_pages;
+    pc.n_buf_pages = q.n_buf_pages; pc.dir = q.dir;
     pieces.push_back(pc);
     acc += q.items;
   }
   const bool dev_ids = flags & KV_FLAG_IDS_ON_DEVICE;
   HostBlob hb;
-  build_blob(pools, c.geom, pieces, ids, c.n_ids, dev_ids, &hb);
+  build_blob(pools, c.geom, pieces.data(), pieces.size(), ids, c.n_ids, dev_ids, &hb);
   Blob b;
   if (ctx->inline_tables && c.geom.kernel != KERNEL_ELEM && hb.bytes.size() <= (size_t)kInlineLarge) {
     b.inl = &hb;  // tables travel inside the kernel parameters: one launch, no copy
     b.d_ids = dev_ids ? ids : nullptr;
     return launch(ctx, c.geom, b, 0, (uint32_t)pieces.size(), acc, cta_cap, s);
   }
-  if (capturing(s)) return KV_ERR_CAPTURE;
+  if (ctx->cur_capturing) return KV_ERR_CAPTURE;
   int rc = upload_blob(ctx, hb, ids, dev_ids, s, &b);
   if (rc) return rc;
-  rc = launch(ctx, c.geom, b, 0, (uint32_t)pieces.size(), acc, cta_cap, s);
-  if (rc) return rc;
-  KV_CUDA(ctx, cudaEventRecord(b.slot->ev, s));
-  return KV_OK;
+  BlobGuard guard(ctx, &b, s);  // records the slot's event behind the launch, on every way out
+  return launch(ctx, c.geom, b, 0, (uint32_t)pieces.size(), acc, cta_cap, s);
 }
 
 int ensure_staging(kv_ctx *ctx) {
   if (ctx->staging) return KV_OK;
+  if (ctx->cur_capturing) return KV_ERR_CAPTURE;  // an allocation would invalidate the capture: reserve the staging first
   if (!ctx->staging_bytes) ctx->staging_bytes = (size_t)512 << 20;  // 256 MiB chunks: measured best with both link directions busy
   KV_CUDA(ctx, cudaMalloc(&ctx->staging, ctx->staging_bytes));
   return KV_OK;
@@ -58,11 +57,17 @@ int run_staged(kv_ctx *ctx, const kv_pool_desc *pools, const Call &c, const int3
   if (rc) return rc;
   const Geom &g = c.geom;
   const uint32_t n_slots = ctx->staging_slots;
+  const bool cap = ctx->cur_capturing;
+  const bool dev_ids = flags & KV_FLAG_IDS_ON_DEVICE;
   // unit of chunking: tokens that are whole pages on both sides
   const uint64_t unit_tokens = (uint64_t)g.Tpool / g.g * g.Tbuf;  // lcm(Tpool, Tbuf)
   const bool layer_first = g.layout == KV_LAYOUT_LAYER_FIRST;
   const uint64_t unit_bytes = unit_tokens * g.tokrow * (layer_first ? g.C : g.LC);
-  size_t slot_bytes = ctx->staging_bytes / n_slots / 256 * 256;
+  // slot i = staging + i * slot_pitch for EVERY call of this ctx; slot_bytes (what a chunk of THIS call may fill) is a
+  // prefix of it.  The per-slot events thus guard the same bytes whatever the chunk size of the call that recorded them
+  // and whatever stream it ran on (two staged calls of one ctx on two streams share the slots safely).
+  const size_t slot_pitch = ctx->staging_bytes / n_slots / 256 * 256;
+  size_t slot_bytes = slot_pitch;
   if (ctx->chunk_bytes) slot_bytes = std::min(slot_bytes, ctx->chunk_bytes / 256 * 256);
   // Equal chunks: at least three per transfer where that leaves >= 64 MiB each (only the first chunk's kernel of an
   // offload, or the last one's of a reload, is not hidden behind a copy), as many as the slot size demands, and the
@@ -87,7 +92,7 @@ int run_staged(kv_ctx *ctx, const kv_pool_desc *pools, const Call &c, const int3
   // A chunk = what one staging slot holds: pieces for the kernel, copies for the copy engine.  Page-first:
   // a run of whole pages, all layers (contiguous in the host buffer).  Layer-first: a range of layers
   // [l0, l0 + nl) of one or more page ranges; every (layer, K|V) of a page range is one contiguous host run.
-  struct Chunk { uint32_t piece_first, n_pieces; uint64_t items; uint32_t l0, nl, sig_n; };
+  struct Chunk { uint32_t piece_first, n_pieces; uint64_t items; uint32_t l0, nl, sig_n; uint64_t id_lo = ~0ull, id_hi = 0; };
   // rows > 1: a strided copy of `rows` runs of `bytes` each, host_pitch apart in the host buffer and dense in the
   // slot (the (layer, K|V) runs of a layer-first page range): ONE 2-D copy-engine transfer instead of `rows`
   struct Copy { uint64_t host, dev_off, bytes; uint64_t rows = 1, host_pitch = 0; };
@@ -123,7 +128,7 @@ int run_staged(kv_ctx *ctx, const kv_pool_desc *pools, const Call &c, const int3
           const uint64_t b1 = std::min((t1 + g.Tbuf - 1) / g.Tbuf, q.n_buf_pages);
           const uint64_t nb = b1 - b0, region = nb * per_buf_page;
           if (fill + region > slot_bytes) close();
-          Piece pc;
+          Piece pc{};
           pc.item_begin = cur.items;
           pc.buf = fill;  // offset within the slot; the slot base is added below
           pc.n_tokens = q.n_tokens > t0 ? std::min(q.n_tokens - t0, t1 - t0) : 0;
@@ -131,6 +136,7 @@ int run_staged(kv_ctx *ctx, const kv_pool_desc *pools, const Call &c, const int3
           pc.n_buf_pages = nb;
           pieces.push_back(pc);
           cur.n_pieces++;
+          cur.id_lo = std::min(cur.id_lo, pc.id_begin); cur.id_hi = std::max(cur.id_hi, pc.id_begin + (q1 - q0));
           cur.items += (q1 - q0) * (g.Tpool / g.g) * nl * g.C * g.subs;
           if (nb) {
             const uint64_t pitch = q.n_buf_pages * row;  // host bytes between consecutive (layer, K|V) runs
@@ -171,15 +177,15 @@ int run_staged(kv_ctx *ctx, const kv_pool_desc *pools, const Call &c, const int3
         const uint64_t span = t1 - t0;  // multiple of Tpool; multiple of unit except at the request's end
         const uint64_t buf_pages = (std::min(t1, q.n_buf_pages * g.Tbuf) - std::min(t0, q.n_buf_pages * g.Tbuf) + g.Tbuf - 1) / g.Tbuf;
         const uint64_t dev_off = fill_tokens * g.tokrow * g.LC;
-        Piece pc;
+        Piece pc{};
         pc.item_begin = cur.items;
-        pc.buf = (uint64_t)(uintptr_t)ctx->staging;  // + slot base, patched per chunk below
-        pc.buf = dev_off;                              // offset within the slot for now
+        pc.buf = dev_off;  // offset within the slot; the slot base is added below
         pc.n_tokens = q.n_tokens > t0 ? std::min(q.n_tokens - t0, span) : 0;
         pc.id_begin = q.id_begin + t0 / g.Tpool;
         pc.n_buf_pages = buf_pages;
         pieces.push_back(pc);
         cur.n_pieces++;
+        cur.id_lo = std::min(cur.id_lo, pc.id_begin); cur.id_hi = std::max(cur.id_hi, pc.id_begin + span / g.Tpool);
         cur.items += items_of(g, span / g.Tpool);
         if (buf_pages)
           cur_copies.push_back(Copy{q.buf + t0 / g.Tbuf * g.buf_page, dev_off, buf_pages * g.buf_page});
@@ -192,26 +198,66 @@ int run_staged(kv_ctx *ctx, const kv_pool_desc *pools, const Call &c, const int3
   }
   // patch slot bases
   for (size_t ci = 0; ci < chunks.size(); ++ci) {
-    const uint64_t base = (uint64_t)(uintptr_t)ctx->staging + (ci % n_slots) * slot_bytes;
+    const uint64_t base = (uint64_t)(uintptr_t)ctx->staging + (ci % n_slots) * slot_pitch;
     for (uint32_t k = 0; k < chunks[ci].n_pieces; ++k) pieces[chunks[ci].piece_first + k].buf += base;
   }
-  HostBlob hb;
-  build_blob(pools, g, pieces, ids, c.n_ids, flags & KV_FLAG_IDS_ON_DEVICE, &hb);
-  Blob b;
-  rc = upload_blob(ctx, hb, ids, flags & KV_FLAG_IDS_ON_DEVICE, s, &b);
-  if (rc) return rc;
-  KV_CUDA(ctx, cudaEventRecord(ctx->ev_entry, s));
-  KV_CUDA(ctx, cudaStreamWaitEvent(ctx->side, ctx->ev_entry, 0));
+  // Tables.  A chunk's launch needs its slab bases, its pieces and ITS page ids (a contiguous range of the call's id
+  // array): a few hundred bytes at the paper's shapes (a 256 MiB chunk of the Qwen3-Omni pool is 170 pages), so each
+  // chunk launch carries them inside its kernel parameters -- no table copy, no pinned ring, and therefore nothing
+  // that a CUDA graph could not replay.  Only calls with a chunk whose tables exceed the parameter space (tens of
+  // thousands of tiny pages per chunk) stage ONE blob for all chunks through the pinned ring; those cannot be captured.
+  const bool layer_range = layer_first;  // layer-first chunks launch over a slab range [l0*C, (l0+nl)*C)
+  bool inline_ok = ctx->inline_tables && g.kernel != KERNEL_ELEM;
+  for (const Chunk &ch : chunks) {
+    const size_t need = (size_t)(layer_range ? ch.nl * g.C : g.LC) * 8 + (size_t)ch.n_pieces * sizeof(Piece) +
+                        (dev_ids ? 0 : (size_t)(ch.id_hi - ch.id_lo) * 4);
+    if (need > (size_t)kInlineLarge) inline_ok = false;
+  }
+  if (cap && !inline_ok) return KV_ERR_CAPTURE;
+  Blob shared;  // the one staged blob of the fallback
+  HostBlob hb_all;
+  if (!inline_ok) {
+    build_blob(pools, g, pieces.data(), pieces.size(), ids, c.n_ids, dev_ids, &hb_all);
+    rc = upload_blob(ctx, hb_all, ids, dev_ids, s, &shared);
+    if (rc) return rc;
+  }
+  BlobGuard guard(ctx, &shared, s);  // no-op for inline tables
+  HostBlob hb_chunk;
+  std::vector<Piece> chunk_pieces;
+  auto launch_chunk = [&](const Chunk &ch) -> int {
+    if (!inline_ok)
+      return launch(ctx, g, shared, ch.piece_first, ch.n_pieces, ch.items, 0, s, ch.l0 * g.C, ch.nl * g.C);
+    chunk_pieces.assign(pieces.begin() + ch.piece_first, pieces.begin() + ch.piece_first + ch.n_pieces);
+    if (!dev_ids)
+      for (Piece &pc : chunk_pieces) pc.id_begin -= ch.id_lo;  // ids of the chunk start at 0 in its own table
+    build_blob(pools, g, chunk_pieces.data(), chunk_pieces.size(), dev_ids ? nullptr : ids + ch.id_lo,
+               dev_ids ? 0 : ch.id_hi - ch.id_lo, dev_ids, &hb_chunk, layer_range ? ch.l0 * g.C : 0,
+               layer_range ? ch.nl * g.C : 0);
+    Blob b;
+    b.inl = &hb_chunk;
+    b.d_ids = dev_ids ? ids : nullptr;
+    return launch(ctx, g, b, 0, ch.n_pieces, ch.items, 0, s, ch.l0 * g.C, ch.nl * g.C);
+  };
+  // Events.  Eager calls order slot reuse across calls with the ctx's per-slot events.  Inside a capture the same
+  // fork / join pattern is recorded with events of its own (a captured record is an edge of the graph, not a real
+  // record), and there is no earlier call to wait for: a replayed graph is ordered against other work of the ctx by
+  // the stream it is launched on (kvtier.h "CUDA graphs").
+  cudaEvent_t ev_entry = cap ? ctx->cap_entry : ctx->ev_entry;
+  cudaEvent_t *ev_full = cap ? ctx->cap_full : ctx->ev_full;
+  cudaEvent_t *ev_free = cap ? ctx->cap_free : ctx->ev_free;
+  std::vector<uint8_t> cap_used(kMaxStagingSlots, 0);  // capture: slots this call has already been through
+  KV_CUDA(ctx, cudaEventRecord(ev_entry, s));
+  KV_CUDA(ctx, cudaStreamWaitEvent(ctx->side, ev_entry, 0));
   for (size_t ci = 0; ci < chunks.size(); ++ci) {
     const uint32_t slot = (uint32_t)(ci % n_slots);
-    uint8_t *slot_base = (uint8_t *)ctx->staging + (size_t)slot * slot_bytes;
+    uint8_t *slot_base = (uint8_t *)ctx->staging + (size_t)slot * slot_pitch;
+    const bool wait_free = cap ? cap_used[slot] != 0 : ctx->free_valid[slot];
     if (g.dir == 0) {  // offload: kernel fills the slot on s, copy engine drains it on side
-      if (ctx->free_valid[slot]) KV_CUDA(ctx, cudaStreamWaitEvent(s, ctx->ev_free[slot], 0));
-      rc = launch(ctx, g, b, chunks[ci].piece_first, chunks[ci].n_pieces, chunks[ci].items, 0, s,
-                  chunks[ci].l0 * g.C, chunks[ci].nl * g.C);
+      if (wait_free) KV_CUDA(ctx, cudaStreamWaitEvent(s, ev_free[slot], 0));
+      rc = launch_chunk(chunks[ci]);
       if (rc) return rc;
-      KV_CUDA(ctx, cudaEventRecord(ctx->ev_full[slot], s));
-      KV_CUDA(ctx, cudaStreamWaitEvent(ctx->side, ctx->ev_full[slot], 0));
+      KV_CUDA(ctx, cudaEventRecord(ev_full[slot], s));
+      KV_CUDA(ctx, cudaStreamWaitEvent(ctx->side, ev_full[slot], 0));
       for (const Copy &cp : copies[ci]) {
         if (cp.rows > 1)
           KV_CUDA(ctx, cudaMemcpy2DAsync((void *)(uintptr_t)cp.host, cp.host_pitch, slot_base + cp.dev_off, cp.bytes,
@@ -221,10 +267,9 @@ int run_staged(kv_ctx *ctx, const kv_pool_desc *pools, const Call &c, const int3
                                        cudaMemcpyDeviceToHost, ctx->side));
         ctx->memcpys++;
       }
-      KV_CUDA(ctx, cudaEventRecord(ctx->ev_free[slot], ctx->side));
-      ctx->free_valid[slot] = true;
+      KV_CUDA(ctx, cudaEventRecord(ev_free[slot], ctx->side));
     } else {  // reload: copy engine fills the slot on side, kernel drains it on s
-      if (ctx->free_valid[slot]) KV_CUDA(ctx, cudaStreamWaitEvent(ctx->side, ctx->ev_free[slot], 0));
+      if (wait_free) KV_CUDA(ctx, cudaStreamWaitEvent(ctx->side, ev_free[slot], 0));
       for (const Copy &cp : copies[ci]) {
         if (cp.rows > 1)
           KV_CUDA(ctx, cudaMemcpy2DAsync(slot_base + cp.dev_off, cp.bytes, (const void *)(uintptr_t)cp.host,
@@ -234,26 +279,24 @@ int run_staged(kv_ctx *ctx, const kv_pool_desc *pools, const Call &c, const int3
                                        cp.bytes, cudaMemcpyHostToDevice, ctx->side));
         ctx->memcpys++;
       }
-      KV_CUDA(ctx, cudaEventRecord(ctx->ev_full[slot], ctx->side));
-      KV_CUDA(ctx, cudaStreamWaitEvent(s, ctx->ev_full[slot], 0));
-      rc = launch(ctx, g, b, chunks[ci].piece_first, chunks[ci].n_pieces, chunks[ci].items, 0, s,
-                  chunks[ci].l0 * g.C, chunks[ci].nl * g.C);
+      KV_CUDA(ctx, cudaEventRecord(ev_full[slot], ctx->side));
+      KV_CUDA(ctx, cudaStreamWaitEvent(s, ev_full[slot], 0));
+      rc = launch_chunk(chunks[ci]);
       if (rc) return rc;
       if (lf.flags && chunks[ci].sig_n) {  // these layers' pages are in the pool: publish
         kvt::kv_signal_range<<<1, 32, 0, s>>>(lf.flags + chunks[ci].l0, chunks[ci].sig_n, lf.value);  // strides over > 32
         KV_CUDA(ctx, cudaGetLastError());
         ctx->launches++;
       }
-      KV_CUDA(ctx, cudaEventRecord(ctx->ev_free[slot], s));
-      ctx->free_valid[slot] = true;
+      KV_CUDA(ctx, cudaEventRecord(ev_free[slot], s));
     }
+    if (cap) cap_used[slot] = 1; else ctx->free_valid[slot] = true;
   }
   if (g.dir == 0) {  // join the copy engine's tail back into s
     const size_t first = chunks.size() > n_slots ? chunks.size() - n_slots : 0;
     for (size_t ci = first; ci < chunks.size(); ++ci)
-      KV_CUDA(ctx, cudaStreamWaitEvent(s, ctx->ev_free[ci % n_slots], 0));
+      KV_CUDA(ctx, cudaStreamWaitEvent(s, ev_free[ci % n_slots], 0));
   }
-  KV_CUDA(ctx, cudaEventRecord(b.slot->ev, s));
   return KV_OK;
 }
 
@@ -304,32 +347,35 @@ int run_host(kv_ctx *ctx, const kv_pool_desc *pools, Call &c, const int32_t *ids
   if (c.reqs.empty()) return KV_OK;  // n == 0: nothing to do, no launch
   if (ctx->host_only) return KV_ERR_NO_DEVICE;
   DeviceGuard guard(ctx);
-  if (capturing(s)) {  // the chunk pipeline (side stream, staging slots, table upload) is not replayable
-    if (mode == KV_HOST_STAGED) return KV_ERR_CAPTURE;
-    m = KV_HOST_DIRECT;
-    ctx->last_mode = (uint64_t)m;
-  }
-  for (Req &q : c.reqs) {
-    uint64_t alias = 0;
-    rc = host_alias(ctx, (const void *)(uintptr_t)q.buf, &alias);
+  std::vector<uint64_t> alias(c.reqs.size());
+  for (size_t i = 0; i < c.reqs.size(); ++i) {
+    rc = host_alias(ctx, (const void *)(uintptr_t)c.reqs[i].buf, &alias[i]);
     if (rc) return rc;
-    if (m == KV_HOST_DIRECT) q.buf = alias;
   }
   if (lf.flags) {
     rc = flag_alias(lf.flags, &lf.flags);
     if (rc) return rc;
   }
-  if (m == KV_HOST_DIRECT) {  // one launch moves every layer: the flags follow it together
-    rc = run_single_launch(ctx, pools, c, ids, flags, ctx->host_max_ctas, s);
-    if (rc || !lf.flags) return rc;
-    for (uint32_t l0 = 0; l0 < c.geom.L; l0 += 32) {
-      kvt::kv_signal_range<<<1, 32, 0, s>>>(lf.flags + l0, std::min(32u, c.geom.L - l0), lf.value);
-      KV_CUDA(ctx, cudaGetLastError());
-      ctx->launches++;
-    }
-    return KV_OK;
+  if (m == KV_HOST_STAGED) {
+    // The chunk pipeline is copies, events and kernels with their tables in the kernel parameters: all of it can be
+    // captured into a CUDA graph.  What cannot: allocating the staging during the capture (reserve it first:
+    // KV_OPT_RESERVE_STAGING, or any earlier staged call) and tables too large for the parameters.  Then an explicit
+    // KV_HOST_STAGED is KV_ERR_CAPTURE and KV_HOST_AUTO takes DIRECT, as it did before staged transfers were capturable.
+    rc = run_staged(ctx, pools, c, ids, flags, s, lf);
+    if (!(rc == KV_ERR_CAPTURE && mode == KV_HOST_AUTO)) return rc;
+    m = KV_HOST_DIRECT;
+    ctx->last_mode = (uint64_t)m;
   }
-  return run_staged(ctx, pools, c, ids, flags, s, lf);
+  // DIRECT: one launch moves every layer (the flags follow it together)
+  for (size_t i = 0; i < c.reqs.size(); ++i) c.reqs[i].buf = alias[i];
+  rc = run_single_launch(ctx, pools, c, ids, flags, ctx->host_max_ctas, s);
+  if (rc || !lf.flags) return rc;
+  for (uint32_t l0 = 0; l0 < c.geom.L; l0 += 32) {
+    kvt::kv_signal_range<<<1, 32, 0, s>>>(lf.flags + l0, std::min(32u, c.geom.L - l0), lf.value);
+    KV_CUDA(ctx, cudaGetLastError());
+    ctx->launches++;
+  }
+  return KV_OK;
 }
 
 int run_device(kv_ctx *ctx, const kv_pool_desc *pools, const Call &c, const int32_t *ids,

@@ -49,6 +49,71 @@ const char *kv_strerror(int status) {
   }
 }
 
+}  // extern "C"
+
+namespace {
+// Frees everything a ctx owns on its device; null-safe member by member, so it also serves a ctx whose creation
+// stopped half way.  The caller has made the ctx's device current.
+void ctx_release(kv_ctx *ctx) {
+  if (ctx->side) cudaStreamSynchronize(ctx->side);
+  for (auto &b : ctx->blobs) {
+    if (b.used && b.ev) cudaEventSynchronize(b.ev);
+    if (b.ev) cudaEventDestroy(b.ev);
+  }
+  for (int i = 0; i < kMaxStagingSlots; ++i) {
+    if (ctx->ev_full[i]) cudaEventDestroy(ctx->ev_full[i]);
+    if (ctx->ev_free[i]) { if (ctx->free_valid[i]) cudaEventSynchronize(ctx->ev_free[i]); cudaEventDestroy(ctx->ev_free[i]); }
+    if (ctx->cap_full[i]) cudaEventDestroy(ctx->cap_full[i]);
+    if (ctx->cap_free[i]) cudaEventDestroy(ctx->cap_free[i]);
+  }
+  if (ctx->blob_arena_h) cudaFreeHost(ctx->blob_arena_h);
+  if (ctx->blob_arena_d) cudaFree(ctx->blob_arena_d);
+  if (ctx->staging) cudaFree(ctx->staging);
+  for (MapSet &m : ctx->map_sets) cudaFree(m.d);
+  if (ctx->d_status) cudaFree(ctx->d_status);
+  if (ctx->ev_entry) cudaEventDestroy(ctx->ev_entry);
+  if (ctx->cap_entry) cudaEventDestroy(ctx->cap_entry);
+  if (ctx->side) cudaStreamDestroy(ctx->side);
+  (void)cudaGetLastError();
+}
+
+cudaError_t ctx_init_device(kv_ctx *ctx, int device) {
+  cudaError_t e;
+  if ((e = cudaDeviceGetAttribute(&ctx->sm_count, cudaDevAttrMultiProcessorCount, device)) != cudaSuccess) return e;
+  if ((e = cudaDeviceGetAttribute(&ctx->max_smem, cudaDevAttrMaxSharedMemoryPerBlockOptin, device)) != cudaSuccess) return e;
+  const void *bulk_kernels[] = {(const void *)kvt::kv_move_bulk<0, false>, (const void *)kvt::kv_move_bulk<kInlineSmall, false>,
+                                (const void *)kvt::kv_move_bulk<kInlineLarge, false>, (const void *)kvt::kv_move_bulk<0, true>,
+                                (const void *)kvt::kv_move_bulk<kInlineSmall, true>, (const void *)kvt::kv_move_bulk<kInlineLarge, true>};
+  for (const void *k : bulk_kernels)
+    if ((e = cudaFuncSetAttribute(k, cudaFuncAttributeMaxDynamicSharedMemorySize, ctx->max_smem - kStaticSmemReserve)) != cudaSuccess) return e;
+  {  // cuTensorMapEncodeTiled without linking libcuda; absent -> HND pools keep to the lane paths
+    void *fn = nullptr;
+    cudaDriverEntryPointQueryResult qr = cudaDriverEntryPointSymbolNotFound;
+    if (cudaGetDriverEntryPoint("cuTensorMapEncodeTiled", &fn, cudaEnableDefault, &qr) == cudaSuccess &&
+        qr == cudaDriverEntryPointSuccess)
+      ctx->encode_tiled = (EncodeTiledFn)fn;
+    else
+      (void)cudaGetLastError();
+  }
+  if ((e = cudaStreamCreateWithFlags(&ctx->side, cudaStreamNonBlocking)) != cudaSuccess) return e;
+  if ((e = cudaEventCreateWithFlags(&ctx->ev_entry, cudaEventDisableTiming)) != cudaSuccess) return e;
+  if ((e = cudaEventCreateWithFlags(&ctx->cap_entry, cudaEventDisableTiming)) != cudaSuccess) return e;
+  for (int i = 0; i < kBlobSlots; ++i)
+    if ((e = cudaEventCreateWithFlags(&ctx->blobs[i].ev, cudaEventDisableTiming)) != cudaSuccess) return e;
+  for (int i = 0; i < kMaxStagingSlots; ++i) {
+    if ((e = cudaEventCreateWithFlags(&ctx->ev_full[i], cudaEventDisableTiming)) != cudaSuccess) return e;
+    if ((e = cudaEventCreateWithFlags(&ctx->ev_free[i], cudaEventDisableTiming)) != cudaSuccess) return e;
+    if ((e = cudaEventCreateWithFlags(&ctx->cap_full[i], cudaEventDisableTiming)) != cudaSuccess) return e;
+    if ((e = cudaEventCreateWithFlags(&ctx->cap_free[i], cudaEventDisableTiming)) != cudaSuccess) return e;
+  }
+  if ((e = cudaMalloc((void **)&ctx->d_status, 256 + kSchedSlots * 16)) != cudaSuccess) return e;
+  if ((e = cudaMemset(ctx->d_status, 0, 256 + kSchedSlots * 16)) != cudaSuccess) return e;
+  return cudaSuccess;
+}
+}  // namespace
+
+extern "C" {
+
 int kv_ctx_create(kv_ctx **out, int device, size_t staging_bytes) {
   if (!out) return KV_ERR_NULL;
   *out = nullptr;
@@ -62,43 +127,19 @@ int kv_ctx_create(kv_ctx **out, int device, size_t staging_bytes) {
     return KV_OK;
   }
   ctx->device = device;
-  auto fail = [&](cudaError_t e) {
-    (void)e;
+  int prev = -1;
+  cudaError_t e = cudaGetDevice(&prev);
+  if (e == cudaSuccess) e = cudaSetDevice(device);
+  if (e == cudaSuccess) {
+    e = ctx_init_device(ctx, device);
+    if (e != cudaSuccess) ctx_release(ctx);  // same teardown as kv_ctx_destroy: nothing created so far leaks
+  }
+  if (prev >= 0 && prev != device) cudaSetDevice(prev);  // the caller's current device is restored on EVERY way out
+  if (e != cudaSuccess) {
     (void)cudaGetLastError();
     delete ctx;
     return KV_ERR_CUDA;
-  };
-  cudaError_t e;
-  int prev = -1;
-  if ((e = cudaGetDevice(&prev)) != cudaSuccess) return fail(e);
-  if ((e = cudaSetDevice(device)) != cudaSuccess) return fail(e);
-  if ((e = cudaDeviceGetAttribute(&ctx->sm_count, cudaDevAttrMultiProcessorCount, device)) != cudaSuccess) return fail(e);
-  if ((e = cudaDeviceGetAttribute(&ctx->max_smem, cudaDevAttrMaxSharedMemoryPerBlockOptin, device)) != cudaSuccess) return fail(e);
-  const void *bulk_kernels[] = {(const void *)kvt::kv_move_bulk<0, false>, (const void *)kvt::kv_move_bulk<kInlineSmall, false>,
-                                (const void *)kvt::kv_move_bulk<kInlineLarge, false>, (const void *)kvt::kv_move_bulk<0, true>,
-                                (const void *)kvt::kv_move_bulk<kInlineSmall, true>, (const void *)kvt::kv_move_bulk<kInlineLarge, true>};
-  for (const void *k : bulk_kernels)
-    if ((e = cudaFuncSetAttribute(k, cudaFuncAttributeMaxDynamicSharedMemorySize, ctx->max_smem - kStaticSmemReserve)) != cudaSuccess) return fail(e);
-  {  // cuTensorMapEncodeTiled without linking libcuda; absent -> HND pools keep to the lane paths
-    void *fn = nullptr;
-    cudaDriverEntryPointQueryResult qr = cudaDriverEntryPointSymbolNotFound;
-    if (cudaGetDriverEntryPoint("cuTensorMapEncodeTiled", &fn, cudaEnableDefault, &qr) == cudaSuccess &&
-        qr == cudaDriverEntryPointSuccess)
-      ctx->encode_tiled = (EncodeTiledFn)fn;
-    else
-      (void)cudaGetLastError();
   }
-  if ((e = cudaStreamCreateWithFlags(&ctx->side, cudaStreamNonBlocking)) != cudaSuccess) return fail(e);
-  if ((e = cudaEventCreateWithFlags(&ctx->ev_entry, cudaEventDisableTiming)) != cudaSuccess) return fail(e);
-  for (int i = 0; i < kBlobSlots; ++i)
-    if ((e = cudaEventCreateWithFlags(&ctx->blobs[i].ev, cudaEventDisableTiming)) != cudaSuccess) return fail(e);
-  for (int i = 0; i < kMaxStagingSlots; ++i) {
-    if ((e = cudaEventCreateWithFlags(&ctx->ev_full[i], cudaEventDisableTiming)) != cudaSuccess) return fail(e);
-    if ((e = cudaEventCreateWithFlags(&ctx->ev_free[i], cudaEventDisableTiming)) != cudaSuccess) return fail(e);
-  }
-  if ((e = cudaMalloc((void **)&ctx->d_status, 256 + kSchedSlots * 16)) != cudaSuccess) return fail(e);
-  if ((e = cudaMemset(ctx->d_status, 0, 256 + kSchedSlots * 16)) != cudaSuccess) return fail(e);
-  if (prev >= 0 && prev != device) cudaSetDevice(prev);
   *out = ctx;
   return KV_OK;
 }
@@ -107,23 +148,7 @@ int kv_ctx_destroy(kv_ctx *ctx) {
   if (!ctx) return KV_ERR_NULL;
   if (!ctx->host_only) {
     DeviceGuard guard(ctx);
-    cudaStreamSynchronize(ctx->side);
-    for (auto &b : ctx->blobs) {
-      if (b.used) cudaEventSynchronize(b.ev);
-      if (b.ev) cudaEventDestroy(b.ev);
-    }
-    for (int i = 0; i < kMaxStagingSlots; ++i) {
-      if (ctx->ev_full[i]) cudaEventDestroy(ctx->ev_full[i]);
-      if (ctx->ev_free[i]) { cudaEventSynchronize(ctx->ev_free[i]); cudaEventDestroy(ctx->ev_free[i]); }
-    }
-    if (ctx->blob_arena_h) cudaFreeHost(ctx->blob_arena_h);
-    if (ctx->blob_arena_d) cudaFree(ctx->blob_arena_d);
-    if (ctx->staging) cudaFree(ctx->staging);
-    for (MapSet &m : ctx->map_sets) cudaFree(m.d);
-    if (ctx->d_status) cudaFree(ctx->d_status);
-    if (ctx->ev_entry) cudaEventDestroy(ctx->ev_entry);
-    if (ctx->side) cudaStreamDestroy(ctx->side);
-    (void)cudaGetLastError();
+    ctx_release(ctx);
   }
   delete ctx;
   return KV_OK;
@@ -140,12 +165,30 @@ int kv_ctx_set_option(kv_ctx *ctx, int option, int64_t v) {
     case KV_OPT_MAX_CTAS: if (v < 0 || v > 65535) return KV_ERR_SIZE; ctx->max_ctas = (uint32_t)v; break;
     case KV_OPT_CHUNK_BYTES: if (v < 0) return KV_ERR_SIZE; ctx->chunk_bytes = (size_t)v; break;
     case KV_OPT_HOST_MAX_CTAS: if (v < 0 || v > 65535) return KV_ERR_SIZE; ctx->host_max_ctas = (uint32_t)v; break;
-    case KV_OPT_STAGING_SLOTS: if (v < 2 || v > kMaxStagingSlots) return KV_ERR_SIZE; ctx->staging_slots = (uint32_t)v; break;
+    case KV_OPT_STAGING_SLOTS:
+      if (v < 2 || v > kMaxStagingSlots) return KV_ERR_SIZE;
+      if ((uint32_t)v != ctx->staging_slots && !ctx->host_only) {
+        // the slots move: nothing may still be using the old ones when the next staged call cuts the buffer anew
+        DeviceGuard guard(ctx);
+        for (int i = 0; i < kMaxStagingSlots; ++i)
+          if (ctx->free_valid[i]) { KV_CUDA(ctx, cudaEventSynchronize(ctx->ev_free[i])); ctx->free_valid[i] = false; }
+      }
+      ctx->staging_slots = (uint32_t)v;
+      break;
     case KV_OPT_L2_HINT: if (v < 0 || v > 1) return KV_ERR_SIZE; ctx->l2_hint = (uint32_t)v; break;
     case KV_OPT_INLINE_TABLES: if (v < 0 || v > 1) return KV_ERR_SIZE; ctx->inline_tables = (uint32_t)v; break;
     case KV_OPT_DYNAMIC: if (v < 0 || v > 1) return KV_ERR_SIZE; ctx->dynamic = (uint32_t)v; break;
     case KV_OPT_TENSOR_MAPS: if (v < 0 || v > 1) return KV_ERR_SIZE; ctx->tensor_maps = (uint32_t)v; break;
     case KV_OPT_PDL: if (v < 0 || v > 1) return KV_ERR_SIZE; ctx->pdl = (uint32_t)v; break;
+    case KV_OPT_RESERVE_STAGING: {
+      if (v < 0) return KV_ERR_SIZE;
+      if (ctx->host_only) return KV_ERR_NO_DEVICE;
+      if (ctx->staging) return (v == 0 || (size_t)v == ctx->staging_bytes) ? KV_OK : KV_ERR_SIZE;
+      if (v) ctx->staging_bytes = (size_t)v;
+      DeviceGuard guard(ctx);
+      ctx->cur_capturing = false;
+      return ensure_staging(ctx);
+    }
     default: return KV_ERR_LAYOUT;
   }
   return KV_OK;
@@ -248,15 +291,17 @@ int kv_chain_hash(kv_ctx *ctx, const uint64_t *ident, const int64_t *tok_offsets
     std::memcpy(pi.tok_off, tok_offsets, n1 * 8);
     std::memcpy(pi.page_off, poff.data(), n1 * 8);
     if (roots) std::memcpy(pi.roots, roots, (size_t)n_sessions * 8);
-    kvt::kv_chain_digest<true><<<(uint32_t)blocks, 128, 0, s>>>(pi);
+    // one launch: a CTA per session digests its pages and then walks its chain (kv_chain.cuh)
+    int64_t longest = 1;
+    for (uint32_t q = 0; q < n_sessions; ++q) longest = std::max(longest, poff[q + 1] - poff[q]);
+    const uint32_t threads = (uint32_t)std::min<int64_t>(1024, (longest + 31) / 32 * 32);
+    kvt::kv_chain_fused<true><<<n_sessions, threads, 0, s>>>(pi);
     KV_CUDA(ctx, cudaGetLastError());
-    kvt::kv_chain_link<true><<<n_sessions, 32, 0, s>>>(pi);
-    KV_CUDA(ctx, cudaGetLastError());
-    ctx->launches += 2;
+    ctx->launches += 1;
     return KV_OK;
   }
   if (capturing(s)) return KV_ERR_CAPTURE;
-  // larger batches: [tok_off: S+1][page_off: S+1][roots: S] staged through the pinned ring
+  // larger batches: two launches, [tok_off: S+1][page_off: S+1][roots: S] staged through the pinned ring
   HostBlob hb;
   hb.bytes.resize((2 * n1 + (roots ? n_sessions : 0)) * 8);
   std::memcpy(hb.bytes.data(), tok_offsets, n1 * 8);
@@ -265,6 +310,7 @@ int kv_chain_hash(kv_ctx *ctx, const uint64_t *ident, const int64_t *tok_offsets
   Blob b;
   int rc = upload_blob(ctx, hb, nullptr, true, s, &b);
   if (rc) return rc;
+  BlobGuard guard_blob(ctx, &b, s);
   j.tok_off = (const int64_t *)b.slot->d;
   j.page_off = j.tok_off + n1;
   j.roots = roots ? (const uint64_t *)(j.page_off + n1) : nullptr;
@@ -273,7 +319,6 @@ int kv_chain_hash(kv_ctx *ctx, const uint64_t *ident, const int64_t *tok_offsets
   kvt::kv_chain_link<false><<<n_sessions, 32, 0, s>>>(j);
   KV_CUDA(ctx, cudaGetLastError());
   ctx->launches += 2;
-  KV_CUDA(ctx, cudaEventRecord(b.slot->ev, s));
   return KV_OK;
 }
 
@@ -313,7 +358,7 @@ int kv_pack(kv_ctx *ctx, const kv_pool_desc *pools, uint32_t layer_count, const 
   const int64_t off[2] = {0, (int64_t)n};
   void *const dsts[1] = {dst};
   const uint64_t nb[1] = {(uint64_t)dst_bytes};
-  if (ctx) ctx->cur_stream = (cudaStream_t)stream;
+  enter(ctx, stream);
   Call c;
   int rc = plan_pack(ctx, pools, layer_count, page_ids, off, 1, layout, dsts, nb, flags, &c);
   if (rc) return rc;
@@ -328,7 +373,7 @@ int kv_unpack(kv_ctx *ctx, const void *src, size_t src_bytes, const int32_t *dst
   const void *const srcs[1] = {src};
   const uint64_t nb[1] = {(uint64_t)src_bytes};
   const uint64_t nt[1] = {n_tokens};
-  if (ctx) ctx->cur_stream = (cudaStream_t)stream;
+  enter(ctx, stream);
   Call c;
   int rc = plan_unpack(ctx, srcs, nb, dst_page_ids, off, nt, 1, pools, layer_count, src_page_size,
                        dst_page_size, layout, flags, &c);
@@ -339,7 +384,7 @@ int kv_unpack(kv_ctx *ctx, const void *src, size_t src_bytes, const int32_t *dst
 int kv_pack_batched(kv_ctx *ctx, const kv_pool_desc *pools, uint32_t layer_count,
                     const int32_t *page_ids, const int64_t *req_offsets, uint32_t n_req, int layout,
                     void *const *dsts, const uint64_t *dst_bytes, uint32_t flags, kv_stream_t stream) {
-  if (ctx) ctx->cur_stream = (cudaStream_t)stream;
+  enter(ctx, stream);
   Call c;
   int rc = plan_pack(ctx, pools, layer_count, page_ids, req_offsets, n_req, layout, dsts, dst_bytes, flags, &c);
   if (rc) return rc;
@@ -351,7 +396,7 @@ int kv_unpack_batched(kv_ctx *ctx, const void *const *srcs, const uint64_t *src_
                       const uint64_t *n_tokens, uint32_t n_req, const kv_pool_desc *pools,
                       uint32_t layer_count, uint32_t src_page_size, uint32_t dst_page_size,
                       int layout, uint32_t flags, kv_stream_t stream) {
-  if (ctx) ctx->cur_stream = (cudaStream_t)stream;
+  enter(ctx, stream);
   Call c;
   int rc = plan_unpack(ctx, srcs, src_bytes, dst_page_ids, req_offsets, n_tokens, n_req, pools,
                        layer_count, src_page_size, dst_page_size, layout, flags, &c);
@@ -359,12 +404,22 @@ int kv_unpack_batched(kv_ctx *ctx, const void *const *srcs, const uint64_t *src_
   return run_device(ctx, pools, c, dst_page_ids, flags, (cudaStream_t)stream);
 }
 
+int kv_submit(kv_ctx *ctx, const kv_pool_desc *pools, uint32_t layer_count, const kv_op *ops, uint32_t n_ops,
+              int layout, uint32_t flags, kv_stream_t stream) {
+  enter(ctx, stream);
+  Call c;
+  std::vector<int32_t> ids;
+  int rc = plan_submit(ctx, pools, layer_count, ops, n_ops, layout, flags, &c, &ids);
+  if (rc) return rc;
+  return run_device(ctx, pools, c, ids.data(), flags, (cudaStream_t)stream);
+}
+
 int kv_repage_batched(kv_ctx *ctx, const kv_pool_desc *src_pools, const int32_t *src_page_ids,
                       const int64_t *src_offsets, const kv_pool_desc *dst_pools,
                       const int32_t *dst_page_ids, const int64_t *dst_offsets,
                       const uint64_t *n_tokens, uint32_t n_req, uint32_t layer_count, uint32_t flags,
                       kv_stream_t stream) {
-  if (ctx) ctx->cur_stream = (cudaStream_t)stream;
+  enter(ctx, stream);
   Call c;
   std::vector<int32_t> ids;
   int rc = plan_repage(ctx, src_pools, src_page_ids, src_offsets, dst_pools, dst_page_ids,
@@ -388,7 +443,7 @@ int kv_cow_append_batched(kv_ctx *ctx, const kv_pool_desc *pools, uint32_t layer
                           const int32_t *old_ids, const int32_t *new_ids, const uint32_t *n_old,
                           const uint32_t *n_app, const void *const *apps, uint32_t n_sessions,
                           uint32_t flags, kv_stream_t stream) {
-  if (ctx) ctx->cur_stream = (cudaStream_t)stream;
+  enter(ctx, stream);
   Call c;
   int rc = plan_cow(ctx, pools, layer_count, old_ids, new_ids, n_old, n_app, apps, n_sessions, flags, &c);
   if (rc) return rc;
@@ -411,7 +466,7 @@ int kv_offload(kv_ctx *ctx, const kv_pool_desc *pools, uint32_t layer_count,
   const int64_t off[2] = {0, (int64_t)n};
   void *const dsts[1] = {host_dst};
   const uint64_t nb[1] = {(uint64_t)host_bytes};
-  if (ctx) ctx->cur_stream = (cudaStream_t)stream;
+  enter(ctx, stream);
   Call c;
   int rc = plan_pack(ctx, pools, layer_count, page_ids, off, 1, layout, dsts, nb, flags, &c);
   if (rc) return rc;
@@ -426,7 +481,7 @@ int kv_reload(kv_ctx *ctx, const void *host_src, size_t host_bytes, const int32_
   const void *const srcs[1] = {host_src};
   const uint64_t nb[1] = {(uint64_t)host_bytes};
   const uint64_t nt[1] = {n_tokens};
-  if (ctx) ctx->cur_stream = (cudaStream_t)stream;
+  enter(ctx, stream);
   Call c;
   int rc = plan_unpack(ctx, srcs, nb, dst_page_ids, off, nt, 1, pools, layer_count, src_page_size,
                        dst_page_size, layout, flags, &c);
@@ -440,7 +495,7 @@ int kv_reload_layerwise_batched(kv_ctx *ctx, const void *const *host_srcs, const
                                 uint32_t layer_count, uint32_t src_page_size, uint32_t dst_page_size,
                                 uint64_t *layer_flags, uint64_t flag_value, int mode, uint32_t flags,
                                 kv_stream_t stream) {
-  if (ctx) ctx->cur_stream = (cudaStream_t)stream;
+  enter(ctx, stream);
   if (!layer_flags) return KV_ERR_NULL;
   if ((uint64_t)(uintptr_t)layer_flags % 8) return KV_ERR_ALIGN;
   Call c;
@@ -481,7 +536,7 @@ int kv_offload_batched(kv_ctx *ctx, const kv_pool_desc *pools, uint32_t layer_co
                        const int32_t *page_ids, const int64_t *req_offsets, uint32_t n_req,
                        int layout, void *const *host_dsts, const uint64_t *host_bytes, int mode,
                        uint32_t flags, kv_stream_t stream) {
-  if (ctx) ctx->cur_stream = (cudaStream_t)stream;
+  enter(ctx, stream);
   Call c;
   int rc = plan_pack(ctx, pools, layer_count, page_ids, req_offsets, n_req, layout, host_dsts, host_bytes, flags, &c);
   if (rc) return rc;
@@ -493,7 +548,7 @@ int kv_reload_batched(kv_ctx *ctx, const void *const *host_srcs, const uint64_t 
                       const uint64_t *n_tokens, uint32_t n_req, const kv_pool_desc *pools,
                       uint32_t layer_count, uint32_t src_page_size, uint32_t dst_page_size,
                       int layout, int mode, uint32_t flags, kv_stream_t stream) {
-  if (ctx) ctx->cur_stream = (cudaStream_t)stream;
+  enter(ctx, stream);
   Call c;
   int rc = plan_unpack(ctx, host_srcs, host_bytes, dst_page_ids, req_offsets, n_tokens, n_req,
                        pools, layer_count, src_page_size, dst_page_size, layout, flags, &c);

@@ -35,7 +35,9 @@ KV_ORDER_NHD, KV_ORDER_HND = 0, 1
 KV_FLAG_VALIDATE, KV_FLAG_IDS_ON_DEVICE = 0x1, 0x2
 (KV_OPT_KERNEL, KV_OPT_STAGE_BYTES, KV_OPT_STAGES_PER_WARP, KV_OPT_WARPS, KV_OPT_STORE_LAG,
  KV_OPT_MAX_CTAS, KV_OPT_CHUNK_BYTES, KV_OPT_HOST_MAX_CTAS, KV_OPT_STAGING_SLOTS,
- KV_OPT_L2_HINT, KV_OPT_INLINE_TABLES, KV_OPT_DYNAMIC, KV_OPT_TENSOR_MAPS, KV_OPT_PDL) = range(14)
+ KV_OPT_L2_HINT, KV_OPT_INLINE_TABLES, KV_OPT_DYNAMIC, KV_OPT_TENSOR_MAPS, KV_OPT_PDL,
+ KV_OPT_RESERVE_STAGING) = range(15)
+KV_OP_PACK, KV_OP_UNPACK, KV_OP_COW_APPEND = 0, 1, 3
 KV_KERNEL_AUTO, KV_KERNEL_BULK, KV_KERNEL_VEC, KV_KERNEL_ELEM = 0, 1, 2, 3
 (KV_STAT_LAUNCHES, KV_STAT_MEMCPYS, KV_STAT_LAST_ITEMS, KV_STAT_LAST_PAYLOAD, KV_STAT_LAST_KERNEL,
  KV_STAT_LAST_HOST_MODE, KV_STAT_LAST_GRID, KV_STAT_LAST_SEGMENT, KV_STAT_LAST_TENSOR_MAPS) = range(9)
@@ -53,6 +55,19 @@ class kv_pool_desc(ctypes.Structure):
         ("elem_bytes", ctypes.c_uint32),
         ("order", ctypes.c_uint32),
         ("page_stride_bytes", ctypes.c_uint64),
+    ]
+
+
+class kv_op(ctypes.Structure):
+    _fields_ = [
+        ("kind", ctypes.c_uint32),
+        ("n_pages", ctypes.c_uint32),
+        ("page_ids", ctypes.c_void_p),
+        ("buf", ctypes.c_void_p),
+        ("buf_bytes", ctypes.c_uint64),
+        ("n_tokens", ctypes.c_uint64),
+        ("n_old", ctypes.c_uint32),
+        ("n_app", ctypes.c_uint32),
     ]
 
 
@@ -103,6 +118,7 @@ _kv_reload_layerwise = _sig("kv_reload_layerwise", _int, _vp, _vp, _sz, _vp, _u3
                             _vp, _u64, _int, _u32, _vp)
 _kv_reload_layerwise_batched = _sig("kv_reload_layerwise_batched", _int, _vp, _vp, _vp, _vp, _vp, _vp, _u32, _pdesc,
                                     _u32, _u32, _u32, _vp, _u64, _int, _u32, _vp)
+_kv_submit = _sig("kv_submit", _int, _vp, _pdesc, _u32, ctypes.POINTER(kv_op), _u32, _int, _u32, _vp)
 _kv_repage = _sig("kv_repage", _int, _vp, _pdesc, _vp, _u32, _pdesc, _vp, _u32, _u32, _u64, _u32, _vp)
 _kv_repage_batched = _sig("kv_repage_batched", _int, _vp, _pdesc, _vp, _vp, _pdesc, _vp, _vp, _vp,
                           _u32, _u32, _u32, _vp)
@@ -465,6 +481,41 @@ def kv_reload_layerwise_batched(ctx: Ctx, host_srcs, dst_page_ids, req_offsets, 
                                            off.ctypes.data, nt.ctypes.data, R, pools.ref, layer_count,
                                            src_page_size, dst_page_size, _ptr(layer_flags), int(flag_value),
                                            mode, flags, _stream(stream, ctx.device)))
+
+
+def op_pack(page_ids, dst, dst_bytes=None):
+    """One KV_OP_PACK of kv_submit: gather `page_ids` into the buffer `dst`."""
+    return (KV_OP_PACK, page_ids, dst, dst_bytes, 0, 0, 0)
+
+
+def op_unpack(src, dst_page_ids, n_tokens, src_bytes=None):
+    """One KV_OP_UNPACK of kv_submit: scatter the buffer `src` (pool page size) into `dst_page_ids`."""
+    return (KV_OP_UNPACK, dst_page_ids, src, src_bytes, int(n_tokens), 0, 0)
+
+
+def op_cow_append(old_id, new_id, n_old, app, n_app):
+    """One KV_OP_COW_APPEND of kv_submit (kv_cow_append's arguments)."""
+    return (KV_OP_COW_APPEND, np.array([old_id, new_id], dtype=np.int32), app, 0, 0, int(n_old), int(n_app))
+
+
+def kv_submit(ctx: Ctx, pools: PoolDesc, layer_count: int, ops, layout=KV_LAYOUT_PAGE_FIRST, flags=0, stream=None):
+    """Several independent transfers on one pool in ONE launch; `ops` is a sequence built with op_pack /
+    op_unpack / op_cow_append (marshalled into the C array of kv_op)."""
+    n = len(ops)
+    arr = (kv_op * max(n, 1))()
+    keep = []
+    for i, (kind, ids, buf, nbytes, n_tokens, n_old, n_app) in enumerate(ops):
+        a = _host_i32(ids)
+        keep.append(a)
+        o = arr[i]
+        o.kind = kind
+        o.n_pages = 0 if kind == KV_OP_COW_APPEND else a.size
+        o.page_ids = a.__array_interface__["data"][0] if a.size else None
+        o.buf = _ptr(buf)
+        o.buf_bytes = 0 if kind == KV_OP_COW_APPEND else (_nbytes(buf) if nbytes is None else int(nbytes))
+        o.n_tokens = n_tokens
+        o.n_old, o.n_app = n_old, n_app
+    _chk(ctx, _kv_submit(ctx.h, pools.ref, layer_count, arr, n, layout, flags, _stream(stream, ctx.device)))
 
 
 def kv_repage(ctx: Ctx, src_pools: PoolDesc, src_page_ids, dst_pools: PoolDesc, dst_page_ids,

@@ -222,6 +222,45 @@ def test_plan_fused_repage_and_cow(ctx):
     kv.kv_cow_append(ctx, d, s.L, 7, 9, 0, None, 0)  # nothing to do: KV_OK, even without a device
 
 
+def test_plan_submit_one_launch_for_a_turn(ctx):
+    """kv_submit (SURVEY.md 8(a) a8 / PAPER.md:L238): a turn's scatter + copy-on-write append + gather planned as ONE
+    launch whose pieces carry their own direction; validation of every operation precedes it."""
+    s = W.QWEN3_OMNI
+    d = fake_pool(s)
+    rng = np.random.default_rng(5)
+    perm = rng.permutation(s.P).astype(np.int32)
+    dst, src, old, new = perm[:100], perm[100:160], int(perm[160]), int(perm[161])
+    ops = [kv.op_unpack(BUF, dst, 100 * s.T, src_bytes=100 * s.page_bytes),
+           kv.op_cow_append(old, new, 5, BUF + (1 << 36), 7),
+           kv.op_pack(src, BUF + (1 << 37), dst_bytes=60 * s.page_bytes)]
+    assert status_of(lambda: kv.kv_submit(ctx, d, s.L, ops, flags=kv.KV_FLAG_VALIDATE)) == kv.KV_ERR_NO_DEVICE
+    assert ctx.stat(kv.KV_STAT_LAST_ITEMS) == 100 * 96 + 96 * 2 + 60 * 96
+    assert ctx.stat(kv.KV_STAT_LAST_PAYLOAD) == 160 * s.page_bytes + 96 * 12 * 1024
+    assert ctx.stat(kv.KV_STAT_LAST_SEGMENT) == 16384 and ctx.stat(kv.KV_STAT_LAST_KERNEL) == kv.KV_KERNEL_VEC  # 240 MiB: AUTO's mid range
+    assert ctx.stat(kv.KV_STAT_LAUNCHES) == 0
+    # a ragged unpack: n_pages must be ceil(n_tokens / T)
+    assert status_of(lambda: kv.kv_submit(ctx, d, s.L, [kv.op_unpack(BUF, dst, 100 * s.T - 16, src_bytes=1 << 40)])) == kv.KV_ERR_SIZE
+    kv_ok = [kv.op_unpack(BUF, dst, 100 * s.T - 15, src_bytes=1 << 40)]
+    assert status_of(lambda: kv.kv_submit(ctx, d, s.L, kv_ok)) == kv.KV_ERR_NO_DEVICE
+    # buffer too small, id out of range, bad kind, device ids
+    assert status_of(lambda: kv.kv_submit(ctx, d, s.L, [kv.op_pack(src, BUF, dst_bytes=59 * s.page_bytes)])) == kv.KV_ERR_SIZE
+    bad = src.copy(); bad[3] = s.P
+    assert status_of(lambda: kv.kv_submit(ctx, d, s.L, [kv.op_pack(bad, BUF, dst_bytes=1 << 40)])) == kv.KV_ERR_PAGE_RANGE
+    assert status_of(lambda: kv.kv_submit(ctx, d, s.L, [(2, src, BUF, 1 << 40, 0, 0, 0)])) == kv.KV_ERR_LAYOUT
+    assert status_of(lambda: kv.kv_submit(ctx, d, s.L, ops, flags=kv.KV_FLAG_IDS_ON_DEVICE)) == kv.KV_ERR_LAYOUT
+    assert status_of(lambda: kv.kv_submit(ctx, d, s.L, [kv.op_cow_append(old, new, 10, BUF, 7)])) == kv.KV_ERR_SIZE
+    assert status_of(lambda: kv.kv_submit(ctx, d, s.L, [kv.op_cow_append(old, old, 1, BUF, 1)])) == kv.KV_ERR_SIZE
+    assert status_of(lambda: kv.kv_submit(ctx, d, s.L, [kv.op_cow_append(old, new, 1, None, 1)])) == kv.KV_ERR_NULL
+    # under KV_FLAG_VALIDATE: two operations writing one page; an operation reading a page another one writes
+    two = [kv.op_unpack(BUF, dst, 100 * s.T, src_bytes=1 << 40), kv.op_cow_append(old, int(dst[7]), 1, BUF, 1)]
+    assert status_of(lambda: kv.kv_submit(ctx, d, s.L, two, flags=kv.KV_FLAG_VALIDATE)) == kv.KV_ERR_DUP_PAGE
+    rw = [kv.op_unpack(BUF, dst, 100 * s.T, src_bytes=1 << 40), kv.op_pack(dst[:3], BUF + (1 << 37), dst_bytes=1 << 40)]
+    assert status_of(lambda: kv.kv_submit(ctx, d, s.L, rw, flags=kv.KV_FLAG_VALIDATE)) == kv.KV_ERR_DUP_PAGE
+    assert status_of(lambda: kv.kv_submit(ctx, d, s.L, rw)) == kv.KV_ERR_NO_DEVICE  # unchecked without the flag
+    kv.kv_submit(ctx, d, s.L, [])  # nothing to do: KV_OK
+    kv.kv_submit(ctx, d, s.L, [kv.op_pack(np.zeros(0, np.int32), BUF, dst_bytes=0), kv.op_cow_append(old, new, 0, None, 0)])
+
+
 def test_plan_hnd_pools(ctx):
     """SURVEY.md 8(f) NEXT-2, HND pools: kernel and segment chosen per direction (DESIGN.md "HND pools");
     a malformed order is KV_ERR_DESC; degenerate HND (one head) plans as a plain copy."""

@@ -22,8 +22,20 @@ def run_bench(*args):
 
 
 def test_reference_arm_prints_the_contract_line():
-    line = run_bench("--impl", "reference", "--steps", "1", "--warmup", "1")
+    line = run_bench("--impl", "reference", "--steps", "2", "--warmup", "1")
     assert BASE_KEYS <= set(line), BASE_KEYS - set(line)
+    # the reference arm honours --steps / --warmup and times the oracle on OUR arm's config: the same `config` object,
+    # the full 512-page prefix per step
+    assert line["steps"] == 2 and line["warmup"] == 1
+    sys.path.insert(0, ROOT)
+    import argparse
+
+    import bench
+    from paper_2606_31093_b200 import workloads as W
+
+    ours = bench.bench_config(argparse.Namespace(prefix_tokens=8192, pool_order="nhd", pool_pages=65536), W.QWEN3_OMNI)
+    assert line["config"] == ours and ours["pages_per_step"] == 512
+    assert "full 512-page prefix" in line["cpu_baseline"]["sample"]
     assert line["impl"] == "reference" and line["metric"] == "kv_pack_unpack_GBps" and line["unit"] == "GB/s"
     assert line["value"] > 0 and line["higher_is_better"] is True and line["vs_baseline"] is None
     assert line["cpu_baseline"]["kind"] == "oracle" and line["cpu_baseline"]["cores"] >= 1
@@ -50,6 +62,17 @@ def test_our_arm_prints_the_contract_line():
     assert line["cpu_baseline"]["kind"] == "oracle" and line["cpu_baseline"]["value"] > 0
     assert set(line["clocks"]) >= {"sm_mhz", "sm_max_mhz", "reasons"}
     assert line["config"]["workload"].startswith("configs[1]")
+    assert line["bit_exact"] is True  # the timed region's last step, checked with torch indexing
+    assert r["traffic"] is None  # a profile figure: emitted only for the profiled configuration (96 GiB pool)
+    # the host-link roofline is measured in the same run: peaks and fractions for offload, reload and both at once
+    h = line["roofline_host"]
+    for k in ("offload", "reload", "duplex"):
+        assert 0 < h[k]["frac"] == pytest.approx(h[k]["achieved"] / h[k]["peak"])
+    assert h["peaks"]["h2d_GBps"] > 0 and h["peaks"]["d2h_GBps"] > 0 and h["peaks"]["duplex_GBps"] > 0
+    assert "per_config" not in line  # needs the 96 GiB pool
+    assert line["peer"]["available"] in (True, False)
+    if line["peer"]["available"]:
+        assert line["peer"]["push"]["bit_exact"] and line["peer"]["pull"]["bit_exact"]
 
 
 @pytest.mark.gpu

@@ -65,6 +65,7 @@ def test_random_configuration(kv, seed):
         A = host_pool(rng, L, C, Ps, Ts, H, D, e, c["pad"], order=c["order_s"])
         B = host_pool(rng, L, C, Pd, Td, H, D, e, c["pad"], order=c["order_d"])
         B2 = ko.HostPool([s.copy() for s in B.slabs], L, C, Pd, Td, H, D, e, B.page_stride_bytes, c["order_d"])
+        pristine = [s.copy() for s in B.slabs]  # the destination pool BEFORE any transfer (step 5 starts from it)
         tA, dA = to_device(A, kv, torch)
         tB, dB = to_device(B, kv, torch)
         tB2, dB2 = to_device(B2, kv, torch)
@@ -102,12 +103,15 @@ def test_random_configuration(kv, seed):
             kv.kv_cow_append_batched(ctx, dB, L, old, new, n_old, n_app, dev, flags=kv.KV_FLAG_VALIDATE)
             ko.cow_append_batched(B, old, new, n_old, n_app, apps)
             assert_pool_equal(tB, B)
-        # 5. the host tier on the same requests: offload A's pages, reload them re-paged into a fresh copy
-        #    of the destination pool; random mode, random pipeline chunk size (multi-chunk, layer ranges,
+        # 5. the host tier on the same requests: offload A's pages, reload them re-paged into a PRISTINE copy of the
+        #    destination pool -- taken before steps 2-4, so none of the bytes the reload must deliver is there yet and a
+        #    reload that writes nothing fails; random mode, random pipeline chunk size (multi-chunk, layer ranges,
         #    page ranges); a chunk smaller than one lcm(Ts, Td) unit is refused with KV_ERR_SIZE -> direct
-        B3 = ko.HostPool([s_.copy() for s_ in B2.slabs], L, C, Pd, Td, H, D, e, B.page_stride_bytes, c["order_d"])
+        B3 = ko.HostPool([s_.copy() for s_ in pristine], L, C, Pd, Td, H, D, e, B.page_stride_bytes, c["order_d"])
+        tB3, dB3 = to_device(B3, kv, torch)  # uploaded BEFORE the oracle touches B3
+        if doff[-1]:
+            assert not all(np.array_equal(a, b) for a, b in zip(pristine, B2.slabs)), "the transfer would be invisible"
         ko.unpack_batched(want, dids, doff, ntok, B3, Ts=Ts, layout=c["layout"])
-        tB3, dB3 = to_device(B2, kv, torch)
         mode = int(rng.choice([kv.KV_HOST_DIRECT, kv.KV_HOST_STAGED, kv.KV_HOST_STAGED]))
         ctx.set_option(kv.KV_OPT_CHUNK_BYTES, int(rng.choice([0, 64 << 10, 256 << 10, 1 << 20])))
         hps = [kv.kv_host_alloc(max(n * page_s, 16)) for n in ns]
