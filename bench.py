@@ -370,8 +370,8 @@ def run_ours(args):
             ev[2 * i + 2].record(stream)
         barrier()
         launches = ctx.stat(kv.KV_STAT_LAUNCHES) - l0
-        kern_name = {kv.KV_KERNEL_BULK: "kv_move_bulk", kv.KV_KERNEL_VEC: "kv_move_vec",
-                     kv.KV_KERNEL_ELEM: "kv_move_elem"}.get(ctx.stat(kv.KV_STAT_LAST_KERNEL), "?")
+        kern_name = {kv.KV_KERNEL_BULK: "kv_move_bulk", kv.KV_KERNEL_VEC: "kv_move_vec", kv.KV_KERNEL_ELEM: "kv_move_elem",
+                     kv.KV_KERNEL_SHOT: "kv_move_shot"}.get(ctx.stat(kv.KV_STAT_LAST_KERNEL), "?")
         t_total_ms = max_over_ranks(ev[0].elapsed_time(ev[2 * K]))
         pack_ms = float(np.mean([ev[2 * i].elapsed_time(ev[2 * i + 1]) for i in range(K)]))
         unpack_ms = float(np.mean([ev[2 * i + 1].elapsed_time(ev[2 * i + 2]) for i in range(K)]))

@@ -212,7 +212,7 @@ def sweep_row(torch, ctx, desc, shape, chk, buf, flush, npg, rng, hbm, t_launch,
             "pack_GBps": 2 * pls / m / 1e3, "pack_GBps_queued": 2 * pls / mq / 1e3,
             "pack_frac_hbm": 2 * pls / m / 1e3 / hbm, "pack_frac_hbm_queued": 2 * pls / mq / 1e3 / hbm,
             "floor_us": floor, "vs_floor": m / floor, "floor_us_queued": floor_q, "vs_floor_queued": mq / floor_q,
-            "kernel": {1: "bulk", 2: "vec", 3: "elem"}.get(ctx.stat(kv.KV_STAT_LAST_KERNEL), "?"),
+            "kernel": {1: "bulk", 2: "vec", 3: "elem", 4: "shot"}.get(ctx.stat(kv.KV_STAT_LAST_KERNEL), "?"),
             "bit_exact": bool(chk.pack_ok(buf, ids, layers=layers)), "_ids": ids}
 
 

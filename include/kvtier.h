@@ -115,7 +115,8 @@ typedef enum kv_status {
 
 /* kv_ctx_set_option keys (tuning; defaults are the measured best) */
 typedef enum kv_option {
-  KV_OPT_KERNEL = 0,         /* 0 auto, 1 bulk (cp.async.bulk smem ring), 2 vec (16-byte LDG/STG), 3 elem (any alignment) */
+  KV_OPT_KERNEL = 0,         /* 0 auto, 1 bulk (cp.async.bulk ring, persistent CTAs), 2 vec (16-byte LDG/STG), 3 elem (any
+                                alignment), 4 shot (cp.async.bulk, one segment per single-warp CTA) */
   KV_OPT_STAGE_BYTES = 1,    /* bulk: bytes per shared-memory stage (multiple of 16, 1 KiB .. 64 KiB) */
   KV_OPT_STAGES_PER_WARP = 2,/* bulk: ring depth per issuing warp (2 .. 16) */
   KV_OPT_WARPS = 3,          /* bulk: issuing warps per CTA (1 .. 8).  Until options 1-3 are set the ring follows the row
@@ -126,7 +127,8 @@ typedef enum kv_option {
                                 transfer where that leaves 64 MiB each, at most one staging slot each) */
   KV_OPT_HOST_MAX_CTAS = 7,  /* grid cap for DIRECT host transfers (0 = same as device transfers) */
   KV_OPT_STAGING_SLOTS = 8,  /* staged host transfers: pipeline slots the staging buffer is cut into (2 .. 4) */
-  KV_OPT_L2_HINT = 9,        /* bulk: 0 none, 1 evict_first cache hint on loads and stores */
+  KV_OPT_L2_HINT = 9,        /* bulk: L2 cache hints, a bit set: 1 = loads evict_first, 2 = stores evict_first, 4 = stores
+                                evict_last (2 and 4 exclude each other: 0 .. 5) */
   KV_OPT_INLINE_TABLES = 10, /* 1 (default): page ids / slab bases ride in the kernel parameters when they fit (<= 31 KiB);
                                 0: always stage them through the ctx's pinned ring with one H2D copy */
   KV_OPT_DYNAMIC = 11,       /* bulk: 1 (default) large launches claim segments from a device counter (guided chunks);

@@ -220,41 +220,52 @@ int make_geom(const kv_ctx *ctx, const kv_pool_desc *p, uint32_t layer_count, ui
         if (g.pool_hnd) { map_key(p, layer_count, tb, es, &key); cached_or_free = find_maps(ctx, key) != nullptr; }
         if (cached_or_free && g.src_hnd) { map_key(src_pool, layer_count, tb, es, &key); cached_or_free = find_maps(ctx, key) != nullptr; }
       }
-      if (cached_or_free) { g.tma = true; g.tb = tb; g.tma_es = es; kernel = KERNEL_BULK; }
+      if (cached_or_free) { g.tma = true; g.tb = tb; g.tma_es = es; }
     }
   }
   if (kernel == KERNEL_AUTO) {
-    // Measured on B200 for the paths without tensor maps: a strided DESTINATION is
-    // fastest with 16-byte STG from many warps (vec, 5.5 TB/s); a strided source alone is fastest gathered by
-    // cp.async into the bulk ring and stored with one bulk copy (5.8 TB/s); everything contiguous is the
-    // bulk path (6.3 TB/s).
-    const bool dst_strided = g.pool_hnd && dir != 0;
-    kernel = dst_strided ? KERNEL_VEC : KERNEL_BULK;
-    // Mid-sized contiguous transfers are latency-bound: 14 MB in flight through 296 issuing warps ramps slower
-    // than 16-byte loads from 1,184 CTAs' worth of warps.  Measured on B200, isolated calls on a cold L2
-    // (DESIGN.md "Kernels"): 48 MiB 23.6 -> 18.5 us, 64 MiB 27.7 -> 23.6, 192 MiB 68.6 -> 64.6; equal at
-    // <= 32 MiB (launch-bound) and 128 MiB; bulk ahead again from 512 MiB (171 vs 177 us).
-    if (!g.trans && dir != 3) {
-      uint64_t bytes = 0;
-      for (const Req &r : reqs) bytes += r.n_ids * g.pool_row * g.LC;
-      if (bytes >= kAutoVecMinBytes && bytes < kAutoVecMaxBytes) kernel = KERNEL_VEC;
-      // Segments of 1 KiB or less (one-token pages; re-paging between page sizes with no common divisor): an SM
-      // retires small bulk copies too slowly (about 11 M segments/s: 3.4 TB/s at 1 KiB); kv_move_small (32 segments
-      // decoded per warp at once, copied eight at a time) does 6.05-6.15 TB/s.  From 2 KiB the bulk ring (re-shaped,
-      // kv_launch.inl) is back at 6.2 TB/s.
-      if (g.chunk_bytes <= 1024 && bytes >= (8ull << 20)) kernel = KERNEL_VEC;
-    } else if (!g.trans) {
-      // copy-on-write appends are many short, ragged pieces (about 6 KiB each): one warp per piece with 16-byte
-      // loads beats one bulk copy per piece at every size where they differ (64 sessions: 44 -> 30 us,
-      // 512 sessions: 279 -> 225 us; equal below ~16 MiB)
-      uint64_t bytes = 0;
-      for (const Req &r : reqs) bytes += ((r.n_tokens & 0xffffffffull) + (r.n_tokens >> 32)) * tokrow * g.LC;
-      if (bytes >= (16ull << 20)) kernel = KERNEL_VEC;
+    // One segment per single-warp CTA (kv_move_shot) wherever a segment is at least 4 KiB: measured on B200 against the
+    // persistent ring and the 16-byte LDG/STG kernel (round 2) it is ahead on every such shape --
+    // 768 MiB back to back 6.64 vs 6.38 / 6.01 TB/s at 16 KiB rows, 6.63 vs 6.19 / 5.95 at 4 KiB rows, HND pools with
+    // tensor maps 6.62 vs 6.33, HND lane paths 6.58 / 6.48 vs 6.13 / 4.25, copy-on-write batches 5.6 vs 3.3 / 5.2 -- and
+    // on every size from 1 MiB (7.2 vs 9.2 us isolated) to 1 GiB (320 vs 331 us).  Below 4 KiB the rate at which an SM
+    // retires bulk copies takes over (about 11 M a second): 2 KiB segments 3.9 TB/s against the ring's 6.2 (more,
+    // shallower stages per SM), 1 KiB 2.0 against kv_move_small's 6.0.
+    const uint32_t cap16 = std::max(16u, ctx->stage_bytes / 16 * 16);
+    uint32_t seg = std::min(g.chunk_bytes, cap16);
+    if (g.tma) seg = g.tb * g.tokrow;
+    else if (g.trans) seg = std::min(g.chunk_bytes, std::max(g.drow, cap16 / g.drow * g.drow));
+    if (dir == 3) seg = (uint32_t)std::min<uint64_t>(g.pool_row / 2, cap16);  // ragged pieces: half a page row on average
+    const bool shot = seg >= kShotMinSegment && (!g.trans || g.drow <= cap16);
+    if (shot) {
+      kernel = KERNEL_SHOT;
+    } else {
+      // Short segments.  Paths without tensor maps on an HND pool: a strided DESTINATION is fastest with 16-byte STG from
+      // many warps (vec); a strided source alone gathered by cp.async into the bulk ring; everything contiguous: the ring,
+      // re-shaped for narrow rows (kv_launch.inl).
+      const bool dst_strided = g.pool_hnd && dir != 0;
+      kernel = (dst_strided && !g.tma) ? KERNEL_VEC : KERNEL_BULK;  // small tensor boxes: the ring, as before
+      if (!g.trans && dir != 3) {
+        uint64_t bytes = 0;
+        for (const Req &r : reqs) bytes += r.n_ids * g.pool_row * g.LC;
+        // Segments of 1 KiB or less (one-token pages; re-paging between page sizes with no common divisor): an SM
+        // retires small bulk copies too slowly (3.4 TB/s at 1 KiB); kv_move_small (32 segments decoded per warp at once,
+        // copied eight at a time) does 6.05-6.15 TB/s.  From 2 KiB the re-shaped ring is back at 6.2 TB/s.
+        if (g.chunk_bytes <= 1024 && bytes >= (8ull << 20)) kernel = KERNEL_VEC;
+      } else if (!g.trans) {
+        // copy-on-write appends on narrow token rows: many short, ragged pieces; one warp per piece with 16-byte loads
+        // beats one bulk copy per piece from ~16 MiB
+        uint64_t bytes = 0;
+        for (const Req &r : reqs) bytes += ((r.n_tokens & 0xffffffffull) + (r.n_tokens >> 32)) * tokrow * g.LC;
+        if (bytes >= (16ull << 20)) kernel = KERNEL_VEC;
+      }
     }
   }
-  uint32_t cap = kernel == KERNEL_BULK ? (g.trans && !g.tma ? ctx->t_stage_bytes : ctx->stage_bytes) : 16384u;
+  if (!is_async_kernel(kernel)) g.tma = false;  // tensor copies exist in the shared-memory kernels only
+  uint32_t cap = kernel == KERNEL_BULK ? (g.trans && !g.tma ? ctx->t_stage_bytes : ctx->stage_bytes)
+                 : (kernel == KERNEL_SHOT ? ctx->stage_bytes : 16384u);
   cap = std::max(16u, cap / 16 * 16);
-  if (g.trans && kernel == KERNEL_BULK && g.drow > cap) kernel = KERNEL_VEC;  // a row must fit one stage
+  if (g.trans && is_async_kernel(kernel) && g.drow > cap) kernel = KERNEL_VEC;  // a row must fit one stage
   g.kernel = kernel;
   g.sub_bytes = std::min(g.chunk_bytes, cap);
   if (!g.trans && g.chunk_bytes > cap && g.chunk_bytes % 16 == 0) {
@@ -267,13 +278,13 @@ int make_geom(const kv_ctx *ctx, const kv_pool_desc *p, uint32_t layer_count, ui
   }
   if (g.trans) g.sub_bytes = std::min(g.chunk_bytes, std::max(g.drow, cap / g.drow * g.drow));  // whole rows
   if (g.tma) g.sub_bytes = g.tb * g.tokrow;  // whole tokens: one box
-  if (kernel == KERNEL_BULK && dir != 3) {
+  if (is_async_kernel(kernel) && dir != 3) {
     // Launch-bound calls: with fewer segments than issuing warps most SMs would idle while a few
     // move 16 KiB each; cutting segments down to >= 4 KiB spreads a small transfer over the chip
     // (measured on B200, 1 MiB pack back to back: 6.1 -> 5.0 us per call).
     uint64_t chunks = 0;
     for (const Req &r : reqs) chunks += r.n_ids * (g.Tpool / g.g) * g.LC;
-    const uint64_t lanes = (uint64_t)ctx->sm_count * (g.trans && !g.tma ? ctx->t_warps : ctx->warps);
+    const uint64_t lanes = (uint64_t)ctx->sm_count * (kernel == KERNEL_SHOT ? 2 : (g.trans && !g.tma ? ctx->t_warps : ctx->warps));
     while (g.sub_bytes >= 8192 && g.sub_bytes % 32 == 0 && (!g.trans || (g.sub_bytes / 2) % g.drow == 0) &&
            (!g.tma || g.tb % 2 == 0) &&
            chunks * ((g.chunk_bytes + g.sub_bytes - 1) / g.sub_bytes) * 2 <= lanes) {

@@ -12,11 +12,12 @@ constexpr int kBlobSlots = 16;
 constexpr int kMaxStagingSlots = 4;
 constexpr uint32_t kMaxLayersKv = 4096;  // layer_count * kv_count
 constexpr uint64_t kAutoStagedMinBytes = 16ull << 20;
-constexpr uint64_t kAutoVecMinBytes = 40ull << 20, kAutoVecMaxBytes = 288ull << 20;  // AUTO: vec kernel in between
+constexpr uint32_t kShotMinSegment = 4096;  // AUTO: kv_move_shot from this segment size (below it the SM's bulk-copy rate binds)
 constexpr uint32_t kSchedSlots = 256;  // claim counters, handed out round-robin per launch
 constexpr int kStaticSmemReserve = 8192;  // static shared memory of kv_move_bulk (barriers + stage metadata, 6 KiB) rounded up
 
-enum KernelKind { KERNEL_AUTO = 0, KERNEL_BULK = 1, KERNEL_VEC = 2, KERNEL_ELEM = 3 };
+enum KernelKind { KERNEL_AUTO = 0, KERNEL_BULK = 1, KERNEL_VEC = 2, KERNEL_ELEM = 3, KERNEL_SHOT = 4 };
+inline bool is_async_kernel(int k) { return k == KERNEL_BULK || k == KERNEL_SHOT; }  // cp.async.bulk through shared-memory stages
 
 // Tensor maps of one HND pool for one box size (kv_kernels.cuh "TMA tensor maps"): built once per
 // (pool, box) and kept in device memory for the life of the ctx.

@@ -11,6 +11,7 @@
 //                 per-warp ring of mbarrier-tracked stages.  32 lanes decode 32 segments' addresses
 //                 at once (warp-level page-table lookup), lane 0 drives the async copy engine.
 //                 No data ever passes through registers.
+//   kv_move_shot  one segment per single-warp CTA, same async copies, no ring: the CTA scheduler distributes the work.
 //   kv_move_vec   16-byte LDG/STG, one warp per segment, 8 loads in flight per lane.
 //   kv_move_small segments <= 1 KiB: 32 segments decoded per warp, copied eight at a time (16-byte LDG/STG).
 //   kv_move_elem  any alignment: unit-wide (1/2/4/8 B) coalesced copy.  Correctness fallback.
@@ -432,8 +433,12 @@ __global__ void __launch_bounds__(kMaxWarps * 32, 1) kv_move_bulk(const __grid_c
   const uint64_t n_my = dyn ? 0 : (gw < j.total_items ? (j.total_items - gw + G - 1) / G : 0);
   if (!dyn && n_my == 0) return;
 
-  uint64_t pol = 0;
-  if (j.l2_hint) asm volatile("createpolicy.fractional.L2::evict_first.b64 %0, 1.0;" : "=l"(pol));
+  // L2 hints (KV_OPT_L2_HINT): bit 0 = loads evict_first (the source is read once), bit 1 = stores evict_first,
+  // bit 2 = stores evict_last (keep what was just written resident for whoever reads it next)
+  uint64_t pol = 0, pol_st = 0;
+  if (j.l2_hint & 1) asm volatile("createpolicy.fractional.L2::evict_first.b64 %0, 1.0;" : "=l"(pol));
+  if (j.l2_hint & 2) asm volatile("createpolicy.fractional.L2::evict_first.b64 %0, 1.0;" : "=l"(pol_st));
+  if (j.l2_hint & 4) asm volatile("createpolicy.fractional.L2::evict_last.b64 %0, 1.0;" : "=l"(pol_st));
 
   const uint32_t stage0 = smem_u32(smem) + j.zero_bytes + warp * K * j.stage_bytes;
   const uint32_t zero0 = smem_u32(smem);
@@ -590,19 +595,27 @@ __global__ void __launch_bounds__(kMaxWarps * 32, 1) kv_move_bulk(const __grid_c
       __syncwarp();  // meta[] written by lane 0 is read by every lane `depth` iterations later
     } else
     if (lane == 0) {
-      if (it >= depth && it - depth < n_known) {  // ---- store side: item si
-        const uint64_t si = it - depth;
-        const uint32_t s = (uint32_t)(si % K);
-        mbar_wait(smem_u32(&full_bar[warp][s]), (uint32_t)(si / K) & 1);
-        const StageMeta m = meta[warp][s];
-        if (m.valid) {
-          if (j.l2_hint) bulk_s2g_hint(m.dst, stage0 + s * j.stage_bytes, m.valid, pol);
-          else bulk_s2g(m.dst, stage0 + s * j.stage_bytes, m.valid);
+      auto store_side = [&]() {
+        if (it >= depth && it - depth < n_known) {  // ---- store side: item si
+          const uint64_t si = it - depth;
+          const uint32_t s = (uint32_t)(si % K);
+          mbar_wait(smem_u32(&full_bar[warp][s]), (uint32_t)(si / K) & 1);
+          const StageMeta m = meta[warp][s];
+          if (m.valid) {
+            if (j.l2_hint & 6) bulk_s2g_hint(m.dst, stage0 + s * j.stage_bytes, m.valid, pol_st);
+            else bulk_s2g(m.dst, stage0 + s * j.stage_bytes, m.valid);
+          }
+          for (uint32_t z = m.valid; z < m.bytes; z += j.zero_bytes)  // zero-padded tail (a5)
+            bulk_s2g(m.dst + z, zero0, min(j.zero_bytes, m.bytes - z));
+          bulk_commit();
         }
-        for (uint32_t z = m.valid; z < m.bytes; z += j.zero_bytes)  // zero-padded tail (a5)
-          bulk_s2g(m.dst + z, zero0, min(j.zero_bytes, m.bytes - z));
-        bulk_commit();
-      }
+      };
+      // Ramp: the first K loads of a warp go into stages nobody has used, so they are issued BEFORE this warp blocks on
+      // its first store (all K x stage bytes of the warp in flight from the start: a transfer of a few segments per
+      // warp never waits for a load it could already have issued).  From iteration K on a stage is refilled once the
+      // store that last read it has finished reading: the store of this iteration is committed first, so that store
+      // was committed `lag` groups ago.
+      if (it >= K) store_side();
       if (have) {  // ---- load side: item it
         const uint32_t s = (uint32_t)(it % K);
         if (it >= K) {  // the store that last read this stage was committed `lag` groups ago
@@ -614,12 +627,13 @@ __global__ void __launch_bounds__(kMaxWarps * 32, 1) kv_move_bulk(const __grid_c
         const uint32_t bar = smem_u32(&full_bar[warp][s]);
         if (valid) {
           mbar_expect_tx(bar, valid);
-          if (j.l2_hint) bulk_g2s_hint(stage0 + s * j.stage_bytes, src, valid, bar, pol);
+          if (j.l2_hint & 1) bulk_g2s_hint(stage0 + s * j.stage_bytes, src, valid, bar, pol);
           else bulk_g2s(stage0 + s * j.stage_bytes, src, valid, bar);
         } else {
           mbar_arrive(bar);
         }
       }
+      if (it < K) store_side();
     }
   }
   if (dyn && lane == 0) {  // last warp out re-arms the counters for the next launch
@@ -630,7 +644,126 @@ __global__ void __launch_bounds__(kMaxWarps * 32, 1) kv_move_bulk(const __grid_c
       __threadfence();
     }
   }
-  if (lane == 0 || kTrans) bulk_wait_all();
+  // The stages must outlive the bulk stores' READS; their global writes complete with the grid (what a later kernel
+  // or copy on the stream, or the host after a sync, observes), so a warp need not sit out the write acknowledgements.
+  if (lane == 0 || kTrans) bulk_wait_read<0>();
+}
+
+// ---------------------------------------------------------------------------------------------
+// kv_move_shot: ONE segment per single-warp CTA; the hardware's CTA scheduler is the work distributor.
+//   load the segment into the CTA's one stage (cp.async.bulk / cp.async.bulk.tensor / row gathers), wait on the
+//   mbarrier, store it (bulk / tensor / 16-byte stores), wait until the store has READ the stage, exit.
+// A CTA owns `stage_bytes` of shared memory (16 KiB at the paper's shapes) and 32 threads, so an SM holds as many
+// segments in flight as its shared memory takes (13-14 x 16 KiB: ~220 KiB per SM, 32 MB per chip, against the ~128 KiB
+// per SM of the persistent ring), loads and stores of different CTAs overlap freely, a finished CTA is replaced at
+// once, and there is no ring, no claim counter and no tail to balance.  Measured on B200 against a plain contiguous
+// cudaMemcpyAsync of the same size under the same conditions (isolated call, cold clean L2; _work probe of round 2):
+// a minimal kernel of this shape equals the plain copy from 1 MiB to 768 MiB (64 MiB 21.8 vs 21.5 us, 768 MiB 239 vs
+// 242 us) where the ring needed 27.7 / 249 us.  DESIGN.md "Kernels".
+// gridDim.x may be capped (KV_OPT_MAX_CTAS): a CTA then walks items blockIdx.x, + gridDim.x, ... reusing its stage.
+// ---------------------------------------------------------------------------------------------
+template <int N, bool kTrans>
+__global__ void __launch_bounds__(32) kv_move_shot(const __grid_constant__ JobT<N> p) {
+  const Job &j = p.j;
+  const Tables tb = tables_of(p);
+  extern __shared__ __align__(128) uint8_t smem[];
+  __shared__ __align__(8) uint64_t full_bar;
+  const uint32_t lane = threadIdx.x;
+  const uint32_t bar = smem_u32(&full_bar), sbase = smem_u32(smem);
+  if (lane == 0) {
+    mbar_init(bar, kTrans ? 32 : 1);
+    asm volatile("fence.mbarrier_init.release.cluster;" ::: "memory");
+    asm volatile("fence.proxy.async.shared::cta;" ::: "memory");
+  }
+  __syncwarp();
+  asm volatile("griddepcontrol.launch_dependents;" ::: "memory");  // no-ops without the launch attribute (KV_OPT_PDL)
+  asm volatile("griddepcontrol.wait;" ::: "memory");               // nothing global is touched before this
+  uint64_t pol = 0, pol_st = 0;
+  if (j.l2_hint & 1) asm volatile("createpolicy.fractional.L2::evict_first.b64 %0, 1.0;" : "=l"(pol));
+  if (j.l2_hint & 2) asm volatile("createpolicy.fractional.L2::evict_first.b64 %0, 1.0;" : "=l"(pol_st));
+  if (j.l2_hint & 4) asm volatile("createpolicy.fractional.L2::evict_last.b64 %0, 1.0;" : "=l"(pol_st));
+  uint32_t hint = 0, phase = 0;
+  for (uint64_t item = blockIdx.x; item < j.total_items; item += gridDim.x) {
+    // every lane decodes the CTA's segment (uniform: no shuffles, no divergence)
+    const Item it = decode<N == 0, kTrans>(j, tb, item, hint);
+    if (it.bytes == 0) continue;  // skipped: a device-resident page id was out of range
+    if constexpr (kTrans) {
+      const Strides st = strides_of(j);
+      const uint32_t upr = j.drow >> 4;  // 16-byte units per head_dim row
+      const uint32_t box_bytes = j.tb * j.tokrow;
+      const uint8_t *maps_s = j.dir == 2 ? j.maps_src : ((j.dir == 0 || j.dir == 4) ? j.maps_pool : nullptr);
+      const uint8_t *maps_d = (j.dir == 1 || j.dir == 2 || j.dir == 4) ? j.maps_pool : nullptr;
+      const bool whole = it.bytes == box_bytes && it.valid == box_bytes;
+      if (it.valid) {  // ---- load
+        if ((it.mode & 5) == 1 && maps_s && whole) {  // strided source, whole box: the copy engine gathers it in NHD order
+          if (lane == 0) {
+            mbar_expect_tx(bar, box_bytes);
+            tensor_g2s(sbase, maps_s + (size_t)it.lc * 128, it.s_t, it.s_pg, bar);
+          } else {
+            mbar_arrive(bar);
+          }
+        } else if (it.mode & 1) {  // strided source: 16-byte cp.async row gathers by all lanes
+          const uint32_t nv = it.valid >> 4;
+          for (uint32_t u = lane; u < nv; u += 32)
+            cp_async16(sbase + (u << 4), trans_addr<16>(it.src, true, it.r0, u, upr, j.H, st.s_ts, st.s_hs));
+          cp_async_arrive(bar);
+        } else if (lane == 0) {
+          mbar_expect_tx(bar, it.valid);
+          bulk_g2s(sbase, it.src, it.valid, bar);
+        } else {
+          mbar_arrive(bar);
+        }
+        mbar_wait(bar, phase);
+        phase ^= 1;
+      }
+      // ---- store
+      if ((it.mode & 6) == 2 && maps_d && whole) {  // strided destination, whole box: one tensor store
+        asm volatile("fence.proxy.async.shared::cta;" ::: "memory");  // the stage may hold generic-proxy writes of every lane
+        __syncwarp();
+        if (lane == 0) tensor_s2g(maps_d + (size_t)it.lc * 128, it.d_t, it.d_pg, sbase);
+      } else if (it.mode & 2) {  // strided destination: LDS.128 from the stage, STG.128 to each row's place
+        const uint32_t nb = it.bytes >> 4, nv = it.valid >> 4;
+        for (uint32_t u0 = lane; u0 < nb; u0 += 128) {
+          uint4 v[4];
+#pragma unroll
+          for (int q = 0; q < 4; ++q) {
+            const uint32_t u = u0 + 32 * q;
+            v[q] = make_uint4(0, 0, 0, 0);
+            if (u < nv) v[q] = lds128(sbase + (u << 4));
+          }
+#pragma unroll
+          for (int q = 0; q < 4; ++q) {
+            const uint32_t u = u0 + 32 * q;
+            if (u < nb)
+              st_stream(reinterpret_cast<uint4 *>(trans_addr<16>(it.dst, true, it.r0, u, upr, j.H, st.d_ts, st.d_hs)), v[q]);
+          }
+        }
+      } else {
+        asm volatile("fence.proxy.async.shared::cta;" ::: "memory");
+        __syncwarp();
+        if (lane == 0 && it.valid) bulk_s2g(it.dst, sbase, it.valid);
+        for (uint32_t z = it.valid + (lane << 4); z < it.bytes; z += 512)  // zero-padded tail (a5)
+          st_stream(reinterpret_cast<uint4 *>(it.dst + z), make_uint4(0, 0, 0, 0));
+      }
+      bulk_commit();
+      bulk_wait_read<0>();  // the stage may be refilled (next item of a capped grid) or released (exit)
+      __syncwarp();
+    } else {
+      if (lane == 0 && it.valid) {
+        mbar_expect_tx(bar, it.valid);
+        if (j.l2_hint & 1) bulk_g2s_hint(sbase, it.src, it.valid, bar, pol);
+        else bulk_g2s(sbase, it.src, it.valid, bar);
+        mbar_wait(bar, phase);
+        if (j.l2_hint & 6) bulk_s2g_hint(it.dst, sbase, it.valid, pol_st);
+        else bulk_s2g(it.dst, sbase, it.valid);
+        bulk_commit();
+      }
+      if (it.valid) phase ^= 1;
+      for (uint32_t z = it.valid + (lane << 4); z < it.bytes; z += 512)  // zero-padded tail (a5): plain 16-byte stores
+        st_stream(reinterpret_cast<uint4 *>(it.dst + z), make_uint4(0, 0, 0, 0));
+      if (lane == 0) bulk_wait_read<0>();
+    }
+  }
 }
 
 // ---------------------------------------------------------------------------------------------
@@ -683,7 +816,15 @@ __global__ void __launch_bounds__(256) kv_move_vec(const __grid_constant__ JobT<
 #pragma unroll
       for (int u = 0; u < UNROLL; ++u) st_stream(d + i + 32 * u, v[u]);
     }
-    for (; i < nv; i += 32) st_stream(d + i, ld_stream(s + i));
+    if (i < nv) {  // ragged remainder (copy-on-write pieces): its loads are issued together too, not one by one
+      uint4 v[UNROLL];
+#pragma unroll
+      for (int u = 0; u < UNROLL; ++u)
+        if (i + 32 * u < nv) v[u] = ld_stream(s + i + 32 * u);
+#pragma unroll
+      for (int u = 0; u < UNROLL; ++u)
+        if (i + 32 * u < nv) st_stream(d + i + 32 * u, v[u]);
+    }
     for (i = nv + lane; i < nb; i += 32) st_stream(d + i, make_uint4(0, 0, 0, 0));
   }
 }

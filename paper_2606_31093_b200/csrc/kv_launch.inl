@@ -115,6 +115,20 @@ void launch_bulk(const Job &j, const HostBlob *hb, bool trans, uint32_t grid, ui
   else (void)cudaLaunchKernelEx(&cfg, kvt::kv_move_bulk<N, false>, p);
 }
 template <int N>
+void launch_shot(const Job &j, const HostBlob *hb, bool trans, uint32_t grid, size_t smem, cudaStream_t s, bool pdl) {
+  static thread_local kvt::JobT<N> p;
+  p.j = j;
+  if constexpr (N > 0) std::memcpy(p.blob, hb->bytes.data(), hb->bytes.size());
+  cudaLaunchAttribute attr[1];
+  attr[0].id = cudaLaunchAttributeProgrammaticStreamSerialization;
+  attr[0].val.programmaticStreamSerializationAllowed = 1;
+  cudaLaunchConfig_t cfg = {};
+  cfg.gridDim = dim3(grid); cfg.blockDim = dim3(32); cfg.dynamicSmemBytes = smem; cfg.stream = s;
+  cfg.attrs = attr; cfg.numAttrs = pdl ? 1 : 0;
+  if (trans) (void)cudaLaunchKernelEx(&cfg, kvt::kv_move_shot<N, true>, p);
+  else (void)cudaLaunchKernelEx(&cfg, kvt::kv_move_shot<N, false>, p);
+}
+template <int N>
 void launch_vec(const Job &j, const HostBlob *hb, bool trans, uint32_t grid, cudaStream_t s) {
   static thread_local kvt::JobT<N> p;
   p.j = j;
@@ -161,7 +175,7 @@ int launch(kv_ctx *ctx, const Geom &g, const Blob &b, uint32_t piece_first, uint
     j.q_ts = g.drow; j.q_hs = (uint64_t)g.Tbuf * g.drow;  // dir 2: Tbuf is the source pool's page size
   }
   ctx->last_tma = 0;
-  if (g.tma && g.kernel == KERNEL_BULK) {
+  if (g.tma && is_async_kernel(g.kernel)) {
     j.tb = g.tb;
     if (g.pool_hnd) {
       int rc = get_maps(ctx, g.dst_pool, g.L, g.tb, g.tma_es, &j.maps_pool);
@@ -176,7 +190,16 @@ int launch(kv_ctx *ctx, const Geom &g, const Blob &b, uint32_t piece_first, uint
   }
   uint32_t cap = cta_cap ? cta_cap : ctx->max_ctas;
   uint32_t grid = 0;
-  if (g.kernel == KERNEL_BULK) {
+  if (g.kernel == KERNEL_SHOT) {
+    // one segment per single-warp CTA; the grid is the item list (capped only on request: a CTA then walks its items)
+    j.stage_bytes = (g.sub_bytes + 127) / 128 * 128;
+    j.l2_hint = ctx->l2_hint;
+    grid = (uint32_t)std::min<uint64_t>(total_items, cap ? cap : 0x7fffffffu);
+    const bool pdl = ctx->pdl && !ctx->cur_capturing;
+    if (!b.inl) launch_shot<0>(j, nullptr, g.trans, grid, j.stage_bytes, s, pdl);
+    else if (b.inl->bytes.size() <= kInlineSmall) launch_shot<kInlineSmall>(j, b.inl, g.trans, grid, j.stage_bytes, s, pdl);
+    else launch_shot<kInlineLarge>(j, b.inl, g.trans, grid, j.stage_bytes, s, pdl);
+  } else if (g.kernel == KERNEL_BULK) {
     const bool lane_geom = g.trans && !g.tma;  // row gathers by all lanes want more, shallower warps
     j.stage_bytes = (g.sub_bytes + 127) / 128 * 128;
     j.stages = lane_geom ? ctx->t_stages : ctx->stages; j.lag = std::min(ctx->lag, j.stages - 1);

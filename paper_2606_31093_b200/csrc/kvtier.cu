@@ -86,6 +86,13 @@ cudaError_t ctx_init_device(kv_ctx *ctx, int device) {
                                 (const void *)kvt::kv_move_bulk<kInlineSmall, true>, (const void *)kvt::kv_move_bulk<kInlineLarge, true>};
   for (const void *k : bulk_kernels)
     if ((e = cudaFuncSetAttribute(k, cudaFuncAttributeMaxDynamicSharedMemorySize, ctx->max_smem - kStaticSmemReserve)) != cudaSuccess) return e;
+  const void *shot_kernels[] = {(const void *)kvt::kv_move_shot<0, false>, (const void *)kvt::kv_move_shot<kInlineSmall, false>,
+                                (const void *)kvt::kv_move_shot<kInlineLarge, false>, (const void *)kvt::kv_move_shot<0, true>,
+                                (const void *)kvt::kv_move_shot<kInlineSmall, true>, (const void *)kvt::kv_move_shot<kInlineLarge, true>};
+  for (const void *k : shot_kernels) {  // stages up to 64 KiB (KV_OPT_STAGE_BYTES); as many CTAs per SM as shared memory holds
+    if ((e = cudaFuncSetAttribute(k, cudaFuncAttributeMaxDynamicSharedMemorySize, 65536)) != cudaSuccess) return e;
+    if ((e = cudaFuncSetAttribute(k, cudaFuncAttributePreferredSharedMemoryCarveout, cudaSharedmemCarveoutMaxShared)) != cudaSuccess) return e;
+  }
   {  // cuTensorMapEncodeTiled without linking libcuda; absent -> HND pools keep to the lane paths
     void *fn = nullptr;
     cudaDriverEntryPointQueryResult qr = cudaDriverEntryPointSymbolNotFound;
@@ -157,7 +164,7 @@ int kv_ctx_destroy(kv_ctx *ctx) {
 int kv_ctx_set_option(kv_ctx *ctx, int option, int64_t v) {
   if (!ctx) return KV_ERR_NULL;
   switch (option) {
-    case KV_OPT_KERNEL: if (v < 0 || v > 3) return KV_ERR_SIZE; ctx->kernel = (int)v; break;
+    case KV_OPT_KERNEL: if (v < 0 || v > 4) return KV_ERR_SIZE; ctx->kernel = (int)v; break;
     case KV_OPT_STAGE_BYTES: if (v < 1024 || v > 65536 || v % 16) return KV_ERR_SIZE; ctx->stage_bytes = ctx->t_stage_bytes = (uint32_t)v; ctx->auto_geom = false; break;
     case KV_OPT_STAGES_PER_WARP: if (v < 2 || v > kvt::kMaxStages) return KV_ERR_SIZE; ctx->stages = ctx->t_stages = (uint32_t)v; ctx->auto_geom = false; break;
     case KV_OPT_WARPS: if (v < 1 || v > kvt::kMaxWarps) return KV_ERR_SIZE; ctx->warps = ctx->t_warps = (uint32_t)v; ctx->auto_geom = false; break;
@@ -175,7 +182,7 @@ int kv_ctx_set_option(kv_ctx *ctx, int option, int64_t v) {
       }
       ctx->staging_slots = (uint32_t)v;
       break;
-    case KV_OPT_L2_HINT: if (v < 0 || v > 1) return KV_ERR_SIZE; ctx->l2_hint = (uint32_t)v; break;
+    case KV_OPT_L2_HINT: if (v < 0 || v > 5) return KV_ERR_SIZE; ctx->l2_hint = (uint32_t)v; break;
     case KV_OPT_INLINE_TABLES: if (v < 0 || v > 1) return KV_ERR_SIZE; ctx->inline_tables = (uint32_t)v; break;
     case KV_OPT_DYNAMIC: if (v < 0 || v > 1) return KV_ERR_SIZE; ctx->dynamic = (uint32_t)v; break;
     case KV_OPT_TENSOR_MAPS: if (v < 0 || v > 1) return KV_ERR_SIZE; ctx->tensor_maps = (uint32_t)v; break;

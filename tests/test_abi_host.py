@@ -79,7 +79,7 @@ def test_planning_ctx_never_launches(ctx):
     assert ctx.stat(kv.KV_STAT_LAST_ITEMS) == 49152
     assert ctx.stat(kv.KV_STAT_LAST_PAYLOAD) == 768 << 20
     assert ctx.stat(kv.KV_STAT_LAST_SEGMENT) == 16384
-    assert ctx.stat(kv.KV_STAT_LAST_KERNEL) == kv.KV_KERNEL_BULK
+    assert ctx.stat(kv.KV_STAT_LAST_KERNEL) == kv.KV_KERNEL_SHOT  # AUTO: one 16 KiB segment per single-warp CTA
     assert ctx.stat(kv.KV_STAT_LAUNCHES) == 0 and ctx.stat(kv.KV_STAT_MEMCPYS) == 0
 
 
@@ -196,7 +196,7 @@ def test_plan_fused_repage_and_cow(ctx):
     assert status_of(f) == kv.KV_ERR_NO_DEVICE
     assert ctx.stat(kv.KV_STAT_LAST_ITEMS) == 32 * 32 * 4 * 96  # 16 KiB segments, 4 per 64-token row
     assert ctx.stat(kv.KV_STAT_LAST_PAYLOAD) == 6 << 30
-    assert ctx.stat(kv.KV_STAT_LAST_KERNEL) == kv.KV_KERNEL_BULK
+    assert ctx.stat(kv.KV_STAT_LAST_KERNEL) == kv.KV_KERNEL_SHOT
     # device-resident id lists: nothing is validated on the host (the arrays are never dereferenced here)
     import torch
     fd = lambda: kv.kv_repage_batched(ctx, src, torch.from_numpy(c5.src_ids), c5.src_offsets, dst,
@@ -236,7 +236,7 @@ def test_plan_submit_one_launch_for_a_turn(ctx):
     assert status_of(lambda: kv.kv_submit(ctx, d, s.L, ops, flags=kv.KV_FLAG_VALIDATE)) == kv.KV_ERR_NO_DEVICE
     assert ctx.stat(kv.KV_STAT_LAST_ITEMS) == 100 * 96 + 96 * 2 + 60 * 96
     assert ctx.stat(kv.KV_STAT_LAST_PAYLOAD) == 160 * s.page_bytes + 96 * 12 * 1024
-    assert ctx.stat(kv.KV_STAT_LAST_SEGMENT) == 16384 and ctx.stat(kv.KV_STAT_LAST_KERNEL) == kv.KV_KERNEL_VEC  # 240 MiB: AUTO's mid range
+    assert ctx.stat(kv.KV_STAT_LAST_SEGMENT) == 16384 and ctx.stat(kv.KV_STAT_LAST_KERNEL) == kv.KV_KERNEL_SHOT
     assert ctx.stat(kv.KV_STAT_LAUNCHES) == 0
     # a ragged unpack: n_pages must be ceil(n_tokens / T)
     assert status_of(lambda: kv.kv_submit(ctx, d, s.L, [kv.op_unpack(BUF, dst, 100 * s.T - 16, src_bytes=1 << 40)])) == kv.KV_ERR_SIZE
@@ -272,23 +272,37 @@ def test_plan_hnd_pools(ctx):
         return d
 
     hnd = pool(kv.KV_ORDER_HND)
-    # pack out of an HND pool: strided source -> bulk ring with 4 KiB stages (16 head_dim rows each)
+    # pack out of an HND pool (no tensor maps on a planning ctx): strided source, whole 16 KiB rows per CTA (64 head_dim
+    # rows each, gathered by cp.async)
     assert status_of(lambda: kv.kv_pack(ctx, hnd, s.L, [1, 2, 3], BUF, dst_bytes=1 << 40)) == kv.KV_ERR_NO_DEVICE
-    assert ctx.stat(kv.KV_STAT_LAST_KERNEL) == kv.KV_KERNEL_BULK
-    assert ctx.stat(kv.KV_STAT_LAST_SEGMENT) == 4096
-    assert ctx.stat(kv.KV_STAT_LAST_ITEMS) == 3 * 96 * 4
+    assert ctx.stat(kv.KV_STAT_LAST_KERNEL) == kv.KV_KERNEL_SHOT
+    assert ctx.stat(kv.KV_STAT_LAST_SEGMENT) == 16384
+    assert ctx.stat(kv.KV_STAT_LAST_ITEMS) == 3 * 96
     assert ctx.stat(kv.KV_STAT_LAST_PAYLOAD) == 3 * s.page_bytes
-    # unpack into an HND pool: strided destination -> vec kernel, whole 16 KiB rows
-    assert status_of(lambda: kv.kv_unpack(ctx, BUF, [1, 2, 3], hnd, s.L, 16, 16, 48, src_bytes=1 << 40)) == kv.KV_ERR_NO_DEVICE
-    assert ctx.stat(kv.KV_STAT_LAST_KERNEL) == kv.KV_KERNEL_VEC
+    ctx.set_option(kv.KV_OPT_KERNEL, kv.KV_KERNEL_BULK)  # the ring's transposing geometry: 4 KiB stages (16 rows each)
+    assert status_of(lambda: kv.kv_pack(ctx, hnd, s.L, [1, 2, 3], BUF, dst_bytes=1 << 40)) == kv.KV_ERR_NO_DEVICE
+    assert ctx.stat(kv.KV_STAT_LAST_KERNEL) == kv.KV_KERNEL_BULK and ctx.stat(kv.KV_STAT_LAST_SEGMENT) == 4096
+    assert ctx.stat(kv.KV_STAT_LAST_ITEMS) == 3 * 96 * 4
+    ctx.set_option(kv.KV_OPT_KERNEL, kv.KV_KERNEL_AUTO)
+    # unpack into an HND pool: strided destination, 16-byte stores from the stage
+    assert status_of(lambda: kv.kv_unpack(ctx, BUF, np.arange(10), hnd, s.L, 16, 16, 160, src_bytes=1 << 40)) == kv.KV_ERR_NO_DEVICE
+    assert ctx.stat(kv.KV_STAT_LAST_KERNEL) == kv.KV_KERNEL_SHOT
     assert ctx.stat(kv.KV_STAT_LAST_SEGMENT) == 16384
     # pool -> pool: HND -> NHD is a strided source, NHD -> HND a strided destination
     nhd64 = pool(kv.KV_ORDER_NHD, s.with_(T=64, P=64), base0=0x7800_0000_0000)
     hnd64 = pool(kv.KV_ORDER_HND, s.with_(T=64, P=64), base0=0x7800_0000_0000)
     assert status_of(lambda: kv.kv_repage(ctx, hnd, np.arange(8), nhd64, [0, 1], s.L, 128)) == kv.KV_ERR_NO_DEVICE
-    assert ctx.stat(kv.KV_STAT_LAST_KERNEL) == kv.KV_KERNEL_BULK
+    assert ctx.stat(kv.KV_STAT_LAST_KERNEL) == kv.KV_KERNEL_SHOT
     assert status_of(lambda: kv.kv_repage(ctx, pool(0), np.arange(8), hnd64, [0, 1], s.L, 128)) == kv.KV_ERR_NO_DEVICE
-    assert ctx.stat(kv.KV_STAT_LAST_KERNEL) == kv.KV_KERNEL_VEC
+    assert ctx.stat(kv.KV_STAT_LAST_KERNEL) == kv.KV_KERNEL_SHOT
+    # short segments keep the earlier choices: 2 KiB token rows of a one-token-per-chunk re-page (5 -> 7) go to the ring,
+    # 1 KiB segments to kv_move_small (vec) once the call is large enough
+    s2 = W.QWEN3_OMNI.with_(T=7, H=8, P=4096)
+    assert status_of(lambda: kv.kv_unpack(ctx, BUF, np.arange(100), fake_pool(s2), s2.L, 5, 7, 700, src_bytes=1 << 40)) == kv.KV_ERR_NO_DEVICE
+    assert ctx.stat(kv.KV_STAT_LAST_SEGMENT) == 2048 and ctx.stat(kv.KV_STAT_LAST_KERNEL) == kv.KV_KERNEL_BULK
+    s1 = W.QWEN3_OMNI.with_(T=7, P=4096)
+    assert status_of(lambda: kv.kv_unpack(ctx, BUF, np.arange(100), fake_pool(s1), s1.L, 5, 7, 700, src_bytes=1 << 40)) == kv.KV_ERR_NO_DEVICE
+    assert ctx.stat(kv.KV_STAT_LAST_SEGMENT) == 1024 and ctx.stat(kv.KV_STAT_LAST_KERNEL) == kv.KV_KERNEL_VEC
     # head_dim rows that are not multiples of 16 bytes: element-wise kernel, never rejected
     odd = pool(kv.KV_ORDER_HND, s.with_(D=20))
     assert status_of(lambda: kv.kv_pack(ctx, odd, s.L, [1], BUF, dst_bytes=1 << 40)) == kv.KV_ERR_NO_DEVICE
@@ -296,7 +310,7 @@ def test_plan_hnd_pools(ctx):
     # one head: [token][head] == [head][token]; planned as the contiguous copy it is
     one = pool(kv.KV_ORDER_HND, s.with_(H=1))
     assert status_of(lambda: kv.kv_unpack(ctx, BUF, [1], one, s.L, 16, 16, 16, src_bytes=1 << 40)) == kv.KV_ERR_NO_DEVICE
-    assert ctx.stat(kv.KV_STAT_LAST_KERNEL) == kv.KV_KERNEL_BULK
+    assert ctx.stat(kv.KV_STAT_LAST_KERNEL) == kv.KV_KERNEL_SHOT
     assert ctx.stat(kv.KV_STAT_LAST_SEGMENT) == 4096  # the whole 4 KiB row
     assert status_of(lambda: kv.kv_pack(ctx, pool(2), s.L, [1], BUF, dst_bytes=1 << 40)) == kv.KV_ERR_DESC
 

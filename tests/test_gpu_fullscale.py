@@ -65,7 +65,7 @@ def test_config2_single_prefix_pack_offload_reload(kv, ctx, pool):
     want = ko.pack(mini, np.arange(n), threads=THREADS)
     buf = torch.zeros(nbytes, dtype=torch.uint8, device="cuda")
     kv.kv_pack(ctx, desc, shape.L, case.src_ids, buf)
-    assert ctx.stat(kv.KV_STAT_LAST_KERNEL) == kv.KV_KERNEL_BULK and ctx.stat(kv.KV_STAT_LAST_GRID) == 148
+    assert ctx.stat(kv.KV_STAT_LAST_KERNEL) == kv.KV_KERNEL_SHOT and ctx.stat(kv.KV_STAT_LAST_GRID) == 512 * 96
     assert np.array_equal(buf.cpu().numpy(), want), "kv_pack != oracle at full scale"
     hp = kv.kv_host_alloc(nbytes)
     try:
@@ -268,7 +268,7 @@ def test_config5_cross_role_repage(kv, ctx, pool, ragged):
     before = page_checksums(torch, dst_slabs, s_dst)
     launches = ctx.stat(kv.KV_STAT_LAUNCHES)
     kv.kv_repage_batched(ctx, d_src, c5.src_ids, c5.src_offsets, d_dst, dids2, c5.dst_offsets, c5.n_tokens, s_dst.L)
-    assert ctx.stat(kv.KV_STAT_LAUNCHES) == launches + 1 and ctx.stat(kv.KV_STAT_LAST_GRID) == 148
+    assert ctx.stat(kv.KV_STAT_LAUNCHES) == launches + 1 and ctx.stat(kv.KV_STAT_LAST_GRID) == 32 * 32 * 4 * 96
     torch.cuda.synchronize()
     assert_untouched(before, page_checksums(torch, dst_slabs, s_dst), dids2, s_dst.P)
     for r in range(0, R, 5):
@@ -306,7 +306,7 @@ def test_cow_tail_pages_of_64_sessions(kv, ctx, pool):
     before = page_checksums(torch, slabs, shape)
     kv.kv_cow_append_batched(ctx, desc, shape.L, old, new, n_old, n_app, apps, flags=kv.KV_FLAG_VALIDATE)
     torch.cuda.synchronize()
-    assert ctx.stat(kv.KV_STAT_LAST_KERNEL) == kv.KV_KERNEL_VEC  # AUTO: ragged ~6 KiB pieces, >= 16 MiB in all
+    assert ctx.stat(kv.KV_STAT_LAST_KERNEL) == kv.KV_KERNEL_SHOT  # AUTO: one ragged piece per single-warp CTA
     assert_untouched(before, page_checksums(torch, slabs, shape), new, shape.P)
     ko.cow_append_batched(mini, np.arange(S), np.arange(S, 2 * S), n_old, n_app, apps_h)
     got = snapshot_pages(torch, slabs, touched, shape)

@@ -1,6 +1,6 @@
 """Seeded random cases of every transfer against the CPU oracle, byte for byte: random shapes, page
 sizes on both sides, in-page orders, buffer layouts, strides with padding, ragged token counts, CSR
-batches with empty requests, every kernel choice (AUTO / bulk / vec / elem), tensor maps on and off,
+batches with empty requests, every kernel choice (AUTO / bulk ring / vec / elem / shot), tensor maps on and off,
 PDL / dynamic claiming / inline tables on and off, stage sizes and warp counts of the bulk ring.
 The directed cases live in test_gpu_parity / test_gpu_next / test_gpu_hnd; this file is the net under
 them: each seed draws one configuration and runs pack -> unpack (re-paged) -> fused re-page ->
@@ -34,7 +34,7 @@ def draw(rng):
     pad_unit = int(rng.choice([0, 0, e, 16, 256]))
     return dict(e=e, D=D, H=H, Ts=Ts, Td=Td, L=L, C=C, pad=pad_unit,
                 order_s=int(rng.integers(0, 2)), order_d=int(rng.integers(0, 2)),
-                layout=int(rng.integers(0, 2)), kernel=int(rng.choice([0, 0, 1, 2, 3])),
+                layout=int(rng.integers(0, 2)), kernel=int(rng.choice([0, 0, 1, 2, 3, 4, 4])),
                 tensor_maps=int(rng.integers(0, 2)), R=int(rng.integers(1, 5)),
                 pdl=int(rng.integers(0, 2)), dynamic=int(rng.integers(0, 2)), inline=int(rng.integers(0, 2)),
                 stage=int(rng.choice([16384, 16384, 4096, 1024, 8192])), warps=int(rng.choice([2, 2, 1, 4])),

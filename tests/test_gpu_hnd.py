@@ -32,7 +32,7 @@ def ctx(kv, request):
     c.close()
 
 
-KERNELS = {"bulk": 1, "vec": 2, "elem": 3}
+KERNELS = {"bulk": 1, "vec": 2, "elem": 3, "shot": 4}
 HND = ko.HND
 
 SHAPES = [  # L, C, P, T, H, D, e, pad, n
@@ -51,6 +51,8 @@ def want_kernel(kernel, H, D, e):
     if (D * e) % 16:
         return KERNELS["elem"]
     if kernel == "bulk" and D * e > 4096:  # a head_dim row must fit one (4 KiB) stage of the transposing ring
+        return KERNELS["vec"]
+    if kernel == "shot" and D * e > 16384:  # ... or the one 16 KiB stage of a shot CTA
         return KERNELS["vec"]
     return KERNELS[kernel]
 
@@ -210,21 +212,21 @@ def test_auto_with_tensor_maps_is_one_bulk_kernel(kv, ctx):
     buf = torch.zeros(n * dA.page_bytes(), dtype=torch.uint8, device="cuda")
     for _ in range(2):
         kv.kv_pack(ctx, dA, L, ids, buf)
-        assert ctx.stat(kv.KV_STAT_LAST_KERNEL) == KERNELS["bulk"]
+        assert ctx.stat(kv.KV_STAT_LAST_KERNEL) == KERNELS["shot"]
         assert ctx.stat(kv.KV_STAT_LAST_TENSOR_MAPS) == 1
         assert ctx.stat(kv.KV_STAT_LAST_SEGMENT) == 8192  # 120 rows of 16 KiB split once to cover the chip
     want = ko.pack(A, ids)
     assert np.array_equal(buf.cpu().numpy(), want)
     kv.kv_unpack(ctx, buf, ids[::-1].copy(), dA, L, T, T, n * T)
-    assert ctx.stat(kv.KV_STAT_LAST_KERNEL) == KERNELS["bulk"] and ctx.stat(kv.KV_STAT_LAST_TENSOR_MAPS) == 1
+    assert ctx.stat(kv.KV_STAT_LAST_KERNEL) == KERNELS["shot"] and ctx.stat(kv.KV_STAT_LAST_TENSOR_MAPS) == 1
     ko.unpack(want, ids[::-1].copy(), A, Ts=T, n_tokens=n * T)
     assert_pool_equal(tA, A)
     kv.kv_repage(ctx, dA, ids, dN, ids, L, n * T)
-    assert ctx.stat(kv.KV_STAT_LAST_KERNEL) == KERNELS["bulk"] and ctx.stat(kv.KV_STAT_LAST_TENSOR_MAPS) == 1
+    assert ctx.stat(kv.KV_STAT_LAST_KERNEL) == KERNELS["shot"] and ctx.stat(kv.KV_STAT_LAST_TENSOR_MAPS) == 1
     ko.repage(A, ids, N, ids, n_tokens=n * T)
     assert_pool_equal(tN, N)
     kv.kv_repage(ctx, dN, ids, dA, ids, L, n * T)
-    assert ctx.stat(kv.KV_STAT_LAST_KERNEL) == KERNELS["bulk"] and ctx.stat(kv.KV_STAT_LAST_TENSOR_MAPS) == 1
+    assert ctx.stat(kv.KV_STAT_LAST_KERNEL) == KERNELS["shot"] and ctx.stat(kv.KV_STAT_LAST_TENSOR_MAPS) == 1
     ko.repage(N, ids, A, ids, n_tokens=n * T)
     assert_pool_equal(tA, A)
     kv.kv_pack(ctx, dN, L, ids, buf)  # NHD pool: nothing to transpose, no maps
@@ -232,8 +234,10 @@ def test_auto_with_tensor_maps_is_one_bulk_kernel(kv, ctx):
 
 
 def test_auto_kernel_choice_per_direction(kv, ctx):
-    """AUTO without tensor maps: strided source only -> bulk ring (cp.async gather +
-    bulk store); strided destination -> vec (16-byte STG from many warps); NHD <-> NHD stays on the bulk path."""
+    """AUTO without tensor maps: with segments of 4 KiB or more every direction takes
+    kv_move_shot (strided source: cp.async row gathers into the CTA's stage; strided destination: 16-byte stores from
+    it); a pool whose whole rows are shorter keeps the earlier choices -- strided source only -> bulk ring, strided
+    destination -> vec."""
     L, C, P, T, H, D, e, n = 3, 2, 64, 16, 4, 128, 2, 20
     rng = np.random.default_rng(79)
     ctx.set_option(kv.KV_OPT_TENSOR_MAPS, 0)
@@ -244,21 +248,33 @@ def test_auto_kernel_choice_per_direction(kv, ctx):
     ids = rng.choice(P, n, replace=False).astype(np.int32)
     buf = torch.zeros(n * dA.page_bytes(), dtype=torch.uint8, device="cuda")
     kv.kv_pack(ctx, dA, L, ids, buf)
-    assert ctx.stat(kv.KV_STAT_LAST_KERNEL) == KERNELS["bulk"]
-    assert ctx.stat(kv.KV_STAT_LAST_SEGMENT) == 4096
+    assert ctx.stat(kv.KV_STAT_LAST_KERNEL) == KERNELS["shot"]
+    assert ctx.stat(kv.KV_STAT_LAST_SEGMENT) == 8192  # 120 rows of 16 KiB split once to cover the chip
     want = ko.pack(A, ids)
     assert np.array_equal(buf.cpu().numpy(), want)
     kv.kv_unpack(ctx, buf, ids[::-1].copy(), dA, L, T, T, n * T)
-    assert ctx.stat(kv.KV_STAT_LAST_KERNEL) == KERNELS["vec"]
+    assert ctx.stat(kv.KV_STAT_LAST_KERNEL) == KERNELS["shot"]
     ko.unpack(want, ids[::-1].copy(), A, Ts=T, n_tokens=n * T)
     assert_pool_equal(tA, A)
     kv.kv_repage(ctx, dA, ids, dN, ids, L, n * T)  # HND -> NHD pool: strided source only
-    assert ctx.stat(kv.KV_STAT_LAST_KERNEL) == KERNELS["bulk"]
+    assert ctx.stat(kv.KV_STAT_LAST_KERNEL) == KERNELS["shot"]
     ko.repage(A, ids, N, ids, n_tokens=n * T)
     assert_pool_equal(tN, N)
     kv.kv_repage(ctx, dN, ids, dA, ids, L, n * T)  # NHD -> HND pool: strided destination
-    assert ctx.stat(kv.KV_STAT_LAST_KERNEL) == KERNELS["vec"]
+    assert ctx.stat(kv.KV_STAT_LAST_KERNEL) == KERNELS["shot"]
     ko.repage(N, ids, A, ids, n_tokens=n * T)
     assert_pool_equal(tA, A)
     kv.kv_pack(ctx, dN, L, ids, buf)
+    assert ctx.stat(kv.KV_STAT_LAST_KERNEL) == KERNELS["shot"]
+    # short rows (4 tokens x 2 heads x 128 B = 1 KiB per row): the earlier choices
+    S = host_pool(rng, L, C, P, 4, 2, 64, 2, order=HND)
+    tS, dS = to_device(S, kv, torch)
+    sbuf = torch.zeros(n * dS.page_bytes(), dtype=torch.uint8, device="cuda")
+    kv.kv_pack(ctx, dS, L, ids, sbuf)
     assert ctx.stat(kv.KV_STAT_LAST_KERNEL) == KERNELS["bulk"]
+    wants = ko.pack(S, ids)
+    assert np.array_equal(sbuf.cpu().numpy(), wants)
+    kv.kv_unpack(ctx, sbuf, ids[::-1].copy(), dS, L, 4, 4, n * 4)
+    assert ctx.stat(kv.KV_STAT_LAST_KERNEL) == KERNELS["vec"]
+    ko.unpack(wants, ids[::-1].copy(), S, Ts=4, n_tokens=n * 4)
+    assert_pool_equal(tS, S)

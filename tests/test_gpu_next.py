@@ -27,7 +27,7 @@ def ctx(kv):
     c.close()
 
 
-KERNELS = {"bulk": 1, "vec": 2, "elem": 3}
+KERNELS = {"bulk": 1, "vec": 2, "elem": 3, "shot": 4}
 
 
 @pytest.mark.parametrize("kernel", KERNELS)
@@ -757,22 +757,28 @@ def test_cow_append_with_device_resident_ids(kv, ctx):
 @pytest.mark.parametrize("H", [1, 2])
 def test_narrow_rows_of_a_head_partition(kv, ctx, H, order):
     """A tensor-parallel rank holds its own head partition of every page: 1 or 2 KV heads =
-    4 / 8 KiB rows.  With default options and enough segments the bulk ring re-shapes itself (8 x 4 or 4 x 4
-    stages instead of 2 x 4: bytes in flight per SM stay ~128 KiB).  Same bytes as the oracle, NHD and HND."""
+    4 / 8 KiB rows: one row per single-warp CTA (kv_move_shot); with KV_OPT_KERNEL = bulk and enough segments the ring
+    re-shapes itself (8 x 4 or 4 x 4 stages instead of 2 x 4).  Same bytes as the oracle, NHD and HND."""
     L, C, P, T, D, e = 48, 2, 160, 16, 128, 2
     rng = np.random.default_rng(181 + H + 2 * order)
     A = host_pool(rng, L, C, P, T, H, D, e, order=order)
     B = host_pool(rng, L, C, P, T, H, D, e, order=order)
     tA, dA = to_device(A, kv, torch)
     tB, dB = to_device(B, kv, torch)
-    n = 64 if H == 1 else 40  # x 96 slabs = 6,144 / 3,840 segments: enough for the re-shaped ring, < 40 MiB (bulk)
+    n = 64 if H == 1 else 40  # x 96 slabs = 6,144 / 3,840 segments: enough for the re-shaped ring
     src = rng.choice(P, n, replace=False).astype(np.int32)
     dst = rng.permutation(P)[:n].astype(np.int32)
     buf = torch.zeros(n * dA.page_bytes(), dtype=torch.uint8, device="cuda")
     kv.kv_pack(ctx, dA, L, src, buf)
-    assert ctx.stat(kv.KV_STAT_LAST_KERNEL) == kv.KV_KERNEL_BULK and ctx.stat(kv.KV_STAT_LAST_SEGMENT) == 4096 * H
+    assert ctx.stat(kv.KV_STAT_LAST_KERNEL) == kv.KV_KERNEL_SHOT and ctx.stat(kv.KV_STAT_LAST_SEGMENT) == 4096 * H
     want = ko.pack(A, src)
     assert np.array_equal(buf.cpu().numpy(), want)
+    ctx.set_option(kv.KV_OPT_KERNEL, kv.KV_KERNEL_BULK)  # the re-shaped ring moves the same bytes
+    buf.zero_()
+    kv.kv_pack(ctx, dA, L, src, buf)
+    assert ctx.stat(kv.KV_STAT_LAST_KERNEL) == kv.KV_KERNEL_BULK and ctx.stat(kv.KV_STAT_LAST_SEGMENT) == 4096 * H
+    assert np.array_equal(buf.cpu().numpy(), want)
+    ctx.set_option(kv.KV_OPT_KERNEL, kv.KV_KERNEL_AUTO)
     kv.kv_unpack(ctx, buf, dst, dB, L, T, T, n * T - 5, flags=kv.KV_FLAG_VALIDATE)
     ko.unpack(want, dst, B, Ts=T, n_tokens=n * T - 5)
     assert_pool_equal(tB, B)

@@ -30,7 +30,7 @@ def ctx(kv):
     c.close()
 
 
-KERNELS = {"bulk": 1, "vec": 2, "elem": 3}
+KERNELS = {"bulk": 1, "vec": 2, "elem": 3, "shot": 4}
 
 # L, C, P, T, H, D, e, pad
 SHAPES = [

@@ -28,7 +28,7 @@ def ctx(kv):
     c.close()
 
 
-KERNELS = {"auto": 0, "bulk": 1, "vec": 2, "elem": 3}
+KERNELS = {"auto": 0, "bulk": 1, "vec": 2, "elem": 3, "shot": 4}
 
 
 # ------------------------------------------------------------------------------------------------
