@@ -72,6 +72,9 @@ def parse():
                     help="in-page order of the pool (BASELINE.json configs are NHD; hnd = the NEXT-2 transposing transfers)")
     ap.add_argument("--host-mode", default="auto", choices=["auto", "direct", "staged"],
                     help="kv_host_mode of the host-tier legs (auto = the library's measured choice)")
+    ap.add_argument("--kernel", default="auto", choices=["auto", "bulk", "vec", "shot"],
+                    help="KV_OPT_KERNEL of every ctx (auto = the library's measured choice; the others reproduce the A/B "
+                         "figures of DESIGN.md: bulk = the persistent ring, shot = one segment per single-warp CTA)")
     ap.add_argument("--seed", type=int, default=0)
     return ap.parse_args()
 
@@ -154,7 +157,7 @@ def bench_config(args, shape):
                     "80 % bar is hardest on among those that are bandwidth-bound (768 MiB per call; configs[3] 26.5 GiB and "
                     "configs[4] 6 GiB run at 1.00-1.02 of the same peak and are carried in per_config, configs[0] is launch-bound)",
         "layers": shape.L, "kv_heads": shape.H, "head_dim": shape.D, "page_size": shape.T,
-        "pool_order": args.pool_order, "pool_pages": args.pool_pages,
+        "pool_order": args.pool_order, "pool_pages": args.pool_pages, "kernel": args.kernel,
         "pool_GiB": round(shape.L * shape.C * args.pool_pages * shape.row_bytes / 2**30, 1),
         "payload_MiB": n * shape.page_bytes / 2**20, "pages_per_step": n, "parallelism": "replicas only",
         "l2": "inputs larger than L2 (768 MiB per op, fresh page ids per step; unpack reads the buffer packed one step earlier)",
@@ -348,6 +351,8 @@ def run_ours(args):
         dst_ids.append(perm[n:].copy())
 
     ctx = kv.Ctx(local)
+    kopt = {"auto": kv.KV_KERNEL_AUTO, "bulk": kv.KV_KERNEL_BULK, "vec": kv.KV_KERNEL_VEC, "shot": kv.KV_KERNEL_SHOT}[args.kernel]
+    ctx.set_option(kv.KV_OPT_KERNEL, kopt)
     stream = torch.cuda.current_stream()
     kv.kv_pack(ctx, desc, shape.L, src_ids[-1], bufs[1])  # buffer read by the first unpack
 
@@ -418,6 +423,7 @@ def run_ours(args):
         host_mode = {1: "direct", 2: "staged"}.get(ctx.stat(kv.KV_STAT_LAST_HOST_MODE), "?")
 
         ctx2 = kv.Ctx(local)  # its own staging, side stream and events: the two directions share nothing
+        ctx2.set_option(kv.KV_OPT_KERNEL, kopt)
         s_off, s_rel = torch.cuda.Stream(), torch.cuda.Stream()
 
         def duplex_step(i):
@@ -519,8 +525,10 @@ def run_ours(args):
             "offload": {"achieved": off_g, "peak": link["d2h_GBps"], "frac": off_g / link["d2h_GBps"]},
             "reload": {"achieved": rel_g, "peak": link["h2d_GBps"], "frac": rel_g / link["h2d_GBps"]},
             "duplex": {"achieved": dup_g, "peak": link["duplex_GBps"], "frac": dup_g / link["duplex_GBps"],
+                       "frac_of_chunked_memcpy": dup_g / link["duplex_chunked_GBps"],
                        "what": "the e2e leg (offload and reload at once, host sync every step) against D2H + H2D "
-                               "cudaMemcpyAsync at once"},
+                               "cudaMemcpyAsync at once (one copy each way); frac_of_chunked_memcpy = against the same plain "
+                               "copies issued as two per direction, the chunking of a staged 768 MiB transfer"},
             "duplex_no_host_sync": dup_nosync,
             "peaks": link, "host_mode": host_mode,
         }

@@ -153,8 +153,8 @@ class Checker:
         return True
 
 
-def link_peaks(torch, nbytes=1 << 30, reps=10):
-    """Pinned cudaMemcpyAsync peaks of the host link, measured here and now (>= 1 GiB, best of 10, each
+def link_peaks(torch, nbytes=1 << 30, reps=20):
+    """Pinned cudaMemcpyAsync peaks of the host link, measured here and now (>= 1 GiB, best of 20, each
     direction) + both directions at once on two streams."""
     a = torch.empty(nbytes, dtype=torch.uint8, device="cuda")
     b = torch.empty(nbytes, dtype=torch.uint8, device="cuda")
@@ -181,37 +181,63 @@ def link_peaks(torch, nbytes=1 << 30, reps=10):
 
     _, t = _events(torch, both, reps, 2)
     duplex = 2 * nbytes / t / 1e3
+    # the same bytes as TWO back-to-back copies per direction (the chunking of a staged 768 MiB transfer): with both
+    # directions busy every copy boundary costs the link ~0.25 ms on this platform, for plain cudaMemcpyAsync too
+    K = 2
+    c = nbytes // K // 4096 * 4096
+
+    def both3():
+        cur = torch.cuda.current_stream()
+        sa.wait_stream(cur)
+        sb.wait_stream(cur)
+        with torch.cuda.stream(sa):
+            for i in range(K):
+                h[i * c:(i + 1) * c].copy_(a[i * c:(i + 1) * c], non_blocking=True)
+        with torch.cuda.stream(sb):
+            for i in range(K):
+                b[i * c:(i + 1) * c].copy_(h2[i * c:(i + 1) * c], non_blocking=True)
+        cur.wait_stream(sa)
+        cur.wait_stream(sb)
+
+    _, t = _events(torch, both3, reps, 2)
+    duplex3 = 2 * K * c / t / 1e3
     del a, b, h, h2
-    return {"h2d_GBps": h2d, "d2h_GBps": d2h, "duplex_GBps": duplex, "bytes": nbytes, "reps": reps,
+    return {"h2d_GBps": h2d, "d2h_GBps": d2h, "duplex_GBps": duplex, "duplex_chunked_GBps": duplex3, "duplex_chunked_copies_each_way": K,
+            "bytes": nbytes, "reps": reps,
             "how": "pinned cudaMemcpyAsync (torch copy_ non_blocking), best of reps, CUDA events; duplex = D2H and H2D "
-                   "of the same size on two streams, 2*bytes / time"}
+                   "of the same size on two streams, 2*bytes / time; duplex_chunked = the same bytes issued as "
+                   "two back-to-back copies per direction (what chunking alone costs plain copies when both directions are busy)"}
 
 
-def empty_launch_us(torch, ctx, reps=20):
-    """What the cheapest launch of this library costs between two events (kv_signal: one thread, one store), issued
-    through the same binding as the transfers: host-inclusive and gated (device only)."""
+def empty_launch_us(torch, reps=30):
+    """What a launch that moves nothing costs between two events on this box: a one-element torch fill_ (a store-only
+    kernel of one thread), after the same L2 flush as the sweep's calls.  With the flush kernels queued ahead the host
+    has issued everything before the GPU gets there, so this is device time: event -> launch -> event."""
     flag = torch.zeros(1, dtype=torch.int64, device="cuda")
-    med, _ = _events(torch, lambda: kv.kv_signal(ctx, flag, 1), reps, 3)
-    med_q, _ = _events(torch, lambda: kv.kv_signal(ctx, flag, 1), reps, 3, gate=True)
-    return med, med_q
+    flush = (torch.empty(64 << 20, dtype=torch.uint8, device="cuda"), torch.zeros(64 << 20, dtype=torch.uint8, device="cuda"))
+    med, _ = _events(torch, lambda: flag.fill_(1), reps, 3, flush)
+    return med
 
 
-def sweep_row(torch, ctx, desc, shape, chk, buf, flush, npg, rng, hbm, t_launch, t_launch_q, layers=32, reps=None):
-    """One point of the transfer-size sweep (pack of npg pages of `layers` layers = npg MiB): isolated call, host cost
-    inside (`us`) and gated (`us_queued`), against the floor launch + 2*payload/peak."""
+def sweep_row(torch, ctx, desc, shape, chk, buf, src, flush, npg, rng, hbm, t_launch, layers=32, reps=None):
+    """One point of the transfer-size sweep (pack of npg pages of `layers` layers = npg MiB): isolated call on a cold,
+    clean L2 (the flush kernels are queued ahead of it, so the host's cost of issuing the call is hidden: device time),
+    against (a) the floor empty launch + 2*payload/peak and (b) a plain contiguous copy of the same bytes (torch copy_
+    = cudaMemcpyAsync device to device, `src` -> `buf`) timed the same way: what the hardware gives a transfer of that
+    size when nothing has to be gathered."""
     pg = layers * shape.C * shape.row_bytes
     pls = npg * pg
     ids = rng.choice(shape.P, npg, replace=False).astype(np.int32)
     reps = reps or (20 if pls <= (256 << 20) else 7)
     fl_ = flush if pls <= FLUSH_UP_TO else None
+    cm, _ = _events(torch, lambda: buf[:pls].copy_(src[:pls]), reps, 2, fl_)
     buf[:pls].fill_(0xEE)
     m, bst = _events(torch, lambda: kv.kv_pack(ctx, desc, layers, ids, buf), reps, 2, fl_)
-    mq, _ = _events(torch, lambda: kv.kv_pack(ctx, desc, layers, ids, buf), reps, 1, fl_, gate=True)
-    floor, floor_q = t_launch + 2 * pls / hbm / 1e3, t_launch_q + 2 * pls / hbm / 1e3
-    return {"MiB": pls >> 20, "n_pages": int(npg), "pack_us": m, "pack_us_best": bst, "pack_us_queued": mq,
-            "pack_GBps": 2 * pls / m / 1e3, "pack_GBps_queued": 2 * pls / mq / 1e3,
-            "pack_frac_hbm": 2 * pls / m / 1e3 / hbm, "pack_frac_hbm_queued": 2 * pls / mq / 1e3 / hbm,
-            "floor_us": floor, "vs_floor": m / floor, "floor_us_queued": floor_q, "vs_floor_queued": mq / floor_q,
+    floor = t_launch + 2 * pls / hbm / 1e3
+    return {"MiB": pls >> 20, "n_pages": int(npg), "pack_us": m, "pack_us_best": bst,
+            "pack_GBps": 2 * pls / m / 1e3, "pack_frac_hbm": 2 * pls / m / 1e3 / hbm,
+            "floor_us": floor, "vs_floor": m / floor,
+            "plain_copy_us": cm, "plain_copy_frac_hbm": 2 * pls / cm / 1e3 / hbm, "vs_plain_copy": m / cm,
             "kernel": {1: "bulk", 2: "vec", 3: "elem", 4: "shot"}.get(ctx.stat(kv.KV_STAT_LAST_KERNEL), "?"),
             "bit_exact": bool(chk.pack_ok(buf, ids, layers=layers)), "_ids": ids}
 
@@ -336,19 +362,20 @@ def compact(ctx, desc, shape, slabs, seed, hbm_peak):
         three_calls_us=us3, three_calls_launches=(l1 - l0) // 9)
 
     # ---- six points of the 1 MiB - 8 GiB sweep (layer_count 32 => 1 MiB pages), isolated calls -------------------
-    t_launch, t_launch_q = empty_launch_us(torch, ctx)
+    t_launch = empty_launch_us(torch)
     sweep = []
     for npg in (1, 16, 64, 256, 1024, 8192):
-        r = sweep_row(torch, ctx, desc, shape, chk, big, flush, npg, rng, hbm_peak, t_launch, t_launch_q)
+        r = sweep_row(torch, ctx, desc, shape, chk, big, big[13 << 30:], flush, npg, rng, hbm_peak, t_launch)
         r.pop("_ids")
         sweep.append(r)
     del big, bufs, flush
-    return {"records": out, "sweep": sweep, "empty_launch_us": t_launch, "empty_launch_us_queued": t_launch_q,
+    return {"records": out, "sweep": sweep, "empty_launch_us": t_launch,
             "check": f"bit_exact: torch index_select / reshape compare of ALL pages on every {LC_STEP}th (layer,K|V) slab, "
                      "destinations poisoned before the timed calls",
             "timing": "records: calls issued back to back between two CUDA events (us per call); sweep and the kv_submit "
-                      "turn: isolated calls on a cold, clean L2 (host cost of the call inside `us`; `us_queued` = the same "
-                      "call queued behind a 200 us spin kernel, i.e. device time only); floor = empty launch + 2*payload/peak"}
+                      "turn: isolated calls on a cold, clean L2 (the flush kernels are queued ahead of the call, so the host's cost "
+                      "of issuing it is hidden: device time); floor = empty launch (one-element fill_) + 2*payload/peak; "
+                      "plain_copy = torch copy_ (cudaMemcpyAsync D2D) of the same bytes, contiguous, timed the same way"}
 
 
 # ------------------------------------------------------------------------------------------------
@@ -790,10 +817,11 @@ def run(ctx, desc, shape, slabs, seed=0, out_dir="gpurun_out", hbm_peak=None):
         pg = Ls * shape.C * row
         sweep = []
         bufS = torch.empty(8 << 30, dtype=torch.uint8, device="cuda")
-        t_launch, t_launch_q = empty_launch_us(torch, ctx)
-        peaks["empty_launch_us"], peaks["empty_launch_us_queued"] = t_launch, t_launch_q
+        srcS = torch.empty(8 << 30, dtype=torch.uint8, device="cuda")
+        t_launch = empty_launch_us(torch)
+        peaks["empty_launch_us"] = t_launch
         for npg in W.sweep_sizes_pages():
-            row_ = sweep_row(torch, ctx, desc, shape, chk, bufS, flush, npg, rng, hbm, t_launch, t_launch_q, layers=Ls)
+            row_ = sweep_row(torch, ctx, desc, shape, chk, bufS, srcS, flush, npg, rng, hbm, t_launch, layers=Ls)
             ids = row_.pop("_ids")
             ok = row_.pop("bit_exact")
             dst = rng.choice(shape.P, npg, replace=False).astype(np.int32)
@@ -836,7 +864,7 @@ def run(ctx, desc, shape, slabs, seed=0, out_dir="gpurun_out", hbm_peak=None):
             row_["reload_pct_link_peak"] = 100 * row_["reload_GBps"] / h2d
             row_["verified"] = bool(ok)
             sweep.append(row_)
-        del bufS
+        del bufS, srcS
         first80 = next((r["MiB"] for r in sweep if r["pack_pct_hbm_peak"] >= 80), None)
         recs.append({"config": "5 sweep", "op": "1 MiB - 8 GiB, layer_count 32", "rows": sweep,
                      "smallest_MiB_reaching_80pct_hbm_pack": first80,
@@ -883,8 +911,7 @@ def markdown(rep: dict) -> str:
     out = [f"Peaks measured in the same run: D2D copy {pk['hbm_copy_GBps_this_run']:.0f} GB/s (read+write), pinned H2D "
            f"{pk['h2d_GBps']:.1f} GB/s, D2H {pk['d2h_GBps']:.1f} GB/s, both at once {pk.get('duplex_memcpy_GBps', 0):.1f} GB/s; denominator for HBM fractions: "
            f"{pk['hbm_peak_GBps']:.1f} GB/s (MEASURED_PEAKS.json). GPU: {rep.get('gpu')}; host cores: {rep.get('cores')}. "
-           f"Empty launch (kv_signal) between two events: {pk.get('empty_launch_us', 0):.1f} us with the host's cost of the call inside, "
-           f"{pk.get('empty_launch_us_queued', 0):.1f} us queued behind a spin kernel (device only).", "",
+           f"Empty launch (one-element fill_) between two events, device time: {pk.get('empty_launch_us', 0):.1f} us.", "",
            f"Checks ({rep.get('check', '')}).", "",
            "| config | op | mode | payload MiB | median us | GB/s | % of peak | verified |",
            "|---|---|---|---:|---:|---:|---:|---|"]
@@ -922,15 +949,15 @@ def markdown(rep: dict) -> str:
     for r in rep["records"]:
         if "rows" not in r:
             continue
-        out += ["", f"{r['config']}: {r['op']} (isolated calls; L2 flushed clean up to 2 GiB; `queued` = the call waits in the stream behind "
-                    "a 200 us spin kernel, so the host's cost of issuing it is outside the interval; floor = empty launch + 2*payload/peak, "
-                    "each measured the same way):", "",
-                "| MiB | kernel | pack us | % HBM | floor us | x floor | queued us | % HBM | floor us | x floor | unpack GB/s | re-page 16->64 GB/s | fused re-page GB/s | offload GB/s (mode) | % link | reload GB/s | % link | verified |",
-                "|---:|---|---:|---:|---:|---:|---:|---:|---:|---:|---:|---:|---:|---:|---:|---:|---:|---|"]
+        out += ["", f"{r['config']}: {r['op']} (isolated calls; L2 flushed clean up to 2 GiB -- the flush kernels are queued ahead of the "
+                    "call, so the host's cost of issuing it is hidden and the interval is device time; floor = empty launch + 2*payload/peak; "
+                    "plain copy = torch copy_ (cudaMemcpyAsync device to device) of the same bytes, contiguous, timed the same way):", "",
+                "| MiB | kernel | pack us | % HBM | floor us | x floor | plain copy us | its % HBM | pack / plain copy | unpack GB/s | re-page 16->64 GB/s | fused re-page GB/s | offload GB/s (mode) | % link | reload GB/s | % link | verified |",
+                "|---:|---|---:|---:|---:|---:|---:|---:|---:|---:|---:|---:|---:|---:|---:|---:|---|"]
         for w in r["rows"]:
             mode = {1: "direct", 2: "staged"}.get(w.get("offload_mode"), "?")
             out.append(f"| {w['MiB']} | {w.get('kernel', '')} | {w['pack_us']:.1f} | {w['pack_pct_hbm_peak']:.1f} | {w['floor_us']:.1f} | {w['vs_floor']:.2f} | "
-                       f"{w['pack_us_queued']:.1f} | {100 * w['pack_frac_hbm_queued']:.1f} | {w['floor_us_queued']:.1f} | {w['vs_floor_queued']:.2f} | "
+                       f"{w['plain_copy_us']:.1f} | {100 * w['plain_copy_frac_hbm']:.1f} | {w['vs_plain_copy']:.2f} | "
                        f"{w['unpack_GBps']:.0f} | {w['repage_GBps']:.0f} | {w.get('repage_fused_GBps', 0):.0f} | "
                        f"{w['offload_GBps']:.1f} ({mode}) | {w['offload_pct_link_peak']:.1f} | {w['reload_GBps']:.1f} | "
                        f"{w['reload_pct_link_peak']:.1f} | {w['verified']} |")

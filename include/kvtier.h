@@ -123,7 +123,7 @@ typedef enum kv_option {
                                 width: ~128 KiB of stages per SM (2 x 4 x 16 KiB ... 8 x 16 x 1 KiB); setting any pins it */
   KV_OPT_STORE_LAG = 4,      /* bulk: stores left in flight before a stage is refilled (1 .. 3) */
   KV_OPT_MAX_CTAS = 5,       /* cap on the grid (0 = SM count x CTAs per SM) */
-  KV_OPT_CHUNK_BYTES = 6,    /* staged host transfers: bytes per pipeline chunk (0 = automatic: equal chunks, at least three per
+  KV_OPT_CHUNK_BYTES = 6,    /* staged host transfers: bytes per pipeline chunk (0 = automatic: equal chunks, at least two per
                                 transfer where that leaves 64 MiB each, at most one staging slot each) */
   KV_OPT_HOST_MAX_CTAS = 7,  /* grid cap for DIRECT host transfers (0 = same as device transfers) */
   KV_OPT_STAGING_SLOTS = 8,  /* staged host transfers: pipeline slots the staging buffer is cut into (2 .. 4) */
@@ -140,7 +140,7 @@ typedef enum kv_option {
                                 and run its prologue while the previous kernel of the stream drains; it touches no
                                 global memory before that kernel has completed (griddepcontrol.wait) */
   KV_OPT_RESERVE_STAGING = 14, /* allocate the staging buffer of STAGED host transfers NOW (value = bytes; 0 = the size given
-                                to kv_ctx_create, else 512 MiB) instead of on the first staged call -- required before a
+                                to kv_ctx_create, else 1 GiB) instead of on the first staged call -- required before a
                                 first staged transfer can be captured.  Already allocated: KV_OK if value is 0 or the
                                 same size, else KV_ERR_SIZE. */
 } kv_option;
@@ -165,7 +165,7 @@ const char *kv_strerror(int status); /* static string, never NULL */
 /* ---- context ------------------------------------------------------------------------------ */
 /* Creates the per-thread context on CUDA device `device`: side stream, events, the ring that
  * stages page-id lists, a device status word and (lazily, on the first STAGED transfer)
- * `staging_bytes` of device staging (0 = 512 MiB = two 256 MiB pipeline slots).  `device` < 0 creates a PLANNING-ONLY ctx
+ * `staging_bytes` of device staging (0 = 1 GiB = two 512 MiB pipeline slots).  `device` < 0 creates a PLANNING-ONLY ctx
  * that touches no CUDA API: every transfer call validates and plans, then returns
  * KV_ERR_NO_DEVICE instead of launching (used by host-side tests). */
 int kv_ctx_create(kv_ctx **out, int device, size_t staging_bytes);

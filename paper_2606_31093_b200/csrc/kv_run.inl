@@ -37,7 +37,10 @@ int run_single_launch(kv_ctx *ctx, const kv_pool_desc *pools, const Call &c, con
 int ensure_staging(kv_ctx *ctx) {
   if (ctx->staging) return KV_OK;
   if (ctx->cur_capturing) return KV_ERR_CAPTURE;  // an allocation would invalidate the capture: reserve the staging first
-  if (!ctx->staging_bytes) ctx->staging_bytes = (size_t)512 << 20;  // 256 MiB chunks: measured best with both link directions busy
+  // 1 GiB = two 512 MiB slots (0.6 % of the 180 GB): with both link directions busy every chunk boundary costs ~0.25 ms,
+  // for plain cudaMemcpyAsync too (768 MiB each way as 1 / 2 / 3 / 6 copies: 99.2 / 96.1 / 96.5 / 93.7 GB/s summed), so
+  // chunks are as large as the pipeline allows
+  if (!ctx->staging_bytes) ctx->staging_bytes = (size_t)1024 << 20;
   KV_CUDA(ctx, cudaMalloc(&ctx->staging, ctx->staging_bytes));
   return KV_OK;
 }
@@ -69,13 +72,14 @@ int run_staged(kv_ctx *ctx, const kv_pool_desc *pools, const Call &c, const int3
   const size_t slot_pitch = ctx->staging_bytes / n_slots / 256 * 256;
   size_t slot_bytes = slot_pitch;
   if (ctx->chunk_bytes) slot_bytes = std::min(slot_bytes, ctx->chunk_bytes / 256 * 256);
-  // Equal chunks: at least three per transfer where that leaves >= 64 MiB each (only the first chunk's kernel of an
-  // offload, or the last one's of a reload, is not hidden behind a copy), as many as the slot size demands, and the
-  // payload divided evenly among them in whole chunking units (no two-page leftover chunk at the end).
+  // Equal chunks: at least two per transfer where that leaves >= 64 MiB each (the first chunk's kernel of an offload, or
+  // the last one's of a reload, is not hidden behind a copy: 0.8 % of a two-chunk transfer; a third chunk would halve
+  // that and cost more than it saves once the other link direction is busy too), as many as the slot size demands, and
+  // the payload divided evenly among them in whole chunking units (no two-page leftover chunk at the end).
   else {
     const uint64_t cap = slot_bytes / unit_bytes * unit_bytes, min_chunk = (uint64_t)64 << 20;
     if (cap < unit_bytes) return KV_ERR_SIZE;  // one chunking unit does not fit a staging slot
-    uint64_t n = std::max<uint64_t>(1, std::min<uint64_t>(3, c.payload / min_chunk));
+    uint64_t n = std::max<uint64_t>(1, std::min<uint64_t>(2, c.payload / min_chunk));
     uint64_t per = cap;
     for (;; ++n) {
       per = ((c.payload + n - 1) / n + unit_bytes - 1) / unit_bytes * unit_bytes;

@@ -33,7 +33,7 @@ def test_reference_arm_prints_the_contract_line():
     import bench
     from paper_2606_31093_b200 import workloads as W
 
-    ours = bench.bench_config(argparse.Namespace(prefix_tokens=8192, pool_order="nhd", pool_pages=65536), W.QWEN3_OMNI)
+    ours = bench.bench_config(argparse.Namespace(prefix_tokens=8192, pool_order="nhd", pool_pages=65536, kernel="auto"), W.QWEN3_OMNI)
     assert line["config"] == ours and ours["pages_per_step"] == 512
     assert "full 512-page prefix" in line["cpu_baseline"]["sample"]
     assert line["impl"] == "reference" and line["metric"] == "kv_pack_unpack_GBps" and line["unit"] == "GB/s"

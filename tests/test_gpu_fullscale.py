@@ -314,7 +314,7 @@ def test_cow_tail_pages_of_64_sessions(kv, ctx, pool):
         assert np.array_equal(x, y), "batched CoW append != oracle"
 
 
-@pytest.mark.parametrize("n", [1, 2, 64, 683, 8192])
+@pytest.mark.parametrize("n", [1, 2, 16, 64, 683, 8192])
 def test_transfer_size_sweep_points(kv, ctx, pool, n):
     """BASELINE.json:configs[4] sweep 1 MiB - 8 GiB (layer_count = 32 => 1 MiB pages; 683 is the
     48-layer cross-check point, ~1 GiB).  Sampled buffer pages vs the oracle + full torch gather."""
