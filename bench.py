@@ -46,13 +46,14 @@ sys.path.insert(0, ROOT)
 
 METRIC = "kv_pack_unpack_GBps"
 UNIT = "GB/s"
-# dram__bytes_read.sum + dram__bytes_write.sum of one kv_move_bulk launch (mean of 4 launches) from an `ncu --set full`
-# capture of THIS command at THIS workload.  It is a profile figure, not something this run measures: it is emitted only
-# when the run's configuration is the profiled one (512 pages, NHD pool, default kernel options), with the file named
-# beside it; otherwise `traffic` is null.  805.4 MB read + 759.3 MB written (the last ~46 MB written are still dirty in
-# L2 at exit).
-NCU_TRAFFIC = {"bytes_per_launch": 1564.6e6, "profile": "profiles/r01_kv_move_bulk_full.md",
-               "workload": {"pages": 512, "pool_order": "nhd", "kernel": "kv_move_bulk"}}
+# dram__bytes_read.sum + dram__bytes_write.sum of one kv_pack launch (mean of 4 launches) from an `ncu --set full` capture of
+# THIS command at THIS workload.  It is a profile figure, not something this run measures: it is emitted only when the run's
+# configuration is a profiled one (512 pages, NHD pool, the kernel the profile captured), with the file named beside it;
+# otherwise `traffic` is null.  kv_move_shot (AUTO's kernel at this size): 805.3 MB read + 753.1 MB written; the round-1
+# ring (--kernel bulk): 805.4 + 759.3 (the last ~50 MB written are still dirty in L2 at exit).
+NCU_TRAFFIC = {"kv_move_shot": {"bytes_per_launch": 1558.4e6, "profile": "profiles/r02_kv_move_shot_full.md"},
+               "kv_move_bulk": {"bytes_per_launch": 1564.6e6, "profile": "profiles/r01_kv_move_bulk_full.md"},
+               "workload": {"pages": 512, "pool_order": "nhd", "min_pool_pages": 8192}}  # r02 was captured on a 12 GiB pool
 REFERENCE_WALL_CAP_S = 150.0  # the reference arm stops adding steps beyond this (and says so); 50 steps need ~8 s
 
 
@@ -482,8 +483,9 @@ def run_ours(args):
     value = world * 4 * payload * K / (t_total_ms * 1e-3) / 1e9
     e2e_value = world * 4 * payload * Ke / (e2e_ms * 1e-3) / 1e9
     achieved = 2 * payload / (pack_ms * 1e-3) / 1e9
-    profiled = (args.pool_order == NCU_TRAFFIC["workload"]["pool_order"] and n == NCU_TRAFFIC["workload"]["pages"]
-                and kern_name == NCU_TRAFFIC["workload"]["kernel"] and args.pool_pages == 65536)
+    profiled = NCU_TRAFFIC.get(kern_name) if (args.pool_order == NCU_TRAFFIC["workload"]["pool_order"]
+                                              and n == NCU_TRAFFIC["workload"]["pages"]
+                                              and args.pool_pages >= NCU_TRAFFIC["workload"]["min_pool_pages"]) else None
     line = {
         "metric": METRIC, "value": value, "unit": UNIT, "n_gpus": world, "steps": K, "warmup": Wm,
         "ms_per_step": t_total_ms / K, "higher_is_better": True, "scaling": "weak",
@@ -510,8 +512,8 @@ def run_ours(args):
         "roofline": {"bound": "hbm", "kernel": f"{kern_name} (kv_pack launch)" if args.pool_order == "nhd"
                      else f"{kern_name}<kTrans> with tensor maps (kv_pack launch, HND pool)", "achieved": achieved,
                      "peak": peak, "unit": "GB/s", "frac": achieved / peak,
-                     "traffic": NCU_TRAFFIC["bytes_per_launch"] if profiled else None,
-                     "traffic_source": (f"ncu --set full capture of this command at this workload, {NCU_TRAFFIC['profile']} "
+                     "traffic": profiled["bytes_per_launch"] if profiled else None,
+                     "traffic_source": (f"ncu --set full capture of this command at this workload, {profiled['profile']} "
                                         "(a profile figure, not measured by this run)") if profiled else None,
                      "algorithmic_bytes": 2 * payload, "peak_source": peak_src,
                      "timing": "mean over the K timed steps of CUDA events on the launch stream around each kv_pack call (one launch; page ids ride in the kernel parameters)"},

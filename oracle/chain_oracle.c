@@ -2,7 +2,7 @@
  * (only tests/, __graft_entry__.smoke() and bench.py's cpu_baseline leg may build, load or call it;
  * it shares nothing with paper_2606_31093_b200/).
  *
- * PAPER.md:L276 (Sec. 4.2, prefix reuse): "Both paths use Chained Paged Hashing: each page ID hashes its
+ * PAPER.md:L276 (Sec. 5.1, Multimodal Prefix Matching): "Both paths use Chained Paged Hashing: each page ID hashes its
  * predecessor together with the current page's content identities, thereby representing the complete
  * page-aligned prefix."  The paper names no hash function and no encoding; reading H1-H4:
  *

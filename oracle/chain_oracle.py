@@ -3,7 +3,7 @@
 Only tests/, ``__graft_entry__.smoke()`` and ``bench.py``'s ``cpu_baseline`` leg may import this
 module; it imports nothing from ``paper_2606_31093_b200`` and the CUDA path imports nothing from here.
 
-PAPER.md:L276 (Sec. 4.2): "each page ID hashes its predecessor together with the current page's content
+PAPER.md:L276 (Sec. 5.1): "each page ID hashes its predecessor together with the current page's content
 identities, thereby representing the complete page-aligned prefix."  The paper names neither the hash
 nor the encoding; readings H1-H4 are stated in
 ``chain_oracle.c``.  Two implementations of the same definition:
