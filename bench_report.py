@@ -849,10 +849,10 @@ def run(ctx, desc, shape, slabs, seed=0, out_dir="gpurun_out", hbm_peak=None):
             m, bst = _events(torch, lambda: kv.kv_repage(ctx, d_src, ids_s, d_dst, dst64, Ls, npg * 16), reps, 2, fl_)
             row_["repage_fused_GBps"], row_["repage_fused_us"] = (pls + nd * Ls * shape.C * 4 * row) / m / 1e3, m
             ok = ok and rep_ok(False)
-            reps_h = 7 if pls <= (1 << 30) else 3
+            reps_h = 7 if pls <= (1 << 30) else 5  # D2H over this pool's VMs is noisy (+-2 % between passes): medians of >= 5
             kv.kv_pack(ctx, desc, Ls, ids, bufS)  # the device-side expectation of the offload
             hv_all[:pls:512] = 0xEE
-            m, bst = _events(torch, lambda: kv.kv_offload(ctx, desc, Ls, ids, hp, pls), reps_h, 1)
+            m, bst = _events(torch, lambda: kv.kv_offload(ctx, desc, Ls, ids, hp, pls), reps_h, 2)
             row_["offload_GBps"], row_["offload_us"], row_["offload_mode"] = pls / m / 1e3, m, ctx.stat(kv.KV_STAT_LAST_HOST_MODE)
             ok = ok and chk.host_equals_device(hp, bufS, npg, layers=Ls)
             chk.poison(dst, layers=Ls)
