@@ -156,6 +156,8 @@ typedef enum kv_stat {
   KV_STAT_LAST_GRID = 6,    /* CTAs of the last launch */
   KV_STAT_LAST_SEGMENT = 7, /* bytes per work item of the last call */
   KV_STAT_LAST_TENSOR_MAPS = 8, /* 1 if the last call's launches used tensor maps for an HND pool side */
+  KV_STAT_LAST_PLAIN = 9,   /* 1 if the last launch was the short kernel of the plain case (kv_move_shot_plain: one request,
+                               equal page sizes, page-first, no zero fill, host ids) */
 } kv_stat;
 
 /* ---- library ------------------------------------------------------------------------------ */

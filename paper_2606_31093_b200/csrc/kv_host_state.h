@@ -78,6 +78,7 @@ struct kv_ctx {
   cudaStream_t cur_stream = nullptr;     // stream of the entry point being served
   bool cur_capturing = false;            // ... and whether it is being captured (queried once per call)
   uint64_t last_tma = 0;
+  uint64_t last_plain = 0;
   size_t chunk_bytes = 0;
   // stats
   uint64_t launches = 0, memcpys = 0, last_items = 0, last_payload = 0, last_kernel = 0,

@@ -95,7 +95,24 @@ struct Job {
   // dir 2 with KV_FLAG_IDS_ON_DEVICE: the caller's device array of SOURCE page ids (then `ids` is the
   // caller's destination array and Piece::buf indexes this one); nullptr: both lists sit in `ids`
   const int32_t *src_ids;
+  // n_pieces == 1 (every single-request call, every chunk of a staged single request): the piece itself.  It arrives
+  // with the header, so a CTA's first load waits for one table level fewer (header -> ids / bases -> data instead of
+  // header -> piece -> ids / bases -> data; each level is a first-touch constant-bank or L2 miss on every SM).
+  Piece one;
+  // Exact n / d for n < 2^32 by ONE 64-bit multiply-high: m = floor(2^64 / d) + 1 (0 stands for d == 1).  The divisors
+  // are launch constants; a hardware-less 32-bit division costs ~20 dependent instructions, and decode chains three.
+  uint64_t m_subs, m_LC, m_cpp_pool, m_cpp_buf;
+  // The plain case -- ONE request, pack or unpack between equal page sizes, page-first buffer, every token valid, page
+  // ids validated on the host: decode takes a short straight path (two multiply-highs, two table reads, six
+  // multiply-adds).  A single-warp CTA hides no latency, so the ~300 dependent instructions of the general decode are
+  // ~0.7 us in front of the first load of every CTA -- nothing at 768 MiB (13 CTAs per SM overlap), a quarter of a
+  // 1 MiB call.
+  uint32_t lean;
+  uint32_t pad2_;
 };
+__device__ __forceinline__ uint32_t fdiv(uint32_t n, uint64_t m) {
+  return m ? (uint32_t)__umul64hi((uint64_t)n, m) : n;
+}
 
 // The lookup tables of a launch: slab bases, page ids, pieces.  They live either in device memory
 // (staged through the ctx's pinned ring, JobT<0>) or, for calls whose tables fit, INSIDE the kernel
@@ -144,12 +161,36 @@ struct Item {
   uint32_t lc, s_pg, s_t, d_pg, d_t;
 };
 
+// SURVEY.md 8(a) a2 for the plain case (Job::lean): flat item -> (page, layer/kv, sub) -> addresses.
+struct Lean { uint64_t src, dst; uint32_t bytes; };
+template <bool kGlobal>
+__device__ __forceinline__ Lean decode_lean(const Job &j, const Tables &tb, uint32_t item) {
+  const uint32_t r1 = fdiv(item, j.m_subs), sub = item - r1 * j.subs;
+  const uint32_t pp = fdiv(r1, j.m_LC), lc = r1 - pp * j.LC;
+  const uint32_t sub_off = sub * j.sub_bytes;
+  const int32_t id = kGlobal ? __ldg(tb.ids + j.one.id_begin + pp) : tb.ids[j.one.id_begin + pp];
+  const uint64_t paddr = ldt<kGlobal>(tb.bases + lc) + (uint64_t)(uint32_t)id * j.page_stride + sub_off;
+  const uint64_t baddr = j.one.buf + (uint64_t)pp * j.buf_page_bytes + (uint64_t)lc * j.buf_row_bytes + sub_off;
+  Lean l;
+  l.bytes = min(j.sub_bytes, j.chunk_bytes - sub_off);
+  l.src = j.dir == 0 ? paddr : baddr;
+  l.dst = j.dir == 0 ? baddr : paddr;
+  return l;
+}
+
 // flat item -> (piece, chunk k, layer/kv, sub) -> addresses.
 template <bool kGlobal, bool kTrans = false>
 // `hint`: the piece this thread's previous item fell into.  A thread's items only grow, so the search starts
 // there and gallops forward: one or two probes where a search over all pieces takes log2(n) dependent loads
 // (2,048 one-page requests in one call: unpack 5.43 -> 5.87 TB/s; 64 requests: unchanged at 6.6).
 __device__ __forceinline__ Item decode(const Job &j, const Tables &tb, uint64_t item, uint32_t &hint) {
+  if (!kTrans && j.lean) {  // launch() sets it: dir 0 / 1, one piece, page-first, Tpool == Tbuf, no padding, host ids
+    const Lean l = decode_lean<kGlobal>(j, tb, (uint32_t)item);
+    Item it;
+    it.mode = 0; it.r0 = 0; it.lc = 0; it.s_pg = it.s_t = it.d_pg = it.d_t = 0;
+    it.src = l.src; it.dst = l.dst; it.bytes = it.valid = l.bytes;
+    return it;
+  }
   uint32_t r = 0;
   if (j.n_pieces > 1) {  // largest r with pieces[r].item_begin <= item
     uint32_t lo = hint < j.n_pieces ? hint : 0;
@@ -168,11 +209,20 @@ __device__ __forceinline__ Item decode(const Job &j, const Tables &tb, uint64_t 
     r = lo;
     hint = r;
   }
-  const Piece *pc = tb.pieces + r;
-  const uint64_t item_begin = ldt<kGlobal>(&pc->item_begin), buf = ldt<kGlobal>(&pc->buf),
-                 n_tokens = ldt<kGlobal>(&pc->n_tokens), id_begin = ldt<kGlobal>(&pc->id_begin);
+  uint64_t item_begin, buf, n_tokens, id_begin, n_buf_pages;
+  uint32_t pdir;
+  if (j.n_pieces > 1) {
+    const Piece *pc = tb.pieces + r;
+    item_begin = ldt<kGlobal>(&pc->item_begin); buf = ldt<kGlobal>(&pc->buf);
+    n_tokens = ldt<kGlobal>(&pc->n_tokens); id_begin = ldt<kGlobal>(&pc->id_begin);
+    n_buf_pages = j.layout ? ldt<kGlobal>(&pc->n_buf_pages) : 0;
+    pdir = j.dir == 4 ? ldt<kGlobal>(&pc->dir) : 0;
+  } else {  // the piece rides in the header
+    item_begin = j.one.item_begin; buf = j.one.buf; n_tokens = j.one.n_tokens; id_begin = j.one.id_begin;
+    n_buf_pages = j.one.n_buf_pages; pdir = j.one.dir;
+  }
   const uint32_t local = (uint32_t)(item - item_begin);
-  const uint32_t dir = j.dir == 4 ? ldt<kGlobal>(&pc->dir) : j.dir;
+  const uint32_t dir = j.dir == 4 ? pdir : j.dir;
   if (dir == 3) {  // copy-on-write append: per (layer,kv) s0 items copy the old
                      // page's first n_old tokens, s1 items append the session's new rows behind them
     const uint32_t n_old = (uint32_t)n_tokens, n_app = (uint32_t)(n_tokens >> 32);
@@ -211,10 +261,10 @@ __device__ __forceinline__ Item decode(const Job &j, const Tables &tb, uint64_t 
     it.valid = it.bytes;
     return it;
   }
-  const uint32_t r1 = local / j.subs, sub = local - r1 * j.subs;
-  const uint32_t k = r1 / j.LC, lc = r1 - k * j.LC;
-  const uint32_t pp = k / j.cpp_pool, pk = k - pp * j.cpp_pool;
-  const uint32_t bp = k / j.cpp_buf, bk = k - bp * j.cpp_buf;
+  const uint32_t r1 = fdiv(local, j.m_subs), sub = local - r1 * j.subs;
+  const uint32_t k = fdiv(r1, j.m_LC), lc = r1 - k * j.LC;
+  const uint32_t pp = fdiv(k, j.m_cpp_pool), pk = k - pp * j.cpp_pool;
+  const uint32_t bp = fdiv(k, j.m_cpp_buf), bk = k - bp * j.cpp_buf;
   const uint64_t sub_off = (uint64_t)sub * j.sub_bytes;
   Item it;
   it.mode = 0; it.r0 = 0;
@@ -251,7 +301,7 @@ __device__ __forceinline__ Item decode(const Job &j, const Tables &tb, uint64_t 
   } else {
     baddr = buf + (uint64_t)bk * j.chunk_bytes + sub_off;
     if (j.layout == 0) baddr += (uint64_t)bp * j.buf_page_bytes + (uint64_t)lc * j.buf_row_bytes;
-    else baddr += ((uint64_t)lc * ldt<kGlobal>(&pc->n_buf_pages) + bp) * j.buf_row_bytes;
+    else baddr += ((uint64_t)lc * n_buf_pages + bp) * j.buf_row_bytes;
   }
   const uint64_t vbytes = vt * j.tokrow;
   it.valid = vbytes > sub_off ? (uint32_t)min(vbytes - sub_off, (uint64_t)it.bytes) : 0u;
@@ -763,6 +813,38 @@ __global__ void __launch_bounds__(32) kv_move_shot(const __grid_constant__ JobT<
         st_stream(reinterpret_cast<uint4 *>(it.dst + z), make_uint4(0, 0, 0, 0));
       if (lane == 0) bulk_wait_read<0>();
     }
+  }
+}
+
+// ---------------------------------------------------------------------------------------------
+// kv_move_shot_plain: kv_move_shot for the plain case only (Job::lean, no L2 hints) -- one request, pack or unpack
+// between equal page sizes, page-first buffer, nothing to zero-fill.  Same copy, a fraction of the code: a single-warp
+// CTA hides no latency, so what sits between its start and its bulk load is paid in full by every small call (measured
+// in CUDA-graph replays of 1-16 MiB packs).  Lane 0 alone works; the other lanes leave at once.
+// ---------------------------------------------------------------------------------------------
+template <int N>
+__global__ void __launch_bounds__(32) kv_move_shot_plain(const __grid_constant__ JobT<N> p) {
+  const Job &j = p.j;
+  const Tables tb = tables_of(p);
+  extern __shared__ __align__(128) uint8_t smem[];
+  __shared__ __align__(8) uint64_t full_bar;
+  asm volatile("griddepcontrol.launch_dependents;" ::: "memory");  // no-ops without the launch attribute (KV_OPT_PDL)
+  if (threadIdx.x != 0) return;
+  const uint32_t bar = smem_u32(&full_bar), sbase = smem_u32(smem);
+  mbar_init(bar, 1);
+  asm volatile("fence.mbarrier_init.release.cluster;" ::: "memory");
+  asm volatile("fence.proxy.async.shared::cta;" ::: "memory");
+  asm volatile("griddepcontrol.wait;" ::: "memory");  // nothing global is touched before this
+  uint32_t phase = 0;
+  for (uint64_t item = blockIdx.x; item < j.total_items; item += gridDim.x) {
+    const Lean l = decode_lean<N == 0>(j, tb, (uint32_t)item);
+    mbar_expect_tx(bar, l.bytes);
+    bulk_g2s(sbase, l.src, l.bytes, bar);
+    mbar_wait(bar, phase);
+    phase ^= 1;
+    bulk_s2g(l.dst, sbase, l.bytes);
+    bulk_commit();
+    bulk_wait_read<0>();  // the stage may be refilled (next item of a capped grid) or released (exit)
   }
 }
 

@@ -38,6 +38,8 @@ struct Blob {
   const Piece *d_pieces = nullptr;
   const int32_t *d_ids = nullptr;  // also set for caller-supplied device ids in inline mode
   const HostBlob *inl = nullptr;   // non-null: inline tables
+  bool caller_ids = false;          // the page ids are the caller's device array (KV_FLAG_IDS_ON_DEVICE): unvalidated
+  const Piece *h_pieces = nullptr; // host copy of the blob's pieces (a single-piece launch carries its piece in the Job header)
 };
 
 int upload_blob(kv_ctx *ctx, const HostBlob &hb, const int32_t *ids, bool ids_on_device,
@@ -72,7 +74,9 @@ int upload_blob(kv_ctx *ctx, const HostBlob &hb, const int32_t *ids, bool ids_on
   out->slot = &slot;
   out->d_bases = (const uint64_t *)slot.d;
   out->d_pieces = (const Piece *)((uint8_t *)slot.d + hb.off_pieces);
+  out->h_pieces = (const Piece *)(hb.bytes.data() + hb.off_pieces);  // the caller's HostBlob outlives its launches
   out->d_ids = ids_on_device ? ids : (const int32_t *)((uint8_t *)slot.d + hb.off_ids);
+  out->caller_ids = ids_on_device;
   return KV_OK;
 }
 
@@ -93,7 +97,10 @@ struct BlobGuard {
   }
 };
 
-constexpr int kInlineSmall = 3840;   // whole parameter block stays under the classic 4 KiB
+#ifndef KV_INLINE_SMALL
+#define KV_INLINE_SMALL 3840
+#endif
+constexpr int kInlineSmall = KV_INLINE_SMALL;   // whole parameter block stays under the classic 4 KiB
 constexpr int kInlineLarge = 31744;  // CUDA 12.1+ large kernel parameters (<= 32,764 B)
 
 template <int N>
@@ -126,6 +133,7 @@ void launch_shot(const Job &j, const HostBlob *hb, bool trans, uint32_t grid, si
   cfg.gridDim = dim3(grid); cfg.blockDim = dim3(32); cfg.dynamicSmemBytes = smem; cfg.stream = s;
   cfg.attrs = attr; cfg.numAttrs = pdl ? 1 : 0;
   if (trans) (void)cudaLaunchKernelEx(&cfg, kvt::kv_move_shot<N, true>, p);
+  else if (j.lean && !j.l2_hint) (void)cudaLaunchKernelEx(&cfg, kvt::kv_move_shot_plain<N>, p);
   else (void)cudaLaunchKernelEx(&cfg, kvt::kv_move_shot<N, false>, p);
 }
 template <int N>
@@ -165,6 +173,17 @@ int launch(kv_ctx *ctx, const Geom &g, const Blob &b, uint32_t piece_first, uint
   j.g = g.g; j.cpp_pool = g.Tpool / g.g; j.cpp_buf = g.Tbuf / g.g;
   j.tokrow = g.tokrow; j.chunk_bytes = g.chunk_bytes; j.sub_bytes = g.sub_bytes; j.subs = g.subs;
   j.num_pages = g.num_pages;
+  if (n_pieces == 1) {
+    const Piece *hp = b.inl ? (const Piece *)(b.inl->bytes.data() + b.inl->off_pieces) : b.h_pieces;
+    if (!hp) return KV_ERR_NULL;  // every Blob is built by build_blob / upload_blob, which keep the host copy
+    j.one = hp[piece_first];
+  }
+  // the short decode path (kv_kernels.cuh Job::lean): host ids only (validated before any launch), nothing to zero-fill
+  j.lean = n_pieces == 1 && (g.dir == 0 || g.dir == 1) && g.layout == KV_LAYOUT_PAGE_FIRST && g.Tpool == g.Tbuf &&
+           !g.trans && !b.caller_ids && j.one.item_begin == 0 && j.one.n_buf_pages * (uint64_t)g.Tbuf <= j.one.n_tokens &&
+           total_items <= 0xffffffffull;
+  auto magic = [](uint32_t d) -> uint64_t { return d <= 1 ? 0ull : ~0ull / d + 1; };  // floor(2^64 / d) + 1 unless d | 2^64
+  j.m_subs = magic(j.subs); j.m_LC = magic(j.LC); j.m_cpp_pool = magic(j.cpp_pool); j.m_cpp_buf = magic(j.cpp_buf);
   if (g.src_pool) { j.src_num_pages = g.src_pool->num_pages; j.src_page_stride = g.src_pool->page_stride_bytes; }
   j.src_ids = g.dev_src_ids;
   j.drow = g.drow; j.H = g.H;
@@ -266,6 +285,7 @@ int launch(kv_ctx *ctx, const Geom &g, const Blob &b, uint32_t piece_first, uint
   KV_CUDA(ctx, cudaGetLastError());
   ctx->launches++;
   ctx->last_grid = grid;
+  ctx->last_plain = g.kernel == KERNEL_SHOT && !g.trans && j.lean && !j.l2_hint;
   return KV_OK;
 }
 

@@ -25,6 +25,7 @@ int run_single_launch(kv_ctx *ctx, const kv_pool_desc *pools, const Call &c, con
   if (ctx->inline_tables && c.geom.kernel != KERNEL_ELEM && hb.bytes.size() <= (size_t)kInlineLarge) {
     b.inl = &hb;  // tables travel inside the kernel parameters: one launch, no copy
     b.d_ids = dev_ids ? ids : nullptr;
+    b.caller_ids = dev_ids;
     return launch(ctx, c.geom, b, 0, (uint32_t)pieces.size(), acc, cta_cap, s);
   }
   if (ctx->cur_capturing) return KV_ERR_CAPTURE;
@@ -240,6 +241,7 @@ int run_staged(kv_ctx *ctx, const kv_pool_desc *pools, const Call &c, const int3
     Blob b;
     b.inl = &hb_chunk;
     b.d_ids = dev_ids ? ids : nullptr;
+    b.caller_ids = dev_ids;
     return launch(ctx, g, b, 0, ch.n_pieces, ch.items, 0, s, ch.l0 * g.C, ch.nl * g.C);
   };
   // Events.  Eager calls order slot reuse across calls with the ctx's per-slot events.  Inside a capture the same

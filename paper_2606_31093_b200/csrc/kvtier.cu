@@ -88,7 +88,9 @@ cudaError_t ctx_init_device(kv_ctx *ctx, int device) {
     if ((e = cudaFuncSetAttribute(k, cudaFuncAttributeMaxDynamicSharedMemorySize, ctx->max_smem - kStaticSmemReserve)) != cudaSuccess) return e;
   const void *shot_kernels[] = {(const void *)kvt::kv_move_shot<0, false>, (const void *)kvt::kv_move_shot<kInlineSmall, false>,
                                 (const void *)kvt::kv_move_shot<kInlineLarge, false>, (const void *)kvt::kv_move_shot<0, true>,
-                                (const void *)kvt::kv_move_shot<kInlineSmall, true>, (const void *)kvt::kv_move_shot<kInlineLarge, true>};
+                                (const void *)kvt::kv_move_shot<kInlineSmall, true>, (const void *)kvt::kv_move_shot<kInlineLarge, true>,
+                                (const void *)kvt::kv_move_shot_plain<0>, (const void *)kvt::kv_move_shot_plain<kInlineSmall>,
+                                (const void *)kvt::kv_move_shot_plain<kInlineLarge>};
   for (const void *k : shot_kernels) {  // stages up to 64 KiB (KV_OPT_STAGE_BYTES); as many CTAs per SM as shared memory holds
     if ((e = cudaFuncSetAttribute(k, cudaFuncAttributeMaxDynamicSharedMemorySize, 65536)) != cudaSuccess) return e;
     if ((e = cudaFuncSetAttribute(k, cudaFuncAttributePreferredSharedMemoryCarveout, cudaSharedmemCarveoutMaxShared)) != cudaSuccess) return e;
@@ -213,6 +215,7 @@ int kv_ctx_get_stat(kv_ctx *ctx, int stat, uint64_t *out) {
     case KV_STAT_LAST_GRID: *out = ctx->last_grid; break;
     case KV_STAT_LAST_SEGMENT: *out = ctx->last_segment; break;
     case KV_STAT_LAST_TENSOR_MAPS: *out = ctx->last_tma; break;
+    case KV_STAT_LAST_PLAIN: *out = ctx->last_plain; break;
     default: return KV_ERR_LAYOUT;
   }
   return KV_OK;

@@ -40,7 +40,7 @@ KV_FLAG_VALIDATE, KV_FLAG_IDS_ON_DEVICE = 0x1, 0x2
 KV_OP_PACK, KV_OP_UNPACK, KV_OP_COW_APPEND = 0, 1, 3
 KV_KERNEL_AUTO, KV_KERNEL_BULK, KV_KERNEL_VEC, KV_KERNEL_ELEM, KV_KERNEL_SHOT = 0, 1, 2, 3, 4
 (KV_STAT_LAUNCHES, KV_STAT_MEMCPYS, KV_STAT_LAST_ITEMS, KV_STAT_LAST_PAYLOAD, KV_STAT_LAST_KERNEL,
- KV_STAT_LAST_HOST_MODE, KV_STAT_LAST_GRID, KV_STAT_LAST_SEGMENT, KV_STAT_LAST_TENSOR_MAPS) = range(9)
+ KV_STAT_LAST_HOST_MODE, KV_STAT_LAST_GRID, KV_STAT_LAST_SEGMENT, KV_STAT_LAST_TENSOR_MAPS, KV_STAT_LAST_PLAIN) = range(10)
 
 
 class kv_pool_desc(ctypes.Structure):

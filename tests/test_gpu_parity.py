@@ -70,6 +70,59 @@ def test_pack_unpack_same_page_size(kv, ctx, kernel, shape):
     assert ctx.stat(kv.KV_STAT_LAST_KERNEL) == KERNELS[kernel]
 
 
+@pytest.mark.parametrize("shape", [SHAPES[0], SHAPES[1], SHAPES[2], SHAPES[4]])
+@pytest.mark.parametrize("variant", ["plain", "plain_capped", "general_l2hint", "plain_batched_1", "general_batched_2"])
+def test_plain_kernel_and_general_kernel_agree_with_the_oracle(kv, ctx, shape, variant):
+    """The plain case (one request, equal page sizes, page-first, nothing to zero-fill, host ids) runs the short
+    kernel kv_move_shot_plain; anything else -- here an L2 hint, or a second request -- the general kv_move_shot.
+    Both must give the oracle's bytes; a capped grid makes every CTA of the plain kernel walk several items (the
+    stage and its mbarrier phase are reused)."""
+    L, C, P, T, H, D, e, pad = shape
+    rng = np.random.default_rng(7 + abs(hash((shape, variant))) % 2**31)
+    if variant == "general_l2hint":
+        ctx.set_option(kv.KV_OPT_L2_HINT, 1)
+    if variant == "plain_capped":
+        ctx.set_option(kv.KV_OPT_MAX_CTAS, 5)
+    A = host_pool(rng, L, C, P, T, H, D, e, pad)
+    B = host_pool(rng, L, C, P, T, H, D, e, pad)
+    n = min(29, P - 3)
+    ids = rng.choice(P, n, replace=False).astype(np.int32)
+    dst = rng.permutation(P)[:n].astype(np.int32)
+    tA, dA = to_device(A, kv, torch)
+    tB, dB = to_device(B, kv, torch)
+    page = dA.page_bytes()
+    buf = torch.full((n * page + 256,), 0xCD, dtype=torch.uint8, device="cuda")
+    want_plain = 0 if variant.startswith("general") else 1
+    if "batched" in variant:
+        n_req = int(variant[-1])
+        cut = [0, n] if n_req == 1 else [0, n // 3, n]
+        off = np.asarray(cut, dtype=np.int64)
+        bufs = [buf[cut[r] * page:cut[r + 1] * page] for r in range(n_req)]
+        kv.kv_pack_batched(ctx, dA, L, ids, off, bufs)
+    else:
+        kv.kv_pack(ctx, dA, L, ids, buf, dst_bytes=n * page)
+    assert ctx.stat(kv.KV_STAT_LAST_KERNEL) == kv.KV_KERNEL_SHOT and ctx.stat(kv.KV_STAT_LAST_PLAIN) == want_plain
+    want = ko.pack(A, ids)
+    got = buf.cpu().numpy()
+    assert np.array_equal(got[:want.size], want)
+    assert np.all(got[want.size:] == 0xCD), "wrote past the end of the buffer"
+    if "batched" in variant:
+        ntok = np.asarray([(cut[r + 1] - cut[r]) * T for r in range(n_req)], dtype=np.uint64)
+        kv.kv_unpack_batched(ctx, bufs, dst, off, ntok, dB, L, T, T)
+    else:
+        kv.kv_unpack(ctx, buf, dst, dB, L, T, T, n * T, src_bytes=n * page)
+    assert ctx.stat(kv.KV_STAT_LAST_PLAIN) == want_plain
+    ko.unpack(want, dst, B, Ts=T, n_tokens=n * T)
+    assert_pool_equal(tB, B)
+    assert_pool_equal(tA, A)
+    # a ragged tail is not the plain case: the last page's unused slots are zero-filled by the general kernel
+    if variant == "plain":
+        kv.kv_unpack(ctx, buf, dst, dB, L, T, T, n * T - 1, src_bytes=n * page)
+        assert ctx.stat(kv.KV_STAT_LAST_PLAIN) == 0
+        ko.unpack(want, dst, B, Ts=T, n_tokens=n * T - 1)
+        assert_pool_equal(tB, B)
+
+
 @pytest.mark.parametrize("kernel", ["bulk", "vec"])
 @pytest.mark.parametrize("Ts,Td,ntok", [(16, 64, 2048), (16, 64, 2048 - 37), (64, 16, 1000),
                                         (16, 24, 500), (3, 5, 77), (16, 16, 16 * 9 - 5), (8, 64, 1)])
