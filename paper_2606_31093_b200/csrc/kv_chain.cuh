@@ -25,12 +25,14 @@ constexpr uint64_t kFnvPrime = 0x100000001b3ull;
 // One FNV-1a step on the two 32-bit halves of h:  h' = (h ^ b) * (2^40 + 0x1b3)  mod 2^64, i.e. with
 // x = lo ^ b:   lo' = low32(x * 0x1b3),   hi' = hi * 0x1b3 + [ high32(x * 0x1b3) + (x << 8) ].
 // The bracket depends on the LOW chain only, so the high half advances by ONE multiply-add per step
-// and the step is bound by the low chain: LOP3 (alu pipe) -> IMAD (fma pipe) -> LOP3.  A bare chain of
-// exactly that pair measures 15.7 cycles per step on B200 (one warp, clock64 around 1.6 M dependent
-// steps; it is the same with IMAD.WIDE or with a 32-bit IMAD on the chain), i.e. 251 cycles = 128 ns per
-// 16-step link at 1,965 MHz: the floor.  Left to itself nvcc chains three dependent ops through the
-// high half (171 ns per link); with the association pinned by the asm below a 2,875-link chain runs at
-// 131 ns per link.
+// and the step is bound by the low chain: LOP3 (alu pipe) -> IMAD.WIDE (fma pipe) -> LOP3.  Bare chains measured on
+// B200 (one warp, clock64 around 1.6 M dependent steps, round 2): xor -> mul.wide 12.4 cycles per step, xor -> 32-bit
+// mul.lo 10.1 -- so 12.4 cycles = 6.3 ns per step, 101 ns per 16-step link at 1,965 MHz is the floor of THIS step, and a
+// 2,875-link chain runs at 102 ns per link (round 1 quoted 15.7 cycles: its probe also carried the high-half chain in
+// program order).  Left to itself nvcc chains three dependent ops through the high half (171 ns per link); the asm
+// below pins the association.  Taking the 32-bit multiply alone onto the chain (high word by a separate mul.hi) would
+// be 19 % shorter, but ptxas fuses the pair back into one IMAD.WIDE, and hiding the pairing from it (an operand it
+// cannot prove equal) moved the whole chain onto the uniform datapath: 427 instead of 288 us.  Not pursued.
 __device__ __forceinline__ void fnv1a_step(uint32_t &lo, uint32_t &hi, uint32_t byte) {
   const uint32_t x = lo ^ byte;
   uint64_t w;
