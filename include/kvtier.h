@@ -86,7 +86,7 @@ typedef enum kv_layout {
 
 /* How a host-tier transfer crosses the host link (BASELINE.json:north_star item 3). */
 typedef enum kv_host_mode {
-  KV_HOST_AUTO = 0,   /* chosen from the measured table in DESIGN.md: STAGED from 16 MiB of payload (either layout), else DIRECT */
+  KV_HOST_AUTO = 0,   /* chosen from the measured table in DESIGN.md: STAGED from 4 MiB of payload (either layout), else DIRECT */
   KV_HOST_DIRECT = 1, /* the kernel stores to / loads from mapped pinned memory over the link */
   KV_HOST_STAGED = 2, /* device staging + copy-engine transfers (1-D, or 2-D for layer-first chunks) on the ctx's side stream, chunk-pipelined */
 } kv_host_mode;
@@ -365,7 +365,7 @@ int kv_reload(kv_ctx *ctx, const void *host_src, size_t host_bytes, const int32_
  * ANOTHER GPU, or a kernel that checks the flag once and does not spin.  Do NOT park a kernel of the same GPU in a
  * loop on these flags: nothing guarantees that it and the transfer's kernels run at the same time (measured on
  * this B200 / driver 580: a spinning kernel on one stream kept a kernel of another stream from starting).
- * Flags are stored in ascending layer order.  KV_HOST_STAGED (AUTO's choice from 16 MiB) streams the buffer
+ * Flags are stored in ascending layer order.  KV_HOST_STAGED (AUTO's choice from 4 MiB) streams the buffer
  * through the ctx's staging in chunks of whole layers (a layer wider than a staging slot is cut by page
  * ranges), copy engine and scatter kernel pipelined, so layer 0 is usable after ~1/layer_count of the
  * transfer; KV_HOST_DIRECT is one launch over all layers followed by all flags.  n_req == 0 or no pages:

@@ -11,7 +11,7 @@ using kvt::Piece;
 constexpr int kBlobSlots = 16;
 constexpr int kMaxStagingSlots = 4;
 constexpr uint32_t kMaxLayersKv = 4096;  // layer_count * kv_count
-constexpr uint64_t kAutoStagedMinBytes = 16ull << 20;
+constexpr uint64_t kAutoStagedMinBytes = 4ull << 20;
 constexpr uint32_t kShotMinSegment = 4096;  // AUTO: kv_move_shot from this segment size (below it the SM's bulk-copy rate binds)
 constexpr uint32_t kSchedSlots = 256;  // claim counters, handed out round-robin per launch
 constexpr int kStaticSmemReserve = 8192;  // static shared memory of kv_move_bulk (barriers + stage metadata, 6 KiB) rounded up

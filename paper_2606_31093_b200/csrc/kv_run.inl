@@ -252,8 +252,15 @@ int run_staged(kv_ctx *ctx, const kv_pool_desc *pools, const Call &c, const int3
   cudaEvent_t *ev_full = cap ? ctx->cap_full : ctx->ev_full;
   cudaEvent_t *ev_free = cap ? ctx->cap_free : ctx->ev_free;
   std::vector<uint8_t> cap_used(kMaxStagingSlots, 0);  // capture: slots this call has already been through
-  KV_CUDA(ctx, cudaEventRecord(ev_entry, s));
-  KV_CUDA(ctx, cudaStreamWaitEvent(ctx->side, ev_entry, 0));
+  // A transfer of ONE chunk has nothing to overlap: its kernel and its copy run back to back on the caller's stream, with
+  // no fork to the side stream and no cross-stream events (each costs a few microseconds: 8 MiB offload 168 -> 16x us
+  // against 155 us for the bare cudaMemcpyAsync).  The slot is still guarded by its event for whoever uses it next.
+  const bool single = chunks.size() == 1;
+  cudaStream_t cs = single ? s : ctx->side;
+  if (!single) {
+    KV_CUDA(ctx, cudaEventRecord(ev_entry, s));
+    KV_CUDA(ctx, cudaStreamWaitEvent(ctx->side, ev_entry, 0));
+  }
   for (size_t ci = 0; ci < chunks.size(); ++ci) {
     const uint32_t slot = (uint32_t)(ci % n_slots);
     uint8_t *slot_base = (uint8_t *)ctx->staging + (size_t)slot * slot_pitch;
@@ -262,31 +269,35 @@ int run_staged(kv_ctx *ctx, const kv_pool_desc *pools, const Call &c, const int3
       if (wait_free) KV_CUDA(ctx, cudaStreamWaitEvent(s, ev_free[slot], 0));
       rc = launch_chunk(chunks[ci]);
       if (rc) return rc;
-      KV_CUDA(ctx, cudaEventRecord(ev_full[slot], s));
-      KV_CUDA(ctx, cudaStreamWaitEvent(ctx->side, ev_full[slot], 0));
+      if (!single) {
+        KV_CUDA(ctx, cudaEventRecord(ev_full[slot], s));
+        KV_CUDA(ctx, cudaStreamWaitEvent(ctx->side, ev_full[slot], 0));
+      }
       for (const Copy &cp : copies[ci]) {
         if (cp.rows > 1)
           KV_CUDA(ctx, cudaMemcpy2DAsync((void *)(uintptr_t)cp.host, cp.host_pitch, slot_base + cp.dev_off, cp.bytes,
-                                         cp.bytes, cp.rows, cudaMemcpyDeviceToHost, ctx->side));
+                                         cp.bytes, cp.rows, cudaMemcpyDeviceToHost, cs));
         else
           KV_CUDA(ctx, cudaMemcpyAsync((void *)(uintptr_t)cp.host, slot_base + cp.dev_off, cp.bytes,
-                                       cudaMemcpyDeviceToHost, ctx->side));
+                                       cudaMemcpyDeviceToHost, cs));
         ctx->memcpys++;
       }
-      KV_CUDA(ctx, cudaEventRecord(ev_free[slot], ctx->side));
+      KV_CUDA(ctx, cudaEventRecord(ev_free[slot], cs));
     } else {  // reload: copy engine fills the slot on side, kernel drains it on s
-      if (wait_free) KV_CUDA(ctx, cudaStreamWaitEvent(ctx->side, ev_free[slot], 0));
+      if (wait_free) KV_CUDA(ctx, cudaStreamWaitEvent(cs, ev_free[slot], 0));
       for (const Copy &cp : copies[ci]) {
         if (cp.rows > 1)
           KV_CUDA(ctx, cudaMemcpy2DAsync(slot_base + cp.dev_off, cp.bytes, (const void *)(uintptr_t)cp.host,
-                                         cp.host_pitch, cp.bytes, cp.rows, cudaMemcpyHostToDevice, ctx->side));
+                                         cp.host_pitch, cp.bytes, cp.rows, cudaMemcpyHostToDevice, cs));
         else
           KV_CUDA(ctx, cudaMemcpyAsync(slot_base + cp.dev_off, (const void *)(uintptr_t)cp.host,
-                                       cp.bytes, cudaMemcpyHostToDevice, ctx->side));
+                                       cp.bytes, cudaMemcpyHostToDevice, cs));
         ctx->memcpys++;
       }
-      KV_CUDA(ctx, cudaEventRecord(ev_full[slot], ctx->side));
-      KV_CUDA(ctx, cudaStreamWaitEvent(s, ev_full[slot], 0));
+      if (!single) {
+        KV_CUDA(ctx, cudaEventRecord(ev_full[slot], ctx->side));
+        KV_CUDA(ctx, cudaStreamWaitEvent(s, ev_full[slot], 0));
+      }
       rc = launch_chunk(chunks[ci]);
       if (rc) return rc;
       if (lf.flags && chunks[ci].sig_n) {  // these layers' pages are in the pool: publish
@@ -298,7 +309,7 @@ int run_staged(kv_ctx *ctx, const kv_pool_desc *pools, const Call &c, const int3
     }
     if (cap) cap_used[slot] = 1; else ctx->free_valid[slot] = true;
   }
-  if (g.dir == 0) {  // join the copy engine's tail back into s
+  if (g.dir == 0 && !single) {  // join the copy engine's tail back into s
     const size_t first = chunks.size() > n_slots ? chunks.size() - n_slots : 0;
     for (size_t ci = first; ci < chunks.size(); ++ci)
       KV_CUDA(ctx, cudaStreamWaitEvent(s, ev_free[ci % n_slots], 0));
@@ -321,8 +332,10 @@ int resolve_mode(const kv_ctx *ctx, int mode, const Call &c, int *out) {
   if (mode != KV_HOST_AUTO && mode != KV_HOST_DIRECT && mode != KV_HOST_STAGED) return KV_ERR_LAYOUT;
   int m = mode;
   // Measured on B200 / PCIe Gen5 x16: the copy engines reach 98-99 % of the
-  // cudaMemcpy peak, SM-issued stores/loads over the link 92 % (128-byte TLP payloads); below
-  // ~16 MiB both are latency-bound and equal, and DIRECT is one launch with no staging traffic.
+  // cudaMemcpy peak, SM-issued stores/loads over the link 92 % (128-byte TLP payloads).  A one-chunk staged
+  // transfer is a kernel and a copy back to back on the caller's stream; it is ahead of DIRECT from 4 MiB
+  // (92 vs 98 us; 8 MiB 167 vs 178; 16 MiB 314 vs 336), level at 2 MiB, behind at 1 MiB (reload 41 vs 38 us),
+  // where DIRECT is one launch with no staging traffic.
   if (m == KV_HOST_AUTO) m = c.payload >= kAutoStagedMinBytes ? KV_HOST_STAGED : KV_HOST_DIRECT;
   (void)ctx;
   *out = m;

@@ -170,7 +170,7 @@ def test_empty_calls_are_ok_even_without_a_device(ctx):
 def test_auto_host_mode_policy(ctx):
     s = W.QWEN3_OMNI
     d = fake_pool(s)
-    for n, want in [(4, kv.KV_HOST_DIRECT), (10, kv.KV_HOST_DIRECT), (11, kv.KV_HOST_STAGED), (512, kv.KV_HOST_STAGED)]:
+    for n, want in [(1, kv.KV_HOST_DIRECT), (2, kv.KV_HOST_DIRECT), (3, kv.KV_HOST_STAGED), (11, kv.KV_HOST_STAGED), (512, kv.KV_HOST_STAGED)]:
         assert status_of(lambda: kv.kv_offload(ctx, d, s.L, np.arange(n), BUF, n * s.page_bytes)) == kv.KV_ERR_NO_DEVICE
         assert ctx.stat(kv.KV_STAT_LAST_HOST_MODE) == want, n
     # layer-first buffers stage too (chunks of whole layers: each (layer, K|V) run of pages is contiguous)
