@@ -76,6 +76,8 @@ def parse():
     ap.add_argument("--kernel", default="auto", choices=["auto", "bulk", "vec", "shot"],
                     help="KV_OPT_KERNEL of every ctx (auto = the library's measured choice; the others reproduce the A/B "
                          "figures of DESIGN.md: bulk = the persistent ring, shot = one segment per single-warp CTA)")
+    ap.add_argument("--lead-chunk-mib", type=int, default=-1,
+                    help="KV_OPT_LEAD_CHUNK of every ctx in MiB (-1 = the library's default; 0 = equal chunks: the A/B figure of DESIGN.md)")
     ap.add_argument("--seed", type=int, default=0)
     return ap.parse_args()
 
@@ -354,6 +356,8 @@ def run_ours(args):
     ctx = kv.Ctx(local)
     kopt = {"auto": kv.KV_KERNEL_AUTO, "bulk": kv.KV_KERNEL_BULK, "vec": kv.KV_KERNEL_VEC, "shot": kv.KV_KERNEL_SHOT}[args.kernel]
     ctx.set_option(kv.KV_OPT_KERNEL, kopt)
+    if args.lead_chunk_mib >= 0:
+        ctx.set_option(kv.KV_OPT_LEAD_CHUNK, args.lead_chunk_mib << 20)
     stream = torch.cuda.current_stream()
     kv.kv_pack(ctx, desc, shape.L, src_ids[-1], bufs[1])  # buffer read by the first unpack
 
@@ -427,6 +431,8 @@ def run_ours(args):
 
         ctx2 = kv.Ctx(local)  # its own staging, side stream and events: the two directions share nothing
         ctx2.set_option(kv.KV_OPT_KERNEL, kopt)
+        if args.lead_chunk_mib >= 0:
+            ctx2.set_option(kv.KV_OPT_LEAD_CHUNK, args.lead_chunk_mib << 20)
         s_off, s_rel = torch.cuda.Stream(), torch.cuda.Stream()
 
         def duplex_step(i):

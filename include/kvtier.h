@@ -143,6 +143,9 @@ typedef enum kv_option {
                                 to kv_ctx_create, else 1 GiB) instead of on the first staged call -- required before a
                                 first staged transfer can be captured.  Already allocated: KV_OK if value is 0 or the
                                 same size, else KV_ERR_SIZE. */
+  KV_OPT_LEAD_CHUNK = 15,    /* staged page-first host transfers of 128 MiB or more: bytes of the short chunk that leads an
+                                offload / ends a reload, so that the one kernel no copy hides is a short one (default
+                                32 MiB; 0 = equal chunks; ignored with KV_OPT_CHUNK_BYTES) */
 } kv_option;
 
 /* kv_ctx_get_stat keys */

@@ -72,18 +72,28 @@ int run_staged(kv_ctx *ctx, const kv_pool_desc *pools, const Call &c, const int3
   // and whatever stream it ran on (two staged calls of one ctx on two streams share the slots safely).
   const size_t slot_pitch = ctx->staging_bytes / n_slots / 256 * 256;
   size_t slot_bytes = slot_pitch;
+  uint64_t lead_bytes = 0;
   if (ctx->chunk_bytes) slot_bytes = std::min(slot_bytes, ctx->chunk_bytes / 256 * 256);
   // Equal chunks: at least two per transfer where that leaves >= 64 MiB each (the first chunk's kernel of an offload, or
   // the last one's of a reload, is not hidden behind a copy: 0.8 % of a two-chunk transfer; a third chunk would halve
   // that and cost more than it saves once the other link direction is busy too), as many as the slot size demands, and
   // the payload divided evenly among them in whole chunking units (no two-page leftover chunk at the end).
+  // From 128 MiB a SHORT chunk (32 MiB) leads an offload, or ends a reload, when KV_OPT_LEAD_CHUNK allows it: the one
+  // kernel that no copy hides -- the first of an offload, the last of a reload -- is then a 32 MiB kernel (~12 us)
+  // instead of one over half the payload (~120 us of a 14.3 ms transfer at 768 MiB), and the short copy beside it is
+  // still long enough (0.57 ms) to hide the neighbouring large chunk's kernel.
   else {
     const uint64_t cap = slot_bytes / unit_bytes * unit_bytes, min_chunk = (uint64_t)64 << 20;
     if (cap < unit_bytes) return KV_ERR_SIZE;  // one chunking unit does not fit a staging slot
-    uint64_t n = std::max<uint64_t>(1, std::min<uint64_t>(2, c.payload / min_chunk));
+    if (ctx->lead_chunk && !lf.flags && !layer_first && c.payload >= 2 * min_chunk) {
+      lead_bytes = std::max<uint64_t>(unit_bytes, ((uint64_t)ctx->lead_chunk + unit_bytes - 1) / unit_bytes * unit_bytes);
+      if (lead_bytes > cap || lead_bytes * 2 > c.payload) lead_bytes = 0;
+    }
+    const uint64_t rest = c.payload - lead_bytes;
+    uint64_t n = lead_bytes ? 1 : std::max<uint64_t>(1, std::min<uint64_t>(2, c.payload / min_chunk));
     uint64_t per = cap;
     for (;; ++n) {
-      per = ((c.payload + n - 1) / n + unit_bytes - 1) / unit_bytes * unit_bytes;
+      per = ((rest + n - 1) / n + unit_bytes - 1) / unit_bytes * unit_bytes;
       if (per <= cap) break;
     }
     slot_bytes = (size_t)std::max<uint64_t>(per, unit_bytes);
@@ -93,6 +103,8 @@ int run_staged(kv_ctx *ctx, const kv_pool_desc *pools, const Call &c, const int3
   if (lf.flags) slot_bytes = std::min<size_t>(slot_bytes, (size_t)64 << 20);
   if (slot_bytes < unit_bytes) return KV_ERR_SIZE;
   const uint64_t chunk_tokens = slot_bytes / unit_bytes * unit_tokens;
+  // an offload's FIRST chunk is the short one; a reload's short chunk is the remainder its equal chunks leave at the end
+  const uint64_t lead_tokens = g.dir == 0 ? lead_bytes / unit_bytes * unit_tokens : 0;
 
   // A chunk = what one staging slot holds: pieces for the kernel, copies for the copy engine.  Page-first:
   // a run of whole pages, all layers (contiguous in the host buffer).  Layer-first: a range of layers
@@ -177,8 +189,10 @@ int run_staged(kv_ctx *ctx, const kv_pool_desc *pools, const Call &c, const int3
       const uint64_t slots_pool = q.n_ids * g.Tpool;
       uint64_t t0 = 0;
       while (t0 < slots_pool) {
-        if (fill_tokens == chunk_tokens) close();
-        const uint64_t t1 = std::min(slots_pool, t0 + (chunk_tokens - fill_tokens));
+        const uint64_t cap_tokens = (lead_tokens && chunks.empty()) ? lead_tokens : chunk_tokens;
+        if (fill_tokens == cap_tokens) close();
+        const uint64_t cap_now = (lead_tokens && chunks.empty()) ? lead_tokens : chunk_tokens;  // (close() may have opened chunk 1)
+        const uint64_t t1 = std::min(slots_pool, t0 + (cap_now - fill_tokens));
         const uint64_t span = t1 - t0;  // multiple of Tpool; multiple of unit except at the request's end
         const uint64_t buf_pages = (std::min(t1, q.n_buf_pages * g.Tbuf) - std::min(t0, q.n_buf_pages * g.Tbuf) + g.Tbuf - 1) / g.Tbuf;
         const uint64_t dev_off = fill_tokens * g.tokrow * g.LC;

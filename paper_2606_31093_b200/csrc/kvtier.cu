@@ -189,6 +189,7 @@ int kv_ctx_set_option(kv_ctx *ctx, int option, int64_t v) {
     case KV_OPT_DYNAMIC: if (v < 0 || v > 1) return KV_ERR_SIZE; ctx->dynamic = (uint32_t)v; break;
     case KV_OPT_TENSOR_MAPS: if (v < 0 || v > 1) return KV_ERR_SIZE; ctx->tensor_maps = (uint32_t)v; break;
     case KV_OPT_PDL: if (v < 0 || v > 1) return KV_ERR_SIZE; ctx->pdl = (uint32_t)v; break;
+    case KV_OPT_LEAD_CHUNK: if (v < 0 || v > (1ll << 30)) return KV_ERR_SIZE; ctx->lead_chunk = (uint32_t)v; break;
     case KV_OPT_RESERVE_STAGING: {
       if (v < 0) return KV_ERR_SIZE;
       if (ctx->host_only) return KV_ERR_NO_DEVICE;

@@ -36,7 +36,7 @@ KV_FLAG_VALIDATE, KV_FLAG_IDS_ON_DEVICE = 0x1, 0x2
 (KV_OPT_KERNEL, KV_OPT_STAGE_BYTES, KV_OPT_STAGES_PER_WARP, KV_OPT_WARPS, KV_OPT_STORE_LAG,
  KV_OPT_MAX_CTAS, KV_OPT_CHUNK_BYTES, KV_OPT_HOST_MAX_CTAS, KV_OPT_STAGING_SLOTS,
  KV_OPT_L2_HINT, KV_OPT_INLINE_TABLES, KV_OPT_DYNAMIC, KV_OPT_TENSOR_MAPS, KV_OPT_PDL,
- KV_OPT_RESERVE_STAGING) = range(15)
+ KV_OPT_RESERVE_STAGING, KV_OPT_LEAD_CHUNK) = range(16)
 KV_OP_PACK, KV_OP_UNPACK, KV_OP_COW_APPEND = 0, 1, 3
 KV_KERNEL_AUTO, KV_KERNEL_BULK, KV_KERNEL_VEC, KV_KERNEL_ELEM, KV_KERNEL_SHOT = 0, 1, 2, 3, 4
 (KV_STAT_LAUNCHES, KV_STAT_MEMCPYS, KV_STAT_LAST_ITEMS, KV_STAT_LAST_PAYLOAD, KV_STAT_LAST_KERNEL,

@@ -218,6 +218,57 @@ def test_staged_offload_and_reload_captured_and_replayed(kv, layout, dev_ids):
 # ONE ctx, staged transfers on TWO streams with different chunk sizes: the slots are fixed pieces of the staging
 # buffer, so the per-slot events order the two calls whatever their chunking (kvtier.h "A kv_ctx ...")
 # ------------------------------------------------------------------------------------------------
+@pytest.mark.parametrize("lead_mib,repage", [(-1, False), (0, False), (100, False), (-1, True), (8, True)])
+def test_staged_transfer_with_a_short_leading_chunk(kv, lead_mib, repage):
+    """Staged page-first transfers of 128 MiB or more lead an offload / end a reload with a SHORT chunk
+    (KV_OPT_LEAD_CHUNK, default 32 MiB) so that the one kernel no copy hides is a short one: unequal chunks, the
+    oracle's bytes (reload also with re-paging 16 -> 64, where a chunk must hold whole pages of both sizes)."""
+    L, C, P, T, H, D, e = 16, 2, 330, 16, 4, 128, 2  # page = 512 KiB; 300 pages = 150 MiB
+    rng = np.random.default_rng(11 + lead_mib + 7 * repage)
+    A = host_pool(rng, L, C, P, T, H, D, e)
+    tA, dA = to_device(A, kv, torch)
+    n = 300
+    ids = rng.choice(P, n, replace=False).astype(np.int32)
+    page = dA.page_bytes()
+    ctx = kv.Ctx(0, staging_bytes=256 << 20)  # two slots of 128 MiB
+    try:
+        if lead_mib >= 0:
+            ctx.set_option(kv.KV_OPT_LEAD_CHUNK, lead_mib << 20)
+        hp = kv.kv_host_alloc(n * page)
+        kv.host_view(hp, n * page)[:] = 0xEE
+        l0, m0 = ctx.stat(kv.KV_STAT_LAUNCHES), ctx.stat(kv.KV_STAT_MEMCPYS)
+        kv.kv_offload(ctx, dA, L, ids, hp, n * page, mode=kv.KV_HOST_STAGED)
+        torch.cuda.synchronize()
+        chunks = ctx.stat(kv.KV_STAT_LAUNCHES) - l0
+        assert chunks == ctx.stat(kv.KV_STAT_MEMCPYS) - m0
+        # equal chunks: two of 75 MiB; a 32 MiB lead: 32 + 118; a 100 MiB lead is more than half the payload: refused
+        assert chunks == (2 if lead_mib in (0, 100) else 2 if lead_mib == -1 else 3)
+        want = ko.pack(A, ids)
+        assert np.array_equal(kv.host_view(hp, n * page), want)
+        if repage:
+            Td, Pd = 64, 90
+            B = host_pool(rng, L, C, Pd, Td, H, D, e)
+            tB, dB = to_device(B, kv, torch)
+            ntok = n * T - 21
+            nd = -(-ntok // Td)
+            dst = rng.permutation(Pd)[:nd].astype(np.int32)
+            kv.kv_reload(ctx, hp, n * page, dst, dB, L, T, Td, ntok, mode=kv.KV_HOST_STAGED)
+            ko.unpack(want, dst, B, Ts=T, n_tokens=ntok)
+        else:
+            B = host_pool(rng, L, C, P, T, H, D, e)
+            tB, dB = to_device(B, kv, torch)
+            dst = rng.permutation(P)[:n].astype(np.int32)
+            kv.kv_reload(ctx, hp, n * page, dst, dB, L, T, T, n * T, mode=kv.KV_HOST_STAGED)
+            ko.unpack(want, dst, B, Ts=T, n_tokens=n * T)
+        torch.cuda.synchronize()
+        assert_pool_equal(tB, B)
+        assert_pool_equal(tA, A)
+    finally:
+        torch.cuda.synchronize()
+        kv.kv_host_free(hp)
+        ctx.close()
+
+
 @pytest.mark.parametrize("rep", range(3))
 def test_two_streams_one_ctx_staged_calls_share_the_slots(kv, rep):
     L, C, P, T, H, D, e = 8, 2, 512, 16, 4, 128, 2  # page = 256 KiB
