@@ -49,9 +49,10 @@ UNIT = "GB/s"
 # dram__bytes_read.sum + dram__bytes_write.sum of one kv_pack launch (mean of 4 launches) from an `ncu --set full` capture of
 # THIS command at THIS workload.  It is a profile figure, not something this run measures: it is emitted only when the run's
 # configuration is a profiled one (512 pages, NHD pool, the kernel the profile captured), with the file named beside it;
-# otherwise `traffic` is null.  kv_move_shot (AUTO's kernel at this size): 805.3 MB read + 753.1 MB written; the round-1
+# otherwise `traffic` is null.  kv_move_shot_plain (AUTO's kernel for this call): 805.3 MB read + 753.0 MB written; the round-1
 # ring (--kernel bulk): 805.4 + 759.3 (the last ~50 MB written are still dirty in L2 at exit).
-NCU_TRAFFIC = {"kv_move_shot": {"bytes_per_launch": 1558.4e6, "profile": "profiles/r02_kv_move_shot_full.md"},
+NCU_TRAFFIC = {"kv_move_shot_plain": {"bytes_per_launch": 1558.3e6, "profile": "profiles/r02_kv_move_shot_plain_full.md"},
+               "kv_move_shot": {"bytes_per_launch": 1558.4e6, "profile": "profiles/r02_kv_move_shot_full.md"},
                "kv_move_bulk": {"bytes_per_launch": 1564.6e6, "profile": "profiles/r01_kv_move_bulk_full.md"},
                "workload": {"pages": 512, "pool_order": "nhd", "min_pool_pages": 8192}}  # r02 was captured on a 12 GiB pool
 REFERENCE_WALL_CAP_S = 150.0  # the reference arm stops adding steps beyond this (and says so); 50 steps need ~8 s
