@@ -496,7 +496,10 @@ def run_ours(args):
                     torch.cuda.synchronize()
                 except Exception:  # noqa: BLE001
                     pass
-            barrier()  # every rank's peer traffic has ended before rank 0 times the other configs on its GPU
+            try:
+                barrier()  # every rank's peer traffic has ended before rank 0 times the other configs on its GPU
+            except Exception as exc:  # noqa: BLE001  (a sticky CUDA error left by a failed peer leg: keep the headline)
+                peer = dict(peer, after=f"{type(exc).__name__}: {exc}"[:300])
             if rank == 0 and args.pool_pages >= 65536 and args.pool_order == "nhd":
                 try:
                     per_config = bench_report.compact(ctx, desc, shape, u8, args.seed, measured_peaks()[0])
@@ -612,9 +615,12 @@ def run_ours(args):
         line["report"] = bench_report.write(rep_full)
         line["report"]["chain_oracle"] = chain_oracle
     if rank == 0:
-        print(json.dumps(line))
-    ctx.close()
-    rep.close()
+        print(json.dumps(line), flush=True)
+    try:
+        ctx.close()
+        rep.close()
+    except Exception:  # noqa: BLE001  (nothing after the line may turn a measured run into a failed one)
+        pass
 
 
 def main():
