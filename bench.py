@@ -484,27 +484,22 @@ def run_ours(args):
         if not args.no_per_config:
             link = bench_report.link_peaks(torch)
             dup_nosync["frac"] = dup_nosync["achieved"] / link["duplex_GBps"]
-            # The legs below come AFTER every timed region of the contract line; a failure in one of them (a box without
-            # peer access between its GPUs, not enough memory beside another rank's pool) is reported in its own key
-            # and never costs the run its headline numbers.
-            try:
-                peer = peer_leg(torch, kv, ctx, shape, local, args.seed)
-            except Exception as exc:  # noqa: BLE001
-                peer = {"available": False, "reason": f"peer leg failed: {type(exc).__name__}: {exc}"[:400]}
-                try:
-                    torch.cuda.set_device(local)
-                    torch.cuda.synchronize()
-                except Exception:  # noqa: BLE001
-                    pass
-            try:
-                barrier()  # every rank's peer traffic has ended before rank 0 times the other configs on its GPU
-            except Exception as exc:  # noqa: BLE001  (a sticky CUDA error left by a failed peer leg: keep the headline)
-                peer = dict(peer, after=f"{type(exc).__name__}: {exc}"[:300])
+            # The legs below come AFTER every timed region of the contract line; a failure in one of them (not enough
+            # memory beside another rank's pool, a box without peer access between its GPUs) is reported in its own key and
+            # never costs the run its headline numbers.  per_config first, then -- behind a barrier, so that no rank's peer
+            # traffic lands on rank 0's GPU while it times the other configs -- the peer leg, last because a fault in a
+            # path that no lease of this build has ever been able to run must not take anything else with it.
             if rank == 0 and args.pool_pages >= 65536 and args.pool_order == "nhd":
                 try:
                     per_config = bench_report.compact(ctx, desc, shape, u8, args.seed, measured_peaks()[0])
                 except Exception as exc:  # noqa: BLE001
                     per_config = {"error": f"{type(exc).__name__}: {exc}"[:400]}
+                torch.cuda.empty_cache()  # another rank's peer leg allocates its destination pool on this GPU
+            try:
+                barrier()
+                peer = peer_leg(torch, kv, ctx, shape, local, args.seed)
+            except Exception as exc:  # noqa: BLE001
+                peer = {"available": False, "reason": f"peer leg failed: {type(exc).__name__}: {exc}"[:400]}
 
     peak, peak_src = measured_peaks()
     value = world * 4 * payload * K / (t_total_ms * 1e-3) / 1e9
