@@ -447,12 +447,16 @@ def run_ours(args):
             duplex_step(i)
         barrier()
         e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+        e_step = [torch.cuda.Event(enable_timing=True) for _ in range(Ke)]
         e0.record(s_off)
         for i in range(Ke):
             duplex_step(Wm + i)
+            e_step[i].record(s_off)  # both streams idle: the step's end on the device clock
         e1.record(s_off)  # both streams were synchronised by the last step
         barrier()
         e2e_ms = max_over_ranks(e0.elapsed_time(e1))
+        torch.cuda.synchronize()
+        step_ms = [(e0 if i == 0 else e_step[i - 1]).elapsed_time(e_step[i]) for i in range(Ke)]
         # the same schedule with the two host syncs per step replaced by cross-stream events (offload i -> reload i+1
         # reads its buffer; reload i+1 -> offload i+2 overwrites it): what the link does when the host never waits
         done_off = [torch.cuda.Event() for _ in range(Ke + 1)]
@@ -528,6 +532,9 @@ def run_ours(args):
                         "on another, both through the C ABI, both streams synchronised every step.  `value` follows the metric's "
                         "convention (bytes read + written on each side of the link = 4*payload per step); link_GBps_payload is what "
                         "crosses the link, both directions summed",
+                "step_ms": {"mean": float(np.mean(step_ms)), "median": float(np.median(step_ms)), "best": float(np.min(step_ms)),
+                            "worst": float(np.max(step_ms)),
+                            "what": "this rank's Ke timed steps one by one (the link peaks beside them are best-of-20 figures)"},
                 "serial_value": world * 4 * payload / (serial_ms * 1e-3) / 1e9,
                 "serial_what": "same two calls on ONE stream, reload reading the buffer the offload just wrote"},
         "gpu_launches": launches,
@@ -550,8 +557,12 @@ def run_ours(args):
             "reload": {"achieved": rel_g, "peak": link["h2d_GBps"], "frac": rel_g / link["h2d_GBps"]},
             "duplex": {"achieved": dup_g, "peak": link["duplex_GBps"], "frac": dup_g / link["duplex_GBps"],
                        "frac_of_chunked_memcpy": dup_g / link["duplex_chunked_GBps"],
+                       "frac_best_step": 2 * payload / (min(step_ms) * 1e-3) / 1e9 / link["duplex_GBps"],
+                       "frac_median_step": 2 * payload / (float(np.median(step_ms)) * 1e-3) / 1e9 / link["duplex_GBps"],
                        "what": "the e2e leg (offload and reload at once, host sync every step) against D2H + H2D "
-                               "cudaMemcpyAsync at once (one copy each way); frac_of_chunked_memcpy = against the same plain "
+                               "cudaMemcpyAsync at once (one copy each way, best of 20); frac_best_step / frac_median_step = "
+                               "the best / median single step of the leg against that same best-of-20 peak (the link on this "
+                               "pool's VMs varies by +-2 % from pass to pass); frac_of_chunked_memcpy = against the same plain "
                                "copies issued as two per direction, the chunking of a staged 768 MiB transfer"},
             "duplex_no_host_sync": dup_nosync,
             "peaks": link, "host_mode": host_mode,

@@ -162,9 +162,9 @@ def link_peaks(torch, nbytes=1 << 30, reps=20):
     h2 = torch.empty(nbytes, dtype=torch.uint8, pin_memory=True)
     h.zero_()
     h2.zero_()  # touch the pages from the CPU once (first DMA passes over untouched pinned pages are slow)
-    _, t = _events(torch, lambda: a.copy_(h, non_blocking=True), reps, 2)
+    m_h2d, t = _events(torch, lambda: a.copy_(h, non_blocking=True), reps, 2)
     h2d = nbytes / t / 1e3
-    _, t = _events(torch, lambda: h.copy_(a, non_blocking=True), reps, 2)
+    m_d2h, t = _events(torch, lambda: h.copy_(a, non_blocking=True), reps, 2)
     d2h = nbytes / t / 1e3
     sa, sb = torch.cuda.Stream(), torch.cuda.Stream()
 
@@ -179,7 +179,7 @@ def link_peaks(torch, nbytes=1 << 30, reps=20):
         cur.wait_stream(sa)
         cur.wait_stream(sb)
 
-    _, t = _events(torch, both, reps, 2)
+    m_dup, t = _events(torch, both, reps, 2)
     duplex = 2 * nbytes / t / 1e3
     # the same bytes as TWO back-to-back copies per direction (the chunking of a staged 768 MiB transfer): with both
     # directions busy every copy boundary costs the link ~0.25 ms on this platform, for plain cudaMemcpyAsync too
@@ -204,6 +204,8 @@ def link_peaks(torch, nbytes=1 << 30, reps=20):
     del a, b, h, h2
     return {"h2d_GBps": h2d, "d2h_GBps": d2h, "duplex_GBps": duplex, "duplex_chunked_GBps": duplex3, "duplex_chunked_copies_each_way": K,
             "bytes": nbytes, "reps": reps,
+            "median": {"h2d_GBps": nbytes / m_h2d / 1e3, "d2h_GBps": nbytes / m_d2h / 1e3, "duplex_GBps": 2 * nbytes / m_dup / 1e3,
+                       "what": "the same passes, median instead of best (how far the link itself varies from pass to pass)"},
             "how": "pinned cudaMemcpyAsync (torch copy_ non_blocking), best of reps, CUDA events; duplex = D2H and H2D "
                    "of the same size on two streams, 2*bytes / time; duplex_chunked = the same bytes issued as "
                    "two back-to-back copies per direction (what chunking alone costs plain copies when both directions are busy)"}
