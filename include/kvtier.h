@@ -33,6 +33,8 @@
  *     STAGED host transfers are capturable too (copy nodes on a forked branch + one kernel node per chunk, each
  *     with its tables in its parameters) once the ctx's staging exists (KV_OPT_RESERVE_STAGING, or any earlier
  *     staged call): KV_HOST_AUTO then captures what it would run eagerly; without staging it captures DIRECT.
+ *     HND pools: a captured call whose pool has no tensor maps in device memory yet carries them in its kernel
+ *     parameters (same kernels); if tables and maps together exceed the parameter space it takes the lane paths.
  *     A graph holding staged transfers uses the ctx's staging buffer at every replay: replay it on the stream on
  *     which the ctx's other staged transfers run, or not at the same time as them.  Otherwise: KV_ERR_CAPTURE.
  *   - A kv_ctx is not thread-safe: one ctx per calling thread.  Calls on different streams are

@@ -27,6 +27,8 @@ struct Geom {
   // HND sides served by tensor copies: box of `tb` whole tokens, element width `tma_es` bytes
   bool tma = false;
   uint32_t tb = 0, tma_es = 0;
+  // the maps travel inside the kernel parameters (a captured call whose pool has no maps in device memory yet)
+  bool tma_inline = false;
 };
 
 struct Req {          // one request as the caller states it
@@ -108,29 +110,37 @@ uint32_t tma_elem_bytes(uint32_t drow) {
   return 0;
 }
 
-// Device array of LC tensor maps for pool `p` (slab = tensor (dim, head, token, page), box (drow, H, tb, 1)).
-// Built on first use: LC encoder calls + one blocking copy; never during stream capture (the caller checks).
-int get_maps(kv_ctx *ctx, const kv_pool_desc *p, uint32_t layer_count, uint32_t tb, uint32_t es, const uint8_t **out) {
-  std::vector<uint64_t> key;
-  map_key(p, layer_count, tb, es, &key);
-  if (const MapSet *m = find_maps(ctx, key)) { *out = (const uint8_t *)m->d; return KV_OK; }
-  const uint32_t LC = layer_count * p->kv_count;
+// Tensor maps of slabs [lc0, lc0 + lc_n) of pool `p` (slab = tensor (dim, head, token, page), box (drow, H, tb, 1)),
+// written to `maps`.  Pure host work: no CUDA call, so it is legal while a stream is being captured.
+int encode_maps(kv_ctx *ctx, const kv_pool_desc *p, uint32_t lc0, uint32_t lc_n, uint32_t tb, uint32_t es, CUtensorMap *maps) {
   const uint32_t drow = p->head_dim * p->elem_bytes;
   static const CUtensorMapDataType kTypes[9] = {CU_TENSOR_MAP_DATA_TYPE_UINT8, CU_TENSOR_MAP_DATA_TYPE_UINT8,
       CU_TENSOR_MAP_DATA_TYPE_UINT16, CU_TENSOR_MAP_DATA_TYPE_UINT16, CU_TENSOR_MAP_DATA_TYPE_UINT32,
       CU_TENSOR_MAP_DATA_TYPE_UINT32, CU_TENSOR_MAP_DATA_TYPE_UINT32, CU_TENSOR_MAP_DATA_TYPE_UINT32,
       CU_TENSOR_MAP_DATA_TYPE_UINT64};
-  std::vector<CUtensorMap> maps(LC);
   const cuuint64_t dims[4] = {drow / es, p->num_heads, p->page_size, p->num_pages};
   const cuuint64_t strides[3] = {(cuuint64_t)p->page_size * drow, drow, p->page_stride_bytes};
   const cuuint32_t box[4] = {drow / es, p->num_heads, tb, 1};
   const cuuint32_t ones[4] = {1, 1, 1, 1};
-  for (uint32_t i = 0; i < LC; ++i) {
-    CUresult r = ctx->encode_tiled(&maps[i], kTypes[es], 4, p->base[i], dims, strides, box, ones,
+  for (uint32_t i = 0; i < lc_n; ++i) {
+    CUresult r = ctx->encode_tiled(&maps[i], kTypes[es], 4, p->base[lc0 + i], dims, strides, box, ones,
                                    CU_TENSOR_MAP_INTERLEAVE_NONE, CU_TENSOR_MAP_SWIZZLE_NONE,
                                    CU_TENSOR_MAP_L2_PROMOTION_L2_256B, CU_TENSOR_MAP_FLOAT_OOB_FILL_NONE);
     if (r != CUDA_SUCCESS) { ctx->last_cuda_error = (int)r; return KV_ERR_CUDA; }
   }
+  return KV_OK;
+}
+
+// Device array of LC tensor maps for pool `p`, cached in the ctx per (pool, box).  Built on first use: LC encoder calls +
+// one blocking copy; never during stream capture (a captured call carries its maps in its parameters instead).
+int get_maps(kv_ctx *ctx, const kv_pool_desc *p, uint32_t layer_count, uint32_t tb, uint32_t es, const uint8_t **out) {
+  std::vector<uint64_t> key;
+  map_key(p, layer_count, tb, es, &key);
+  if (const MapSet *m = find_maps(ctx, key)) { *out = (const uint8_t *)m->d; return KV_OK; }
+  const uint32_t LC = layer_count * p->kv_count;
+  std::vector<CUtensorMap> maps(LC);
+  int rc = encode_maps(ctx, p, 0, LC, tb, es, maps.data());
+  if (rc) return rc;
   if (ctx->map_sets.size() >= kMaxMapSets) {  // rare: drop everything once nothing can still be reading it
     KV_CUDA(ctx, cudaDeviceSynchronize());
     for (MapSet &m : ctx->map_sets) cudaFree(m.d);
@@ -220,7 +230,18 @@ int make_geom(const kv_ctx *ctx, const kv_pool_desc *p, uint32_t layer_count, ui
         if (g.pool_hnd) { map_key(p, layer_count, tb, es, &key); cached_or_free = find_maps(ctx, key) != nullptr; }
         if (cached_or_free && g.src_hnd) { map_key(src_pool, layer_count, tb, es, &key); cached_or_free = find_maps(ctx, key) != nullptr; }
       }
-      if (cached_or_free) { g.tma = true; g.tb = tb; g.tma_es = es; }
+      if (cached_or_free) {
+        g.tma = true; g.tb = tb; g.tma_es = es;
+      } else if (ctx->inline_tables) {
+        // Capturing, and (one of) the pool(s) has no maps in device memory yet: encode them on the host and let them
+        // ride in the kernel parameters beside the tables, if everything fits there (one-request device transfers and
+        // DIRECT host transfers always do at the paper's shapes: 96 slabs x 128 B = 12 KiB).  Otherwise: lane paths.
+        uint64_t n_ids = 0;
+        for (const Req &r : reqs) n_ids += r.n_ids + (dir == 2 ? r.n_buf_pages : 0);
+        const uint64_t tables = (uint64_t)g.LC * 8 * (src_pool ? 2 : 1) + reqs.size() * sizeof(Piece) + n_ids * 4;
+        const uint64_t maps = (uint64_t)g.LC * sizeof(CUtensorMap) * ((g.pool_hnd ? 1 : 0) + (g.src_hnd ? 1 : 0));
+        if (tables + 128 + maps <= (uint64_t)kInlineLarge) { g.tma = true; g.tma_inline = true; g.tb = tb; g.tma_es = es; }
+      }
     }
   }
   if (kernel == KERNEL_AUTO) {

@@ -9,6 +9,8 @@ using kvt::Job;
 using kvt::Piece;
 
 constexpr int kBlobSlots = 16;
+constexpr int kInlineSmall = 3840;   // inline tables: the whole parameter block stays under the classic 4 KiB
+constexpr int kInlineLarge = 31744;  // CUDA 12.1+ large kernel parameters (<= 32,764 B)
 constexpr int kMaxStagingSlots = 4;
 constexpr uint32_t kMaxLayersKv = 4096;  // layer_count * kv_count
 constexpr uint64_t kAutoStagedMinBytes = 4ull << 20;

@@ -91,6 +91,11 @@ struct Job {
   // engine does the [head][token] <-> [token][head] transposition.
   const uint8_t *maps_pool;   // nullptr: the pool side does not use tensor copies
   const uint8_t *maps_src;    // dir 2: the source pool's maps
+  // The maps may instead ride INSIDE the kernel parameters (JobT<N>::blob, 64-byte aligned; 0 = they do not): a call
+  // captured into a CUDA graph before its pool's maps exist in device memory cannot build them there (an allocation
+  // and a blocking copy), but encoding a map is pure host work, and the copy engine reads a map from parameter space
+  // as well as from global memory.
+  uint32_t off_maps_pool, off_maps_src;
   uint32_t tb;                // tokens per box; a "full" item has bytes == valid == tb * tokrow
   // dir 2 with KV_FLAG_IDS_ON_DEVICE: the caller's device array of SOURCE page ids (then `ids` is the
   // caller's destination array and Piece::buf indexes this one); nullptr: both lists sit in `ids`
@@ -125,7 +130,7 @@ struct Tables {
 template <int N>
 struct JobT {
   Job j;
-  alignas(8) uint8_t blob[N];  // [bases: LC x u64][pieces][ids]
+  alignas(64) uint8_t blob[N];  // [bases: LC x u64][pieces][ids][64-byte aligned: tensor maps, if they travel here]
 };
 template <>
 struct JobT<0> {
@@ -561,8 +566,13 @@ __global__ void __launch_bounds__(kMaxWarps * 32, 1) kv_move_bulk(const __grid_c
       const uint32_t box_bytes = j.tb * j.tokrow;
       // (a mixed launch has one pool: whichever side of an item is strided is that pool; bit 2 of the mode keeps
       // copy-on-write rows on the lane paths)
-      const uint8_t *maps_s = j.dir == 2 ? j.maps_src : ((j.dir == 0 || j.dir == 4) ? j.maps_pool : nullptr);
-      const uint8_t *maps_d = (j.dir == 1 || j.dir == 2 || j.dir == 4) ? j.maps_pool : nullptr;
+      const uint8_t *mp = j.maps_pool, *ms = j.maps_src;
+      if constexpr (N > 0) {  // maps carried in the parameters (a first-ever captured call)
+        if (j.off_maps_pool) mp = p.blob + j.off_maps_pool;
+        if (j.off_maps_src) ms = p.blob + j.off_maps_src;
+      }
+      const uint8_t *maps_s = j.dir == 2 ? ms : ((j.dir == 0 || j.dir == 4) ? mp : nullptr);
+      const uint8_t *maps_d = (j.dir == 1 || j.dir == 2 || j.dir == 4) ? mp : nullptr;
       if (it >= depth && it - depth < n_known) {  // ---- store side: item si
         const uint64_t si = it - depth;
         const uint32_t s = (uint32_t)(si % K);
@@ -741,8 +751,13 @@ __global__ void __launch_bounds__(32) kv_move_shot(const __grid_constant__ JobT<
       const Strides st = strides_of(j);
       const uint32_t upr = j.drow >> 4;  // 16-byte units per head_dim row
       const uint32_t box_bytes = j.tb * j.tokrow;
-      const uint8_t *maps_s = j.dir == 2 ? j.maps_src : ((j.dir == 0 || j.dir == 4) ? j.maps_pool : nullptr);
-      const uint8_t *maps_d = (j.dir == 1 || j.dir == 2 || j.dir == 4) ? j.maps_pool : nullptr;
+      const uint8_t *mp = j.maps_pool, *ms = j.maps_src;
+      if constexpr (N > 0) {  // maps carried in the parameters (a first-ever captured call)
+        if (j.off_maps_pool) mp = p.blob + j.off_maps_pool;
+        if (j.off_maps_src) ms = p.blob + j.off_maps_src;
+      }
+      const uint8_t *maps_s = j.dir == 2 ? ms : ((j.dir == 0 || j.dir == 4) ? mp : nullptr);
+      const uint8_t *maps_d = (j.dir == 1 || j.dir == 2 || j.dir == 4) ? mp : nullptr;
       const bool whole = it.bytes == box_bytes && it.valid == box_bytes;
       if (it.valid) {  // ---- load
         if ((it.mode & 5) == 1 && maps_s && whole) {  // strided source, whole box: the copy engine gathers it in NHD order

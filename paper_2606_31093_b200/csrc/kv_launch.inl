@@ -11,6 +11,7 @@ namespace {
 struct HostBlob {
   std::vector<uint8_t> bytes;
   size_t off_pieces = 0, off_ids = 0;
+  size_t off_maps_pool = 0, off_maps_src = 0;  // tensor maps carried in the blob (0 = none); 64-byte aligned
 };
 
 // `pieces` / `n_pieces`: the pieces of the launch(es) the blob serves.  lc0 / lc_n: only the slab bases
@@ -28,6 +29,28 @@ void build_blob(const kv_pool_desc *p, const Geom &g, const Piece *pieces, size_
     for (uint32_t i = 0; i < lc_n; ++i) ((uint64_t *)h)[lc_n + i] = (uint64_t)(uintptr_t)g.src_pool->base[lc0 + i];
   if (n_pieces) std::memcpy(h + hb->off_pieces, pieces, n_pieces * sizeof(Piece));
   if (!ids_on_device && n_ids) std::memcpy(h + hb->off_ids, ids, (size_t)n_ids * 4);
+}
+
+// A captured HND call whose pool has no maps in device memory yet (Geom::tma_inline): the maps of slabs
+// [lc0, lc0 + lc_n) are encoded on the host and appended to the blob, 64-byte aligned (the blob itself is 64-byte
+// aligned inside the kernel parameters).
+int append_maps(kv_ctx *ctx, const Geom &g, HostBlob *hb, uint32_t lc0 = 0, uint32_t lc_n = 0) {
+  hb->off_maps_pool = hb->off_maps_src = 0;
+  if (!g.tma_inline) return KV_OK;
+  if (!lc_n) lc_n = g.LC;
+  auto add = [&](const kv_pool_desc *p, size_t *off) -> int {
+    const size_t at = (hb->bytes.size() + 63) / 64 * 64;
+    hb->bytes.resize(at + (size_t)lc_n * sizeof(CUtensorMap));
+    *off = at;
+    std::vector<CUtensorMap> maps(lc_n);  // (the vector's storage satisfies the encoder's alignment; the blob's may not)
+    int rc = encode_maps(ctx, p, lc0, lc_n, g.tb, g.tma_es, maps.data());
+    if (rc) return rc;
+    std::memcpy(hb->bytes.data() + at, maps.data(), (size_t)lc_n * sizeof(CUtensorMap));
+    return KV_OK;
+  };
+  if (g.pool_hnd) { int rc = add(g.dst_pool, &hb->off_maps_pool); if (rc) return rc; }
+  if (g.src_hnd) { int rc = add(g.src_pool, &hb->off_maps_src); if (rc) return rc; }
+  return KV_OK;
 }
 
 // Tables of a launch: either resident in device memory (slot of the pinned ring) or carried
@@ -97,11 +120,6 @@ struct BlobGuard {
   }
 };
 
-#ifndef KV_INLINE_SMALL
-#define KV_INLINE_SMALL 3840
-#endif
-constexpr int kInlineSmall = KV_INLINE_SMALL;   // whole parameter block stays under the classic 4 KiB
-constexpr int kInlineLarge = 31744;  // CUDA 12.1+ large kernel parameters (<= 32,764 B)
 
 template <int N>
 void launch_bulk(const Job &j, const HostBlob *hb, bool trans, uint32_t grid, uint32_t block, size_t smem,
@@ -194,7 +212,13 @@ int launch(kv_ctx *ctx, const Geom &g, const Blob &b, uint32_t piece_first, uint
     j.q_ts = g.drow; j.q_hs = (uint64_t)g.Tbuf * g.drow;  // dir 2: Tbuf is the source pool's page size
   }
   ctx->last_tma = 0;
-  if (g.tma && is_async_kernel(g.kernel)) {
+  if (g.tma && is_async_kernel(g.kernel) && g.tma_inline) {
+    if (!b.inl || (g.pool_hnd && !b.inl->off_maps_pool) || (g.src_hnd && !b.inl->off_maps_src)) return KV_ERR_CAPTURE;
+    j.tb = g.tb;
+    j.off_maps_pool = (uint32_t)b.inl->off_maps_pool;
+    j.off_maps_src = (uint32_t)b.inl->off_maps_src;
+    ctx->last_tma = 1;
+  } else if (g.tma && is_async_kernel(g.kernel)) {
     j.tb = g.tb;
     if (g.pool_hnd) {
       int rc = get_maps(ctx, g.dst_pool, g.L, g.tb, g.tma_es, &j.maps_pool);

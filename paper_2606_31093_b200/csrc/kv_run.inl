@@ -21,6 +21,8 @@ int run_single_launch(kv_ctx *ctx, const kv_pool_desc *pools, const Call &c, con
   const bool dev_ids = flags & KV_FLAG_IDS_ON_DEVICE;
   HostBlob hb;
   build_blob(pools, c.geom, pieces.data(), pieces.size(), ids, c.n_ids, dev_ids, &hb);
+  int rcm = append_maps(ctx, c.geom, &hb);
+  if (rcm) return rcm;
   Blob b;
   if (ctx->inline_tables && c.geom.kernel != KERNEL_ELEM && hb.bytes.size() <= (size_t)kInlineLarge) {
     b.inl = &hb;  // tables travel inside the kernel parameters: one launch, no copy
@@ -228,8 +230,9 @@ int run_staged(kv_ctx *ctx, const kv_pool_desc *pools, const Call &c, const int3
   const bool layer_range = layer_first;  // layer-first chunks launch over a slab range [l0*C, (l0+nl)*C)
   bool inline_ok = ctx->inline_tables && g.kernel != KERNEL_ELEM;
   for (const Chunk &ch : chunks) {
-    const size_t need = (size_t)(layer_range ? ch.nl * g.C : g.LC) * 8 + (size_t)ch.n_pieces * sizeof(Piece) +
-                        (dev_ids ? 0 : (size_t)(ch.id_hi - ch.id_lo) * 4);
+    const size_t n_lc = layer_range ? ch.nl * g.C : g.LC;
+    const size_t need = n_lc * 8 + (size_t)ch.n_pieces * sizeof(Piece) + (dev_ids ? 0 : (size_t)(ch.id_hi - ch.id_lo) * 4) +
+                        (g.tma_inline ? 64 + n_lc * sizeof(CUtensorMap) : 0);
     if (need > (size_t)kInlineLarge) inline_ok = false;
   }
   if (cap && !inline_ok) return KV_ERR_CAPTURE;
@@ -252,6 +255,8 @@ int run_staged(kv_ctx *ctx, const kv_pool_desc *pools, const Call &c, const int3
     build_blob(pools, g, chunk_pieces.data(), chunk_pieces.size(), dev_ids ? nullptr : ids + ch.id_lo,
                dev_ids ? 0 : ch.id_hi - ch.id_lo, dev_ids, &hb_chunk, layer_range ? ch.l0 * g.C : 0,
                layer_range ? ch.nl * g.C : 0);
+    int rcm = append_maps(ctx, g, &hb_chunk, layer_range ? ch.l0 * g.C : 0, layer_range ? ch.nl * g.C : 0);
+    if (rcm) return rcm;
     Blob b;
     b.inl = &hb_chunk;
     b.d_ids = dev_ids ? ids : nullptr;

@@ -364,35 +364,78 @@ def test_peer_enable_errors_on_this_box(kv, ctx):
 
 
 def test_cuda_graph_capture_of_hnd_transfer_uses_cached_tensor_maps(kv, ctx):
-    """Tensor maps are built (device allocation + blocking copy) on a pool's first use, which a capturing
-    stream cannot do: a first-ever captured HND call takes the lane paths, a warmed-up one the maps."""
+    """Tensor maps are built in device memory (an allocation + a blocking copy) on a pool's first use, which a
+    capturing stream cannot do.  A first-ever captured HND call therefore carries its maps INSIDE its kernel
+    parameters (encoding a map is pure host work); a warmed-up one uses the cached device copies.  Both replay the
+    oracle's bytes: pack, unpack, HND -> HND re-page and a staged offload, each captured before any live call."""
     L, C, P, T, H, D, e = 3, 2, 128, 16, 4, 128, 2
     rng = np.random.default_rng(101)
     A = host_pool(rng, L, C, P, T, H, D, e, order=ko.HND)
+    B = host_pool(rng, L, C, P, T, H, D, e, order=ko.HND)
+    Cq = host_pool(rng, L, C, 40, 64, H, D, e, order=ko.HND)  # re-page destination: 64-token pages
     tA, dA = to_device(A, kv, torch)
+    tB, dB = to_device(B, kv, torch)
+    tC, dC = to_device(Cq, kv, torch)
     n = 60
     ids = rng.choice(P, n, replace=False).astype(np.int32)
-    buf = torch.zeros(n * dA.page_bytes(), dtype=torch.uint8, device="cuda")
-    want = ko.pack(A, ids)
-    side = torch.cuda.Stream()
-    g = torch.cuda.CUDAGraph()
-    with torch.cuda.graph(g, stream=side):
-        kv.kv_pack(ctx, dA, L, ids, buf, stream=side)
-    assert ctx.stat(kv.KV_STAT_LAST_TENSOR_MAPS) == 0
-    g.replay()
-    torch.cuda.synchronize()
-    assert np.array_equal(buf.cpu().numpy(), want)
-    kv.kv_pack(ctx, dA, L, ids, buf)  # live call builds and caches the maps
-    assert ctx.stat(kv.KV_STAT_LAST_TENSOR_MAPS) == 1
-    torch.cuda.synchronize()
-    g2 = torch.cuda.CUDAGraph()
-    with torch.cuda.graph(g2, stream=side):
-        kv.kv_pack(ctx, dA, L, ids, buf, stream=side)
-    assert ctx.stat(kv.KV_STAT_LAST_TENSOR_MAPS) == 1
-    buf.zero_()
-    g2.replay()
-    torch.cuda.synchronize()
-    assert np.array_equal(buf.cpu().numpy(), want)
+    dst = rng.permutation(P)[:n].astype(np.int32)
+    dst64 = rng.permutation(40)[:n * T // 64].astype(np.int32)
+    nbytes = n * dA.page_bytes()
+    buf = torch.zeros(nbytes, dtype=torch.uint8, device="cuda")
+    hp = kv.kv_host_alloc(nbytes)
+    try:
+        kv.host_view(hp, nbytes)[:] = 0
+        ctx.set_option(kv.KV_OPT_RESERVE_STAGING, 0)  # a captured STAGED transfer needs the staging to exist
+        want = ko.pack(A, ids)
+        side = torch.cuda.Stream()
+        g = torch.cuda.CUDAGraph()
+        with torch.cuda.graph(g, stream=side):
+            kv.kv_pack(ctx, dA, L, ids, buf, stream=side)
+            assert ctx.stat(kv.KV_STAT_LAST_TENSOR_MAPS) == 1  # maps in the parameters
+            kv.kv_unpack(ctx, buf, dst, dB, L, T, T, n * T, stream=side)
+            assert ctx.stat(kv.KV_STAT_LAST_TENSOR_MAPS) == 1
+            kv.kv_repage(ctx, dA, ids, dC, dst64, L, n * T, stream=side)
+            assert ctx.stat(kv.KV_STAT_LAST_TENSOR_MAPS) == 1
+            kv.kv_offload(ctx, dA, L, ids, hp, nbytes, mode=kv.KV_HOST_STAGED, stream=side)
+            assert ctx.stat(kv.KV_STAT_LAST_TENSOR_MAPS) == 1
+        g.replay()
+        torch.cuda.synchronize()
+        assert np.array_equal(buf.cpu().numpy(), want)
+        assert np.array_equal(kv.host_view(hp, nbytes), want)
+        ko.unpack(want, dst, B, Ts=T, n_tokens=n * T)
+        assert_pool_equal(tB, B)
+        ko.unpack(want, dst64, Cq, Ts=T, n_tokens=n * T)
+        assert_pool_equal(tC, Cq)
+        assert_pool_equal(tA, A)
+        kv.kv_pack(ctx, dA, L, ids, buf)  # live call builds and caches the maps in device memory
+        assert ctx.stat(kv.KV_STAT_LAST_TENSOR_MAPS) == 1
+        torch.cuda.synchronize()
+        g2 = torch.cuda.CUDAGraph()
+        with torch.cuda.graph(g2, stream=side):
+            kv.kv_pack(ctx, dA, L, ids, buf, stream=side)
+        assert ctx.stat(kv.KV_STAT_LAST_TENSOR_MAPS) == 1
+        buf.zero_()
+        g2.replay()
+        torch.cuda.synchronize()
+        assert np.array_equal(buf.cpu().numpy(), want)
+        # tensor maps switched off: a captured call takes the lane paths, as a live one does
+        ctx2 = kv.Ctx(0)
+        try:
+            ctx2.set_option(kv.KV_OPT_TENSOR_MAPS, 0)
+            g3 = torch.cuda.CUDAGraph()
+            with torch.cuda.graph(g3, stream=side):
+                kv.kv_pack(ctx2, dA, L, ids, buf, stream=side)
+            assert ctx2.stat(kv.KV_STAT_LAST_TENSOR_MAPS) == 0
+            buf.zero_()
+            g3.replay()
+            torch.cuda.synchronize()
+            assert np.array_equal(buf.cpu().numpy(), want)
+        finally:
+            torch.cuda.synchronize()
+            ctx2.close()
+    finally:
+        torch.cuda.synchronize()
+        kv.kv_host_free(hp)
 
 
 # ------------------------------------------------------------------------------------------------
