@@ -601,7 +601,7 @@ def run(ctx, desc, shape, slabs, seed=0, out_dir="gpurun_out", hbm_peak=None):
         rec("2 prefix", "offload and reload at once (two ctxs, two streams)", "auto", 2 * pl, 2 * pl, 2 * n,
             lambda: both(lambda: kv.kv_offload(ctx, desc, L, c2.src_ids, hp, pl, stream=sa),
                          lambda: kv.kv_reload(ctx2, hp + pl, pl, c2.dst_ids, desc, L, T, T, n * T, stream=sb)),
-            reps=7, link=duplex, before=lambda: (poison_host(), chk.poison(c2.dst_ids)),
+            reps=15, link=duplex, before=lambda: (poison_host(), chk.poison(c2.dst_ids)),  # the shared link varies by +-5 % from pass to pass
             check=lambda: chk.host_equals_device(hp, buf, n) and chk.unpack_ok(buf, c2.dst_ids))
         torch.cuda.synchronize()
         ctx2.close()

@@ -127,8 +127,9 @@ typedef enum kv_option {
   KV_OPT_MAX_CTAS = 5,       /* cap on the grid (0 = SM count x CTAs per SM) */
   KV_OPT_CHUNK_BYTES = 6,    /* staged host transfers: bytes per pipeline chunk (0 = automatic: equal chunks, at least two per
                                 transfer where that leaves 64 MiB each, at most one staging slot each) */
-  KV_OPT_HOST_MAX_CTAS = 7,  /* grid cap for DIRECT host transfers (default 64: the link saturates with far fewer CTAs than
-                                HBM, and small transfers finish sooner -- 1 MiB 39 -> 34 us; 0 = same as device transfers) */
+  KV_OPT_HOST_MAX_CTAS = 7,  /* grid cap for DIRECT host transfers (0 = automatic: 64 CTAs up to 16 MiB of payload -- the link
+                                saturates with far fewer CTAs than HBM and small transfers finish sooner, 1 MiB 39 -> 34 us --
+                                and the device grid above) */
   KV_OPT_STAGING_SLOTS = 8,  /* staged host transfers: pipeline slots the staging buffer is cut into (2 .. 4) */
   KV_OPT_L2_HINT = 9,        /* bulk: L2 cache hints, a bit set: 1 = loads evict_first, 2 = stores evict_first, 4 = stores
                                 evict_last (2 and 4 exclude each other: 0 .. 5) */

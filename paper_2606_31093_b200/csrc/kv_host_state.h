@@ -68,7 +68,7 @@ struct kv_ctx {
   int last_cuda_error = 0;
   // options
   int kernel = KERNEL_AUTO;
-  uint32_t stage_bytes = 16384, stages = 4, warps = 2, lag = 2, max_ctas = 0, host_max_ctas = 64;
+  uint32_t stage_bytes = 16384, stages = 4, warps = 2, lag = 2, max_ctas = 0, host_max_ctas = 0;
   uint32_t lead_chunk = 32u << 20;  // KV_OPT_LEAD_CHUNK: bytes of the short leading (offload) / trailing (reload) chunk; 0 = equal chunks
   bool auto_geom = true;  // ring geometry follows the segment size until the caller sets stages / warps / stage bytes
   // bulk geometry of transposing transfers (an HND pool): rows are gathered with 16-byte cp.async by all

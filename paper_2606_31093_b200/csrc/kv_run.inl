@@ -406,7 +406,12 @@ int run_host(kv_ctx *ctx, const kv_pool_desc *pools, Call &c, const int32_t *ids
   }
   // DIRECT: one launch moves every layer (the flags follow it together)
   for (size_t i = 0; i < c.reqs.size(); ++i) c.reqs[i].buf = alias[i];
-  rc = run_single_launch(ctx, pools, c, ids, flags, ctx->host_max_ctas, s);
+  // Small DIRECT transfers (the only ones AUTO still sends this way) finish sooner with few CTAs: the link saturates with
+  // far fewer of them than HBM (1 MiB: 39 us with 256 CTAs, 34 with 64; 2 MiB 58 -> 54).  Large ones keep the device
+  // grid: with the general kernel (batches, layer-first buffers) 64 CTAs cost 2-3 % of the link (26.5 GiB batched
+  // 52.7 -> 50.8 GB/s).
+  const uint32_t cta_cap = ctx->host_max_ctas ? ctx->host_max_ctas : (c.payload <= ((uint64_t)16 << 20) ? 64u : 0u);
+  rc = run_single_launch(ctx, pools, c, ids, flags, cta_cap, s);
   if (rc || !lf.flags) return rc;
   for (uint32_t l0 = 0; l0 < c.geom.L; l0 += 32) {
     kvt::kv_signal_range<<<1, 32, 0, s>>>(lf.flags + l0, std::min(32u, c.geom.L - l0), lf.value);
