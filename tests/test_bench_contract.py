@@ -69,6 +69,12 @@ def test_our_arm_prints_the_contract_line():
     for k in ("offload", "reload", "duplex"):
         assert 0 < h[k]["frac"] == pytest.approx(h[k]["achieved"] / h[k]["peak"])
     assert h["peaks"]["h2d_GBps"] > 0 and h["peaks"]["d2h_GBps"] > 0 and h["peaks"]["duplex_GBps"] > 0
+    # the e2e leg's steps one by one, and the link peaks' medians beside their best-of-20 figures
+    sm = e["step_ms"]
+    assert 0 < sm["best"] <= sm["median"] <= sm["worst"] and sm["best"] <= sm["mean"] <= sm["worst"]
+    assert h["duplex"]["frac_best_step"] >= h["duplex"]["frac_median_step"] > 0
+    assert 0 < h["peaks"]["median"]["duplex_GBps"] <= h["peaks"]["duplex_GBps"]
+    assert r["kernel"].startswith("kv_move_shot_plain")  # the plain single-request case takes the short kernel
     assert "per_config" not in line  # needs the 96 GiB pool
     assert line["peer"]["available"] in (True, False)
     if line["peer"]["available"]:
