@@ -717,7 +717,7 @@ __global__ void __launch_bounds__(kMaxWarps * 32, 1) kv_move_bulk(const __grid_c
 // segments in flight as its shared memory takes (13-14 x 16 KiB: ~220 KiB per SM, 32 MB per chip, against the ~128 KiB
 // per SM of the persistent ring), loads and stores of different CTAs overlap freely, a finished CTA is replaced at
 // once, and there is no ring, no claim counter and no tail to balance.  Measured on B200 against a plain contiguous
-// cudaMemcpyAsync of the same size under the same conditions (isolated call, cold clean L2; _work probe of round 2):
+// cudaMemcpyAsync of the same size under the same conditions (isolated call, cold clean L2; a one-off probe of round 2):
 // a minimal kernel of this shape equals the plain copy from 1 MiB to 768 MiB (64 MiB 21.8 vs 21.5 us, 768 MiB 239 vs
 // 242 us) where the ring needed 27.7 / 249 us.  DESIGN.md "Kernels".
 // gridDim.x may be capped (KV_OPT_MAX_CTAS): a CTA then walks items blockIdx.x, + gridDim.x, ... reusing its stage.
