@@ -557,10 +557,13 @@ def run_ours(args):
             "reload": {"achieved": rel_g, "peak": link["h2d_GBps"], "frac": rel_g / link["h2d_GBps"]},
             "duplex": {"achieved": dup_g, "peak": link["duplex_GBps"], "frac": dup_g / link["duplex_GBps"],
                        "frac_of_chunked_memcpy": dup_g / link["duplex_chunked_GBps"],
+                       "frac_of_median_memcpy": dup_g / link["median"]["duplex_GBps"],
                        "frac_best_step": 2 * payload / (min(step_ms) * 1e-3) / 1e9 / link["duplex_GBps"],
                        "frac_median_step": 2 * payload / (float(np.median(step_ms)) * 1e-3) / 1e9 / link["duplex_GBps"],
                        "what": "the e2e leg (offload and reload at once, host sync every step) against D2H + H2D "
-                               "cudaMemcpyAsync at once (one copy each way, best of 20); frac_best_step / frac_median_step = "
+                               "cudaMemcpyAsync at once (one copy each way, best of 20); frac_of_median_memcpy = the leg's MEAN "
+                               "against the MEDIAN of those 20 plain passes (mean against best is not like against like when "
+                               "the link itself spreads); frac_best_step / frac_median_step = "
                                "the best / median single step of the leg against that same best-of-20 peak (the link on this "
                                "pool's VMs varies by +-2 % from pass to pass); frac_of_chunked_memcpy = against the same plain "
                                "copies issued as two per direction, the chunking of a staged 768 MiB transfer"},

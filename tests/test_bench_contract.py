@@ -73,6 +73,7 @@ def test_our_arm_prints_the_contract_line():
     sm = e["step_ms"]
     assert 0 < sm["best"] <= sm["median"] <= sm["worst"] and sm["best"] <= sm["mean"] <= sm["worst"]
     assert h["duplex"]["frac_best_step"] >= h["duplex"]["frac_median_step"] > 0
+    assert h["duplex"]["frac_of_median_memcpy"] >= h["duplex"]["frac"] > 0
     assert 0 < h["peaks"]["median"]["duplex_GBps"] <= h["peaks"]["duplex_GBps"]
     assert r["kernel"].startswith("kv_move_shot_plain")  # the plain single-request case takes the short kernel
     assert "per_config" not in line  # needs the 96 GiB pool
