@@ -453,6 +453,27 @@ def run(ctx, desc, shape, slabs, seed=0, out_dir="gpurun_out", hbm_peak=None):
     rec("2 prefix", "unpack", "device", pl, 2 * pl, n,
         lambda: kv.kv_unpack(ctx, buf, c2.dst_ids, desc, L, T, T, n * T), reps=20, warm=3,
         before=lambda: chk.poison(c2.dst_ids), check=lambda: chk.unpack_ok(buf, c2.dst_ids))
+    # What the paper's "PyTorch fallback for unsupported layouts" would pay for the same two transfers on
+    # this GPU: plain torch indexing, one gather / scatter per (layer, K|V) slab (96 launches each) -- context beside the
+    # kernel's figure, not a baseline the library uses (it has no PyTorch path).
+    idx_src = torch.as_tensor(c2.src_ids.astype(np.int64), device="cuda")
+    idx_dst = torch.as_tensor(c2.dst_ids.astype(np.int64), device="cuda")
+    slab_rows = [s_.view(shape.P, row) for s_ in slabs]
+    buf3 = buf.view(n, LC, row)
+    tbuf = {}
+
+    def torch_pack():
+        tbuf["x"] = torch.stack([sr.index_select(0, idx_src) for sr in slab_rows], dim=1)  # [page][layer*kv][row]: page-first
+
+    def torch_unpack():
+        for lc_, sr in enumerate(slab_rows):
+            sr.index_copy_(0, idx_dst, buf3[:, lc_])
+
+    rec("2 prefix", "pack by torch index_select + stack (the paper's PyTorch-fallback shape)", "torch, 97 launches", pl, 2 * pl, n,
+        torch_pack, reps=7, warm=2, check=lambda: bool(torch.equal(tbuf["x"].view(-1), buf)))
+    tbuf.clear()
+    rec("2 prefix", "unpack by torch index_copy_ per slab (the paper's PyTorch-fallback shape)", "torch, 96 launches", pl, 2 * pl, n,
+        torch_unpack, reps=7, warm=2, before=lambda: chk.poison(c2.dst_ids), check=lambda: chk.unpack_ok(buf, c2.dst_ids))
     # ---- fragmentation (SURVEY.md 8(d) "structure of the workloads" (i)): the same 512 pages in runs of r
     # consecutive ids (run starts drawn at random, runs disjoint); r = 1 is the aged pool of the configs,
     # r = n a fresh one.  Consecutive pages are adjacent within a slab but stay a page apart in the buffer,
