@@ -170,11 +170,13 @@ def test_staged_offload_and_reload_captured_and_replayed(kv, layout, dev_ids):
         d_dst = torch.from_numpy(dst0).cuda()
         # without a staging buffer an explicit STAGED cannot be captured (an allocation would break the capture)
         g0 = torch.cuda.CUDAGraph()
+        flag0 = torch.zeros(1, dtype=torch.int64, device="cuda")  # (allocated before the capture: no allocation inside one)
+        torch.cuda.synchronize()
         with torch.cuda.graph(g0, stream=side):
             with pytest.raises(kv.KvError) as ei:
                 kv.kv_offload(ctx, dA, L, src0, hp, nbytes, mode=kv.KV_HOST_STAGED, layout=layout, stream=side)
             assert ei.value.status == kv.KV_ERR_CAPTURE
-            kv.kv_signal(ctx, torch.zeros(1, dtype=torch.int64, device="cuda"), 1, stream=side)  # a graph must not be empty
+            kv.kv_signal(ctx, flag0, 1, stream=side)  # a graph must not be empty
         ctx.set_option(kv.KV_OPT_RESERVE_STAGING, 0)
         memcpys = ctx.stat(kv.KV_STAT_MEMCPYS)
         g = torch.cuda.CUDAGraph()
