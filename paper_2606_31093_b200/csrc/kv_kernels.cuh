@@ -107,9 +107,10 @@ struct Job {
   // Exact n / d for n < 2^32 by ONE 64-bit multiply-high: m = floor(2^64 / d) + 1 (0 stands for d == 1).  The divisors
   // are launch constants; a hardware-less 32-bit division costs ~20 dependent instructions, and decode chains three.
   uint64_t m_subs, m_LC, m_cpp_pool, m_cpp_buf;
-  // The plain case -- ONE request, pack or unpack between equal page sizes, page-first buffer, every token valid, page
-  // ids validated on the host: decode takes a short straight path (two multiply-highs, two table reads, six
-  // multiply-adds).  A single-warp CTA hides no latency, so the ~300 dependent instructions of the general decode are
+  // The plain case -- pack or unpack between equal page sizes, page-first buffer(s), every token valid, page ids
+  // validated on the host; 1 = ONE request (its piece rides in `one`), 2 = a batch of such requests (the plain kernel
+  // finds an item's piece by binary search; the general kernel ignores the value 2): decode takes a short straight path
+  // (two multiply-highs, two table reads, six multiply-adds).  A single-warp CTA hides no latency, so the ~300 dependent instructions of the general decode are
   // ~0.7 us in front of the first load of every CTA -- nothing at 768 MiB (13 CTAs per SM overlap), a quarter of a
   // 1 MiB call.
   uint32_t lean;
@@ -168,14 +169,15 @@ struct Item {
 
 // SURVEY.md 8(a) a2 for the plain case (Job::lean): flat item -> (page, layer/kv, sub) -> addresses.
 struct Lean { uint64_t src, dst; uint32_t bytes; };
+// `item` counts within the piece; buf / id_begin are the piece's (Job::one for a one-request launch).
 template <bool kGlobal>
-__device__ __forceinline__ Lean decode_lean(const Job &j, const Tables &tb, uint32_t item) {
+__device__ __forceinline__ Lean decode_lean(const Job &j, const Tables &tb, uint32_t item, uint64_t buf, uint64_t id_begin) {
   const uint32_t r1 = fdiv(item, j.m_subs), sub = item - r1 * j.subs;
   const uint32_t pp = fdiv(r1, j.m_LC), lc = r1 - pp * j.LC;
   const uint32_t sub_off = sub * j.sub_bytes;
-  const int32_t id = kGlobal ? __ldg(tb.ids + j.one.id_begin + pp) : tb.ids[j.one.id_begin + pp];
+  const int32_t id = kGlobal ? __ldg(tb.ids + id_begin + pp) : tb.ids[id_begin + pp];
   const uint64_t paddr = ldt<kGlobal>(tb.bases + lc) + (uint64_t)(uint32_t)id * j.page_stride + sub_off;
-  const uint64_t baddr = j.one.buf + (uint64_t)pp * j.buf_page_bytes + (uint64_t)lc * j.buf_row_bytes + sub_off;
+  const uint64_t baddr = buf + (uint64_t)pp * j.buf_page_bytes + (uint64_t)lc * j.buf_row_bytes + sub_off;
   Lean l;
   l.bytes = min(j.sub_bytes, j.chunk_bytes - sub_off);
   l.src = j.dir == 0 ? paddr : baddr;
@@ -189,8 +191,8 @@ template <bool kGlobal, bool kTrans = false>
 // there and gallops forward: one or two probes where a search over all pieces takes log2(n) dependent loads
 // (2,048 one-page requests in one call: unpack 5.43 -> 5.87 TB/s; 64 requests: unchanged at 6.6).
 __device__ __forceinline__ Item decode(const Job &j, const Tables &tb, uint64_t item, uint32_t &hint) {
-  if (!kTrans && j.lean) {  // launch() sets it: dir 0 / 1, one piece, page-first, Tpool == Tbuf, no padding, host ids
-    const Lean l = decode_lean<kGlobal>(j, tb, (uint32_t)item);
+  if (!kTrans && j.lean == 1) {  // launch() sets it: dir 0 / 1, one piece, page-first, Tpool == Tbuf, no padding, host ids
+    const Lean l = decode_lean<kGlobal>(j, tb, (uint32_t)item, j.one.buf, j.one.id_begin);
     Item it;
     it.mode = 0; it.r0 = 0; it.lc = 0; it.s_pg = it.s_t = it.d_pg = it.d_t = 0;
     it.src = l.src; it.dst = l.dst; it.bytes = it.valid = l.bytes;
@@ -852,7 +854,17 @@ __global__ void __launch_bounds__(32) kv_move_shot_plain(const __grid_constant__
   asm volatile("griddepcontrol.wait;" ::: "memory");  // nothing global is touched before this
   uint32_t phase = 0;
   for (uint64_t item = blockIdx.x; item < j.total_items; item += gridDim.x) {
-    const Lean l = decode_lean<N == 0>(j, tb, (uint32_t)item);
+    uint64_t item_begin = 0, buf = j.one.buf, id_begin = j.one.id_begin;
+    if (j.n_pieces > 1) {  // a batch (Job::lean == 2): largest r with pieces[r].item_begin <= item
+      uint32_t lo = 0, hi = j.n_pieces;
+      while (hi - lo > 1) {
+        const uint32_t mid = (lo + hi) >> 1;
+        if (ldt<N == 0>(&tb.pieces[mid].item_begin) <= item) lo = mid; else hi = mid;
+      }
+      const Piece *pc = tb.pieces + lo;
+      item_begin = ldt<N == 0>(&pc->item_begin); buf = ldt<N == 0>(&pc->buf); id_begin = ldt<N == 0>(&pc->id_begin);
+    }
+    const Lean l = decode_lean<N == 0>(j, tb, (uint32_t)(item - item_begin), buf, id_begin);
     mbar_expect_tx(bar, l.bytes);
     bulk_g2s(sbase, l.src, l.bytes, bar);
     mbar_wait(bar, phase);

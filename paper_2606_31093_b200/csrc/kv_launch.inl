@@ -197,9 +197,15 @@ int launch(kv_ctx *ctx, const Geom &g, const Blob &b, uint32_t piece_first, uint
     j.one = hp[piece_first];
   }
   // the short decode path (kv_kernels.cuh Job::lean): host ids only (validated before any launch), nothing to zero-fill
-  j.lean = n_pieces == 1 && (g.dir == 0 || g.dir == 1) && g.layout == KV_LAYOUT_PAGE_FIRST && g.Tpool == g.Tbuf &&
-           !g.trans && !b.caller_ids && j.one.item_begin == 0 && j.one.n_buf_pages * (uint64_t)g.Tbuf <= j.one.n_tokens &&
-           total_items <= 0xffffffffull;
+  j.lean = 0;
+  if ((g.dir == 0 || g.dir == 1) && g.layout == KV_LAYOUT_PAGE_FIRST && g.Tpool == g.Tbuf && !g.trans && !b.caller_ids &&
+      total_items <= 0xffffffffull) {
+    const Piece *hp = b.inl ? (const Piece *)(b.inl->bytes.data() + b.inl->off_pieces) : b.h_pieces;
+    bool full = hp != nullptr && hp[piece_first].item_begin == 0;
+    for (uint32_t k = 0; full && k < n_pieces; ++k)  // nothing to zero-fill in any request
+      full = hp[piece_first + k].n_buf_pages * (uint64_t)g.Tbuf <= hp[piece_first + k].n_tokens;
+    if (full) j.lean = n_pieces == 1 ? 1 : 2;
+  }
   auto magic = [](uint32_t d) -> uint64_t { return d <= 1 ? 0ull : ~0ull / d + 1; };  // floor(2^64 / d) + 1 unless d | 2^64
   j.m_subs = magic(j.subs); j.m_LC = magic(j.LC); j.m_cpp_pool = magic(j.cpp_pool); j.m_cpp_buf = magic(j.cpp_buf);
   if (g.src_pool) { j.src_num_pages = g.src_pool->num_pages; j.src_page_stride = g.src_pool->page_stride_bytes; }

@@ -71,17 +71,19 @@ def test_pack_unpack_same_page_size(kv, ctx, kernel, shape):
 
 
 @pytest.mark.parametrize("shape", [SHAPES[0], SHAPES[1], SHAPES[2], SHAPES[4]])
-@pytest.mark.parametrize("variant", ["plain", "plain_capped", "general_l2hint", "plain_batched_1", "general_batched_2"])
+@pytest.mark.parametrize("variant", ["plain", "plain_capped", "general_l2hint", "plain_batched_1", "plain_batched_2",
+                                     "plain_batched_5_capped"])
 def test_plain_kernel_and_general_kernel_agree_with_the_oracle(kv, ctx, shape, variant):
-    """The plain case (one request, equal page sizes, page-first, nothing to zero-fill, host ids) runs the short
-    kernel kv_move_shot_plain; anything else -- here an L2 hint, or a second request -- the general kv_move_shot.
-    Both must give the oracle's bytes; a capped grid makes every CTA of the plain kernel walk several items (the
-    stage and its mbarrier phase are reused)."""
+    """The plain case (equal page sizes, page-first, nothing to zero-fill, host ids; one request or a batch of such
+    requests, whose pieces the kernel then finds by binary search) runs the short kernel kv_move_shot_plain; anything
+    else -- here an L2 hint, or a ragged tail in one request of the batch -- the general kv_move_shot.  Both must give
+    the oracle's bytes; a capped grid makes every CTA of the plain kernel walk several items (the stage and its
+    mbarrier phase are reused, and consecutive items fall into different pieces)."""
     L, C, P, T, H, D, e, pad = shape
     rng = np.random.default_rng(7 + abs(hash((shape, variant))) % 2**31)
     if variant == "general_l2hint":
         ctx.set_option(kv.KV_OPT_L2_HINT, 1)
-    if variant == "plain_capped":
+    if variant.endswith("capped"):
         ctx.set_option(kv.KV_OPT_MAX_CTAS, 5)
     A = host_pool(rng, L, C, P, T, H, D, e, pad)
     B = host_pool(rng, L, C, P, T, H, D, e, pad)
@@ -94,8 +96,8 @@ def test_plain_kernel_and_general_kernel_agree_with_the_oracle(kv, ctx, shape, v
     buf = torch.full((n * page + 256,), 0xCD, dtype=torch.uint8, device="cuda")
     want_plain = 0 if variant.startswith("general") else 1
     if "batched" in variant:
-        n_req = int(variant[-1])
-        cut = [0, n] if n_req == 1 else [0, n // 3, n]
+        n_req = int(variant.split("_")[2])
+        cut = {1: [0, n], 2: [0, n // 3, n], 5: [0, 1, 1, n // 2, n - 2, n]}[n_req]  # (5: with an empty request)
         off = np.asarray(cut, dtype=np.int64)
         bufs = [buf[cut[r] * page:cut[r + 1] * page] for r in range(n_req)]
         kv.kv_pack_batched(ctx, dA, L, ids, off, bufs)
@@ -120,6 +122,12 @@ def test_plain_kernel_and_general_kernel_agree_with_the_oracle(kv, ctx, shape, v
         kv.kv_unpack(ctx, buf, dst, dB, L, T, T, n * T - 1, src_bytes=n * page)
         assert ctx.stat(kv.KV_STAT_LAST_PLAIN) == 0
         ko.unpack(want, dst, B, Ts=T, n_tokens=n * T - 1)
+        assert_pool_equal(tB, B)
+    if variant == "plain_batched_2":  # ... nor is a batch one of whose requests has one
+        ntok = np.asarray([(cut[1] - cut[0]) * T - 3, (cut[2] - cut[1]) * T], dtype=np.uint64)
+        kv.kv_unpack_batched(ctx, bufs, dst, off, ntok, dB, L, T, T)
+        assert ctx.stat(kv.KV_STAT_LAST_PLAIN) == 0
+        ko.unpack_batched([want[cut[r] * page:cut[r + 1] * page] for r in range(2)], dst, off, ntok, B, Ts=T)
         assert_pool_equal(tB, B)
 
 
