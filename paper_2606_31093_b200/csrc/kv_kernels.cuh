@@ -839,7 +839,9 @@ __global__ void __launch_bounds__(32) kv_move_shot(const __grid_constant__ JobT<
 // CTA hides no latency, so what sits between its start and its bulk load is paid in full by every small call (measured
 // in CUDA-graph replays of 1-16 MiB packs).  Lane 0 alone works; the other lanes leave at once.
 // ---------------------------------------------------------------------------------------------
-template <int N>
+// kTrans: the pool is HND and its whole-token boxes move by tensor copies (Job::tb, the per-slab maps): the pool side of an
+// item is (slab lc, first token, page) instead of an address; the buffer side is the same contiguous run.
+template <int N, bool kTrans>
 __global__ void __launch_bounds__(32) kv_move_shot_plain(const __grid_constant__ JobT<N> p) {
   const Job &j = p.j;
   const Tables tb = tables_of(p);
@@ -864,12 +866,30 @@ __global__ void __launch_bounds__(32) kv_move_shot_plain(const __grid_constant__
       const Piece *pc = tb.pieces + lo;
       item_begin = ldt<N == 0>(&pc->item_begin); buf = ldt<N == 0>(&pc->buf); id_begin = ldt<N == 0>(&pc->id_begin);
     }
-    const Lean l = decode_lean<N == 0>(j, tb, (uint32_t)(item - item_begin), buf, id_begin);
-    mbar_expect_tx(bar, l.bytes);
-    bulk_g2s(sbase, l.src, l.bytes, bar);
-    mbar_wait(bar, phase);
-    phase ^= 1;
-    bulk_s2g(l.dst, sbase, l.bytes);
+    if constexpr (kTrans) {
+      const uint8_t *maps = j.maps_pool;
+      if constexpr (N > 0) { if (j.off_maps_pool) maps = p.blob + j.off_maps_pool; }  // a first-ever captured call
+      const uint32_t local = (uint32_t)(item - item_begin);
+      const uint32_t r1 = fdiv(local, j.m_subs), sub = local - r1 * j.subs;
+      const uint32_t pp = fdiv(r1, j.m_LC), lc = r1 - pp * j.LC;
+      const int32_t id = (N == 0) ? __ldg(tb.ids + id_begin + pp) : tb.ids[id_begin + pp];
+      const uint64_t baddr = buf + (uint64_t)pp * j.buf_page_bytes + (uint64_t)lc * j.buf_row_bytes + (uint64_t)sub * j.sub_bytes;
+      const uint32_t bytes = j.sub_bytes, t = sub * j.tb;  // whole boxes only (Job::lean)
+      mbar_expect_tx(bar, bytes);
+      if (j.dir == 0) tensor_g2s(sbase, maps + (size_t)lc * 128, t, (uint32_t)id, bar);  // the copy engine gathers the box in NHD order
+      else bulk_g2s(sbase, baddr, bytes, bar);
+      mbar_wait(bar, phase);
+      phase ^= 1;
+      if (j.dir == 0) bulk_s2g(baddr, sbase, bytes);
+      else tensor_s2g(maps + (size_t)lc * 128, t, (uint32_t)id, sbase);  // ... and scatters it back into the HND page
+    } else {
+      const Lean l = decode_lean<N == 0>(j, tb, (uint32_t)(item - item_begin), buf, id_begin);
+      mbar_expect_tx(bar, l.bytes);
+      bulk_g2s(sbase, l.src, l.bytes, bar);
+      mbar_wait(bar, phase);
+      phase ^= 1;
+      bulk_s2g(l.dst, sbase, l.bytes);
+    }
     bulk_commit();
     bulk_wait_read<0>();  // the stage may be refilled (next item of a capped grid) or released (exit)
   }

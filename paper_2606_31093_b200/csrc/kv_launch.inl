@@ -150,8 +150,10 @@ void launch_shot(const Job &j, const HostBlob *hb, bool trans, uint32_t grid, si
   cudaLaunchConfig_t cfg = {};
   cfg.gridDim = dim3(grid); cfg.blockDim = dim3(32); cfg.dynamicSmemBytes = smem; cfg.stream = s;
   cfg.attrs = attr; cfg.numAttrs = pdl ? 1 : 0;
-  if (trans) (void)cudaLaunchKernelEx(&cfg, kvt::kv_move_shot<N, true>, p);
-  else if (j.lean && !j.l2_hint) (void)cudaLaunchKernelEx(&cfg, kvt::kv_move_shot_plain<N>, p);
+  if (j.lean && !j.l2_hint) {  // the plain case (for an HND pool: whole boxes by tensor copies)
+    if (trans) (void)cudaLaunchKernelEx(&cfg, kvt::kv_move_shot_plain<N, true>, p);
+    else (void)cudaLaunchKernelEx(&cfg, kvt::kv_move_shot_plain<N, false>, p);
+  } else if (trans) (void)cudaLaunchKernelEx(&cfg, kvt::kv_move_shot<N, true>, p);
   else (void)cudaLaunchKernelEx(&cfg, kvt::kv_move_shot<N, false>, p);
 }
 template <int N>
@@ -198,7 +200,8 @@ int launch(kv_ctx *ctx, const Geom &g, const Blob &b, uint32_t piece_first, uint
   }
   // the short decode path (kv_kernels.cuh Job::lean): host ids only (validated before any launch), nothing to zero-fill
   j.lean = 0;
-  if ((g.dir == 0 || g.dir == 1) && g.layout == KV_LAYOUT_PAGE_FIRST && g.Tpool == g.Tbuf && !g.trans && !b.caller_ids &&
+  if ((g.dir == 0 || g.dir == 1) && g.layout == KV_LAYOUT_PAGE_FIRST && g.Tpool == g.Tbuf && !b.caller_ids &&
+      (!g.trans || (g.tma && g.pool_hnd && g.kernel == KERNEL_SHOT && g.chunk_bytes % g.sub_bytes == 0)) &&
       total_items <= 0xffffffffull) {
     const Piece *hp = b.inl ? (const Piece *)(b.inl->bytes.data() + b.inl->off_pieces) : b.h_pieces;
     bool full = hp != nullptr && hp[piece_first].item_begin == 0;
@@ -315,7 +318,7 @@ int launch(kv_ctx *ctx, const Geom &g, const Blob &b, uint32_t piece_first, uint
   KV_CUDA(ctx, cudaGetLastError());
   ctx->launches++;
   ctx->last_grid = grid;
-  ctx->last_plain = g.kernel == KERNEL_SHOT && !g.trans && j.lean && !j.l2_hint;
+  ctx->last_plain = g.kernel == KERNEL_SHOT && j.lean && !j.l2_hint;
   return KV_OK;
 }
 

@@ -89,8 +89,10 @@ cudaError_t ctx_init_device(kv_ctx *ctx, int device) {
   const void *shot_kernels[] = {(const void *)kvt::kv_move_shot<0, false>, (const void *)kvt::kv_move_shot<kInlineSmall, false>,
                                 (const void *)kvt::kv_move_shot<kInlineLarge, false>, (const void *)kvt::kv_move_shot<0, true>,
                                 (const void *)kvt::kv_move_shot<kInlineSmall, true>, (const void *)kvt::kv_move_shot<kInlineLarge, true>,
-                                (const void *)kvt::kv_move_shot_plain<0>, (const void *)kvt::kv_move_shot_plain<kInlineSmall>,
-                                (const void *)kvt::kv_move_shot_plain<kInlineLarge>};
+                                (const void *)kvt::kv_move_shot_plain<0, false>, (const void *)kvt::kv_move_shot_plain<kInlineSmall, false>,
+                                (const void *)kvt::kv_move_shot_plain<kInlineLarge, false>, (const void *)kvt::kv_move_shot_plain<0, true>,
+                                (const void *)kvt::kv_move_shot_plain<kInlineSmall, true>,
+                                (const void *)kvt::kv_move_shot_plain<kInlineLarge, true>};
   for (const void *k : shot_kernels) {  // stages up to 64 KiB (KV_OPT_STAGE_BYTES); as many CTAs per SM as shared memory holds
     if ((e = cudaFuncSetAttribute(k, cudaFuncAttributeMaxDynamicSharedMemorySize, 65536)) != cudaSuccess) return e;
     if ((e = cudaFuncSetAttribute(k, cudaFuncAttributePreferredSharedMemoryCarveout, cudaSharedmemCarveoutMaxShared)) != cudaSuccess) return e;

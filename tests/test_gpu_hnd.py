@@ -278,3 +278,54 @@ def test_auto_kernel_choice_per_direction(kv, ctx):
     assert ctx.stat(kv.KV_STAT_LAST_KERNEL) == KERNELS["vec"]
     ko.unpack(wants, ids[::-1].copy(), S, Ts=4, n_tokens=n * 4)
     assert_pool_equal(tS, S)
+
+
+@pytest.mark.parametrize("variant", ["plain", "plain_capped", "general_l2hint", "plain_batched_3", "general_ragged"])
+@pytest.mark.parametrize("shape", [SHAPES[0], SHAPES[1], SHAPES[2], SHAPES[3]])
+def test_hnd_plain_kernel_and_general_kernel_agree_with_the_oracle(kv, variant, shape):
+    """HND pools: the plain case (equal page sizes, page-first, nothing to zero-fill, host ids, whole boxes by tensor
+    copies) takes the short kernel kv_move_shot_plain<.., kTrans> -- one tensor copy on the pool side, one bulk copy on
+    the buffer side, per single-warp CTA; an L2 hint or a ragged tail the general kernel.  Same bytes either way."""
+    L, C, P, T, H, D, e, pad, n = shape
+    rng = np.random.default_rng(3 + abs(hash((shape, variant))) % 2**31)
+    ctx = kv.Ctx(0)
+    try:
+        if variant == "general_l2hint":
+            ctx.set_option(kv.KV_OPT_L2_HINT, 1)
+        if variant.endswith("capped"):
+            ctx.set_option(kv.KV_OPT_MAX_CTAS, 7)
+        A = host_pool(rng, L, C, P, T, H, D, e, pad, order=HND)
+        B = host_pool(rng, L, C, P, T, H, D, e, pad, order=HND)
+        tA, dA = to_device(A, kv, torch)
+        tB, dB = to_device(B, kv, torch)
+        src = rng.choice(P, n, replace=False).astype(np.int32)
+        dst = rng.permutation(P)[:n].astype(np.int32)
+        page = dA.page_bytes()
+        buf = torch.full((n * page + 256,), 0xCD, dtype=torch.uint8, device="cuda")
+        want_plain = 0 if variant.startswith("general") else 1
+        ntok_all = n * T - (5 if variant == "general_ragged" and T > 5 else (1 if variant == "general_ragged" else 0))
+        if "batched" in variant:
+            cut = [0, n // 4, n // 4, n]  # an empty request in the middle
+            off = np.asarray(cut, dtype=np.int64)
+            bufs = [buf[cut[r] * page:cut[r + 1] * page] for r in range(3)]
+            kv.kv_pack_batched(ctx, dA, L, src, off, bufs)
+        else:
+            kv.kv_pack(ctx, dA, L, src, buf, dst_bytes=n * page)
+        assert ctx.stat(kv.KV_STAT_LAST_KERNEL) == kv.KV_KERNEL_SHOT and ctx.stat(kv.KV_STAT_LAST_TENSOR_MAPS) == 1
+        assert ctx.stat(kv.KV_STAT_LAST_PLAIN) == (0 if variant == "general_l2hint" else 1)  # a pack has no tail to pad
+        want = ko.pack(A, src)
+        got = buf.cpu().numpy()
+        assert np.array_equal(got[:want.size], want)
+        assert np.all(got[want.size:] == 0xCD), "wrote past the end of the buffer"
+        if "batched" in variant:
+            ntok = np.asarray([(cut[r + 1] - cut[r]) * T for r in range(3)], dtype=np.uint64)
+            kv.kv_unpack_batched(ctx, bufs, dst, off, ntok, dB, L, T, T)
+        else:
+            kv.kv_unpack(ctx, buf, dst, dB, L, T, T, ntok_all, src_bytes=n * page)
+        assert ctx.stat(kv.KV_STAT_LAST_PLAIN) == want_plain
+        ko.unpack(want, dst, B, Ts=T, n_tokens=ntok_all)
+        assert_pool_equal(tB, B)
+        assert_pool_equal(tA, A)
+    finally:
+        torch.cuda.synchronize()
+        ctx.close()
