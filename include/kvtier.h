@@ -109,6 +109,9 @@ typedef enum kv_status {
                              the kernel parameters (~31 KiB: about 7,500 page ids per launch), the element-wise
                              fallback kernel is needed, or mode is KV_HOST_STAGED and the ctx has no staging buffer
                              yet.  Nothing was enqueued. */
+  KV_ERR_STATIC_LIMIT = -12, /* kv_pack_static only: the request needs more table space than the library's fixed,
+                             built-in device array holds (more than KV_STATIC_MAX_PAGES page ids or more than
+                             KV_STATIC_MAX_SLABS layer x K/V slabs).  Nothing was enqueued; split the request. */
 } kv_status;
 
 /* flags (bit set) */
@@ -271,6 +274,59 @@ int kv_unpack_batched(kv_ctx *ctx, const void *const *srcs, const uint64_t *src_
                       const uint64_t *n_tokens, uint32_t n_req, const kv_pool_desc *pools,
                       uint32_t layer_count, uint32_t src_page_size, uint32_t dst_page_size,
                       int layout, uint32_t flags, kv_stream_t stream);
+
+/* ---- kv_pack without any allocation (for callers that must not allocate) ----------------------
+ * Who this is for.  Every other entry point needs a kv_ctx, and a ctx allocates: kv_ctx_create takes device memory,
+ * a stream and events, and a transfer whose lookup tables (slab bases + page ids) outgrow the kernel parameters
+ * (about 7,500 page ids) makes the ctx grow a pinned + device table arena INSIDE the call.  Some callers cannot live
+ * with that:
+ *   - a serving engine that has handed (nearly) all HBM to its KV pools: cudaMalloc would fail, or succeed only by
+ *     evicting something the engine counted on;
+ *   - a latency-critical step: cudaMalloc / cudaFree synchronise the whole device, so one allocation in a transfer
+ *     call stalls every stream of the process, not only the caller's;
+ *   - a process whose memory is owned by a pool allocator (or a sandbox / MPS client with a fixed memory budget) and
+ *     whose rules forbid raw CUDA allocations from a library.
+ * kv_pack_static is kv_pack for them: same bytes, no ctx, and neither it nor anything it calls ever calls cudaMalloc,
+ * cudaMallocHost, cudaFree, cudaStreamCreate, cudaEventCreate or any other allocating routine.
+ *
+ * What it does.  dst[p][l][c][t][h][d] = POOL[l][c][page_ids[p]][t][h][d] for p < n, the first `layer_count` layers of
+ * `pools`, page-first (KV_LAYOUT_PAGE_FIRST): byte for byte what kv_pack writes.  The kernel is the library's
+ * kv_move_shot_plain in its tables-in-device-memory form -- the form that otherwise reads its tables from the ctx's
+ * allocated arena.  Here the tables live in ONE fixed array that is part of the library image (a file-scope
+ * `static __device__` array in kvtier.cu, 256-byte aligned, KV_STATIC_TABLE_BYTES = 270,592 bytes, about 264 KiB).  The
+ * driver places a copy of it on every GPU on which this process uses the library, when the library's device code is
+ * loaded there, and that copy stays until the process exits; no call allocates or frees it.
+ *   device      CUDA device that owns `pools`, `dst` and `stream` (0 .. 63).  Made current for the call and restored.
+ *   pools       as kv_pack.  Restrictions of this entry point: NHD pools only (KV_ERR_LAYOUT for an HND pool), and every
+ *               slab base, the page stride, the token row (num_heads*head_dim*elem_bytes) and `dst` must be multiples
+ *               of 16 bytes (KV_ERR_ALIGN): there is no element-wise fallback here.
+ *   page_ids    HOST int32[n], sequence order, duplicates allowed; consumed before the call returns.
+ *   dst         device-accessible memory (device, or mapped pinned host), >= n*layer_count*kv_count*row bytes.
+ *   cuda_error  may be NULL; receives the cudaError_t behind a KV_ERR_CUDA (there is no ctx to ask).
+ * Limits: n <= KV_STATIC_MAX_PAGES (65,536 page ids: a 1M-token prefix at 16 tokens per page) and
+ * layer_count*kv_count <= KV_STATIC_MAX_SLABS (1,024).  Anything larger is refused with KV_ERR_STATIC_LIMIT before
+ * anything is enqueued -- the array cannot grow; split the request into several calls on the same stream.
+ *
+ * First call on a device.  The array's name is not a device address in host code; the first call on each device asks
+ * the runtime for that device's address of it (cudaGetSymbolAddress, with the device current), reads the SM count and
+ * sets the kernel's shared-memory preference, and remembers the result for the life of the process.  This may make the
+ * driver load the library's device code onto that GPU.  Make this first call (n = 1 is enough) during start-up, BEFORE
+ * the stream is put into CUDA-graph capture: the set-up calls are not stream work and do not belong in a capture.
+ *
+ * Sharing.  All calls on one device use the SAME array.  A call overwrites the table prefix it needs (header, slab
+ * bases, page ids) with small fill launches ahead of its copy kernel, all on `stream`; whatever a previous call left
+ * behind that prefix is never read, and the one word that has to be zero at kernel start (the kernels' status word, in
+ * the header) is rewritten as zero by every call.  Calls on ONE stream are therefore safe back to back.  Calls whose
+ * GPU work can overlap -- two streams without an event between them, two host threads, two graphs replayed at once --
+ * race on the tables and copy the wrong pages: order them (one stream, or events) yourself.  Nothing detects it.
+ * Other errors as kv_pack: KV_ERR_NULL, KV_ERR_DESC, KV_ERR_SIZE (dst_bytes too small, device out of range,
+ * more than 2^31-1 segments), KV_ERR_PAGE_RANGE, KV_ERR_CUDA.  A call that returns a validation error (anything but
+ * KV_ERR_CUDA) has written nothing.  n == 0: KV_OK, nothing enqueued. */
+#define KV_STATIC_MAX_PAGES 65536u
+#define KV_STATIC_MAX_SLABS 1024u
+#define KV_STATIC_TABLE_BYTES (256u + KV_STATIC_MAX_SLABS * 8u + KV_STATIC_MAX_PAGES * 4u)
+int kv_pack_static(int device, const kv_pool_desc *pools, uint32_t layer_count, const int32_t *page_ids, uint32_t n,
+                   void *dst, size_t dst_bytes, kv_stream_t stream, int *cuda_error);
 
 /* ---- several independent transfers in ONE launch ----------
  * A serving turn issues small transfers back to back -- scatter a matched prefix into fresh pages, extend the

@@ -9,6 +9,7 @@
 #include <cuda_runtime.h>
 
 #include <algorithm>
+#include <atomic>
 #include <cstring>
 #include <new>
 #include <numeric>
@@ -45,6 +46,8 @@ const char *kv_strerror(int status) {
     case KV_ERR_DESC: return "malformed kv_pool_desc";
     case KV_ERR_NO_DEVICE: return "planning-only context: nothing launched";
     case KV_ERR_CAPTURE: return "call cannot be captured into a CUDA graph (tables exceed the kernel parameters, or staged host mode)";
+    case KV_ERR_STATIC_LIMIT:
+      return "request exceeds the fixed table array of kv_pack_static (at most 65536 page ids and 1024 layer x K/V slabs per call): split it";
     default: return "unknown kvtier status";
   }
 }
@@ -570,3 +573,192 @@ int kv_reload_batched(kv_ctx *ctx, const void *const *host_srcs, const uint64_t 
 }
 
 }  // extern "C"
+
+
+// =============================================================================================
+// kv_pack_static -- kv_pack for callers that must not allocate (include/kvtier.h, "kv_pack without any allocation").
+//
+// The tables-in-device-memory form of kv_move_shot_plain (JobT<0>) normally reads slab bases and page ids from the
+// ctx's table arena, which upload_blob allocates (cudaMalloc + cudaMallocHost) inside the call.  Here the same kernel
+// reads them from the array below, which is part of the library image: nobody allocates it, nobody frees it, and this
+// code path contains no allocating CUDA call (its only working storage on the host is one thread_local parameter block).
+// =============================================================================================
+namespace {
+
+static_assert(sizeof(void *) == 8, "slab bases are copied as 64-bit addresses");
+constexpr uint32_t kStaticHeader = 256;  // bytes [0, 256): the kernels' status word (word 0) and padding, zero at kernel start
+static_assert(KV_STATIC_TABLE_BYTES == kStaticHeader + KV_STATIC_MAX_SLABS * 8u + KV_STATIC_MAX_PAGES * 4u, "kvtier.h states this size");
+static_assert(KV_STATIC_TABLE_BYTES % 16 == 0, "filled in 16-byte units");
+
+// [header: 256 B][slab bases: LC x u64, padded to 16 B][page ids: n x i32, padded to 16 B] of the call in flight.
+// One copy per GPU that loads this library, held until the process exits.  In HOST code this name is only a handle for
+// cudaGetSymbolAddress -- never a device address; DEVICE code (kv_static_fill) may use it directly.
+static __device__ __align__(256) unsigned char g_kv_static_tables[KV_STATIC_TABLE_BYTES];
+
+// Writes one slice of the call's table image into the array.  The slice travels in the kernel parameters, so the
+// caller's host arrays are consumed when the launch returns and no host-to-device copy (and no pinned staging) exists.
+constexpr uint32_t kStaticFillChunk = 28672;  // with the 16-byte head: 28,688 B of the 32,764 B a parameter block may have
+struct StaticFill {
+  uint32_t off;    // byte offset in the array, multiple of 16
+  uint32_t bytes;  // multiple of 16
+  uint32_t pad_[2];
+  alignas(16) uint8_t data[kStaticFillChunk];
+};
+__global__ void __launch_bounds__(256) kv_static_fill(const __grid_constant__ StaticFill p) {
+  for (uint32_t i = threadIdx.x * 16; i < p.bytes; i += blockDim.x * 16)
+    *reinterpret_cast<uint4 *>(g_kv_static_tables + p.off + i) = *reinterpret_cast<const uint4 *>(p.data + i);
+}
+
+// What the first call on a device learns and every later call reuses.  `tables` is written last (release) and read first
+// (acquire); two threads racing through the set-up of one device compute the same values.
+constexpr int kStaticMaxDevices = 64;
+struct StaticDevice {
+  std::atomic<uint8_t *> tables{nullptr};  // THIS device's address of g_kv_static_tables
+  int sm_count = 0;
+};
+StaticDevice g_static_device[kStaticMaxDevices];
+
+// `device` is current.  No allocation: a symbol lookup, an attribute query, a function attribute.
+cudaError_t static_setup(int device, uint8_t **tables, int *sm_count) {
+  StaticDevice &d = g_static_device[device];
+  uint8_t *t = d.tables.load(std::memory_order_acquire);
+  if (!t) {
+    void *sym = nullptr;
+    cudaError_t e = cudaGetSymbolAddress(&sym, g_kv_static_tables);
+    if (e != cudaSuccess) return e;
+    if (!sym) return cudaErrorInvalidSymbol;
+    int sms = 0;
+    if ((e = cudaDeviceGetAttribute(&sms, cudaDevAttrMultiProcessorCount, device)) != cudaSuccess) return e;
+    // as many single-warp CTAs per SM as shared memory holds (what kv_ctx_create asks for, for the same kernel)
+    if ((e = cudaFuncSetAttribute((const void *)kvt::kv_move_shot_plain<0, false>, cudaFuncAttributePreferredSharedMemoryCarveout,
+                                  cudaSharedmemCarveoutMaxShared)) != cudaSuccess) return e;
+    d.sm_count = sms;
+    t = (uint8_t *)sym;
+    d.tables.store(t, std::memory_order_release);
+  }
+  *tables = t;
+  *sm_count = d.sm_count;
+  return cudaSuccess;
+}
+
+}  // namespace
+
+extern "C" int kv_pack_static(int device, const kv_pool_desc *pools, uint32_t layer_count, const int32_t *page_ids,
+                              uint32_t n, void *dst, size_t dst_bytes, kv_stream_t stream, int *cuda_error) {
+  if (cuda_error) *cuda_error = 0;
+  // ---- validation: all of it before the first CUDA call
+  if (device < 0 || device >= kStaticMaxDevices) return KV_ERR_SIZE;
+  int rc = check_desc(pools, layer_count);
+  if (rc) return rc;
+  const uint32_t LC = layer_count * pools->kv_count;
+  if (LC > KV_STATIC_MAX_SLABS || n > KV_STATIC_MAX_PAGES) return KV_ERR_STATIC_LIMIT;
+  if (pools->order == KV_ORDER_HND && pools->num_heads > 1 && pools->page_size > 1) return KV_ERR_LAYOUT;
+  const uint64_t tokrow = (uint64_t)pools->num_heads * pools->head_dim * pools->elem_bytes;
+  const uint64_t row = tokrow * pools->page_size;  // one page of one (layer, K|V); check_desc bounds it by 2^32-1
+  if (!n) return KV_OK;
+  if (!page_ids || !dst) return KV_ERR_NULL;
+  if ((uint64_t)dst_bytes < (uint64_t)n * LC * row) return KV_ERR_SIZE;
+  if ((tokrow | pools->page_stride_bytes | (uint64_t)(uintptr_t)dst) % 16) return KV_ERR_ALIGN;
+  for (uint32_t i = 0; i < LC; ++i)
+    if ((uint64_t)(uintptr_t)pools->base[i] % 16) return KV_ERR_ALIGN;
+  rc = check_ids(page_ids, n, pools->num_pages);
+  if (rc) return rc;
+
+  // ---- device set-up (first call on this device) with the device current; restored on every way out
+  struct Restore {
+    int prev = -1;
+    ~Restore() { if (prev >= 0) cudaSetDevice(prev); }
+  } restore;
+  auto fail = [&](cudaError_t e) {
+    if (cuda_error) *cuda_error = (int)e;
+    (void)cudaGetLastError();
+    return (int)KV_ERR_CUDA;
+  };
+  int cur = -1;
+  cudaError_t e = cudaGetDevice(&cur);
+  if (e != cudaSuccess) return fail(e);
+  if (cur != device) {
+    if ((e = cudaSetDevice(device)) != cudaSuccess) return fail(e);
+    restore.prev = cur;
+  }
+  uint8_t *tables = nullptr;
+  int sm_count = 0;
+  if ((e = static_setup(device, &tables, &sm_count)) != cudaSuccess) return fail(e);
+
+  // ---- segments: a page row of one (layer, K|V), cut like the library cuts it for kv_move_shot (kv_geom.inl)
+  const uint32_t cap = 16384, chunk = (uint32_t)row;
+  uint32_t sub = std::min(chunk, cap);
+  if (chunk > cap) {  // equal pieces instead of full stages and a crumb
+    const uint32_t k = (chunk + cap - 1) / cap, even = ((chunk + k - 1) / k + 127) / 128 * 128;
+    if (even <= cap) sub = even;
+  }
+  while (sub >= 8192 && sub % 32 == 0 &&  // launch-sized calls: spread few segments over the chip
+         (uint64_t)n * LC * ((chunk + sub - 1) / sub) * 2 <= (uint64_t)sm_count * 2)
+    sub /= 2;
+  const uint32_t subs = (chunk + sub - 1) / sub;
+  const uint64_t total_items = (uint64_t)n * LC * subs;
+  if (total_items > 0x7fffffffull) return KV_ERR_SIZE;
+
+  // ---- the call's table image -> the array, slice by slice (header first: it re-zeroes the status word)
+  const uint32_t off_bases = kStaticHeader;
+  const uint32_t off_ids = off_bases + (LC * 8 + 15) / 16 * 16;
+  cudaStream_t s = (cudaStream_t)stream;
+  static thread_local StaticFill fill;
+  uint32_t at = 0;       // array offset of fill.data[0]
+  uint32_t have = 0;     // bytes of fill.data in use
+  auto flush = [&]() -> cudaError_t {
+    if (!have) return cudaSuccess;
+    fill.off = at;
+    fill.bytes = (have + 15) / 16 * 16;
+    std::memset(fill.data + have, 0, fill.bytes - have);
+    kv_static_fill<<<1, 256, 0, s>>>(fill);
+    at += fill.bytes;
+    have = 0;
+    return cudaGetLastError();
+  };
+  auto emit = [&](const void *src, size_t bytes) -> cudaError_t {  // src == nullptr: zeros
+    const uint8_t *q = (const uint8_t *)src;
+    while (bytes) {
+      const size_t m = std::min<size_t>(bytes, kStaticFillChunk - have);
+      if (q) { std::memcpy(fill.data + have, q, m); q += m; }
+      else std::memset(fill.data + have, 0, m);
+      have += (uint32_t)m;
+      bytes -= m;
+      if (have == kStaticFillChunk) {
+        cudaError_t fe = flush();
+        if (fe != cudaSuccess) return fe;
+      }
+    }
+    return cudaSuccess;
+  };
+  if ((e = emit(nullptr, kStaticHeader)) != cudaSuccess) return fail(e);
+  if ((e = emit(pools->base, (size_t)LC * 8)) != cudaSuccess) return fail(e);
+  if ((e = emit(nullptr, off_ids - off_bases - LC * 8)) != cudaSuccess) return fail(e);
+  if ((e = emit(page_ids, (size_t)n * 4)) != cudaSuccess) return fail(e);
+  if ((e = flush()) != cudaSuccess) return fail(e);
+
+  // ---- the copy: kv_move_shot_plain, tables in device memory (JobT<0>), one request, every token valid
+  kvt::JobT<0> p{};
+  Job &j = p.j;
+  j.bases = (const uint64_t *)(tables + off_bases);
+  j.ids = (const int32_t *)(tables + off_ids);
+  j.status = (uint32_t *)tables;
+  j.total_items = total_items;
+  j.page_stride = pools->page_stride_bytes;
+  j.buf_row_bytes = row;
+  j.buf_page_bytes = row * LC;
+  j.n_pieces = 1; j.LC = LC; j.dir = 0; j.layout = KV_LAYOUT_PAGE_FIRST;
+  j.g = pools->page_size; j.cpp_pool = 1; j.cpp_buf = 1;
+  j.tokrow = (uint32_t)tokrow; j.chunk_bytes = chunk; j.sub_bytes = sub; j.subs = subs;
+  j.num_pages = pools->num_pages;
+  j.stage_bytes = (sub + 127) / 128 * 128;
+  j.drow = pools->head_dim * pools->elem_bytes; j.H = pools->num_heads;
+  j.one.item_begin = 0; j.one.buf = (uint64_t)(uintptr_t)dst; j.one.n_tokens = (uint64_t)n * pools->page_size;
+  j.one.id_begin = 0; j.one.n_buf_pages = n; j.one.dir = 0;
+  auto magic = [](uint32_t d) -> uint64_t { return d <= 1 ? 0ull : ~0ull / d + 1; };
+  j.m_subs = magic(subs); j.m_LC = magic(LC); j.m_cpp_pool = 0; j.m_cpp_buf = 0;
+  j.lean = 1;
+  kvt::kv_move_shot_plain<0, false><<<(uint32_t)total_items, 32, j.stage_bytes, s>>>(p);
+  if ((e = cudaGetLastError()) != cudaSuccess) return fail(e);
+  return KV_OK;
+}

@@ -29,6 +29,9 @@ KV_OK = 0
 KV_ERR_NULL, KV_ERR_SIZE, KV_ERR_PAGE_RANGE, KV_ERR_DUP_PAGE, KV_ERR_LAYOUT = -1, -2, -3, -4, -5
 KV_ERR_ALIGN, KV_ERR_CUDA, KV_ERR_HOST_MEM, KV_ERR_DESC, KV_ERR_NO_DEVICE = -6, -7, -8, -9, -10
 KV_ERR_CAPTURE = -11
+KV_ERR_STATIC_LIMIT = -12
+KV_STATIC_MAX_PAGES, KV_STATIC_MAX_SLABS = 65536, 1024
+KV_STATIC_TABLE_BYTES = 256 + KV_STATIC_MAX_SLABS * 8 + KV_STATIC_MAX_PAGES * 4
 KV_LAYOUT_PAGE_FIRST, KV_LAYOUT_LAYER_FIRST = 0, 1
 KV_HOST_AUTO, KV_HOST_DIRECT, KV_HOST_STAGED = 0, 1, 2
 KV_ORDER_NHD, KV_ORDER_HND = 0, 1
@@ -100,6 +103,7 @@ _kv_host_free = _sig("kv_host_free", _int, _vp)
 _kv_host_register = _sig("kv_host_register", _int, _vp, _sz)
 _kv_host_unregister = _sig("kv_host_unregister", _int, _vp)
 _kv_pack = _sig("kv_pack", _int, _vp, _pdesc, _u32, _vp, _u32, _int, _vp, _sz, _u32, _vp)
+_kv_pack_static = _sig("kv_pack_static", _int, _int, _pdesc, _u32, _vp, _u32, _vp, _sz, _vp, ctypes.POINTER(_int))
 _kv_unpack = _sig("kv_unpack", _int, _vp, _vp, _sz, _vp, _u32, _pdesc, _u32, _u32, _u32, _u64,
                   _int, _u32, _vp)
 _kv_pack_batched = _sig("kv_pack_batched", _int, _vp, _pdesc, _u32, _vp, _vp, _u32, _int, _vp,
@@ -378,6 +382,27 @@ def kv_pack(ctx: Ctx, pools: PoolDesc, layer_count: int, page_ids, dst, dst_byte
     nb = _nbytes(dst) if dst_bytes is None else int(dst_bytes)
     _chk(ctx, _kv_pack(ctx.h, pools.ref, layer_count, p, n, layout, _ptr(dst), nb, flags,
                        _stream(stream, ctx.device)))
+
+
+def kv_pack_static(pools: PoolDesc, layer_count: int, page_ids, dst, dst_bytes=None, device: int = 0, stream=None):
+    """kv_pack for callers that must not allocate: no Ctx, and the library calls no cudaMalloc / cudaFree on this path.
+
+    Meant for code that runs where an allocation is not an option -- an engine whose KV pools already own the GPU's
+    memory, a latency-critical step that cannot afford the device-wide sync of cudaMalloc, a process bound to a fixed
+    memory budget.  The lookup tables live in a fixed array inside the library (KV_STATIC_TABLE_BYTES per GPU), so a
+    call takes at most KV_STATIC_MAX_PAGES page ids and KV_STATIC_MAX_SLABS layer x K/V slabs (KvError with
+    KV_ERR_STATIC_LIMIT beyond that), NHD pools, 16-byte aligned rows, host page ids, page-first layout.  Every call on a
+    device shares that array: issue them on one stream (or order them with events); overlapping calls race.  The first
+    call on a device looks the array up -- make it before capturing the stream into a CUDA graph.  include/kvtier.h has
+    the full contract."""
+    a = _host_i32(page_ids)
+    n = a.size
+    nb = _nbytes(dst) if dst_bytes is None else int(dst_bytes)
+    err = _int(0)
+    rc = _kv_pack_static(int(device), pools.ref, layer_count, a.__array_interface__["data"][0] if n else None, n,
+                         _ptr(dst), nb, _stream(stream, int(device)), ctypes.byref(err))
+    if rc:
+        raise KvError(rc, int(err.value) if rc == KV_ERR_CUDA else 0)
 
 
 def kv_unpack(ctx: Ctx, src, dst_page_ids, pools: PoolDesc, layer_count: int, src_page_size: int,
