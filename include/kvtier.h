@@ -88,9 +88,14 @@ typedef enum kv_layout {
 
 /* How a host-tier transfer crosses the host link (BASELINE.json:north_star item 3). */
 typedef enum kv_host_mode {
-  KV_HOST_AUTO = 0,   /* chosen from the measured table in DESIGN.md: STAGED from 4 MiB of payload (either layout), else DIRECT */
+  KV_HOST_AUTO = 0,   /* chosen from the measured table in DESIGN.md: STAGED from 4 MiB of payload (either layout), else DIRECT.
+                         If the ctx has no staging buffer and cannot get one -- the allocation fails because the KV pools
+                         fill HBM, or the stream is being captured -- AUTO runs DIRECT instead of failing, and after a
+                         failed allocation it does not try again until KV_OPT_RESERVE_STAGING succeeds (the failure's
+                         cudaError_t stays readable through kv_last_cuda_error) */
   KV_HOST_DIRECT = 1, /* the kernel stores to / loads from mapped pinned memory over the link */
-  KV_HOST_STAGED = 2, /* device staging + copy-engine transfers (1-D, or 2-D for layer-first chunks) on the ctx's side stream, chunk-pipelined */
+  KV_HOST_STAGED = 2, /* device staging + copy-engine transfers (1-D, or 2-D for layer-first chunks) on the ctx's side stream,
+                         chunk-pipelined.  Asked for explicitly, a staging allocation that fails is KV_ERR_CUDA */
 } kv_host_mode;
 
 typedef enum kv_status {

@@ -56,6 +56,10 @@ struct kv_ctx {
   // staging for KV_HOST_STAGED
   void *staging = nullptr;
   size_t staging_bytes = 0;
+  // The staging allocation failed (the usual reason: the KV pools fill HBM).  KV_HOST_AUTO then takes DIRECT, which needs
+  // no staging, and does not ask again -- a failing cudaMalloc still synchronises the device -- until a
+  // KV_OPT_RESERVE_STAGING succeeds.  An explicit KV_HOST_STAGED keeps trying and keeps reporting KV_ERR_CUDA.
+  bool staging_denied = false;
   // Slot i is ALWAYS the bytes [i * pitch, (i + 1) * pitch) of `staging`, pitch = staging_bytes / staging_slots: a
   // call whose chunks are smaller uses a prefix of each slot.  The per-slot events therefore guard the same memory for
   // every call, whatever its chunk size and whichever stream it runs on.

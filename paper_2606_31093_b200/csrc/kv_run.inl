@@ -44,7 +44,15 @@ int ensure_staging(kv_ctx *ctx) {
   // for plain cudaMemcpyAsync too (768 MiB each way as 1 / 2 / 3 / 6 copies: 99.2 / 96.1 / 96.5 / 93.7 GB/s summed), so
   // chunks are as large as the pipeline allows
   if (!ctx->staging_bytes) ctx->staging_bytes = (size_t)1024 << 20;
-  KV_CUDA(ctx, cudaMalloc(&ctx->staging, ctx->staging_bytes));
+  const cudaError_t e = cudaMalloc(&ctx->staging, ctx->staging_bytes);
+  if (e != cudaSuccess) {
+    ctx->staging = nullptr;
+    ctx->staging_denied = true;  // KV_HOST_AUTO stops asking (run_host)
+    ctx->last_cuda_error = (int)e;
+    (void)cudaGetLastError();
+    return KV_ERR_CUDA;
+  }
+  ctx->staging_denied = false;
   return KV_OK;
 }
 
@@ -393,6 +401,19 @@ int run_host(kv_ctx *ctx, const kv_pool_desc *pools, Call &c, const int32_t *ids
   if (lf.flags) {
     rc = flag_alias(lf.flags, &lf.flags);
     if (rc) return rc;
+  }
+  if (m == KV_HOST_STAGED && mode == KV_HOST_AUTO && !ctx->staging) {
+    // AUTO prefers the staged pipeline but the ctx has no staging yet: this call would allocate it.  No staging to be
+    // had -- the stream is being captured, or the allocation fails or has failed before (HBM is full of KV pools: the
+    // normal state of a serving engine) -- is no reason to fail a transfer that DIRECT can do without any staging.
+    // Nothing has been enqueued at this point.
+    if (ctx->staging_denied) m = KV_HOST_DIRECT;
+    else {
+      rc = ensure_staging(ctx);
+      if (rc == KV_ERR_CUDA || rc == KV_ERR_CAPTURE) m = KV_HOST_DIRECT;
+      else if (rc) return rc;
+    }
+    ctx->last_mode = (uint64_t)m;
   }
   if (m == KV_HOST_STAGED) {
     // The chunk pipeline is copies, events and kernels with their tables in the kernel parameters: all of it can be

@@ -250,6 +250,57 @@ def test_offload_reload_host_tier(kv, ctx, mode, Td):
         kv.kv_host_free(hp)
 
 
+def test_auto_runs_direct_when_the_staging_cannot_be_allocated(kv):
+    """A serving engine's KV pools fill HBM, so the staging that the first KV_HOST_AUTO transfer of 4 MiB or more
+    allocates may not be there to get.  AUTO must then move the bytes with DIRECT (which needs no staging) instead of
+    failing, and must not ask again on every call; an explicit KV_HOST_STAGED reports the failure; reserving a staging
+    that does fit brings the staged pipeline back.  The failure is forced with a 64 TiB staging size."""
+    L, C, P, T, H, D, e = 6, 2, 256, 16, 4, 128, 2   # page = 192 KiB
+    rng = np.random.default_rng(41)
+    A = host_pool(rng, L, C, P, T, H, D, e)
+    tA, dA = to_device(A, kv, torch)
+    n = 100                                           # 18.75 MiB: AUTO wants STAGED
+    ids = rng.permutation(P)[:n].astype(np.int32)
+    nbytes = n * dA.page_bytes()
+    want = ko.pack(A, ids)
+    hp = kv.kv_host_alloc(nbytes)
+    c = kv.Ctx(0, staging_bytes=1 << 46)
+    try:
+        hv = kv.host_view(hp, nbytes)
+        for attempt in range(2):  # the second call finds the denial recorded and goes straight to DIRECT
+            hv[:] = 0xEE
+            kv.kv_offload(c, dA, L, ids, hp, nbytes, mode=kv.KV_HOST_AUTO)
+            torch.cuda.synchronize()
+            assert np.array_equal(hv, want)
+            assert c.stat(kv.KV_STAT_LAST_HOST_MODE) == kv.KV_HOST_DIRECT
+            assert c.last_cuda_error() == 2  # cudaErrorMemoryAllocation, kept for the caller to see
+        hv[:] = 0xEE
+        with pytest.raises(kv.KvError) as ei:
+            kv.kv_offload(c, dA, L, ids, hp, nbytes, mode=kv.KV_HOST_STAGED)
+        assert ei.value.status == kv.KV_ERR_CUDA
+        torch.cuda.synchronize()
+        assert np.all(hv == 0xEE), "a failed call wrote to the host buffer"
+        hv[:] = want
+        B = host_pool(rng, L, C, n + 5, T, H, D, e)
+        tB, dB = to_device(B, kv, torch)
+        dst = rng.permutation(n + 5)[:n].astype(np.int32)
+        kv.kv_reload(c, hp, nbytes, dst, dB, L, T, T, n * T, mode=kv.KV_HOST_AUTO)
+        torch.cuda.synchronize()
+        assert c.stat(kv.KV_STAT_LAST_HOST_MODE) == kv.KV_HOST_DIRECT
+        ko.unpack(want, dst, B, Ts=T, n_tokens=n * T)
+        assert_pool_equal(tB, B)
+        c.set_option(kv.KV_OPT_RESERVE_STAGING, 8 << 20)  # a size that fits: the staged pipeline is back
+        hv[:] = 0xEE
+        kv.kv_offload(c, dA, L, ids, hp, nbytes, mode=kv.KV_HOST_AUTO)
+        torch.cuda.synchronize()
+        assert c.stat(kv.KV_STAT_LAST_HOST_MODE) == kv.KV_HOST_STAGED
+        assert np.array_equal(hv, want)
+    finally:
+        torch.cuda.synchronize()
+        c.close()
+        kv.kv_host_free(hp)
+
+
 @pytest.mark.parametrize("mode", ["direct", "staged"])
 def test_offload_reload_batched(kv, ctx, mode):
     m = {"direct": kv.KV_HOST_DIRECT, "staged": kv.KV_HOST_STAGED}[mode]
