@@ -9,8 +9,13 @@ using kvt::Job;
 using kvt::Piece;
 
 constexpr int kBlobSlots = 16;
-constexpr int kInlineSmall = 3840;   // inline tables: the whole parameter block stays under the classic 4 KiB
-constexpr int kInlineLarge = 31744;  // CUDA 12.1+ large kernel parameters (<= 32,764 B)
+// Inline tables.  Small: the WHOLE parameter block (Job header + blob) stays within the classic 4 KiB, so the launch does
+// not take the large-parameter path; the size follows the header, whatever it grows to.  Large: CUDA 12.1+ kernel
+// parameters (<= 32,764 B).
+constexpr int kInlineSmall = (4096 - (int)offsetof(kvt::JobT<1>, blob)) / 64 * 64;
+constexpr int kInlineLarge = 31744;
+static_assert(kInlineSmall >= 2048 && sizeof(kvt::JobT<kInlineSmall>) <= 4096, "small inline tables: parameter block over 4 KiB");
+static_assert(sizeof(kvt::JobT<kInlineLarge>) <= 32764, "large inline tables: parameter block over the 32,764-byte limit");
 constexpr int kMaxStagingSlots = 4;
 constexpr uint32_t kMaxLayersKv = 4096;  // layer_count * kv_count
 constexpr uint64_t kAutoStagedMinBytes = 4ull << 20;
