@@ -37,6 +37,9 @@
  *     parameters (same kernels); if tables and maps together exceed the parameter space it takes the lane paths.
  *     A graph holding staged transfers uses the ctx's staging buffer at every replay: replay it on the stream on
  *     which the ctx's other staged transfers run, or not at the same time as them.  Otherwise: KV_ERR_CAPTURE.
+ *     While a capture that holds a staged transfer of a ctx is still open (before cudaStreamEndCapture), the ctx's side
+ *     stream belongs to it: an EAGER multi-chunk staged transfer of the same ctx on another stream is refused with
+ *     KV_ERR_CAPTURE (explicit KV_HOST_STAGED) or runs DIRECT (KV_HOST_AUTO) instead of leaking into that graph.
  *   - A kv_ctx is not thread-safe: one ctx per calling thread.  Calls on different streams are
  *     independent when their destination page sets are disjoint; staged host transfers of ONE ctx issued on
  *     different streams share its staging slots and are ordered against one another slot by slot.
@@ -113,7 +116,8 @@ typedef enum kv_status {
   KV_ERR_CAPTURE = -11,   /* `stream` is capturing a CUDA graph and this call is not replayable: its tables exceed
                              the kernel parameters (~31 KiB: about 7,500 page ids per launch), the element-wise
                              fallback kernel is needed, or mode is KV_HOST_STAGED and the ctx has no staging buffer
-                             yet.  Nothing was enqueued. */
+                             yet.  Also: an eager KV_HOST_STAGED transfer while another stream's open capture holds the
+                             ctx's side stream.  Nothing was enqueued. */
   KV_ERR_STATIC_LIMIT = -12, /* kv_pack_static only: the request needs more table space than the library's fixed,
                              built-in device array holds (more than KV_STATIC_MAX_PAGES page ids or more than
                              KV_STATIC_MAX_SLABS layer x K/V slabs).  Nothing was enqueued; split the request. */

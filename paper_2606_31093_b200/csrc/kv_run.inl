@@ -244,6 +244,11 @@ int run_staged(kv_ctx *ctx, const kv_pool_desc *pools, const Call &c, const int3
     if (need > (size_t)kInlineLarge) inline_ok = false;
   }
   if (cap && !inline_ok) return KV_ERR_CAPTURE;
+  // An eager transfer of several chunks forks to the ctx's side stream.  While a staged transfer of this ctx is being
+  // captured on another stream -- between its cudaStreamBeginCapture and cudaStreamEndCapture -- the side stream is part
+  // of that capture: work enqueued onto it now would end up inside the foreign graph or invalidate it.  Refuse before
+  // anything is enqueued (KV_HOST_AUTO then runs DIRECT, run_host).
+  if (!cap && chunks.size() > 1 && capturing(ctx->side)) return KV_ERR_CAPTURE;
   Blob shared;  // the one staged blob of the fallback
   HostBlob hb_all;
   if (!inline_ok) {

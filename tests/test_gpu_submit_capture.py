@@ -216,6 +216,54 @@ def test_staged_offload_and_reload_captured_and_replayed(kv, layout, dev_ids):
         kv.kv_host_free(hp)
 
 
+def test_eager_staged_call_while_a_capture_of_the_same_ctx_is_open(kv):
+    """Between cudaStreamBeginCapture and EndCapture of a graph that holds a staged transfer, the ctx's side stream is
+    part of that capture.  An eager multi-chunk staged transfer of the same ctx on ANOTHER stream must not enqueue onto
+    it: explicit KV_HOST_STAGED is refused (KV_ERR_CAPTURE, nothing written), KV_HOST_AUTO moves the bytes with DIRECT,
+    and the graph under construction stays valid and replays the oracle's bytes."""
+    L, C, P, T, H, D, e = 6, 2, 256, 16, 4, 128, 2  # page = 192 KiB
+    rng = np.random.default_rng(97)
+    A = host_pool(rng, L, C, P, T, H, D, e)
+    tA, dA = to_device(A, kv, torch)
+    n = 100
+    nbytes = n * dA.page_bytes()  # 18.75 MiB through 2 x 4 MiB slots: five chunks
+    ctx = kv.Ctx(0, staging_bytes=8 << 20)
+    h_graph, h_eager = kv.kv_host_alloc(nbytes), kv.kv_host_alloc(nbytes)
+    try:
+        v_graph, v_eager = kv.host_view(h_graph, nbytes), kv.host_view(h_eager, nbytes)
+        v_graph[:] = 0
+        v_eager[:] = 0xEE
+        ids_g = rng.choice(P, n, replace=False).astype(np.int32)
+        ids_e = rng.choice(P, n, replace=False).astype(np.int32)
+        ctx.set_option(kv.KV_OPT_RESERVE_STAGING, 0)
+        cap_stream, other = torch.cuda.Stream(), torch.cuda.Stream()
+        g = torch.cuda.CUDAGraph()
+        torch.cuda.synchronize()
+        with torch.cuda.graph(g, stream=cap_stream, capture_error_mode="thread_local"):
+            kv.kv_offload(ctx, dA, L, ids_g, h_graph, nbytes, mode=kv.KV_HOST_STAGED, stream=cap_stream)
+            # the capture is still open: the side stream is inside it
+            with pytest.raises(kv.KvError) as ei:
+                kv.kv_offload(ctx, dA, L, ids_e, h_eager, nbytes, mode=kv.KV_HOST_STAGED, stream=other)
+            assert ei.value.status == kv.KV_ERR_CAPTURE
+            kv.kv_offload(ctx, dA, L, ids_e, h_eager, nbytes, mode=kv.KV_HOST_AUTO, stream=other)
+            assert ctx.stat(kv.KV_STAT_LAST_HOST_MODE) == kv.KV_HOST_DIRECT
+        other.synchronize()
+        assert np.array_equal(v_eager, ko.pack(A, ids_e)), "the eager AUTO call (DIRECT) != oracle"
+        assert np.all(v_graph == 0), "a captured transfer ran before its graph was launched"
+        g.replay()
+        torch.cuda.synchronize()
+        assert np.array_equal(v_graph, ko.pack(A, ids_g)), "the graph captured around the refused call != oracle"
+        v_eager[:] = 0xEE  # with the capture closed, the eager staged pipeline is available again
+        kv.kv_offload(ctx, dA, L, ids_e, h_eager, nbytes, mode=kv.KV_HOST_STAGED, stream=other)
+        other.synchronize()
+        assert np.array_equal(v_eager, ko.pack(A, ids_e))
+    finally:
+        torch.cuda.synchronize()
+        ctx.close()
+        kv.kv_host_free(h_graph)
+        kv.kv_host_free(h_eager)
+
+
 # ------------------------------------------------------------------------------------------------
 # ONE ctx, staged transfers on TWO streams with different chunk sizes: the slots are fixed pieces of the staging
 # buffer, so the per-slot events order the two calls whatever their chunking (kvtier.h "A kv_ctx ...")
