@@ -12,7 +12,7 @@ prefix = 512 fragmented pages (768 MiB), fresh page ids every step.
   e2e       = the same metric with HOST buffers: kv_offload (pool -> pinned host) + kv_reload
               (pinned host -> pool) + stream sync per step; H2D/D2H inside the timed region
               (SURVEY.md 8(a) a6/a7).
-  roofline  = dominant kernel kv_move_bulk (the pack launch): algorithmic bytes 2*payload per
+  roofline  = dominant kernel kv_move_shot_plain (the pack launch): algorithmic bytes 2*payload per
               launch / its mean duration from CUDA events on the launch stream, against the
               measured HBM copy peak in MEASURED_PEAKS.json.
   cpu_baseline = the oracle (oracle/kv_oracle.c, as it stands) on the box's host cores, on a

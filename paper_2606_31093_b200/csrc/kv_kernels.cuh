@@ -1,20 +1,26 @@
 // kv_kernels.cuh -- sm_100a kernels of the paged-KV tier transfer.
 //
-// Every transfer (pack, unpack, re-page, batched, direct host offload/reload) is ONE launch of
-// one of three kernels over a flat list of work items ("segments").  A segment is a run of bytes
-// that is contiguous on BOTH sides: g = gcd(Tpool, Tbuf) tokens of one (layer, K|V) of one page,
-// cut into pieces of at most `sub_bytes`.  The pool side hops between 2*L slabs by page id
-// (PAPER.md:L207 addressing); the buffer side is the dense lower-tier representation
-// (BASELINE.json:configs[0]).
+// Every transfer (pack, unpack, re-page, copy-on-write append, batched, kv_submit, direct host offload/reload, every chunk
+// of a staged host transfer) is ONE launch of one of the kernels below over a flat list of work items ("segments").  A
+// segment is a run of bytes that is contiguous on BOTH sides: g = gcd(Tpool, Tbuf) tokens of one (layer, K|V) of one
+// page, cut into pieces of at most `sub_bytes`.  The pool side hops between 2*L slabs by page id (PAPER.md:L207
+// addressing); the buffer side is the dense lower-tier representation (BASELINE.json:configs[0]).
 //
-//   kv_move_bulk  the B200 path: cp.async.bulk (SASS UBLKCP) global -> shared -> global through a
-//                 per-warp ring of mbarrier-tracked stages.  32 lanes decode 32 segments' addresses
-//                 at once (warp-level page-table lookup), lane 0 drives the async copy engine.
-//                 No data ever passes through registers.
-//   kv_move_shot  one segment per single-warp CTA, same async copies, no ring: the CTA scheduler distributes the work.
-//   kv_move_vec   16-byte LDG/STG, one warp per segment, 8 loads in flight per lane.
-//   kv_move_small segments <= 1 KiB: 32 segments decoded per warp, copied eight at a time (16-byte LDG/STG).
-//   kv_move_elem  any alignment: unit-wide (1/2/4/8 B) coalesced copy.  Correctness fallback.
+//   kv_move_shot        the B200 path, AUTO's choice for segments of 4 KiB or more (every shape of the paper): ONE
+//                       segment per single-warp CTA, moved global -> shared -> global by cp.async.bulk (SASS UBLKCP) or,
+//                       for an HND pool, by cp.async.bulk.tensor through per-slab tensor maps (UTMALDG / UTMASTG: the
+//                       copy engine does the [head][token] transposition).  13 CTAs = 208 KiB in flight per SM; the CTA
+//                       scheduler is the work distributor.  No payload byte passes through registers.
+//   kv_move_shot_plain  its short form for the plain case (equal page sizes, page-first, nothing to zero-fill, host ids;
+//                       one request or a batch): ~170 instructions, lane 0 alone works.  What small calls and the
+//                       headline config run.
+//   kv_move_bulk        persistent CTAs, a per-warp ring of mbarrier-tracked stages, 32 segments decoded per warp at
+//                       once, guided claiming from a device counter: AUTO's choice for 2-4 KiB segments, where the rate
+//                       at which one SM retires bulk copies binds the one-shot kernel.
+//   kv_move_vec         16-byte LDG/STG, one warp per segment, 8 loads in flight per lane (strided HND destinations
+//                       without tensor maps, large copy-on-write batches on narrow rows).
+//   kv_move_small       segments <= 1 KiB: 32 segments decoded per warp, copied eight at a time (16-byte LDG/STG).
+//   kv_move_elem        any alignment: unit-wide (1/2/4/8 B) coalesced copy.  Correctness fallback.
 //
 // This file shares nothing with oracle/.
 #pragma once

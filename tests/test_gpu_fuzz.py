@@ -150,9 +150,10 @@ MEDIUM = [  # Ts, Td, H, order_s, order_d, layout, tokens: sizes at which AUTO's
 
 @pytest.mark.parametrize("Ts,Td,H,order_s,order_d,layout,ntok", MEDIUM)
 def test_medium_sizes_with_default_options(kv, Ts, Td, H, order_s, order_d, layout, ntok):
-    """Tens of MiB per call with nothing overridden: the sizes at which the automatic choices engage -- the vec kernel
-    from 40 MiB, kv_move_small for segments <= 1 KiB, the ring re-shaped for narrow rows, guided claiming, tensor
-    maps -- through pack -> re-paging unpack -> fused re-page, against the oracle."""
+    """Tens of MiB per call with nothing overridden: the sizes at which the automatic choices engage -- kv_move_shot
+    (general form: gcd chunking, zero tails, tensor maps on HND pools) for segments of 4 KiB or more, the ring re-shaped
+    for narrow rows with guided claiming for 2-4 KiB, kv_move_small for segments <= 1 KiB -- through pack -> re-paging
+    unpack -> fused re-page, against the oracle."""
     L, C, D, e = 12, 2, 128, 2
     rng = np.random.default_rng(hash((Ts, Td, H, order_s, order_d, layout, ntok)) % 2**31)
     ctx = kv.Ctx(0)
