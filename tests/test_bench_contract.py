@@ -24,8 +24,9 @@ def run_bench(*args):
 def test_reference_arm_prints_the_contract_line():
     line = run_bench("--impl", "reference", "--steps", "2", "--warmup", "1")
     assert BASE_KEYS <= set(line), BASE_KEYS - set(line)
-    # the reference arm honours --steps / --warmup and times the oracle on OUR arm's config: the same `config` object,
-    # the full 512-page prefix per step
+    # the reference arm honours --steps / --warmup and times the oracle on OUR arm's workload -- same shape, the full
+    # 512-page prefix per step, same byte convention -- and states the pool it really ran on (a host pool bounded by
+    # RAM), not our arm's 96 GiB device pool
     assert line["steps"] == 2 and line["warmup"] == 1
     sys.path.insert(0, ROOT)
     import argparse
@@ -34,7 +35,11 @@ def test_reference_arm_prints_the_contract_line():
     from paper_2606_31093_b200 import workloads as W
 
     ours = bench.bench_config(argparse.Namespace(prefix_tokens=8192, pool_order="nhd", pool_pages=65536, kernel="auto"), W.QWEN3_OMNI)
-    assert line["config"] == ours and ours["pages_per_step"] == 512
+    own = {"pool_pages", "pool_GiB", "kernel", "pool"}
+    assert {k: v for k, v in line["config"].items() if k not in own} == {k: v for k, v in ours.items() if k not in own}
+    assert ours["pages_per_step"] == 512
+    assert line["config"]["pool_pages"] == bench.ORACLE_POOL_PAGES and line["config"]["pool_GiB"] == 6.0
+    assert line["config"]["kernel"].startswith("n/a") and "host-resident" in line["config"]["pool"]
     assert "full 512-page prefix" in line["cpu_baseline"]["sample"]
     assert line["impl"] == "reference" and line["metric"] == "kv_pack_unpack_GBps" and line["unit"] == "GB/s"
     assert line["value"] > 0 and line["higher_is_better"] is True and line["vs_baseline"] is None
@@ -65,6 +70,8 @@ def test_our_arm_prints_the_contract_line():
     assert line["bit_exact"] is True  # the timed region's last step, checked with torch indexing
     assert r["traffic"] is None  # a profile figure: emitted only for a profiled configuration (a pool of at least 12 GiB)
     # the host-link roofline is measured in the same run: peaks and fractions for offload, reload and both at once
+    assert r["host"]["offload"] == line["roofline_host"]["offload"] and 0 < r["host"]["duplex"]["frac"]
+    assert e["offload_frac"] == r["host"]["offload"]["frac"] and e["reload_frac"] == r["host"]["reload"]["frac"]
     h = line["roofline_host"]
     for k in ("offload", "reload", "duplex"):
         assert 0 < h[k]["frac"] == pytest.approx(h[k]["achieved"] / h[k]["peak"])
