@@ -50,11 +50,16 @@ UNIT = "GB/s"
 # THIS command at THIS workload.  It is a profile figure, not something this run measures: it is emitted only when the run's
 # configuration is a profiled one (512 pages, NHD pool, the kernel the profile captured), with the file named beside it;
 # otherwise `traffic` is null.  kv_move_shot_plain (AUTO's kernel for this call): 805.3 MB read + 753.0 MB written; the round-1
-# ring (--kernel bulk): 805.4 + 759.3 (the last ~50 MB written are still dirty in L2 at exit).
+# ring (--kernel bulk): 805.4 + 759.3 (the last ~50 MB written are still dirty in L2 at exit).  Those three captures ran on a
+# 12 GiB pool (--pool-pages 8192); "pool96" is the round-3 capture of the plain kernel on the 96 GiB pool the default run times.
 NCU_TRAFFIC = {"kv_move_shot_plain": {"bytes_per_launch": 1558.3e6, "profile": "profiles/r02_kv_move_shot_plain_full.md"},
                "kv_move_shot": {"bytes_per_launch": 1558.4e6, "profile": "profiles/r02_kv_move_shot_full.md"},
                "kv_move_bulk": {"bytes_per_launch": 1564.6e6, "profile": "profiles/r01_kv_move_bulk_full.md"},
-               "workload": {"pages": 512, "pool_order": "nhd", "min_pool_pages": 8192}}  # r02 was captured on a 12 GiB pool
+               "workload": {"pages": 512, "pool_order": "nhd", "min_pool_pages": 8192},  # r02 was captured on a 12 GiB pool
+               # round 3: the same command captured ON the 96 GiB pool (single-pass metric list: no save/restore), mean of 7 kv_pack
+               # launches, 806.62 MB read + 750.38 MB written; used when the run's pool is that pool
+               "pool96": {"pool_pages": 65536,
+                          "kv_move_shot_plain": {"bytes_per_launch": 1557.0e6, "profile": "profiles/r03_pool96_dram.md"}}}
 REFERENCE_WALL_CAP_S = 150.0  # the reference arm stops adding steps beyond this (and says so); 50 steps need ~8 s
 
 
@@ -520,6 +525,8 @@ def run_ours(args):
     profiled = NCU_TRAFFIC.get(kern_name) if (args.pool_order == NCU_TRAFFIC["workload"]["pool_order"]
                                               and n == NCU_TRAFFIC["workload"]["pages"]
                                               and args.pool_pages >= NCU_TRAFFIC["workload"]["min_pool_pages"]) else None
+    if profiled and args.pool_pages == NCU_TRAFFIC["pool96"]["pool_pages"]:
+        profiled = NCU_TRAFFIC["pool96"].get(kern_name, profiled)  # a capture on this very pool, where one exists
     line = {
         "metric": METRIC, "value": value, "unit": UNIT, "n_gpus": world, "steps": K, "warmup": Wm,
         "ms_per_step": t_total_ms / K, "higher_is_better": True, "scaling": "weak",

@@ -197,11 +197,10 @@ def test_hnd_degenerate_orders_are_plain_copies(kv, ctx):
         assert np.array_equal(buf.cpu().numpy(), ko.pack(A, ids))
 
 
+@pytest.mark.parametrize("ctx", [1], indirect=True, ids=["tensormaps"])  # a test ABOUT tensor maps: no "lanes" case is generated
 def test_auto_with_tensor_maps_is_one_bulk_kernel(kv, ctx):
-    """AUTO with tensor maps (the default): every direction of an HND transfer is the bulk ring, whole-token
+    """AUTO with tensor maps (the default): every direction of an HND transfer is one async-copy kernel, whole-token
     boxes moved by cp.async.bulk.tensor; the second call on the same pool reuses the cached maps."""
-    if not ctx.tensor_maps:
-        pytest.skip("tensor maps switched off in this parametrisation")
     L, C, P, T, H, D, e, n = 3, 2, 64, 16, 4, 128, 2, 20
     rng = np.random.default_rng(83)
     A = host_pool(rng, L, C, P, T, H, D, e, order=HND)

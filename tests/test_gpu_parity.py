@@ -131,14 +131,16 @@ def test_plain_kernel_and_general_kernel_agree_with_the_oracle(kv, ctx, shape, v
         assert_pool_equal(tB, B)
 
 
-@pytest.mark.parametrize("kernel", ["bulk", "vec"])
+@pytest.mark.parametrize("kernel", ["bulk", "vec", "shot", "auto"])
 @pytest.mark.parametrize("Ts,Td,ntok", [(16, 64, 2048), (16, 64, 2048 - 37), (64, 16, 1000),
                                         (16, 24, 500), (3, 5, 77), (16, 16, 16 * 9 - 5), (8, 64, 1)])
 def test_repage_unpack(kv, ctx, kernel, Ts, Td, ntok):
-    """SURVEY.md 8(a) a5; BASELINE.json:configs[4]: sequence order preserved, zero-padded tail."""
+    """SURVEY.md 8(a) a5; BASELINE.json:configs[4]: sequence order preserved, zero-padded tail.  "shot" is the general
+    form of the kernel AUTO picks at the paper's shapes (kv_move_shot: gcd chunking, zero tail); "auto" is whatever the
+    library chooses for the shape (0 = KV_OPT_KERNEL's default)."""
     L, C, H, D, e = 3, 2, 4, 128, 2
     rng = np.random.default_rng(Ts * 1000 + Td)
-    ctx.set_option(kv.KV_OPT_KERNEL, KERNELS[kernel])
+    ctx.set_option(kv.KV_OPT_KERNEL, KERNELS.get(kernel, 0))
     n_src, n_dst = -(-ntok // Ts), -(-ntok // Td)
     P = n_dst + 7
     src = rng.integers(0, 256, size=n_src * L * C * Ts * H * D * e, dtype=np.uint8)
@@ -151,12 +153,14 @@ def test_repage_unpack(kv, ctx, kernel, Ts, Td, ntok):
 
 
 @pytest.mark.parametrize("layout", [0, 1])
-@pytest.mark.parametrize("kernel", ["bulk", "vec", "elem"])
+@pytest.mark.parametrize("kernel", ["bulk", "vec", "elem", "shot", "auto"])
 def test_batched_csr_with_empty_requests_and_layouts(kv, ctx, kernel, layout):
-    """SURVEY.md 8(a) a8; BASELINE.json:configs[3] (variable-length, CSR-encoded)."""
+    """SURVEY.md 8(a) a8; BASELINE.json:configs[3] (variable-length, CSR-encoded).  With "shot" / "auto" the pack is the
+    plain kernel's batched form (pieces by binary search) when page-first and the general kv_move_shot when layer-first;
+    the ragged re-paging unpack is the general kernel either way."""
     L, C, P, T, H, D, e = 4, 2, 300, 16, 2, 64, 2
     rng = np.random.default_rng(11 + layout)
-    ctx.set_option(kv.KV_OPT_KERNEL, KERNELS[kernel])
+    ctx.set_option(kv.KV_OPT_KERNEL, KERNELS.get(kernel, 0))
     A = host_pool(rng, L, C, P, T, H, D, e)
     tA, dA = to_device(A, kv, torch)
     counts = np.array([5, 0, 33, 1, 0, 17, 64])
