@@ -71,6 +71,32 @@ def test_config3_session_and_config4_batch_shapes(kv, ctx):
         assert np.array_equal(got[poff[s]:poff[s] + k], got[:k])
 
 
+@pytest.mark.parametrize("T", [16, 5])
+def test_thousands_of_ragged_sessions(kv, ctx, T):
+    """The two-launch path of large batches (digests of all pages at once, then a warp per session along the chain) on
+    1,500 sessions of very unequal length -- a tenth empty, a tenth shorter than a page, one far longer than the rest --
+    with and without per-session roots, against the oracle."""
+    rng = np.random.default_rng(1500 + T)
+    S = 1500
+    lens = np.floor(np.exp(rng.uniform(np.log(16), np.log(4000), size=S))).astype(np.int64)
+    kind = rng.random(S)
+    lens[kind < 0.1] = 0
+    sub = (kind >= 0.1) & (kind < 0.2)
+    lens[sub] = rng.integers(1, T, size=int(sub.sum()))
+    lens[777] = 20000
+    off = np.zeros(S + 1, dtype=np.int64)
+    np.cumsum(lens, out=off[1:])
+    ident = rng.integers(0, 2**64, size=int(off[-1]), dtype=np.uint64)
+    want, wpoff = co.chain_batched(ident, off, T, threads=8)
+    got, poff = run(kv, ctx, ident, off, T)
+    assert np.array_equal(poff, wpoff) and np.array_equal(got, want)
+    assert int((np.diff(poff) == 0).sum()) >= 250  # the empty and sub-page sessions yield no ids
+    roots = rng.integers(0, 2**64, size=S, dtype=np.uint64)
+    want_r, _ = co.chain_batched(ident, off, T, roots, threads=8)
+    got_r, _ = run(kv, ctx, ident, off, T, roots=roots)
+    assert np.array_equal(got_r, want_r)
+
+
 def test_empty_sessions_tails_and_offsets_not_at_zero(kv, ctx):
     rng = np.random.default_rng(9)
     ident = rng.integers(0, 2**64, size=500, dtype=np.uint64)
