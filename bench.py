@@ -558,7 +558,8 @@ def run_ours(args):
                      else f"{kern_name}<kTrans> with tensor maps (kv_pack launch, HND pool)", "achieved": achieved,
                      "peak": peak, "unit": "GB/s", "frac": achieved / peak,
                      "traffic": profiled["bytes_per_launch"] if profiled else None,
-                     "traffic_source": (f"ncu --set full capture of this command at this workload, {profiled['profile']} "
+                     "traffic_source": (f"ncu capture of this command at this workload (r02 profiles: --set full on a 12 GiB pool; "
+                                        f"r03_pool96: a single-pass --metrics list on the 96 GiB pool), {profiled['profile']} "
                                         "(a profile figure, not measured by this run)") if profiled else None,
                      "algorithmic_bytes": 2 * payload, "peak_source": peak_src,
                      "timing": "mean over the K timed steps of CUDA events on the launch stream around each kv_pack call (one launch; page ids ride in the kernel parameters)"},
